@@ -1,0 +1,425 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the SPH offload hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--layout split|aos]
+
+A step = one pass of the whole hot path over BASELINE.json:configs[1] (262,144 particles, 64^3 glass-like
+lattice, 16^3 cells, 57,344 tasks): zero, pack DENSITY_IN, density loop, unpack DENSITY_OUT, ghost, zero,
+pack FORCE_IN, force loop, unpack FORCE_OUT -- 9 kernel launches, inputs resident in HBM.
+value = particles/s through that step (whole job: all ranks' particles / max-over-ranks time).
+`e2e` = the same step through the C ABI with HOST (pinned) particle arrays: the substructs the loops read are
+uploaded, the ones they write are downloaded, every step, inside the timed region.
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particles/s pack+unpack and pair-interactions/s; % of HBM / host-link roofline"
+WORKLOAD = "configs[1]: 262144 particles, 64^3 glass-like lattice, 16^3 cells, density loop then force loop"
+N_SM, LANES_PER_SM = 148, 128
+# algorithmic FP32 work of the loops: 8 flop per ordered candidate pair (3 sub, 1 mul,
+# 2 fma, 1 compare) + per neighbour hit 25 flop (density) / 60 flop (force)
+FLOP_CAND, FLOP_HIT_DENSITY, FLOP_HIT_FORCE = 8.0, 25.0, 60.0
+NGB_CONFIG1 = 63.04    # (32/3) pi (1.2348)^3: neighbours per particle incl. self at h = 1.2348 dx
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason samples taken DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(index)],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, reasons = [], set()
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1]))
+                out["sm_max_mhz"] = float(r[2])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if sm:
+            out["sm_mhz"] = statistics.median(sm)
+        out["reasons"], out["samples"] = sorted(reasons), len(sm)
+        return out
+
+
+def dist_setup(n_gpus):
+    """one process per GPU under torchrun; returns (rank, world, device index)"""
+    import torch
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if world > 1:
+        import torch.distributed as dist
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        if torch.cuda.is_available():
+            torch.cuda.set_device(local)
+        dist.init_process_group(backend=backend)
+    return rank, world, local
+
+
+def dist_barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def dist_max(value, world, device="cpu"):
+    """max over ranks of a python float (timing rule: the slowest rank defines the step)"""
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def dist_sum(value, world, device="cpu"):
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# --------------------------------------------------------------------------------------------- our arm
+
+class Workload:
+    """configs[1] resident on the current device in one layout, one batch holding every task of a loop."""
+
+    def __init__(self, sph, torch, ps, cells, tasks, layout_name):
+        self.sph, self.torch = sph, torch
+        self.layout_name = layout_name
+        self.layout = sph.sph_layout_aos() if layout_name == "aos" else sph.sph_layout_split()
+        self.n = ps.shape[0]
+        self.store = sph.sph_store_create(self.layout, self.n)
+        sph.sph_store_import_aos(self.store, ps)
+        sph.sph_store_set_cells(self.store, cells)
+        self.batch = sph.sph_batch_create(self.store, tasks)
+        self.info = sph.sph_batch_get_info(self.batch)
+        self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+        self.rec = [sph.sph_attrset_record_bytes(s) for s in self.sets]
+        self.bufs = [torch.empty(sph.sph_batch_buffer_bytes(self.batch, s), dtype=torch.uint8, device="cuda") for s in self.sets]
+        self.params = sph.sph_params(np.float32(5.0 / 3.0), 0.8, 3.0)
+        # host mirrors of the substruct arrays for the end-to-end leg (pinned)
+        self.host = []
+        for s in range(self.layout.n_sub):
+            nb = self.n * self.layout.stride[s]
+            h = torch.empty(nb, dtype=torch.uint8).pin_memory()
+            self.host.append(h)
+        # which substructs a step reads from / writes to the host copy
+        f = sph.FIELD
+        ins = {self.layout.loc[f[k]].sub for k in ("x", "h", "mass", "v", "u")}
+        outs = {self.layout.loc[f[k]].sub for k in ("rho", "rho_dh", "wcount", "wcount_dh", "P", "c_s", "a", "du_dt", "v_sig")}
+        self.subs_in, self.subs_out = sorted(ins), sorted(outs)
+        for s in range(self.layout.n_sub):
+            sph.sph_store_download_sub(self.store, s, self.host[s])
+        torch.cuda.synchronize()
+
+    # the nine launches of a step, as (name, callable)
+    def launches(self, stream=None):
+        stream = stream if stream is not None else self.torch.cuda.current_stream()
+        sph, st, b, S, B, p = self.sph, self.store, self.batch, self.sets, self.bufs, self.params
+        return [
+            ("zero_density_out", lambda: sph.sph_store_zero(st, S[1], stream)),
+            ("pack_density_in", lambda: sph.sph_pack(st, b, S[0], B[0], stream)),
+            ("density", lambda: sph.sph_density(b, B[0], B[1], stream)),
+            ("unpack_density_out", lambda: sph.sph_unpack(st, b, S[1], B[1], sph.SPH_UNPACK_REDUCE, stream)),
+            ("ghost", lambda: sph.sph_ghost(st, p, stream)),
+            ("zero_force_out", lambda: sph.sph_store_zero(st, S[3], stream)),
+            ("pack_force_in", lambda: sph.sph_pack(st, b, S[2], B[2], stream)),
+            ("force", lambda: sph.sph_force(b, B[2], B[3], p, stream)),
+            ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], sph.SPH_UNPACK_REDUCE, stream)),
+        ]
+
+    def step(self, stream=None):
+        for _, fn in self.launches(stream):
+            fn()
+
+    def step_e2e(self, stream=None):
+        stream = stream if stream is not None else self.torch.cuda.current_stream()
+        for s in self.subs_in:
+            self.sph.sph_store_upload_sub(self.store, s, self.host[s], stream)
+        self.step(stream)
+        for s in self.subs_out:
+            self.sph.sph_store_download_sub(self.store, s, self.host[s], stream)
+
+    def e2e_bytes(self):
+        return (sum(self.n * self.layout.stride[s] for s in self.subs_in), sum(self.n * self.layout.stride[s] for s in self.subs_out))
+
+    def algorithmic(self):
+        """algorithmic bytes / flop per launch: every record byte once, every touched store
+        field once per particle per launch (re-reads of a cell by its 27 tasks are cache hits, not algorithmic traffic)."""
+        n, inst, cand = self.n, self.info.n_instances, self.info.n_candidates
+        r = self.rec
+        return {
+            "pack_density_in": {"bound": "hbm", "bytes": n * 32 + inst * r[0]},
+            "unpack_density_out": {"bound": "hbm", "bytes": inst * r[1] + n * 2 * 16},
+            "pack_force_in": {"bound": "hbm", "bytes": n * 64 + inst * r[2]},
+            "unpack_force_out": {"bound": "hbm", "bytes": inst * r[3] + n * 2 * 20},
+            "density": {"bound": "alu", "flop": cand * FLOP_CAND + n * NGB_CONFIG1 * FLOP_HIT_DENSITY},
+            "force": {"bound": "alu", "flop": cand * FLOP_CAND + n * (NGB_CONFIG1 - 1) * FLOP_HIT_FORCE},
+        }
+
+    def close(self):
+        self.sph.sph_batch_destroy(self.batch)
+        self.sph.sph_store_destroy(self.store)
+
+
+def build_config1(sph, seed):
+    import sph_inputs as si
+    parts = si.config1(seed=seed)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 16)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    hmax = np.full(cells.shape[0], ps["h"].max(), dtype=np.float32)      # constant h in configs[1]
+    tasks, n_self, n_pair = sph.sph_tasks_build(cells, hmax)
+    return ps, cells, tasks
+
+
+def time_steps(torch, fn, steps, warmup, flush, world):
+    """per-step CUDA-event times [ms]; L2 flushed (untimed) before every step; barrier + sync on both sides"""
+    for _ in range(warmup):
+        flush()
+        fn()
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush()
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def run_ours(args):
+    import torch
+    rank, world, local = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    import paper_2606_23891_b200 as sph
+    torch.cuda.set_device(local)
+    hbm_peak, sm_max_mhz, peak_src = measured_peaks()
+    ps, cells, tasks = build_config1(sph, seed=1 + rank)          # weak scaling: every rank owns its own box
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)                            # 256 MB > 126 MB L2
+
+    results = {}
+    for name in ([args.layout] if args.layout != "both" else ["split", "aos"]):
+        w = Workload(sph, torch, ps, cells, tasks, name)
+        sampler = ClockSampler(local) if rank == 0 else None
+        t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, world)
+        clocks = sampler.stop() if sampler else None
+        t_e2e = time_steps(torch, w.step_e2e, args.steps, args.warmup, flush, world)
+        # per-kernel durations: events around each launch of each timed-length step (same stream, L2 flushed per step)
+        per = {k: [] for k, _ in w.launches()}
+        for _ in range(args.steps):
+            flush()
+            evs = []
+            for k, fn in w.launches():
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record()
+                evs.append((k, a, b))
+            torch.cuda.synchronize()
+            for k, a, b in evs:
+                per[k].append(a.elapsed_time(b))
+        results[name] = {"w": w, "ms": sum(t_ms) / len(t_ms), "ms_e2e": sum(t_e2e) / len(t_e2e), "clocks": clocks,
+                         "per": {k: sum(v) / len(v) for k, v in per.items()}}
+
+    primary = "split" if "split" in results else args.layout
+    R = results[primary]
+    w = R["w"]
+    ms = dist_max(R["ms"], world, "cuda")
+    ms_e2e = dist_max(R["ms_e2e"], world, "cuda")
+    total_particles = dist_sum(float(w.n), world, "cuda")
+    alg = w.algorithmic()
+    alu_peak = N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12          # TFLOP/s at the maximum SM clock
+    kernels = {}
+    for k, d in R["per"].items():
+        e = {"ms": round(d, 5)}
+        if k in alg:
+            if alg[k]["bound"] == "hbm":
+                e.update(bound="hbm", achieved=round(alg[k]["bytes"] / (d * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s")
+            else:
+                e.update(bound="alu", achieved=round(alg[k]["flop"] / (d * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s")
+            e["frac"] = round(e["achieved"] / e["peak"], 4)
+        kernels[k] = e
+    dominant = max(R["per"], key=R["per"].get)
+    traffic = None
+    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch (from ncu --set full)
+    if os.path.exists(tfile):
+        for line in open(tfile):
+            c = line.strip().split(",")
+            if len(c) >= 3 and c[0] == dominant and c[1] == primary:
+                traffic = float(c[2])
+    roof = dict(kernels[dominant])
+    roof.pop("ms", None)
+    roof.update(kernel=dominant, traffic=traffic, peak_source=peak_src + (" HBM copy bandwidth" if roof.get("bound") == "hbm"
+                else " max SM clock x 148 SMs x 128 FP32 lanes x 2"), launch_ms=round(R["per"][dominant], 5))
+    bi, bo = w.e2e_bytes()
+    cand = w.info.n_candidates
+    line = {
+        "metric": METRIC, "value": total_particles / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "layout": primary, "store": "HBM", "tasks": int(w.info.n_tasks), "instances_per_loop": int(w.info.n_instances),
+                   "candidate_pairs_per_loop": int(cand), "l2": "flushed before every step (256 MB fill, untimed)",
+                   "sharding": "one independent box per rank, no collective"},
+        "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},
+        "instances_per_s": {k: w.info.n_instances / (R["per"][k] * 1e-3) for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out")},
+        "e2e": {"value": total_particles / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
+                "ms_per_step": ms_e2e},
+        "gpu_launches": 9 * args.steps,
+        "clocks": R["clocks"],
+        "roofline": roof,
+        "kernels": kernels,
+    }
+    for other, Ro in results.items():
+        if other != primary:
+            line[other] = {"value": Ro["w"].n * world / (dist_max(Ro["ms"], world, "cuda") * 1e-3), "ms_per_step": Ro["ms"],
+                           "e2e_value": Ro["w"].n * world / (dist_max(Ro["ms_e2e"], world, "cuda") * 1e-3),
+                           "e2e_bytes": list(Ro["w"].e2e_bytes()),
+                           "kernels_ms": {k: round(v, 5) for k, v in Ro["per"].items()}}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(budget_s=args.cpu_budget)
+    for Ro in results.values():
+        Ro["w"].close()
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+# --------------------------------------------------------------------------------------------- oracle arm
+
+def oracle_sample_step(orc, ps, cells, tasks, n_self_sample):
+    """one oracle pass (pack, density, unpack, ghost, pack, force, unpack) over the tasks whose first cell is among
+    the first n_self_sample cells; returns the seconds it took"""
+    sel = tasks[tasks["ci"] < n_self_sample]
+    t0 = time.perf_counter()
+    orc.density_cycle(ps, cells, sel)
+    orc.ghost(ps, float(np.float32(5.0 / 3.0)))
+    orc.force_cycle(ps, cells, sel)
+    return time.perf_counter() - t0
+
+
+def oracle_setup():
+    import oracle as orc
+    import sph_inputs as si
+    parts = si.config1(seed=1)
+    perm, cells = orc.cells_build_grid(parts["x"], 16)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    tasks, _, _ = orc.tasks_build(cells, np.full(cells.shape[0], ps["h"].max(), dtype=np.float32))
+    cores = min(os.cpu_count() or 1, 64)
+    orc.set_threads(cores)
+    return orc, ps, cells, tasks, cores
+
+
+def cpu_baseline(budget_s=20.0):
+    """the oracle as it stands, on the host cores, on a bounded sample of configs[1] (about budget_s of CPU wall time)"""
+    orc, ps, cells, tasks, cores = oracle_setup()
+    n_cells = cells.shape[0]
+    probe = 64
+    t_probe = oracle_sample_step(orc, ps, cells, tasks, probe)
+    m = int(max(probe, min(n_cells, probe * budget_s / max(t_probe, 1e-3))))
+    t = oracle_sample_step(orc, ps, cells, tasks, m)
+    particles = int(cells["count"][:m].sum())
+    return {"value": particles / t, "unit": "particles/s", "cores": cores, "kind": "oracle",
+            "sample": f"tasks of the first {m} of {n_cells} cells of configs[1] ({particles} particles), one full step, {t:.1f} s"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    orc, ps, cells, tasks, cores = oracle_setup()
+    n_cells = cells.shape[0]
+    probe = 32
+    t_probe = oracle_sample_step(orc, ps, cells, tasks, probe)
+    per_step_budget = max(0.5, 150.0 / (args.steps + args.warmup))
+    m = int(max(8, min(n_cells, probe * per_step_budget / max(t_probe, 1e-3))))
+    for _ in range(args.warmup):
+        oracle_sample_step(orc, ps, cells, tasks, m)
+    times = [oracle_sample_step(orc, ps, cells, tasks, m) for _ in range(args.steps)]
+    particles = int(cells["count"][:m].sum())
+    sec = sum(times) / len(times)
+    value = particles / sec
+    sample = f"tasks of the first {m} of {n_cells} cells of configs[1] ({particles} particles) per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "layout": "aos", "store": "host DRAM", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "particles/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layout", default="both", choices=["split", "aos", "both"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,467 @@
+// Host side of the C ABI: errors, layouts, attribute sets, the pack/unpack "programs", the particle store
+// and the argument checks in front of every launch.  (include/sph_b200.h documents each entry point.)
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "internal.h"
+
+namespace sph {
+
+static thread_local char g_err[512] = "";
+
+int32_t fail(int32_t code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int field_ncomp(int f) { return (f == SPH_X || f == SPH_V || f == SPH_A || f == SPH_ROT_V) ? 3 : 1; }
+int field_elem_bytes(int f) { return f == SPH_X || f == SPH_ID ? 8 : (f == SPH_TIME_BIN ? 1 : 4); }
+bool field_is_f32(int f) { return f != SPH_X && f != SPH_ID && f != SPH_TIME_BIN; }
+int comp_record_bytes(int f, uint32_t flags) {
+    if (f == SPH_X) return (flags & SPH_ATTR_X_REL_F32) ? 4 : 8;
+    if (f == SPH_ID) return 8;
+    return 4;
+}
+
+int32_t attrset_check(const sph_attrset* set, uint32_t* rec_bytes) {
+    if (!set) return fail(SPH_ERR_INVALID_ARG, "attribute set is NULL");
+    if (set->n == 0 || set->n > SPH_MAX_ATTR) return fail(SPH_ERR_LAYOUT, "attribute set has %u entries (1..%d)", set->n, SPH_MAX_ATTR);
+    if (set->flags & ~SPH_ATTR_X_REL_F32) return fail(SPH_ERR_LAYOUT, "unknown attribute-set flags 0x%x", set->flags);
+    bool seen[SPH_NFIELDS][3] = {};
+    uint32_t bytes = 0;
+    for (uint32_t k = 0; k < set->n; ++k) {
+        const sph_attr& a = set->ent[k];
+        if (a.field >= SPH_NFIELDS) return fail(SPH_ERR_LAYOUT, "entry %u: field %u does not exist", k, a.field);
+        if (a.ncomp < 1 || a.comp0 + a.ncomp > field_ncomp(a.field))
+            return fail(SPH_ERR_LAYOUT, "entry %u: components [%u, %u) out of range for field %u", k, a.comp0, a.comp0 + a.ncomp, a.field);
+        for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
+            if (seen[a.field][c]) return fail(SPH_ERR_LAYOUT, "field %u component %u is listed twice", a.field, c);
+            seen[a.field][c] = true;
+        }
+        bytes += a.ncomp * comp_record_bytes(a.field, set->flags);
+    }
+    if (bytes / 4 > (uint32_t)kMaxRecWords) return fail(SPH_ERR_LAYOUT, "record of %u bytes is too long", bytes);
+    if (rec_bytes) *rec_bytes = bytes;
+    return SPH_OK;
+}
+
+static uint32_t make_div_magic(uint32_t d) {
+    // smallest m with (g*m)>>16 == g/d for all g < 32*d + 4
+    for (uint32_t m = (65536 + d - 1) / d;; ++m) {
+        bool ok = true;
+        for (uint32_t g = 0; g < 32 * d + 4 && ok; ++g) ok = ((g * m) >> 16) == g / d;
+        if (ok) return m;
+    }
+}
+
+static void finish_program(const sph_layout& layout, Program* prog, bool stage) {
+    prog->div_magic = make_div_magic(prog->rec_words);
+    // substructs touched, staging layout (pack only) and 16-byte chunk masks
+    prog->n_sub_used = 0;
+    uint32_t smem = 0;
+    for (uint32_t s = 0; s < layout.n_sub; ++s) {
+        bool used = false;
+        uint32_t mask = 0;
+        const uint32_t stride = layout.stride[s];
+        const bool pow2 = stride >= 32 && (stride & (stride - 1)) == 0 && stride <= 512;
+        for (uint32_t w = 0; w < prog->rec_words; ++w) {
+            const WordDesc& wd = prog->word[w];
+            if (wd.kind == W_SKIP || wd.sub != s) continue;
+            used = true;
+            const uint32_t nbytes = wd.kind == W_XREL ? 8 : (wd.kind == W_TIMEBIN || wd.kind == W_ASSIGN_BYTE ? 1 : 4);
+            for (uint32_t b = wd.off; b < wd.off + nbytes; ++b) mask |= 1u << (b / 16);
+        }
+        if (!used) continue;
+        const uint32_t u = prog->n_sub_used++;
+        prog->sub_used[u] = (uint8_t)s;
+        prog->chunk_mask[u] = pow2 ? mask : 0xFFFFFFFFu;
+        prog->smem_base[u] = smem;
+        if (stage) smem += 32 * stride + 32;
+        for (uint32_t w = 0; w < prog->rec_words; ++w)
+            if (prog->word[w].kind != W_SKIP && prog->word[w].sub == s) prog->word[w].used_idx = (uint8_t)u;
+    }
+    prog->smem_per_warp = (smem + 15) & ~15u;
+}
+
+int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog) {
+    uint32_t rec_bytes = 0;
+    if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
+    std::memset(prog, 0, sizeof(*prog));
+    prog->rec_words = rec_bytes / 4;
+    uint32_t w = 0;
+    for (uint32_t k = 0; k < set.n; ++k) {
+        const sph_attr& a = set.ent[k];
+        const auto& loc = layout.loc[a.field];
+        for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
+            const uint16_t off = (uint16_t)(loc.off + c * field_elem_bytes(a.field));
+            if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32)) {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_XREL, (uint8_t)c, 0, 0};
+            } else if (a.field == SPH_X || a.field == SPH_ID) {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_COPY, 0, 0, 0};
+                prog->word[w++] = WordDesc{(uint16_t)(off + 4), loc.sub, (uint8_t)W_COPY, 0, 0, 0};
+            } else if (a.field == SPH_TIME_BIN) {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_TIMEBIN, 0, 0, 0};
+            } else {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_COPY, 0, 0, 0};
+            }
+        }
+    }
+    finish_program(layout, prog, true);
+    return SPH_OK;
+}
+
+int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, int32_t mode, Program* prog) {
+    uint32_t rec_bytes = 0;
+    if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
+    if (mode != SPH_UNPACK_REDUCE && mode != SPH_UNPACK_ASSIGN) return fail(SPH_ERR_INVALID_ARG, "unknown unpack mode %d", mode);
+    std::memset(prog, 0, sizeof(*prog));
+    prog->rec_words = rec_bytes / 4;
+    uint32_t w = 0;
+    for (uint32_t k = 0; k < set.n; ++k) {
+        const sph_attr& a = set.ent[k];
+        const auto& loc = layout.loc[a.field];
+        if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32))
+            return fail(SPH_ERR_UNSUPPORTED, "X packed as relative f32 cannot be unpacked (the frame shift is not invertible in f32)");
+        const bool is_sum = a.field == SPH_RHO || a.field == SPH_RHO_DH || a.field == SPH_WCOUNT || a.field == SPH_WCOUNT_DH ||
+                            a.field == SPH_A || a.field == SPH_DU_DT;
+        for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
+            const uint16_t off = (uint16_t)(loc.off + c * field_elem_bytes(a.field));
+            if (a.field == SPH_X || a.field == SPH_ID) {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_ASSIGN, 0, 0, 0};
+                prog->word[w++] = WordDesc{(uint16_t)(off + 4), loc.sub, (uint8_t)W_ASSIGN, 0, 0, 0};
+            } else if (a.field == SPH_TIME_BIN) {
+                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_ASSIGN_BYTE, 0, 0, 0};
+            } else {
+                uint8_t kind = W_ASSIGN;
+                if (mode == SPH_UNPACK_REDUCE && is_sum) kind = W_SUM;
+                if (mode == SPH_UNPACK_REDUCE && a.field == SPH_V_SIG) kind = W_MAX;
+                prog->word[w++] = WordDesc{off, loc.sub, kind, 0, 0, 0};
+            }
+        }
+    }
+    finish_program(layout, prog, false);
+    return SPH_OK;
+}
+
+static int32_t store_check(const sph_store* s) {
+    if (!s) return fail(SPH_ERR_INVALID_ARG, "store is NULL");
+    return SPH_OK;
+}
+
+}  // namespace sph
+
+using namespace sph;
+
+extern "C" {
+
+int32_t sph_last_error(char* msg, size_t cap) {
+    if (!msg || cap == 0) return SPH_ERR_INVALID_ARG;
+    std::snprintf(msg, cap, "%s", g_err);
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------ layouts
+
+static void set_loc(sph_layout* l, int field, uint8_t sub, uint16_t off) { l->loc[field].sub = sub; l->loc[field].pad = 0; l->loc[field].off = off; }
+
+int32_t sph_layout_aos(sph_layout* out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    std::memset(out, 0, sizeof(*out));
+    out->n_sub = 1;
+    out->stride[0] = SPH_AOS_BYTES;
+    static const uint16_t off[SPH_NFIELDS] = {0, 24, 36, 48, 52, 56, 60, 64, 68, 72, 76, 80, 84, 96, 100, 104, 112, 120};
+    for (int f = 0; f < SPH_NFIELDS; ++f) set_loc(out, f, 0, off[f]);
+    return SPH_OK;
+}
+
+int32_t sph_layout_split(sph_layout* out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    std::memset(out, 0, sizeof(*out));
+    out->n_sub = 6;
+    const uint32_t stride[6] = {32, 16, 24, 20, 16, 16};
+    for (int s = 0; s < 6; ++s) out->stride[s] = stride[s];
+    set_loc(out, SPH_X, 0, 0);       set_loc(out, SPH_H, 0, 24);        set_loc(out, SPH_MASS, 0, 28);
+    set_loc(out, SPH_RHO, 1, 0);     set_loc(out, SPH_RHO_DH, 1, 4);    set_loc(out, SPH_WCOUNT, 1, 8);  set_loc(out, SPH_WCOUNT_DH, 1, 12);
+    set_loc(out, SPH_V, 2, 0);       set_loc(out, SPH_U, 2, 12);        set_loc(out, SPH_P, 2, 16);      set_loc(out, SPH_CS, 2, 20);
+    set_loc(out, SPH_A, 3, 0);       set_loc(out, SPH_DU_DT, 3, 12);    set_loc(out, SPH_V_SIG, 3, 16);
+    set_loc(out, SPH_ID, 4, 0);      set_loc(out, SPH_TIME_BIN, 4, 8);
+    set_loc(out, SPH_DIV_V, 5, 0);   set_loc(out, SPH_ROT_V, 5, 4);
+    return SPH_OK;
+}
+
+int32_t sph_layout_validate(const sph_layout* l) {
+    if (!l) return fail(SPH_ERR_INVALID_ARG, "layout is NULL");
+    if (l->n_sub < 1 || l->n_sub > SPH_MAX_SUB) return fail(SPH_ERR_LAYOUT, "n_sub = %u (1..%d)", l->n_sub, SPH_MAX_SUB);
+    std::vector<std::vector<uint8_t>> used(l->n_sub);
+    for (uint32_t s = 0; s < l->n_sub; ++s) {
+        if (l->stride[s] == 0 || l->stride[s] % 4 != 0 || l->stride[s] > 4096) return fail(SPH_ERR_LAYOUT, "substruct %u: stride %u", s, l->stride[s]);
+        used[s].assign(l->stride[s], 0);
+    }
+    for (int f = 0; f < SPH_NFIELDS; ++f) {
+        const auto& loc = l->loc[f];
+        if (loc.sub >= l->n_sub) return fail(SPH_ERR_LAYOUT, "field %d: substruct %u does not exist", f, loc.sub);
+        const uint32_t eb = field_elem_bytes(f), nb = eb * field_ncomp(f);
+        const uint32_t align = f == SPH_TIME_BIN ? 1 : (eb == 8 ? 8 : 4);
+        if (loc.off % align) return fail(SPH_ERR_LAYOUT, "field %d: offset %u is not %u-byte aligned", f, loc.off, align);
+        if (eb == 8 && l->stride[loc.sub] % 8) return fail(SPH_ERR_LAYOUT, "field %d: 8-byte member in a substruct of stride %u", f, l->stride[loc.sub]);
+        if (loc.off + nb > l->stride[loc.sub]) return fail(SPH_ERR_LAYOUT, "field %d: [%u, %u) exceeds stride %u", f, loc.off, loc.off + nb, l->stride[loc.sub]);
+        for (uint32_t b = loc.off; b < loc.off + nb; ++b) {
+            if (used[loc.sub][b]) return fail(SPH_ERR_LAYOUT, "field %d overlaps another field at substruct %u byte %u", f, loc.sub, b);
+            used[loc.sub][b] = 1;
+        }
+    }
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------ attribute sets
+
+int32_t sph_attrset_canonical(int32_t which, sph_attrset* out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    std::memset(out, 0, sizeof(*out));
+    auto add = [&](int field) { out->ent[out->n++] = sph_attr{(uint8_t)field, 0, (uint8_t)field_ncomp(field), 0}; };
+    switch (which) {
+        case SPH_SET_DENSITY_IN: out->flags = SPH_ATTR_X_REL_F32; add(SPH_X); add(SPH_H); add(SPH_MASS); break;
+        case SPH_SET_DENSITY_OUT: add(SPH_RHO); add(SPH_RHO_DH); add(SPH_WCOUNT); add(SPH_WCOUNT_DH); break;
+        case SPH_SET_FORCE_IN:
+            out->flags = SPH_ATTR_X_REL_F32;
+            add(SPH_X); add(SPH_H); add(SPH_MASS); add(SPH_RHO); add(SPH_RHO_DH); add(SPH_V); add(SPH_U); add(SPH_P); add(SPH_CS);
+            break;
+        case SPH_SET_FORCE_OUT: add(SPH_A); add(SPH_DU_DT); add(SPH_V_SIG); break;
+        default: return fail(SPH_ERR_INVALID_ARG, "unknown canonical attribute set %d", which);
+    }
+    return SPH_OK;
+}
+
+int32_t sph_attrset_record_bytes(const sph_attrset* set, uint32_t* bytes_out) {
+    if (!bytes_out) return fail(SPH_ERR_INVALID_ARG, "bytes_out is NULL");
+    return attrset_check(set, bytes_out);
+}
+
+// ------------------------------------------------------------------ store
+
+int32_t sph_store_sub_bytes(const sph_layout* layout, uint64_t n, uint32_t sub, uint64_t* bytes_out) {
+    if (!layout || !bytes_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    if (sub >= layout->n_sub) return fail(SPH_ERR_RANGE, "substruct %u of %u", sub, layout->n_sub);
+    *bytes_out = ((n * layout->stride[sub] + kTailBytes + 255) / 256) * 256;
+    return SPH_OK;
+}
+
+int32_t sph_store_create(const sph_layout* layout, uint64_t n, int32_t mem_kind, void* const* ext_ptrs, sph_store** out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (int32_t rc = sph_layout_validate(layout)) return rc;
+    if (mem_kind != SPH_MEM_DEVICE && mem_kind != SPH_MEM_HOST_PINNED) return fail(SPH_ERR_INVALID_ARG, "mem_kind %d", mem_kind);
+    if (n == 0 || n >= (1ull << 32) - 64) return fail(SPH_ERR_RANGE, "n = %llu particles (1 .. 2^32-65)", (unsigned long long)n);
+    sph_store* s = new (std::nothrow) sph_store();
+    if (!s) return fail(SPH_ERR_ALLOC, "host allocation failed");
+    s->layout = *layout;
+    s->n = n;
+    s->mem_kind = mem_kind;
+    for (uint32_t k = 0; k < layout->n_sub; ++k) {
+        sph_store_sub_bytes(layout, n, k, &s->bytes[k]);
+        if (ext_ptrs) {
+            if (!ext_ptrs[k] || ((uintptr_t)ext_ptrs[k] & 255)) { delete s; return fail(SPH_ERR_INVALID_ARG, "ext_ptrs[%u] is NULL or not 256-byte aligned", k); }
+            s->base[k] = (char*)ext_ptrs[k];
+        } else {
+            cudaError_t e = mem_kind == SPH_MEM_DEVICE ? cudaMalloc((void**)&s->base[k], s->bytes[k])
+                                                       : cudaHostAlloc((void**)&s->base[k], s->bytes[k], cudaHostAllocMapped | cudaHostAllocPortable);
+            if (e != cudaSuccess) {
+                sph_store_destroy(s);
+                return fail(e == cudaErrorMemoryAllocation ? SPH_ERR_ALLOC : SPH_ERR_CUDA, "store allocation of %llu bytes: %s",
+                            (unsigned long long)s->bytes[k], cudaGetErrorString(e));
+            }
+            s->owned[k] = true;
+            e = mem_kind == SPH_MEM_DEVICE ? cudaMemset(s->base[k], 0, s->bytes[k]) : (std::memset(s->base[k], 0, s->bytes[k]), cudaSuccess);
+            if (e != cudaSuccess) { sph_store_destroy(s); return fail(SPH_ERR_CUDA, "cudaMemset: %s", cudaGetErrorString(e)); }
+        }
+    }
+    *out = s;
+    return SPH_OK;
+}
+
+int32_t sph_store_destroy(sph_store* s) {
+    if (!s) return SPH_OK;
+    for (uint32_t k = 0; k < SPH_MAX_SUB; ++k)
+        if (s->owned[k] && s->base[k]) { if (s->mem_kind == SPH_MEM_DEVICE) cudaFree(s->base[k]); else cudaFreeHost(s->base[k]); }
+    delete s;
+    return SPH_OK;
+}
+
+int32_t sph_store_sub_ptr(const sph_store* s, uint32_t sub, void** ptr_out) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!ptr_out) return fail(SPH_ERR_INVALID_ARG, "ptr_out is NULL");
+    if (sub >= s->layout.n_sub) return fail(SPH_ERR_RANGE, "substruct %u of %u", sub, s->layout.n_sub);
+    *ptr_out = s->base[sub];
+    return SPH_OK;
+}
+
+static int32_t sub_copy_check(const sph_store* s, uint32_t sub, const void* host, uint64_t bytes) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!host) return fail(SPH_ERR_INVALID_ARG, "host pointer is NULL");
+    if (sub >= s->layout.n_sub) return fail(SPH_ERR_RANGE, "substruct %u of %u", sub, s->layout.n_sub);
+    if (bytes != s->n * s->layout.stride[sub])
+        return fail(SPH_ERR_RANGE, "%llu bytes given, substruct %u holds %llu", (unsigned long long)bytes, sub, (unsigned long long)(s->n * s->layout.stride[sub]));
+    return SPH_OK;
+}
+
+int32_t sph_store_upload_sub(sph_store* s, uint32_t sub, const void* host_src, uint64_t bytes, void* stream) {
+    if (int32_t rc = sub_copy_check(s, sub, host_src, bytes)) return rc;
+    SPH_CUDA_TRY(cudaMemcpyAsync(s->base[sub], host_src, bytes, cudaMemcpyDefault, (cudaStream_t)stream));
+    return SPH_OK;
+}
+
+int32_t sph_store_download_sub(const sph_store* s, uint32_t sub, void* host_dst, uint64_t bytes, void* stream) {
+    if (int32_t rc = sub_copy_check(s, sub, host_dst, bytes)) return rc;
+    SPH_CUDA_TRY(cudaMemcpyAsync(host_dst, s->base[sub], bytes, cudaMemcpyDefault, (cudaStream_t)stream));
+    return SPH_OK;
+}
+
+// host-side (de)interleave between the canonical AoS record and one substruct array
+static void transform(const sph_layout& aos, const sph_layout& lay, uint32_t sub, const char* src_aos, char* sub_buf, uint64_t n, bool to_sub) {
+    for (int f = 0; f < SPH_NFIELDS; ++f) {
+        if (lay.loc[f].sub != sub) continue;
+        const uint32_t nb = field_elem_bytes(f) * field_ncomp(f), so = aos.loc[f].off, dof = lay.loc[f].off, st = lay.stride[sub];
+        if (to_sub) for (uint64_t p = 0; p < n; ++p) std::memcpy(sub_buf + p * st + dof, src_aos + p * SPH_AOS_BYTES + so, nb);
+        else        for (uint64_t p = 0; p < n; ++p) std::memcpy(const_cast<char*>(src_aos) + p * SPH_AOS_BYTES + so, sub_buf + p * st + dof, nb);
+    }
+}
+
+int32_t sph_store_import_aos(sph_store* s, const void* host_aos, uint64_t n) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!host_aos) return fail(SPH_ERR_INVALID_ARG, "host_aos is NULL");
+    if (n != s->n) return fail(SPH_ERR_RANGE, "n = %llu but the store holds %llu", (unsigned long long)n, (unsigned long long)s->n);
+    sph_layout aos;
+    sph_layout_aos(&aos);
+    SPH_CUDA_TRY(cudaDeviceSynchronize());
+    for (uint32_t k = 0; k < s->layout.n_sub; ++k) {
+        const uint64_t nb = n * s->layout.stride[k];
+        if (s->mem_kind == SPH_MEM_HOST_PINNED) {
+            std::memset(s->base[k], 0, nb);
+            transform(aos, s->layout, k, (const char*)host_aos, s->base[k], n, true);
+        } else {
+            std::vector<char> tmp;
+            try { tmp.assign(nb, 0); } catch (...) { return fail(SPH_ERR_ALLOC, "host staging of %llu bytes", (unsigned long long)nb); }
+            transform(aos, s->layout, k, (const char*)host_aos, tmp.data(), n, true);
+            SPH_CUDA_TRY(cudaMemcpy(s->base[k], tmp.data(), nb, cudaMemcpyHostToDevice));
+        }
+    }
+    return SPH_OK;
+}
+
+int32_t sph_store_export_aos(const sph_store* s, void* host_aos, uint64_t n) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!host_aos) return fail(SPH_ERR_INVALID_ARG, "host_aos is NULL");
+    if (n != s->n) return fail(SPH_ERR_RANGE, "n = %llu but the store holds %llu", (unsigned long long)n, (unsigned long long)s->n);
+    sph_layout aos;
+    sph_layout_aos(&aos);
+    SPH_CUDA_TRY(cudaDeviceSynchronize());
+    std::memset(host_aos, 0, n * SPH_AOS_BYTES);
+    for (uint32_t k = 0; k < s->layout.n_sub; ++k) {
+        const uint64_t nb = n * s->layout.stride[k];
+        if (s->mem_kind == SPH_MEM_HOST_PINNED) {
+            transform(aos, s->layout, k, (const char*)host_aos, s->base[k], n, false);
+        } else {
+            std::vector<char> tmp;
+            try { tmp.resize(nb); } catch (...) { return fail(SPH_ERR_ALLOC, "host staging of %llu bytes", (unsigned long long)nb); }
+            SPH_CUDA_TRY(cudaMemcpy(tmp.data(), s->base[k], nb, cudaMemcpyDeviceToHost));
+            transform(aos, s->layout, k, (const char*)host_aos, tmp.data(), n, false);
+        }
+    }
+    return SPH_OK;
+}
+
+int32_t sph_store_set_cells(sph_store* s, const sph_cell* cells, uint32_t n_cells) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!cells || n_cells == 0) return fail(SPH_ERR_INVALID_ARG, "no cells");
+    std::vector<std::pair<uint64_t, uint64_t>> ranges;
+    ranges.reserve(n_cells);
+    for (uint32_t c = 0; c < n_cells; ++c) {
+        if (cells[c].first + cells[c].count > s->n) return fail(SPH_ERR_RANGE, "cell %u: [%llu, +%u) exceeds the store (%llu)", c,
+                                                               (unsigned long long)cells[c].first, cells[c].count, (unsigned long long)s->n);
+        if (cells[c].count) ranges.emplace_back(cells[c].first, cells[c].first + cells[c].count);
+    }
+    std::sort(ranges.begin(), ranges.end());
+    for (size_t k = 1; k < ranges.size(); ++k)
+        if (ranges[k].first < ranges[k - 1].second) return fail(SPH_ERR_RANGE, "cell ranges overlap at particle %llu", (unsigned long long)ranges[k].first);
+    s->cells.assign(cells, cells + n_cells);
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------ hot path entry points
+
+int32_t sph_store_zero(sph_store* s, const sph_attrset* set, void* stream) {
+    if (int32_t rc = store_check(s)) return rc;
+    uint32_t rb;
+    if (int32_t rc = attrset_check(set, &rb)) return rc;
+    for (uint32_t k = 0; k < set->n; ++k)
+        if (!field_is_f32(set->ent[k].field)) return fail(SPH_ERR_UNSUPPORTED, "sph_store_zero handles f32 fields only (field %u)", set->ent[k].field);
+    Program prog;
+    if (int32_t rc = build_unpack_program(s->layout, *set, SPH_UNPACK_ASSIGN, &prog)) return rc;
+    return launch_zero(s->view(), s->n, prog, (cudaStream_t)stream);
+}
+
+int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes, void* stream) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
+    Program prog;
+    if (int32_t rc = build_pack_program(s->layout, *set, &prog)) return rc;
+    const OffsetTable* ot = find_offsets(b, prog.rec_words * 4);
+    if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
+    if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
+    if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    return launch_pack(s->view(), b, prog, ot->d_off128, (char*)d_buf, (cudaStream_t)stream);
+}
+
+int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
+    Program prog;
+    if (int32_t rc = build_unpack_program(s->layout, *set, mode, &prog)) return rc;
+    const OffsetTable* ot = find_offsets(b, prog.rec_words * 4);
+    if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
+    if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
+    if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    bool all_assign = true;
+    for (uint32_t w = 0; w < prog.rec_words; ++w) all_assign &= prog.word[w].kind == W_ASSIGN || prog.word[w].kind == W_ASSIGN_BYTE;
+    return launch_unpack(s->view(), b, prog, ot->d_off128, (const char*)d_buf, all_assign, (cudaStream_t)stream);
+}
+
+static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, uint32_t rec_in,
+                          uint32_t rec_out, const OffsetTable** oin, const OffsetTable** oout) {
+    if (!b || !d_in || !d_out) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    *oin = find_offsets(b, rec_in);
+    *oout = find_offsets(b, rec_out);
+    if (!*oin || !*oout) return fail(SPH_ERR_INVALID_ARG, "canonical offset tables missing");
+    if (in_bytes < (*oin)->total) return fail(SPH_ERR_RANGE, "input buffer of %llu bytes, %llu needed", (unsigned long long)in_bytes, (unsigned long long)(*oin)->total);
+    if (out_bytes < (*oout)->total) return fail(SPH_ERR_RANGE, "output buffer of %llu bytes, %llu needed", (unsigned long long)out_bytes, (unsigned long long)(*oout)->total);
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    return SPH_OK;
+}
+
+int32_t sph_density(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, void* stream) {
+    const OffsetTable *oin = nullptr, *oout = nullptr;
+    if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 20, 16, &oin, &oout)) return rc;
+    return launch_density(b, oin->d_off128, oout->d_off128, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+}
+
+int32_t sph_force(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, const sph_params* prm, void* stream) {
+    if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
+    const OffsetTable *oin = nullptr, *oout = nullptr;
+    if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 52, 20, &oin, &oout)) return rc;
+    return launch_force(b, oin->d_off128, oout->d_off128, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+}
+
+int32_t sph_ghost(sph_store* s, const sph_params* prm, void* stream) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
+    return launch_ghost(s->view(), s->n, s->layout, *prm, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,192 @@
+// Batches ("bundles"): the immutable device tables every kernel of the hot path indexes.
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+#include "internal.h"
+
+using namespace sph;
+
+namespace {
+
+template <class T>
+int32_t upload(const std::vector<T>& v, T** d) {
+    *d = nullptr;
+    if (v.empty()) return SPH_OK;
+    cudaError_t e = cudaMalloc((void**)d, v.size() * sizeof(T));
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? SPH_ERR_ALLOC : SPH_ERR_CUDA, "cudaMalloc(%zu): %s", v.size() * sizeof(T), cudaGetErrorString(e));
+    e = cudaMemcpy(*d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return fail(SPH_ERR_CUDA, "cudaMemcpy: %s", cudaGetErrorString(e));
+    return SPH_OK;
+}
+
+}  // namespace
+
+namespace sph {
+
+const OffsetTable* find_offsets(const sph_batch* b, uint32_t rec_bytes) {
+    auto it = b->offsets.find(rec_bytes);
+    return it == b->offsets.end() ? nullptr : &it->second;
+}
+
+// Block offsets for one record size: every block starts at the next multiple of 128 bytes, every segment at
+// the next multiple of 256 bytes (a segment is laid out exactly like a stand-alone batch of its tasks).
+int32_t ensure_offsets(sph_batch* b, uint32_t rec_bytes, const OffsetTable** out) {
+    auto it = b->offsets.find(rec_bytes);
+    if (it != b->offsets.end()) { if (out) *out = &it->second; return SPH_OK; }
+    OffsetTable ot;
+    ot.h_off.resize(b->n_sides);
+    std::vector<uint32_t> off128(b->n_sides);
+    uint64_t run = 0;
+    const uint64_t tps = b->tasks_per_segment ? b->tasks_per_segment : b->n_tasks;
+    for (uint64_t t = 0; t < b->n_tasks; ++t) {
+        if (t % tps == 0) { run = (run + 255) / 256 * 256; ot.seg_off.push_back(run); }
+        for (uint32_t s = b->task_side0[t]; s < b->task_side0[t + 1]; ++s) {
+            ot.h_off[s] = run;
+            off128[s] = (uint32_t)(run / 128);
+            run = (run + (uint64_t)b->sides[s].count * rec_bytes + 127) / 128 * 128;
+        }
+    }
+    ot.total = run;
+    if (run / 128 >= (1ull << 32)) return fail(SPH_ERR_RANGE, "buffer of %llu bytes exceeds the 512 GiB offset range", (unsigned long long)run);
+    if (int32_t rc = upload(off128, &ot.d_off128)) return rc;
+    auto ins = b->offsets.emplace(rec_bytes, std::move(ot));
+    if (out) *out = &ins.first->second;
+    return SPH_OK;
+}
+
+}  // namespace sph
+
+extern "C" {
+
+int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t n_tasks, uint32_t tasks_per_segment, sph_batch** out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!store || !tasks || n_tasks == 0) return fail(SPH_ERR_INVALID_ARG, "store or tasks is NULL, or no tasks");
+    if (store->cells.empty()) return fail(SPH_ERR_INVALID_ARG, "the store has no cell table (sph_store_set_cells)");
+    if (n_tasks >= (1ull << 31)) return fail(SPH_ERR_RANGE, "too many tasks");
+    const uint32_t n_cells = (uint32_t)store->cells.size();
+    sph_batch* b = new (std::nothrow) sph_batch();
+    if (!b) return fail(SPH_ERR_ALLOC, "host allocation failed");
+    b->n_tasks = n_tasks;
+    b->store_n = store->n;
+    b->tasks_per_segment = tasks_per_segment;
+    b->n_segments = tasks_per_segment ? (uint32_t)((n_tasks + tasks_per_segment - 1) / tasks_per_segment) : 1;
+    std::vector<double> frames;
+    std::vector<uint32_t> chunk_side;
+    b->task_side0.resize(n_tasks + 1);
+    b->sides.reserve(2 * n_tasks);
+    frames.reserve(6 * n_tasks);
+    for (uint64_t t = 0; t < n_tasks; ++t) {
+        const sph_task& tk = tasks[t];
+        b->task_side0[t] = (uint32_t)b->sides.size();
+        if (tk.ci < 0 || (uint32_t)tk.ci >= n_cells || tk.cj < -1 || (tk.cj >= 0 && (uint32_t)tk.cj >= n_cells) || tk.cj == tk.ci) {
+            delete b;
+            return fail(SPH_ERR_RANGE, "task %llu references cells (%d, %d); the store has %u", (unsigned long long)t, tk.ci, tk.cj, n_cells);
+        }
+        for (int side = 0; side < (tk.cj >= 0 ? 2 : 1); ++side) {
+            const uint32_t c = (uint32_t)(side == 0 ? tk.ci : tk.cj);
+            const sph_cell& ce = store->cells[c];
+            SideRec sr{(uint32_t)ce.first, ce.count, (uint32_t)chunk_side.size(), c};
+            const uint32_t sidx = (uint32_t)b->sides.size();
+            for (uint32_t k = 0; k < ce.count; k += 32) chunk_side.push_back(sidx);
+            b->sides.push_back(sr);
+            const double* fr = side == 0 ? tk.frame_i : tk.frame_j;
+            frames.insert(frames.end(), fr, fr + 3);
+            b->n_instances += ce.count;
+            b->max_count = std::max(b->max_count, ce.count);
+        }
+        const uint64_t ni = store->cells[tk.ci].count;
+        if (tk.cj >= 0) { ++b->n_pair; b->n_candidates += 2 * ni * store->cells[tk.cj].count; }
+        else { ++b->n_self; b->n_candidates += ni * ni; }
+    }
+    b->task_side0[n_tasks] = (uint32_t)b->sides.size();
+    b->n_sides = (uint32_t)b->sides.size();
+    b->n_chunks = (uint32_t)chunk_side.size();
+
+    // per-cell occurrence lists in ascending (task, side) order = ascending side index
+    std::vector<uint32_t> occ_count(n_cells, 0);
+    for (const SideRec& s : b->sides) ++occ_count[s.cell];
+    std::vector<uint32_t> occ_start(n_cells + 1, 0);
+    for (uint32_t c = 0; c < n_cells; ++c) occ_start[c + 1] = occ_start[c] + occ_count[c];
+    std::vector<uint32_t> occ_side(b->n_sides), cur(occ_start.begin(), occ_start.end() - 1);
+    for (uint32_t s = 0; s < b->n_sides; ++s) occ_side[cur[b->sides[s].cell]++] = s;
+    std::vector<CellChunk> cell_chunks;
+    for (uint32_t c = 0; c < n_cells; ++c) {
+        if (!occ_count[c]) continue;
+        ++b->n_cells_touched;
+        const sph_cell& ce = store->cells[c];
+        for (uint32_t k = 0; k < ce.count; k += 32)
+            cell_chunks.push_back(CellChunk{(uint32_t)ce.first + k, std::min(32u, ce.count - k), k, occ_start[c], occ_count[c]});
+    }
+    b->n_cell_chunks = (uint32_t)cell_chunks.size();
+    b->n_occ = b->n_sides;
+
+    // loop scheduling order: heaviest tasks first (counts differ by 30x on the octree configs)
+    std::vector<uint32_t> order(n_tasks);
+    std::iota(order.begin(), order.end(), 0u);
+    auto work = [&](uint32_t t) {
+        const uint64_t ni = store->cells[tasks[t].ci].count;
+        return tasks[t].cj >= 0 ? 2 * ni * store->cells[tasks[t].cj].count : ni * ni;
+    };
+    bool uniform = true;
+    for (uint64_t t = 1; t < n_tasks && uniform; ++t) uniform = work((uint32_t)t) == work(0);
+    if (!uniform) std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return work(x) > work(y); });
+
+    int32_t rc = upload(b->sides, &b->d_sides);
+    if (!rc) rc = upload(frames, &b->d_frames);
+    if (!rc) rc = upload(chunk_side, &b->d_chunk_side);
+    if (!rc) rc = upload(b->task_side0, &b->d_task_side0);
+    if (!rc) rc = upload(order, &b->d_task_order);
+    if (!rc) rc = upload(cell_chunks, &b->d_cell_chunks);
+    if (!rc) rc = upload(occ_side, &b->d_occ_side);
+    for (uint32_t rec : {16u, 20u, 52u})
+        if (!rc) rc = ensure_offsets(b, rec, nullptr);
+    if (rc) { sph_batch_destroy(b); return rc; }
+    *out = b;
+    return SPH_OK;
+}
+
+int32_t sph_batch_destroy(sph_batch* b) {
+    if (!b) return SPH_OK;
+    cudaFree(b->d_sides); cudaFree(b->d_frames); cudaFree(b->d_chunk_side); cudaFree(b->d_task_side0);
+    cudaFree(b->d_task_order); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_side);
+    for (auto& kv : b->offsets) cudaFree(kv.second.d_off128);
+    delete b;
+    return SPH_OK;
+}
+
+int32_t sph_batch_get_info(const sph_batch* b, sph_batch_info* info) {
+    if (!b || !info) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    info->n_tasks = b->n_tasks; info->n_self = b->n_self; info->n_pair = b->n_pair; info->n_sides = b->n_sides;
+    info->n_instances = b->n_instances; info->n_candidates = b->n_candidates; info->n_cells_touched = b->n_cells_touched;
+    info->n_segments = b->n_segments; info->max_count = b->max_count;
+    return SPH_OK;
+}
+
+int32_t sph_batch_buffer_bytes(sph_batch* b, const sph_attrset* set, uint64_t* bytes_out) {
+    if (!b || !bytes_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    uint32_t rec;
+    if (int32_t rc = attrset_check(set, &rec)) return rc;
+    const OffsetTable* ot;
+    if (int32_t rc = ensure_offsets(b, rec, &ot)) return rc;
+    *bytes_out = ot->total;
+    return SPH_OK;
+}
+
+int32_t sph_batch_block_offsets(sph_batch* b, const sph_attrset* set, uint64_t* off_out, uint64_t* seg_off_out) {
+    if (!b || !off_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    uint32_t rec;
+    if (int32_t rc = attrset_check(set, &rec)) return rc;
+    const OffsetTable* ot;
+    if (int32_t rc = ensure_offsets(b, rec, &ot)) return rc;
+    for (uint64_t t = 0; t < b->n_tasks; ++t) {
+        off_out[2 * t] = ot->h_off[b->task_side0[t]];
+        off_out[2 * t + 1] = b->task_side0[t + 1] - b->task_side0[t] == 2 ? ot->h_off[b->task_side0[t] + 1] : UINT64_MAX;
+    }
+    if (seg_off_out) std::copy(ot->seg_off.begin(), ot->seg_off.end(), seg_off_out);
+    return SPH_OK;
+}
+
+}  // extern "C"

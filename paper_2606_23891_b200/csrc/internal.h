@@ -1,0 +1,138 @@
+// Internal declarations of libsph_b200 (not part of the C ABI; see include/sph_b200.h).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <map>
+#include <vector>
+
+#include "sph_b200.h"
+
+namespace sph {
+
+int32_t fail(int32_t code, const char* fmt, ...);
+#define SPH_CUDA_TRY(expr)                                                                             \
+    do {                                                                                               \
+        cudaError_t e_ = (expr);                                                                       \
+        if (e_ != cudaSuccess) return ::sph::fail(SPH_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+    } while (0)
+
+// ---- field metadata ----
+int field_ncomp(int field);                 // 3 for X, V, A, ROT_V, else 1
+int field_elem_bytes(int field);            // bytes of one component in the STORE: X 8, ID 8, TIME_BIN 1, else 4
+int comp_record_bytes(int field, uint32_t flags);   // bytes of one component in a RECORD
+bool field_is_f32(int field);
+int32_t attrset_check(const sph_attrset* set, uint32_t* rec_bytes);
+
+constexpr int kMaxRecWords = 48;   // all 26 scalars + raw x (6 words) + id (2 words) = 33; a little slack
+constexpr uint32_t kTailBytes = 64;   // readable slack after every substruct array
+
+// ---- device-side views ----
+struct StoreView {
+    char* base[SPH_MAX_SUB];
+    uint32_t stride[SPH_MAX_SUB];
+};
+
+// one block of a buffer = one side of one task
+struct SideRec {
+    uint32_t first;    // first particle of the cell
+    uint32_t count;    // particles in the cell
+    uint32_t chunk0;   // index of the block's first 32-particle chunk in the pack chunk table
+    uint32_t cell;
+};
+
+// one 32-particle slice of a cell that occurs in the batch (work item of unpack)
+struct CellChunk {
+    uint32_t first;    // first particle of the slice
+    uint32_t count;    // 1..32
+    uint32_t k0;       // offset of the slice inside its cell (multiple of 32)
+    uint32_t occ0;     // [occ0, occ0 + nocc): the cell's blocks in ascending (task, side) order
+    uint32_t nocc;
+};
+
+// word kinds of the pack / unpack programs
+enum : uint32_t { W_COPY = 0, W_XREL = 1, W_TIMEBIN = 2,            // pack
+                  W_SUM = 3, W_MAX = 4, W_ASSIGN = 5, W_ASSIGN_BYTE = 6, W_SKIP = 7 };   // unpack
+
+// Per record word: where it lives in the store.  Built on the host from (layout, attribute set).
+struct WordDesc {
+    uint16_t off;      // byte offset inside the substruct
+    uint8_t sub;       // substruct
+    uint8_t kind;      // W_*
+    uint8_t dim;       // W_XREL: coordinate axis
+    uint8_t used_idx;  // index of `sub` in Program::sub_used
+    uint16_t pad;
+};
+
+struct Program {
+    uint32_t rec_words;
+    uint32_t div_magic;            // k = (g * div_magic) >> 16 == g / rec_words for g < 32 * rec_words + 4
+    uint32_t n_sub_used;
+    uint32_t smem_per_warp;        // bytes of staging per warp (pack)
+    uint8_t sub_used[SPH_MAX_SUB];
+    uint32_t chunk_mask[SPH_MAX_SUB];   // per used substruct: needed 16-byte chunks (power-of-two strides), else ~0
+    uint32_t smem_base[SPH_MAX_SUB];    // staging offset of each used substruct inside the warp's region
+    WordDesc word[kMaxRecWords];
+};
+
+int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog);
+int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, int32_t mode, Program* prog);
+
+struct OffsetTable {
+    uint32_t* d_off128 = nullptr;          // per side: block start in units of 128 bytes
+    std::vector<uint64_t> h_off;           // per side, bytes
+    std::vector<uint64_t> seg_off;         // per segment, bytes
+    uint64_t total = 0;
+};
+
+}  // namespace sph
+
+struct sph_store {
+    sph_layout layout;
+    uint64_t n = 0;
+    int32_t mem_kind = SPH_MEM_DEVICE;
+    char* base[SPH_MAX_SUB] = {};
+    bool owned[SPH_MAX_SUB] = {};
+    uint64_t bytes[SPH_MAX_SUB] = {};
+    std::vector<sph_cell> cells;
+    sph::StoreView view() const {
+        sph::StoreView v{};
+        for (uint32_t s = 0; s < layout.n_sub; ++s) { v.base[s] = base[s]; v.stride[s] = layout.stride[s]; }
+        return v;
+    }
+};
+
+struct sph_batch {
+    uint64_t n_tasks = 0, n_self = 0, n_pair = 0;
+    uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0;
+    uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
+    std::vector<sph::SideRec> sides;          // host copy
+    std::vector<uint32_t> task_side0;         // n_tasks + 1
+    // device tables
+    sph::SideRec* d_sides = nullptr;
+    double* d_frames = nullptr;               // 3 per side
+    uint32_t* d_chunk_side = nullptr;         // pack chunk -> side
+    uint32_t* d_task_side0 = nullptr;         // task -> first side (n_tasks + 1 entries)
+    uint32_t* d_task_order = nullptr;         // loop scheduling order: tasks by decreasing work
+    sph::CellChunk* d_cell_chunks = nullptr;
+    uint32_t* d_occ_side = nullptr;
+    std::map<uint32_t, sph::OffsetTable> offsets;   // by record bytes
+};
+
+namespace sph {
+const OffsetTable* find_offsets(const sph_batch* batch, uint32_t rec_bytes);
+int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
+
+// kernel launchers (kernels_*.cu)
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf, cudaStream_t st);
+int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, const char* d_buf,
+                      bool last_only, cudaStream_t st);
+int32_t launch_density(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out, cudaStream_t st);
+int32_t launch_force(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out,
+                     const sph_params& prm, cudaStream_t st);
+int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);
+int32_t launch_ghost(const StoreView& view, uint64_t n, const sph_layout& layout, const sph_params& prm, cudaStream_t st);
+}  // namespace sph

@@ -1,0 +1,66 @@
+"""Test-side helpers that drive the CUDA path through the Python binding (GPU tests only)."""
+import numpy as np
+import torch
+
+import paper_2606_23891_b200 as sph
+from sph_inputs.format import PART_DTYPE
+
+PARAMS = sph.sph_params(np.float32(5.0 / 3.0), 0.8, 3.0)
+GAMMA = float(np.float32(5.0 / 3.0))       # the value both sides use
+
+
+def to_attrset(oset):
+    """oracle-style (entries, flags) -> sph_attrset"""
+    return sph.make_attrset(oset[0], oset[1])
+
+
+class GpuCase:
+    """A store + one batch on cuda:0, built from oracle-sorted particles, cells and tasks."""
+
+    def __init__(self, parts_sorted, cells, tasks, layout="aos", tasks_per_segment=0, mem_kind=sph.SPH_MEM_DEVICE):
+        self.layout = sph.sph_layout_aos() if layout == "aos" else (sph.sph_layout_split() if layout == "split" else layout)
+        self.n = parts_sorted.shape[0]
+        self.store = sph.sph_store_create(self.layout, self.n, mem_kind)
+        sph.sph_store_import_aos(self.store, np.ascontiguousarray(parts_sorted))
+        sph.sph_store_set_cells(self.store, np.ascontiguousarray(cells).view(sph.CELL_DTYPE))
+        self.tasks = np.ascontiguousarray(tasks).view(sph.TASK_DTYPE)
+        self.batch = sph.sph_batch_create(self.store, self.tasks, tasks_per_segment)
+
+    def buffer(self, aset, fill=0xCD):
+        nbytes = sph.sph_batch_buffer_bytes(self.batch, aset)
+        return torch.full((nbytes,), fill, dtype=torch.uint8, device="cuda")
+
+    def pack(self, aset, fill=0xCD):
+        buf = self.buffer(aset, fill)
+        sph.sph_pack(self.store, self.batch, aset, buf)
+        torch.cuda.synchronize()
+        return buf
+
+    def export(self):
+        out = np.zeros(self.n, dtype=PART_DTYPE)
+        sph.sph_store_export_aos(self.store, out)
+        return out
+
+    def close(self):
+        sph.sph_batch_destroy(self.batch)
+        sph.sph_store_destroy(self.store)
+
+
+def valid_mask(off, cells, tasks, rec_bytes, total):
+    """boolean mask of the bytes a buffer's blocks occupy (pad bytes are unspecified, so excluded)."""
+    m = np.zeros(total, dtype=bool)
+    for t in range(tasks.shape[0]):
+        for side, c in ((0, int(tasks["ci"][t])), (1, int(tasks["cj"][t]))):
+            if c < 0:
+                continue
+            o = int(off[2 * t + side])
+            m[o:o + int(cells["count"][c]) * rec_bytes] = True
+    return m
+
+
+def canon(parts):
+    """canonical bytes of a record array: pad bytes (108..111, 121..127) zeroed."""
+    raw = parts.view(np.uint8).reshape(-1, 128).copy()
+    raw[:, 108:112] = 0
+    raw[:, 121:128] = 0
+    return raw

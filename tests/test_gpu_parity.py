@@ -1,0 +1,438 @@
+"""Parity of the CUDA path against the oracle, element by element, through the C ABI (needs a B200).
+
+Standards (BASELINE.json:north_star): pack and unpack bit-exact; rho, wcount within 2e-5
+relative, the sign-changing h-derivatives within 2e-5 of their natural scale (reading C32); a and du/dt within 1e-4
+relative or 1e-6 * max absolute; v_sig within 1e-4 except particles with a neighbour on the cut-off (C31).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle as orc
+import paper_2606_23891_b200 as sph
+import sph_inputs as si
+from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask
+from orc_setup import raw_copy, sort_grid, sort_octree
+
+pytestmark = pytest.mark.gpu
+
+CUSTOM = ([(orc.V, 1, 2), (orc.X, 0, 3), (orc.ID, 0, 1), (orc.TIME_BIN, 0, 1), (orc.ROT_V, 2, 1), (orc.CS, 0, 1)], 0)
+# reading C21: the configs[3] sweep lists of 4-byte scalar components
+PACK_SWEEP = [(orc.X, 0), (orc.X, 1), (orc.X, 2), (orc.H, 0), (orc.MASS, 0), (orc.RHO, 0), (orc.RHO_DH, 0), (orc.V, 0), (orc.V, 1),
+              (orc.V, 2), (orc.U, 0), (orc.P, 0), (orc.CS, 0), (orc.WCOUNT, 0), (orc.WCOUNT_DH, 0), (orc.A, 0), (orc.A, 1), (orc.A, 2),
+              (orc.DU_DT, 0), (orc.V_SIG, 0)]
+UNPACK_SWEEP = [(orc.RHO, 0), (orc.RHO_DH, 0), (orc.WCOUNT, 0), (orc.WCOUNT_DH, 0), (orc.A, 0), (orc.A, 1), (orc.A, 2), (orc.DU_DT, 0),
+                (orc.V_SIG, 0), (orc.DIV_V, 0), (orc.ROT_V, 0), (orc.ROT_V, 1), (orc.ROT_V, 2), (orc.P, 0), (orc.CS, 0), (orc.U, 0),
+                (orc.V, 0), (orc.V, 1), (orc.V, 2), (orc.H, 0)]
+SWEEP_K = [3, 5, 8, 13, 16, 20]
+
+
+def sweep_set(lst, k, flags):
+    return ([(f, c, 1) for f, c in lst[:k]], flags)
+
+
+def fill_all_fields(ps, seed):
+    """give every member a distinct seeded value so that a wrong offset shows"""
+    rng = np.random.default_rng(seed)
+    for name in ("v", "a", "rot_v"):
+        ps[name] = rng.standard_normal((ps.shape[0], 3)).astype(np.float32)
+    for name in ("u", "du_dt", "rho", "rho_dh", "wcount", "wcount_dh", "div_v", "P", "c_s", "v_sig"):
+        ps[name] = (rng.random(ps.shape[0]) + 0.5).astype(np.float32)
+    ps["time_bin"] = rng.integers(-100, 100, ps.shape[0]).astype(np.int8)
+    return ps
+
+
+_CASES = {}
+
+
+def case(name):
+    """(parts sorted, cells, tasks) of the named small workload, built once by the oracle's builders."""
+    if name not in _CASES:
+        if name == "config0":                  # BASELINE.json:configs[0]
+            ps, cells, tasks, _, _ = sort_grid(si.config0(seed=1), 4)
+        elif name == "ragged":                 # counts 20..55, variable h and mass, 3^3 cells
+            ps, cells, tasks, _, _ = sort_grid(si.jittered_lattice(10, 2, jitter=0.6, sigma_v=0.3, h_spread=0.25, mass_spread=0.5,
+                                                                   u_spread=0.4), 3)
+        elif name == "octree":                 # counts 7..1303: several 32-chunks, ragged tails, tp = 32/64/128 paths, multi-tile sources
+            ps, cells, tasks, _, _ = sort_octree(si.clumpy_mixture(20000, seed=5, n_clumps=3, frac_clumps=0.6, sigma=0.05,
+                                                                   h_cap=1.0 / 24), 150)
+        elif name == "bigcells":               # counts 10..667, wide cells with large h
+            ps, cells, tasks, _, _ = sort_octree(si.clumpy_mixture(20000, seed=8, n_clumps=2, frac_clumps=0.5, sigma=0.08,
+                                                                   h_cap=1.0 / 10), 700)
+        else:
+            raise KeyError(name)
+        _CASES[name] = (fill_all_fields(ps, 17), cells, tasks)
+    ps, cells, tasks = _CASES[name]
+    return raw_copy(ps), cells, tasks
+
+
+def physical(ps, cells, tasks):
+    """replace the seeded filler by physically consistent density-loop results (oracle) so the force loop is sane"""
+    orc.set_threads(8)
+    orc.density_cycle(ps, cells, tasks)
+    orc.ghost(ps, GAMMA)
+    return ps
+
+
+# ------------------------------------------------------------------ store
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+def test_import_export_roundtrip(layout):
+    ps, cells, tasks = case("ragged")
+    g = GpuCase(ps, cells, tasks, layout)
+    assert np.array_equal(canon(g.export()), canon(ps))
+    g.close()
+
+
+def test_store_over_caller_memory():
+    ps, cells, tasks = case("ragged")
+    lay = sph.sph_layout_split()
+    bufs = [torch.zeros(sph.sph_store_sub_bytes(lay, ps.shape[0], s), dtype=torch.uint8, device="cuda") for s in range(lay.n_sub)]
+    store = sph.sph_store_create(lay, ps.shape[0], sph.SPH_MEM_DEVICE, bufs)
+    sph.sph_store_import_aos(store, ps)
+    assert sph.sph_store_sub_ptr(store, 2) == bufs[2].data_ptr()
+    s2 = bufs[2].cpu().numpy()[:ps.shape[0] * 24].view(np.float32).reshape(-1, 6)        # S2 = {v[3], u, P, c_s}
+    assert np.array_equal(s2[:, :3], ps["v"]) and np.array_equal(s2[:, 3], ps["u"]) and np.array_equal(s2[:, 5], ps["c_s"])
+    sph.sph_store_destroy(store)
+
+
+# ------------------------------------------------------------------ pack: bit-exact
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+def test_pack_bit_exact(name, layout):
+    ps, cells, tasks = case(name)
+    g = GpuCase(ps, cells, tasks, layout)
+    sets = [orc.DENSITY_IN, orc.FORCE_IN, orc.DENSITY_OUT, orc.FORCE_OUT, CUSTOM] + [sweep_set(PACK_SWEEP, k, orc.FLAG_X_REL_F32) for k in SWEEP_K]
+    for oset in sets:
+        aset = to_attrset(oset)
+        rec = orc.record_bytes(oset)
+        ref = orc.pack(ps, cells, tasks, oset)
+        off_o, total = orc.block_offsets(cells, tasks, rec)
+        off_g, _ = sph.sph_batch_block_offsets(g.batch, aset)
+        assert np.array_equal(off_g, off_o) and sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        got = g.pack(aset).cpu().numpy()
+        m = valid_mask(off_o, cells, tasks, rec, total)
+        assert np.array_equal(got[m], ref[m]), (name, layout, rec)
+    g.close()
+
+
+# ------------------------------------------------------------------ loops
+
+def _density_tol(ref4, got4, h, m_unit):
+    unit = m_unit / (np.pi * h ** 3)                # size of one neighbour's contribution: m W(0, h)
+    d = np.abs(got4 - ref4)
+    assert np.all(d[:, 0] <= 2e-5 * np.abs(ref4[:, 0]) + 1e-6 * unit)
+    assert np.all(d[:, 2] <= 2e-5 * np.abs(ref4[:, 2]) + 1e-6 * unit / m_unit)
+    assert np.all(d[:, 1] <= 2e-5 * np.maximum(np.abs(ref4[:, 1]), ref4[:, 0] / h) + 1e-6 * unit / h)
+    assert np.all(d[:, 3] <= 2e-5 * np.maximum(np.abs(ref4[:, 3]), ref4[:, 2] / h) + 1e-6 * unit / h / m_unit)
+
+
+def _records(buf, off, cells, tasks, rec_words):
+    """concatenate all blocks' records -> (n_instances, rec_words) f32 and the particle index of each row"""
+    rows, pidx = [], []
+    for t in range(tasks.shape[0]):
+        for side, c in ((0, int(tasks["ci"][t])), (1, int(tasks["cj"][t]))):
+            if c < 0:
+                continue
+            o, k = int(off[2 * t + side]), int(cells["count"][c])
+            rows.append(buf[o:o + 4 * rec_words * k].view(np.float32).reshape(k, rec_words))
+            pidx.append(np.arange(int(cells["first"][c]), int(cells["first"][c]) + k))
+    return np.concatenate(rows), np.concatenate(pidx)
+
+
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells"])
+def test_density_loop_vs_oracle(name):
+    ps, cells, tasks = case(name)
+    orc.set_threads(8)
+    buf_in = orc.pack(ps, cells, tasks, orc.DENSITY_IN)
+    ref = orc.density(cells, tasks, buf_in)
+    g = GpuCase(ps, cells, tasks)
+    d_in = torch.from_numpy(buf_in).cuda()
+    d_out = g.buffer(to_attrset(orc.DENSITY_OUT))
+    sph.sph_density(g.batch, d_in, d_out)
+    torch.cuda.synchronize()
+    off, _ = orc.block_offsets(cells, tasks, 16)
+    r4, pidx = _records(ref, off, cells, tasks, 4)
+    g4, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 4)
+    _density_tol(r4.astype(np.float64), g4.astype(np.float64), ps["h"][pidx].astype(np.float64), float(ps["mass"].max()))
+    g.close()
+
+
+def _near_cutoff(ps, cells, tasks, buf_in, rel=1e-5):
+    """particles that have a neighbour with |r - R_cut| < rel * R_cut in some task (v_sig is discontinuous there, C31)."""
+    off, _ = orc.block_offsets(cells, tasks, 52)
+    flagged = np.zeros(ps.shape[0], dtype=bool)
+    for t in range(tasks.shape[0]):
+        ci, cj = int(tasks["ci"][t]), int(tasks["cj"][t])
+        ki = int(cells["count"][ci])
+        ri = buf_in[int(off[2 * t]):int(off[2 * t]) + 52 * ki].view(np.float32).reshape(ki, 13).astype(np.float64)
+        if cj < 0:
+            rj, kj, fj = ri, ki, int(cells["first"][ci])
+        else:
+            kj, fj = int(cells["count"][cj]), int(cells["first"][cj])
+            rj = buf_in[int(off[2 * t + 1]):int(off[2 * t + 1]) + 52 * kj].view(np.float32).reshape(kj, 13).astype(np.float64)
+        d = np.sqrt(((ri[:, None, :3] - rj[None, :, :3]) ** 2).sum(-1))
+        cut = 2 * np.maximum(ri[:, None, 3], rj[None, :, 3])
+        near = np.abs(d - cut) < rel * cut
+        flagged[int(cells["first"][ci]):int(cells["first"][ci]) + ki] |= near.any(1)
+        flagged[fj:fj + kj] |= near.any(0)
+    return flagged
+
+
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells"])
+def test_force_loop_vs_oracle(name):
+    ps, cells, tasks = case(name)
+    ps = physical(ps, cells, tasks)
+    buf_in = orc.pack(ps, cells, tasks, orc.FORCE_IN)
+    ref = orc.force(cells, tasks, buf_in, 0.8, 3.0)
+    g = GpuCase(ps, cells, tasks)
+    d_in = torch.from_numpy(buf_in).cuda()
+    d_out = g.buffer(to_attrset(orc.FORCE_OUT))
+    sph.sph_force(g.batch, d_in, d_out, PARAMS)
+    torch.cuda.synchronize()
+    off, _ = orc.block_offsets(cells, tasks, 20)
+    r5, pidx = _records(ref, off, cells, tasks, 5)
+    g5, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 5)
+    r5, g5 = r5.astype(np.float64), g5.astype(np.float64)
+    amax, dumax = np.abs(r5[:, :3]).max(), np.abs(r5[:, 3]).max()
+    assert np.all(np.abs(g5[:, :3] - r5[:, :3]) <= np.maximum(1e-4 * np.abs(r5[:, :3]), 1e-6 * amax))
+    assert np.all(np.abs(g5[:, 3] - r5[:, 3]) <= np.maximum(1e-4 * np.abs(r5[:, 3]), 1e-6 * dumax))
+    exempt = _near_cutoff(ps, cells, tasks, buf_in)[pidx]
+    ok = np.abs(g5[:, 4] - r5[:, 4]) <= 1e-4 * np.abs(r5[:, 4])
+    assert np.all(ok | exempt) and exempt.mean() < 0.01
+    g.close()
+
+
+# ------------------------------------------------------------------ unpack: bit-exact
+
+def _random_result_buffer(total, seed):
+    rng = np.random.default_rng(seed)
+    vals = (rng.standard_normal(total // 4) * 10.0 ** rng.integers(-3, 4, total // 4)).astype(np.float32)
+    return vals.view(np.uint8).copy()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+def test_unpack_bit_exact_stage_isolated(name, layout):
+    ps, cells, tasks = case(name)
+    g = GpuCase(ps, cells, tasks, layout)
+    sets = [(orc.DENSITY_OUT, orc.MODE_REDUCE), (orc.FORCE_OUT, orc.MODE_REDUCE), (orc.FORCE_OUT, orc.MODE_ASSIGN)]
+    sets += [(sweep_set(UNPACK_SWEEP, k, 0), orc.MODE_REDUCE) for k in SWEEP_K]
+    for n_set, (oset, mode) in enumerate(sets):
+        aset = to_attrset(oset)
+        rec = orc.record_bytes(oset)
+        _, total = orc.block_offsets(cells, tasks, rec)
+        buf = _random_result_buffer(total, 100 + n_set)
+        ref = raw_copy(ps)
+        orc.unpack(ref, cells, tasks, oset, buf, mode)
+        sph.sph_store_import_aos(g.store, ps)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        sph.sph_unpack(g.store, g.batch, aset, torch.from_numpy(buf).cuda(), mode)
+        assert np.array_equal(canon(g.export()), canon(ref)), (name, layout, rec, mode)
+    g.close()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+def test_pack_then_unpack_identity(layout):
+    ps, cells, tasks = case("octree")
+    oset = ([(orc.X, 0, 3), (orc.V, 0, 3), (orc.RHO, 0, 1), (orc.ID, 0, 1), (orc.TIME_BIN, 0, 1), (orc.ROT_V, 1, 1)], 0)
+    aset = to_attrset(oset)
+    g = GpuCase(ps, cells, tasks, layout)
+    buf = g.pack(aset)
+    scr = raw_copy(ps)
+    for name in ("x", "v", "rho", "id", "time_bin", "rot_v", "mass", "P"):
+        scr[name] = (scr[name] * 0 + 77).astype(scr[name].dtype)
+    sph.sph_store_import_aos(g.store, scr)
+    sph.sph_unpack(g.store, g.batch, aset, buf, sph.SPH_UNPACK_ASSIGN)
+    got = g.export()
+    expect = raw_copy(scr)
+    for name in ("x", "v", "rho", "id", "time_bin"):
+        expect[name] = ps[name]
+    expect["rot_v"][:, 1] = ps["rot_v"][:, 1]
+    assert np.array_equal(canon(got), canon(expect))
+    g.close()
+
+
+# ------------------------------------------------------------------ whole pipeline
+
+def gpu_step(g, do_force=True):
+    s_in, s_out = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN), sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_OUT)
+    f_in, f_out = sph.sph_attrset_canonical(sph.SPH_SET_FORCE_IN), sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT)
+    b_in, b_out = g.buffer(s_in), g.buffer(s_out)
+    sph.sph_store_zero(g.store, s_out)
+    sph.sph_pack(g.store, g.batch, s_in, b_in)
+    sph.sph_density(g.batch, b_in, b_out)
+    sph.sph_unpack(g.store, g.batch, s_out, b_out, sph.SPH_UNPACK_REDUCE)
+    sph.sph_ghost(g.store, PARAMS)
+    if do_force:
+        c_in, c_out = g.buffer(f_in), g.buffer(f_out)
+        sph.sph_store_zero(g.store, f_out)
+        sph.sph_pack(g.store, g.batch, f_in, c_in)
+        sph.sph_force(g.batch, c_in, c_out, PARAMS)
+        sph.sph_unpack(g.store, g.batch, f_out, c_out, sph.SPH_UNPACK_REDUCE)
+    torch.cuda.synchronize()
+    return g.export()
+
+
+def check_store_physics(got, ref):
+    h = ref["h"].astype(np.float64)
+    for name, dname in (("rho", "rho_dh"), ("wcount", "wcount_dh")):
+        r, v = ref[name].astype(np.float64), got[name].astype(np.float64)
+        assert np.max(np.abs(v - r) / r) <= 2e-5, name
+        rd, vd = ref[dname].astype(np.float64), got[dname].astype(np.float64)
+        assert np.max(np.abs(vd - rd) / np.maximum(np.abs(rd), r / h)) <= 2e-5, dname
+    assert np.max(np.abs(got["P"] - ref["P"]) / ref["P"]) <= 2e-5 and np.max(np.abs(got["c_s"] - ref["c_s"]) / ref["c_s"]) <= 1e-6
+    a_r, a_g = ref["a"].astype(np.float64), got["a"].astype(np.float64)
+    assert np.all(np.abs(a_g - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * np.abs(a_r).max()))
+    d_r, d_g = ref["du_dt"].astype(np.float64), got["du_dt"].astype(np.float64)
+    assert np.all(np.abs(d_g - d_r) <= np.maximum(1e-4 * np.abs(d_r), 1e-6 * np.abs(d_r).max()))
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+def test_full_step_vs_oracle(name, layout):
+    ps, cells, tasks = case(name)
+    ref = raw_copy(ps)
+    orc.set_threads(8)
+    orc.density_cycle(ref, cells, tasks)
+    orc.ghost(ref, GAMMA)
+    orc.force_cycle(ref, cells, tasks)
+    g = GpuCase(ps, cells, tasks, layout)
+    got = gpu_step(g)
+    check_store_physics(got, ref)
+    vs_ok = np.abs(got["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
+    assert vs_ok.mean() > 0.99
+    # fields no loop writes are untouched, bit for bit
+    for fld in ("x", "v", "mass", "h", "u", "div_v", "rot_v", "id", "time_bin"):
+        assert np.array_equal(got[fld], ps[fld]), fld
+    # invariants on the GPU output (north_star: total momentum change <= 1e-6 relative)
+    m = got["mass"].astype(np.float64)
+    a = got["a"].astype(np.float64)
+    assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+    en = m * (np.einsum("ij,ij->i", got["v"].astype(np.float64), a) + got["du_dt"])
+    assert abs(en.sum()) <= 1e-5 * np.abs(m * got["du_dt"].astype(np.float64)).sum()
+    g.close()
+
+
+def test_aos_and_split_stores_agree_bitwise():
+    ps, cells, tasks = case("ragged")
+    ga, gs = GpuCase(ps, cells, tasks, "aos"), GpuCase(ps, cells, tasks, "split")
+    assert np.array_equal(canon(gpu_step(ga)), canon(gpu_step(gs)))
+    ga.close()
+    gs.close()
+
+
+# ------------------------------------------------------------------ segments (batches of a fixed task count)
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+def test_segmented_batch_equals_standalone_batches(layout):
+    ps, cells, tasks = case("ragged")
+    ps = physical(ps, cells, tasks)
+    seg = 50
+    g = GpuCase(ps, cells, tasks, layout, tasks_per_segment=seg)
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_FORCE_IN)
+    whole = g.pack(aset).cpu().numpy()
+    off, seg_off = sph.sph_batch_block_offsets(g.batch, aset)
+    info = sph.sph_batch_get_info(g.batch)
+    assert info.n_segments == -(-tasks.shape[0] // seg) == seg_off.shape[0] and np.all(seg_off % 256 == 0)
+    for b in range(info.n_segments):
+        t = tasks[b * seg:(b + 1) * seg]
+        ref = orc.pack(ps, cells, t, orc.FORCE_IN)
+        off_o, total = orc.block_offsets(cells, t, 52)
+        m = valid_mask(off_o, cells, t, 52, total)
+        assert np.array_equal(whole[int(seg_off[b]):int(seg_off[b]) + total][m], ref[m])
+    # force + unpack through the segmented batch == oracle run batch by batch
+    out = g.buffer(sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT))
+    sph.sph_store_zero(g.store, sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT))
+    sph.sph_force(g.batch, torch.from_numpy(whole).cuda(), out, PARAMS)
+    sph.sph_unpack(g.store, g.batch, sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT), out, sph.SPH_UNPACK_REDUCE)
+    ref = raw_copy(ps)
+    orc.force_cycle(ref, cells, tasks, batch=seg)
+    got = g.export()
+    a_r = ref["a"].astype(np.float64)
+    assert np.all(np.abs(got["a"] - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * np.abs(a_r).max()))
+    g.close()
+
+
+def test_batches_in_sequence_equal_oracle_bitwise_unpack():
+    """per-batch calls in batch order reduce in the same order as one oracle pass over all tasks"""
+    ps, cells, tasks = case("ragged")
+    oset, aset = orc.FORCE_OUT, sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT)
+    g = GpuCase(ps, cells, tasks, "split")
+    ref = raw_copy(ps)
+    nb = 64
+    for s in range(0, tasks.shape[0], nb):
+        t = np.ascontiguousarray(tasks[s:s + nb])
+        _, total = orc.block_offsets(cells, t, 20)
+        buf = _random_result_buffer(total, 500 + s)
+        orc.unpack(ref, cells, t, oset, buf, orc.MODE_REDUCE)
+        batch = sph.sph_batch_create(g.store, t.view(sph.TASK_DTYPE))
+        sph.sph_unpack(g.store, batch, aset, torch.from_numpy(buf).cuda(), sph.SPH_UNPACK_REDUCE)
+        torch.cuda.synchronize()
+        sph.sph_batch_destroy(batch)
+    assert np.array_equal(canon(g.export()), canon(ref))
+    g.close()
+
+
+# ------------------------------------------------------------------ edge cases and errors
+
+def test_empty_and_tiny_cells():
+    parts = np.zeros(5, dtype=si.PART_DTYPE)
+    parts["x"] = [[0.1, 0.1, 0.1], [0.12, 0.1, 0.1], [0.6, 0.6, 0.6], [0.62, 0.6, 0.6], [0.61, 0.62, 0.6]]
+    parts["h"], parts["mass"], parts["u"] = 0.05, 1.0, 1.0
+    ps, cells, tasks, ns, npair = sort_grid(parts, 4)          # 64 cells, 62 of them empty
+    assert (cells["count"] == 0).sum() == 62
+    ref = raw_copy(ps)
+    orc.density_cycle(ref, cells, tasks)
+    orc.ghost(ref, GAMMA)
+    orc.force_cycle(ref, cells, tasks)
+    g = GpuCase(ps, cells, tasks, "split")
+    got = gpu_step(g)
+    check_store_physics(got, ref)
+    g.close()
+
+
+def test_argument_errors():
+    ps, cells, tasks = case("ragged")
+    g = GpuCase(ps, cells, tasks)
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN)
+    small = torch.zeros(128, dtype=torch.uint8, device="cuda")
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack(g.store, g.batch, aset, small)
+    assert e.value.code == 3
+    odd = sph.make_attrset([("x", 0, 3), ("id", 0, 1)])                    # 32-byte records: table not prepared yet
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack(g.store, g.batch, odd, torch.zeros(1 << 20, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == 1
+    with pytest.raises(sph.SphError) as e:                                # relative coordinates cannot be unpacked
+        sph.sph_unpack(g.store, g.batch, aset, g.buffer(aset), sph.SPH_UNPACK_ASSIGN)
+    assert e.value.code == 6
+    bad = tasks.copy()
+    bad["cj"][-1] = cells.shape[0]
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_batch_create(g.store, np.ascontiguousarray(bad).view(sph.TASK_DTYPE))
+    assert e.value.code == 3
+    badcells = cells.copy()
+    badcells["first"][3] = ps.shape[0]
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_store_set_cells(g.store, np.ascontiguousarray(badcells).view(sph.CELL_DTYPE))
+    assert e.value.code == 3
+    g.close()
+
+
+def test_streams_are_honoured():
+    ps, cells, tasks = case("config0")
+    g = GpuCase(ps, cells, tasks)
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN)
+    st = torch.cuda.Stream()
+    buf = g.buffer(aset)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        sph.sph_pack(g.store, g.batch, aset, buf, stream=st)
+    st.synchronize()
+    ref = orc.pack(ps, cells, tasks, orc.DENSITY_IN)
+    off, total = orc.block_offsets(cells, tasks, 20)
+    m = valid_mask(off, cells, tasks, 20, total)
+    assert np.array_equal(buf.cpu().numpy()[m], ref[m])
+    g.close()

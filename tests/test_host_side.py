@@ -1,0 +1,154 @@
+"""Host logic of the library (no GPU): exported symbols, layouts, attribute sets, cell / task builders.
+
+The builders are cross-checked against the oracle's independent ones: same permutation, same cells, same
+task list and frames.
+"""
+import ctypes
+import re
+import os
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import paper_2606_23891_b200 as sph
+import sph_inputs as si
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "sph_b200.h")).read()
+    declared = set(re.findall(r"^int32_t\s+(sph_\w+)\s*\(", header, flags=re.M))
+    assert declared == set(sph.EXPORTS)
+    lib = ctypes.CDLL(sph.lib_path())
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_library_is_built_for_sm_100a_only():
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", sph.lib_path()], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_\d+a?", out))
+    assert archs == {"sm_100a"}, out
+
+
+def test_layouts():
+    aos, split = sph.sph_layout_aos(), sph.sph_layout_split()
+    assert aos.n_sub == 1 and aos.stride[0] == 128
+    # canonical offsets = the numpy dtype both sides use as exchange format
+    for f, name in enumerate(si.FIELDS):
+        assert aos.loc[f].off == si.PART_DTYPE.fields[name][1] and aos.loc[f].sub == 0
+    assert split.n_sub == 6 and list(split.stride)[:6] == [32, 16, 24, 20, 16, 16]      # 124 bytes of payload
+    groups = {0: ["x", "h", "mass"], 1: ["rho", "rho_dh", "wcount", "wcount_dh"], 2: ["v", "u", "P", "c_s"],
+              3: ["a", "du_dt", "v_sig"], 4: ["id", "time_bin"], 5: ["div_v", "rot_v"]}
+    for s, names in groups.items():
+        for name in names:
+            assert split.loc[sph.FIELD[name]].sub == s
+    sph.sph_layout_validate(aos)
+    sph.sph_layout_validate(split)
+    bad = sph.sph_layout_split()
+    bad.loc[sph.FIELD["h"]].off = 20          # overlaps x[2]
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_layout_validate(bad)
+    assert e.value.code == 2
+    bad = sph.sph_layout_aos()
+    bad.loc[sph.FIELD["id"]].off = 124        # runs past the stride
+    with pytest.raises(sph.SphError):
+        sph.sph_layout_validate(bad)
+    bad = sph.sph_layout_aos()
+    bad.n_sub = 9
+    with pytest.raises(sph.SphError):
+        sph.sph_layout_validate(bad)
+
+
+def test_attribute_sets():
+    for which, rec, oset in [(sph.SPH_SET_DENSITY_IN, 20, orc.DENSITY_IN), (sph.SPH_SET_DENSITY_OUT, 16, orc.DENSITY_OUT),
+                             (sph.SPH_SET_FORCE_IN, 52, orc.FORCE_IN), (sph.SPH_SET_FORCE_OUT, 20, orc.FORCE_OUT)]:
+        a = sph.sph_attrset_canonical(which)
+        assert sph.sph_attrset_record_bytes(a) == rec == orc.record_bytes(oset)
+        assert [(a.ent[k].field, a.ent[k].comp0, a.ent[k].ncomp) for k in range(a.n)] == [tuple(e) for e in oset[0]]
+        assert a.flags == oset[1]
+    assert sph.sph_attrset_record_bytes(sph.make_attrset([("x", 0, 3), ("id", 0, 1), ("time_bin", 0, 1)])) == 36
+    for entries in ([("v", 0, 2), ("v", 1, 1)], [("mass", 0, 2)], [(18, 0, 1)], []):
+        with pytest.raises(sph.SphError) as e:
+            sph.sph_attrset_record_bytes(sph.make_attrset(entries))
+        assert e.value.code == 2
+
+
+def test_store_sub_bytes_and_errors():
+    split = sph.sph_layout_split()
+    assert sph.sph_store_sub_bytes(split, 1000, 3) >= 1000 * 20 + 64
+    assert sph.sph_store_sub_bytes(split, 1000, 3) % 256 == 0
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_store_sub_bytes(split, 1000, 6)
+    assert e.value.code == 3 and "substruct" in str(e.value)
+
+
+@pytest.mark.parametrize("cpd,n_side,seed", [(4, 12, 1), (3, 10, 2), (5, 11, 3)])
+def test_grid_builder_matches_oracle(cpd, n_side, seed):
+    parts = si.jittered_lattice(n_side, seed, jitter=0.9)
+    perm_o, cells_o = orc.cells_build_grid(parts["x"], cpd)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], cpd)
+    assert np.array_equal(perm, perm_o)
+    assert cells.tobytes() == cells_o.tobytes()
+    ps = parts[perm.astype(np.int64)]
+    hmax = orc.cell_hmax(ps, cells_o)
+    tasks_o, ns_o, np_o = orc.tasks_build(cells_o, hmax)
+    tasks, ns, npair = sph.sph_tasks_build(cells, hmax)
+    assert (ns, npair) == (ns_o, np_o)
+    assert tasks.tobytes() == tasks_o.tobytes()
+
+
+def test_task_rule_with_large_h_matches_oracle():
+    parts = si.jittered_lattice(12, 4, jitter=0.3, eta=1.1 / 1.0, h_spread=0.3)      # 2h up to ~2.5 dx > width 2 dx
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 6)
+    ps = parts[perm.astype(np.int64)]
+    hmax = orc.cell_hmax(ps, cells)
+    tasks_o, ns_o, np_o = orc.tasks_build(cells.view(orc.CELL_DTYPE), hmax)
+    tasks, ns, npair = sph.sph_tasks_build(cells, hmax)
+    assert npair == np_o > 216 * 13
+    assert tasks.tobytes() == tasks_o.tobytes()
+
+
+def test_tasks_reject_box_too_small_for_cutoff():
+    parts = si.jittered_lattice(6, 5, eta=1.2348)
+    parts["h"] = 0.2                           # 2h = 0.4: with 3 cells per dim a second image is within reach
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 3)
+    hmax = orc.cell_hmax(parts[perm.astype(np.int64)], cells)
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_tasks_build(cells, hmax)
+    assert e.value.code == 3
+    with pytest.raises(ValueError):
+        orc.tasks_build(cells.view(orc.CELL_DTYPE), hmax)
+
+
+@pytest.mark.parametrize("seed,leaf", [(3, 100), (6, 37)])
+def test_octree_builder_matches_oracle(seed, leaf):
+    parts = si.clumpy_mixture(20000, seed=seed, n_clumps=4, frac_clumps=0.7, sigma=0.03, h_cap=1.0 / 32)
+    perm_o, cells_o = orc.cells_build_octree(parts["x"], parts["h"], leaf)
+    perm, cells = sph.sph_cells_build_octree(parts["x"], parts["h"], leaf)
+    assert np.array_equal(perm, perm_o)
+    assert cells.tobytes() == cells_o.tobytes()
+    ps = parts[perm.astype(np.int64)]
+    hmax = orc.cell_hmax(ps, cells_o)
+    tasks_o, ns_o, np_o = orc.tasks_build(cells_o, hmax)
+    tasks, ns, npair = sph.sph_tasks_build(cells, hmax)
+    assert (ns, npair) == (ns_o, np_o)
+    assert tasks.tobytes() == tasks_o.tobytes()
+
+
+def test_grid_builder_rejects_out_of_box():
+    x = np.array([[0.1, 0.2, 1.0]])
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_cells_build_grid(x, 4)
+    assert e.value.code == 3
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_store_create(sph.sph_layout_aos(), 128)
+    assert e.value.code == 5
