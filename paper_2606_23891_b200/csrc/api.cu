@@ -50,68 +50,83 @@ int32_t attrset_check(const sph_attrset* set, uint32_t* rec_bytes) {
     return SPH_OK;
 }
 
-static uint32_t make_div_magic(uint32_t d) {
-    // smallest m with (g*m)>>16 == g/d for all g < 32*d + 4
-    for (uint32_t m = (65536 + d - 1) / d;; ++m) {
-        bool ok = true;
-        for (uint32_t g = 0; g < 32 * d + 4 && ok; ++g) ok = ((g * m) >> 16) == g / d;
-        if (ok) return m;
-    }
-}
-
-static void finish_program(const sph_layout& layout, Program* prog, bool stage) {
-    prog->div_magic = make_div_magic(prog->rec_words);
-    // substructs touched, staging layout (pack only) and 16-byte chunk masks
-    prog->n_sub_used = 0;
-    uint32_t smem = 0;
-    for (uint32_t s = 0; s < layout.n_sub; ++s) {
-        bool used = false;
-        uint32_t mask = 0;
-        const uint32_t stride = layout.stride[s];
-        const bool pow2 = stride >= 32 && (stride & (stride - 1)) == 0 && stride <= 512;
-        for (uint32_t w = 0; w < prog->rec_words; ++w) {
-            const WordDesc& wd = prog->word[w];
-            if (wd.kind == W_SKIP || wd.sub != s) continue;
-            used = true;
-            const uint32_t nbytes = wd.kind == W_XREL ? 8 : (wd.kind == W_TIMEBIN || wd.kind == W_ASSIGN_BYTE ? 1 : 4);
-            for (uint32_t b = wd.off; b < wd.off + nbytes; ++b) mask |= 1u << (b / 16);
-        }
-        if (!used) continue;
-        const uint32_t u = prog->n_sub_used++;
-        prog->sub_used[u] = (uint8_t)s;
-        prog->chunk_mask[u] = pow2 ? mask : 0xFFFFFFFFu;
-        prog->smem_base[u] = smem;
-        if (stage) smem += 32 * stride + 32;
-        for (uint32_t w = 0; w < prog->rec_words; ++w)
-            if (prog->word[w].kind != W_SKIP && prog->word[w].sub == s) prog->word[w].used_idx = (uint8_t)u;
-    }
-    prog->smem_per_warp = (smem + 15) & ~15u;
-}
-
+// PACK program: which substruct arrays to stage (and which 16-byte pieces of them), the pre-pass, and for every
+// record word the staging offset it is copied from.
 int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog) {
     uint32_t rec_bytes = 0;
     if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
     std::memset(prog, 0, sizeof(*prog));
     prog->rec_words = rec_bytes / 4;
+    // 1) record words as (substruct, byte offset, bytes needed there), before staging offsets are known
+    struct Raw { uint8_t sub; uint16_t off; uint8_t kind; } raw[kMaxRecWords];
     uint32_t w = 0;
+    bool need[SPH_MAX_SUB][4096 / 16] = {};   // 16-byte pieces of each substruct that hold requested bytes
+    bool used[SPH_MAX_SUB] = {};
+    auto mark = [&](uint8_t sub, uint32_t off, uint32_t nbytes) {
+        used[sub] = true;
+        for (uint32_t b = off; b < off + nbytes; ++b) need[sub][b / 16] = true;
+    };
     for (uint32_t k = 0; k < set.n; ++k) {
         const sph_attr& a = set.ent[k];
         const auto& loc = layout.loc[a.field];
         for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
             const uint16_t off = (uint16_t)(loc.off + c * field_elem_bytes(a.field));
             if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32)) {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_XREL, (uint8_t)c, 0, 0};
+                // the pre-pass leaves f32(x[c] - frame[c]) at x + 4c; it reads all three coordinates
+                raw[w++] = Raw{loc.sub, (uint16_t)(loc.off + 4 * c), (uint8_t)W_XREL};
+                mark(loc.sub, loc.off, 24);
             } else if (a.field == SPH_X || a.field == SPH_ID) {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_COPY, 0, 0, 0};
-                prog->word[w++] = WordDesc{(uint16_t)(off + 4), loc.sub, (uint8_t)W_COPY, 0, 0, 0};
+                raw[w++] = Raw{loc.sub, off, (uint8_t)W_COPY};
+                raw[w++] = Raw{loc.sub, (uint16_t)(off + 4), (uint8_t)W_COPY};
+                mark(loc.sub, off, 8);
             } else if (a.field == SPH_TIME_BIN) {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_TIMEBIN, 0, 0, 0};
+                raw[w++] = Raw{loc.sub, off, (uint8_t)W_TIMEBIN};
+                mark(loc.sub, off, 1);
             } else {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_COPY, 0, 0, 0};
+                raw[w++] = Raw{loc.sub, off, (uint8_t)W_COPY};
+                mark(loc.sub, off, 4);
             }
         }
     }
-    finish_program(layout, prog, true);
+    // 2) staging layout: every used substruct gets 32 structs' worth of space, particle 0 of a chunk at smem_base
+    uint32_t smem = 0, base_of[SPH_MAX_SUB] = {};
+    for (uint32_t s = 0; s < layout.n_sub; ++s) {
+        if (!used[s]) continue;
+        PackSub& su = prog->su[prog->n_sub_used++];
+        const uint32_t stride = layout.stride[s];
+        su.sub = s;
+        su.stride = stride;
+        su.gran = stride % 16 == 0 ? 16 : (stride % 8 == 0 ? 8 : 4);
+        su.mask = 0xFFFFFFFFu;
+        if (su.gran == 16 && stride >= 32 && stride <= 512 && (stride & (stride - 1)) == 0) {
+            su.mask = 0;
+            for (uint32_t c = 0; c < stride / 16; ++c) if (need[s][c]) su.mask |= 1u << c;
+        }
+        su.smem_base = base_of[s] = smem;
+        smem += (32 * stride + 15) & ~15u;
+    }
+    // 3) words -> staging offsets; pre-pass parameters
+    for (uint32_t k = 0; k < prog->rec_words; ++k) {
+        WordDesc& wd = prog->word[k];
+        wd.sub = raw[k].sub;
+        wd.kind = raw[k].kind;
+        wd.stride = (uint16_t)layout.stride[raw[k].sub];
+        wd.a = base_of[raw[k].sub] + raw[k].off;
+        if (raw[k].kind == W_XREL) {
+            prog->xrel = 1;
+            prog->x_src = base_of[raw[k].sub] + layout.loc[SPH_X].off;
+            prog->x_stride = layout.stride[raw[k].sub];
+        } else if (raw[k].kind == W_TIMEBIN) {
+            prog->tb = 1;
+            prog->tb_src = wd.a;
+            prog->tb_stride = wd.stride;
+            prog->tb_dst = smem;
+            wd.a = smem;
+            wd.stride = 4;
+            smem += 128;
+        }
+    }
+    prog->smem_per_warp = (smem + 15) & ~15u;
     return SPH_OK;
 }
 
@@ -125,26 +140,26 @@ int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, i
     for (uint32_t k = 0; k < set.n; ++k) {
         const sph_attr& a = set.ent[k];
         const auto& loc = layout.loc[a.field];
+        const uint16_t stride = (uint16_t)layout.stride[loc.sub];
         if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32))
             return fail(SPH_ERR_UNSUPPORTED, "X packed as relative f32 cannot be unpacked (the frame shift is not invertible in f32)");
         const bool is_sum = a.field == SPH_RHO || a.field == SPH_RHO_DH || a.field == SPH_WCOUNT || a.field == SPH_WCOUNT_DH ||
                             a.field == SPH_A || a.field == SPH_DU_DT;
         for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
-            const uint16_t off = (uint16_t)(loc.off + c * field_elem_bytes(a.field));
+            const uint32_t off = loc.off + c * field_elem_bytes(a.field);
             if (a.field == SPH_X || a.field == SPH_ID) {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_ASSIGN, 0, 0, 0};
-                prog->word[w++] = WordDesc{(uint16_t)(off + 4), loc.sub, (uint8_t)W_ASSIGN, 0, 0, 0};
+                prog->word[w++] = WordDesc{off, stride, loc.sub, (uint8_t)W_ASSIGN};
+                prog->word[w++] = WordDesc{off + 4, stride, loc.sub, (uint8_t)W_ASSIGN};
             } else if (a.field == SPH_TIME_BIN) {
-                prog->word[w++] = WordDesc{off, loc.sub, (uint8_t)W_ASSIGN_BYTE, 0, 0, 0};
+                prog->word[w++] = WordDesc{off, stride, loc.sub, (uint8_t)W_ASSIGN_BYTE};
             } else {
                 uint8_t kind = W_ASSIGN;
                 if (mode == SPH_UNPACK_REDUCE && is_sum) kind = W_SUM;
                 if (mode == SPH_UNPACK_REDUCE && a.field == SPH_V_SIG) kind = W_MAX;
-                prog->word[w++] = WordDesc{off, loc.sub, kind, 0, 0, 0};
+                prog->word[w++] = WordDesc{off, stride, loc.sub, kind};
             }
         }
     }
-    finish_program(layout, prog, false);
     return SPH_OK;
 }
 
@@ -430,7 +445,7 @@ int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, con
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
     bool all_assign = true;
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_assign &= prog.word[w].kind == W_ASSIGN || prog.word[w].kind == W_ASSIGN_BYTE;
-    return launch_unpack(s->view(), b, prog, ot->d_off128, (const char*)d_buf, all_assign, (cudaStream_t)stream);
+    return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, (cudaStream_t)stream);
 }
 
 static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, uint32_t rec_in,

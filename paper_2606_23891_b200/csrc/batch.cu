@@ -2,7 +2,6 @@
 #include <algorithm>
 #include <cstring>
 #include <new>
-#include <numeric>
 
 #include "internal.h"
 
@@ -51,6 +50,9 @@ int32_t ensure_offsets(sph_batch* b, uint32_t rec_bytes, const OffsetTable** out
     ot.total = run;
     if (run / 128 >= (1ull << 32)) return fail(SPH_ERR_RANGE, "buffer of %llu bytes exceeds the 512 GiB offset range", (unsigned long long)run);
     if (int32_t rc = upload(off128, &ot.d_off128)) return rc;
+    std::vector<uint32_t> occ_off128(b->occ_side.size());
+    for (size_t o = 0; o < occ_off128.size(); ++o) occ_off128[o] = off128[b->occ_side[o]];
+    if (int32_t rc = upload(occ_off128, &ot.d_occ_off128)) { cudaFree(ot.d_off128); return rc; }
     auto ins = b->offsets.emplace(rec_bytes, std::move(ot));
     if (out) *out = &ins.first->second;
     return SPH_OK;
@@ -74,7 +76,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     b->tasks_per_segment = tasks_per_segment;
     b->n_segments = tasks_per_segment ? (uint32_t)((n_tasks + tasks_per_segment - 1) / tasks_per_segment) : 1;
     std::vector<double> frames;
-    std::vector<uint32_t> chunk_side;
+    std::vector<uint32_t> chunk_side, chunk_src;
     b->task_side0.resize(n_tasks + 1);
     b->sides.reserve(2 * n_tasks);
     frames.reserve(6 * n_tasks);
@@ -90,7 +92,8 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
             const sph_cell& ce = store->cells[c];
             SideRec sr{(uint32_t)ce.first, ce.count, (uint32_t)chunk_side.size(), c};
             const uint32_t sidx = (uint32_t)b->sides.size();
-            for (uint32_t k = 0; k < ce.count; k += 32) chunk_side.push_back(sidx);
+            const uint32_t partner = tk.cj >= 0 ? (side == 0 ? sidx + 1 : sidx - 1) : sidx;
+            for (uint32_t k = 0; k < ce.count; k += 32) { chunk_side.push_back(sidx); chunk_src.push_back(partner); }
             b->sides.push_back(sr);
             const double* fr = side == 0 ? tk.frame_i : tk.frame_j;
             frames.insert(frames.end(), fr, fr + 3);
@@ -110,7 +113,9 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     for (const SideRec& s : b->sides) ++occ_count[s.cell];
     std::vector<uint32_t> occ_start(n_cells + 1, 0);
     for (uint32_t c = 0; c < n_cells; ++c) occ_start[c + 1] = occ_start[c] + occ_count[c];
-    std::vector<uint32_t> occ_side(b->n_sides), cur(occ_start.begin(), occ_start.end() - 1);
+    std::vector<uint32_t>& occ_side = b->occ_side;
+    occ_side.resize(b->n_sides);
+    std::vector<uint32_t> cur(occ_start.begin(), occ_start.end() - 1);
     for (uint32_t s = 0; s < b->n_sides; ++s) occ_side[cur[b->sides[s].cell]++] = s;
     std::vector<CellChunk> cell_chunks;
     for (uint32_t c = 0; c < n_cells; ++c) {
@@ -123,24 +128,12 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     b->n_cell_chunks = (uint32_t)cell_chunks.size();
     b->n_occ = b->n_sides;
 
-    // loop scheduling order: heaviest tasks first (counts differ by 30x on the octree configs)
-    std::vector<uint32_t> order(n_tasks);
-    std::iota(order.begin(), order.end(), 0u);
-    auto work = [&](uint32_t t) {
-        const uint64_t ni = store->cells[tasks[t].ci].count;
-        return tasks[t].cj >= 0 ? 2 * ni * store->cells[tasks[t].cj].count : ni * ni;
-    };
-    bool uniform = true;
-    for (uint64_t t = 1; t < n_tasks && uniform; ++t) uniform = work((uint32_t)t) == work(0);
-    if (!uniform) std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return work(x) > work(y); });
-
     int32_t rc = upload(b->sides, &b->d_sides);
     if (!rc) rc = upload(frames, &b->d_frames);
     if (!rc) rc = upload(chunk_side, &b->d_chunk_side);
     if (!rc) rc = upload(b->task_side0, &b->d_task_side0);
-    if (!rc) rc = upload(order, &b->d_task_order);
+    if (!rc) rc = upload(chunk_src, &b->d_chunk_src);
     if (!rc) rc = upload(cell_chunks, &b->d_cell_chunks);
-    if (!rc) rc = upload(occ_side, &b->d_occ_side);
     for (uint32_t rec : {16u, 20u, 52u})
         if (!rc) rc = ensure_offsets(b, rec, nullptr);
     if (rc) { sph_batch_destroy(b); return rc; }
@@ -151,8 +144,8 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
     cudaFree(b->d_sides); cudaFree(b->d_frames); cudaFree(b->d_chunk_side); cudaFree(b->d_task_side0);
-    cudaFree(b->d_task_order); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_side);
-    for (auto& kv : b->offsets) cudaFree(kv.second.d_off128);
+    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks);
+    for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;
 }

@@ -54,27 +54,39 @@ struct CellChunk {
 };
 
 // word kinds of the pack / unpack programs
-enum : uint32_t { W_COPY = 0, W_XREL = 1, W_TIMEBIN = 2,            // pack
+enum : uint32_t { W_COPY = 0, W_XREL = 1, W_TIMEBIN = 2,            // pack (host side only: the kernel sees plain copies)
                   W_SUM = 3, W_MAX = 4, W_ASSIGN = 5, W_ASSIGN_BYTE = 6, W_SKIP = 7 };   // unpack
 
-// Per record word: where it lives in the store.  Built on the host from (layout, attribute set).
+// Per record word: where it comes from / goes to.  Built on the host from (layout, attribute set).
+//   pack:   a = byte offset of the word of particle 0 inside the warp's staging area (after the pre-pass every word
+//           is a plain 4-byte copy), stride = bytes between consecutive particles there
+//   unpack: a = byte offset inside the substruct, stride = the substruct's stride, sub, kind
 struct WordDesc {
-    uint16_t off;      // byte offset inside the substruct
-    uint8_t sub;       // substruct
-    uint8_t kind;      // W_*
-    uint8_t dim;       // W_XREL: coordinate axis
-    uint8_t used_idx;  // index of `sub` in Program::sub_used
-    uint16_t pad;
+    uint32_t a;
+    uint16_t stride;
+    uint8_t sub;
+    uint8_t kind;
+};
+
+// One substruct array a pack program draws from, staged per 32-particle chunk with particle 0 at smem_base.
+struct PackSub {
+    const char* base;     // the substruct array (filled in at launch from the store)
+    uint32_t sub;
+    uint32_t stride;
+    uint32_t gran;        // 16, 8 or 4: the largest power of two that divides the stride (cp.async size)
+    uint32_t mask;        // gran == 16 and power-of-two stride in [32, 512]: bit c set = 16-byte piece c of the struct is needed
+    uint32_t smem_base;   // 16-byte aligned
 };
 
 struct Program {
     uint32_t rec_words;
-    uint32_t div_magic;            // k = (g * div_magic) >> 16 == g / rec_words for g < 32 * rec_words + 4
     uint32_t n_sub_used;
     uint32_t smem_per_warp;        // bytes of staging per warp (pack)
-    uint8_t sub_used[SPH_MAX_SUB];
-    uint32_t chunk_mask[SPH_MAX_SUB];   // per used substruct: needed 16-byte chunks (power-of-two strides), else ~0
-    uint32_t smem_base[SPH_MAX_SUB];    // staging offset of each used substruct inside the warp's region
+    // pack pre-pass, one lane per particle: x (3 f64 at x_src + k x_stride) -> f32(x - frame) written over its first 12 bytes;
+    // time_bin (1 byte at tb_src + k tb_stride) -> zero-extended word at tb_dst + 4k
+    uint32_t xrel, x_src, x_stride;
+    uint32_t tb, tb_src, tb_stride, tb_dst;
+    PackSub su[SPH_MAX_SUB];
     WordDesc word[kMaxRecWords];
 };
 
@@ -83,6 +95,7 @@ int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, i
 
 struct OffsetTable {
     uint32_t* d_off128 = nullptr;          // per side: block start in units of 128 bytes
+    uint32_t* d_occ_off128 = nullptr;      // per occurrence (cell-major, ascending side): the same, for the ordered unpack
     std::vector<uint64_t> h_off;           // per side, bytes
     std::vector<uint64_t> seg_off;         // per segment, bytes
     uint64_t total = 0;
@@ -110,15 +123,15 @@ struct sph_batch {
     uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0;
     uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
     std::vector<sph::SideRec> sides;          // host copy
+    std::vector<uint32_t> occ_side;           // host copy of the occurrence lists
     std::vector<uint32_t> task_side0;         // n_tasks + 1
     // device tables
     sph::SideRec* d_sides = nullptr;
     double* d_frames = nullptr;               // 3 per side
     uint32_t* d_chunk_side = nullptr;         // pack chunk -> side
     uint32_t* d_task_side0 = nullptr;         // task -> first side (n_tasks + 1 entries)
-    uint32_t* d_task_order = nullptr;         // loop scheduling order: tasks by decreasing work
+    uint32_t* d_chunk_src = nullptr;          // pack chunk -> the side its targets gather from (partner side; itself for self tasks)
     sph::CellChunk* d_cell_chunks = nullptr;
-    uint32_t* d_occ_side = nullptr;
     std::map<uint32_t, sph::OffsetTable> offsets;   // by record bytes
 };
 
@@ -128,7 +141,7 @@ int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable**
 
 // kernel launchers (kernels_*.cu)
 int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf, cudaStream_t st);
-int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, const char* d_buf,
+int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out,

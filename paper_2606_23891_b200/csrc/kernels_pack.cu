@@ -1,14 +1,18 @@
 // PACK and UNPACK kernels: pure data movement, HBM-bound.
 //
-// pack: one warp per 32-particle chunk of a block.  The warp (1) stages the 16-byte pieces of the substruct
-// arrays that hold the requested fields into shared memory with coalesced cp.async (only the pieces that are
-// needed: for the 128-byte AoS record that is the difference between touching 2 and 4 sectors), then
-// (2) re-slices them into the compact record stream and writes it with coalesced 16-byte stores.
+// pack: one warp per 32-particle chunk of a block (one side of one task).  The warp
+//   (1) stages the pieces of the substruct arrays that hold the requested fields into shared memory with
+//       coalesced cp.async (16 bytes when the stride allows, else 8 or 4; for power-of-two strides only the
+//       16-byte pieces that are needed: for the 128-byte AoS record that is the difference between touching 2
+//       and 4 sectors), particle 0 of the chunk always landing at the same staging offset;
+//   (2) pre-pass, one lane per particle: x -> f32(x - frame) in place (one f64 subtraction, one RN conversion);
+//   (3) re-slices the staging area into the compact record stream, 16 bytes per lane and store.  Which staging
+//       word feeds which output word is the same for every chunk, so each lane computes its map once per launch.
 //
-// unpack: one warp per 32-particle chunk of a CELL.  The warp walks the cell's blocks in ascending task order,
-// reading each block's slice with coalesced 16-byte loads, and applies the per-field operator in f32 in that
-// order (bit-reproducible, no atomics, no races: a particle is owned by exactly one warp per launch); the store
-// fields are read and written once per launch.
+// unpack: one warp per 32-particle chunk of a CELL.  The warp walks the cell's blocks in ascending (task, side)
+// order, reading each block's slice with coalesced 16-byte loads (a round of independent loads in flight before
+// the first add), and applies the per-field operator in f32 in that order (bit-reproducible, no atomics, no races:
+// a particle is owned by exactly one warp per launch); the store fields are read and written once per launch.
 #include "internal.h"
 
 namespace sph {
@@ -16,41 +20,41 @@ namespace sph {
 namespace {
 
 constexpr int kPackWarps = 8;
-constexpr int kUnpackWarps = 8;
+constexpr int kUnpackWarps = 4;
 
-struct SWord {          // word descriptor as the kernels use it (shared memory copy)
-    uint32_t a;         // pack: staging byte offset of the word inside the warp's region (without the per-chunk shift)
-                        // unpack: byte offset inside the substruct
-    uint32_t b;         // stride | kind << 16 | dim << 20 | used_idx << 24
-};
-
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem));
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
+    if constexpr (BYTES == 16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem));
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem), "n"(BYTES));
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-__device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
-    asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-__device__ __forceinline__ uint4 ld_stream16(const void* p) {
+__device__ __forceinline__ uint4 ld_once16(const void* p) {   // records are read exactly once: keep them out of L1
     uint4 v;
-    asm volatile("ld.global.cs.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
     return v;
 }
 
+template <int NIT>
 __global__ void __launch_bounds__(kPackWarps * 32)
-pack_kernel(StoreView view, Program prog, const SideRec* __restrict__ sides, const double* __restrict__ frames,
+pack_kernel(Program prog, const SideRec* __restrict__ sides, const double* __restrict__ frames,
             const uint32_t* __restrict__ chunk_side, const uint32_t* __restrict__ off128, uint32_t n_chunks, char* __restrict__ buf) {
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ SWord s_word[kMaxRecWords];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (uint32_t w = threadIdx.x; w < prog.rec_words; w += blockDim.x) {
-        const WordDesc wd = prog.word[w];
-        s_word[w].a = prog.smem_base[wd.used_idx] + wd.off;
-        s_word[w].b = view.stride[wd.sub] | (uint32_t)wd.kind << 16 | (uint32_t)wd.dim << 20 | (uint32_t)wd.used_idx << 24;
-    }
-    __syncthreads();
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned char* stage = smem + (size_t)warp * prog.smem_per_warp;
-    const uint32_t rec_words = prog.rec_words;
+    const uint32_t R = prog.rec_words;
+
+    // which staging word feeds output word g = 4 (lane + 32 it) + j of a chunk's record stream
+    uint32_t src[NIT][4];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t g = 4 * (lane + 32 * it) + j;
+            const uint32_t k = g / R, w = g - k * R;
+            src[it][j] = k < 32 ? prog.word[w].a + k * prog.word[w].stride : 0;
+        }
 
     for (uint32_t chunk = blockIdx.x * kPackWarps + warp; chunk < n_chunks; chunk += gridDim.x * kPackWarps) {
         const uint32_t side = chunk_side[chunk];
@@ -58,57 +62,61 @@ pack_kernel(StoreView view, Program prog, const SideRec* __restrict__ sides, con
         const uint32_t k0 = (chunk - sr.chunk0) * 32;
         const uint32_t n = min(32u, sr.count - k0);
         const uint64_t p0 = (uint64_t)sr.first + k0;
+        const uint32_t o128 = off128[side];
 
-        // (1) stage the needed 16-byte pieces of every substruct the record draws from
+        // (1) stage
         for (uint32_t u = 0; u < prog.n_sub_used; ++u) {
-            const uint32_t s = prog.sub_used[u], stride = view.stride[s], mask = prog.chunk_mask[u];
-            const uint64_t byte0 = p0 * stride;
-            const uint64_t a0 = byte0 & ~15ull;
-            const uint32_t nvec = (uint32_t)(((byte0 + (uint64_t)n * stride + 15) & ~15ull) - a0) >> 4;
-            const char* src = view.base[s] + a0;
-            unsigned char* dst = stage + prog.smem_base[u];
-            if (mask == 0xFFFFFFFFu) {
-                for (uint32_t v = lane; v < nvec; v += 32) cp_async16(dst + 16 * v, src + 16 * v);
-            } else {   // power-of-two stride: skip the pieces no requested field lives in
-                const uint32_t per = stride >> 4;
-                for (uint32_t v = lane; v < nvec; v += 32)
-                    if (mask >> (v & (per - 1)) & 1) cp_async16(dst + 16 * v, src + 16 * v);
+            const PackSub su = prog.su[u];
+            const char* g = su.base + p0 * su.stride;
+            unsigned char* dst = stage + su.smem_base;
+            const uint32_t nbytes = n * su.stride;
+            if (su.gran == 16) {
+                const uint32_t nvec = nbytes >> 4;
+                if (su.mask == 0xFFFFFFFFu) {
+                    for (uint32_t v = lane; v < nvec; v += 32) cp_async<16>(dst + 16 * v, g + 16 * v);
+                } else {
+                    const uint32_t per = su.stride >> 4;
+                    for (uint32_t v = lane; v < nvec; v += 32)
+                        if (su.mask >> (v & (per - 1)) & 1) cp_async<16>(dst + 16 * v, g + 16 * v);
+                }
+            } else if (su.gran == 8) {
+                for (uint32_t v = lane; v < (nbytes >> 3); v += 32) cp_async<8>(dst + 8 * v, g + 8 * v);
+            } else {
+                for (uint32_t v = lane; v < (nbytes >> 2); v += 32) cp_async<4>(dst + 4 * v, g + 4 * v);
             }
         }
         cp_async_wait_all();
         __syncwarp();
 
-        // (2) re-slice into records
-        const double fx = frames[3 * side], fy = frames[3 * side + 1], fz = frames[3 * side + 2];
-        char* out = buf + (uint64_t)off128[side] * 128 + (uint64_t)k0 * rec_words * 4;
-        const uint32_t total = n * rec_words, nvec_out = (total + 3) >> 2;
-        for (uint32_t v = lane; v < nvec_out; v += 32) {
-            uint32_t o[4];
+        // (2) pre-pass (each lane touches only its own particle's bytes)
+        if (prog.xrel && lane < n) {
+            unsigned char* px = stage + prog.x_src + lane * prog.x_stride;
+            const double x0 = *reinterpret_cast<const double*>(px), x1 = *reinterpret_cast<const double*>(px + 8),
+                         x2 = *reinterpret_cast<const double*>(px + 16);
+            const double* f = frames + 3 * (size_t)side;
+            const float r0 = __double2float_rn(__dsub_rn(x0, f[0])), r1 = __double2float_rn(__dsub_rn(x1, f[1])),
+                        r2 = __double2float_rn(__dsub_rn(x2, f[2]));
+            *reinterpret_cast<float2*>(px) = make_float2(r0, r1);
+            *reinterpret_cast<float*>(px + 8) = r2;
+        }
+        if (prog.tb && lane < n)
+            *reinterpret_cast<uint32_t*>(stage + prog.tb_dst + 4 * lane) = stage[prog.tb_src + lane * prog.tb_stride];
+        __syncwarp();
+
+        // (3) re-slice into records
+        char* out = buf + (uint64_t)o128 * 128 + (uint64_t)k0 * R * 4;
+        const uint32_t nvec_out = (n * R + 3) >> 2;   // a last partial vector spills into the block's pad bytes
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t g = 4 * v + j;
-                const uint32_t k = (g * prog.div_magic) >> 16;
-                const uint32_t w = g - k * rec_words;
-                const SWord sw = s_word[w];
-                const uint32_t stride = sw.b & 0xFFFF, kind = (sw.b >> 16) & 0xF;
-                const uint32_t shift = (uint32_t)(p0 * stride) & 15u;   // where particle 0 of the chunk sits in its staged piece
-                const unsigned char* src = stage + sw.a + shift + k * stride;
-                uint32_t val = 0;
-                if (g < total) {
-                    if (kind == W_COPY) {
-                        val = *reinterpret_cast<const uint32_t*>(src);
-                    } else if (kind == W_XREL) {
-                        const uint2 raw = *reinterpret_cast<const uint2*>(src);
-                        const uint32_t dim = (sw.b >> 20) & 0xF;
-                        const double f = dim == 0 ? fx : (dim == 1 ? fy : fz);
-                        val = __float_as_uint(__double2float_rn(__dsub_rn(__hiloint2double((int)raw.y, (int)raw.x), f)));
-                    } else {   // W_TIMEBIN
-                        val = *src;
-                    }
-                }
-                o[j] = val;
+        for (int it = 0; it < NIT; ++it) {
+            const uint32_t v = lane + 32 * it;
+            if (v < nvec_out) {
+                uint4 o;
+                o.x = *reinterpret_cast<const uint32_t*>(stage + src[it][0]);
+                o.y = *reinterpret_cast<const uint32_t*>(stage + src[it][1]);
+                o.z = *reinterpret_cast<const uint32_t*>(stage + src[it][2]);
+                o.w = *reinterpret_cast<const uint32_t*>(stage + src[it][3]);
+                *reinterpret_cast<uint4*>(out + 16 * v) = o;
             }
-            st_stream16(out + 16 * v, make_uint4(o[0], o[1], o[2], o[3]));
         }
         __syncwarp();   // the staging region is reused by the next chunk
     }
@@ -116,61 +124,89 @@ pack_kernel(StoreView view, Program prog, const SideRec* __restrict__ sides, con
 
 // ---------------------------------------------------------------------------------------------------------
 
-template <bool kLastOnly>
+// meta word of the hoisted unpack map: store byte offset relative to the chunk's first particle | sub << 20 | kind << 24
+__device__ __forceinline__ char* word_ptr(const StoreView* s_view, uint32_t meta, uint64_t first) {
+    const uint32_t sub = (meta >> 20) & 0xF;
+    return s_view->base[sub] + first * s_view->stride[sub] + (meta & 0xFFFFF);
+}
+
+template <int NIT, bool kLastOnly>
 __global__ void __launch_bounds__(kUnpackWarps * 32)
-unpack_kernel(StoreView view, Program prog, const SideRec* __restrict__ sides, const CellChunk* __restrict__ cell_chunks,
-              const uint32_t* __restrict__ occ_side, const uint32_t* __restrict__ off128, uint32_t n_cell_chunks, const char* __restrict__ buf) {
-    __shared__ SWord s_word[kMaxRecWords];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (uint32_t w = threadIdx.x; w < prog.rec_words; w += blockDim.x) {
-        const WordDesc wd = prog.word[w];
-        s_word[w].a = wd.off;
-        s_word[w].b = view.stride[wd.sub] | (uint32_t)wd.kind << 16 | (uint32_t)wd.sub << 24;
-    }
+unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
+              uint32_t n_cell_chunks, const char* __restrict__ buf) {
+    constexpr int UNR = NIT >= 8 ? 1 : (NIT >= 4 ? 2 : (NIT >= 2 ? 4 : 8));   // blocks whose records are in flight together
+    __shared__ StoreView s_view;     // indexed per lane (the substruct differs from word to word)
+    if (threadIdx.x == 0) s_view = view;
     __syncthreads();
-    const uint32_t rec_words = prog.rec_words;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t R = prog.rec_words;
+    uint32_t meta[NIT][4];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t g = 4 * (lane + 32 * it) + j;
+            const uint32_t k = g / R, w = g - k * R;
+            meta[it][j] = k < 32 ? (k * prog.word[w].stride + prog.word[w].a) | (uint32_t)prog.word[w].sub << 20 | (uint32_t)prog.word[w].kind << 24
+                                 : (uint32_t)W_SKIP << 24;
+        }
 
     for (uint32_t cc = blockIdx.x * kUnpackWarps + warp; cc < n_cell_chunks; cc += gridDim.x * kUnpackWarps) {
         const CellChunk ch = cell_chunks[cc];
-        const uint32_t total = ch.count * rec_words, nvec = (total + 3) >> 2;
-        const uint64_t slice = (uint64_t)ch.k0 * rec_words * 4;
-        for (uint32_t v = lane; v < nvec; v += 32) {
-            // the four record words this lane owns -> (particle, field word), store address, operator
-            char* dst[4];
-            uint32_t kind[4];
-            float acc[4];
+        const uint32_t total = ch.count * R, nvec = (total + 3) >> 2;
+        const char* slice = buf + (uint64_t)ch.k0 * R * 4 + 16 * lane;
+        float acc[NIT][4];
+        uint32_t kind[NIT][4];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const uint32_t g = 4 * v + j;
-                const uint32_t k = (g * prog.div_magic) >> 16;
-                const uint32_t w = g - k * rec_words;
-                const SWord sw = s_word[w];
-                const uint32_t stride = sw.b & 0xFFFF, sub = sw.b >> 24;
-                kind[j] = g < total ? (sw.b >> 16) & 0xF : (uint32_t)W_SKIP;
-                dst[j] = view.base[sub] + ((uint64_t)ch.first + k) * stride + sw.a;
-                acc[j] = 0.f;
-                if (kind[j] == W_SUM || kind[j] == W_MAX) acc[j] = *reinterpret_cast<const float*>(dst[j]);
+                const uint32_t g = 4 * (lane + 32 * it) + j;
+                kind[it][j] = g < total ? meta[it][j] >> 24 : (uint32_t)W_SKIP;
+                acc[it][j] = 0.f;
+                if (!kLastOnly && (kind[it][j] == W_SUM || kind[it][j] == W_MAX))
+                    acc[it][j] = *reinterpret_cast<const float*>(word_ptr(&s_view, meta[it][j], ch.first));
             }
-            uint32_t o = kLastOnly ? ch.nocc - 1 : 0;
-#pragma unroll 4
-            for (; o < ch.nocc; ++o) {
-                const uint32_t side = occ_side[ch.occ0 + o];
-                const uint4 r = ld_stream16(buf + (uint64_t)off128[side] * 128 + slice + 16 * v);
-                const float rv[4] = {__uint_as_float(r.x), __uint_as_float(r.y), __uint_as_float(r.z), __uint_as_float(r.w)};
+        for (uint32_t ob = kLastOnly ? ch.nocc - 1 : 0; ob < ch.nocc; ob += 32) {
+            const uint32_t lim = min(32u, ch.nocc - ob);
+            const uint32_t tbl = lane < lim ? occ_off128[ch.occ0 + ob + lane] : 0;
+            for (uint32_t u0 = 0; u0 < lim; u0 += UNR) {
+                uint4 r[UNR][NIT];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    if (kind[j] == W_SUM) acc[j] = __fadd_rn(acc[j], rv[j]);
-                    else if (kind[j] == W_MAX) acc[j] = fmaxf(acc[j], rv[j]);
-                    else acc[j] = rv[j];
+                for (int u = 0; u < UNR; ++u) {
+                    const uint32_t o128 = __shfl_sync(0xFFFFFFFFu, tbl, (u0 + u) & 31);
+                    if (u0 + u < lim) {
+#pragma unroll
+                        for (int it = 0; it < NIT; ++it)
+                            if (lane + 32 * it < nvec) r[u][it] = ld_once16(slice + (uint64_t)o128 * 128 + 512 * it);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < UNR; ++u) {
+                    if (u0 + u < lim) {
+#pragma unroll
+                        for (int it = 0; it < NIT; ++it) {
+                            const float rv[4] = {__uint_as_float(r[u][it].x), __uint_as_float(r[u][it].y), __uint_as_float(r[u][it].z),
+                                                 __uint_as_float(r[u][it].w)};
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const float s = __fadd_rn(acc[it][j], rv[j]), m = fmaxf(acc[it][j], rv[j]);
+                                acc[it][j] = kind[it][j] == W_SUM ? s : (kind[it][j] == W_MAX ? m : rv[j]);
+                            }
+                        }
+                    }
                 }
             }
+        }
+#pragma unroll
+        for (int it = 0; it < NIT; ++it)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                if (kind[j] == W_SKIP) continue;
-                if (kind[j] == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(dst[j]) = (unsigned char)__float_as_uint(acc[j]);
-                else *reinterpret_cast<float*>(dst[j]) = acc[j];
+                if (kind[it][j] == W_SKIP) continue;
+                char* dst = word_ptr(&s_view, meta[it][j], ch.first);
+                if (kind[it][j] == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(dst) = (unsigned char)__float_as_uint(acc[it][j]);
+                else *reinterpret_cast<float*>(dst) = acc[it][j];
             }
-        }
     }
 }
 
@@ -181,7 +217,7 @@ __global__ void zero_kernel(StoreView view, Program prog, uint64_t n) {
     for (uint64_t g = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; g < total; g += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t p = g / prog.rec_words;
         const WordDesc wd = prog.word[g - p * prog.rec_words];
-        *reinterpret_cast<float*>(view.base[wd.sub] + p * view.stride[wd.sub] + wd.off) = 0.f;
+        *reinterpret_cast<float*>(view.base[wd.sub] + p * wd.stride + wd.a) = 0.f;
     }
 }
 
@@ -209,37 +245,66 @@ int32_t sm_count(int* out) {
     return SPH_OK;
 }
 
+template <int NIT>
+int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf,
+                        uint32_t grid, size_t smem, cudaStream_t st) {
+    static size_t configured = 0;
+    if (smem > 48 * 1024 && smem > configured) {
+        SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_sides, b->d_frames, b->d_chunk_side, d_off128, b->n_chunks, d_buf);
+    return SPH_OK;
+}
+
+template <int NIT>
+void launch_unpack_nit(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
+                       bool last_only, uint32_t grid, cudaStream_t st) {
+    if (last_only)
+        unpack_kernel<NIT, true><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf);
+    else
+        unpack_kernel<NIT, false><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf);
+}
+
 }  // namespace
 
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf, cudaStream_t st) {
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_off128, char* d_buf, cudaStream_t st) {
     if (b->n_chunks == 0) return SPH_OK;
+    Program prog = prog_in;
+    for (uint32_t u = 0; u < prog.n_sub_used; ++u) prog.su[u].base = view.base[prog.su[u].sub];
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
     const size_t smem = (size_t)prog.smem_per_warp * kPackWarps;
     if (smem > 200 * 1024) return fail(SPH_ERR_UNSUPPORTED, "layout needs %zu bytes of staging per CTA", smem);
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
     const uint32_t want = (b->n_chunks + kPackWarps - 1) / kPackWarps;
     const uint32_t grid = min(want, (uint32_t)sms * 8);
-    pack_kernel<<<grid, kPackWarps * 32, smem, st>>>(view, prog, b->d_sides, b->d_frames, b->d_chunk_side, d_off128, b->n_chunks, d_buf);
+    const uint32_t nit = (prog.rec_words + 3) / 4;   // 16-byte vectors per lane for a full chunk: ceil(32 R / 4 / 32)
+    int32_t rc;
+    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_off128, d_buf, grid, smem, st);
+    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_off128, d_buf, grid, smem, st);
+    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_off128, d_buf, grid, smem, st);
+    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_off128, d_buf, grid, smem, st);
+    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_off128, d_buf, grid, smem, st);
+    else rc = launch_pack_nit<12>(b, prog, d_off128, d_buf, grid, smem, st);
+    if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
 
-int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, const char* d_buf,
+int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, cudaStream_t st) {
     if (b->n_cell_chunks == 0) return SPH_OK;
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
     const uint32_t want = (b->n_cell_chunks + kUnpackWarps - 1) / kUnpackWarps;
-    const uint32_t grid = min(want, (uint32_t)sms * 8);
-    if (last_only)
-        unpack_kernel<true><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_sides, b->d_cell_chunks, b->d_occ_side, d_off128, b->n_cell_chunks, d_buf);
-    else
-        unpack_kernel<false><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_sides, b->d_cell_chunks, b->d_occ_side, d_off128, b->n_cell_chunks, d_buf);
+    const uint32_t grid = min(want, (uint32_t)sms * 16);
+    const uint32_t nit = (prog.rec_words + 3) / 4;
+    if (nit <= 1) launch_unpack_nit<1>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    else if (nit <= 2) launch_unpack_nit<2>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    else if (nit <= 4) launch_unpack_nit<4>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    else if (nit <= 6) launch_unpack_nit<6>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    else if (nit <= 9) launch_unpack_nit<9>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    else launch_unpack_nit<12>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
