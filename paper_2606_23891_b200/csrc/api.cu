@@ -57,6 +57,7 @@ int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Pro
     if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
     std::memset(prog, 0, sizeof(*prog));
     prog->rec_words = rec_bytes / 4;
+    prog->xw[0] = prog->xw[1] = prog->xw[2] = 0xFFFFFFFFu;
     // 1) record words as (substruct, byte offset, bytes needed there), before staging offsets are known
     struct Raw { uint8_t sub; uint16_t off; uint8_t kind; } raw[kMaxRecWords];
     uint32_t w = 0;
@@ -73,6 +74,7 @@ int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Pro
             const uint16_t off = (uint16_t)(loc.off + c * field_elem_bytes(a.field));
             if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32)) {
                 // the pre-pass leaves f32(x[c] - frame[c]) at x + 4c; it reads all three coordinates
+                prog->xw[c] = w;
                 raw[w++] = Raw{loc.sub, (uint16_t)(loc.off + 4 * c), (uint8_t)W_XREL};
                 mark(loc.sub, loc.off, 24);
             } else if (a.field == SPH_X || a.field == SPH_ID) {
@@ -430,7 +432,7 @@ int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set,
     if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
     if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
-    return launch_pack(s->view(), b, prog, ot->d_off128, (char*)d_buf, (cudaStream_t)stream);
+    return launch_pack(s->view(), b, prog, ot->d_occ_off128, (char*)d_buf, (cudaStream_t)stream);
 }
 
 int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {

@@ -134,6 +134,9 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     if (!rc) rc = upload(b->task_side0, &b->d_task_side0);
     if (!rc) rc = upload(chunk_src, &b->d_chunk_src);
     if (!rc) rc = upload(cell_chunks, &b->d_cell_chunks);
+    std::vector<double> occ_frames(3 * (size_t)b->n_sides);
+    for (uint32_t o = 0; o < b->n_sides; ++o) std::copy_n(&frames[3 * (size_t)occ_side[o]], 3, &occ_frames[3 * (size_t)o]);
+    if (!rc) rc = upload(occ_frames, &b->d_occ_frames);
     for (uint32_t rec : {16u, 20u, 52u})
         if (!rc) rc = ensure_offsets(b, rec, nullptr);
     if (rc) { sph_batch_destroy(b); return rc; }
@@ -144,7 +147,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
     cudaFree(b->d_sides); cudaFree(b->d_frames); cudaFree(b->d_chunk_side); cudaFree(b->d_task_side0);
-    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks);
+    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;

@@ -85,6 +85,7 @@ struct Program {
     // pack pre-pass, one lane per particle: x (3 f64 at x_src + k x_stride) -> f32(x - frame) written over its first 12 bytes;
     // time_bin (1 byte at tb_src + k tb_stride) -> zero-extended word at tb_dst + 4k
     uint32_t xrel, x_src, x_stride;
+    uint32_t xw[3];                // record word that holds f32(x[c] - frame[c]), or 0xFFFFFFFF
     uint32_t tb, tb_src, tb_stride, tb_dst;
     PackSub su[SPH_MAX_SUB];
     WordDesc word[kMaxRecWords];
@@ -128,6 +129,7 @@ struct sph_batch {
     // device tables
     sph::SideRec* d_sides = nullptr;
     double* d_frames = nullptr;               // 3 per side
+    double* d_occ_frames = nullptr;           // 3 per occurrence (cell-major, ascending side): the frame of that side
     uint32_t* d_chunk_side = nullptr;         // pack chunk -> side
     uint32_t* d_task_side0 = nullptr;         // task -> first side (n_tasks + 1 entries)
     uint32_t* d_chunk_src = nullptr;          // pack chunk -> the side its targets gather from (partner side; itself for self tasks)
@@ -140,7 +142,7 @@ const OffsetTable* find_offsets(const sph_batch* batch, uint32_t rec_bytes);
 int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
 
 // kernel launchers (kernels_*.cu)
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf, cudaStream_t st);
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out, cudaStream_t st);

@@ -13,6 +13,8 @@
 // order, reading each block's slice with coalesced 16-byte loads (a round of independent loads in flight before
 // the first add), and applies the per-field operator in f32 in that order (bit-reproducible, no atomics, no races:
 // a particle is owned by exactly one warp per launch); the store fields are read and written once per launch.
+#include <algorithm>
+
 #include "internal.h"
 
 namespace sph {
@@ -30,6 +32,9 @@ __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
         asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem), "n"(BYTES));
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void st_stream16(void* p, uint4 v) {   // records are written once and read by another kernel
+    asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 __device__ __forceinline__ uint4 ld_once16(const void* p) {   // records are read exactly once: keep them out of L1
     uint4 v;
     asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
@@ -38,12 +43,14 @@ __device__ __forceinline__ uint4 ld_once16(const void* p) {   // records are rea
 
 template <int NIT>
 __global__ void __launch_bounds__(kPackWarps * 32)
-pack_kernel(Program prog, const SideRec* __restrict__ sides, const double* __restrict__ frames,
-            const uint32_t* __restrict__ chunk_side, const uint32_t* __restrict__ off128, uint32_t n_chunks, char* __restrict__ buf) {
+pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
+            const double* __restrict__ occ_frames, uint32_t n_cell_chunks, uint32_t slices, char* __restrict__ buf) {
     extern __shared__ __align__(16) unsigned char smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    unsigned char* stage = smem + (size_t)warp * prog.smem_per_warp;
     const uint32_t R = prog.rec_words;
+    const uint32_t templ_bytes = 128 * R;                           // 32 records
+    unsigned char* stage = smem + (size_t)warp * (prog.smem_per_warp + 2 * templ_bytes);
+    unsigned char* templ = stage + prog.smem_per_warp;              // two copies, used alternately
 
     // which staging word feeds output word g = 4 (lane + 32 it) + j of a chunk's record stream
     uint32_t src[NIT][4];
@@ -55,19 +62,28 @@ pack_kernel(Program prog, const SideRec* __restrict__ sides, const double* __res
             const uint32_t k = g / R, w = g - k * R;
             src[it][j] = k < 32 ? prog.word[w].a + k * prog.word[w].stride : 0;
         }
+    const uint32_t xw0 = prog.xw[0], xw1 = prog.xw[1], xw2 = prog.xw[2];
 
-    for (uint32_t chunk = blockIdx.x * kPackWarps + warp; chunk < n_chunks; chunk += gridDim.x * kPackWarps) {
-        const uint32_t side = chunk_side[chunk];
-        const SideRec sr = sides[side];
-        const uint32_t k0 = (chunk - sr.chunk0) * 32;
-        const uint32_t n = min(32u, sr.count - k0);
-        const uint64_t p0 = (uint64_t)sr.first + k0;
-        const uint32_t o128 = off128[side];
+    const uint32_t n_items = n_cell_chunks * slices;
+    for (uint32_t item = blockIdx.x * kPackWarps + warp; item < n_items; item += gridDim.x * kPackWarps) {
+        const uint32_t cc = item / slices, sl = item - cc * slices;
+        const CellChunk ch = cell_chunks[cc];
+        const uint32_t per = (ch.nocc + slices - 1) / slices;
+        const uint32_t ob = sl * per, oe = min(ch.nocc, ob + per);
+        if (ob >= oe) continue;
+        const uint32_t n = ch.count;
+        // first occurrence's block offset and frame: in flight while the chunk is staged
+        uint32_t o128 = __ldg(occ_off128 + ch.occ0 + ob);
+        double f0 = 0., f1 = 0., f2 = 0.;
+        if (prog.xrel) {
+            const double* f = occ_frames + 3 * (size_t)(ch.occ0 + ob);
+            f0 = __ldg(f); f1 = __ldg(f + 1); f2 = __ldg(f + 2);
+        }
 
-        // (1) stage
+        // (1) stage the chunk's structs (once per item, not once per occurrence)
         for (uint32_t u = 0; u < prog.n_sub_used; ++u) {
             const PackSub su = prog.su[u];
-            const char* g = su.base + p0 * su.stride;
+            const char* g = su.base + (uint64_t)ch.first * su.stride;
             unsigned char* dst = stage + su.smem_base;
             const uint32_t nbytes = n * su.stride;
             if (su.gran == 16) {
@@ -75,9 +91,9 @@ pack_kernel(Program prog, const SideRec* __restrict__ sides, const double* __res
                 if (su.mask == 0xFFFFFFFFu) {
                     for (uint32_t v = lane; v < nvec; v += 32) cp_async<16>(dst + 16 * v, g + 16 * v);
                 } else {
-                    const uint32_t per = su.stride >> 4;
+                    const uint32_t per16 = su.stride >> 4;
                     for (uint32_t v = lane; v < nvec; v += 32)
-                        if (su.mask >> (v & (per - 1)) & 1) cp_async<16>(dst + 16 * v, g + 16 * v);
+                        if (su.mask >> (v & (per16 - 1)) & 1) cp_async<16>(dst + 16 * v, g + 16 * v);
                 }
             } else if (su.gran == 8) {
                 for (uint32_t v = lane; v < (nbytes >> 3); v += 32) cp_async<8>(dst + 8 * v, g + 8 * v);
@@ -88,37 +104,59 @@ pack_kernel(Program prog, const SideRec* __restrict__ sides, const double* __res
         cp_async_wait_all();
         __syncwarp();
 
-        // (2) pre-pass (each lane touches only its own particle's bytes)
+        // (2) one lane per particle: keep x in registers (it is re-based for every occurrence); widen time_bin
+        double x0 = 0., x1 = 0., x2 = 0.;
         if (prog.xrel && lane < n) {
-            unsigned char* px = stage + prog.x_src + lane * prog.x_stride;
-            const double x0 = *reinterpret_cast<const double*>(px), x1 = *reinterpret_cast<const double*>(px + 8),
-                         x2 = *reinterpret_cast<const double*>(px + 16);
-            const double* f = frames + 3 * (size_t)side;
-            const float r0 = __double2float_rn(__dsub_rn(x0, f[0])), r1 = __double2float_rn(__dsub_rn(x1, f[1])),
-                        r2 = __double2float_rn(__dsub_rn(x2, f[2]));
-            *reinterpret_cast<float2*>(px) = make_float2(r0, r1);
-            *reinterpret_cast<float*>(px + 8) = r2;
+            const unsigned char* px = stage + prog.x_src + lane * prog.x_stride;
+            x0 = *reinterpret_cast<const double*>(px); x1 = *reinterpret_cast<const double*>(px + 8); x2 = *reinterpret_cast<const double*>(px + 16);
         }
         if (prog.tb && lane < n)
             *reinterpret_cast<uint32_t*>(stage + prog.tb_dst + 4 * lane) = stage[prog.tb_src + lane * prog.tb_stride];
         __syncwarp();
 
-        // (3) re-slice into records
-        char* out = buf + (uint64_t)o128 * 128 + (uint64_t)k0 * R * 4;
+        // (3) re-slice the staging area into the record stream (both template copies); the x words are patched below
         const uint32_t nvec_out = (n * R + 3) >> 2;   // a last partial vector spills into the block's pad bytes
 #pragma unroll
         for (int it = 0; it < NIT; ++it) {
             const uint32_t v = lane + 32 * it;
-            if (v < nvec_out) {
+            if (v < 8 * R) {
                 uint4 o;
                 o.x = *reinterpret_cast<const uint32_t*>(stage + src[it][0]);
                 o.y = *reinterpret_cast<const uint32_t*>(stage + src[it][1]);
                 o.z = *reinterpret_cast<const uint32_t*>(stage + src[it][2]);
                 o.w = *reinterpret_cast<const uint32_t*>(stage + src[it][3]);
-                *reinterpret_cast<uint4*>(out + 16 * v) = o;
+                *reinterpret_cast<uint4*>(templ + 16 * v) = o;
+                *reinterpret_cast<uint4*>(templ + templ_bytes + 16 * v) = o;
             }
         }
-        __syncwarp();   // the staging region is reused by the next chunk
+        __syncwarp();   // the x words written here are overwritten by other lanes below
+
+        // (4) one copy of the template per occurrence of the cell (task side), x re-based to that side's frame
+        const uint64_t chunk_off = (uint64_t)ch.k0 * R * 4 + 16 * lane;
+        for (uint32_t o = ob; o < oe; ++o) {
+            unsigned char* T = templ + ((o - ob) & 1) * templ_bytes;
+            char* out = buf + (uint64_t)o128 * 128 + chunk_off;
+            if (prog.xrel && lane < n) {
+                float* rec = reinterpret_cast<float*>(T) + lane * R;
+                if (xw0 != 0xFFFFFFFFu) rec[xw0] = __double2float_rn(__dsub_rn(x0, f0));
+                if (xw1 != 0xFFFFFFFFu) rec[xw1] = __double2float_rn(__dsub_rn(x1, f1));
+                if (xw2 != 0xFFFFFFFFu) rec[xw2] = __double2float_rn(__dsub_rn(x2, f2));
+            }
+            if (o + 1 < oe) {   // next occurrence's table entries, in flight during this copy
+                o128 = __ldg(occ_off128 + ch.occ0 + o + 1);
+                if (prog.xrel) {
+                    const double* f = occ_frames + 3 * (size_t)(ch.occ0 + o + 1);
+                    f0 = __ldg(f); f1 = __ldg(f + 1); f2 = __ldg(f + 2);
+                }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int it = 0; it < NIT; ++it) {
+                const uint32_t v = lane + 32 * it;
+                if (v < nvec_out) st_stream16(out + 512 * it, *reinterpret_cast<const uint4*>(T + 16 * v));
+            }
+        }
+        __syncwarp();   // staging and templates are reused by the next item
     }
 }
 
@@ -246,14 +284,20 @@ int32_t sm_count(int* out) {
 }
 
 template <int NIT>
-int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_off128, char* d_buf,
-                        uint32_t grid, size_t smem, cudaStream_t st) {
+int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms, cudaStream_t st) {
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = smem;
     }
-    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_sides, b->d_frames, b->d_chunk_side, d_off128, b->n_chunks, d_buf);
+    // resident CTAs per SM (shared memory and 64 warps bound it); a cell's occurrences are split into `slices` items
+    // when there are fewer cell chunks than about two rounds of resident warps
+    const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(64 / kPackWarps, (220 * 1024) / (smem + 1024)));
+    const uint32_t resident_warps = (uint32_t)sms * per_sm * kPackWarps;
+    const uint32_t slices = std::min(8u, std::max(1u, (2 * resident_warps + b->n_cell_chunks - 1) / b->n_cell_chunks));
+    const uint64_t items = (uint64_t)b->n_cell_chunks * slices;
+    const uint32_t grid = (uint32_t)std::min<uint64_t>((items + kPackWarps - 1) / kPackWarps, (uint64_t)sms * per_sm);
+    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_cell_chunks, d_occ_off128, b->d_occ_frames, b->n_cell_chunks, slices, d_buf);
     return SPH_OK;
 }
 
@@ -268,24 +312,22 @@ void launch_unpack_nit(const StoreView& view, const sph_batch* b, const Program&
 
 }  // namespace
 
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_off128, char* d_buf, cudaStream_t st) {
-    if (b->n_chunks == 0) return SPH_OK;
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_occ_off128, char* d_buf, cudaStream_t st) {
+    if (b->n_cell_chunks == 0) return SPH_OK;
     Program prog = prog_in;
     for (uint32_t u = 0; u < prog.n_sub_used; ++u) prog.su[u].base = view.base[prog.su[u].sub];
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
-    const size_t smem = (size_t)prog.smem_per_warp * kPackWarps;
+    const size_t smem = ((size_t)prog.smem_per_warp + 2 * 128 * (size_t)prog.rec_words) * kPackWarps;
     if (smem > 200 * 1024) return fail(SPH_ERR_UNSUPPORTED, "layout needs %zu bytes of staging per CTA", smem);
-    const uint32_t want = (b->n_chunks + kPackWarps - 1) / kPackWarps;
-    const uint32_t grid = min(want, (uint32_t)sms * 8);
     const uint32_t nit = (prog.rec_words + 3) / 4;   // 16-byte vectors per lane for a full chunk: ceil(32 R / 4 / 32)
     int32_t rc;
-    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_off128, d_buf, grid, smem, st);
-    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_off128, d_buf, grid, smem, st);
-    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_off128, d_buf, grid, smem, st);
-    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_off128, d_buf, grid, smem, st);
-    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_off128, d_buf, grid, smem, st);
-    else rc = launch_pack_nit<12>(b, prog, d_off128, d_buf, grid, smem, st);
+    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    else rc = launch_pack_nit<12>(b, prog, d_occ_off128, d_buf, smem, sms, st);
     if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
