@@ -240,8 +240,31 @@ def time_steps(torch, fn, steps, warmup, flush, world):
     return [a.elapsed_time(b) for a, b in ev]
 
 
+def run_other_workload(args):
+    """configs[2..4] and the link probe (bench_workloads.py); single GPU, same JSON contract"""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if int(os.environ.get("RANK", 0)) != 0:
+        return
+    import paper_2606_23891_b200 as sph
+    import bench_workloads as bw
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
+    hbm_peak, sm_max_mhz, peak_src = measured_peaks()
+    common = {"hbm_peak": hbm_peak, "alu_peak": N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12, "peak_source": peak_src}
+    sampler = ClockSampler(0)
+    body = bw.RUNNERS[args.workload](args, sph, torch, common)
+    clocks = sampler.stop()
+    line = {"metric": METRIC, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "data": "synthetic", "clocks": clocks, "peak_source": peak_src}
+    line.update(body)
+    print(json.dumps(line))
+
+
 def run_ours(args):
     import torch
+    if args.workload != "config1":
+        return run_other_workload(args)
     rank, world, local = dist_setup(args.gpus)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
@@ -410,6 +433,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="both", choices=["split", "aos", "both"])
+    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4", "link"],
+                    help="config1 = BASELINE.json:configs[1] (the default bench line); the others are described in bench_workloads.py")
+    ap.add_argument("--n", type=int, default=0, help="particle count for config2/3/4 (default: the full size of BASELINE.json)")
+    ap.add_argument("--skip-zero-copy", action="store_true", help="config4: time the staged pipeline only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     args = ap.parse_args()

@@ -1,0 +1,542 @@
+"""Workloads of bench.py beyond the default one (BASELINE.json:configs[2..4] and the host-link probe).
+
+    python bench.py --workload config2     2^21 particles, Sod-like; pack FORCE_IN / force / unpack FORCE_OUT in bundles of 512 tasks, store in HBM
+    python bench.py --workload config3     2^24 clustered particles, octree; pack-only / unpack-only sweep over 3..20 fields, store in pinned host
+                                           memory, mapped zero-copy versus stage-then-H2D, AoS and split-AoS
+    python bench.py --workload config4     2^26 particles, whole step streamed in bundles of 4,096 tasks over 2 streams, store in pinned host memory
+    python bench.py --workload link        pinned H2D / D2H / both-ways copy bandwidth of this box (the host-link roofline)
+
+`--n N` shrinks the particle count (a power of two for config3/4, N = planes * 128 * 128 is kept for config2) for quick
+runs; the default is the full size of BASELINE.json.  Everything here is harness: the path itself runs in libsph_b200.
+Inputs are seeded and synthetic (sph_inputs/); no part of this file touches oracle/.
+"""
+import json
+import math
+import time
+
+import numpy as np
+
+GAMMA = float(np.float32(5.0 / 3.0))
+SWEEP_K = [3, 5, 8, 13, 16, 20]
+# reading C21: the configs[3] sweeps are prefixes of these lists of 4-byte scalar components
+PACK_SWEEP = [("x", 0), ("x", 1), ("x", 2), ("h", 0), ("mass", 0), ("rho", 0), ("rho_dh", 0), ("v", 0), ("v", 1), ("v", 2), ("u", 0), ("P", 0),
+              ("c_s", 0), ("wcount", 0), ("wcount_dh", 0), ("a", 0), ("a", 1), ("a", 2), ("du_dt", 0), ("v_sig", 0)]
+UNPACK_SWEEP = [("rho", 0), ("rho_dh", 0), ("wcount", 0), ("wcount_dh", 0), ("a", 0), ("a", 1), ("a", 2), ("du_dt", 0), ("v_sig", 0), ("div_v", 0),
+                ("rot_v", 0), ("rot_v", 1), ("rot_v", 2), ("P", 0), ("c_s", 0), ("u", 0), ("v", 0), ("v", 1), ("v", 2), ("h", 0)]
+
+
+def sweep_set(sph, lst, k, flags):
+    return sph.make_attrset([(f, c, 1) for f, c in lst[:k]], flags)
+
+
+def subs_of(sph, layout, comps):
+    """substruct indices that hold the given (field, comp) list"""
+    return sorted({layout.loc[sph.FIELD[f]].sub for f, _ in comps})
+
+
+def ev_time(torch, fn, reps=1, stream=None):
+    """milliseconds of fn() (average of reps back-to-back calls), CUDA events on the launching stream"""
+    st = stream if stream is not None else torch.cuda.current_stream()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(st)
+    for _ in range(reps):
+        fn()
+    b.record(st)
+    b.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def timed(torch, fn, steps, warmup, before=None):
+    """list of per-step ms; `before` (untimed) runs ahead of every step"""
+    out = []
+    for k in range(warmup + steps):
+        if before:
+            before()
+        torch.cuda.synchronize()
+        ms = ev_time(torch, fn)
+        if k >= warmup:
+            out.append(ms)
+    return out
+
+
+def link_probe(torch, nbytes=1 << 30, reps=5):
+    """pinned cudaMemcpyAsync bandwidth: H2D, D2H, and both at once on two streams [GB/s of payload per direction]"""
+    h_a = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    h_b = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d_a = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    d_b = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    res = {}
+
+    def best(fn):
+        t = []
+        for _ in range(reps + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            t.append(time.perf_counter() - t0)
+        return min(t[1:])
+
+    def h2d():
+        with torch.cuda.stream(s1):
+            d_a.copy_(h_a, non_blocking=True)
+
+    def d2h():
+        with torch.cuda.stream(s2):
+            h_b.copy_(d_b, non_blocking=True)
+
+    res["h2d_gbs"] = nbytes / best(h2d) / 1e9
+    res["d2h_gbs"] = nbytes / best(d2h) / 1e9
+    res["bidir_each_gbs"] = nbytes / best(lambda: (h2d(), d2h())) / 1e9
+    res["bytes"] = nbytes
+    return res
+
+
+# ------------------------------------------------------------------------------------------------- configs[2]
+
+def iterate_h_on_gpu(sph, torch, ps, cells, tasks, n_target=48.0, tol=0.01, max_iter=12):
+    """48-neighbour condition (reading C20): Newton on h with wcount, wcount_dh from the library's own density loop.
+    Setup for the bench workload (untimed); the parity tests use the oracle's iteration instead."""
+    layout = sph.sph_layout_split()
+    n = ps.shape[0]
+    store = sph.sph_store_create(layout, n)
+    sph.sph_store_set_cells(store, cells)
+    sph.sph_store_import_aos(store, ps)
+    batch = sph.sph_batch_create(store, tasks)
+    s_in, s_out = sph.sph_attrset_canonical(0), sph.sph_attrset_canonical(1)
+    b_in = torch.empty(sph.sph_batch_buffer_bytes(batch, s_in), dtype=torch.uint8, device="cuda")
+    b_out = torch.empty(sph.sph_batch_buffer_bytes(batch, s_out), dtype=torch.uint8, device="cuda")
+    h_cap = np.float32(0.4999 * cells["width"].min())
+    k_n = 32.0 / 3.0 * math.pi
+    sub_h, sub_o = layout.loc[sph.FIELD["h"]].sub, layout.loc[sph.FIELD["wcount"]].sub
+    host_h = np.zeros((n, layout.stride[sub_h] // 4), dtype=np.float32)     # S0 = {x f64[3], h, mass}: h is word 6
+    host_o = np.zeros((n, layout.stride[sub_o] // 4), dtype=np.float32)     # S1 = {rho, rho_dh, wcount, wcount_dh}
+    sph.sph_store_download_sub(store, sub_h, host_h)
+    torch.cuda.synchronize()
+    hw = layout.loc[sph.FIELD["h"]].off // 4
+    wc_w, wcd_w = layout.loc[sph.FIELD["wcount"]].off // 4, layout.loc[sph.FIELD["wcount_dh"]].off // 4
+    worst = None
+    for it in range(max_iter):
+        sph.sph_store_zero(store, s_out)
+        sph.sph_pack(store, batch, s_in, b_in)
+        sph.sph_density(batch, b_in, b_out)
+        sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE)
+        sph.sph_store_download_sub(store, sub_o, host_o)
+        torch.cuda.synchronize()
+        h = host_h[:, hw].astype(np.float64)
+        wc, wcd = host_o[:, wc_w].astype(np.float64), host_o[:, wcd_w].astype(np.float64)
+        f = k_n * h ** 3 * wc - n_target
+        worst = float(np.abs(f).max())
+        if worst <= tol:
+            break
+        df = k_n * (3.0 * h ** 2 * wc + h ** 3 * wcd)
+        step = np.where(df > 0, f / np.where(df > 0, df, 1.0), -0.1 * h)
+        h_new = np.clip(h - step, 0.8 * h, 1.25 * h)
+        host_h[:, hw] = np.minimum(h_new, h_cap).astype(np.float32)
+        sph.sph_store_upload_sub(store, sub_h, host_h)
+        torch.cuda.synchronize()
+    out = host_h[:, hw].copy()
+    sph.sph_batch_destroy(batch)
+    sph.sph_store_destroy(store)
+    return out, worst, it + 1
+
+
+def build_config2(sph, torch, seed, n):
+    """-> particles in cell order with h (48 neighbours), rho, rho_dh, u (P = 1 | 0.1), P, c_s set; cells; tasks"""
+    import sph_inputs as si
+    scale = max(1, int(round((2 ** 21 / n) ** (1.0 / 3.0))))
+    n_yz, n_left, n_right, cpd = 128 // scale, 102 // scale, 26 // scale, 32 // scale
+    parts = si.config2_positions(seed, n_yz=n_yz, n_left=n_left, n_right=n_right)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], cpd)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    width = float(cells["width"][0])
+    ps["h"] = np.minimum(ps["h"], np.float32(0.4999 * width))
+    hmax = np.full(cells.shape[0], np.float32(0.4999 * width), dtype=np.float32)
+    tasks, n_self, n_pair = sph.sph_tasks_build(cells, hmax)
+    h, worst, iters = iterate_h_on_gpu(sph, torch, ps, cells, tasks)
+    ps["h"] = h
+    # density pass -> rho, rho_dh; u from the target pressure; ghost -> P, c_s
+    layout = sph.sph_layout_aos()
+    store = sph.sph_store_create(layout, ps.shape[0])
+    sph.sph_store_set_cells(store, cells)
+    sph.sph_store_import_aos(store, ps)
+    batch = sph.sph_batch_create(store, tasks)
+    s_in, s_out = sph.sph_attrset_canonical(0), sph.sph_attrset_canonical(1)
+    b_in = torch.empty(sph.sph_batch_buffer_bytes(batch, s_in), dtype=torch.uint8, device="cuda")
+    b_out = torch.empty(sph.sph_batch_buffer_bytes(batch, s_out), dtype=torch.uint8, device="cuda")
+    sph.sph_store_zero(store, s_out)
+    sph.sph_pack(store, batch, s_in, b_in)
+    sph.sph_density(batch, b_in, b_out)
+    sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE)
+    torch.cuda.synchronize()
+    sph.sph_store_export_aos(store, ps)
+    p_target = np.where(ps["x"][:, 0] < 0.5, 1.0, 0.1)
+    ps["u"] = (p_target / ((GAMMA - 1.0) * ps["rho"].astype(np.float64))).astype(np.float32)
+    sph.sph_store_import_aos(store, ps)
+    sph.sph_ghost(store, sph.sph_params(np.float32(GAMMA), 0.8, 3.0))
+    torch.cuda.synchronize()
+    sph.sph_store_export_aos(store, ps)
+    sph.sph_batch_destroy(batch)
+    sph.sph_store_destroy(store)
+    del b_in, b_out
+    info = {"cells_per_dim": cpd, "h_iterations": iters, "worst_neighbour_error": worst, "h_min": float(h.min()), "h_max": float(h.max()),
+            "per_cell_min": int(cells["count"].min()), "per_cell_max": int(cells["count"].max())}
+    return ps, cells, tasks, info
+
+
+def run_config2(args, sph, torch, common):
+    hbm_peak, alu_peak = common["hbm_peak"], common["alu_peak"]
+    n = args.n or (1 << 21)
+    ps, cells, tasks, setup = build_config2(sph, torch, 1, n)
+    n = ps.shape[0]
+    params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
+    s_in, s_out = sph.sph_attrset_canonical(2), sph.sph_attrset_canonical(3)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)
+    out = {}
+    for name in ("split", "aos"):
+        layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
+        store = sph.sph_store_create(layout, n)
+        sph.sph_store_set_cells(store, cells)
+        sph.sph_store_import_aos(store, ps)
+        batch = sph.sph_batch_create(store, tasks, 512)                    # 896 bundles of 512 tasks under one launch per stage
+        info = sph.sph_batch_get_info(batch)
+        b_in = torch.empty(sph.sph_batch_buffer_bytes(batch, s_in), dtype=torch.uint8, device="cuda")
+        b_out = torch.empty(sph.sph_batch_buffer_bytes(batch, s_out), dtype=torch.uint8, device="cuda")
+        stages = [("zero_force_out", lambda: sph.sph_store_zero(store, s_out)),
+                  ("pack_force_in", lambda: sph.sph_pack(store, batch, s_in, b_in)),
+                  ("force", lambda: sph.sph_force(batch, b_in, b_out, params)),
+                  ("unpack_force_out", lambda: sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE))]
+        step = lambda: [fn() for _, fn in stages]
+        t = timed(torch, step, args.steps, args.warmup, before=flush)
+        per = {k: [] for k, _ in stages}
+        for _ in range(args.steps):
+            flush()
+            torch.cuda.synchronize()
+            for k, fn in stages:
+                per[k].append(ev_time(torch, fn))
+        per = {k: sum(v) / len(v) for k, v in per.items()}
+        # one bundle alone (isolated latency of pack + force + unpack of 512 pair tasks)
+        one = sph.sph_batch_create(store, tasks[info.n_self:info.n_self + 512])
+        o_in = torch.empty(sph.sph_batch_buffer_bytes(one, s_in), dtype=torch.uint8, device="cuda")
+        o_out = torch.empty(sph.sph_batch_buffer_bytes(one, s_out), dtype=torch.uint8, device="cuda")
+        one_step = lambda: (sph.sph_pack(store, one, s_in, o_in), sph.sph_force(one, o_in, o_out, params),
+                            sph.sph_unpack(store, one, s_out, o_out, sph.SPH_UNPACK_REDUCE))
+        t_one = timed(torch, one_step, args.steps, args.warmup, before=flush)
+        sph.sph_batch_destroy(one)
+        inst, cand = info.n_instances, info.n_candidates
+        alg = {"pack_force_in": n * 64 + inst * 52, "unpack_force_out": inst * 20 + n * 2 * 20}
+        kern = {}
+        for k, ms in per.items():
+            e = {"ms": round(ms, 4)}
+            if k in alg:
+                e.update(bound="hbm", achieved=round(alg[k] / (ms * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s")
+                e["frac"] = round(e["achieved"] / hbm_peak, 4)
+                e["instances_per_s"] = inst / (ms * 1e-3)
+            if k == "force":
+                e.update(bound="alu", candidate_pairs_per_s=cand / (ms * 1e-3))
+            kern[k] = e
+        out[name] = {"ms_per_step": sum(t) / len(t), "kernels": kern, "single_bundle_ms": sum(t_one) / len(t_one),
+                     "tasks": int(info.n_tasks), "bundles": int(info.n_segments), "instances": int(inst), "candidate_pairs": int(cand)}
+        sph.sph_batch_destroy(batch)
+        sph.sph_store_destroy(store)
+        del b_in, b_out, o_in, o_out
+    P = out["split"]
+    dominant = max(("pack_force_in", "force", "unpack_force_out"), key=lambda k: P["kernels"][k]["ms"])
+    roof = {k: v for k, v in P["kernels"][dominant].items() if k != "ms"}
+    roof.update(kernel=dominant, launch_ms=P["kernels"][dominant]["ms"], traffic=None)
+    return {
+        "value": n / (P["ms_per_step"] * 1e-3), "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
+        "config": {"workload": f"configs[2]: {n} particles, Sod-like two-density lattice, h by the 48-neighbour condition, force loop in bundles of 512 tasks",
+                   "layout": "split", "store": "HBM", "l2": "flushed before every step (256 MB fill, untimed)", "setup": setup,
+                   "tasks": P["tasks"], "bundles": P["bundles"], "instances": P["instances"], "candidate_pairs": P["candidate_pairs"]},
+        "gpu_launches": 4 * args.steps, "roofline": roof, "kernels": P["kernels"], "single_bundle_ms": P["single_bundle_ms"],
+        "aos": {"ms_per_step": out["aos"]["ms_per_step"], "kernels": out["aos"]["kernels"], "single_bundle_ms": out["aos"]["single_bundle_ms"]},
+        "e2e": None,
+    }
+
+
+# ------------------------------------------------------------------------------------------------- configs[3], configs[4]: common setup
+
+def build_clumpy(sph, which, seed, n):
+    """clustered particles -> octree (<= 400 per leaf) -> cell order, cells, tasks"""
+    import sph_inputs as si
+    t0 = time.perf_counter()
+    parts = si.config3(seed, n) if which == 3 else si.config4(seed, n)
+    t1 = time.perf_counter()
+    perm, cells = sph.sph_cells_build_octree(parts["x"], parts["h"], 400)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    del parts
+    hmax = np.maximum.reduceat(ps["h"], cells["first"].astype(np.int64)).astype(np.float32)
+    tasks, n_self, n_pair = sph.sph_tasks_build(cells, hmax)
+    cnt = cells["count"]
+    info = {"cells": int(cells.shape[0]), "per_cell_min": int(cnt.min()), "per_cell_max": int(cnt.max()), "per_cell_mean": round(float(cnt.mean()), 1),
+            "per_cell_median": float(np.median(cnt)), "self_tasks": int(n_self), "pair_tasks": int(n_pair),
+            "generate_s": round(t1 - t0, 1), "cells_and_tasks_s": round(time.perf_counter() - t1, 1)}
+    return ps, cells, tasks, info
+
+
+class HostStore:
+    """A store in pinned host memory the GPU maps (zero-copy), doubling as the host side of the staged path."""
+
+    def __init__(self, sph, torch, layout, ps, cells):
+        self.sph, self.layout, self.n = sph, layout, ps.shape[0]
+        self.host = [torch.empty(sph.sph_store_sub_bytes(layout, self.n, s), dtype=torch.uint8).pin_memory() for s in range(layout.n_sub)]
+        self.store = sph.sph_store_create(layout, self.n, sph.SPH_MEM_HOST_PINNED, ext=self.host)
+        sph.sph_store_import_aos(self.store, ps)
+        sph.sph_store_set_cells(self.store, cells)
+
+    def sub(self, s):
+        """the substruct array without its tail bytes (what upload / download move)"""
+        return self.host[s][: self.n * self.layout.stride[s]]
+
+    def close(self):
+        self.sph.sph_store_destroy(self.store)
+        self.host = None
+
+
+def field_bytes(comps):
+    return sum(8 if f == "x" else 4 for f, _ in comps)
+
+
+def run_config3(args, sph, torch, common):
+    n = args.n or (1 << 24)
+    ps, cells, tasks, setup = build_clumpy(sph, 3, 1, n)
+    link = link_probe(torch)
+    rows = []
+    best = {}
+    for name in ("split", "aos"):
+        layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
+        hs = HostStore(sph, torch, layout, ps, cells)
+        dev = sph.sph_store_create(layout, n)
+        sph.sph_store_set_cells(dev, cells)
+        batch = sph.sph_batch_create(hs.store, tasks)
+        info = sph.sph_batch_get_info(batch)
+        inst = info.n_instances
+        big = sweep_set(sph, PACK_SWEEP, 20, sph.SPH_ATTR_X_REL_F32)
+        buf = torch.zeros(sph.sph_batch_buffer_bytes(batch, big), dtype=torch.uint8, device="cuda")
+        for k in SWEEP_K:
+            # ---- pack
+            comps = PACK_SWEEP[:k]
+            aset = sweep_set(sph, PACK_SWEEP, k, sph.SPH_ATTR_X_REL_F32)
+            sph.sph_batch_buffer_bytes(batch, aset)
+            subs = subs_of(sph, layout, comps)
+            useful = n * field_bytes(comps)                       # link-minimal: every needed store byte crosses once
+            staged_bytes = sum(n * layout.stride[s] for s in subs)
+
+            def zc():
+                sph.sph_pack(hs.store, batch, aset, buf)
+
+            def staged():
+                for s in subs:
+                    sph.sph_store_upload_sub(dev, s, hs.sub(s))
+                sph.sph_pack(dev, batch, aset, buf)
+
+            for mode, fn, moved in (("zero-copy", zc, None), ("staged", staged, staged_bytes)):
+                t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
+                rows.append({"op": "pack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
+                             "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),
+                             "moved_link_gbs": None if moved is None else round(moved / (t * 1e-3) / 1e9, 2),
+                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["h2d_gbs"], 3)})
+            # ---- unpack (REDUCE: += for the sums, max for v_sig, = for the rest)
+            comps = UNPACK_SWEEP[:k]
+            aset = sweep_set(sph, UNPACK_SWEEP, k, 0)
+            sph.sph_batch_buffer_bytes(batch, aset)
+            subs = subs_of(sph, layout, comps)
+            useful = n * 4 * k                                    # every result field lands in the host store once
+            staged_bytes = sum(n * layout.stride[s] for s in subs)
+
+            def zc_u():
+                sph.sph_unpack(hs.store, batch, aset, buf, sph.SPH_UNPACK_REDUCE)
+
+            def staged_u():
+                sph.sph_unpack(dev, batch, aset, buf, sph.SPH_UNPACK_REDUCE)
+                for s in subs:
+                    sph.sph_store_download_sub(dev, s, hs.sub(s))
+
+            for mode, fn, moved in (("zero-copy", zc_u, None), ("staged", staged_u, staged_bytes)):
+                t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
+                rows.append({"op": "unpack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
+                             "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),
+                             "moved_link_gbs": None if moved is None else round(moved / (t * 1e-3) / 1e9, 2),
+                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["d2h_gbs"], 3)})
+        setup.update(tasks=int(info.n_tasks), instances=int(inst))
+        sph.sph_batch_destroy(batch)
+        sph.sph_store_destroy(dev)
+        hs.close()
+        del buf
+    def pick(op, layout, k):
+        c = [r for r in rows if r["op"] == op and r["layout"] == layout and r["k"] == k]
+        return min(c, key=lambda r: r["ms"])
+    p13, u13 = pick("pack", "split", 13), pick("unpack", "split", 13)
+    ms = p13["ms"] + u13["ms"]
+    useful13 = n * (field_bytes(PACK_SWEEP[:13]) + 4 * 13)
+    roof = {"bound": "host-link", "achieved": round(useful13 / (ms * 1e-3) / 1e9, 2), "peak": round(link["h2d_gbs"], 2), "unit": "GB/s",
+            "frac": round(useful13 / (ms * 1e-3) / 1e9 / link["h2d_gbs"], 3), "traffic": None, "kernel": "pack + unpack, 13 fields, split-AoS, best mode",
+            "peak_source": "pinned H2D copy bandwidth measured in this run"}
+    return {"value": n / (ms * 1e-3), "unit": "particles/s", "ms_per_step": ms, "dtype": "u8",
+            "config": {"workload": f"configs[3]: {n} clustered particles, octree <= 400 per leaf, pack-only / unpack-only sweep, store in pinned host memory",
+                       "layout": "split", "store": "pinned host", "l2": "inputs larger than L2", "setup": setup, "link": link,
+                       "step": "pack 13 fields + unpack 13 fields, each in its faster mode"},
+            "gpu_launches": 2 * args.steps, "roofline": roof, "sweep": rows, "e2e": None}
+
+
+# ------------------------------------------------------------------------------------------------- configs[4]
+
+class Pipeline:
+    """The whole offload step streamed in bundles of `bundle` tasks over two streams, captured once as a CUDA graph.
+
+    mode "staged":    per loop the substructs the loop reads are copied H2D into a device staging store, bundles run against
+                      it (pack -> loop -> unpack on alternating streams, unpacks chained in bundle order so the reduction order
+                      is the task order), the substructs the loop wrote are copied D2H into the host store.
+    mode "zero-copy": the same kernels read and write the mapped host store directly over the host link.
+    """
+
+    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode):
+        self.sph, self.torch, self.layout, self.hs, self.mode = sph, torch, layout, hs, mode
+        n = hs.n
+        self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+        self.params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
+        if mode == "staged":
+            self.dev = sph.sph_store_create(layout, n)
+            sph.sph_store_set_cells(self.dev, cells)
+            self.work = self.dev
+        else:
+            self.dev = None
+            self.work = hs.store
+        self.batches = []
+        for lo, hi in ((0, n_self), (n_self, tasks.shape[0])):          # homogeneous bundles: self tasks, then pair tasks (C22)
+            for s in range(lo, hi, bundle):
+                self.batches.append(sph.sph_batch_create(hs.store, tasks[s:min(hi, s + bundle)]))
+        need = [0, 0, 0, 0]
+        self.instances = 0
+        self.candidates = 0
+        for b in self.batches:
+            for k in range(4):
+                need[k] = max(need[k], sph.sph_batch_buffer_bytes(b, self.sets[k]))
+            info = sph.sph_batch_get_info(b)
+            self.instances += info.n_instances
+            self.candidates += info.n_candidates
+        self.bufs = [[torch.empty(max(nb, 256), dtype=torch.uint8, device="cuda") for nb in need] for _ in range(2)]
+        self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        self.copy = torch.cuda.Stream()
+        F = sph.FIELD
+        sub = lambda names: sorted({layout.loc[F[k]].sub for k in names})
+        self.up_density, self.down_density = sub(["x", "h", "mass"]), sub(["rho", "rho_dh", "wcount", "wcount_dh"])
+        self.up_force = [s for s in sub(["v", "u", "P", "c_s"]) if s not in self.up_density and s not in self.down_density]
+        self.down_force = sorted(set(sub(["a", "du_dt", "v_sig"]) + sub(["P", "c_s"])))
+        self.h2d_bytes = sum(n * layout.stride[s] for s in self.up_density + self.up_force) if mode == "staged" else 0
+        self.d2h_bytes = sum(n * layout.stride[s] for s in self.down_density + self.down_force) if mode == "staged" else 0
+        self.launches = 0
+
+    def _loop(self, root, k_in, k_out, kernel, ups, downs):
+        sph, torch = self.sph, self.torch
+        s_in, s_out = self.sets[k_in], self.sets[k_out]
+        if self.mode == "staged":
+            self.copy.wait_stream(root)
+            for s in ups:
+                sph.sph_store_upload_sub(self.dev, s, self.hs.sub(s), self.copy)
+            root.wait_stream(self.copy)
+        sph.sph_store_zero(self.work, s_out, root)
+        self.launches += 1
+        for st in self.streams:
+            st.wait_stream(root)
+        prev = None
+        for b, batch in enumerate(self.batches):
+            st, bufs = self.streams[b & 1], self.bufs[b & 1]
+            sph.sph_pack(self.work, batch, s_in, bufs[k_in], st)
+            kernel(batch, bufs[k_in], bufs[k_out], st)
+            if prev is not None:
+                st.wait_event(prev)                                       # unpacks in bundle order
+            sph.sph_unpack(self.work, batch, s_out, bufs[k_out], sph.SPH_UNPACK_REDUCE, st)
+            prev = torch.cuda.Event()
+            prev.record(st)
+            self.launches += 3
+        for st in self.streams:
+            root.wait_stream(st)
+        if self.mode == "staged" and downs:
+            self.copy.wait_stream(root)
+            for s in downs:
+                sph.sph_store_download_sub(self.dev, s, self.hs.sub(s), self.copy)
+            # the copy-out overlaps whatever follows on `root`; joined at the end of the step
+
+    def step(self, root):
+        sph = self.sph
+        self.launches = 0
+        self._loop(root, 0, 1, lambda b, i, o, st: sph.sph_density(b, i, o, st), self.up_density, self.down_density)
+        if self.mode == "staged":
+            for s in self.up_force:
+                sph.sph_store_upload_sub(self.dev, s, self.hs.sub(s), root)
+        sph.sph_ghost(self.work, self.params, root)
+        self.launches += 1
+        self._loop(root, 2, 3, lambda b, i, o, st: sph.sph_force(b, i, o, self.params, st), [], self.down_force)
+        if self.mode == "staged":
+            root.wait_stream(self.copy)
+
+    def capture(self):
+        torch = self.torch
+        root = torch.cuda.Stream()
+        with torch.cuda.stream(root):
+            self.step(root)                                               # warm-up outside the capture (first-call attribute setting)
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=root):
+            self.step(root)
+        return self.graph
+
+    def close(self):
+        for b in self.batches:
+            self.sph.sph_batch_destroy(b)
+        if self.dev is not None:
+            self.sph.sph_store_destroy(self.dev)
+
+
+def run_config4(args, sph, torch, common):
+    n = args.n or (1 << 26)
+    ps, cells, tasks, setup = build_clumpy(sph, 4, 1, n)
+    n_self = int(cells.shape[0])
+    link = link_probe(torch)
+    res = {}
+    for name in ("split", "aos"):
+        layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
+        hs = HostStore(sph, torch, layout, ps, cells)
+        for mode in ("staged", "zero-copy"):
+            if mode == "zero-copy" and args.skip_zero_copy:
+                continue
+            pl = Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, mode)
+            t0 = time.perf_counter()
+            g = pl.capture()
+            cap_s = time.perf_counter() - t0
+            t = timed(torch, g.replay, args.steps, min(args.warmup, 2))
+            ms = sum(t) / len(t)
+            res[f"{name}/{mode}"] = {"ms_per_step": ms, "particles_per_s": n / (ms * 1e-3), "bundles": len(pl.batches), "launches_per_step": pl.launches,
+                                     "h2d_bytes_per_step": pl.h2d_bytes, "d2h_bytes_per_step": pl.d2h_bytes,
+                                     "link_gbs": round((pl.h2d_bytes + pl.d2h_bytes) / (ms * 1e-3) / 1e9, 2) if mode == "staged" else None,
+                                     "instances_per_loop": int(pl.instances), "candidate_pairs_per_loop": int(pl.candidates),
+                                     "capture_s": round(cap_s, 1)}
+            pl.close()
+            del pl, g
+        hs.close()
+    key = min((k for k in res if k.startswith("split")), key=lambda k: res[k]["ms_per_step"])
+    P = res[key]
+    link_time = max(P["h2d_bytes_per_step"] / link["h2d_gbs"], P["d2h_bytes_per_step"] / link["d2h_gbs"]) / 1e9 * 1e3 if P["h2d_bytes_per_step"] else None
+    roof = {"bound": "host-link", "achieved": P["link_gbs"], "peak": round(link["h2d_gbs"], 2), "unit": "GB/s",
+            "frac": None if not P["link_gbs"] else round(P["link_gbs"] / (link["h2d_gbs"] + link["d2h_gbs"]), 3), "traffic": None,
+            "kernel": "whole step (H2D + pack/loop/unpack bundles + D2H)", "link_bound_ms": link_time,
+            "peak_source": "pinned H2D / D2H copy bandwidth measured in this run"}
+    return {"value": P["particles_per_s"], "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
+            "config": {"workload": f"configs[4]: {n} particles (uniform + clumps), whole step in bundles of 4096 tasks over 2 streams, store in pinned host memory",
+                       "layout": key, "store": "pinned host", "l2": "inputs larger than L2", "setup": setup, "link": link},
+            "gpu_launches": P["launches_per_step"] * args.steps, "roofline": roof, "variants": res,
+            "e2e": {"value": P["particles_per_s"], "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes_per_step"],
+                    "d2h_bytes_per_step": P["d2h_bytes_per_step"], "ms_per_step": P["ms_per_step"]}}
+
+
+def run_link(args, sph, torch, common):
+    link = link_probe(torch, reps=10)
+    return {"value": link["h2d_gbs"], "unit": "GB/s", "ms_per_step": None, "dtype": "u8", "metric": "pinned host-link copy bandwidth",
+            "config": {"workload": "link: 1 GiB pinned cudaMemcpyAsync, best of 10", "link": link}, "gpu_launches": 0, "roofline": None, "e2e": None}
+
+
+RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link}

@@ -465,14 +465,14 @@ static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_byte
 int32_t sph_density(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, void* stream) {
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 20, 16, &oin, &oout)) return rc;
-    return launch_density(b, oin->d_off128, oout->d_off128, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+    return launch_density(b, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
 }
 
 int32_t sph_force(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, const sph_params* prm, void* stream) {
     if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 52, 20, &oin, &oout)) return rc;
-    return launch_force(b, oin->d_off128, oout->d_off128, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    return launch_force(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
 }
 
 int32_t sph_ghost(sph_store* s, const sph_params* prm, void* stream) {

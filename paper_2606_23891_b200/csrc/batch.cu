@@ -139,6 +139,21 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     if (!rc) rc = upload(occ_frames, &b->d_occ_frames);
     for (uint32_t rec : {16u, 20u, 52u})
         if (!rc) rc = ensure_offsets(b, rec, nullptr);
+    // loop work items (one per 32-particle target chunk), for the canonical record sizes of the two loops
+    if (!rc && b->max_count >= (1u << 26)) rc = fail(SPH_ERR_RANGE, "a cell of %u particles is too large for the loop item table", b->max_count);
+    if (!rc) {
+        const std::vector<uint64_t>&o16 = find_offsets(b, 16)->h_off, &o20 = find_offsets(b, 20)->h_off, &o52 = find_offsets(b, 52)->h_off;
+        std::vector<LoopItem> dens(b->n_chunks), forc(b->n_chunks);
+        for (uint32_t ch = 0; ch < b->n_chunks; ++ch) {
+            const uint32_t tgt = chunk_side[ch], src = chunk_src[ch];
+            const uint32_t kc = ch - b->sides[tgt].chunk0;                       // chunk index inside the block
+            const uint32_t nt_ns = std::min(32u, b->sides[tgt].count - 32 * kc) | b->sides[src].count << 6;
+            dens[ch] = LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4, nt_ns};
+            forc[ch] = LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5, nt_ns};
+        }
+        rc = upload(dens, &b->d_items_density);
+        if (!rc) rc = upload(forc, &b->d_items_force);
+    }
     if (rc) { sph_batch_destroy(b); return rc; }
     *out = b;
     return SPH_OK;
@@ -147,7 +162,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
     cudaFree(b->d_sides); cudaFree(b->d_frames); cudaFree(b->d_chunk_side); cudaFree(b->d_task_side0);
-    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames);
+    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;

@@ -53,6 +53,15 @@ struct CellChunk {
     uint32_t nocc;
 };
 
+// work item of the density / force loops: 32 targets of one block against the block they gather from.
+// Offsets in units of 128 bytes into the loop's input / output buffer (chunk starts are multiples of 128 bytes).
+struct LoopItem {
+    uint32_t tin128;     // the targets' input records
+    uint32_t sin128;     // first input record of the source block
+    uint32_t tout128;    // the targets' result records
+    uint32_t nt_ns;      // targets (1..32) | sources << 6
+};
+
 // word kinds of the pack / unpack programs
 enum : uint32_t { W_COPY = 0, W_XREL = 1, W_TIMEBIN = 2,            // pack (host side only: the kernel sees plain copies)
                   W_SUM = 3, W_MAX = 4, W_ASSIGN = 5, W_ASSIGN_BYTE = 6, W_SKIP = 7 };   // unpack
@@ -134,6 +143,8 @@ struct sph_batch {
     uint32_t* d_task_side0 = nullptr;         // task -> first side (n_tasks + 1 entries)
     uint32_t* d_chunk_src = nullptr;          // pack chunk -> the side its targets gather from (partner side; itself for self tasks)
     sph::CellChunk* d_cell_chunks = nullptr;
+    sph::LoopItem* d_items_density = nullptr; // one per 32-particle target chunk (20-byte in, 16-byte out records)
+    sph::LoopItem* d_items_force = nullptr;   // (52-byte in, 20-byte out records)
     std::map<uint32_t, sph::OffsetTable> offsets;   // by record bytes
 };
 
@@ -145,9 +156,8 @@ int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable**
 int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, cudaStream_t st);
-int32_t launch_density(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out, cudaStream_t st);
-int32_t launch_force(const sph_batch* b, const uint32_t* d_off_in, const uint32_t* d_off_out, const char* d_in, char* d_out,
-                     const sph_params& prm, cudaStream_t st);
+int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
+int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);
 int32_t launch_ghost(const StoreView& view, uint64_t n, const sph_layout& layout, const sph_params& prm, cudaStream_t st);
 }  // namespace sph
