@@ -162,6 +162,15 @@ int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, i
             }
         }
     }
+    for (uint32_t k = 0; k + 3 < prog->rec_words; ++k) {
+        const WordDesc& a = prog->word[k];
+        bool ok = a.stride % 16 == 0 && a.a % 16 == 0;
+        for (uint32_t j = 0; j < 4 && ok; ++j) {
+            const WordDesc& b = prog->word[k + j];
+            ok = b.sub == a.sub && b.a == a.a + 4 * j && b.kind != W_ASSIGN_BYTE;
+        }
+        prog->vec4[k] = ok;
+    }
     return SPH_OK;
 }
 

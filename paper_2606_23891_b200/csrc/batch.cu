@@ -121,6 +121,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     for (uint32_t c = 0; c < n_cells; ++c) {
         if (!occ_count[c]) continue;
         ++b->n_cells_touched;
+        b->max_nocc = std::max(b->max_nocc, occ_count[c]);
         const sph_cell& ce = store->cells[c];
         for (uint32_t k = 0; k < ce.count; k += 32)
             cell_chunks.push_back(CellChunk{(uint32_t)ce.first + k, std::min(32u, ce.count - k), k, occ_start[c], occ_count[c]});

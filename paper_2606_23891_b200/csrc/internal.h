@@ -98,6 +98,7 @@ struct Program {
     uint32_t tb, tb_src, tb_stride, tb_dst;
     PackSub su[SPH_MAX_SUB];
     WordDesc word[kMaxRecWords];
+    uint8_t vec4[kMaxRecWords];    // unpack: words w..w+3 are 16 contiguous, 16-byte aligned bytes of one substruct (all plain f32 words)
 };
 
 int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog);
@@ -130,7 +131,7 @@ struct sph_store {
 
 struct sph_batch {
     uint64_t n_tasks = 0, n_self = 0, n_pair = 0;
-    uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0;
+    uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
     uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
     std::vector<sph::SideRec> sides;          // host copy
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists

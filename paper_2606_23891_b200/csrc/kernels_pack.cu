@@ -35,11 +35,6 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ void st_stream16(void* p, uint4 v) {   // records are written once and read by another kernel
     asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-__device__ __forceinline__ uint4 ld_once16(const void* p) {   // records are read exactly once: keep them out of L1
-    uint4 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-    return v;
-}
 
 template <int NIT>
 __global__ void __launch_bounds__(kPackWarps * 32)
@@ -162,89 +157,168 @@ pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint3
 
 // ---------------------------------------------------------------------------------------------------------
 
-// meta word of the hoisted unpack map: store byte offset relative to the chunk's first particle | sub << 20 | kind << 24
-__device__ __forceinline__ char* word_ptr(const StoreView* s_view, uint32_t meta, uint64_t first) {
-    const uint32_t sub = (meta >> 20) & 0xF;
-    return s_view->base[sub] + first * s_view->stride[sub] + (meta & 0xFFFFF);
-}
-
-template <int NIT, bool kLastOnly>
+// One warp per 32-particle chunk of a cell.
+//  (1) fetch: the chunk's slice of every block the cell occurs in (up to `slots` per round, normally all of them) is
+//      copied into the warp's shared-memory ring with 16-byte cp.async -- no registers are held while the loads are
+//      in flight, so a warp keeps 14-17 KB outstanding and an SM close to 200 KB;
+//  (2) reduce: one lane per particle walks the slices in ascending (task, side) order.  With the lane owning a
+//      record, the operator of word j (+=, max, =) is the same in every lane: no per-lane dispatch, no divergence.
+//      Records are read with VEC-word shared loads (stride = record length: conflict-free when R / VEC is odd).
+//  Words are processed in groups of GW; a record longer than GW keeps its running values in a scratch slot.
+// The descriptor and block-offset table of the warp's next chunk are fetched while the current slices are in flight.
+template <int VEC, int GW>
 __global__ void __launch_bounds__(kUnpackWarps * 32)
 unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
-              uint32_t n_cell_chunks, const char* __restrict__ buf) {
-    constexpr int UNR = NIT >= 8 ? 1 : (NIT >= 4 ? 2 : (NIT >= 2 ? 4 : 8));   // blocks whose records are in flight together
-    __shared__ StoreView s_view;     // indexed per lane (the substruct differs from word to word)
-    if (threadIdx.x == 0) s_view = view;
-    __syncthreads();
+              uint32_t n_cell_chunks, const char* __restrict__ buf, uint32_t slots, uint32_t last_only, uint32_t all_sum) {
+    extern __shared__ __align__(16) unsigned char smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t R = prog.rec_words;
-    uint32_t meta[NIT][4];
+    const uint32_t slot_bytes = 128 * R;
+    const bool single = R <= GW;                       // the whole record lives in registers; else slot 0 is the scratch
+    unsigned char* wbase = smem + (size_t)warp * (slots + (single ? 0u : 1u)) * slot_bytes;
+    float* scratch = reinterpret_cast<float*>(wbase);  // [R][32]
+    unsigned char* ring = wbase + (single ? 0u : slot_bytes);
+
+    auto rounds_of = [&](const CellChunk& c, uint32_t* o_begin, uint32_t* per_round) {
+        *o_begin = last_only ? c.nocc - 1 : 0;
+        const uint32_t n_o = c.nocc - *o_begin, n_rounds = (n_o + slots - 1) / slots;
+        *per_round = (n_o + n_rounds - 1) / n_rounds;                     // <= slots <= 32
+    };
+    auto first_table = [&](const CellChunk& c) {
+        uint32_t o_begin, per_round;
+        rounds_of(c, &o_begin, &per_round);
+        return lane < min(per_round, c.nocc - o_begin) ? __ldg(occ_off128 + c.occ0 + o_begin + lane) : 0u;
+    };
+    // store access of word w of the lane's particle p
+    auto word_addr = [&](uint32_t w, uint64_t p) { return view.base[prog.word[w].sub] + p * prog.word[w].stride + prog.word[w].a; };
+    auto is_reduced = [&](uint32_t w) { return prog.word[w].kind == W_SUM || prog.word[w].kind == W_MAX; };
+
+    // one group of words [g0, g0 + nw) reduced over the `lim` slices of the ring, in slice order
+    auto reduce_group = [&](float (&acc)[GW], uint32_t g0, uint32_t nw, uint32_t lim) {
+        const unsigned char* rec = ring + (lane * R + g0) * 4;
+        uint32_t m_sum[GW], m_red[GW];
 #pragma unroll
-    for (int it = 0; it < NIT; ++it)
+        for (int j = 0; j < GW; ++j) {
+            const uint32_t kind = (uint32_t)j < nw ? prog.word[g0 + j].kind : (uint32_t)W_SKIP;
+            m_sum[j] = kind == W_SUM ? 0xFFFFFFFFu : 0u;
+            m_red[j] = kind == W_SUM || kind == W_MAX ? 0xFFFFFFFFu : 0u;
+        }
+#pragma unroll 4
+        for (uint32_t u = 0; u < lim; ++u, rec += slot_bytes) {
+            float rv[GW];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t g = 4 * (lane + 32 * it) + j;
-            const uint32_t k = g / R, w = g - k * R;
-            meta[it][j] = k < 32 ? (k * prog.word[w].stride + prog.word[w].a) | (uint32_t)prog.word[w].sub << 20 | (uint32_t)prog.word[w].kind << 24
-                                 : (uint32_t)W_SKIP << 24;
+            for (int j = 0; j < GW; j += VEC) {
+                if ((uint32_t)j >= nw) { for (int q = 0; q < VEC; ++q) rv[j + q] = 0.f; continue; }
+                if constexpr (VEC == 4) {
+                    const float4 t = *reinterpret_cast<const float4*>(rec + 4 * j);
+                    rv[j] = t.x; rv[j + 1] = t.y; rv[j + 2] = t.z; rv[j + 3] = t.w;
+                } else if constexpr (VEC == 2) {
+                    const float2 t = *reinterpret_cast<const float2*>(rec + 4 * j);
+                    rv[j] = t.x; rv[j + 1] = t.y;
+                } else {
+                    rv[j] = *reinterpret_cast<const float*>(rec + 4 * j);
+                }
+            }
+            if (all_sum) {
+#pragma unroll
+                for (int j = 0; j < GW; ++j) acc[j] = __fadd_rn(acc[j], rv[j]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < GW; ++j) {   // bit-select, not a branch: sum where m_sum, max where m_red only, else the record's value
+                    const uint32_t s = __float_as_uint(__fadd_rn(acc[j], rv[j])), m = __float_as_uint(fmaxf(acc[j], rv[j]));
+                    const uint32_t t = (s & m_sum[j]) | (m & ~m_sum[j]);
+                    acc[j] = __uint_as_float((t & m_red[j]) | (__float_as_uint(rv[j]) & ~m_red[j]));
+                }
+            }
+        }
+    };
+
+    const uint32_t cc_step = gridDim.x * kUnpackWarps;
+    uint32_t cc = blockIdx.x * kUnpackWarps + warp;
+    CellChunk ch_next{};
+    uint32_t tbl_next = 0;
+    if (cc < n_cell_chunks) { ch_next = cell_chunks[cc]; tbl_next = first_table(ch_next); }
+    for (; cc < n_cell_chunks; cc += cc_step) {
+        const CellChunk ch = ch_next;
+        const uint32_t tbl_first = tbl_next;
+        const uint32_t nvec = (ch.count * R + 3) >> 2;
+        const char* slice = buf + (uint64_t)ch.k0 * R * 4 + 16 * lane;
+        const bool live = lane < ch.count;
+        const uint64_t p = (uint64_t)ch.first + lane;
+        uint32_t o_begin, per_round;
+        rounds_of(ch, &o_begin, &per_round);
+
+        // running values: the store's own for the reduced words (issued before the slices are waited for)
+        float acc[GW];
+        if (single) {
+#pragma unroll
+            for (int j = 0; j < GW; ++j) acc[j] = 0.f;
+#pragma unroll
+            for (int j = 0; j < GW; ++j) {
+                if ((uint32_t)j >= R || !live) continue;
+                if (j % 4 == 0 && j + 3 < GW && prog.vec4[j]) {
+                    const float4 t = *reinterpret_cast<const float4*>(word_addr(j, p));
+                    acc[j] = t.x; if (j + 1 < GW) acc[j + 1] = t.y; if (j + 2 < GW) acc[j + 2] = t.z; if (j + 3 < GW) acc[j + 3] = t.w;
+                } else if (!(j >= 4 * (j / 4) && prog.vec4[4 * (j / 4)] && 4 * (j / 4) + 3 < GW) && is_reduced(j)) {
+                    acc[j] = *reinterpret_cast<const float*>(word_addr(j, p));
+                }
+            }
+        } else {
+            for (uint32_t w = 0; w < R; ++w)
+                scratch[w * 32 + lane] = live && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
         }
 
-    for (uint32_t cc = blockIdx.x * kUnpackWarps + warp; cc < n_cell_chunks; cc += gridDim.x * kUnpackWarps) {
-        const CellChunk ch = cell_chunks[cc];
-        const uint32_t total = ch.count * R, nvec = (total + 3) >> 2;
-        const char* slice = buf + (uint64_t)ch.k0 * R * 4 + 16 * lane;
-        float acc[NIT][4];
-        uint32_t kind[NIT][4];
-#pragma unroll
-        for (int it = 0; it < NIT; ++it)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t g = 4 * (lane + 32 * it) + j;
-                kind[it][j] = g < total ? meta[it][j] >> 24 : (uint32_t)W_SKIP;
-                acc[it][j] = 0.f;
-                if (!kLastOnly && (kind[it][j] == W_SUM || kind[it][j] == W_MAX))
-                    acc[it][j] = *reinterpret_cast<const float*>(word_ptr(&s_view, meta[it][j], ch.first));
+        for (uint32_t ob = o_begin; ob < ch.nocc; ob += per_round) {
+            const uint32_t lim = min(per_round, ch.nocc - ob);
+            const uint32_t tbl = ob == o_begin ? tbl_first : (lane < lim ? __ldg(occ_off128 + ch.occ0 + ob + lane) : 0u);
+            for (uint32_t u = 0; u < lim; ++u) {
+                const char* src = slice + (uint64_t)__shfl_sync(0xFFFFFFFFu, tbl, u) * 128;
+                unsigned char* dst = ring + u * slot_bytes + 16 * lane;
+                for (uint32_t v = lane; v < nvec; v += 32, src += 512, dst += 512) cp_async<16>(dst, src);
             }
-        for (uint32_t ob = kLastOnly ? ch.nocc - 1 : 0; ob < ch.nocc; ob += 32) {
-            const uint32_t lim = min(32u, ch.nocc - ob);
-            const uint32_t tbl = lane < lim ? occ_off128[ch.occ0 + ob + lane] : 0;
-            for (uint32_t u0 = 0; u0 < lim; u0 += UNR) {
-                uint4 r[UNR][NIT];
+            if (ob == o_begin && cc + cc_step < n_cell_chunks) {   // next chunk's tables, while this chunk's slices are in flight
+                ch_next = cell_chunks[cc + cc_step];
+                tbl_next = first_table(ch_next);
+            }
+            cp_async_wait_all();
+            __syncwarp();
+            if (single) {
+                reduce_group(acc, 0, R, lim);
+            } else {
+                for (uint32_t g0 = 0; g0 < R; g0 += GW) {
+                    const uint32_t nw = min((uint32_t)GW, R - g0);
+                    float a2[GW];
 #pragma unroll
-                for (int u = 0; u < UNR; ++u) {
-                    const uint32_t o128 = __shfl_sync(0xFFFFFFFFu, tbl, (u0 + u) & 31);
-                    if (u0 + u < lim) {
+                    for (int j = 0; j < GW; ++j) a2[j] = (uint32_t)j < nw ? scratch[(g0 + j) * 32 + lane] : 0.f;
+                    reduce_group(a2, g0, nw, lim);
 #pragma unroll
-                        for (int it = 0; it < NIT; ++it)
-                            if (lane + 32 * it < nvec) r[u][it] = ld_once16(slice + (uint64_t)o128 * 128 + 512 * it);
-                    }
+                    for (int j = 0; j < GW; ++j) if ((uint32_t)j < nw) scratch[(g0 + j) * 32 + lane] = a2[j];
                 }
+            }
+            __syncwarp();     // the ring is refilled by the next round / the next chunk
+        }
+
+        if (!live) continue;
+        if (single) {
 #pragma unroll
-                for (int u = 0; u < UNR; ++u) {
-                    if (u0 + u < lim) {
-#pragma unroll
-                        for (int it = 0; it < NIT; ++it) {
-                            const float rv[4] = {__uint_as_float(r[u][it].x), __uint_as_float(r[u][it].y), __uint_as_float(r[u][it].z),
-                                                 __uint_as_float(r[u][it].w)};
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) {
-                                const float s = __fadd_rn(acc[it][j], rv[j]), m = fmaxf(acc[it][j], rv[j]);
-                                acc[it][j] = kind[it][j] == W_SUM ? s : (kind[it][j] == W_MAX ? m : rv[j]);
-                            }
-                        }
-                    }
+            for (int j = 0; j < GW; ++j) {
+                if ((uint32_t)j >= R) continue;
+                const int j4 = 4 * (j / 4);
+                if (j4 + 3 < GW && prog.vec4[j4]) {
+                    if (j == j4) *reinterpret_cast<float4*>(word_addr(j, p)) = make_float4(acc[j4], acc[j4 + 1 < GW ? j4 + 1 : j4], acc[j4 + 2 < GW ? j4 + 2 : j4], acc[j4 + 3 < GW ? j4 + 3 : j4]);
+                } else if (prog.word[j].kind == W_ASSIGN_BYTE) {
+                    *reinterpret_cast<unsigned char*>(word_addr(j, p)) = (unsigned char)__float_as_uint(acc[j]);
+                } else {
+                    *reinterpret_cast<float*>(word_addr(j, p)) = acc[j];
                 }
+            }
+        } else {
+            for (uint32_t w = 0; w < R; ++w) {
+                const float v = scratch[w * 32 + lane];
+                if (prog.word[w].kind == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(word_addr(w, p)) = (unsigned char)__float_as_uint(v);
+                else *reinterpret_cast<float*>(word_addr(w, p)) = v;
             }
         }
-#pragma unroll
-        for (int it = 0; it < NIT; ++it)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (kind[it][j] == W_SKIP) continue;
-                char* dst = word_ptr(&s_view, meta[it][j], ch.first);
-                if (kind[it][j] == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(dst) = (unsigned char)__float_as_uint(acc[it][j]);
-                else *reinterpret_cast<float*>(dst) = acc[it][j];
-            }
     }
 }
 
@@ -301,13 +375,26 @@ int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t*
     return SPH_OK;
 }
 
-template <int NIT>
-void launch_unpack_nit(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                       bool last_only, uint32_t grid, cudaStream_t st) {
-    if (last_only)
-        unpack_kernel<NIT, true><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf);
-    else
-        unpack_kernel<NIT, false><<<grid, kUnpackWarps * 32, 0, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf);
+constexpr uint32_t kUnpackRingBytes = 17408;   // per warp: 27 slices of 32 x 20-byte records fit (a cell of a periodic grid occurs 27 times)
+
+template <int VEC, int GW>
+int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
+                        bool last_only, bool all_sum, int sms, cudaStream_t st) {
+    const uint32_t slot_bytes = 128 * prog.rec_words;
+    const uint32_t extra = prog.rec_words <= (uint32_t)GW ? 0 : 1;      // scratch slot of a long record
+    const uint32_t slots = last_only ? 1u : std::max(1u, std::min(std::min(32u, b->max_nocc), kUnpackRingBytes / slot_bytes));
+    const size_t smem = (size_t)kUnpackWarps * (slots + extra) * slot_bytes;
+    static size_t configured = 0;
+    if (smem > 48 * 1024 && smem > configured) {
+        SPH_CUDA_TRY(cudaFuncSetAttribute(unpack_kernel<VEC, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(16, (227 * 1024) / (smem + 1024)));
+    const uint32_t want = (b->n_cell_chunks + kUnpackWarps - 1) / kUnpackWarps;
+    const uint32_t grid = std::min(want, (uint32_t)sms * per_sm);
+    unpack_kernel<VEC, GW><<<grid, kUnpackWarps * 32, smem, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf, slots,
+                                                                   last_only ? 1u : 0u, all_sum ? 1u : 0u);
+    return SPH_OK;
 }
 
 }  // namespace
@@ -338,15 +425,16 @@ int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& 
     if (b->n_cell_chunks == 0) return SPH_OK;
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
-    const uint32_t want = (b->n_cell_chunks + kUnpackWarps - 1) / kUnpackWarps;
-    const uint32_t grid = min(want, (uint32_t)sms * 16);
-    const uint32_t nit = (prog.rec_words + 3) / 4;
-    if (nit <= 1) launch_unpack_nit<1>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
-    else if (nit <= 2) launch_unpack_nit<2>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
-    else if (nit <= 4) launch_unpack_nit<4>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
-    else if (nit <= 6) launch_unpack_nit<6>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
-    else if (nit <= 9) launch_unpack_nit<9>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
-    else launch_unpack_nit<12>(view, b, prog, d_occ_off128, d_buf, last_only, grid, st);
+    bool all_sum = true;
+    for (uint32_t w = 0; w < prog.rec_words; ++w) all_sum &= prog.word[w].kind == W_SUM;
+    const uint32_t R = prog.rec_words;
+    int32_t rc;
+    if (R % 4 == 0) rc = R % 8 == 0 ? launch_unpack_t<4, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st)
+                                    : launch_unpack_t<4, 4>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
+    else if (R % 2 == 0) rc = launch_unpack_t<2, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
+    else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
+    else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
+    if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
