@@ -93,7 +93,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
             SideRec sr{(uint32_t)ce.first, ce.count, (uint32_t)chunk_side.size(), c};
             const uint32_t sidx = (uint32_t)b->sides.size();
             const uint32_t partner = tk.cj >= 0 ? (side == 0 ? sidx + 1 : sidx - 1) : sidx;
-            for (uint32_t k = 0; k < ce.count; k += 32) { chunk_side.push_back(sidx); chunk_src.push_back(partner); }
+            for (uint32_t k = 0; k < ce.count; k += kLoopTargets) { chunk_side.push_back(sidx); chunk_src.push_back(partner); }
             b->sides.push_back(sr);
             const double* fr = side == 0 ? tk.frame_i : tk.frame_j;
             frames.insert(frames.end(), fr, fr + 3);
@@ -129,28 +129,24 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     b->n_cell_chunks = (uint32_t)cell_chunks.size();
     b->n_occ = b->n_sides;
 
-    int32_t rc = upload(b->sides, &b->d_sides);
-    if (!rc) rc = upload(frames, &b->d_frames);
-    if (!rc) rc = upload(chunk_side, &b->d_chunk_side);
-    if (!rc) rc = upload(b->task_side0, &b->d_task_side0);
-    if (!rc) rc = upload(chunk_src, &b->d_chunk_src);
-    if (!rc) rc = upload(cell_chunks, &b->d_cell_chunks);
+    int32_t rc = upload(cell_chunks, &b->d_cell_chunks);
     std::vector<double> occ_frames(3 * (size_t)b->n_sides);
     for (uint32_t o = 0; o < b->n_sides; ++o) std::copy_n(&frames[3 * (size_t)occ_side[o]], 3, &occ_frames[3 * (size_t)o]);
     if (!rc) rc = upload(occ_frames, &b->d_occ_frames);
     for (uint32_t rec : {16u, 20u, 52u})
         if (!rc) rc = ensure_offsets(b, rec, nullptr);
     // loop work items (one per 32-particle target chunk), for the canonical record sizes of the two loops
-    if (!rc && b->max_count >= (1u << 26)) rc = fail(SPH_ERR_RANGE, "a cell of %u particles is too large for the loop item table", b->max_count);
+    if (!rc && b->max_count >= (1u << 25)) rc = fail(SPH_ERR_RANGE, "a cell of %u particles is too large for the loop item table", b->max_count);
     if (!rc) {
         const std::vector<uint64_t>&o16 = find_offsets(b, 16)->h_off, &o20 = find_offsets(b, 20)->h_off, &o52 = find_offsets(b, 52)->h_off;
         std::vector<LoopItem> dens(b->n_chunks), forc(b->n_chunks);
         for (uint32_t ch = 0; ch < b->n_chunks; ++ch) {
             const uint32_t tgt = chunk_side[ch], src = chunk_src[ch];
             const uint32_t kc = ch - b->sides[tgt].chunk0;                       // chunk index inside the block
-            const uint32_t nt_ns = std::min(32u, b->sides[tgt].count - 32 * kc) | b->sides[src].count << 6;
-            dens[ch] = LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4, nt_ns};
-            forc[ch] = LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5, nt_ns};
+            const uint32_t nt_ns = std::min(kLoopTargets, b->sides[tgt].count - kLoopTargets * kc) | b->sides[src].count << 7;
+            const uint32_t u = kLoopTargets / 32;                                // 32 records of r bytes = r units of 128 bytes
+            dens[ch] = LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5 * u, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns};
+            forc[ch] = LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13 * u, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns};
         }
         rc = upload(dens, &b->d_items_density);
         if (!rc) rc = upload(forc, &b->d_items_force);
@@ -162,8 +158,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
-    cudaFree(b->d_sides); cudaFree(b->d_frames); cudaFree(b->d_chunk_side); cudaFree(b->d_task_side0);
-    cudaFree(b->d_chunk_src); cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
+    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;

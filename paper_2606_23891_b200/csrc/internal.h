@@ -40,7 +40,7 @@ struct StoreView {
 struct SideRec {
     uint32_t first;    // first particle of the cell
     uint32_t count;    // particles in the cell
-    uint32_t chunk0;   // index of the block's first 32-particle chunk in the pack chunk table
+    uint32_t chunk0;   // index of the block's first 64-target chunk in the loop item tables
     uint32_t cell;
 };
 
@@ -53,13 +53,14 @@ struct CellChunk {
     uint32_t nocc;
 };
 
-// work item of the density / force loops: 32 targets of one block against the block they gather from.
+// work item of the density / force loops: up to 64 targets of one block (two per lane) against the block they gather from.
 // Offsets in units of 128 bytes into the loop's input / output buffer (chunk starts are multiples of 128 bytes).
+constexpr uint32_t kLoopTargets = 64;
 struct LoopItem {
     uint32_t tin128;     // the targets' input records
     uint32_t sin128;     // first input record of the source block
     uint32_t tout128;    // the targets' result records
-    uint32_t nt_ns;      // targets (1..32) | sources << 6
+    uint32_t nt_ns;      // targets (1..64) | sources << 7
 };
 
 // word kinds of the pack / unpack programs
@@ -137,14 +138,9 @@ struct sph_batch {
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists
     std::vector<uint32_t> task_side0;         // n_tasks + 1
     // device tables
-    sph::SideRec* d_sides = nullptr;
-    double* d_frames = nullptr;               // 3 per side
     double* d_occ_frames = nullptr;           // 3 per occurrence (cell-major, ascending side): the frame of that side
-    uint32_t* d_chunk_side = nullptr;         // pack chunk -> side
-    uint32_t* d_task_side0 = nullptr;         // task -> first side (n_tasks + 1 entries)
-    uint32_t* d_chunk_src = nullptr;          // pack chunk -> the side its targets gather from (partner side; itself for self tasks)
     sph::CellChunk* d_cell_chunks = nullptr;
-    sph::LoopItem* d_items_density = nullptr; // one per 32-particle target chunk (20-byte in, 16-byte out records)
+    sph::LoopItem* d_items_density = nullptr; // one per 64-target chunk of a block (20-byte in, 16-byte out records)
     sph::LoopItem* d_items_force = nullptr;   // (52-byte in, 20-byte out records)
     std::map<uint32_t, sph::OffsetTable> offsets;   // by record bytes
 };
