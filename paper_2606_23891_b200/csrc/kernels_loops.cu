@@ -133,26 +133,26 @@ __device__ __forceinline__ FilterTarget filter_target(float x, float y, float z,
     return FilterTarget{dup2(-2.0f * x), dup2(-2.0f * y), dup2(-2.0f * z), dup2(nt)};
 }
 
-// Phase 1 over the first `cnt` tile entries for the lane's two targets: bit (31 - j) of m[0] = "source j may be a
-// neighbour of target A" (j < 32), m[1] likewise for sources 32..63; m[2], m[3] for target B.
-__device__ __forceinline__ void filter_masks(FilterTile& f, uint32_t cnt, uint32_t lane, const FilterTarget& A, const FilterTarget& B, uint32_t (&m)[4]) {
-    const uint32_t n4 = (cnt + 3) & ~3u;
-    if (lane < n4 - cnt) filter_put(f, cnt + lane, 0.f, 0.f, 0.f, kNever);
-    __syncwarp();
-    const uint32_t np = n4 >> 1, np0 = min(np, 16u);
+// Phase 1 over the first `cnt` tile entries for the lane's targets: bit (31 - j) of m[0] = "source j may be a
+// neighbour of target A" (j < 32), m[1] likewise for sources 32..63; m[2], m[3] for target B (DUAL only).
+template <bool DUAL>
+__device__ __forceinline__ void filter_masks(const FilterTile& f, uint32_t cnt, const FilterTarget& A, const FilterTarget& B, uint32_t (&m)[4]) {
+    const uint32_t np = ((cnt + 3) & ~3u) >> 1, np0 = min(np, 16u);
     uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
     auto test2 = [&](uint32_t p, uint32_t& ma, uint32_t& mb) {
         const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(&f.a[p]);
         const ulonglong2 b = *reinterpret_cast<const ulonglong2*>(&f.b[p]);
         const u64 ta = fma2(A.mx2, a.x, fma2(A.my2, a.y, fma2(A.mz2, b.x, add2(b.y, A.nt2))));
-        const u64 tb = fma2(B.mx2, a.x, fma2(B.my2, a.y, fma2(B.mz2, b.x, add2(b.y, B.nt2))));
         uint32_t lo, hi;
         asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(ta));
         ma = __funnelshift_l(lo, ma, 1);      // (m << 1) | sign(t_lo)
         ma = __funnelshift_l(hi, ma, 1);
-        asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(tb));
-        mb = __funnelshift_l(lo, mb, 1);
-        mb = __funnelshift_l(hi, mb, 1);
+        if constexpr (DUAL) {
+            const u64 tb = fma2(B.mx2, a.x, fma2(B.my2, a.y, fma2(B.mz2, b.x, add2(b.y, B.nt2))));
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(tb));
+            mb = __funnelshift_l(lo, mb, 1);
+            mb = __funnelshift_l(hi, mb, 1);
+        }
     };
     for (uint32_t p = 0; p < np0; p += 2) { test2(p, a0, b0); test2(p + 1, a0, b0); }
     a0 <<= 32 - 2 * np0; b0 <<= 32 - 2 * np0;
@@ -163,16 +163,55 @@ __device__ __forceinline__ void filter_masks(FilterTile& f, uint32_t cnt, uint32
     m[0] = a0; m[1] = a1; m[2] = b0; m[3] = b1;
 }
 
-// next hit of each of the two targets in one half of the tile (32 = the dummy when a target has none left)
-__device__ __forceinline__ void next_hits(uint32_t& ma, uint32_t& mb, uint32_t* ja, uint32_t* jb) {
-    *ja = __clz(ma); *jb = __clz(mb);
-    ma &= ~shr_clamp(0x80000000u, *ja);
-    mb &= ~shr_clamp(0x80000000u, *jb);
+// pads the filter tile to a multiple of four entries and returns the bounding box of its first cnt sources
+struct Box { float lox, hix, loy, hiy, loz, hiz; };
+__device__ __forceinline__ Box tile_box(FilterTile& f, uint32_t cnt, uint32_t lane) {
+    const uint32_t n4 = (cnt + 3) & ~3u;
+    if (lane < n4 - cnt) filter_put(f, cnt + lane, 0.f, 0.f, 0.f, kNever);
+    __syncwarp();
+    // entries lane and lane + 32 of the tile
+    const float* a = reinterpret_cast<const float*>(&f.a[lane >> 1]) + (lane & 1);
+    const float* b = reinterpret_cast<const float*>(&f.b[lane >> 1]) + (lane & 1);
+    const bool v0 = lane < cnt, v1 = lane + 32 < cnt;
+    const float x0 = a[0], y0 = a[2], z0 = b[0];
+    const float x1 = v1 ? a[64] : x0, y1 = v1 ? a[66] : y0, z1 = v1 ? b[64] : z0;      // + 16 float4 = + 64 floats
+    Box bx;
+    bx.lox = warp_min(fminf(x0, x1), v0); bx.hix = warp_max(fmaxf(x0, x1), v0);
+    bx.loy = warp_min(fminf(y0, y1), v0); bx.hiy = warp_max(fmaxf(y0, y1), v0);
+    bx.loz = warp_min(fminf(z0, z1), v0); bx.hiz = warp_max(fmaxf(z0, z1), v0);
+    return bx;
+}
+// squared distance from a point to a box
+__device__ __forceinline__ float box_dist2(const Box& b, float x, float y, float z) {
+    const float dx = fmaxf(fmaxf(b.lox - x, x - b.hix), 0.f), dy = fmaxf(fmaxf(b.loy - y, y - b.hiy), 0.f), dz = fmaxf(fmaxf(b.loz - z, z - b.hiz), 0.f);
+    return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
 }
 
-// the lane's two targets as a pair: value of A in the low half, of B in the high half
-__device__ __forceinline__ u64 load2(const float* rec, uint32_t stride, uint32_t word, uint32_t lane, bool vA, bool vB, float idle) {
-    return pack2(vA ? rec[stride * lane + word] : idle, vB ? rec[stride * (lane + 32) + word] : idle);
+// the next two hits of a pass: of targets A and B (dual), or the next two of target A (single); 32 = the dummy
+__device__ __forceinline__ bool next_hits(bool dual, uint32_t& ma, uint32_t& mb, uint32_t* ja, uint32_t* jb) {
+    if (dual) {
+        if ((ma | mb) == 0) return false;
+        *ja = __clz(ma); *jb = __clz(mb);
+        ma &= ~shr_clamp(0x80000000u, *ja);
+        mb &= ~shr_clamp(0x80000000u, *jb);
+    } else {
+        if (ma == 0) return false;
+        *ja = __clz(ma);
+        ma &= ~shr_clamp(0x80000000u, *ja);
+        *jb = __clz(ma);
+        ma &= ~shr_clamp(0x80000000u, *jb);
+    }
+    return true;
+}
+
+// Which of the item's targets can have a neighbour in the tile: the active ones are numbered through (A targets
+// first, lane order) into sm_act; returns their count.  aA / aB: is the lane's own target lane / lane + 32 active.
+__device__ __forceinline__ uint32_t compact_targets(uint32_t* sm_act, bool aA, bool aB, uint32_t lane, uint32_t lt) {
+    const uint32_t bA = __ballot_sync(kFull, aA), bB = __ballot_sync(kFull, aB), nA = __popc(bA);
+    if (aA) sm_act[__popc(bA & lt)] = lane;
+    if (aB) sm_act[nA + __popc(bB & lt)] = lane + 32;
+    __syncwarp();
+    return nA + __popc(bB);
 }
 
 // ------------------------------------------------------------------------------------------------- density
@@ -180,11 +219,14 @@ __device__ __forceinline__ u64 load2(const float* rec, uint32_t stride, uint32_t
 struct DensityWarpSmem {
     FilterTile f;
     float4 tile[2 * kHalf];  // x, y, z, m of the compacted sources; entries 32 and 65 are the dummy
-    float tgt[64 * 5];       // landing area of an item's 64 DENSITY_IN records: xr0 xr1 xr2 h m
+    float4 tgt[64];          // the item's targets: x, y, z, h
+    float4 acc[64];          // their running sums: m w, m (3w + q w'), w, (3w + q w')
+    float raw[64 * 5];       // landing area of an item's 64 DENSITY_IN records: xr0 xr1 xr2 h m
     float src[2][32 * 5];    // landing areas of the source rounds (double-buffered)
+    uint32_t act[64];        // the active targets of the flush
 };
 
-__global__ void __launch_bounds__(kLoopWarps * 32)
+__global__ void __launch_bounds__(kLoopWarps * 32, 5)
 density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items) {
     __shared__ __align__(16) DensityWarpSmem s_all[kLoopWarps];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -197,7 +239,7 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
     const u64 kTwo = dup2(2.0f), kThree = dup2(3.0f), kQuarter = dup2(0.25f), kM075 = dup2(-0.75f);
 
     uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
-    fetch_records<5, 64>(sm.tgt, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
+    fetch_records<5, 64>(sm.raw, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
     fetch_records<5, 32>(sm.src[0], in + (uint64_t)iw.y * 128, min(32u, iw.w >> 7), lane);
     uint32_t buf = 0;
 
@@ -210,52 +252,73 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
         if (has_next) iw_next = __ldg(reinterpret_cast<const uint4*>(items) + item + step);
         cp_async_wait_all();          // this item's targets and first source round
         __syncwarp();
+        // the lane's own two targets (lane, lane + 32): table entries, zeroed sums, reach box of the whole item
         const bool vA = lane < n_t, vB = lane + 32 < n_t;
-        const u64 x2 = load2(sm.tgt, 5, 0, lane, vA, vB, 0.f), y2 = load2(sm.tgt, 5, 1, lane, vA, vB, 0.f), z2 = load2(sm.tgt, 5, 2, lane, vA, vB, 0.f);
-        float xA, xB, yA, yB, zA, zB;
-        unpack2(x2, xA, xB); unpack2(y2, yA, yB); unpack2(z2, zA, zB);
-        const float hA = vA ? sm.tgt[5 * lane + 3] : 0.f, hB = vB ? sm.tgt[5 * (lane + 32) + 3] : 0.f;
-        __syncwarp();                 // sm.tgt may now receive the next item's targets
-        const float inv_hA = vA ? 1.0f / hA : 0.f, inv_hB = vB ? 1.0f / hB : 0.f;
-        const float reach = 2.0f * warp_max_pos(fmaxf(hA, hB)) * kReachSlack;
-        const float lox = warp_min(vB ? fminf(xA, xB) : xA, vA) - reach, hix = warp_max(vB ? fmaxf(xA, xB) : xA, vA) + reach;
-        const float loy = warp_min(vB ? fminf(yA, yB) : yA, vA) - reach, hiy = warp_max(vB ? fmaxf(yA, yB) : yA, vA) + reach;
-        const float loz = warp_min(vB ? fminf(zA, zB) : zA, vA) - reach, hiz = warp_max(vB ? fmaxf(zA, zB) : zA, vA) + reach;
+        float4 oA = make_float4(0.f, 0.f, 0.f, 0.f), oB = oA;
+        if (vA) { const float* r = sm.raw + 5 * lane; oA = make_float4(r[0], r[1], r[2], r[3]); }
+        if (vB) { const float* r = sm.raw + 5 * (lane + 32); oB = make_float4(r[0], r[1], r[2], r[3]); }
+        sm.tgt[lane] = oA; sm.tgt[lane + 32] = oB;
+        sm.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f); sm.acc[lane + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncwarp();                 // sm.raw may now receive the next item's targets
+        const float reach = 2.0f * warp_max_pos(fmaxf(oA.w, oB.w)) * kReachSlack;
+        const float lox = warp_min(vB ? fminf(oA.x, oB.x) : oA.x, vA) - reach, hix = warp_max(vB ? fmaxf(oA.x, oB.x) : oA.x, vA) + reach;
+        const float loy = warp_min(vB ? fminf(oA.y, oB.y) : oA.y, vA) - reach, hiy = warp_max(vB ? fmaxf(oA.y, oB.y) : oA.y, vA) + reach;
+        const float loz = warp_min(vB ? fminf(oA.z, oB.z) : oA.z, vA) - reach, hiz = warp_max(vB ? fmaxf(oA.z, oB.z) : oA.z, vA) + reach;
         const float bx = fmaxf(fabsf(lox), fabsf(hix)), by = fmaxf(fabsf(loy), fabsf(hiy)), bz = fmaxf(fabsf(loz), fabsf(hiz));
         const float eps = kFilterEps * fmaf(bx, bx, fmaf(by, by, bz * bz));
-        const FilterTarget fA = filter_target(xA, yA, zA, vA ? fmaf(xA, xA, fmaf(yA, yA, zA * zA)) - 4.0f * hA * hA - eps : kNever);
-        const FilterTarget fB = filter_target(xB, yB, zB, vB ? fmaf(xB, xB, fmaf(yB, yB, zB * zB)) - 4.0f * hB * hB - eps : kNever);
-        u64 s_mw = 0, s_mg = 0, s_w = 0, s_g = 0;     // sums of m w, m (3w + q w'), w, (3w + q w') for (A, B)
+        const float cutA = 4.0f * oA.w * oA.w, cutB = 4.0f * oB.w * oB.w;
 
-        // phase 2 over one half of the tile
-        auto hits = [&](uint32_t ma, uint32_t mb, const float4* half) {
-            while ((ma | mb) != 0) {
-                uint32_t ja, jb;
-                next_hits(ma, mb, &ja, &jb);
-                const float4 a = half[ja], b = half[jb];
-                const u64 dx = sub2(x2, pack2(a.x, b.x)), dy = sub2(y2, pack2(a.y, b.y)), dz = sub2(z2, pack2(a.z, b.z));
-                const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-                float r2a, r2b;
-                unpack2(r2, r2a, r2b);
-                // a filter false positive has r2 >= (2h)^2: q clamps to 2 where w = w' = 0 exactly (and so does the dummy)
-                const float qa = fminf(sqrt_approx(r2a) * inv_hA, 2.0f), qb = fminf(sqrt_approx(r2b) * inv_hB, 2.0f);
-                const u64 q = pack2(qa, qb), u = pack2(fminf(qa - 1.0f, 0.f), fminf(qb - 1.0f, 0.f));   // u = -(1 - q)+
-                const u64 t = sub2(kTwo, q);                                                                // t = (2 - q)+
-                const u64 tt = mul2(t, t), uu = mul2(u, u);
-                const u64 w = fma2(mul2(kQuarter, t), tt, mul2(u, uu));      // 0.25 t^3 - (1 - q)+^3
-                const u64 dw = fma2(kThree, uu, mul2(kM075, tt));            // -0.75 t^2 + 3 (1 - q)+^2
-                const u64 g = fma2(q, dw, mul2(kThree, w));
-                const u64 m = pack2(a.w, b.w);
-                s_mw = fma2(m, w, s_mw); s_mg = fma2(m, g, s_mg);
-                s_w = add2(s_w, w); s_g = add2(s_g, g);
-            }
-        };
         auto flush = [&](uint32_t cnt) {
+            // targets that can reach the tile's bounding box get a lane (or half of one); the others sit this flush out
+            const Box box = tile_box(sm.f, cnt, lane);
+            const bool aA = vA && box_dist2(box, oA.x, oA.y, oA.z) < cutA * kReachSlack, aB = vB && box_dist2(box, oB.x, oB.y, oB.z) < cutB * kReachSlack;
+            const uint32_t n_act = compact_targets(sm.act, aA, aB, lane, lt);
+            if (n_act == 0) return;
+            const bool dual = n_act > 32;                // else: one target per lane, two of its hits per iteration
+            const bool wA = lane < n_act, wB = dual && lane + 32 < n_act;
+            const uint32_t tA = wA ? sm.act[lane] : 0, tB = wB ? sm.act[lane + 32] : tA;
+            const float4 pA = sm.tgt[tA], pB = sm.tgt[tB];
+            const float inv_hA = wA ? 1.0f / pA.w : 0.f, inv_hB = dual ? (wB ? 1.0f / pB.w : 0.f) : inv_hA;
+            const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - 4.0f * pA.w * pA.w - eps : kNever);
+            const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - 4.0f * pB.w * pB.w - eps : kNever);
             uint32_t m[4];
-            filter_masks(sm.f, cnt, lane, fA, fB, m);
+            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
+            u64 s_mw = 0, s_mg = 0, s_w = 0, s_g = 0;
+            // phase 2 over one half of the tile
+            auto hits = [&](uint32_t ma, uint32_t mb, const float4* half) {
+                uint32_t ja, jb;
+                while (next_hits(dual, ma, mb, &ja, &jb)) {
+                    const float4 a = half[ja], b = half[jb];
+                    const u64 dx = sub2(x2, pack2(a.x, b.x)), dy = sub2(y2, pack2(a.y, b.y)), dz = sub2(z2, pack2(a.z, b.z));
+                    const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                    float r2a, r2b;
+                    unpack2(r2, r2a, r2b);
+                    // a filter false positive has r2 >= (2h)^2: q clamps to 2 where w = w' = 0 exactly (and so does the dummy)
+                    const float qa = fminf(sqrt_approx(r2a) * inv_hA, 2.0f), qb = fminf(sqrt_approx(r2b) * inv_hB, 2.0f);
+                    const u64 q = pack2(qa, qb), u = pack2(fminf(qa - 1.0f, 0.f), fminf(qb - 1.0f, 0.f));   // u = -(1 - q)+
+                    const u64 t = sub2(kTwo, q);                                                                // t = (2 - q)+
+                    const u64 tt = mul2(t, t), uu = mul2(u, u);
+                    const u64 w = fma2(mul2(kQuarter, t), tt, mul2(u, uu));      // 0.25 t^3 - (1 - q)+^3
+                    const u64 dw = fma2(kThree, uu, mul2(kM075, tt));            // -0.75 t^2 + 3 (1 - q)+^2
+                    const u64 g = fma2(q, dw, mul2(kThree, w));
+                    const u64 mm = pack2(a.w, b.w);
+                    s_mw = fma2(mm, w, s_mw); s_mg = fma2(mm, g, s_mg);
+                    s_w = add2(s_w, w); s_g = add2(s_g, g);
+                }
+            };
             hits(m[0], m[2], sm.tile);
             if (cnt > 32) hits(m[1], m[3], sm.tile + kHalf);
-            __syncwarp();
+            float mw0, mw1, mg0, mg1, w0, w1, g0, g1;
+            unpack2(s_mw, mw0, mw1); unpack2(s_mg, mg0, mg1); unpack2(s_w, w0, w1); unpack2(s_g, g0, g1);
+            if (dual) {
+                if (wA) { float4 c = sm.acc[tA]; c.x += mw0; c.y += mg0; c.z += w0; c.w += g0; sm.acc[tA] = c; }
+                if (wB) { float4 c = sm.acc[tB]; c.x += mw1; c.y += mg1; c.z += w1; c.w += g1; sm.acc[tB] = c; }
+            } else if (wA) {
+                float4 c = sm.acc[tA];
+                c.x += mw0 + mw1; c.y += mg0 + mg1; c.z += w0 + w1; c.w += g0 + g1;
+                sm.acc[tA] = c;
+            }
         };
 
         uint32_t cnt = 0;
@@ -267,7 +330,7 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
             if (r + 1 < n_rounds) {
                 fetch_records<5, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 20, min(32u, n_s - j0 - 32), lane);
             } else if (has_next) {
-                fetch_records<5, 64>(sm.tgt, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+                fetch_records<5, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
                 fetch_records<5, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
             }
             float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -278,7 +341,7 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
                 ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
             }
             const uint32_t ball = __ballot_sync(kFull, ok), c = __popc(ball);
-            if (cnt + c > kTile) { flush(cnt); cnt = 0; }
+            if (cnt + c > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
             if (ok) {
                 const uint32_t pos = cnt + __popc(ball & lt);
                 sm.tile[pos + (pos >> 5)] = s;        // half * 33 + index in the half
@@ -288,16 +351,18 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
             buf ^= 1;
         }
         if (cnt) flush(cnt);
-        float mwA, mwB, mgA, mgB, wA, wB, gA, gB;
-        unpack2(s_mw, mwA, mwB); unpack2(s_mg, mgA, mgB); unpack2(s_w, wA, wB); unpack2(s_g, gA, gB);
+        __syncwarp();
         if (vA) {
-            const float n3 = kInvPi * inv_hA * inv_hA * inv_hA, n4 = n3 * inv_hA;
-            reinterpret_cast<float4*>(tout)[lane] = make_float4(mwA * n3, -mgA * n4, wA * n3, -gA * n4);
+            const float ih = 1.0f / oA.w, n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
+            const float4 c = sm.acc[lane];
+            reinterpret_cast<float4*>(tout)[lane] = make_float4(c.x * n3, -c.y * n4, c.z * n3, -c.w * n4);
         }
         if (vB) {
-            const float n3 = kInvPi * inv_hB * inv_hB * inv_hB, n4 = n3 * inv_hB;
-            reinterpret_cast<float4*>(tout)[lane + 32] = make_float4(mwB * n3, -mgB * n4, wB * n3, -gB * n4);
+            const float ih = 1.0f / oB.w, n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
+            const float4 c = sm.acc[lane + 32];
+            reinterpret_cast<float4*>(tout)[lane + 32] = make_float4(c.x * n3, -c.y * n4, c.z * n3, -c.w * n4);
         }
+        __syncwarp();                 // sm.tgt / sm.acc are rewritten by the next item
         iw = iw_next;
     }
 }
@@ -306,12 +371,16 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
 
 struct ForceWarpSmem {
     FilterTile f;
-    float4 ta[2 * kHalf];    // x, y, z, 4 h^2           (entries 32 and 65: the dummy)
-    float4 tb[2 * kHalf];    // vx, vy, vz, m
-    float4 tc[2 * kHalf];    // rho, A = P / (Omega rho^2), c_s, 1/h
-    float tgt[64 * 13];      // landing area of an item's 64 FORCE_IN records: xr0 xr1 xr2 h m rho rho_dh v0 v1 v2 u P cs
-                             // (and, at the end of the item, of its 64 x 5 results)
+    float4 ta[2 * kHalf];    // sources: x, y, z, 4 h^2           (entries 32 and 65: the dummy)
+    float4 tb[2 * kHalf];    //          vx, vy, vz, m
+    float4 tc[2 * kHalf];    //          rho, A = P / (Omega rho^2), c_s, 1/h
+    float4 t0[64];           // targets: x, y, z, 4 h^2
+    float4 t1[64];           //          vx, vy, vz, c_s
+    float4 t2[64];           //          1/h, 1/(pi h^4), rho, A
+    float raw[64 * 13];      // landing area of an item's 64 FORCE_IN records: xr0 xr1 xr2 h m rho rho_dh v0 v1 v2 u P cs;
+                             // once the target table is built: the 64 x 5 running results, in FORCE_OUT record layout
     float src[2][32 * 13];   // landing areas of the source rounds (double-buffered)
+    uint32_t act[64];        // the active targets of the flush
 };
 
 // -0.75 (2 - q)+^2 + 3 (1 - q)+^2 = w'(q) of the cubic spline for a pair of q
@@ -323,7 +392,7 @@ __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree,
     return fma2(kThree, mul2(u, u), mul2(kM075, mul2(t, t)));
 }
 
-__global__ void __launch_bounds__(kLoopWarps * 32)
+__global__ void __launch_bounds__(kLoopWarps * 32, 4)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -341,7 +410,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
               kOneHalf2 = dup2(1.5f), kInvPi2 = dup2(kInvPi), kMBeta2 = dup2(-beta), kMAlpha2 = dup2(-alpha);
 
     uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
-    fetch_records<13, 64>(sm.tgt, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
+    fetch_records<13, 64>(sm.raw, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
     fetch_records<13, 32>(sm.src[0], in + (uint64_t)iw.y * 128, min(32u, iw.w >> 7), lane);
     uint32_t buf = 0;
 
@@ -354,85 +423,111 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         if (has_next) iw_next = __ldg(reinterpret_cast<const uint4*>(items) + item + step);
         cp_async_wait_all();          // this item's targets and first source round
         __syncwarp();
+        // the lane's own two targets (lane, lane + 32): table entries; bounding box of the whole item
         const bool vA = lane < n_t, vB = lane + 32 < n_t;
-        const u64 x2 = load2(sm.tgt, 13, 0, lane, vA, vB, 0.f), y2 = load2(sm.tgt, 13, 1, lane, vA, vB, 0.f), z2 = load2(sm.tgt, 13, 2, lane, vA, vB, 0.f);
-        const u64 h2 = load2(sm.tgt, 13, 3, lane, vA, vB, 0.f), rho2 = load2(sm.tgt, 13, 5, lane, vA, vB, 1.f), rho_dh2 = load2(sm.tgt, 13, 6, lane, vA, vB, 0.f);
-        const u64 vx2 = load2(sm.tgt, 13, 7, lane, vA, vB, 0.f), vy2 = load2(sm.tgt, 13, 8, lane, vA, vB, 0.f), vz2 = load2(sm.tgt, 13, 9, lane, vA, vB, 0.f);
-        const u64 P2 = load2(sm.tgt, 13, 11, lane, vA, vB, 0.f), c2 = load2(sm.tgt, 13, 12, lane, vA, vB, 0.f);
-        __syncwarp();                 // sm.tgt may now receive the next item's targets (it is parked until the last round)
-        float xA, xB, yA, yB, zA, zB, hA, hB, rhoA, rhoB, rdA, rdB, PA, PB;
-        unpack2(x2, xA, xB); unpack2(y2, yA, yB); unpack2(z2, zA, zB); unpack2(h2, hA, hB);
-        unpack2(rho2, rhoA, rhoB); unpack2(rho_dh2, rdA, rdB); unpack2(P2, PA, PB);
-        const float hc2A = 4.0f * hA * hA, hc2B = 4.0f * hB * hB;
-        const float inv_hA = vA ? 1.0f / hA : 0.f, inv_hB = vB ? 1.0f / hB : 0.f;
-        const u64 inv_h2 = pack2(inv_hA, inv_hB);
-        const u64 n42 = pack2(kInvPi * (inv_hA * inv_hA) * (inv_hA * inv_hA), kInvPi * (inv_hB * inv_hB) * (inv_hB * inv_hB));
-        const u64 A2 = pack2(PA / ((1.0f + hA * rdA / (3.0f * rhoA)) * rhoA * rhoA), PB / ((1.0f + hB * rdB / (3.0f * rhoB)) * rhoB * rhoB));
-        const float reach_t = 2.0f * warp_max_pos(fmaxf(hA, hB));
-        const float lox = warp_min(vB ? fminf(xA, xB) : xA, vA), hix = warp_max(vB ? fmaxf(xA, xB) : xA, vA);
-        const float loy = warp_min(vB ? fminf(yA, yB) : yA, vA), hiy = warp_max(vB ? fmaxf(yA, yB) : yA, vA);
-        const float loz = warp_min(vB ? fminf(zA, zB) : zA, vA), hiz = warp_max(vB ? fmaxf(zA, zB) : zA, vA);
-        const float ri2A = fmaf(xA, xA, fmaf(yA, yA, zA * zA)), ri2B = fmaf(xB, xB, fmaf(yB, yB, zB * zB));
-        const float ri2_max = warp_max_pos(fmaxf(ri2A, ri2B));
-        u64 ax = 0, ay = 0, az = 0, du = 0;
-        float vsigA = 0.f, vsigB = 0.f;
-        float tile_hc2 = 0.f, tile_b2 = 0.f;      // over the tile being filled: largest (2 h_j)^2, largest |s|^2 (warp-uniform)
-
-        // phase 2 over one half of the tile.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j)
-        // is the same number and a_i += -m (..) (x_i - x_j) / r becomes one fma with e.
-        auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
-            while ((ma | mb) != 0) {
-                uint32_t ja, jb;
-                next_hits(ma, mb, &ja, &jb);
-                const float4 a = sm.ta[base + ja], b = sm.ta[base + jb];
-                const u64 ex = sub2(pack2(a.x, b.x), x2), ey = sub2(pack2(a.y, b.y), y2), ez = sub2(pack2(a.z, b.z), z2);
-                const u64 r2 = fma2(ez, ez, fma2(ey, ey, mul2(ex, ex)));
-                float r2a, r2b;
-                unpack2(r2, r2a, r2b);
-                // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
-                // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
-                const bool hitA = r2a < fmaxf(hc2A, a.w) && r2a > 0.f, hitB = r2b < fmaxf(hc2B, b.w) && r2b > 0.f;
-                r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
-                const u64 r2s = pack2(r2a, r2b);
-                u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
-                rinv = mul2(rinv, fma2(mul2(mul2(kMHalf2, r2s), rinv), rinv, kOneHalf2));      // one Newton step: ~1 ulp
-                const u64 r = mul2(r2s, rinv);
-                const float4 va = sm.tb[base + ja], vb = sm.tb[base + jb], ca = sm.tc[base + ja], cb = sm.tc[base + jb];
-                const u64 ihj = pack2(ca.w, cb.w);
-                const u64 Gi = mul2(spline_dw2(mul2(r, inv_h2), kTwo, kOne, kThree, kM075), n42);
-                const u64 ih2 = mul2(ihj, ihj);
-                const u64 Gj = mul2(spline_dw2(mul2(r, ihj), kTwo, kOne, kThree, kM075), mul2(mul2(ih2, ih2), kInvPi2));
-                const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
-                const u64 vr = mul2(fma2(wz, ez, fma2(wy, ey, mul2(wx, ex))), rinv);
-                float vra, vrb;
-                unpack2(vr, vra, vrb);
-                const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
-                const u64 vs = fma2(kMBeta2, mu, add2(c2, pack2(ca.z, cb.z)));
-                float rsa, rsb, vsa, vsb;
-                unpack2(add2(rho2, pack2(ca.x, cb.x)), rsa, rsb);
-                unpack2(vs, vsa, vsb);
-                const u64 visc = mul2(mul2(mul2(kMAlpha2, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
-                const u64 vG = mul2(mul2(visc, kHalf2), add2(Gi, Gj));
-                const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
-                const u64 m = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
-                const u64 fr = mul2(mul2(m, add2(add2(AG, BG), vG)), rinv);
-                ax = fma2(fr, ex, ax); ay = fma2(fr, ey, ay); az = fma2(fr, ez, az);
-                du = fma2(mul2(m, fma2(kHalf2, vG, AG)), vr, du);
-                vsigA = fmaxf(vsigA, hitA ? vsa : 0.f); vsigB = fmaxf(vsigB, hitB ? vsb : 0.f);
+        float4 oA = make_float4(0.f, 0.f, 0.f, 0.f), oB = oA;      // x, y, z, 4 h^2
+        float hA = 0.f, hB = 0.f;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const uint32_t t = lane + 32 * k;
+            float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0, p2 = make_float4(0.f, 0.f, 1.f, 0.f);
+            if (t < n_t) {
+                const float* r = sm.raw + 13 * t;
+                const float h = r[3], rho = r[5], ih = 1.0f / h;
+                p0 = make_float4(r[0], r[1], r[2], 4.0f * h * h);
+                p1 = make_float4(r[7], r[8], r[9], r[12]);
+                p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11] / ((1.0f + h * r[6] / (3.0f * rho)) * rho * rho));
+                if (k == 0) hA = h; else hB = h;
             }
-        };
+            sm.t0[t] = p0; sm.t1[t] = p1; sm.t2[t] = p2;
+            if (k == 0) oA = p0; else oB = p0;
+        }
+        __syncwarp();                 // every lane has read its records: sm.raw becomes the result area
+        for (uint32_t v = lane; v < 80; v += 32) reinterpret_cast<float4*>(sm.raw)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float reach_t = 2.0f * warp_max_pos(fmaxf(hA, hB));
+        const float lox = warp_min(vB ? fminf(oA.x, oB.x) : oA.x, vA), hix = warp_max(vB ? fmaxf(oA.x, oB.x) : oA.x, vA);
+        const float loy = warp_min(vB ? fminf(oA.y, oB.y) : oA.y, vA), hiy = warp_max(vB ? fmaxf(oA.y, oB.y) : oA.y, vA);
+        const float loz = warp_min(vB ? fminf(oA.z, oB.z) : oA.z, vA), hiz = warp_max(vB ? fmaxf(oA.z, oB.z) : oA.z, vA);
+        const float ri2_max = warp_max_pos(fmaxf(fmaf(oA.x, oA.x, fmaf(oA.y, oA.y, oA.z * oA.z)), fmaf(oB.x, oB.x, fmaf(oB.y, oB.y, oB.z * oB.z))));
+        float tile_hc2 = 0.f, tile_b2 = 0.f;      // over the tile being filled: largest (2 h_j)^2, largest |s|^2 (warp-uniform)
+        __syncwarp();
+
         auto flush = [&](uint32_t cnt) {
-            // filter cut-off of a target: max((2 h_i)^2, largest (2 h_j)^2 in the tile) -- a superset of max(2h_i, 2h_j) per pair
-            const float cutA = fmaxf(hc2A, tile_hc2), cutB = fmaxf(hc2B, tile_hc2);
-            const float b2 = 3.0f * fmaxf(tile_b2, ri2_max);
-            const FilterTarget fA = filter_target(xA, yA, zA, vA ? ri2A - cutA - kFilterEps * (b2 + cutA) : kNever);
-            const FilterTarget fB = filter_target(xB, yB, zB, vB ? ri2B - cutB - kFilterEps * (b2 + cutB) : kNever);
+            // cut-off of a target against this tile: max((2 h_i)^2, largest (2 h_j)^2 in the tile) -- a superset of max(2h_i, 2h_j) per pair.
+            // Targets that cannot reach the tile's bounding box sit this flush out; the others get a lane (or half of one).
+            const Box box = tile_box(sm.f, cnt, lane);
+            const bool aA = vA && box_dist2(box, oA.x, oA.y, oA.z) < fmaxf(oA.w, tile_hc2) * kReachSlack;
+            const bool aB = vB && box_dist2(box, oB.x, oB.y, oB.z) < fmaxf(oB.w, tile_hc2) * kReachSlack;
+            const uint32_t n_act = compact_targets(sm.act, aA, aB, lane, lt);
+            const float hc2_tile = tile_hc2, b2 = 3.0f * fmaxf(tile_b2, ri2_max);
+            tile_hc2 = 0.f; tile_b2 = 0.f;
+            if (n_act == 0) return;
+            const bool dual = n_act > 32;                // else: one target per lane, two of its hits per iteration
+            const bool wA = lane < n_act, wB = dual && lane + 32 < n_act;
+            const uint32_t tA = wA ? sm.act[lane] : 0, tB = wB ? sm.act[lane + 32] : tA;
+            const float4 pA = sm.t0[tA], pB = sm.t0[tB];
+            const float cutA = fmaxf(pA.w, hc2_tile), cutB = fmaxf(pB.w, hc2_tile);
+            const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - cutA - kFilterEps * (b2 + cutA) : kNever);
+            const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - cutB - kFilterEps * (b2 + cutB) : kNever);
             uint32_t m[4];
-            filter_masks(sm.f, cnt, lane, fA, fB, m);
+            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
+            const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
+            const u64 vx2 = pack2(qA.x, qB.x), vy2 = pack2(qA.y, qB.y), vz2 = pack2(qA.z, qB.z), c2 = pack2(qA.w, qB.w);
+            const u64 inv_h2 = pack2(sA.x, sB.x), n42 = pack2(sA.y, sB.y), rho2 = pack2(sA.z, sB.z), A2 = pack2(sA.w, sB.w);
+            const float hc2A = pA.w, hc2B = pB.w;
+            u64 ax = 0, ay = 0, az = 0, du = 0;
+            float vsig0 = 0.f, vsig1 = 0.f;
+
+            // phase 2 over one half of the tile.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j)
+            // is the same number and a_i += -m (..) (x_i - x_j) / r becomes one fma with e.
+            auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
+                uint32_t ja, jb;
+                while (next_hits(dual, ma, mb, &ja, &jb)) {
+                    const float4 a = sm.ta[base + ja], b = sm.ta[base + jb];
+                    const u64 ex = sub2(pack2(a.x, b.x), x2), ey = sub2(pack2(a.y, b.y), y2), ez = sub2(pack2(a.z, b.z), z2);
+                    const u64 r2 = fma2(ez, ez, fma2(ey, ey, mul2(ex, ex)));
+                    float r2a, r2b;
+                    unpack2(r2, r2a, r2b);
+                    // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
+                    // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
+                    const bool hitA = r2a < fmaxf(hc2A, a.w) && r2a > 0.f, hitB = r2b < fmaxf(hc2B, b.w) && r2b > 0.f;
+                    r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
+                    const u64 r2s = pack2(r2a, r2b);
+                    u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
+                    rinv = mul2(rinv, fma2(mul2(mul2(kMHalf2, r2s), rinv), rinv, kOneHalf2));      // one Newton step: ~1 ulp
+                    const u64 r = mul2(r2s, rinv);
+                    const float4 va = sm.tb[base + ja], vb = sm.tb[base + jb], ca = sm.tc[base + ja], cb = sm.tc[base + jb];
+                    const u64 ihj = pack2(ca.w, cb.w);
+                    const u64 Gi = mul2(spline_dw2(mul2(r, inv_h2), kTwo, kOne, kThree, kM075), n42);
+                    const u64 ih2 = mul2(ihj, ihj);
+                    const u64 Gj = mul2(spline_dw2(mul2(r, ihj), kTwo, kOne, kThree, kM075), mul2(mul2(ih2, ih2), kInvPi2));
+                    const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
+                    const u64 vr = mul2(fma2(wz, ez, fma2(wy, ey, mul2(wx, ex))), rinv);
+                    float vra, vrb;
+                    unpack2(vr, vra, vrb);
+                    const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
+                    const u64 vs = fma2(kMBeta2, mu, add2(c2, pack2(ca.z, cb.z)));
+                    float rsa, rsb, vsa, vsb;
+                    unpack2(add2(rho2, pack2(ca.x, cb.x)), rsa, rsb);
+                    unpack2(vs, vsa, vsb);
+                    const u64 visc = mul2(mul2(mul2(kMAlpha2, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
+                    const u64 vG = mul2(mul2(visc, kHalf2), add2(Gi, Gj));
+                    const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
+                    const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
+                    const u64 fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
+                    ax = fma2(fr, ex, ax); ay = fma2(fr, ey, ay); az = fma2(fr, ez, az);
+                    du = fma2(mul2(mm, fma2(kHalf2, vG, AG)), vr, du);
+                    vsig0 = fmaxf(vsig0, hitA ? vsa : 0.f); vsig1 = fmaxf(vsig1, hitB ? vsb : 0.f);
+                }
+            };
             hits(m[0], m[2], 0);
             if (cnt > 32) hits(m[1], m[3], kHalf);
-            tile_hc2 = 0.f; tile_b2 = 0.f;
-            __syncwarp();
+            float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
+            unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
+            if (!dual) { ax0 += ax1; ay0 += ay1; az0 += az1; du0 += du1; vsig0 = fmaxf(vsig0, vsig1); }
+            if (wA) { float* o = sm.raw + 5 * tA; o[0] += ax0; o[1] += ay0; o[2] += az0; o[3] += du0; o[4] = fmaxf(o[4], vsig0); }
+            if (wB) { float* o = sm.raw + 5 * tB; o[0] += ax1; o[1] += ay1; o[2] += az1; o[3] += du1; o[4] = fmaxf(o[4], vsig1); }
         };
 
         uint32_t cnt = 0;
@@ -440,7 +535,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         for (uint32_t r = 0; r < n_rounds; ++r) {
             const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
             if (r > 0) { cp_async_wait_all(); __syncwarp(); }
-            // one step ahead: the next round of this item (the next item's records are fetched after the results have left sm.tgt)
+            // one step ahead: the next round of this item (the next item's records are fetched once the results have left sm.raw)
             if (r + 1 < n_rounds) fetch_records<13, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 52, min(32u, n_s - j0 - 32), lane);
             float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
             float s2 = 0.f;
@@ -458,7 +553,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                 }
             }
             const uint32_t ball = __ballot_sync(kFull, ok), n_ok = __popc(ball);
-            if (cnt + n_ok > kTile) { flush(cnt); cnt = 0; }
+            if (cnt + n_ok > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
             if (ok) {
                 const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);      // half * 33 + index in the half
                 sm.ta[e] = a; sm.tb[e] = b; sm.tc[e] = c;
@@ -470,17 +565,13 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             buf ^= 1;
         }
         if (cnt) flush(cnt);
-        // results through shared memory so the 20-byte records leave as coalesced 16-byte stores
-        float axA, axB, ayA, ayB, azA, azB, duA, duB;
-        unpack2(ax, axA, axB); unpack2(ay, ayA, ayB); unpack2(az, azA, azB); unpack2(du, duA, duB);
-        if (vA) { float* o = sm.tgt + 5 * lane; o[0] = axA; o[1] = ayA; o[2] = azA; o[3] = duA; o[4] = vsigA; }
-        if (vB) { float* o = sm.tgt + 5 * (lane + 32); o[0] = axB; o[1] = ayB; o[2] = azB; o[3] = duB; o[4] = vsigB; }
         __syncwarp();
+        // the running results are already in FORCE_OUT record layout: they leave as coalesced 16-byte stores
         const uint32_t nvec = (n_t * 5 + 3) >> 2;
-        for (uint32_t v = lane; v < nvec; v += 32) reinterpret_cast<uint4*>(tout)[v] = reinterpret_cast<const uint4*>(sm.tgt)[v];
+        for (uint32_t v = lane; v < nvec; v += 32) reinterpret_cast<uint4*>(tout)[v] = reinterpret_cast<const uint4*>(sm.raw)[v];
         __syncwarp();
         if (has_next) {
-            fetch_records<13, 64>(sm.tgt, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+            fetch_records<13, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
             fetch_records<13, 32>(sm.src[buf], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
         }
         iw = iw_next;
