@@ -58,6 +58,10 @@ __device__ __forceinline__ float rcp_approx(float x) {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+__device__ __forceinline__ float rcp_fast(float x) {    // rcp.approx + one Newton step: within 1 ulp for normal x
+    const float r = rcp_approx(x);
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
 __device__ __forceinline__ uint32_t lanemask_lt() {
     uint32_t m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
@@ -278,7 +282,7 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
             const bool wA = lane < n_act, wB = dual && lane + 32 < n_act;
             const uint32_t tA = wA ? sm.act[lane] : 0, tB = wB ? sm.act[lane + 32] : tA;
             const float4 pA = sm.tgt[tA], pB = sm.tgt[tB];
-            const float inv_hA = wA ? 1.0f / pA.w : 0.f, inv_hB = dual ? (wB ? 1.0f / pB.w : 0.f) : inv_hA;
+            const float inv_hA = wA ? rcp_fast(pA.w) : 0.f, inv_hB = dual ? (wB ? rcp_fast(pB.w) : 0.f) : inv_hA;
             const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - 4.0f * pA.w * pA.w - eps : kNever);
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - 4.0f * pB.w * pB.w - eps : kNever);
             uint32_t m[4];
@@ -353,12 +357,12 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
         if (cnt) flush(cnt);
         __syncwarp();
         if (vA) {
-            const float ih = 1.0f / oA.w, n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
+            const float ih = rcp_fast(oA.w), n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
             const float4 c = sm.acc[lane];
             reinterpret_cast<float4*>(tout)[lane] = make_float4(c.x * n3, -c.y * n4, c.z * n3, -c.w * n4);
         }
         if (vB) {
-            const float ih = 1.0f / oB.w, n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
+            const float ih = rcp_fast(oB.w), n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
             const float4 c = sm.acc[lane + 32];
             reinterpret_cast<float4*>(tout)[lane + 32] = make_float4(c.x * n3, -c.y * n4, c.z * n3, -c.w * n4);
         }
@@ -433,10 +437,10 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0, p2 = make_float4(0.f, 0.f, 1.f, 0.f);
             if (t < n_t) {
                 const float* r = sm.raw + 13 * t;
-                const float h = r[3], rho = r[5], ih = 1.0f / h;
+                const float h = r[3], rho = r[5], ih = rcp_fast(h);
                 p0 = make_float4(r[0], r[1], r[2], 4.0f * h * h);
                 p1 = make_float4(r[7], r[8], r[9], r[12]);
-                p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11] / ((1.0f + h * r[6] / (3.0f * rho)) * rho * rho));
+                p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11] * rcp_fast(fmaf(h * r[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho));
                 if (k == 0) hA = h; else hB = h;
             }
             sm.t0[t] = p0; sm.t1[t] = p1; sm.t2[t] = p2;
@@ -548,7 +552,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                 ok = a.x > lox - reach && a.x < hix + reach && a.y > loy - reach && a.y < hiy + reach && a.z > loz - reach && a.z < hiz + reach;
                 if (ok) {
                     b = make_float4(rec[7], rec[8], rec[9], rec[4]);
-                    c = make_float4(rho, rec[11] / ((1.0f + h * rec[6] / (3.0f * rho)) * rho * rho), rec[12], 1.0f / h);
+                    c = make_float4(rho, rec[11] * rcp_fast(fmaf(h * rec[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho), rec[12], rcp_fast(h));
                     s2 = fmaf(a.x, a.x, fmaf(a.y, a.y, a.z * a.z));
                 }
             }
