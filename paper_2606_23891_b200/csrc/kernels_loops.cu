@@ -387,6 +387,14 @@ struct ForceWarpSmem {
     uint32_t act[64];        // the active targets of the flush
 };
 
+// sum += a * b with the rounding error of the addition carried in c (Kahan), for a pair of sums
+__device__ __forceinline__ void kahan(u64& sum, u64& c, u64 a, u64 b) {
+    const u64 y = fma2(a, b, c);          // c holds minus the error so far
+    const u64 t = add2(sum, y);
+    c = sub2(y, sub2(t, sum));            // y - (t - sum): what the addition dropped
+    sum = t;
+}
+
 // -0.75 (2 - q)+^2 + 3 (1 - q)+^2 = w'(q) of the cubic spline for a pair of q
 __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree, u64 kM075) {
     float ta, tb, ua, ub;
@@ -480,7 +488,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const u64 vx2 = pack2(qA.x, qB.x), vy2 = pack2(qA.y, qB.y), vz2 = pack2(qA.z, qB.z), c2 = pack2(qA.w, qB.w);
             const u64 inv_h2 = pack2(sA.x, sB.x), n42 = pack2(sA.y, sB.y), rho2 = pack2(sA.z, sB.z), A2 = pack2(sA.w, sB.w);
             const float hc2A = pA.w, hc2B = pB.w;
-            u64 ax = 0, ay = 0, az = 0, du = 0;
+            u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
             float vsig0 = 0.f, vsig1 = 0.f;
 
             // phase 2 over one half of the tile.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j)
@@ -520,7 +528,9 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                     const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
                     const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
                     const u64 fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
-                    ax = fma2(fr, ex, ax); ay = fma2(fr, ey, ay); az = fma2(fr, ez, az);
+                    // a sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan) adds
+                    // keep the rounding of the running sums out of the 1e-6 max|a| budget
+                    kahan(ax, cx, fr, ex); kahan(ay, cy, fr, ey); kahan(az, cz, fr, ez);
                     du = fma2(mul2(mm, fma2(kHalf2, vG, AG)), vr, du);
                     vsig0 = fmaxf(vsig0, hitA ? vsa : 0.f); vsig1 = fmaxf(vsig1, hitB ? vsb : 0.f);
                 }
