@@ -408,7 +408,7 @@ def run_reference(args):
     n_cells = cells.shape[0]
     probe = 32
     t_probe = oracle_sample_step(orc, ps, cells, tasks, probe)
-    per_step_budget = max(0.5, 150.0 / (args.steps + args.warmup))
+    per_step_budget = max(0.5, args.ref_budget / (args.steps + args.warmup))
     m = int(max(8, min(n_cells, probe * per_step_budget / max(t_probe, 1e-3))))
     for _ in range(args.warmup):
         oracle_sample_step(orc, ps, cells, tasks, m)
@@ -439,6 +439,7 @@ def main():
     ap.add_argument("--skip-zero-copy", action="store_true", help="config4: time the staged pipeline only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--ref-budget", type=float, default=150.0, help="--impl reference: seconds of oracle work over all steps")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
