@@ -21,8 +21,8 @@ namespace sph {
 
 namespace {
 
-constexpr int kPackWarps = 8;
-constexpr int kUnpackWarps = 4;
+constexpr int kPackWarps = 4;
+constexpr int kUnpackWarps = 2;
 
 template <int BYTES>
 __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
@@ -36,16 +36,55 @@ __device__ __forceinline__ void st_stream16(void* p, uint4 v) {   // records are
     asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// ---- bulk copies (TMA without a tensor map: cp.async.bulk) and the mbarrier they complete on ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared, size a multiple of 16 bytes, both addresses 16-byte aligned; completes (in bytes) on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// shared -> global, member of the issuing thread's current bulk group
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+
+constexpr int kPackK = 2;                      // record-stream templates per set; two sets alternate
+constexpr uint32_t kPackTableOcc = 32;         // occurrences whose block offsets and frames are staged at a time
+constexpr uint32_t kPackTableBytes = kPackTableOcc * (4 + 24);
+
 template <int NIT>
 __global__ void __launch_bounds__(kPackWarps * 32)
 pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
             const double* __restrict__ occ_frames, uint32_t n_cell_chunks, uint32_t slices, char* __restrict__ buf) {
-    extern __shared__ __align__(16) unsigned char smem[];
+    extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t R = prog.rec_words;
     const uint32_t templ_bytes = 128 * R;                           // 32 records
-    unsigned char* stage = smem + (size_t)warp * (prog.smem_per_warp + 2 * templ_bytes);
-    unsigned char* templ = stage + prog.smem_per_warp;              // two copies, used alternately
+    unsigned char* stage = smem + (size_t)warp * (prog.smem_per_warp + 2 * kPackK * templ_bytes + 2 * kPackTableBytes);
+    unsigned char* templ = stage + prog.smem_per_warp;              // 2 sets of kPackK copies
+    unsigned char* tables = templ + 2 * kPackK * templ_bytes;       // 2 x { double frames[32][3]; uint32_t off128[32]; }
 
     // which staging word feeds output word g = 4 (lane + 32 it) + j of a chunk's record stream
     uint32_t src[NIT][4];
@@ -58,29 +97,34 @@ pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint3
             src[it][j] = k < 32 ? prog.word[w].a + k * prog.word[w].stride : 0;
         }
     const uint32_t xw0 = prog.xw[0], xw1 = prog.xw[1], xw2 = prog.xw[2];
+    const bool xrel = prog.xrel != 0;
 
-    const uint32_t n_items = n_cell_chunks * slices;
-    for (uint32_t item = blockIdx.x * kPackWarps + warp; item < n_items; item += gridDim.x * kPackWarps) {
-        const uint32_t cc = item / slices, sl = item - cc * slices;
-        const CellChunk ch = cell_chunks[cc];
-        const uint32_t per = (ch.nocc + slices - 1) / slices;
-        const uint32_t ob = sl * per, oe = min(ch.nocc, ob + per);
-        if (ob >= oe) continue;
-        const uint32_t n = ch.count;
-        // first occurrence's block offset and frame: in flight while the chunk is staged
-        uint32_t o128 = __ldg(occ_off128 + ch.occ0 + ob);
-        double f0 = 0., f1 = 0., f2 = 0.;
-        if (prog.xrel) {
-            const double* f = occ_frames + 3 * (size_t)(ch.occ0 + ob);
-            f0 = __ldg(f); f1 = __ldg(f + 1); f2 = __ldg(f + 2);
+    // item -> its cell chunk and its slice [ob, oe) of the cell's occurrences (empty for a short cell)
+    const uint32_t n_items = n_cell_chunks * slices, item_step = gridDim.x * kPackWarps;
+    auto item_range = [&](uint32_t it, CellChunk* c, uint32_t* o_b, uint32_t* o_e) {
+        const uint32_t cc = it / slices, sl = it - cc * slices;
+        *c = cell_chunks[cc];
+        const uint32_t per = (c->nocc + slices - 1) / slices;
+        *o_b = min(c->nocc, sl * per); *o_e = min(c->nocc, *o_b + per);
+    };
+    // block offsets and frames of occurrences [o0, o0 + cnt) of a cell -> table t (asynchronous)
+    auto stage_table = [&](const CellChunk& c, uint32_t o0, uint32_t cnt, uint32_t t) {
+        unsigned char* tb = tables + t * kPackTableBytes;
+        if (lane < cnt) {
+            cp_async<4>(tb + 24 * kPackTableOcc + 4 * lane, occ_off128 + c.occ0 + o0 + lane);
+            if (xrel) {
+                const double* f = occ_frames + 3 * (size_t)(c.occ0 + o0 + lane);
+                cp_async<8>(tb + 24 * lane, f); cp_async<8>(tb + 24 * lane + 8, f + 1); cp_async<8>(tb + 24 * lane + 16, f + 2);
+            }
         }
-
-        // (1) stage the chunk's structs (once per item, not once per occurrence)
+    };
+    // the chunk's structs -> the staging area (asynchronous)
+    auto stage_chunk = [&](const CellChunk& c) {
         for (uint32_t u = 0; u < prog.n_sub_used; ++u) {
             const PackSub su = prog.su[u];
-            const char* g = su.base + (uint64_t)ch.first * su.stride;
+            const char* g = su.base + (uint64_t)c.first * su.stride;
             unsigned char* dst = stage + su.smem_base;
-            const uint32_t nbytes = n * su.stride;
+            const uint32_t nbytes = c.count * su.stride;
             if (su.gran == 16) {
                 const uint32_t nvec = nbytes >> 4;
                 if (su.mask == 0xFFFFFFFFu) {
@@ -96,105 +140,176 @@ pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint3
                 for (uint32_t v = lane; v < (nbytes >> 2); v += 32) cp_async<4>(dst + 4 * v, g + 4 * v);
             }
         }
+    };
+
+    uint32_t item = blockIdx.x * kPackWarps + warp;
+    if (item >= n_items) return;
+    CellChunk ch, ch_next{};
+    uint32_t ob, oe, ob_next = 0, oe_next = 0, tcur = 0;
+    item_range(item, &ch, &ob, &oe);
+    if (ob < oe) { stage_chunk(ch); stage_table(ch, ob, min(kPackTableOcc, oe - ob), 0); }
+
+    for (; item < n_items; item += item_step, tcur ^= 1) {
+        const bool has_next = item + item_step < n_items;
+        if (has_next) item_range(item + item_step, &ch_next, &ob_next, &oe_next);     // in flight during the template build
         cp_async_wait_all();
         __syncwarp();
-
-        // (2) one lane per particle: keep x in registers (it is re-based for every occurrence); widen time_bin
+        const uint32_t n = ch.count;
+        const bool live = ob < oe && lane < n;
+        // (1) one lane per particle: keep x in registers (it is re-based for every occurrence); widen time_bin
         double x0 = 0., x1 = 0., x2 = 0.;
-        if (prog.xrel && lane < n) {
+        if (xrel && live) {
             const unsigned char* px = stage + prog.x_src + lane * prog.x_stride;
             x0 = *reinterpret_cast<const double*>(px); x1 = *reinterpret_cast<const double*>(px + 8); x2 = *reinterpret_cast<const double*>(px + 16);
         }
-        if (prog.tb && lane < n)
+        if (prog.tb && live)
             *reinterpret_cast<uint32_t*>(stage + prog.tb_dst + 4 * lane) = stage[prog.tb_src + lane * prog.tb_stride];
+        if (lane < kPackK) bulk_wait_read<0>();       // the previous item's bulk stores have read the templates
         __syncwarp();
 
-        // (3) re-slice the staging area into the record stream (both template copies); the x words are patched below
-        const uint32_t nvec_out = (n * R + 3) >> 2;   // a last partial vector spills into the block's pad bytes
-#pragma unroll
-        for (int it = 0; it < NIT; ++it) {
-            const uint32_t v = lane + 32 * it;
-            if (v < 8 * R) {
-                uint4 o;
-                o.x = *reinterpret_cast<const uint32_t*>(stage + src[it][0]);
-                o.y = *reinterpret_cast<const uint32_t*>(stage + src[it][1]);
-                o.z = *reinterpret_cast<const uint32_t*>(stage + src[it][2]);
-                o.w = *reinterpret_cast<const uint32_t*>(stage + src[it][3]);
-                *reinterpret_cast<uint4*>(templ + 16 * v) = o;
-                *reinterpret_cast<uint4*>(templ + templ_bytes + 16 * v) = o;
-            }
-        }
-        __syncwarp();   // the x words written here are overwritten by other lanes below
-
-        // (4) one copy of the template per occurrence of the cell (task side), x re-based to that side's frame
-        const uint64_t chunk_off = (uint64_t)ch.k0 * R * 4 + 16 * lane;
-        for (uint32_t o = ob; o < oe; ++o) {
-            unsigned char* T = templ + ((o - ob) & 1) * templ_bytes;
-            char* out = buf + (uint64_t)o128 * 128 + chunk_off;
-            if (prog.xrel && lane < n) {
-                float* rec = reinterpret_cast<float*>(T) + lane * R;
-                if (xw0 != 0xFFFFFFFFu) rec[xw0] = __double2float_rn(__dsub_rn(x0, f0));
-                if (xw1 != 0xFFFFFFFFu) rec[xw1] = __double2float_rn(__dsub_rn(x1, f1));
-                if (xw2 != 0xFFFFFFFFu) rec[xw2] = __double2float_rn(__dsub_rn(x2, f2));
-            }
-            if (o + 1 < oe) {   // next occurrence's table entries, in flight during this copy
-                o128 = __ldg(occ_off128 + ch.occ0 + o + 1);
-                if (prog.xrel) {
-                    const double* f = occ_frames + 3 * (size_t)(ch.occ0 + o + 1);
-                    f0 = __ldg(f); f1 = __ldg(f + 1); f2 = __ldg(f + 2);
-                }
-            }
-            __syncwarp();
+        // (2) re-slice the staging area into the record stream, every template copy; the x words are patched per occurrence
+        if (ob < oe) {
 #pragma unroll
             for (int it = 0; it < NIT; ++it) {
                 const uint32_t v = lane + 32 * it;
-                if (v < nvec_out) st_stream16(out + 512 * it, *reinterpret_cast<const uint4*>(T + 16 * v));
+                if (v < 8 * R) {
+                    uint4 o;
+                    o.x = *reinterpret_cast<const uint32_t*>(stage + src[it][0]);
+                    o.y = *reinterpret_cast<const uint32_t*>(stage + src[it][1]);
+                    o.z = *reinterpret_cast<const uint32_t*>(stage + src[it][2]);
+                    o.w = *reinterpret_cast<const uint32_t*>(stage + src[it][3]);
+#pragma unroll
+                    for (int c = 0; c < 2 * kPackK; ++c) *reinterpret_cast<uint4*>(templ + c * templ_bytes + 16 * v) = o;
+                }
             }
         }
-        __syncwarp();   // staging and templates are reused by the next item
+        __syncwarp();   // the staging area is free: the next item's structs and table travel during this item's copies
+        if (has_next && ob_next < oe_next) { stage_chunk(ch_next); stage_table(ch_next, ob_next, min(kPackTableOcc, oe_next - ob_next), tcur ^ 1); }
+
+        // (3) one bulk copy (TMA) of a template per occurrence of the cell (task side), x re-based to that side's frame.
+        //     Occurrences go in groups of kPackK; the two template sets alternate, so a group is patched while the previous
+        //     group's copies are still reading the other set.
+        const uint32_t bytes = (n * R * 4 + 15) & ~15u;      // a last partial vector spills into the block's pad bytes
+        const uint64_t chunk_off = (uint64_t)ch.k0 * R * 4;
+        unsigned char* tb = tables + tcur * kPackTableBytes;
+        uint32_t t0 = ob;                                    // first occurrence the table holds
+        for (uint32_t o = ob, g = 0; o < oe; o += kPackK, ++g) {
+            if (o + kPackK > t0 + kPackTableOcc && t0 + kPackTableOcc < oe) {     // a cell with many occurrences: refill the table
+                __syncwarp();
+                t0 = o;
+                if (lane < min(kPackTableOcc, oe - t0)) {
+                    reinterpret_cast<uint32_t*>(tb + 24 * kPackTableOcc)[lane] = __ldg(occ_off128 + ch.occ0 + t0 + lane);
+                    const double* f = occ_frames + 3 * (size_t)(ch.occ0 + t0 + lane);
+                    double* d = reinterpret_cast<double*>(tb + 24 * lane);
+                    if (xrel) { d[0] = __ldg(f); d[1] = __ldg(f + 1); d[2] = __ldg(f + 2); }
+                }
+            }
+            unsigned char* set = templ + (g & 1) * kPackK * templ_bytes;
+            if (g >= 2 && lane < kPackK) bulk_wait_read<1>();     // the group before last has read this set
+            __syncwarp();
+            if (xrel && live) {
+#pragma unroll
+                for (int k = 0; k < kPackK; ++k) {
+                    if (o + k < oe) {
+                        const double* f = reinterpret_cast<const double*>(tb + 24 * (o + k - t0));
+                        float* rec = reinterpret_cast<float*>(set + k * templ_bytes) + lane * R;
+                        if (xw0 != 0xFFFFFFFFu) rec[xw0] = __double2float_rn(__dsub_rn(x0, f[0]));
+                        if (xw1 != 0xFFFFFFFFu) rec[xw1] = __double2float_rn(__dsub_rn(x1, f[1]));
+                        if (xw2 != 0xFFFFFFFFu) rec[xw2] = __double2float_rn(__dsub_rn(x2, f[2]));
+                    }
+                }
+            }
+            fence_proxy_async();      // template words written through the generic proxy are read by the bulk copy
+            __syncwarp();
+            if (lane < kPackK) {
+                if (o + lane < oe) {
+                    const uint32_t o128 = reinterpret_cast<const uint32_t*>(tb + 24 * kPackTableOcc)[o + lane - t0];
+                    bulk_s2g(buf + (uint64_t)o128 * 128 + chunk_off, set + lane * templ_bytes, bytes);
+                }
+                bulk_commit();
+            }
+        }
+        ch = ch_next; ob = ob_next; oe = oe_next;
     }
+    if (lane < kPackK) bulk_wait_read<0>();    // shared memory must outlive the copies that read it
 }
 
 // ---------------------------------------------------------------------------------------------------------
 
-// One warp per 32-particle chunk of a cell.
-//  (1) fetch: the chunk's slice of every block the cell occurs in (up to `slots` per round, normally all of them) is
-//      copied into the warp's shared-memory ring with 16-byte cp.async -- no registers are held while the loads are
-//      in flight, so a warp keeps 14-17 KB outstanding and an SM close to 200 KB;
+// One warp per 32-particle chunk of a cell, as a two-stage pipeline of ROUNDS (a round = up to `slots` of the blocks the
+// cell occurs in, normally all of them):
+//  (1) fetch: the chunk's slice of every block of the round travels global -> shared memory as ONE bulk copy (TMA,
+//      cp.async.bulk) per slice, each issued by its own lane and all completing on the ring's mbarrier: a whole round is
+//      one instruction per lane, holds no registers while in flight, and the NEXT round (of this chunk, or the first of
+//      the warp's next chunk) is issued into the other ring before the current one is waited for, so every warp always
+//      has 14-17 KB outstanding;
 //  (2) reduce: one lane per particle walks the slices in ascending (task, side) order.  With the lane owning a
 //      record, the operator of word j (+=, max, =) is the same in every lane: no per-lane dispatch, no divergence.
 //      Records are read with VEC-word shared loads (stride = record length: conflict-free when R / VEC is odd).
 //  Words are processed in groups of GW; a record longer than GW keeps its running values in a scratch slot.
-// The descriptor and block-offset table of the warp's next chunk are fetched while the current slices are in flight.
+// The store's own values of the next chunk (the starting point of its sums) are loaded one round ahead as well.
 template <int VEC, int GW>
 __global__ void __launch_bounds__(kUnpackWarps * 32)
 unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
               uint32_t n_cell_chunks, const char* __restrict__ buf, uint32_t slots, uint32_t last_only, uint32_t all_sum) {
-    extern __shared__ __align__(16) unsigned char smem[];
+    extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t R = prog.rec_words;
     const uint32_t slot_bytes = 128 * R;
-    const bool single = R <= GW;                       // the whole record lives in registers; else slot 0 is the scratch
-    unsigned char* wbase = smem + (size_t)warp * (slots + (single ? 0u : 1u)) * slot_bytes;
-    float* scratch = reinterpret_cast<float*>(wbase);  // [R][32]
-    unsigned char* ring = wbase + (single ? 0u : slot_bytes);
+    const bool single = R <= GW;                       // the whole record lives in registers; else one slot of scratch
+    const uint32_t ring_bytes = slots * slot_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem) + 2 * warp;       // one mbarrier per ring
+    unsigned char* wbase = smem + 128 + (size_t)warp * (2 * ring_bytes + (single ? 0u : slot_bytes));
+    float* scratch = reinterpret_cast<float*>(wbase + 2 * ring_bytes);   // [R][32]
 
-    auto rounds_of = [&](const CellChunk& c, uint32_t* o_begin, uint32_t* per_round) {
-        *o_begin = last_only ? c.nocc - 1 : 0;
-        const uint32_t n_o = c.nocc - *o_begin, n_rounds = (n_o + slots - 1) / slots;
-        *per_round = (n_o + n_rounds - 1) / n_rounds;                     // <= slots <= 32
-    };
-    auto first_table = [&](const CellChunk& c) {
-        uint32_t o_begin, per_round;
-        rounds_of(c, &o_begin, &per_round);
-        return lane < min(per_round, c.nocc - o_begin) ? __ldg(occ_off128 + c.occ0 + o_begin + lane) : 0u;
-    };
-    // store access of word w of the lane's particle p
+    const uint32_t cc_step = gridDim.x * kUnpackWarps;
+    const uint32_t cc0 = blockIdx.x * kUnpackWarps + warp;
+    if (cc0 >= n_cell_chunks) return;
+    if (lane == 0) { mbar_init(bars, 1); mbar_init(bars + 1, 1); fence_mbar_init(); }
+    __syncwarp();
+
+    // store access of word w of particle p
     auto word_addr = [&](uint32_t w, uint64_t p) { return view.base[prog.word[w].sub] + p * prog.word[w].stride + prog.word[w].a; };
     auto is_reduced = [&](uint32_t w) { return prog.word[w].kind == W_SUM || prog.word[w].kind == W_MAX; };
 
-    // one group of words [g0, g0 + nw) reduced over the `lim` slices of the ring, in slice order
-    auto reduce_group = [&](float (&acc)[GW], uint32_t g0, uint32_t nw, uint32_t lim) {
+    // the running values of a chunk start from the store's own (reduced words only)
+    auto load_own = [&](float (&a)[GW], const CellChunk& c) {
+#pragma unroll
+        for (int j = 0; j < GW; ++j) a[j] = 0.f;
+        if (!single || lane >= c.count) return;
+        const uint64_t p = (uint64_t)c.first + lane;
+#pragma unroll
+        for (int j = 0; j < GW; ++j) {
+            if ((uint32_t)j >= R) continue;
+            if (j % 4 == 0 && j + 3 < GW && prog.vec4[j]) {
+                const float4 t = *reinterpret_cast<const float4*>(word_addr(j, p));
+                a[j] = t.x; if (j + 1 < GW) a[j + 1] = t.y; if (j + 2 < GW) a[j + 2] = t.z; if (j + 3 < GW) a[j + 3] = t.w;
+            } else if (!(prog.vec4[4 * (j / 4)] && 4 * (j / 4) + 3 < GW) && is_reduced(j)) {
+                a[j] = *reinterpret_cast<const float*>(word_addr(j, p));
+            }
+        }
+    };
+
+    // a cursor over the rounds of the warp's chunks
+    struct Cur { CellChunk ch; uint32_t cc, ob, per_round; };
+    auto enter = [&](Cur& c, uint32_t cc, const CellChunk& ch) {
+        c.cc = cc; c.ch = ch;
+        c.ob = last_only ? ch.nocc - 1 : 0;
+        const uint32_t n_o = ch.nocc - c.ob, n_rounds = (n_o + slots - 1) / slots;
+        c.per_round = (n_o + n_rounds - 1) / n_rounds;                    // <= slots <= 32
+    };
+    // one round into ring r: lane u fetches the chunk's slice of block (ob + u)
+    auto issue = [&](const Cur& c, uint32_t r) {
+        const uint32_t lim = min(c.per_round, c.ch.nocc - c.ob);
+        const uint32_t bytes = (c.ch.count * R * 4 + 15) & ~15u;          // a last partial vector reads into the block's pad bytes
+        const uint32_t tbl = lane < lim ? __ldg(occ_off128 + c.ch.occ0 + c.ob + lane) : 0u;
+        if (lane == 0) mbar_expect_tx(bars + r, lim * bytes);
+        __syncwarp();
+        if (lane < lim) bulk_g2s(wbase + r * ring_bytes + lane * slot_bytes, buf + (uint64_t)tbl * 128 + (uint64_t)c.ch.k0 * R * 4, bytes, bars + r);
+    };
+
+    // one group of words [g0, g0 + nw) reduced over the `lim` slices of a ring, in slice order
+    auto reduce_group = [&](float (&acc)[GW], const unsigned char* ring, uint32_t g0, uint32_t nw, uint32_t lim) {
         const unsigned char* rec = ring + (lane * R + g0) * 4;
         uint32_t m_sum[GW], m_red[GW];
 #pragma unroll
@@ -233,92 +348,80 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
         }
     };
 
-    const uint32_t cc_step = gridDim.x * kUnpackWarps;
-    uint32_t cc = blockIdx.x * kUnpackWarps + warp;
-    CellChunk ch_next{};
-    uint32_t tbl_next = 0;
-    if (cc < n_cell_chunks) { ch_next = cell_chunks[cc]; tbl_next = first_table(ch_next); }
-    for (; cc < n_cell_chunks; cc += cc_step) {
-        const CellChunk ch = ch_next;
-        const uint32_t tbl_first = tbl_next;
-        const uint32_t nvec = (ch.count * R + 3) >> 2;
-        const char* slice = buf + (uint64_t)ch.k0 * R * 4 + 16 * lane;
-        const bool live = lane < ch.count;
-        const uint64_t p = (uint64_t)ch.first + lane;
-        uint32_t o_begin, per_round;
-        rounds_of(ch, &o_begin, &per_round);
-
-        // running values: the store's own for the reduced words (issued before the slices are waited for)
-        float acc[GW];
-        if (single) {
+    Cur F;                                   // the round being fetched; the consumer follows one round behind
+    enter(F, cc0, cell_chunks[cc0]);
+    CellChunk ch_pre{};                      // descriptor of the warp's next chunk, loaded a chunk ahead
+    if (cc0 + cc_step < n_cell_chunks) ch_pre = cell_chunks[cc0 + cc_step];
+    float acc[GW], acc_pre[GW];
+    load_own(acc_pre, F.ch);
+    issue(F, 0);
+    bool f_valid = true;
+    for (uint32_t it = 0; f_valid; ++it) {
+        const Cur C = F;
+        const bool c_first = C.ob == (last_only ? C.ch.nocc - 1 : 0u);
+        const uint32_t lim = min(C.per_round, C.ch.nocc - C.ob);
+        const bool c_last = C.ob + lim >= C.ch.nocc;
+        if (c_first) {
 #pragma unroll
-            for (int j = 0; j < GW; ++j) acc[j] = 0.f;
-#pragma unroll
-            for (int j = 0; j < GW; ++j) {
-                if ((uint32_t)j >= R || !live) continue;
-                if (j % 4 == 0 && j + 3 < GW && prog.vec4[j]) {
-                    const float4 t = *reinterpret_cast<const float4*>(word_addr(j, p));
-                    acc[j] = t.x; if (j + 1 < GW) acc[j + 1] = t.y; if (j + 2 < GW) acc[j + 2] = t.z; if (j + 3 < GW) acc[j + 3] = t.w;
-                } else if (!(j >= 4 * (j / 4) && prog.vec4[4 * (j / 4)] && 4 * (j / 4) + 3 < GW) && is_reduced(j)) {
-                    acc[j] = *reinterpret_cast<const float*>(word_addr(j, p));
-                }
+            for (int j = 0; j < GW; ++j) acc[j] = acc_pre[j];
+        }
+        // advance the fetch cursor and put its round in flight (the other ring was released at the end of the previous iteration)
+        F.ob += F.per_round;
+        if (F.ob >= F.ch.nocc) {
+            const uint32_t cc = F.cc + cc_step;
+            f_valid = cc < n_cell_chunks;
+            if (f_valid) {
+                enter(F, cc, ch_pre);
+                if (cc + cc_step < n_cell_chunks) ch_pre = cell_chunks[cc + cc_step];
+                load_own(acc_pre, F.ch);
             }
-        } else {
+        }
+        if (f_valid) issue(F, (it + 1) & 1);
+
+        const unsigned char* ring = wbase + (it & 1) * ring_bytes;
+        const bool live = lane < C.ch.count;
+        const uint64_t p = (uint64_t)C.ch.first + lane;
+        if (!single && c_first)
             for (uint32_t w = 0; w < R; ++w)
                 scratch[w * 32 + lane] = live && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
-        }
-
-        for (uint32_t ob = o_begin; ob < ch.nocc; ob += per_round) {
-            const uint32_t lim = min(per_round, ch.nocc - ob);
-            const uint32_t tbl = ob == o_begin ? tbl_first : (lane < lim ? __ldg(occ_off128 + ch.occ0 + ob + lane) : 0u);
-            for (uint32_t u = 0; u < lim; ++u) {
-                const char* src = slice + (uint64_t)__shfl_sync(0xFFFFFFFFu, tbl, u) * 128;
-                unsigned char* dst = ring + u * slot_bytes + 16 * lane;
-                for (uint32_t v = lane; v < nvec; v += 32, src += 512, dst += 512) cp_async<16>(dst, src);
-            }
-            if (ob == o_begin && cc + cc_step < n_cell_chunks) {   // next chunk's tables, while this chunk's slices are in flight
-                ch_next = cell_chunks[cc + cc_step];
-                tbl_next = first_table(ch_next);
-            }
-            cp_async_wait_all();
-            __syncwarp();
-            if (single) {
-                reduce_group(acc, 0, R, lim);
-            } else {
-                for (uint32_t g0 = 0; g0 < R; g0 += GW) {
-                    const uint32_t nw = min((uint32_t)GW, R - g0);
-                    float a2[GW];
-#pragma unroll
-                    for (int j = 0; j < GW; ++j) a2[j] = (uint32_t)j < nw ? scratch[(g0 + j) * 32 + lane] : 0.f;
-                    reduce_group(a2, g0, nw, lim);
-#pragma unroll
-                    for (int j = 0; j < GW; ++j) if ((uint32_t)j < nw) scratch[(g0 + j) * 32 + lane] = a2[j];
-                }
-            }
-            __syncwarp();     // the ring is refilled by the next round / the next chunk
-        }
-
-        if (!live) continue;
+        mbar_wait(bars + (it & 1), (it >> 1) & 1);
         if (single) {
-#pragma unroll
-            for (int j = 0; j < GW; ++j) {
-                if ((uint32_t)j >= R) continue;
-                const int j4 = 4 * (j / 4);
-                if (j4 + 3 < GW && prog.vec4[j4]) {
-                    if (j == j4) *reinterpret_cast<float4*>(word_addr(j, p)) = make_float4(acc[j4], acc[j4 + 1 < GW ? j4 + 1 : j4], acc[j4 + 2 < GW ? j4 + 2 : j4], acc[j4 + 3 < GW ? j4 + 3 : j4]);
-                } else if (prog.word[j].kind == W_ASSIGN_BYTE) {
-                    *reinterpret_cast<unsigned char*>(word_addr(j, p)) = (unsigned char)__float_as_uint(acc[j]);
-                } else {
-                    *reinterpret_cast<float*>(word_addr(j, p)) = acc[j];
-                }
-            }
+            reduce_group(acc, ring, 0, R, lim);
         } else {
-            for (uint32_t w = 0; w < R; ++w) {
-                const float v = scratch[w * 32 + lane];
-                if (prog.word[w].kind == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(word_addr(w, p)) = (unsigned char)__float_as_uint(v);
-                else *reinterpret_cast<float*>(word_addr(w, p)) = v;
+            for (uint32_t g0 = 0; g0 < R; g0 += GW) {
+                const uint32_t nw = min((uint32_t)GW, R - g0);
+                float a2[GW];
+#pragma unroll
+                for (int j = 0; j < GW; ++j) a2[j] = (uint32_t)j < nw ? scratch[(g0 + j) * 32 + lane] : 0.f;
+                reduce_group(a2, ring, g0, nw, lim);
+#pragma unroll
+                for (int j = 0; j < GW; ++j) if ((uint32_t)j < nw) scratch[(g0 + j) * 32 + lane] = a2[j];
             }
         }
+        if (c_last && live) {
+            if (single) {
+#pragma unroll
+                for (int j = 0; j < GW; ++j) {
+                    if ((uint32_t)j >= R) continue;
+                    const int j4 = 4 * (j / 4);
+                    if (j4 + 3 < GW && prog.vec4[j4]) {
+                        if (j == j4) *reinterpret_cast<float4*>(word_addr(j, p)) = make_float4(acc[j4], acc[j4 + 1 < GW ? j4 + 1 : j4], acc[j4 + 2 < GW ? j4 + 2 : j4], acc[j4 + 3 < GW ? j4 + 3 : j4]);
+                    } else if (prog.word[j].kind == W_ASSIGN_BYTE) {
+                        *reinterpret_cast<unsigned char*>(word_addr(j, p)) = (unsigned char)__float_as_uint(acc[j]);
+                    } else {
+                        *reinterpret_cast<float*>(word_addr(j, p)) = acc[j];
+                    }
+                }
+            } else {
+                for (uint32_t w = 0; w < R; ++w) {
+                    const float v = scratch[w * 32 + lane];
+                    if (prog.word[w].kind == W_ASSIGN_BYTE) *reinterpret_cast<unsigned char*>(word_addr(w, p)) = (unsigned char)__float_as_uint(v);
+                    else *reinterpret_cast<float*>(word_addr(w, p)) = v;
+                }
+            }
+        }
+        fence_proxy_async();          // this ring's generic-proxy reads are ordered before the bulk copy that refills it
+        __syncwarp();
     }
 }
 
@@ -383,7 +486,7 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
     const uint32_t slot_bytes = 128 * prog.rec_words;
     const uint32_t extra = prog.rec_words <= (uint32_t)GW ? 0 : 1;      // scratch slot of a long record
     const uint32_t slots = last_only ? 1u : std::max(1u, std::min(std::min(32u, b->max_nocc), kUnpackRingBytes / slot_bytes));
-    const size_t smem = (size_t)kUnpackWarps * (slots + extra) * slot_bytes;
+    const size_t smem = 128 + (size_t)kUnpackWarps * (2 * slots + extra) * slot_bytes;      // mbarriers, then two rings (+ scratch) per warp
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         SPH_CUDA_TRY(cudaFuncSetAttribute(unpack_kernel<VEC, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -405,7 +508,7 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
     for (uint32_t u = 0; u < prog.n_sub_used; ++u) prog.su[u].base = view.base[prog.su[u].sub];
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
-    const size_t smem = ((size_t)prog.smem_per_warp + 2 * 128 * (size_t)prog.rec_words) * kPackWarps;
+    const size_t smem = ((size_t)prog.smem_per_warp + 2 * kPackK * 128 * (size_t)prog.rec_words + 2 * kPackTableBytes) * kPackWarps;
     if (smem > 200 * 1024) return fail(SPH_ERR_UNSUPPORTED, "layout needs %zu bytes of staging per CTA", smem);
     const uint32_t nit = (prog.rec_words + 3) / 4;   // 16-byte vectors per lane for a full chunk: ceil(32 R / 4 / 32)
     int32_t rc;
