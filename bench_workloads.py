@@ -300,6 +300,67 @@ def field_bytes(comps):
     return sum(8 if f == "x" else 4 for f, _ in comps)
 
 
+def cell_slabs(cells, n_slabs):
+    """[(cell_first, cell_count, particle_first, particle_count)]: contiguous cell ranges of about equal particle counts"""
+    first = cells["first"].astype(np.int64)
+    end = first + cells["count"].astype(np.int64)
+    n = int(end[-1])
+    cuts = [0]
+    for k in range(1, n_slabs):
+        c = int(np.searchsorted(end, k * n // n_slabs))
+        cuts.append(max(c, cuts[-1]))
+    cuts.append(cells.shape[0])
+    out = []
+    for c0, c1 in zip(cuts[:-1], cuts[1:]):
+        if c1 > c0:
+            out.append((c0, c1 - c0, int(first[c0]), int(end[c1 - 1] - first[c0])))
+    return out
+
+
+class Streamed:
+    """The host-resident store streamed slab by slab over two streams: the copy of slab k + 1 overlaps the kernel of slab k
+    (sph_store_upload_range / sph_pack_cells, sph_unpack_cells / sph_store_download_range)."""
+
+    def __init__(self, sph, torch, cells, n_slabs=16):
+        self.sph, self.torch = sph, torch
+        self.slabs = cell_slabs(cells, n_slabs)
+        self.copy_s, self.work_s = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def _fork(self):
+        ev = self.torch.cuda.Event()
+        ev.record()
+        self.copy_s.wait_event(ev)
+        self.work_s.wait_event(ev)
+
+    def _join(self):
+        for st in (self.copy_s, self.work_s):
+            ev = self.torch.cuda.Event()
+            ev.record(st)
+            self.torch.cuda.current_stream().wait_event(ev)
+
+    def pack(self, dev, hs, batch, aset, buf, subs):
+        self._fork()
+        for c0, nc, p0, npart in self.slabs:
+            for s in subs:
+                self.sph.sph_store_upload_range(dev, s, hs.host[s], p0, npart, self.copy_s)
+            ev = self.torch.cuda.Event()
+            ev.record(self.copy_s)
+            self.work_s.wait_event(ev)
+            self.sph.sph_pack_cells(dev, batch, aset, buf, c0, nc, self.work_s)
+        self._join()
+
+    def unpack(self, dev, hs, batch, aset, buf, subs, mode):
+        self._fork()
+        for c0, nc, p0, npart in self.slabs:
+            self.sph.sph_unpack_cells(dev, batch, aset, buf, c0, nc, mode, self.work_s)
+            ev = self.torch.cuda.Event()
+            ev.record(self.work_s)
+            self.copy_s.wait_event(ev)
+            for s in subs:
+                self.sph.sph_store_download_range(dev, s, hs.host[s], p0, npart, self.copy_s)
+        self._join()
+
+
 def run_config3(args, sph, torch, common):
     n = args.n or (1 << 24)
     ps, cells, tasks, setup = build_clumpy(sph, 3, 1, n)
@@ -314,6 +375,7 @@ def run_config3(args, sph, torch, common):
         batch = sph.sph_batch_create(hs.store, tasks)
         info = sph.sph_batch_get_info(batch)
         inst = info.n_instances
+        streamed = Streamed(sph, torch, cells, n_slabs=16)
         big = sweep_set(sph, PACK_SWEEP, 20, sph.SPH_ATTR_X_REL_F32)
         buf = torch.zeros(sph.sph_batch_buffer_bytes(batch, big), dtype=torch.uint8, device="cuda")
         for k in SWEEP_K:
@@ -333,7 +395,10 @@ def run_config3(args, sph, torch, common):
                     sph.sph_store_upload_sub(dev, s, hs.sub(s))
                 sph.sph_pack(dev, batch, aset, buf)
 
-            for mode, fn, moved in (("zero-copy", zc, None), ("staged", staged, staged_bytes)):
+            def streamed_p():
+                streamed.pack(dev, hs, batch, aset, buf, subs)
+
+            for mode, fn, moved in (("zero-copy", zc, None), ("staged", staged, staged_bytes), ("streamed", streamed_p, staged_bytes)):
                 t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
                 rows.append({"op": "pack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
                              "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),
@@ -355,7 +420,10 @@ def run_config3(args, sph, torch, common):
                 for s in subs:
                     sph.sph_store_download_sub(dev, s, hs.sub(s))
 
-            for mode, fn, moved in (("zero-copy", zc_u, None), ("staged", staged_u, staged_bytes)):
+            def streamed_u():
+                streamed.unpack(dev, hs, batch, aset, buf, subs, sph.SPH_UNPACK_REDUCE)
+
+            for mode, fn, moved in (("zero-copy", zc_u, None), ("staged", staged_u, staged_bytes), ("streamed", streamed_u, staged_bytes)):
                 t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
                 rows.append({"op": "unpack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
                              "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),

@@ -144,6 +144,12 @@ int32_t sph_store_sub_ptr(const sph_store* store, uint32_t sub, void** ptr_out);
  * substructs a loop reads / writes have to cross the host link; with AoS the whole 128-byte records do. */
 int32_t sph_store_upload_sub(sph_store* store, uint32_t sub, const void* host_src, uint64_t bytes, void* stream);
 int32_t sph_store_download_sub(const sph_store* store, uint32_t sub, void* host_dst, uint64_t bytes, void* stream);
+/* The same for the particles [first, first + count) of one substruct array: host_base [host] is the START of the host
+ * array (n*stride bytes in the store's layout); bytes (first*stride .. (first+count)*stride) are copied.  Cells are
+ * contiguous particle ranges, so the structs of a range of cells can cross the link while the kernels
+ * work on the cells that crossed before (sph_pack_cells / sph_unpack_cells). */
+int32_t sph_store_upload_range(sph_store* store, uint32_t sub, const void* host_base, uint64_t first, uint64_t count, void* stream);
+int32_t sph_store_download_range(const sph_store* store, uint32_t sub, void* host_base, uint64_t first, uint64_t count, void* stream);
 
 /* ---- cell grid / octree and task list (host, setup) ---- */
 /* x3 [host, n*3 f64 in [0, box)].  perm_out [host, n]: perm_out[k] = input index of the k-th particle in cell
@@ -194,6 +200,15 @@ int32_t sph_force(const sph_batch* batch, const void* d_in, uint64_t in_bytes, v
  * X with X_REL_F32 cannot be unpacked (SPH_ERR_UNSUPPORTED). */
 int32_t sph_unpack(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,
                    int32_t mode, void* stream);
+/* PACK / UNPACK restricted to the blocks of cells [cell_first, cell_first + cell_count) of the store's cell table
+ * (every occurrence of those cells in the batch, at its place in d_buf; the other blocks are left alone).  Both kernels
+ * are cell-centric -- a cell's particles are read (written) once and copied to (reduced from) all its blocks -- so
+ * calls over disjoint cell ranges that cover the table are together exactly sph_pack / sph_unpack, and each call only
+ * touches the store's particles of its own cells: the unit of the streamed host-resident path. */
+int32_t sph_pack_cells(const sph_store* store, const sph_batch* batch, const sph_attrset* set, void* d_buf, uint64_t buf_bytes,
+                       uint32_t cell_first, uint32_t cell_count, void* stream);
+int32_t sph_unpack_cells(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,
+                         int32_t mode, uint32_t cell_first, uint32_t cell_count, void* stream);
 /* GHOST: P = (gamma-1) rho u, c_s = sqrt(gamma (gamma-1) u) for every particle. */
 int32_t sph_ghost(sph_store* store, const sph_params* params, void* stream);
 

@@ -18,8 +18,9 @@ __all__ = [
     "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_attrset_canonical", "make_attrset",
     "sph_attrset_record_bytes", "sph_store_sub_bytes", "sph_store_create", "sph_store_destroy", "sph_store_import_aos",
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
+    "sph_store_upload_range", "sph_store_download_range",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
-    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_unpack", "sph_ghost",
+    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_unpack", "sph_unpack_cells", "sph_ghost",
 ]
 
 SPH_NFIELDS, SPH_MAX_SUB, SPH_MAX_ATTR = 18, 8, 32
@@ -36,6 +37,7 @@ EXPORTS = [
     "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_attrset_canonical",
     "sph_attrset_record_bytes", "sph_store_sub_bytes", "sph_store_create", "sph_store_destroy", "sph_store_import_aos",
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
+    "sph_store_upload_range", "sph_store_download_range", "sph_pack_cells", "sph_unpack_cells",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_free", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_unpack", "sph_ghost",
 ]
@@ -221,6 +223,15 @@ def sph_store_download_sub(store, sub: int, host_dst, stream=None) -> None:
     _check(_lib.sph_store_download_sub(store, C.c_uint32(sub), _ptr(host_dst), C.c_uint64(_nbytes(host_dst)), _stream(stream)))
 
 
+def sph_store_upload_range(store, sub: int, host_base, first: int, count: int, stream=None) -> None:
+    """host_base: the whole host substruct array; particles [first, first + count) are copied"""
+    _check(_lib.sph_store_upload_range(store, C.c_uint32(sub), _ptr(host_base), C.c_uint64(first), C.c_uint64(count), _stream(stream)))
+
+
+def sph_store_download_range(store, sub: int, host_base, first: int, count: int, stream=None) -> None:
+    _check(_lib.sph_store_download_range(store, C.c_uint32(sub), _ptr(host_base), C.c_uint64(first), C.c_uint64(count), _stream(stream)))
+
+
 def sph_cells_build_grid(x: np.ndarray, cells_per_dim: int, box: float = 1.0):
     """-> (perm u64[n], cells[cells_per_dim^3])"""
     x = np.ascontiguousarray(x, dtype=np.float64)
@@ -293,6 +304,11 @@ def sph_pack(store, batch, aset: sph_attrset, d_buf, stream=None) -> None:
     _check(_lib.sph_pack(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), _stream(stream)))
 
 
+def sph_pack_cells(store, batch, aset: sph_attrset, d_buf, cell_first: int, cell_count: int, stream=None) -> None:
+    _check(_lib.sph_pack_cells(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_uint32(cell_first), C.c_uint32(cell_count),
+                               _stream(stream)))
+
+
 def sph_density(batch, d_in, d_out, stream=None) -> None:
     _check(_lib.sph_density(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)), _stream(stream)))
 
@@ -304,6 +320,11 @@ def sph_force(batch, d_in, d_out, params: sph_params, stream=None) -> None:
 
 def sph_unpack(store, batch, aset: sph_attrset, d_buf, mode: int = SPH_UNPACK_REDUCE, stream=None) -> None:
     _check(_lib.sph_unpack(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), _stream(stream)))
+
+
+def sph_unpack_cells(store, batch, aset: sph_attrset, d_buf, cell_first: int, cell_count: int, mode: int = SPH_UNPACK_REDUCE, stream=None) -> None:
+    _check(_lib.sph_unpack_cells(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), C.c_uint32(cell_first),
+                                 C.c_uint32(cell_count), _stream(stream)))
 
 
 def sph_ghost(store, params: sph_params, stream=None) -> None:

@@ -347,6 +347,31 @@ int32_t sph_store_download_sub(const sph_store* s, uint32_t sub, void* host_dst,
     return SPH_OK;
 }
 
+static int32_t range_copy_check(const sph_store* s, uint32_t sub, const void* host, uint64_t first, uint64_t count) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!host) return fail(SPH_ERR_INVALID_ARG, "host pointer is NULL");
+    if (sub >= s->layout.n_sub) return fail(SPH_ERR_RANGE, "substruct %u of %u", sub, s->layout.n_sub);
+    if (first > s->n || count > s->n - first)
+        return fail(SPH_ERR_RANGE, "particles [%llu, +%llu) exceed the store (%llu)", (unsigned long long)first, (unsigned long long)count, (unsigned long long)s->n);
+    return SPH_OK;
+}
+
+int32_t sph_store_upload_range(sph_store* s, uint32_t sub, const void* host_base, uint64_t first, uint64_t count, void* stream) {
+    if (int32_t rc = range_copy_check(s, sub, host_base, first, count)) return rc;
+    if (count == 0) return SPH_OK;
+    const uint64_t st = s->layout.stride[sub];
+    SPH_CUDA_TRY(cudaMemcpyAsync(s->base[sub] + first * st, (const char*)host_base + first * st, count * st, cudaMemcpyDefault, (cudaStream_t)stream));
+    return SPH_OK;
+}
+
+int32_t sph_store_download_range(const sph_store* s, uint32_t sub, void* host_base, uint64_t first, uint64_t count, void* stream) {
+    if (int32_t rc = range_copy_check(s, sub, host_base, first, count)) return rc;
+    if (count == 0) return SPH_OK;
+    const uint64_t st = s->layout.stride[sub];
+    SPH_CUDA_TRY(cudaMemcpyAsync((char*)host_base + first * st, s->base[sub] + first * st, count * st, cudaMemcpyDefault, (cudaStream_t)stream));
+    return SPH_OK;
+}
+
 // host-side (de)interleave between the canonical AoS record and one substruct array
 static void transform(const sph_layout& aos, const sph_layout& lay, uint32_t sub, const char* src_aos, char* sub_buf, uint64_t n, bool to_sub) {
     for (int f = 0; f < SPH_NFIELDS; ++f) {
@@ -431,7 +456,18 @@ int32_t sph_store_zero(sph_store* s, const sph_attrset* set, void* stream) {
     return launch_zero(s->view(), s->n, prog, (cudaStream_t)stream);
 }
 
-int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes, void* stream) {
+// cells [cell_first, +cell_count) of the store's table -> the batch's cell chunks [cc0, cc0 + ncc)
+static int32_t cell_range(const sph_batch* b, uint32_t cell_first, uint32_t cell_count, uint32_t* cc0, uint32_t* ncc) {
+    const uint32_t n_cells = (uint32_t)b->cell_chunk0.size() - 1;
+    if (cell_first > n_cells || cell_count > n_cells - cell_first)
+        return fail(SPH_ERR_RANGE, "cells [%u, +%u) exceed the cell table (%u)", cell_first, cell_count, n_cells);
+    *cc0 = b->cell_chunk0[cell_first];
+    *ncc = b->cell_chunk0[cell_first + cell_count] - *cc0;
+    return SPH_OK;
+}
+
+int32_t sph_pack_cells(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes,
+                       uint32_t cell_first, uint32_t cell_count, void* stream) {
     if (int32_t rc = store_check(s)) return rc;
     if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
     if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
@@ -441,10 +477,18 @@ int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set,
     if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
     if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
-    return launch_pack(s->view(), b, prog, ot->d_occ_off128, (char*)d_buf, (cudaStream_t)stream);
+    uint32_t cc0 = 0, ncc = 0;
+    if (int32_t rc = cell_range(b, cell_first, cell_count, &cc0, &ncc)) return rc;
+    return launch_pack(s->view(), b, prog, ot->d_occ_off128, (char*)d_buf, cc0, ncc, (cudaStream_t)stream);
 }
 
-int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {
+int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes, void* stream) {
+    if (!b) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    return sph_pack_cells(s, b, set, d_buf, buf_bytes, 0, (uint32_t)b->cell_chunk0.size() - 1, stream);
+}
+
+int32_t sph_unpack_cells(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode,
+                         uint32_t cell_first, uint32_t cell_count, void* stream) {
     if (int32_t rc = store_check(s)) return rc;
     if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
     if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
@@ -454,9 +498,16 @@ int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, con
     if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
     if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    uint32_t cc0 = 0, ncc = 0;
+    if (int32_t rc = cell_range(b, cell_first, cell_count, &cc0, &ncc)) return rc;
     bool all_assign = true;
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_assign &= prog.word[w].kind == W_ASSIGN || prog.word[w].kind == W_ASSIGN_BYTE;
-    return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, (cudaStream_t)stream);
+    return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, cc0, ncc, (cudaStream_t)stream);
+}
+
+int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {
+    if (!b) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    return sph_unpack_cells(s, b, set, d_buf, buf_bytes, mode, 0, (uint32_t)b->cell_chunk0.size() - 1, stream);
 }
 
 static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, uint32_t rec_in,

@@ -118,7 +118,9 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     std::vector<uint32_t> cur(occ_start.begin(), occ_start.end() - 1);
     for (uint32_t s = 0; s < b->n_sides; ++s) occ_side[cur[b->sides[s].cell]++] = s;
     std::vector<CellChunk> cell_chunks;
+    b->cell_chunk0.assign(n_cells + 1, 0);
     for (uint32_t c = 0; c < n_cells; ++c) {
+        b->cell_chunk0[c] = (uint32_t)cell_chunks.size();
         if (!occ_count[c]) continue;
         ++b->n_cells_touched;
         b->max_nocc = std::max(b->max_nocc, occ_count[c]);
@@ -127,6 +129,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
             cell_chunks.push_back(CellChunk{(uint32_t)ce.first + k, std::min(32u, ce.count - k), k, occ_start[c], occ_count[c]});
     }
     b->n_cell_chunks = (uint32_t)cell_chunks.size();
+    b->cell_chunk0[n_cells] = b->n_cell_chunks;
     b->n_occ = b->n_sides;
 
     int32_t rc = upload(cell_chunks, &b->d_cell_chunks);

@@ -137,6 +137,7 @@ struct sph_batch {
     std::vector<sph::SideRec> sides;          // host copy
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists
     std::vector<uint32_t> task_side0;         // n_tasks + 1
+    std::vector<uint32_t> cell_chunk0;        // n_cells + 1: first 32-particle cell chunk of every cell of the store's table
     // device tables
     double* d_occ_frames = nullptr;           // 3 per occurrence (cell-major, ascending side): the frame of that side
     sph::CellChunk* d_cell_chunks = nullptr;
@@ -150,9 +151,11 @@ const OffsetTable* find_offsets(const sph_batch* batch, uint32_t rec_bytes);
 int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
 
 // kernel launchers (kernels_*.cu)
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, cudaStream_t st);
+// [cc0, cc0 + ncc): the cell chunks to work on
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf,
+                    uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                      bool last_only, cudaStream_t st);
+                      bool last_only, uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);

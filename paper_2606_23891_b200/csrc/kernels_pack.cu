@@ -32,9 +32,6 @@ __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
         asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem), "n"(BYTES));
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-__device__ __forceinline__ void st_stream16(void* p, uint4 v) {   // records are written once and read by another kernel
-    asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
 
 // ---- bulk copies (TMA without a tensor map: cp.async.bulk) and the mbarrier they complete on ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -461,7 +458,8 @@ int32_t sm_count(int* out) {
 }
 
 template <int NIT>
-int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms, cudaStream_t st) {
+int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms,
+                        uint32_t cc0, uint32_t ncc, cudaStream_t st) {
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -471,10 +469,10 @@ int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t*
     // when there are fewer cell chunks than about two rounds of resident warps
     const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(64 / kPackWarps, (220 * 1024) / (smem + 1024)));
     const uint32_t resident_warps = (uint32_t)sms * per_sm * kPackWarps;
-    const uint32_t slices = std::min(8u, std::max(1u, (2 * resident_warps + b->n_cell_chunks - 1) / b->n_cell_chunks));
-    const uint64_t items = (uint64_t)b->n_cell_chunks * slices;
+    const uint32_t slices = std::min(8u, std::max(1u, (2 * resident_warps + ncc - 1) / ncc));
+    const uint64_t items = (uint64_t)ncc * slices;
     const uint32_t grid = (uint32_t)std::min<uint64_t>((items + kPackWarps - 1) / kPackWarps, (uint64_t)sms * per_sm);
-    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_cell_chunks, d_occ_off128, b->d_occ_frames, b->n_cell_chunks, slices, d_buf);
+    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_cell_chunks + cc0, d_occ_off128, b->d_occ_frames, ncc, slices, d_buf);
     return SPH_OK;
 }
 
@@ -482,7 +480,7 @@ constexpr uint32_t kUnpackRingBytes = 17408;   // per warp: 27 slices of 32 x 20
 
 template <int VEC, int GW>
 int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                        bool last_only, bool all_sum, int sms, cudaStream_t st) {
+                        bool last_only, bool all_sum, int sms, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
     const uint32_t slot_bytes = 128 * prog.rec_words;
     const uint32_t extra = prog.rec_words <= (uint32_t)GW ? 0 : 1;      // scratch slot of a long record
     const uint32_t slots = last_only ? 1u : std::max(1u, std::min(std::min(32u, b->max_nocc), kUnpackRingBytes / slot_bytes));
@@ -493,17 +491,18 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
         configured = smem;
     }
     const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(16, (227 * 1024) / (smem + 1024)));
-    const uint32_t want = (b->n_cell_chunks + kUnpackWarps - 1) / kUnpackWarps;
+    const uint32_t want = (ncc + kUnpackWarps - 1) / kUnpackWarps;
     const uint32_t grid = std::min(want, (uint32_t)sms * per_sm);
-    unpack_kernel<VEC, GW><<<grid, kUnpackWarps * 32, smem, st>>>(view, prog, b->d_cell_chunks, d_occ_off128, b->n_cell_chunks, d_buf, slots,
+    unpack_kernel<VEC, GW><<<grid, kUnpackWarps * 32, smem, st>>>(view, prog, b->d_cell_chunks + cc0, d_occ_off128, ncc, d_buf, slots,
                                                                    last_only ? 1u : 0u, all_sum ? 1u : 0u);
     return SPH_OK;
 }
 
 }  // namespace
 
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_occ_off128, char* d_buf, cudaStream_t st) {
-    if (b->n_cell_chunks == 0) return SPH_OK;
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_occ_off128, char* d_buf,
+                    uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+    if (ncc == 0) return SPH_OK;
     Program prog = prog_in;
     for (uint32_t u = 0; u < prog.n_sub_used; ++u) prog.su[u].base = view.base[prog.su[u].sub];
     int sms = 0;
@@ -512,31 +511,31 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
     if (smem > 200 * 1024) return fail(SPH_ERR_UNSUPPORTED, "layout needs %zu bytes of staging per CTA", smem);
     const uint32_t nit = (prog.rec_words + 3) / 4;   // 16-byte vectors per lane for a full chunk: ceil(32 R / 4 / 32)
     int32_t rc;
-    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_occ_off128, d_buf, smem, sms, st);
-    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_occ_off128, d_buf, smem, sms, st);
-    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_occ_off128, d_buf, smem, sms, st);
-    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_occ_off128, d_buf, smem, sms, st);
-    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_occ_off128, d_buf, smem, sms, st);
-    else rc = launch_pack_nit<12>(b, prog, d_occ_off128, d_buf, smem, sms, st);
+    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    else rc = launch_pack_nit<12>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
     if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
 
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                      bool last_only, cudaStream_t st) {
-    if (b->n_cell_chunks == 0) return SPH_OK;
+                      bool last_only, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+    if (ncc == 0) return SPH_OK;
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
     bool all_sum = true;
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_sum &= prog.word[w].kind == W_SUM;
     const uint32_t R = prog.rec_words;
     int32_t rc;
-    if (R % 4 == 0) rc = R % 8 == 0 ? launch_unpack_t<4, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st)
-                                    : launch_unpack_t<4, 4>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
-    else if (R % 2 == 0) rc = launch_unpack_t<2, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
-    else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
-    else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, st);
+    if (R % 4 == 0) rc = R % 8 == 0 ? launch_unpack_t<4, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st)
+                                    : launch_unpack_t<4, 4>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
+    else if (R % 2 == 0) rc = launch_unpack_t<2, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
+    else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
+    else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
     if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;

@@ -234,6 +234,75 @@ def test_unpack_bit_exact_stage_isolated(name, layout):
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["ragged", "octree"])
+def test_streamed_cell_ranges_equal_oracle(name, layout):
+    """The streamed host-resident path: the store's structs cross the link slab by slab (sph_store_upload_range), every slab
+    is packed as soon as it is there (sph_pack_cells); results are unpacked slab by slab (sph_unpack_cells) and each
+    slab's particles downloaded (sph_store_download_range).  Buffers and host store must equal the oracle's bit for bit."""
+    ps, cells, tasks = case(name)
+    n_cells = cells.shape[0]
+    g = GpuCase(ps, cells, tasks, layout)
+    lay = g.layout
+    # host store in the store's own layout (pinned), device store scrambled so that a missing upload shows
+    host = [torch.empty(g.n * lay.stride[s], dtype=torch.uint8).pin_memory() for s in range(lay.n_sub)]
+    for s in range(lay.n_sub):
+        sph.sph_store_download_sub(g.store, s, host[s])
+    torch.cuda.synchronize()
+    junk = raw_copy(ps)
+    junk.view(np.uint8)[:] = 0x5A
+    sph.sph_store_import_aos(g.store, junk)
+    bounds = [0, 1, n_cells // 3, n_cells // 3, (2 * n_cells) // 3 + 1, n_cells]      # ragged slabs, one of them empty
+    copy_s, work_s = torch.cuda.Stream(), torch.cuda.Stream()
+
+    oset = orc.FORCE_IN
+    aset, rec = to_attrset(oset), orc.record_bytes(oset)
+    ref = orc.pack(ps, cells, tasks, oset)
+    off_o, total = orc.block_offsets(cells, tasks, rec)
+    buf = g.buffer(aset)
+    for c0, c1 in zip(bounds[:-1], bounds[1:]):
+        first = int(cells["first"][c0]) if c0 < n_cells else g.n
+        last = int(cells["first"][c1 - 1]) + int(cells["count"][c1 - 1]) if c1 > c0 else first
+        for s in range(lay.n_sub):
+            sph.sph_store_upload_range(g.store, s, host[s], first, last - first, copy_s)
+        ev = torch.cuda.Event()
+        ev.record(copy_s)
+        work_s.wait_event(ev)
+        sph.sph_pack_cells(g.store, g.batch, aset, buf, c0, c1 - c0, work_s)
+    torch.cuda.synchronize()
+    m = valid_mask(off_o, cells, tasks, rec, total)
+    assert np.array_equal(buf.cpu().numpy()[m], ref[m]), (name, layout)
+
+    oset = orc.FORCE_OUT
+    aset, rec = to_attrset(oset), orc.record_bytes(oset)
+    _, total = orc.block_offsets(cells, tasks, rec)
+    res = _random_result_buffer(total, 77)
+    want = raw_copy(ps)
+    orc.unpack(want, cells, tasks, oset, res, orc.MODE_REDUCE)
+    assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+    d_res = torch.from_numpy(res).cuda()
+    for c0, c1 in zip(bounds[:-1], bounds[1:]):
+        first = int(cells["first"][c0]) if c0 < n_cells else g.n
+        last = int(cells["first"][c1 - 1]) + int(cells["count"][c1 - 1]) if c1 > c0 else first
+        sph.sph_unpack_cells(g.store, g.batch, aset, d_res, c0, c1 - c0, orc.MODE_REDUCE, work_s)
+        ev = torch.cuda.Event()
+        ev.record(work_s)
+        copy_s.wait_event(ev)
+        for s in range(lay.n_sub):
+            sph.sph_store_download_range(g.store, s, host[s], first, last - first, copy_s)
+    torch.cuda.synchronize()
+    assert np.array_equal(canon(g.export()), canon(want)), (name, layout)
+    # the host store holds the same bytes as the device store
+    for s in range(lay.n_sub):
+        dev = torch.empty_like(host[s])
+        sph.sph_store_download_sub(g.store, s, dev)
+        torch.cuda.synchronize()
+        assert torch.equal(dev, host[s]), (name, layout, s)
+    with pytest.raises(sph.SphError):
+        sph.sph_pack_cells(g.store, g.batch, aset, d_res, n_cells, 1)
+    g.close()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
 def test_pack_then_unpack_identity(layout):
     ps, cells, tasks = case("octree")
     oset = ([(orc.X, 0, 3), (orc.V, 0, 3), (orc.RHO, 0, 1), (orc.ID, 0, 1), (orc.TIME_BIN, 0, 1), (orc.ROT_V, 1, 1)], 0)
