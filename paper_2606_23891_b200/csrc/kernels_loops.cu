@@ -36,6 +36,7 @@ typedef unsigned long long u64;            // a pair of f32 (lo = target A, hi =
 constexpr int kLoopWarps = 4;
 constexpr int kTile = 64;                  // compacted sources per flush: two halves of 32, one mask word each per target
 constexpr int kHalf = 33;                  // tile entries per half: 32 sources + the dummy (where __clz(0) = 32 points)
+constexpr int kUnitCap = 96;               // units (target, <= 4 neighbours) evaluated per window of a flush, 32 at a time
 constexpr float kInvPi = 0.318309886183790671538f;
 constexpr float kNever = 1.0e30f;          // |s|^2 of a filter pad entry / threshold of an idle target: never a hit
 constexpr float kFar = 1.0e15f;            // coordinates of the dummy source (r^2 = 3e30 stays finite)
@@ -441,14 +442,6 @@ struct ForceWarpSmem {
     uint64_t bar[2];         // [0]: the mbarrier the record fetches complete on
 };
 
-// sum += a * b with the rounding error of the addition carried in c (Kahan), for a pair of sums
-__device__ __forceinline__ void kahan(u64& sum, u64& c, u64 a, u64 b) {
-    const u64 y = fma2(a, b, c);          // c holds minus the error so far
-    const u64 t = add2(sum, y);
-    c = sub2(y, sub2(t, sum));            // y - (t - sum): what the addition dropped
-    sum = t;
-}
-
 // -0.75 (2 - q)+^2 + 3 (1 - q)+^2 = w'(q) of the cubic spline for a pair of q
 __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree, u64 kM075) {
     float ta, tb, ua, ub;
@@ -538,65 +531,147 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - cutB - kFilterEps * (b2 + cutB) : kNever);
             uint32_t m[4];
             if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
-            const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
-            const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
-            const u64 vx2 = pack2(qA.x, qB.x), vy2 = pack2(qA.y, qB.y), vz2 = pack2(qA.z, qB.z), c2 = pack2(qA.w, qB.w);
-            const u64 inv_h2 = pack2(sA.x, sB.x), n42 = pack2(sA.y, sB.y), rho2 = pack2(sA.z, sB.z), A2 = pack2(sA.w, sB.w);
-            const float hc2A = pA.w, hc2B = pB.w;
-            u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
-            float vsig0 = 0.f, vsig1 = 0.f;
+            __syncwarp();     // the filter has read sm.f: its first bytes now hold the unit list
 
-            // phase 2 over one half of the tile.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j)
-            // is the same number and a_i += -m (..) (x_i - x_j) / r becomes one fma with e.
-            auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
-                uint32_t ja, jb;
-                while (next_hits(dual, ma, mb, &ja, &jb)) {
-                    const float4 a = sm.ta[base + ja], b = sm.ta[base + jb];
-                    const u64 ex = sub2(pack2(a.x, b.x), x2), ey = sub2(pack2(a.y, b.y), y2), ez = sub2(pack2(a.z, b.z), z2);
-                    const u64 r2 = fma2(ez, ez, fma2(ey, ey, mul2(ex, ex)));
-                    float r2a, r2b;
-                    unpack2(r2, r2a, r2b);
-                    // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
-                    // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
-                    const bool hitA = r2a < fmaxf(hc2A, a.w) && r2a > 0.f, hitB = r2b < fmaxf(hc2B, b.w) && r2b > 0.f;
-                    r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
-                    const u64 r2s = pack2(r2a, r2b);
-                    u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
-                    rinv = mul2(rinv, fma2(mul2(mul2(kMHalf2, r2s), rinv), rinv, kOneHalf2));      // one Newton step: ~1 ulp
-                    const u64 r = mul2(r2s, rinv);
-                    const float4 va = sm.tb[base + ja], vb = sm.tb[base + jb], ca = sm.tc[base + ja], cb = sm.tc[base + jb];
-                    const u64 ihj = pack2(ca.w, cb.w);
-                    const u64 Gi = mul2(spline_dw2(mul2(r, inv_h2), kTwo, kOne, kThree, kM075), n42);
-                    const u64 ih2 = mul2(ihj, ihj);
-                    const u64 Gj = mul2(spline_dw2(mul2(r, ihj), kTwo, kOne, kThree, kM075), mul2(mul2(ih2, ih2), kInvPi2));
-                    const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
-                    const u64 vr = mul2(fma2(wz, ez, fma2(wy, ey, mul2(wx, ex))), rinv);
-                    float vra, vrb;
-                    unpack2(vr, vra, vrb);
-                    const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
-                    const u64 vs = fma2(kMBeta2, mu, add2(c2, pack2(ca.z, cb.z)));
-                    float rsa, rsb, vsa, vsb;
-                    unpack2(add2(rho2, pack2(ca.x, cb.x)), rsa, rsb);
-                    unpack2(vs, vsa, vsb);
-                    const u64 visc = mul2(mul2(mul2(kMAlpha2, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
-                    const u64 vG = mul2(mul2(visc, kHalf2), add2(Gi, Gj));
-                    const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
-                    const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
-                    const u64 fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
-                    // a sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan) adds
-                    // keep the rounding of the running sums out of the 1e-6 max|a| budget
-                    kahan(ax, cx, fr, ex); kahan(ay, cy, fr, ey); kahan(az, cz, fr, ez);
-                    du = fma2(mul2(mm, fma2(kHalf2, vG, AG)), vr, du);
-                    vsig0 = fmaxf(vsig0, hitA ? vsa : 0.f); vsig1 = fmaxf(vsig1, hitB ? vsb : 0.f);
+            // Phase 2 in UNITS of up to four neighbours of one target.  Inside a cell pair the number of neighbours per target is
+            // heavy-tailed (0 .. ~30: targets next to the other cell against targets three layers away), so a lane that walks its
+            // own target's neighbours leaves most of the warp idle.  Instead:
+            //   (a) every lane cuts its targets' hit masks into units (target, <= 4 tile entries); a warp prefix sum numbers them;
+            //   (b) the units are evaluated 32 at a time, one per lane, two neighbours per iteration in packed f32x2 arithmetic
+            //       (at most two iterations), each unit leaving its partial sums in shared memory;
+            //   (c) the lane that made a unit adds its partial sums to the target's running sums, in unit order (= source order,
+            //       so the result does not depend on how units fell on lanes), a with compensated (Kahan) adds.
+            // kUnitCap units are in flight at a time; a flush with more takes several windows.
+            uint32_t* upos = reinterpret_cast<uint32_t*>(&sm.f);                        // [kUnitCap] the unit's (up to) four bits of a mask word
+            unsigned char* utgt = reinterpret_cast<unsigned char*>(upos + kUnitCap);    // [kUnitCap] the unit's target
+            float4* part_a = reinterpret_cast<float4*>(sm.raw + 320);                   // [kUnitCap] a (3), du
+            float* part_v = sm.raw + 320 + 4 * kUnitCap;                                // [kUnitCap] v_sig
+            const uint32_t nuA = ((__popc(m[0]) + 3) >> 2) + ((__popc(m[1]) + 3) >> 2), nuB = ((__popc(m[2]) + 3) >> 2) + ((__popc(m[3]) + 3) >> 2);
+            const uint32_t nu = nuA + nuB;
+            float axA = 0.f, ayA = 0.f, azA = 0.f, duA = 0.f, cxA = 0.f, cyA = 0.f, czA = 0.f, vsA = 0.f;
+            float axB = 0.f, ayB = 0.f, azB = 0.f, duB = 0.f, cxB = 0.f, cyB = 0.f, czB = 0.f, vsB = 0.f;
+            uint32_t cw = 0, mw = m[0];                 // the mask word being cut (0, 1: target A; 2, 3: target B) and what is left of it
+            const uint32_t m1 = m[1], m2 = m[2], m3 = m[3];
+            const uint32_t max_nu = __reduce_max_sync(kFull, nu);
+            // Units are numbered RANK-major (all lanes' first units, then all second units, ...): making the units and adding
+            // up their partial sums then takes as many warp-wide steps as the busiest lane has units, whatever the spread.
+            for (uint32_t r = 0; r < max_nu;) {
+                // (a) the next ranks, as many as fit into a window of kUnitCap units
+                const uint32_t r0 = r;
+                uint32_t cum = 0;
+                while (r < max_nu) {
+                    const uint32_t bal = __ballot_sync(kFull, nu > r), n_r = __popc(bal);
+                    if (cum + n_r > (uint32_t)kUnitCap) break;
+                    if (nu > r) {
+                        while (mw == 0) { ++cw; mw = cw == 1 ? m1 : (cw == 2 ? m2 : m3); }
+                        // the unit = the word's next (up to) four set bits, as a mask; the evaluating lane decodes them
+                        const uint32_t before = mw;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) mw &= ~shr_clamp(0x80000000u, __clz(mw));      // __clz(0) = 32: the shift gives 0, nothing cleared
+                        const uint32_t pos = before ^ mw;
+                        const uint32_t idx = cum + __popc(bal & lt);
+                        upos[idx] = pos;
+                        utgt[idx] = (unsigned char)((r < nuA ? tA : tB) | ((cw & 1) << 7));      // bit 7: the tile's second half
+                    }
+                    cum += n_r; ++r;
                 }
-            };
-            hits(m[0], m[2], 0);
-            if (cnt > 32) hits(m[1], m[3], kHalf);
-            float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
-            unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
-            if (!dual) { ax0 += ax1; ay0 += ay1; az0 += az1; du0 += du1; vsig0 = fmaxf(vsig0, vsig1); }
-            if (wA) { float* o = sm.raw + 5 * tA; o[0] += ax0; o[1] += ay0; o[2] += az0; o[3] += du0; o[4] = fmaxf(o[4], vsig0); }
-            if (wB) { float* o = sm.raw + 5 * tB; o[0] += ax1; o[1] += ay1; o[2] += az1; o[3] += du1; o[4] = fmaxf(o[4], vsig1); }
+                __syncwarp();
+
+                // (b) evaluation.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j) is the same
+                // number and a_i += -m (..) (x_i - x_j) / r becomes one fma with e.
+                for (uint32_t u0 = 0; u0 < cum; u0 += 32) {
+                    const uint32_t u = u0 + lane;
+                    const bool valid = u < cum;
+                    uint32_t um = valid ? upos[u] : 0u;
+                    const uint32_t tw = valid ? utgt[u] : 0u, t = tw & 127u, ebase = (tw >> 7) * kHalf;
+                    uint32_t e[4];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const uint32_t j = __clz(um);
+                        um &= ~shr_clamp(0x80000000u, j);
+                        e[q] = ebase + j;
+                    }
+                    const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
+                    const u64 x2 = dup2(P.x), y2 = dup2(P.y), z2 = dup2(P.z), vx2 = dup2(Q.x), vy2 = dup2(Q.y), vz2 = dup2(Q.z), c2 = dup2(Q.w);
+                    const u64 inv_h2 = dup2(S.x), n42 = dup2(S.y), rho2 = dup2(S.z), A2 = dup2(S.w);
+                    u64 ax = 0, ay = 0, az = 0, du = 0;
+                    float vsig0 = 0.f, vsig1 = 0.f;
+                    auto two = [&](uint32_t ja, uint32_t jb) {
+                        const float4 a = sm.ta[ja], b = sm.ta[jb];
+                        const u64 ex = sub2(pack2(a.x, b.x), x2), ey = sub2(pack2(a.y, b.y), y2), ez = sub2(pack2(a.z, b.z), z2);
+                        const u64 r2 = fma2(ez, ez, fma2(ey, ey, mul2(ex, ex)));
+                        float r2a, r2b;
+                        unpack2(r2, r2a, r2b);
+                        // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
+                        // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
+                        const bool hitA = r2a < fmaxf(P.w, a.w) && r2a > 0.f, hitB = r2b < fmaxf(P.w, b.w) && r2b > 0.f;
+                        r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
+                        const u64 r2s = pack2(r2a, r2b);
+                        u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
+                        rinv = mul2(rinv, fma2(mul2(mul2(kMHalf2, r2s), rinv), rinv, kOneHalf2));      // one Newton step: ~1 ulp
+                        const u64 rr = mul2(r2s, rinv);
+                        const float4 va = sm.tb[ja], vb = sm.tb[jb], ca = sm.tc[ja], cb = sm.tc[jb];
+                        const u64 ihj = pack2(ca.w, cb.w);
+                        const u64 Gi = mul2(spline_dw2(mul2(rr, inv_h2), kTwo, kOne, kThree, kM075), n42);
+                        const u64 ih2 = mul2(ihj, ihj);
+                        const u64 Gj = mul2(spline_dw2(mul2(rr, ihj), kTwo, kOne, kThree, kM075), mul2(mul2(ih2, ih2), kInvPi2));
+                        const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
+                        const u64 vr = mul2(fma2(wz, ez, fma2(wy, ey, mul2(wx, ex))), rinv);
+                        float vra, vrb;
+                        unpack2(vr, vra, vrb);
+                        const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
+                        const u64 vs = fma2(kMBeta2, mu, add2(c2, pack2(ca.z, cb.z)));
+                        float rsa, rsb, vsa, vsb;
+                        unpack2(add2(rho2, pack2(ca.x, cb.x)), rsa, rsb);
+                        unpack2(vs, vsa, vsb);
+                        const u64 visc = mul2(mul2(mul2(kMAlpha2, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
+                        const u64 vG = mul2(mul2(visc, kHalf2), add2(Gi, Gj));
+                        const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
+                        const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
+                        const u64 fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
+                        ax = fma2(fr, ex, ax); ay = fma2(fr, ey, ay); az = fma2(fr, ez, az);
+                        du = fma2(mul2(mm, fma2(kHalf2, vG, AG)), vr, du);
+                        vsig0 = fmaxf(vsig0, hitA ? vsa : 0.f); vsig1 = fmaxf(vsig1, hitB ? vsb : 0.f);
+                    };
+                    two(e[0], e[1]);
+                    if (__any_sync(kFull, e[2] != ebase + 32u)) two(e[2], e[3]);
+                    if (valid) {
+                        float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
+                        unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
+                        part_a[u] = make_float4(ax0 + ax1, ay0 + ay1, az0 + az1, du0 + du1);
+                        part_v[u] = fmaxf(vsig0, vsig1);
+                    }
+                }
+                __syncwarp();
+
+                // (c) a sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan)
+                // adds keep the rounding of the running sums out of the 1e-6 max|a| budget
+                uint32_t c2 = 0;
+                for (uint32_t q = r0; q < r; ++q) {
+                    const uint32_t bal = __ballot_sync(kFull, nu > q);
+                    if (nu > q) {
+                        const uint32_t idx = c2 + __popc(bal & lt);
+                        const float4 pa = part_a[idx];
+                        const float pv = part_v[idx];
+                        float y, t;
+                        if (q < nuA) {
+                            y = pa.x + cxA; t = axA + y; cxA = y - (t - axA); axA = t;      // c holds minus the error so far
+                            y = pa.y + cyA; t = ayA + y; cyA = y - (t - ayA); ayA = t;
+                            y = pa.z + czA; t = azA + y; czA = y - (t - azA); azA = t;
+                            duA += pa.w; vsA = fmaxf(vsA, pv);
+                        } else {
+                            y = pa.x + cxB; t = axB + y; cxB = y - (t - axB); axB = t;
+                            y = pa.y + cyB; t = ayB + y; cyB = y - (t - ayB); ayB = t;
+                            y = pa.z + czB; t = azB + y; czB = y - (t - azB); azB = t;
+                            duB += pa.w; vsB = fmaxf(vsB, pv);
+                        }
+                    }
+                    c2 += __popc(bal);
+                }
+                __syncwarp();     // the unit list and the partial sums are rewritten by the next window / flush
+            }
+            if (wA) { float* o = sm.raw + 5 * tA; o[0] += axA; o[1] += ayA; o[2] += azA; o[3] += duA; o[4] = fmaxf(o[4], vsA); }
+            if (wB) { float* o = sm.raw + 5 * tB; o[0] += axB; o[1] += ayB; o[2] += azB; o[3] += duB; o[4] = fmaxf(o[4], vsB); }
         };
 
         uint32_t cnt = 0;
