@@ -215,12 +215,49 @@ class Workload:
             fn()
 
     def step_e2e(self, stream=None):
-        stream = stream if stream is not None else self.torch.cuda.current_stream()
-        for s in self.subs_in:
-            self.sph.sph_store_upload_sub(self.store, s, self.host[s], stream)
-        self.step(stream)
-        for s in self.subs_out:
-            self.sph.sph_store_download_sub(self.store, s, self.host[s], stream)
+        """The step with the particle arrays in pinned HOST memory.  Uploads run on a copy stream ahead of the kernels that need
+        them, downloads on a second one as soon as a substruct holds its final values, so that with split-AoS the force
+        inputs cross during the density loop and the density results during the force loop; with AoS (one substruct) there is
+        nothing to overlap.  The calling stream waits for the last download: its events bracket the whole step."""
+        torch, sph = self.torch, self.sph
+        main = stream if stream is not None else torch.cuda.current_stream()
+        if not hasattr(self, "_e2e"):
+            f, loc = sph.FIELD, self.layout.loc
+            sub = lambda names: {loc[f[k]].sub for k in names}
+            d_in, f_in = sub(("x", "h", "mass")), sub(("v", "u"))
+            d_out, g_out, f_out = sub(("rho", "rho_dh", "wcount", "wcount_dh")), sub(("P", "c_s")), sub(("a", "du_dt", "v_sig"))
+            self._e2e = {"up": torch.cuda.Stream(), "down": torch.cuda.Stream(), "up1": sorted(d_in), "up2": sorted(f_in - d_in),
+                         "down1": sorted(d_out - g_out - f_out), "down2": sorted(g_out - f_out), "down3": sorted(f_out)}
+        E = self._e2e
+        up, down = E["up"], E["down"]
+        ev = lambda st: (lambda e: (e.record(st), e)[1])(torch.cuda.Event())
+        L = dict(self.launches(main))
+        start = ev(main)
+        up.wait_event(start)
+        down.wait_event(start)
+        for s in E["up1"]:
+            sph.sph_store_upload_sub(self.store, s, self.host[s], up)
+        e1 = ev(up)
+        for s in E["up2"]:
+            sph.sph_store_upload_sub(self.store, s, self.host[s], up)
+        e2 = ev(up)
+        main.wait_event(e1)
+        for k in ("zero_density_out", "pack_density_in", "density", "unpack_density_out"):
+            L[k]()
+        down.wait_event(ev(main))
+        for s in E["down1"]:
+            sph.sph_store_download_sub(self.store, s, self.host[s], down)
+        main.wait_event(e2)
+        L["ghost"]()
+        down.wait_event(ev(main))
+        for s in E["down2"]:
+            sph.sph_store_download_sub(self.store, s, self.host[s], down)
+        for k in ("zero_force_out", "pack_force_in", "force", "unpack_force_out"):
+            L[k]()
+        down.wait_event(ev(main))
+        for s in E["down3"]:
+            sph.sph_store_download_sub(self.store, s, self.host[s], down)
+        main.wait_event(ev(down))
 
     def e2e_bytes(self):
         return (sum(self.n * self.layout.stride[s] for s in self.subs_in), sum(self.n * self.layout.stride[s] for s in self.subs_out))
