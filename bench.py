@@ -4,8 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--layout split|aos]
 
 A step = one pass of the whole hot path over BASELINE.json:configs[1] (262,144 particles, 64^3 glass-like
-lattice, 16^3 cells, 57,344 tasks): zero, pack DENSITY_IN, density loop, unpack DENSITY_OUT, ghost, zero,
-pack FORCE_IN, force loop, unpack FORCE_OUT -- 9 kernel launches, inputs resident in HBM.
+lattice, 16^3 cells, 57,344 tasks): pack DENSITY_IN, density loop, unpack DENSITY_OUT (the sums start from zero),
+ghost, pack FORCE_IN, force loop, unpack FORCE_OUT -- 7 kernel launches, inputs resident in HBM.
 value = particles/s through that step (whole job: all ranks' particles / max-over-ranks time).
 `e2e` = the same step through the C ABI with HOST (pinned) particle arrays: the substructs the loops read are
 uploaded, the ones they write are downloaded, every step, inside the timed region.
@@ -194,20 +194,20 @@ class Workload:
             sph.sph_store_download_sub(self.store, s, self.host[s])
         torch.cuda.synchronize()
 
-    # the nine launches of a step, as (name, callable)
+    # the seven launches of a step, as (name, callable)
     def launches(self, stream=None):
         stream = stream if stream is not None else self.torch.cuda.current_stream()
         sph, st, b, S, B, p = self.sph, self.store, self.batch, self.sets, self.bufs, self.params
+        # "zero the outputs of the loop about to run" is fused into the unpack (SPH_UNPACK_REDUCE_ZERO: one batch holds the whole
+        # loop, so every particle's sums start from 0 there) -- bit-identical to sph_store_zero + SPH_UNPACK_REDUCE
         return [
-            ("zero_density_out", lambda: sph.sph_store_zero(st, S[1], stream)),
             ("pack_density_in", lambda: sph.sph_pack(st, b, S[0], B[0], stream)),
             ("density", lambda: sph.sph_density(b, B[0], B[1], stream)),
-            ("unpack_density_out", lambda: sph.sph_unpack(st, b, S[1], B[1], sph.SPH_UNPACK_REDUCE, stream)),
+            ("unpack_density_out", lambda: sph.sph_unpack(st, b, S[1], B[1], sph.SPH_UNPACK_REDUCE_ZERO, stream)),
             ("ghost", lambda: sph.sph_ghost(st, p, stream)),
-            ("zero_force_out", lambda: sph.sph_store_zero(st, S[3], stream)),
             ("pack_force_in", lambda: sph.sph_pack(st, b, S[2], B[2], stream)),
             ("force", lambda: sph.sph_force(b, B[2], B[3], p, stream)),
-            ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], sph.SPH_UNPACK_REDUCE, stream)),
+            ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], sph.SPH_UNPACK_REDUCE_ZERO, stream)),
         ]
 
     def step(self, stream=None):
@@ -242,7 +242,7 @@ class Workload:
             sph.sph_store_upload_sub(self.store, s, self.host[s], up)
         e2 = ev(up)
         main.wait_event(e1)
-        for k in ("zero_density_out", "pack_density_in", "density", "unpack_density_out"):
+        for k in ("pack_density_in", "density", "unpack_density_out"):
             L[k]()
         down.wait_event(ev(main))
         for s in E["down1"]:
@@ -252,7 +252,7 @@ class Workload:
         down.wait_event(ev(main))
         for s in E["down2"]:
             sph.sph_store_download_sub(self.store, s, self.host[s], down)
-        for k in ("zero_force_out", "pack_force_in", "force", "unpack_force_out"):
+        for k in ("pack_force_in", "force", "unpack_force_out"):
             L[k]()
         down.wait_event(ev(main))
         for s in E["down3"]:
@@ -269,9 +269,9 @@ class Workload:
         r = self.rec
         return {
             "pack_density_in": {"bound": "hbm", "bytes": n * 32 + inst * r[0]},
-            "unpack_density_out": {"bound": "hbm", "bytes": inst * r[1] + n * 2 * 16},
+            "unpack_density_out": {"bound": "hbm", "bytes": inst * r[1] + n * 16},       # REDUCE_ZERO: the fields are written, not read
             "pack_force_in": {"bound": "hbm", "bytes": n * 64 + inst * r[2]},
-            "unpack_force_out": {"bound": "hbm", "bytes": inst * r[3] + n * 2 * 20},
+            "unpack_force_out": {"bound": "hbm", "bytes": inst * r[3] + n * 20},
             "density": {"bound": "alu", "flop": cand * FLOP_CAND + n * NGB_CONFIG1 * FLOP_HIT_DENSITY},
             "force": {"bound": "alu", "flop": cand * FLOP_CAND + n * (NGB_CONFIG1 - 1) * FLOP_HIT_FORCE},
         }
@@ -409,7 +409,7 @@ def run_ours(args):
         "instances_per_s": {k: w.info.n_instances / (R["per"][k] * 1e-3) for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out")},
         "e2e": {"value": total_particles / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
                 "ms_per_step": ms_e2e},
-        "gpu_launches": 9 * args.steps,
+        "gpu_launches": 7 * args.steps,
         "clocks": R["clocks"],
         "roofline": roof,
         "kernels": kernels,

@@ -96,7 +96,11 @@ enum { SPH_MEM_DEVICE = 0, SPH_MEM_HOST_PINNED = 1 };
 enum { SPH_UNPACK_REDUCE = 0,   /* per-field operator: += for RHO, RHO_DH, WCOUNT, WCOUNT_DH, A, DU_DT; max for V_SIG;
                                    overwrite for every other field -- applied in ascending task order, side i
                                    before side j, in f32 (bit-reproducible) */
-       SPH_UNPACK_ASSIGN = 1 }; /* overwrite for every field, same order (last task wins) */
+       SPH_UNPACK_ASSIGN = 1,   /* overwrite for every field, same order (last task wins) */
+       SPH_UNPACK_REDUCE_ZERO = 2 }; /* SPH_UNPACK_REDUCE preceded by "zero the outputs" for the particles of the cells the call
+                                   * touches: the sums start from 0 instead of the store's values (bit-identical to
+                                   * sph_store_zero + SPH_UNPACK_REDUCE for those particles; others are left alone).  For the
+                                   * first (or only) batch of a loop: saves a launch and the read of the fields. */
 
 typedef struct sph_store sph_store;
 typedef struct sph_batch sph_batch;

@@ -13,7 +13,7 @@ from . import build as _build
 
 __all__ = [
     "SphError", "lib_path", "sph_layout", "sph_attr", "sph_attrset", "sph_params", "sph_batch_info", "CELL_DTYPE", "TASK_DTYPE",
-    "FIELD", "SPH_ATTR_X_REL_F32", "SPH_MEM_DEVICE", "SPH_MEM_HOST_PINNED", "SPH_UNPACK_REDUCE", "SPH_UNPACK_ASSIGN",
+    "FIELD", "SPH_ATTR_X_REL_F32", "SPH_MEM_DEVICE", "SPH_MEM_HOST_PINNED", "SPH_UNPACK_REDUCE", "SPH_UNPACK_ASSIGN", "SPH_UNPACK_REDUCE_ZERO",
     "SPH_SET_DENSITY_IN", "SPH_SET_DENSITY_OUT", "SPH_SET_FORCE_IN", "SPH_SET_FORCE_OUT", "EXPORTS",
     "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_attrset_canonical", "make_attrset",
     "sph_attrset_record_bytes", "sph_store_sub_bytes", "sph_store_create", "sph_store_destroy", "sph_store_import_aos",
@@ -29,7 +29,7 @@ FIELD = {name: i for i, name in enumerate(
      "id", "time_bin"])}
 SPH_ATTR_X_REL_F32 = 1
 SPH_MEM_DEVICE, SPH_MEM_HOST_PINNED = 0, 1
-SPH_UNPACK_REDUCE, SPH_UNPACK_ASSIGN = 0, 1
+SPH_UNPACK_REDUCE, SPH_UNPACK_ASSIGN, SPH_UNPACK_REDUCE_ZERO = 0, 1, 2
 SPH_SET_DENSITY_IN, SPH_SET_DENSITY_OUT, SPH_SET_FORCE_IN, SPH_SET_FORCE_OUT = 0, 1, 2, 3
 
 #: every symbol include/sph_b200.h declares

@@ -135,7 +135,7 @@ int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Pro
 int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, int32_t mode, Program* prog) {
     uint32_t rec_bytes = 0;
     if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
-    if (mode != SPH_UNPACK_REDUCE && mode != SPH_UNPACK_ASSIGN) return fail(SPH_ERR_INVALID_ARG, "unknown unpack mode %d", mode);
+    if (mode != SPH_UNPACK_REDUCE && mode != SPH_UNPACK_ASSIGN && mode != SPH_UNPACK_REDUCE_ZERO) return fail(SPH_ERR_INVALID_ARG, "unknown unpack mode %d", mode);
     std::memset(prog, 0, sizeof(*prog));
     prog->rec_words = rec_bytes / 4;
     uint32_t w = 0;
@@ -156,8 +156,8 @@ int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, i
                 prog->word[w++] = WordDesc{off, stride, loc.sub, (uint8_t)W_ASSIGN_BYTE};
             } else {
                 uint8_t kind = W_ASSIGN;
-                if (mode == SPH_UNPACK_REDUCE && is_sum) kind = W_SUM;
-                if (mode == SPH_UNPACK_REDUCE && a.field == SPH_V_SIG) kind = W_MAX;
+                if (mode != SPH_UNPACK_ASSIGN && is_sum) kind = W_SUM;
+                if (mode != SPH_UNPACK_ASSIGN && a.field == SPH_V_SIG) kind = W_MAX;
                 prog->word[w++] = WordDesc{off, stride, loc.sub, kind};
             }
         }
@@ -502,7 +502,7 @@ int32_t sph_unpack_cells(sph_store* s, const sph_batch* b, const sph_attrset* se
     if (int32_t rc = cell_range(b, cell_first, cell_count, &cc0, &ncc)) return rc;
     bool all_assign = true;
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_assign &= prog.word[w].kind == W_ASSIGN || prog.word[w].kind == W_ASSIGN_BYTE;
-    return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, cc0, ncc, (cudaStream_t)stream);
+    return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, mode == SPH_UNPACK_REDUCE_ZERO, cc0, ncc, (cudaStream_t)stream);
 }
 
 int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {

@@ -155,7 +155,7 @@ int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable**
 int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf,
                     uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                      bool last_only, uint32_t cc0, uint32_t ncc, cudaStream_t st);
+                      bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);

@@ -248,7 +248,7 @@ pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint3
 template <int VEC, int GW>
 __global__ void __launch_bounds__(kUnpackWarps * 32)
 unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
-              uint32_t n_cell_chunks, const char* __restrict__ buf, uint32_t slots, uint32_t last_only, uint32_t all_sum) {
+              uint32_t n_cell_chunks, const char* __restrict__ buf, uint32_t slots, uint32_t last_only, uint32_t all_sum, uint32_t from_zero) {
     extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t R = prog.rec_words;
@@ -273,7 +273,7 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
     auto load_own = [&](float (&a)[GW], const CellChunk& c) {
 #pragma unroll
         for (int j = 0; j < GW; ++j) a[j] = 0.f;
-        if (!single || lane >= c.count) return;
+        if (!single || from_zero || lane >= c.count) return;
         const uint64_t p = (uint64_t)c.first + lane;
 #pragma unroll
         for (int j = 0; j < GW; ++j) {
@@ -380,7 +380,7 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
         const uint64_t p = (uint64_t)C.ch.first + lane;
         if (!single && c_first)
             for (uint32_t w = 0; w < R; ++w)
-                scratch[w * 32 + lane] = live && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
+                scratch[w * 32 + lane] = live && !from_zero && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
         mbar_wait(bars + (it & 1), (it >> 1) & 1);
         if (single) {
             reduce_group(acc, ring, 0, R, lim);
@@ -480,7 +480,7 @@ constexpr uint32_t kUnpackRingBytes = 17408;   // per warp: 27 slices of 32 x 20
 
 template <int VEC, int GW>
 int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                        bool last_only, bool all_sum, int sms, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+                        bool last_only, bool all_sum, bool from_zero, int sms, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
     const uint32_t slot_bytes = 128 * prog.rec_words;
     const uint32_t extra = prog.rec_words <= (uint32_t)GW ? 0 : 1;      // scratch slot of a long record
     const uint32_t slots = last_only ? 1u : std::max(1u, std::min(std::min(32u, b->max_nocc), kUnpackRingBytes / slot_bytes));
@@ -494,7 +494,7 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
     const uint32_t want = (ncc + kUnpackWarps - 1) / kUnpackWarps;
     const uint32_t grid = std::min(want, (uint32_t)sms * per_sm);
     unpack_kernel<VEC, GW><<<grid, kUnpackWarps * 32, smem, st>>>(view, prog, b->d_cell_chunks + cc0, d_occ_off128, ncc, d_buf, slots,
-                                                                   last_only ? 1u : 0u, all_sum ? 1u : 0u);
+                                                                   last_only ? 1u : 0u, all_sum ? 1u : 0u, from_zero ? 1u : 0u);
     return SPH_OK;
 }
 
@@ -523,7 +523,7 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
 }
 
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
-                      bool last_only, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+                      bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st) {
     if (ncc == 0) return SPH_OK;
     int sms = 0;
     if (int32_t rc = sm_count(&sms)) return rc;
@@ -531,11 +531,11 @@ int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& 
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_sum &= prog.word[w].kind == W_SUM;
     const uint32_t R = prog.rec_words;
     int32_t rc;
-    if (R % 4 == 0) rc = R % 8 == 0 ? launch_unpack_t<4, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st)
-                                    : launch_unpack_t<4, 4>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
-    else if (R % 2 == 0) rc = launch_unpack_t<2, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
-    else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
-    else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, sms, cc0, ncc, st);
+    if (R % 4 == 0) rc = R % 8 == 0 ? launch_unpack_t<4, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st)
+                                    : launch_unpack_t<4, 4>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
+    else if (R % 2 == 0) rc = launch_unpack_t<2, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
+    else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
+    else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
     if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;

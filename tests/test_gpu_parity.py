@@ -234,6 +234,33 @@ def test_unpack_bit_exact_stage_isolated(name, layout):
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["config0", "octree"])
+def test_unpack_reduce_zero_equals_zero_then_reduce(name, layout):
+    """SPH_UNPACK_REDUCE_ZERO = "zero the outputs" fused into the unpack: bit-identical to the oracle's zero + REDUCE."""
+    ps, cells, tasks = case(name)
+    g = GpuCase(ps, cells, tasks, layout)
+    for n_set, oset in enumerate([orc.DENSITY_OUT, orc.FORCE_OUT, sweep_set(UNPACK_SWEEP, 13, 0)]):
+        aset = to_attrset(oset)
+        rec = orc.record_bytes(oset)
+        _, total = orc.block_offsets(cells, tasks, rec)
+        buf = _random_result_buffer(total, 300 + n_set)
+        ref = raw_copy(ps)
+        for f, c, _n in oset[0]:                              # zero the reduced fields (every cell occurs in these batches)
+            name_f = ("x", "v", "a", "mass", "h", "u", "du_dt", "rho", "rho_dh", "wcount", "wcount_dh", "div_v", "rot_v", "P", "c_s", "v_sig",
+                      "id", "time_bin")[f]
+            if name_f in ("rho", "rho_dh", "wcount", "wcount_dh", "du_dt", "v_sig"):
+                ref[name_f] = 0
+            elif name_f == "a":
+                ref["a"][:, c:c + _n] = 0
+        orc.unpack(ref, cells, tasks, oset, buf, orc.MODE_REDUCE)
+        sph.sph_store_import_aos(g.store, ps)                 # the store holds non-zero values in those fields
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        sph.sph_unpack(g.store, g.batch, aset, torch.from_numpy(buf).cuda(), sph.SPH_UNPACK_REDUCE_ZERO)
+        assert np.array_equal(canon(g.export()), canon(ref)), (name, layout, rec)
+    g.close()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
 @pytest.mark.parametrize("name", ["ragged", "octree"])
 def test_streamed_cell_ranges_equal_oracle(name, layout):
     """The streamed host-resident path: the store's structs cross the link slab by slab (sph_store_upload_range), every slab
