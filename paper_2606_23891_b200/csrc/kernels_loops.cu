@@ -33,10 +33,22 @@ namespace {
 
 typedef unsigned long long u64;            // a pair of f32 (lo = target A, hi = target B)
 
-constexpr int kLoopWarps = 4;
+#ifndef SPH_LOOP_WARPS
+#define SPH_LOOP_WARPS 4
+#endif
+#ifndef SPH_FORCE_MINB
+#define SPH_FORCE_MINB 4
+#endif
+#ifndef SPH_DENS_MINB
+#define SPH_DENS_MINB 5
+#endif
+#ifndef SPH_UNIT_CAP
+#define SPH_UNIT_CAP 96
+#endif
+constexpr int kLoopWarps = SPH_LOOP_WARPS;
 constexpr int kTile = 64;                  // compacted sources per flush: two halves of 32, one mask word each per target
 constexpr int kHalf = 33;                  // tile entries per half: 32 sources + the dummy (where __clz(0) = 32 points)
-constexpr int kUnitCap = 96;               // units (target, <= 4 neighbours) evaluated per window of a flush, 32 at a time
+constexpr int kUnitCap = SPH_UNIT_CAP;               // units (target, <= 4 neighbours) evaluated per window of a flush, 32 at a time
 constexpr float kInvPi = 0.318309886183790671538f;
 constexpr float kNever = 1.0e30f;          // |s|^2 of a filter pad entry / threshold of an idle target: never a hit
 constexpr float kFar = 1.0e15f;            // coordinates of the dummy source (r^2 = 3e30 stays finite)
@@ -284,7 +296,7 @@ struct DensityWarpSmem {
     uint32_t act[64];        // the active targets of the flush
 };
 
-__global__ void __launch_bounds__(kLoopWarps * 32, 5)
+__global__ void __launch_bounds__(kLoopWarps * 32, SPH_DENS_MINB)
 density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items) {
     __shared__ __align__(16) DensityWarpSmem s_all[kLoopWarps];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -451,7 +463,7 @@ __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree,
     return fma2(kThree, mul2(u, u), mul2(kM075, mul2(t, t)));
 }
 
-__global__ void __launch_bounds__(kLoopWarps * 32, 4)
+__global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
