@@ -168,7 +168,8 @@ class Workload:
     def __init__(self, sph, torch, ps, cells, tasks, layout_name):
         self.sph, self.torch = sph, torch
         self.layout_name = layout_name
-        self.layout = sph.sph_layout_aos() if layout_name == "aos" else sph.sph_layout_split()
+        from paper_2606_23891_b200 import layouts as _layouts
+        self.layout = _layouts.layout(sph, layout_name)
         self.n = ps.shape[0]
         self.store = sph.sph_store_create(self.layout, self.n)
         sph.sph_store_import_aos(self.store, ps)
@@ -330,8 +331,65 @@ def run_other_workload(args):
     print(json.dumps(line))
 
 
+def run_layouts(args):
+    """configs[1] through every particle layout of the paper (Fig. 2's axis): pack + unpack time per layout
+    in HBM, the whole step, and the end-to-end step with the store's arrays in pinned host memory"""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if int(os.environ.get("RANK", 0)) != 0:
+        return
+    import paper_2606_23891_b200 as sph
+    from paper_2606_23891_b200 import layouts
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
+    ps, cells, tasks = build_config1(sph, seed=1)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)
+    sampler = ClockSampler(0)
+    rows = {}
+    for name in layouts.NAMES:
+        w = Workload(sph, torch, ps, cells, tasks, name)
+        t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, 1)
+        t_e2e = time_steps(torch, w.step_e2e, args.steps, args.warmup, flush, 1)
+        per = {k: [] for k, _ in w.launches()}
+        for _ in range(args.steps):
+            flush()
+            evs = []
+            for k, fn in w.launches():
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record()
+                evs.append((k, a, b))
+            torch.cuda.synchronize()
+            for k, a, b in evs:
+                per[k].append(a.elapsed_time(b))
+        per = {k: sum(v) / len(v) for k, v in per.items()}
+        pu = sum(per[k] for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out"))
+        bi, bo = w.e2e_bytes()
+        rows[name] = {"substructs": [int(w.layout.stride[s]) for s in range(w.layout.n_sub)], "ms_per_step": round(sum(t_ms) / len(t_ms), 5),
+                      "pack_unpack_ms": round(pu, 5), "e2e_ms_per_step": round(sum(t_e2e) / len(t_e2e), 5), "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
+                      "kernels_ms": {k: round(v, 5) for k, v in per.items()}}
+        w.close()
+    clocks = sampler.stop()
+    base = rows["aos"]
+    for r in rows.values():
+        r["pack_unpack_vs_aos"] = round(r["pack_unpack_ms"] / base["pack_unpack_ms"], 3)
+        r["e2e_vs_aos"] = round(r["e2e_ms_per_step"] / base["e2e_ms_per_step"], 3)
+    best = min(rows, key=lambda k: rows[k]["e2e_ms_per_step"])
+    n = ps.shape[0]
+    print(json.dumps({"metric": METRIC, "value": n / (rows[best]["ms_per_step"] * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": rows[best]["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": WORKLOAD + "; every particle layout of the paper", "layout": best, "store": "HBM (step) / pinned host (e2e)",
+                                 "l2": "flushed before every step (256 MB fill, untimed)"},
+                      "e2e": {"value": n / (rows[best]["e2e_ms_per_step"] * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": rows[best]["h2d_bytes_per_step"],
+                              "d2h_bytes_per_step": rows[best]["d2h_bytes_per_step"]},
+                      "gpu_launches": 7 * args.steps, "clocks": clocks, "roofline": None, "layouts": rows}))
+
+
 def run_ours(args):
     import torch
+    if args.workload == "layouts":
+        return run_layouts(args)
     if args.workload != "config1":
         return run_other_workload(args)
     rank, world, local = dist_setup(args.gpus)
@@ -507,8 +565,8 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--layout", default="both", choices=["split", "aos", "both"])
-    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4", "link"],
+    ap.add_argument("--layout", default="both", help="split | aos | both, or any layout name of paper_2606_23891_b200/layouts.py")
+    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4", "link", "layouts"],
                     help="config1 = BASELINE.json:configs[1] (the default bench line); the others are described in bench_workloads.py")
     ap.add_argument("--n", type=int, default=0, help="particle count for config2/3/4 (default: the full size of BASELINE.json)")
     ap.add_argument("--skip-zero-copy", action="store_true", help="config4: time the staged pipeline only")

@@ -124,6 +124,13 @@ int32_t sph_layout_aos(sph_layout* out);     /* 1 substruct, the canonical 128-b
 int32_t sph_layout_split(sph_layout* out);   /* S0 {x,h,mass} 32 | S1 {rho,rho_dh,wcount,wcount_dh} 16 | S2 {v,u,P,c_s} 24 |
                                                 S3 {a,du_dt,v_sig} 20 | S4 {id,time_bin} 16 | S5 {div_v,rot_v} 16 */
 int32_t sph_layout_validate(const sph_layout* layout);   /* SPH_ERR_LAYOUT if fields overlap, misaligned or out of stride */
+/* Any other struct split (random-order AoS, the kernel-driven sAoS variants, their splits by data
+ * type): fields [host, n_fields <= SPH_NFIELDS field ids, every field exactly once] are laid out group by group,
+ * group_sizes [host, n_groups <= SPH_MAX_SUB, sum = n_fields]; inside a substruct members follow one another in the given
+ * order at their natural alignment (x, id: 8; time_bin: 1; else 4), the stride is rounded up to the largest member
+ * alignment (at least 4) and to min_stride [host, n_groups strides or NULL] where given (e.g. 128 for a padded AoS record). */
+int32_t sph_layout_from_groups(const uint8_t* fields, uint32_t n_fields, const uint32_t* group_sizes, uint32_t n_groups,
+                               const uint32_t* min_stride, sph_layout* out);
 int32_t sph_attrset_canonical(int32_t which, sph_attrset* out);
 int32_t sph_attrset_record_bytes(const sph_attrset* set, uint32_t* bytes_out);   /* SPH_ERR_LAYOUT: a component listed twice */
 

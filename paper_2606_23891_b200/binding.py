@@ -15,7 +15,7 @@ __all__ = [
     "SphError", "lib_path", "sph_layout", "sph_attr", "sph_attrset", "sph_params", "sph_batch_info", "CELL_DTYPE", "TASK_DTYPE",
     "FIELD", "SPH_ATTR_X_REL_F32", "SPH_MEM_DEVICE", "SPH_MEM_HOST_PINNED", "SPH_UNPACK_REDUCE", "SPH_UNPACK_ASSIGN", "SPH_UNPACK_REDUCE_ZERO",
     "SPH_SET_DENSITY_IN", "SPH_SET_DENSITY_OUT", "SPH_SET_FORCE_IN", "SPH_SET_FORCE_OUT", "EXPORTS",
-    "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_attrset_canonical", "make_attrset",
+    "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_layout_from_groups", "sph_attrset_canonical", "make_attrset",
     "sph_attrset_record_bytes", "sph_store_sub_bytes", "sph_store_create", "sph_store_destroy", "sph_store_import_aos",
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
     "sph_store_upload_range", "sph_store_download_range",
@@ -34,7 +34,7 @@ SPH_SET_DENSITY_IN, SPH_SET_DENSITY_OUT, SPH_SET_FORCE_IN, SPH_SET_FORCE_OUT = 0
 
 #: every symbol include/sph_b200.h declares
 EXPORTS = [
-    "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_attrset_canonical",
+    "sph_last_error", "sph_layout_aos", "sph_layout_split", "sph_layout_validate", "sph_layout_from_groups", "sph_attrset_canonical",
     "sph_attrset_record_bytes", "sph_store_sub_bytes", "sph_store_create", "sph_store_destroy", "sph_store_import_aos",
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
     "sph_store_upload_range", "sph_store_download_range", "sph_pack_cells", "sph_unpack_cells",
@@ -148,6 +148,17 @@ def sph_layout_split() -> sph_layout:
 
 def sph_layout_validate(layout: sph_layout) -> None:
     _check(_lib.sph_layout_validate(C.byref(layout)))
+
+
+def sph_layout_from_groups(groups, min_stride=None) -> sph_layout:
+    """groups: list of lists of field ids or names, every field exactly once; min_stride: optional stride floor per group"""
+    flat = np.array([FIELD[f] if isinstance(f, str) else int(f) for g in groups for f in g], dtype=np.uint8)
+    sizes = np.array([len(g) for g in groups], dtype=np.uint32)
+    ms = None if min_stride is None else np.ascontiguousarray(min_stride, dtype=np.uint32)
+    out = sph_layout()
+    _check(_lib.sph_layout_from_groups(_ptr(flat), C.c_uint32(flat.shape[0]), _ptr(sizes), C.c_uint32(sizes.shape[0]),
+                                       _ptr(ms) if ms is not None else None, C.byref(out)))
+    return out
 
 
 def sph_attrset_canonical(which: int) -> sph_attrset:

@@ -220,6 +220,37 @@ int32_t sph_layout_split(sph_layout* out) {
     return SPH_OK;
 }
 
+int32_t sph_layout_from_groups(const uint8_t* fields, uint32_t n_fields, const uint32_t* group_sizes, uint32_t n_groups,
+                               const uint32_t* min_stride, sph_layout* out) {
+    if (!fields || !group_sizes || !out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    if (n_fields != SPH_NFIELDS) return fail(SPH_ERR_LAYOUT, "%u fields listed, every one of the %d must appear once", n_fields, SPH_NFIELDS);
+    if (n_groups < 1 || n_groups > SPH_MAX_SUB) return fail(SPH_ERR_LAYOUT, "n_groups = %u (1..%d)", n_groups, SPH_MAX_SUB);
+    bool seen[SPH_NFIELDS] = {};
+    std::memset(out, 0, sizeof(*out));
+    out->n_sub = n_groups;
+    uint32_t k = 0;
+    for (uint32_t g = 0; g < n_groups; ++g) {
+        uint32_t off = 0, max_align = 4;
+        if (group_sizes[g] == 0) return fail(SPH_ERR_LAYOUT, "group %u is empty", g);
+        for (uint32_t i = 0; i < group_sizes[g]; ++i, ++k) {
+            if (k >= n_fields) return fail(SPH_ERR_LAYOUT, "group sizes exceed the field list");
+            const int f = fields[k];
+            if (f >= SPH_NFIELDS || seen[f]) return fail(SPH_ERR_LAYOUT, "field %d is unknown or listed twice", f);
+            seen[f] = true;
+            const uint32_t eb = field_elem_bytes(f), align = f == SPH_TIME_BIN ? 1 : (eb == 8 ? 8 : 4);
+            off = (off + align - 1) / align * align;
+            set_loc(out, f, g, off);
+            off += eb * field_ncomp(f);
+            max_align = std::max(max_align, align);
+        }
+        uint32_t stride = (off + max_align - 1) / max_align * max_align;
+        if (min_stride && min_stride[g] > stride) stride = (min_stride[g] + max_align - 1) / max_align * max_align;
+        out->stride[g] = stride;
+    }
+    if (k != n_fields) return fail(SPH_ERR_LAYOUT, "group sizes cover %u of %u fields", k, n_fields);
+    return sph_layout_validate(out);
+}
+
 int32_t sph_layout_validate(const sph_layout* l) {
     if (!l) return fail(SPH_ERR_INVALID_ARG, "layout is NULL");
     if (l->n_sub < 1 || l->n_sub > SPH_MAX_SUB) return fail(SPH_ERR_LAYOUT, "n_sub = %u (1..%d)", l->n_sub, SPH_MAX_SUB);

@@ -117,6 +117,36 @@ def test_pack_bit_exact(name, layout):
     g.close()
 
 
+@pytest.mark.parametrize("variant", ["random-order", "pack-density", "pack-force", "pack-density-type", "pack-force-type"])
+def test_paper_layout_variants_bit_exact(variant):
+    """The paper's other layouts run through the same kernels: import / export, pack and unpack are
+    byte-identical to the oracle's whatever the store's layout."""
+    from paper_2606_23891_b200 import layouts
+    ps, cells, tasks = case("ragged")
+    g = GpuCase(ps, cells, tasks, layouts.layout(sph, variant, seed=5))
+    assert np.array_equal(canon(g.export()), canon(ps))
+    for oset in (orc.DENSITY_IN, orc.FORCE_IN, sweep_set(PACK_SWEEP, 20, orc.FLAG_X_REL_F32)):
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        ref = orc.pack(ps, cells, tasks, oset)
+        off_o, total = orc.block_offsets(cells, tasks, rec)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        got = g.pack(aset).cpu().numpy()
+        m = valid_mask(off_o, cells, tasks, rec, total)
+        assert np.array_equal(got[m], ref[m]), (variant, rec)
+    for n_set, (oset, mode) in enumerate([(orc.DENSITY_OUT, orc.MODE_REDUCE), (orc.FORCE_OUT, orc.MODE_REDUCE), (sweep_set(UNPACK_SWEEP, 20, 0), orc.MODE_REDUCE),
+                                          (orc.FORCE_OUT, orc.MODE_ASSIGN)]):
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        _, total = orc.block_offsets(cells, tasks, rec)
+        buf = _random_result_buffer(total, 500 + n_set)
+        ref = raw_copy(ps)
+        orc.unpack(ref, cells, tasks, oset, buf, mode)
+        sph.sph_store_import_aos(g.store, ps)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        sph.sph_unpack(g.store, g.batch, aset, torch.from_numpy(buf).cuda(), mode)
+        assert np.array_equal(canon(g.export()), canon(ref)), (variant, rec, mode)
+    g.close()
+
+
 # ------------------------------------------------------------------ loops
 
 def _density_tol(ref4, got4, h, m_unit):

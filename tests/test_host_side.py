@@ -62,6 +62,37 @@ def test_layouts():
         sph.sph_layout_validate(bad)
 
 
+def test_paper_layout_variants():
+    """random-order AoS, kernel-driven sAoS variants and their splits by type, via sph_layout_from_groups"""
+    from paper_2606_23891_b200 import layouts
+    sizes = {"x": 24, "v": 12, "a": 12, "rot_v": 12, "id": 8, "time_bin": 1}
+    for name in layouts.NAMES:
+        lay = layouts.layout(sph, name, seed=3)
+        sph.sph_layout_validate(lay)
+        spans = {}
+        for fname, f in sph.FIELD.items():
+            loc = lay.loc[f]
+            nb = sizes.get(fname, 4)
+            assert loc.sub < lay.n_sub and loc.off + nb <= lay.stride[loc.sub], (name, fname)
+            spans.setdefault(loc.sub, []).append((loc.off, loc.off + nb))
+        for sub, sp in spans.items():                      # no two members overlap
+            sp.sort()
+            assert all(a[1] <= b[0] for a, b in zip(sp[:-1], sp[1:])), (name, sub)
+    # the density inputs of pack-force live in the 64-byte force struct; pack-density keeps them in a 32-byte one
+    pf, pd = layouts.layout(sph, "pack-force"), layouts.layout(sph, "pack-density")
+    assert pf.stride[pf.loc[sph.FIELD["x"]].sub] == 64 and pd.stride[pd.loc[sph.FIELD["x"]].sub] == 32
+    assert {pf.loc[sph.FIELD[k]].sub for k in ("x", "h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s")} == {0}
+    ro = layouts.layout(sph, "random-order", seed=3)
+    assert ro.n_sub == 1 and ro.stride[0] == 128
+    assert [ro.loc[f].off for f in range(18)] != [sph.sph_layout_aos().loc[f].off for f in range(18)]
+    with pytest.raises(sph.SphError):                      # a field twice
+        sph.sph_layout_from_groups([["x", "x"] + layouts.AOS_ORDER[2:]])
+    with pytest.raises(sph.SphError):                      # a field missing
+        sph.sph_layout_from_groups([layouts.AOS_ORDER[:-1]])
+    with pytest.raises(sph.SphError):                      # more substructs than SPH_MAX_SUB
+        sph.sph_layout_from_groups([[f] for f in layouts.AOS_ORDER[:9]] + [layouts.AOS_ORDER[9:]])
+
+
 def test_attribute_sets():
     for which, rec, oset in [(sph.SPH_SET_DENSITY_IN, 20, orc.DENSITY_IN), (sph.SPH_SET_DENSITY_OUT, 16, orc.DENSITY_OUT),
                              (sph.SPH_SET_FORCE_IN, 52, orc.FORCE_IN), (sph.SPH_SET_FORCE_OUT, 20, orc.FORCE_OUT)]:
