@@ -463,6 +463,67 @@ __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree,
     return fma2(kThree, mul2(u, u), mul2(kM075, mul2(t, t)));
 }
 
+// The force terms of two (target, neighbour) pairs in packed f32x2 arithmetic (lo: first pair, hi: second pair).
+// e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j) is the same number and
+// a_i += -m (..) (x_i - x_j) / r becomes one fma with e:  a_i += fr * e,  du_i += dg * vr,  v_sig_i = max(v_sig_i, vs).
+struct ForceTargets2 {      // the targets' constants, one target per half
+    u64 x, y, z, vx, vy, vz, cs, inv_h, n4, rho, A;
+    float hc2a, hc2b;       // (2 h_i)^2
+};
+struct ForcePair2 {
+    u64 fr, ex, ey, ez, dg, vr;
+    float vsa, vsb;         // the pair's signal velocity, 0 for a miss
+};
+struct ForceConsts2 {
+    u64 two, one, three, m075, half, mhalf, onehalf, invpi, mbeta, malpha;
+};
+__device__ __forceinline__ ForcePair2 force_pair2(const ForceTargets2& T, const ForceConsts2& K, const float4& a, const float4& b,
+                                                  const float4& va, const float4& vb, const float4& ca, const float4& cb) {
+    ForcePair2 o;
+    o.ex = sub2(pack2(a.x, b.x), T.x); o.ey = sub2(pack2(a.y, b.y), T.y); o.ez = sub2(pack2(a.z, b.z), T.z);
+    const u64 r2 = fma2(o.ez, o.ez, fma2(o.ey, o.ey, mul2(o.ex, o.ex)));
+    float r2a, r2b;
+    unpack2(r2, r2a, r2b);
+    // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
+    // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
+    const bool hitA = r2a < fmaxf(T.hc2a, a.w) && r2a > 0.f, hitB = r2b < fmaxf(T.hc2b, b.w) && r2b > 0.f;
+    r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
+    const u64 r2s = pack2(r2a, r2b);
+    u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
+    rinv = mul2(rinv, fma2(mul2(mul2(K.mhalf, r2s), rinv), rinv, K.onehalf));      // one Newton step: ~1 ulp
+    const u64 r = mul2(r2s, rinv);
+    const u64 ihj = pack2(ca.w, cb.w);
+    const u64 Gi = mul2(spline_dw2(mul2(r, T.inv_h), K.two, K.one, K.three, K.m075), T.n4);
+    const u64 ih2 = mul2(ihj, ihj);
+    const u64 Gj = mul2(spline_dw2(mul2(r, ihj), K.two, K.one, K.three, K.m075), mul2(mul2(ih2, ih2), K.invpi));
+    const u64 wx = sub2(pack2(va.x, vb.x), T.vx), wy = sub2(pack2(va.y, vb.y), T.vy), wz = sub2(pack2(va.z, vb.z), T.vz);
+    o.vr = mul2(fma2(wz, o.ez, fma2(wy, o.ey, mul2(wx, o.ex))), rinv);
+    float vra, vrb;
+    unpack2(o.vr, vra, vrb);
+    const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
+    const u64 vs = fma2(K.mbeta, mu, add2(T.cs, pack2(ca.z, cb.z)));
+    float rsa, rsb, vsa, vsb;
+    unpack2(add2(T.rho, pack2(ca.x, cb.x)), rsa, rsb);
+    unpack2(vs, vsa, vsb);
+    const u64 visc = mul2(mul2(mul2(K.malpha, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
+    const u64 vG = mul2(mul2(visc, K.half), add2(Gi, Gj));
+    const u64 AG = mul2(T.A, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
+    const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
+    o.fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
+    o.dg = mul2(mm, fma2(K.half, vG, AG));
+    o.vsa = hitA ? vsa : 0.f; o.vsb = hitB ? vsb : 0.f;
+    return o;
+}
+
+// sum += a * b with the rounding error of the addition carried in c (Kahan), for a pair of sums
+__device__ __forceinline__ void kahan2(u64& sum, u64& c, u64 a, u64 b) {
+    const u64 y = fma2(a, b, c);          // c holds minus the error so far
+    const u64 t = add2(sum, y);
+    c = sub2(y, sub2(t, sum));            // y - (t - sum): what the addition dropped
+    sum = t;
+}
+
+template <bool UNITS>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
     extern __shared__ __align__(16) unsigned char s_raw[];
@@ -477,8 +538,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         sm.tb[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
         sm.tc[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    const u64 kTwo = dup2(2.0f), kOne = dup2(1.0f), kThree = dup2(3.0f), kM075 = dup2(-0.75f), kHalf2 = dup2(0.5f), kMHalf2 = dup2(-0.5f),
-              kOneHalf2 = dup2(1.5f), kInvPi2 = dup2(kInvPi), kMBeta2 = dup2(-beta), kMAlpha2 = dup2(-alpha);
+    const ForceConsts2 K{dup2(2.0f), dup2(1.0f), dup2(3.0f), dup2(-0.75f), dup2(0.5f), dup2(-0.5f), dup2(1.5f), dup2(kInvPi), dup2(-beta), dup2(-alpha)};
 
     uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
     FetchGroup fg{&sm.bar[0], 0u};
@@ -543,144 +603,131 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - cutB - kFilterEps * (b2 + cutB) : kNever);
             uint32_t m[4];
             if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
-            __syncwarp();     // the filter has read sm.f: its first bytes now hold the unit list
-
-            // Phase 2 in UNITS of up to four neighbours of one target.  Inside a cell pair the number of neighbours per target is
-            // heavy-tailed (0 .. ~30: targets next to the other cell against targets three layers away), so a lane that walks its
-            // own target's neighbours leaves most of the warp idle.  Instead:
-            //   (a) every lane cuts its targets' hit masks into units (target, <= 4 tile entries); a warp prefix sum numbers them;
-            //   (b) the units are evaluated 32 at a time, one per lane, two neighbours per iteration in packed f32x2 arithmetic
-            //       (at most two iterations), each unit leaving its partial sums in shared memory;
-            //   (c) the lane that made a unit adds its partial sums to the target's running sums, in unit order (= source order,
-            //       so the result does not depend on how units fell on lanes), a with compensated (Kahan) adds.
-            // kUnitCap units are in flight at a time; a flush with more takes several windows.
-            uint32_t* upos = reinterpret_cast<uint32_t*>(&sm.f);                        // [kUnitCap] the unit's (up to) four bits of a mask word
-            unsigned char* utgt = reinterpret_cast<unsigned char*>(upos + kUnitCap);    // [kUnitCap] the unit's target
-            float4* part_a = reinterpret_cast<float4*>(sm.raw + 320);                   // [kUnitCap] a (3), du
-            float* part_v = sm.raw + 320 + 4 * kUnitCap;                                // [kUnitCap] v_sig
-            const uint32_t nuA = ((__popc(m[0]) + 3) >> 2) + ((__popc(m[1]) + 3) >> 2), nuB = ((__popc(m[2]) + 3) >> 2) + ((__popc(m[3]) + 3) >> 2);
-            const uint32_t nu = nuA + nuB;
-            float axA = 0.f, ayA = 0.f, azA = 0.f, duA = 0.f, cxA = 0.f, cyA = 0.f, czA = 0.f, vsA = 0.f;
-            float axB = 0.f, ayB = 0.f, azB = 0.f, duB = 0.f, cxB = 0.f, cyB = 0.f, czB = 0.f, vsB = 0.f;
-            uint32_t cw = 0, mw = m[0];                 // the mask word being cut (0, 1: target A; 2, 3: target B) and what is left of it
-            const uint32_t m1 = m[1], m2 = m[2], m3 = m[3];
-            const uint32_t max_nu = __reduce_max_sync(kFull, nu);
-            // Units are numbered RANK-major (all lanes' first units, then all second units, ...): making the units and adding
-            // up their partial sums then takes as many warp-wide steps as the busiest lane has units, whatever the spread.
-            for (uint32_t r = 0; r < max_nu;) {
-                // (a) the next ranks, as many as fit into a window of kUnitCap units
-                const uint32_t r0 = r;
-                uint32_t cum = 0;
-                while (r < max_nu) {
-                    const uint32_t bal = __ballot_sync(kFull, nu > r), n_r = __popc(bal);
-                    if (cum + n_r > (uint32_t)kUnitCap) break;
-                    if (nu > r) {
-                        while (mw == 0) { ++cw; mw = cw == 1 ? m1 : (cw == 2 ? m2 : m3); }
-                        // the unit = the word's next (up to) four set bits, as a mask; the evaluating lane decodes them
-                        const uint32_t before = mw;
+            // Phase 2, two ways (two instantiations of the kernel; the launcher picks one from the batch's mean block size).
+            //  WALK: every lane walks the set bits of its own targets' masks, one neighbour of target A and one of target B per
+            //        iteration (or two of target A when it has one target).  Best when the targets have about as many neighbours
+            //        each (a cell against itself, large cells).
+            //  UNITS: inside a pair of small cells the number of neighbours per target is heavy-tailed (0 .. ~30: targets next to
+            //        the other cell against targets three layers away) and walking leaves most of the warp idle.  Instead
+            //        (a) every lane cuts its masks into units (target, <= 4 set bits of one mask word), numbered RANK-major over the
+            //            lanes (all first units, then all second units, ...: making the units, and adding up their partial sums,
+            //            takes as many warp steps as the busiest lane has units);
+            //        (b) the units are evaluated 32 at a time, one per lane, each leaving its partial sums in shared memory;
+            //        (c) the lane that made a unit adds its partial sums to the target's running sums, in unit order.
+            // Acceleration sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan)
+            // adds keep the rounding of the running sums out of the 1e-6 max|a| budget, in both ways.
+            const uint32_t cA0 = __popc(m[0]), cA1 = __popc(m[1]), cB0 = __popc(m[2]), cB1 = __popc(m[3]);
+            const uint32_t nuA = ((cA0 + 3) >> 2) + ((cA1 + 3) >> 2), nuB = ((cB0 + 3) >> 2) + ((cB1 + 3) >> 2), nu = nuA + nuB;
+            float axA = 0.f, ayA = 0.f, azA = 0.f, duA = 0.f, vsA = 0.f, axB = 0.f, ayB = 0.f, azB = 0.f, duB = 0.f, vsB = 0.f;
+            if constexpr (!UNITS) {
+                const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
+                const ForceTargets2 T{pack2(pA.x, pB.x), pack2(pA.y, pB.y), pack2(pA.z, pB.z), pack2(qA.x, qB.x), pack2(qA.y, qB.y), pack2(qA.z, qB.z),
+                                      pack2(qA.w, qB.w), pack2(sA.x, sB.x), pack2(sA.y, sB.y), pack2(sA.z, sB.z), pack2(sA.w, sB.w), pA.w, pB.w};
+                u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
+                float vsig0 = 0.f, vsig1 = 0.f;
+                auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
+                    uint32_t ja, jb;
+                    while (next_hits(dual, ma, mb, &ja, &jb)) {
+                        const ForcePair2 o = force_pair2(T, K, sm.ta[base + ja], sm.ta[base + jb], sm.tb[base + ja], sm.tb[base + jb], sm.tc[base + ja], sm.tc[base + jb]);
+                        kahan2(ax, cx, o.fr, o.ex); kahan2(ay, cy, o.fr, o.ey); kahan2(az, cz, o.fr, o.ez);
+                        du = fma2(o.dg, o.vr, du);
+                        vsig0 = fmaxf(vsig0, o.vsa); vsig1 = fmaxf(vsig1, o.vsb);
+                    }
+                };
+                hits(m[0], m[2], 0);
+                if (cnt > 32) hits(m[1], m[3], kHalf);
+                unpack2(ax, axA, axB); unpack2(ay, ayA, ayB); unpack2(az, azA, azB); unpack2(du, duA, duB);
+                vsA = vsig0; vsB = vsig1;
+                if (!dual) { axA += axB; ayA += ayB; azA += azB; duA += duB; vsA = fmaxf(vsA, vsB); }
+            } else {
+                const uint32_t max_nu = __reduce_max_sync(kFull, nu);
+                __syncwarp();     // the filter has read sm.f: its first bytes now hold the unit list
+                uint32_t* upos = reinterpret_cast<uint32_t*>(&sm.f);                        // [kUnitCap] the unit's (up to) four bits of a mask word
+                unsigned char* utgt = reinterpret_cast<unsigned char*>(upos + kUnitCap);    // [kUnitCap] the unit's target | tile half << 7
+                float4* part_a = reinterpret_cast<float4*>(sm.raw + 320);                   // [kUnitCap] a (3), du
+                float* part_v = sm.raw + 320 + 4 * kUnitCap;                                // [kUnitCap] v_sig
+                float cxA = 0.f, cyA = 0.f, czA = 0.f, cxB = 0.f, cyB = 0.f, czB = 0.f;
+                uint32_t cw = 0, mw = m[0];             // the mask word being cut (0, 1: target A; 2, 3: target B) and what is left of it
+                const uint32_t m1 = m[1], m2 = m[2], m3 = m[3];
+                for (uint32_t r = 0; r < max_nu;) {
+                    // (a) the next ranks, as many as fit into a window of kUnitCap units
+                    const uint32_t r0 = r;
+                    uint32_t cum = 0;
+                    while (r < max_nu) {
+                        const uint32_t bal = __ballot_sync(kFull, nu > r), n_r = __popc(bal);
+                        if (cum + n_r > (uint32_t)kUnitCap) break;
+                        if (nu > r) {
+                            while (mw == 0) { ++cw; mw = cw == 1 ? m1 : (cw == 2 ? m2 : m3); }
+                            const uint32_t before = mw;
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) mw &= ~shr_clamp(0x80000000u, __clz(mw));      // __clz(0) = 32: the shift gives 0, nothing cleared
-                        const uint32_t pos = before ^ mw;
-                        const uint32_t idx = cum + __popc(bal & lt);
-                        upos[idx] = pos;
-                        utgt[idx] = (unsigned char)((r < nuA ? tA : tB) | ((cw & 1) << 7));      // bit 7: the tile's second half
+                            for (int q = 0; q < 4; ++q) mw &= ~shr_clamp(0x80000000u, __clz(mw));      // __clz(0) = 32: the shift gives 0, nothing cleared
+                            const uint32_t idx = cum + __popc(bal & lt);
+                            upos[idx] = before ^ mw;
+                            utgt[idx] = (unsigned char)((r < nuA ? tA : tB) | ((cw & 1) << 7));
+                        }
+                        cum += n_r; ++r;
                     }
-                    cum += n_r; ++r;
-                }
-                __syncwarp();
+                    __syncwarp();
 
-                // (b) evaluation.  e = x_j - x_i and v_j - v_i are used (both signs flipped): (v_i - v_j).(x_i - x_j) is the same
-                // number and a_i += -m (..) (x_i - x_j) / r becomes one fma with e.
-                for (uint32_t u0 = 0; u0 < cum; u0 += 32) {
-                    const uint32_t u = u0 + lane;
-                    const bool valid = u < cum;
-                    uint32_t um = valid ? upos[u] : 0u;
-                    const uint32_t tw = valid ? utgt[u] : 0u, t = tw & 127u, ebase = (tw >> 7) * kHalf;
-                    uint32_t e[4];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
+                    // (b) evaluation: both halves of the packed arithmetic serve the unit's target
+                    for (uint32_t u0 = 0; u0 < cum; u0 += 32) {
+                        const uint32_t u = u0 + lane;
+                        const bool valid = u < cum;
+                        uint32_t um = valid ? upos[u] : 0u;
+                        const uint32_t tw = valid ? utgt[u] : 0u, t = tw & 127u, ebase = (tw >> 7) * kHalf;
+                        uint32_t e[4];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const uint32_t j = __clz(um);
-                        um &= ~shr_clamp(0x80000000u, j);
-                        e[q] = ebase + j;
-                    }
-                    const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
-                    const u64 x2 = dup2(P.x), y2 = dup2(P.y), z2 = dup2(P.z), vx2 = dup2(Q.x), vy2 = dup2(Q.y), vz2 = dup2(Q.z), c2 = dup2(Q.w);
-                    const u64 inv_h2 = dup2(S.x), n42 = dup2(S.y), rho2 = dup2(S.z), A2 = dup2(S.w);
-                    u64 ax = 0, ay = 0, az = 0, du = 0;
-                    float vsig0 = 0.f, vsig1 = 0.f;
-                    auto two = [&](uint32_t ja, uint32_t jb) {
-                        const float4 a = sm.ta[ja], b = sm.ta[jb];
-                        const u64 ex = sub2(pack2(a.x, b.x), x2), ey = sub2(pack2(a.y, b.y), y2), ez = sub2(pack2(a.z, b.z), z2);
-                        const u64 r2 = fma2(ez, ez, fma2(ey, ey, mul2(ex, ex)));
-                        float r2a, r2b;
-                        unpack2(r2, r2a, r2b);
-                        // the exact cut-off; r = 0 is the particle itself.  A miss (filter false positive, dummy) is carried along
-                        // with r^2 = 1 and mass 0: every term stays finite and contributes exactly zero.
-                        const bool hitA = r2a < fmaxf(P.w, a.w) && r2a > 0.f, hitB = r2b < fmaxf(P.w, b.w) && r2b > 0.f;
-                        r2a = hitA ? r2a : 1.0f; r2b = hitB ? r2b : 1.0f;
-                        const u64 r2s = pack2(r2a, r2b);
-                        u64 rinv = pack2(rsqrtf(r2a), rsqrtf(r2b));
-                        rinv = mul2(rinv, fma2(mul2(mul2(kMHalf2, r2s), rinv), rinv, kOneHalf2));      // one Newton step: ~1 ulp
-                        const u64 rr = mul2(r2s, rinv);
-                        const float4 va = sm.tb[ja], vb = sm.tb[jb], ca = sm.tc[ja], cb = sm.tc[jb];
-                        const u64 ihj = pack2(ca.w, cb.w);
-                        const u64 Gi = mul2(spline_dw2(mul2(rr, inv_h2), kTwo, kOne, kThree, kM075), n42);
-                        const u64 ih2 = mul2(ihj, ihj);
-                        const u64 Gj = mul2(spline_dw2(mul2(rr, ihj), kTwo, kOne, kThree, kM075), mul2(mul2(ih2, ih2), kInvPi2));
-                        const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
-                        const u64 vr = mul2(fma2(wz, ez, fma2(wy, ey, mul2(wx, ex))), rinv);
-                        float vra, vrb;
-                        unpack2(vr, vra, vrb);
-                        const u64 mu = pack2(fminf(vra, 0.f), fminf(vrb, 0.f));
-                        const u64 vs = fma2(kMBeta2, mu, add2(c2, pack2(ca.z, cb.z)));
-                        float rsa, rsb, vsa, vsb;
-                        unpack2(add2(rho2, pack2(ca.x, cb.x)), rsa, rsb);
-                        unpack2(vs, vsa, vsb);
-                        const u64 visc = mul2(mul2(mul2(kMAlpha2, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
-                        const u64 vG = mul2(mul2(visc, kHalf2), add2(Gi, Gj));
-                        const u64 AG = mul2(A2, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
-                        const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
-                        const u64 fr = mul2(mul2(mm, add2(add2(AG, BG), vG)), rinv);
-                        ax = fma2(fr, ex, ax); ay = fma2(fr, ey, ay); az = fma2(fr, ez, az);
-                        du = fma2(mul2(mm, fma2(kHalf2, vG, AG)), vr, du);
-                        vsig0 = fmaxf(vsig0, hitA ? vsa : 0.f); vsig1 = fmaxf(vsig1, hitB ? vsb : 0.f);
-                    };
-                    two(e[0], e[1]);
-                    if (__any_sync(kFull, e[2] != ebase + 32u)) two(e[2], e[3]);
-                    if (valid) {
-                        float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
-                        unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
-                        part_a[u] = make_float4(ax0 + ax1, ay0 + ay1, az0 + az1, du0 + du1);
-                        part_v[u] = fmaxf(vsig0, vsig1);
-                    }
-                }
-                __syncwarp();
-
-                // (c) a sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan)
-                // adds keep the rounding of the running sums out of the 1e-6 max|a| budget
-                uint32_t c2 = 0;
-                for (uint32_t q = r0; q < r; ++q) {
-                    const uint32_t bal = __ballot_sync(kFull, nu > q);
-                    if (nu > q) {
-                        const uint32_t idx = c2 + __popc(bal & lt);
-                        const float4 pa = part_a[idx];
-                        const float pv = part_v[idx];
-                        float y, t;
-                        if (q < nuA) {
-                            y = pa.x + cxA; t = axA + y; cxA = y - (t - axA); axA = t;      // c holds minus the error so far
-                            y = pa.y + cyA; t = ayA + y; cyA = y - (t - ayA); ayA = t;
-                            y = pa.z + czA; t = azA + y; czA = y - (t - azA); azA = t;
-                            duA += pa.w; vsA = fmaxf(vsA, pv);
-                        } else {
-                            y = pa.x + cxB; t = axB + y; cxB = y - (t - axB); axB = t;
-                            y = pa.y + cyB; t = ayB + y; cyB = y - (t - ayB); ayB = t;
-                            y = pa.z + czB; t = azB + y; czB = y - (t - azB); azB = t;
-                            duB += pa.w; vsB = fmaxf(vsB, pv);
+                        for (int q = 0; q < 4; ++q) {
+                            const uint32_t j = __clz(um);
+                            um &= ~shr_clamp(0x80000000u, j);
+                            e[q] = ebase + j;
+                        }
+                        const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
+                        const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w};
+                        u64 ax = 0, ay = 0, az = 0, du = 0;
+                        float vsig = 0.f;
+                        auto two = [&](uint32_t ja, uint32_t jb) {
+                            const ForcePair2 o = force_pair2(T, K, sm.ta[ja], sm.ta[jb], sm.tb[ja], sm.tb[jb], sm.tc[ja], sm.tc[jb]);
+                            ax = fma2(o.fr, o.ex, ax); ay = fma2(o.fr, o.ey, ay); az = fma2(o.fr, o.ez, az);
+                            du = fma2(o.dg, o.vr, du);
+                            vsig = fmaxf(vsig, fmaxf(o.vsa, o.vsb));
+                        };
+                        two(e[0], e[1]);
+                        if (__any_sync(kFull, e[2] != ebase + 32u)) two(e[2], e[3]);
+                        if (valid) {
+                            float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
+                            unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
+                            part_a[u] = make_float4(ax0 + ax1, ay0 + ay1, az0 + az1, du0 + du1);
+                            part_v[u] = vsig;
                         }
                     }
-                    c2 += __popc(bal);
+                    __syncwarp();
+
+                    // (c) partial sums -> the targets' running sums
+                    uint32_t c2 = 0;
+                    for (uint32_t q = r0; q < r; ++q) {
+                        const uint32_t bal = __ballot_sync(kFull, nu > q);
+                        if (nu > q) {
+                            const uint32_t idx = c2 + __popc(bal & lt);
+                            const float4 pa = part_a[idx];
+                            const float pv = part_v[idx];
+                            float y, t;
+                            if (q < nuA) {
+                                y = pa.x + cxA; t = axA + y; cxA = y - (t - axA); axA = t;      // c holds minus the error so far
+                                y = pa.y + cyA; t = ayA + y; cyA = y - (t - ayA); ayA = t;
+                                y = pa.z + czA; t = azA + y; czA = y - (t - azA); azA = t;
+                                duA += pa.w; vsA = fmaxf(vsA, pv);
+                            } else {
+                                y = pa.x + cxB; t = axB + y; cxB = y - (t - axB); axB = t;
+                                y = pa.y + cyB; t = ayB + y; cyB = y - (t - ayB); ayB = t;
+                                y = pa.z + czB; t = azB + y; czB = y - (t - azB); azB = t;
+                                duB += pa.w; vsB = fmaxf(vsB, pv);
+                            }
+                        }
+                        c2 += __popc(bal);
+                    }
+                    __syncwarp();     // the unit list and the partial sums are rewritten by the next window / flush
                 }
-                __syncwarp();     // the unit list and the partial sums are rewritten by the next window / flush
             }
             if (wA) { float* o = sm.raw + 5 * tA; o[0] += axA; o[1] += ayA; o[2] += azA; o[3] += duA; o[4] = fmaxf(o[4], vsA); }
             if (wB) { float* o = sm.raw + 5 * tB; o[0] += axB; o[1] += ayB; o[2] += azB; o[3] += duB; o[4] = fmaxf(o[4], vsB); }
@@ -758,14 +805,22 @@ int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaSt
     return SPH_OK;
 }
 
+#ifndef SPH_UNITS_MAX_MEAN_BLOCK
+#define SPH_UNITS_MAX_MEAN_BLOCK 80
+#endif
+
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
     if (b->n_chunks == 0) return SPH_OK;
-    static uint32_t full_grid = 0;
+    static uint32_t full_grid[2] = {0, 0};
     constexpr size_t smem = sizeof(ForceWarpSmem) * kLoopWarps;
-    if (!full_grid)
-        if (int32_t rc = loop_grid(force_kernel, smem, &full_grid)) return rc;
-    const uint32_t grid = min((b->n_chunks + kLoopWarps - 1) / kLoopWarps, full_grid);
-    force_kernel<<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_chunks, prm.alpha, prm.beta);
+    // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
+    // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
+    const bool units = b->n_sides && b->n_instances <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * b->n_sides;
+    if (!full_grid[units])
+        if (int32_t rc = units ? loop_grid(force_kernel<true>, smem, &full_grid[1]) : loop_grid(force_kernel<false>, smem, &full_grid[0])) return rc;
+    const uint32_t grid = min((b->n_chunks + kLoopWarps - 1) / kLoopWarps, full_grid[units]);
+    if (units) force_kernel<true><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_chunks, prm.alpha, prm.beta);
+    else force_kernel<false><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_chunks, prm.alpha, prm.beta);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

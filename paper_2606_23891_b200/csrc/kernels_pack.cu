@@ -21,8 +21,17 @@ namespace sph {
 
 namespace {
 
-constexpr int kPackWarps = 4;
-constexpr int kUnpackWarps = 2;
+#ifndef SPH_PACK_WARPS
+#define SPH_PACK_WARPS 4
+#endif
+#ifndef SPH_PACK_K
+#define SPH_PACK_K 4
+#endif
+#ifndef SPH_UNPACK_WARPS
+#define SPH_UNPACK_WARPS 2
+#endif
+constexpr int kPackWarps = SPH_PACK_WARPS;
+constexpr int kUnpackWarps = SPH_UNPACK_WARPS;
 
 template <int BYTES>
 __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
@@ -67,7 +76,7 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 
-constexpr int kPackK = 2;                      // record-stream templates per set; two sets alternate
+constexpr int kPackK = SPH_PACK_K;                      // record-stream templates per set; two sets alternate
 constexpr uint32_t kPackTableOcc = 32;         // occurrences whose block offsets and frames are staged at a time
 constexpr uint32_t kPackTableBytes = kPackTableOcc * (4 + 24);
 
