@@ -171,6 +171,7 @@ class Workload:
         from paper_2606_23891_b200 import layouts as _layouts
         self.layout = _layouts.layout(sph, layout_name)
         self.n = ps.shape[0]
+        self.cells = cells
         self.store = sph.sph_store_create(self.layout, self.n)
         sph.sph_store_import_aos(self.store, ps)
         sph.sph_store_set_cells(self.store, cells)
@@ -218,8 +219,8 @@ class Workload:
     def step_e2e(self, stream=None):
         """The step with the particle arrays in pinned HOST memory.  Uploads run on a copy stream ahead of the kernels that need
         them, downloads on a second one as soon as a substruct holds its final values, so that with split-AoS the force
-        inputs cross during the density loop and the density results during the force loop; with AoS (one substruct) there is
-        nothing to overlap.  The calling stream waits for the last download: its events bracket the whole step."""
+        inputs cross during the density loop and the density results during the force loop; the first pack and the last unpack
+        are streamed in four slabs of cells (sph_pack_cells / sph_unpack_cells) against their copies.  The calling stream waits for the last download: its events bracket the whole step."""
         torch, sph = self.torch, self.sph
         main = stream if stream is not None else torch.cuda.current_stream()
         if not hasattr(self, "_e2e"):
@@ -229,6 +230,8 @@ class Workload:
             d_out, g_out, f_out = sub(("rho", "rho_dh", "wcount", "wcount_dh")), sub(("P", "c_s")), sub(("a", "du_dt", "v_sig"))
             self._e2e = {"up": torch.cuda.Stream(), "down": torch.cuda.Stream(), "up1": sorted(d_in), "up2": sorted(f_in - d_in),
                          "down1": sorted(d_out - g_out - f_out), "down2": sorted(g_out - f_out), "down3": sorted(f_out)}
+            from bench_workloads import cell_slabs
+            self._e2e["slabs"] = cell_slabs(self.cells, 4)
         E = self._e2e
         up, down = E["up"], E["down"]
         ev = lambda st: (lambda e: (e.record(st), e)[1])(torch.cuda.Event())
@@ -236,14 +239,17 @@ class Workload:
         start = ev(main)
         up.wait_event(start)
         down.wait_event(start)
-        for s in E["up1"]:
-            sph.sph_store_upload_sub(self.store, s, self.host[s], up)
-        e1 = ev(up)
+        # the density inputs cross slab by slab (ranges of cells); each slab is packed as soon as it is there
+        S, B, st, b = self.sets, self.bufs, self.store, self.batch
+        for c0, nc, p0, npart in E["slabs"]:
+            for s in E["up1"]:
+                sph.sph_store_upload_range(st, s, self.host[s], p0, npart, up)
+            main.wait_event(ev(up))
+            sph.sph_pack_cells(st, b, S[0], B[0], c0, nc, main)
         for s in E["up2"]:
             sph.sph_store_upload_sub(self.store, s, self.host[s], up)
         e2 = ev(up)
-        main.wait_event(e1)
-        for k in ("pack_density_in", "density", "unpack_density_out"):
+        for k in ("density", "unpack_density_out"):
             L[k]()
         down.wait_event(ev(main))
         for s in E["down1"]:
@@ -253,12 +259,28 @@ class Workload:
         down.wait_event(ev(main))
         for s in E["down2"]:
             sph.sph_store_download_sub(self.store, s, self.host[s], down)
-        for k in ("pack_force_in", "force", "unpack_force_out"):
+        for k in ("pack_force_in", "force"):
             L[k]()
-        down.wait_event(ev(main))
-        for s in E["down3"]:
-            sph.sph_store_download_sub(self.store, s, self.host[s], down)
+        # the force results are reduced slab by slab; each slab's particles leave as soon as they are final
+        for c0, nc, p0, npart in E["slabs"]:
+            sph.sph_unpack_cells(st, b, S[3], B[3], c0, nc, sph.SPH_UNPACK_REDUCE_ZERO, main)
+            down.wait_event(ev(main))
+            for s in E["down3"]:
+                sph.sph_store_download_range(st, s, self.host[s], p0, npart, down)
         main.wait_event(ev(down))
+
+    def capture_e2e(self):
+        """step_e2e captured once as a CUDA graph (copies, kernels and the cross-stream events): a replay costs one launch on
+        the host instead of ~50 calls through ctypes, which would otherwise bound a 0.9 ms step"""
+        torch = self.torch
+        root = torch.cuda.Stream()
+        with torch.cuda.stream(root):
+            self.step_e2e(root)                      # warm-up outside the capture (first-call attribute setting)
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=root):
+            self.step_e2e(root)
+        return self.graph
 
     def e2e_bytes(self):
         return (sum(self.n * self.layout.stride[s] for s in self.subs_in), sum(self.n * self.layout.stride[s] for s in self.subs_out))
@@ -278,6 +300,7 @@ class Workload:
         }
 
     def close(self):
+        self.graph = None
         self.sph.sph_batch_destroy(self.batch)
         self.sph.sph_store_destroy(self.store)
 
@@ -350,7 +373,8 @@ def run_layouts(args):
     for name in layouts.NAMES:
         w = Workload(sph, torch, ps, cells, tasks, name)
         t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, 1)
-        t_e2e = time_steps(torch, w.step_e2e, args.steps, args.warmup, flush, 1)
+        g_e2e = w.capture_e2e()
+        t_e2e = time_steps(torch, g_e2e.replay, args.steps, args.warmup, flush, 1)
         per = {k: [] for k, _ in w.launches()}
         for _ in range(args.steps):
             flush()
@@ -408,7 +432,8 @@ def run_ours(args):
         sampler = ClockSampler(local) if rank == 0 else None
         t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, world)
         clocks = sampler.stop() if sampler else None
-        t_e2e = time_steps(torch, w.step_e2e, args.steps, args.warmup, flush, world)
+        g_e2e = w.capture_e2e()
+        t_e2e = time_steps(torch, g_e2e.replay, args.steps, args.warmup, flush, world)
         # per-kernel durations: events around each launch of each timed-length step (same stream, L2 flushed per step)
         per = {k: [] for k, _ in w.launches()}
         for _ in range(args.steps):
@@ -462,7 +487,8 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "layout": primary, "store": "HBM", "tasks": int(w.info.n_tasks), "instances_per_loop": int(w.info.n_instances),
                    "candidate_pairs_per_loop": int(cand), "l2": "flushed before every step (256 MB fill, untimed)",
-                   "sharding": "one independent box per rank, no collective"},
+                   "sharding": "one independent box per rank, no collective",
+                   "e2e": "host-resident particle arrays; the step's copies and kernels captured once as a CUDA graph, one replay per step"},
         "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},
         "instances_per_s": {k: w.info.n_instances / (R["per"][k] * 1e-3) for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out")},
         "e2e": {"value": total_particles / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
