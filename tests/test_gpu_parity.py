@@ -386,21 +386,25 @@ def test_pack_then_unpack_identity(layout):
 
 # ------------------------------------------------------------------ whole pipeline
 
-def gpu_step(g, do_force=True):
+def gpu_step(g, do_force=True, fused_zero=False):
+    """fused_zero: bench.py's launch configuration -- no sph_store_zero launches, the unpacks start their sums from zero"""
+    mode = sph.SPH_UNPACK_REDUCE_ZERO if fused_zero else sph.SPH_UNPACK_REDUCE
     s_in, s_out = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN), sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_OUT)
     f_in, f_out = sph.sph_attrset_canonical(sph.SPH_SET_FORCE_IN), sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT)
     b_in, b_out = g.buffer(s_in), g.buffer(s_out)
-    sph.sph_store_zero(g.store, s_out)
+    if not fused_zero:
+        sph.sph_store_zero(g.store, s_out)
     sph.sph_pack(g.store, g.batch, s_in, b_in)
     sph.sph_density(g.batch, b_in, b_out)
-    sph.sph_unpack(g.store, g.batch, s_out, b_out, sph.SPH_UNPACK_REDUCE)
+    sph.sph_unpack(g.store, g.batch, s_out, b_out, mode)
     sph.sph_ghost(g.store, PARAMS)
     if do_force:
         c_in, c_out = g.buffer(f_in), g.buffer(f_out)
-        sph.sph_store_zero(g.store, f_out)
+        if not fused_zero:
+            sph.sph_store_zero(g.store, f_out)
         sph.sph_pack(g.store, g.batch, f_in, c_in)
         sph.sph_force(g.batch, c_in, c_out, PARAMS)
-        sph.sph_unpack(g.store, g.batch, f_out, c_out, sph.SPH_UNPACK_REDUCE)
+        sph.sph_unpack(g.store, g.batch, f_out, c_out, mode)
     torch.cuda.synchronize()
     return g.export()
 
