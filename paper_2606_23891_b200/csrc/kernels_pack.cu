@@ -247,8 +247,8 @@ pack_kernel(Program prog, const CellChunk* __restrict__ cell_chunks, const uint3
 //  (1) fetch: the chunk's slice of every block of the round travels global -> shared memory as ONE bulk copy (TMA,
 //      cp.async.bulk) per slice, each issued by its own lane and all completing on the ring's mbarrier: a whole round is
 //      one instruction per lane, holds no registers while in flight, and the NEXT round (of this chunk, or the first of
-//      the warp's next chunk) is issued into the other ring before the current one is waited for, so every warp always
-//      has 14-17 KB outstanding;
+//      the warp's next chunk) is issued into the other ring before the current one is waited for; rings are small (9
+//      slices, ~5 KB) so that 18 warps share an SM: one warp's reduction overlaps the other warps' fetches;
 //  (2) reduce: one lane per particle walks the slices in ascending (task, side) order.  With the lane owning a
 //      record, the operator of word j (+=, max, =) is the same in every lane: no per-lane dispatch, no divergence.
 //      Records are read with VEC-word shared loads (stride = record length: conflict-free when R / VEC is odd).
@@ -317,6 +317,28 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
     // one group of words [g0, g0 + nw) reduced over the `lim` slices of a ring, in slice order
     auto reduce_group = [&](float (&acc)[GW], const unsigned char* ring, uint32_t g0, uint32_t nw, uint32_t lim) {
         const unsigned char* rec = ring + (lane * R + g0) * 4;
+        if constexpr (VEC == 1) {
+            // odd record length: scalar shared loads are conflict-free, so every word runs its own loop over the slices with its
+            // operator hoisted out of it (warp-uniform): one load and one operation per slice and word, loads batched ahead
+            if (!all_sum) {
+#pragma unroll
+                for (int j = 0; j < GW; ++j) {
+                    if ((uint32_t)j >= nw) continue;
+                    const uint32_t kind = prog.word[g0 + j].kind;
+                    const unsigned char* rj = rec + 4 * j;
+                    if (kind == W_SUM) {
+#pragma unroll 9
+                        for (uint32_t u = 0; u < lim; ++u) acc[j] = __fadd_rn(acc[j], *reinterpret_cast<const float*>(rj + u * slot_bytes));
+                    } else if (kind == W_MAX) {
+#pragma unroll 9
+                        for (uint32_t u = 0; u < lim; ++u) acc[j] = fmaxf(acc[j], *reinterpret_cast<const float*>(rj + u * slot_bytes));
+                    } else {
+                        acc[j] = *reinterpret_cast<const float*>(rj + (lim - 1) * slot_bytes);      // overwrite: the last slice wins
+                    }
+                }
+                return;
+            }
+        }
         uint32_t m_sum[GW], m_red[GW];
 #pragma unroll
         for (int j = 0; j < GW; ++j) {
@@ -391,9 +413,15 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
             for (uint32_t w = 0; w < R; ++w)
                 scratch[w * 32 + lane] = live && !from_zero && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
         mbar_wait(bars + (it & 1), (it >> 1) & 1);
+#ifdef SPH_DEBUG_SKIP_REDUCE
+        if (single) {
+            acc[0] += *reinterpret_cast<const float*>(ring + lane * 4);
+        } else {
+#else
         if (single) {
             reduce_group(acc, ring, 0, R, lim);
         } else {
+#endif
             for (uint32_t g0 = 0; g0 < R; g0 += GW) {
                 const uint32_t nw = min((uint32_t)GW, R - g0);
                 float a2[GW];
@@ -485,7 +513,15 @@ int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t*
     return SPH_OK;
 }
 
-constexpr uint32_t kUnpackRingBytes = 17408;   // per warp: 27 slices of 32 x 20-byte records fit (a cell of a periodic grid occurs 27 times)
+#ifndef SPH_UNPACK_MAXCTA
+#define SPH_UNPACK_MAXCTA 16
+#endif
+#ifndef SPH_UNPACK_RING
+#define SPH_UNPACK_RING 5760
+#endif
+constexpr uint32_t kUnpackRingBytes = SPH_UNPACK_RING;   // per ring: 9 slices of 32 x 20-byte records -- a cell of a periodic grid (27 blocks) takes three
+                                                          // rounds; small rings let 9 CTAs (18 warps) share an SM, which is what overlaps one warp's reduction
+                                                          // with the others' fetches (measured: 27-slice rings 0.36 ms, 9-slice rings 0.23 ms on configs[2])   // per warp: 27 slices of 32 x 20-byte records fit (a cell of a periodic grid occurs 27 times)
 
 template <int VEC, int GW>
 int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
@@ -499,7 +535,7 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
         SPH_CUDA_TRY(cudaFuncSetAttribute(unpack_kernel<VEC, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = smem;
     }
-    const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(16, (227 * 1024) / (smem + 1024)));
+    const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(SPH_UNPACK_MAXCTA, (227 * 1024) / (smem + 1024)));
     const uint32_t want = (ncc + kUnpackWarps - 1) / kUnpackWarps;
     const uint32_t grid = std::min(want, (uint32_t)sms * per_sm);
     unpack_kernel<VEC, GW><<<grid, kUnpackWarps * 32, smem, st>>>(view, prog, b->d_cell_chunks + cc0, d_occ_off128, ncc, d_buf, slots,
