@@ -413,15 +413,9 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
             for (uint32_t w = 0; w < R; ++w)
                 scratch[w * 32 + lane] = live && !from_zero && is_reduced(w) ? *reinterpret_cast<const float*>(word_addr(w, p)) : 0.f;
         mbar_wait(bars + (it & 1), (it >> 1) & 1);
-#ifdef SPH_DEBUG_SKIP_REDUCE
-        if (single) {
-            acc[0] += *reinterpret_cast<const float*>(ring + lane * 4);
-        } else {
-#else
         if (single) {
             reduce_group(acc, ring, 0, R, lim);
         } else {
-#endif
             for (uint32_t g0 = 0; g0 < R; g0 += GW) {
                 const uint32_t nw = min((uint32_t)GW, R - g0);
                 float a2[GW];
