@@ -296,6 +296,43 @@ def test_unpack_reduce_zero_equals_zero_then_reduce(name, layout):
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
 @pytest.mark.parametrize("name", ["ragged", "octree"])
+def test_host_resident_store_zero_copy(name, layout):
+    """SPH_MEM_HOST_PINNED: the kernels read and write the store in mapped pinned host memory over the link.
+    Pack bytes, unpack results and a whole step must equal the HBM-resident store's / the oracle's bit for bit."""
+    ps, cells, tasks = case(name)
+    ps = physical(ps, cells, tasks)
+    g = GpuCase(ps, cells, tasks, layout, mem_kind=sph.SPH_MEM_HOST_PINNED)
+    for oset in (orc.DENSITY_IN, orc.FORCE_IN, sweep_set(PACK_SWEEP, 13, orc.FLAG_X_REL_F32)):
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        ref = orc.pack(ps, cells, tasks, oset)
+        off_o, total = orc.block_offsets(cells, tasks, rec)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        got = g.pack(aset).cpu().numpy()
+        m = valid_mask(off_o, cells, tasks, rec, total)
+        assert np.array_equal(got[m], ref[m]), (name, layout, rec)
+    for n_set, (oset, mode) in enumerate([(orc.FORCE_OUT, orc.MODE_REDUCE), (sweep_set(UNPACK_SWEEP, 13, 0), orc.MODE_REDUCE)]):
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        _, total = orc.block_offsets(cells, tasks, rec)
+        buf = _random_result_buffer(total, 700 + n_set)
+        ref = raw_copy(ps)
+        orc.unpack(ref, cells, tasks, oset, buf, mode)
+        sph.sph_store_import_aos(g.store, ps)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        sph.sph_unpack(g.store, g.batch, aset, torch.from_numpy(buf).cuda(), mode)
+        torch.cuda.synchronize()
+        assert np.array_equal(canon(g.export()), canon(ref)), (name, layout, rec)
+    # the whole step: the same bits as with the store in HBM
+    sph.sph_store_import_aos(g.store, ps)
+    got_host = gpu_step(g, fused_zero=True)
+    d = GpuCase(ps, cells, tasks, layout)
+    got_dev = gpu_step(d, fused_zero=True)
+    assert np.array_equal(canon(got_host), canon(got_dev)), (name, layout)
+    d.close()
+    g.close()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["ragged", "octree"])
 def test_streamed_cell_ranges_equal_oracle(name, layout):
     """The streamed host-resident path: the store's structs cross the link slab by slab (sph_store_upload_range), every slab
     is packed as soon as it is there (sph_pack_cells); results are unpacked slab by slab (sph_unpack_cells) and each
