@@ -462,7 +462,8 @@ def run_ours(args):
         e = {"ms": round(d, 5)}
         if k in alg:
             if alg[k]["bound"] == "hbm":
-                e.update(bound="hbm", achieved=round(alg[k]["bytes"] / (d * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s")
+                e.update(bound="hbm", achieved=round(alg[k]["bytes"] / (d * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s",
+                         frac_of_nominal_8tbs=round(alg[k]["bytes"] / (d * 1e-3) / 1e9 / 8000.0, 4))
             else:
                 e.update(bound="alu", achieved=round(alg[k]["flop"] / (d * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s")
             e["frac"] = round(e["achieved"] / e["peak"], 4)
