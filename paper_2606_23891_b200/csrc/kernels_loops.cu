@@ -48,6 +48,10 @@ typedef unsigned long long u64;            // a pair of f32 (lo = target A, hi =
 constexpr int kLoopWarps = SPH_LOOP_WARPS;
 constexpr int kTile = 64;                  // compacted sources per flush: two halves of 32, one mask word each per target
 constexpr int kHalf = 33;                  // tile entries per half: 32 sources + the dummy (where __clz(0) = 32 points)
+#ifndef SPH_UNIT_BITS
+#define SPH_UNIT_BITS 4
+#endif
+constexpr uint32_t kUnitBits = SPH_UNIT_BITS;      // neighbours per unit (even)
 constexpr int kUnitCap = SPH_UNIT_CAP;               // units (target, <= 4 neighbours) evaluated per window of a flush, 32 at a time
 constexpr float kInvPi = 0.318309886183790671538f;
 constexpr float kNever = 1.0e30f;          // |s|^2 of a filter pad entry / threshold of an idle target: never a hit
@@ -617,7 +621,8 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             // Acceleration sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan)
             // adds keep the rounding of the running sums out of the 1e-6 max|a| budget, in both ways.
             const uint32_t cA0 = __popc(m[0]), cA1 = __popc(m[1]), cB0 = __popc(m[2]), cB1 = __popc(m[3]);
-            const uint32_t nuA = ((cA0 + 3) >> 2) + ((cA1 + 3) >> 2), nuB = ((cB0 + 3) >> 2) + ((cB1 + 3) >> 2), nu = nuA + nuB;
+            const uint32_t nuA = (cA0 + kUnitBits - 1) / kUnitBits + (cA1 + kUnitBits - 1) / kUnitBits;
+            const uint32_t nuB = (cB0 + kUnitBits - 1) / kUnitBits + (cB1 + kUnitBits - 1) / kUnitBits, nu = nuA + nuB;
             float axA = 0.f, ayA = 0.f, azA = 0.f, duA = 0.f, vsA = 0.f, axB = 0.f, ayB = 0.f, azB = 0.f, duB = 0.f, vsB = 0.f;
             if constexpr (!UNITS) {
                 const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
@@ -660,7 +665,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                             while (mw == 0) { ++cw; mw = cw == 1 ? m1 : (cw == 2 ? m2 : m3); }
                             const uint32_t before = mw;
 #pragma unroll
-                            for (int q = 0; q < 4; ++q) mw &= ~shr_clamp(0x80000000u, __clz(mw));      // __clz(0) = 32: the shift gives 0, nothing cleared
+                            for (int q = 0; q < kUnitBits; ++q) mw &= ~shr_clamp(0x80000000u, __clz(mw));      // __clz(0) = 32: the shift gives 0, nothing cleared
                             const uint32_t idx = cum + __popc(bal & lt);
                             upos[idx] = before ^ mw;
                             utgt[idx] = (unsigned char)((r < nuA ? tA : tB) | ((cw & 1) << 7));
@@ -675,9 +680,9 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                         const bool valid = u < cum;
                         uint32_t um = valid ? upos[u] : 0u;
                         const uint32_t tw = valid ? utgt[u] : 0u, t = tw & 127u, ebase = (tw >> 7) * kHalf;
-                        uint32_t e[4];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
+                        uint32_t e[kUnitBits];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
+                        for (int q = 0; q < kUnitBits; ++q) {
                             const uint32_t j = __clz(um);
                             um &= ~shr_clamp(0x80000000u, j);
                             e[q] = ebase + j;
@@ -693,7 +698,9 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                             vsig = fmaxf(vsig, fmaxf(o.vsa, o.vsb));
                         };
                         two(e[0], e[1]);
-                        if (__any_sync(kFull, e[2] != ebase + 32u)) two(e[2], e[3]);
+#pragma unroll
+                        for (int q = 2; q < kUnitBits; q += 2)
+                            if (__any_sync(kFull, e[q] != ebase + 32u)) two(e[q], e[q + 1]);
                         if (valid) {
                             float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
                             unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
