@@ -295,6 +295,44 @@ def test_unpack_reduce_zero_equals_zero_then_reduce(name, layout):
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
+def test_partial_batches_pair_only_self_only_and_untouched_cells(layout):
+    """Batches that hold only pair tasks, only self tasks, or the tasks of a few cells: buffers and store equal the oracle's,
+    and SPH_UNPACK_REDUCE_ZERO leaves the particles of cells the batch does not touch alone."""
+    ps, cells, tasks = case("config0")       # 4^3 cells: the tasks of one cell touch 27 of the 64
+    n_self = int((tasks["cj"] < 0).sum())
+    subsets = {"self": tasks[:n_self], "pair": tasks[n_self:], "few": tasks[(tasks["ci"] == 5) | (tasks["cj"] == 5)]}
+    for label, sel in subsets.items():
+        sel = np.ascontiguousarray(sel)
+        g = GpuCase(ps, cells, sel, layout)
+        oset = orc.FORCE_IN
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        ref = orc.pack(ps, cells, sel, oset)
+        off_o, total = orc.block_offsets(cells, sel, rec)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        m = valid_mask(off_o, cells, sel, rec, total)
+        assert np.array_equal(g.pack(aset).cpu().numpy()[m], ref[m]), (label, layout)
+        oset = orc.FORCE_OUT
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        _, total = orc.block_offsets(cells, sel, rec)
+        buf = _random_result_buffer(total, 900)
+        touched = np.zeros(ps.shape[0], dtype=bool)
+        for key in ("ci", "cj"):
+            for c in sel[key][sel[key] >= 0]:
+                touched[int(cells["first"][c]):int(cells["first"][c]) + int(cells["count"][c])] = True
+        want = raw_copy(ps)
+        for name_f in ("a", "du_dt", "v_sig"):
+            want[name_f][touched] = 0
+        orc.unpack(want, cells, sel, oset, buf, orc.MODE_REDUCE)
+        assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
+        sph.sph_unpack(g.store, g.batch, aset, torch.from_numpy(buf).cuda(), sph.SPH_UNPACK_REDUCE_ZERO)
+        got = g.export()
+        assert np.array_equal(canon(got), canon(want)), (label, layout)
+        if label == "few":
+            assert not touched.all() and np.array_equal(canon(got)[~touched], canon(ps)[~touched])
+        g.close()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
 @pytest.mark.parametrize("name", ["ragged", "octree"])
 def test_host_resident_store_zero_copy(name, layout):
     """SPH_MEM_HOST_PINNED: the kernels read and write the store in mapped pinned host memory over the link.
