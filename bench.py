@@ -490,7 +490,9 @@ def run_ours(args):
                    "candidate_pairs_per_loop": int(cand), "l2": "flushed before every step (256 MB fill, untimed)",
                    "sharding": "one independent box per rank, no collective",
                    "e2e": "host-resident particle arrays; the step's copies and kernels captured once as a CUDA graph, one replay per step"},
-        "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},
+        "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},      # ordered candidate pairs
+        "neighbour_pairs_per_s": {"density": total_particles / world * NGB_CONFIG1 / (R["per"]["density"] * 1e-3),                       # pairs inside the cut-off
+                                  "force": total_particles / world * (NGB_CONFIG1 - 1) / (R["per"]["force"] * 1e-3)},
         "instances_per_s": {k: w.info.n_instances / (R["per"][k] * 1e-3) for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out")},
         "e2e": {"value": total_particles / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
                 "ms_per_step": ms_e2e},
