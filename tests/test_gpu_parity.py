@@ -59,6 +59,9 @@ def case(name):
         elif name == "bigcells":               # counts 10..667, wide cells with large h
             ps, cells, tasks, _, _ = sort_octree(si.clumpy_mixture(20000, seed=8, n_clumps=2, frac_clumps=0.5, sigma=0.08,
                                                                    h_cap=1.0 / 10), 700)
+        elif name == "hugecells":              # 27 cells of ~1,450 particles, variable h and mass: 46 chunks per cell, sources in 46 rounds, many flushes
+            ps, cells, tasks, _, _ = sort_grid(si.jittered_lattice(34, 4, jitter=0.9, eta=0.8, sigma_v=0.3, h_spread=0.3, mass_spread=0.4,
+                                                                   u_spread=0.3), 3)
         else:
             raise KeyError(name)
         _CASES[name] = (fill_all_fields(ps, 17), cells, tasks)
@@ -99,7 +102,7 @@ def test_store_over_caller_memory():
 # ------------------------------------------------------------------ pack: bit-exact
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
-@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "hugecells"])
 def test_pack_bit_exact(name, layout):
     ps, cells, tasks = case(name)
     g = GpuCase(ps, cells, tasks, layout)
@@ -171,7 +174,7 @@ def _records(buf, off, cells, tasks, rec_words):
     return np.concatenate(rows), np.concatenate(pidx)
 
 
-@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells", "hugecells"])
 def test_density_loop_vs_oracle(name):
     ps, cells, tasks = case(name)
     orc.set_threads(8)
@@ -210,7 +213,7 @@ def _near_cutoff(ps, cells, tasks, buf_in, rel=1e-5):
     return flagged
 
 
-@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells", "hugecells"])
 def test_force_loop_vs_oracle(name):
     ps, cells, tasks = case(name)
     ps = physical(ps, cells, tasks)
@@ -247,7 +250,7 @@ def _random_result_buffer(total, seed):
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
-@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "hugecells"])
 def test_unpack_bit_exact_stage_isolated(name, layout):
     ps, cells, tasks = case(name)
     g = GpuCase(ps, cells, tasks, layout)
@@ -499,7 +502,7 @@ def check_store_physics(got, ref):
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
-@pytest.mark.parametrize("name", ["config0", "ragged", "octree"])
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "hugecells"])
 def test_full_step_vs_oracle(name, layout):
     ps, cells, tasks = case(name)
     ref = raw_copy(ps)
