@@ -329,8 +329,13 @@ def test_octree_cells():
         f, k = int(cells["first"][c]), int(cells["count"][c])
         x = ps["x"][f:f + k]
         assert np.all(x >= cells["origin"][c]) and np.all(x < cells["origin"][c] + cells["width"][c])
-        # a leaf is either small enough or could not be split without violating width >= 2 hmax
-        assert k <= 100 or cells["width"][c] / 2 < 2 * hmax[c] * (1 + 1e-6) or True
+        # a leaf is either small enough or could not be split: one of its non-empty octants would be narrower than
+        # 2 hmax of the particles in that octant (the octants are recomputed here from the positions)
+        if k > 100:
+            half = 0.5 * cells["width"][c]
+            octant = ((x >= cells["origin"][c] + half) * np.array([4, 2, 1])).sum(axis=1)
+            hh = ps["h"][f:f + k].astype(np.float64)
+            assert any(half < 2.0 * hh[octant == o].max() for o in np.unique(octant))
         assert cells["width"][c] >= 2 * hmax[c] or cells["width"][c] == 1.0
     assert len(set(cells["width"].tolist())) > 1            # really adaptive
     assert cells["count"].max() <= 100 or np.any(cells["width"] / 2 < 2 * hmax)
@@ -501,6 +506,54 @@ def test_unpack_reduce_operators_and_order():
     orc.unpack(parts, cells, tasks, attrset, buf2, orc.MODE_REDUCE)
     assert np.all(parts["rho"][:5] == np.float32(2.0 ** 24 + 2.0))      # (1 + 1) + 2^24 is exact
     assert np.all(parts["rho"][5:] == np.float32(2.0 ** 24))            # (1 + 2^24) rounds to 2^24, then + 1 rounds back
+
+
+def test_zero_clears_the_listed_components_and_nothing_else():
+    # a store whose every member is non-zero: after zero(set) the listed components are +0.0, every other byte is unchanged
+    # (catches a zero that does nothing, one that clears whole fields instead of components, one that touches neighbours)
+    n = 23
+    parts = _pattern_store(n)
+    raw0 = parts.view(np.uint8).reshape(n, 128).copy()
+    assert np.all(parts["rho"] != 0) and np.all(parts["a"] != 0) and np.all(parts["v_sig"] != 0)
+    orc.zero(parts, ([(orc.RHO, 0, 1), (orc.A, 1, 2), (orc.V_SIG, 0, 1)], 0))
+    raw1 = parts.view(np.uint8).reshape(n, 128)
+    cleared = np.zeros(128, dtype=bool)
+    for off in (64, 36 + 4, 36 + 8, 104):            # rho @64, a[1] @40, a[2] @44, v_sig @104 (reading C16)
+        cleared[off:off + 4] = True
+    assert np.all(raw1[:, cleared] == 0)
+    assert np.array_equal(raw1[:, ~cleared], raw0[:, ~cleared])
+    # the canonical output sets: every output of the loop about to run is zero, inputs are untouched
+    parts = _pattern_store(n)
+    keep = {k: parts[k].copy() for k in ("x", "v", "mass", "h", "u", "P", "c_s", "id", "time_bin", "div_v", "rot_v")}
+    orc.zero(parts, orc.DENSITY_OUT)
+    for k in ("rho", "rho_dh", "wcount", "wcount_dh"):
+        assert np.all(parts[k] == 0)
+    assert np.all(parts["a"] != 0) and np.all(parts["du_dt"] != 0) and np.all(parts["v_sig"] != 0)
+    orc.zero(parts, orc.FORCE_OUT)
+    for k in ("a", "du_dt", "v_sig"):
+        assert np.all(parts[k] == 0)
+    for k, v in keep.items():
+        assert np.array_equal(parts[k], v)
+    with pytest.raises(ValueError):
+        orc.zero(parts, ([(orc.X, 0, 3)], 0))          # not an f32 member
+
+
+def test_cycles_start_from_zero_whatever_the_store_held():
+    # density_cycle / force_cycle zero their outputs first: running them on a store that already holds results (or
+    # garbage) gives the same bits as on a fresh store -- and not twice the sums
+    parts = si.jittered_lattice(12, seed=11, h_spread=0.1, mass_spread=0.2, u_spread=0.2)
+    ps, cells, tasks, ns, npair = sort_grid(parts, 4)
+    fresh = raw_copy(ps)
+    orc.density_cycle(fresh, cells, tasks)
+    orc.ghost(fresh, GAMMA)
+    orc.force_cycle(fresh, cells, tasks)
+    again = raw_copy(fresh)                             # outputs of a whole step are in the store
+    again["v_sig"] = 1.0e6                              # a max that did not restart from 0 would keep this
+    orc.density_cycle(again, cells, tasks)
+    orc.ghost(again, GAMMA)
+    orc.force_cycle(again, cells, tasks)
+    assert np.array_equal(again.view(np.uint8), fresh.view(np.uint8))
+    assert np.all(fresh["rho"] > 0) and np.all(fresh["v_sig"] > 0)
 
 
 def test_unpack_rejects_relative_coordinates():
