@@ -180,18 +180,20 @@ int32_t sph_tasks_build(const sph_cell* cells, const float* hmax_per_cell, uint3
 int32_t sph_free(void* p);
 
 /* ---- batches (bundles) ---- */
-/* Builds the device tables of a batch of tasks [host array] against the store's cell table: block table, per
- * record-size block offsets, 32-particle chunk table, per-cell occurrence lists for the ordered unpack.
- * tasks_per_segment = 0: one segment.  Immutable afterwards.  Synchronous. */
+/* Builds the device tables of a batch of tasks [host array] against the store's cell table: block table, chunk tables,
+ * per-cell occurrence lists for the cell-centric kernels.  tasks_per_segment = 0: one segment.  Immutable afterwards.
+ * Synchronous.  The batch is tied to the cell table (not to the store object): it may be used with any store of the same
+ * particle count whose cell table is the same (SPH_ERR_INVALID_ARG otherwise). */
 int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t n_tasks, uint32_t tasks_per_segment, sph_batch** out);
 int32_t sph_batch_destroy(sph_batch* batch);
 int32_t sph_batch_get_info(const sph_batch* batch, sph_batch_info* info_out);
-/* Bytes of the buffer that holds this batch for this attribute set (also prepares the batch's offset table for
- * that record size; must be called once per record size before pack/unpack use it). */
-int32_t sph_batch_buffer_bytes(sph_batch* batch, const sph_attrset* set, uint64_t* bytes_out);
+/* Bytes of the buffer that holds this batch for this attribute set.  A pure query: the batch is not changed as far as any
+ * caller can observe (block offsets for a record size are derived from the immutable block table the first time any call
+ * needs them, under a lock; sph_pack / sph_unpack accept any attribute set whether or not this was called). */
+int32_t sph_batch_buffer_bytes(const sph_batch* batch, const sph_attrset* set, uint64_t* bytes_out);
 /* Byte offset of every block for this attribute set: off_out [host, 2*n_tasks], off[2t] side i, off[2t+1] side j
  * (UINT64_MAX for self tasks).  seg_off_out [host, n_segments] may be NULL. */
-int32_t sph_batch_block_offsets(sph_batch* batch, const sph_attrset* set, uint64_t* off_out, uint64_t* seg_off_out);
+int32_t sph_batch_block_offsets(const sph_batch* batch, const sph_attrset* set, uint64_t* off_out, uint64_t* seg_off_out);
 
 /* ---- the hot path ---- */
 /* Sets the listed f32 components of every particle to 0 ("zero the outputs of the loop about to run"). */

@@ -11,7 +11,8 @@
 // What fixes each step (PAPER.md = /root/reference/PAPER.md; "reading Cn" =
 // DESIGN.md section "Readings of the paper"):
 //   particle record ........ PAPER.md:47-58 Table 1 + BASELINE.json:configs[0]   (C16)
-//   cells .................. PAPER.md:66   (particles sorted by cell)
+//   cells .................. PAPER.md:66   (particles sorted by cell; inside a cell by the Morton code of
+//                            their position, reading C26)
 //   tasks / bundles ........ PAPER.md:70, 76
 //   pack ................... PAPER.md:78, 102 ("only the required quantities are buffered",
 //                            "coordinates shifted to facilitate periodic boundary conditions") (C6, C7)
@@ -216,6 +217,30 @@ void force_block(const float* tgt, uint32_t n_t, const float* src, uint32_t n_s,
     }
 }
 
+// ---- order of the particles inside a cell (reading C26): ascending Morton code of the position inside the cell
+// on a 32 x 32 x 32 sub-grid; equal codes keep generator order.  Sub-cell index along d:
+// k_d = clamp(floor((x_d - origin_d) / width * 32), 0, 31); code bit 3b+2 = bit b of k_0 (x), 3b+1 of k_1, 3b of k_2.
+uint32_t morton_in_cell(const double* x, const double* origin, double width) {
+    uint32_t k[3];
+    for (int d = 0; d < 3; ++d) {
+        double f = std::floor((x[d] - origin[d]) / width * 32.0);
+        if (f < 0.0) f = 0.0;
+        if (f > 31.0) f = 31.0;
+        k[d] = (uint32_t)f;
+    }
+    uint32_t code = 0;
+    for (int b = 0; b < 5; ++b)
+        for (int d = 0; d < 3; ++d) code |= ((k[d] >> b) & 1u) << (3 * b + (2 - d));
+    return code;
+}
+
+// stable sort of idx[lo, hi) by the Morton code inside the cell (origin, width)
+void sort_cell_by_morton(const double* x3, std::vector<uint64_t>& idx, uint64_t lo, uint64_t hi, const double* origin, double width) {
+    std::stable_sort(idx.begin() + lo, idx.begin() + hi, [&](uint64_t a, uint64_t b) {
+        return morton_in_cell(x3 + 3 * a, origin, width) < morton_in_cell(x3 + 3 * b, origin, width);
+    });
+}
+
 // periodic minimum gap between [oa, oa+wa] and [ob, ob+wb] along one axis; *shift = image shift of b
 double axis_gap(double oa, double wa, double ob, double wb, double box, double* shift, double* second_best) {
     double best = 1e300, second = 1e300, best_s = 0;
@@ -246,7 +271,7 @@ int orc_record_bytes(const Attr* attrs, int n_attr, uint32_t flags) {
     return record_bytes(attrs, n_attr, flags);
 }
 
-// ---- cells: uniform periodic grid (C25 row-major cell index, C26 stable order) ----
+// ---- cells: uniform periodic grid (C25 row-major cell index, C26 Morton order inside a cell) ----
 // x3: n*3 doubles in [0, box).  perm_out[k] = generator index of the k-th particle in cell order.
 int orc_cells_build_grid(const double* x3, uint64_t n, uint32_t cpd, double box, uint64_t* perm_out, Cell* cells_out) {
     const uint64_t nc = (uint64_t)cpd * cpd * cpd;
@@ -266,8 +291,8 @@ int orc_cells_build_grid(const double* x3, uint64_t n, uint32_t cpd, double box,
     }
     std::vector<uint64_t> start(nc + 1, 0);
     for (uint64_t c = 0; c < nc; ++c) start[c + 1] = start[c] + count[c];
-    std::vector<uint64_t> fill(start.begin(), start.end() - 1);
-    for (uint64_t p = 0; p < n; ++p) perm_out[fill[cell_of[p]]++] = p;    // stable
+    std::vector<uint64_t> fill(start.begin(), start.end() - 1), idx(n);
+    for (uint64_t p = 0; p < n; ++p) idx[fill[cell_of[p]]++] = p;         // by cell, generator order inside
     const double w = box / cpd;
     for (uint64_t c = 0; c < nc; ++c) {
         Cell& ce = cells_out[c];
@@ -275,14 +300,16 @@ int orc_cells_build_grid(const double* x3, uint64_t n, uint32_t cpd, double box,
         ce.origin[0] = (double)(c / ((uint64_t)cpd * cpd)) * w;
         ce.origin[1] = (double)((c / cpd) % cpd) * w;
         ce.origin[2] = (double)(c % cpd) * w;
+        sort_cell_by_morton(x3, idx, start[c], start[c + 1], ce.origin, w);   // C26
     }
+    std::copy(idx.begin(), idx.end(), perm_out);
     return 0;
 }
 
 // ---- cells: octree (C21): split a node while it holds more than max_per_leaf
 // particles and every non-empty child would still be at least as wide as 2*hmax of its own
 // particles.  Leaves in depth-first order, child octant code = 4*bx + 2*by + bz; empty leaves
-// are dropped.  Returns the number of leaves (or < 0); cells_out may be NULL to count only.
+// are dropped; inside a leaf the particles are in Morton order (C26).  Returns the number of leaves (or < 0); cells_out may be NULL to count only.
 static void octree_rec(const double* x3, const float* h, std::vector<uint64_t>& idx, uint64_t lo, uint64_t hi,
                        const double origin[3], double width, uint32_t max_per_leaf, uint32_t depth,
                        std::vector<Cell>& leaves, std::vector<uint64_t>& scratch) {
@@ -306,6 +333,7 @@ static void octree_rec(const double* x3, const float* h, std::vector<uint64_t>& 
         Cell ce; ce.first = lo; ce.count = (uint32_t)cnt; ce.pad = 0; ce.width = width;
         for (int d = 0; d < 3; ++d) ce.origin[d] = origin[d];
         leaves.push_back(ce);
+        sort_cell_by_morton(x3, idx, lo, hi, origin, width);              // C26
         return;
     }
     uint64_t cstart[9]; cstart[0] = lo;

@@ -253,6 +253,7 @@ int32_t sph_layout_from_groups(const uint8_t* fields, uint32_t n_fields, const u
 
 int32_t sph_layout_validate(const sph_layout* l) {
     if (!l) return fail(SPH_ERR_INVALID_ARG, "layout is NULL");
+    SPH_API_BEGIN
     if (l->n_sub < 1 || l->n_sub > SPH_MAX_SUB) return fail(SPH_ERR_LAYOUT, "n_sub = %u (1..%d)", l->n_sub, SPH_MAX_SUB);
     std::vector<std::vector<uint8_t>> used(l->n_sub);
     for (uint32_t s = 0; s < l->n_sub; ++s) {
@@ -273,6 +274,7 @@ int32_t sph_layout_validate(const sph_layout* l) {
         }
     }
     return SPH_OK;
+    SPH_API_END
 }
 
 // ------------------------------------------------------------------ attribute sets
@@ -460,18 +462,25 @@ int32_t sph_store_export_aos(const sph_store* s, void* host_aos, uint64_t n) {
 int32_t sph_store_set_cells(sph_store* s, const sph_cell* cells, uint32_t n_cells) {
     if (int32_t rc = store_check(s)) return rc;
     if (!cells || n_cells == 0) return fail(SPH_ERR_INVALID_ARG, "no cells");
+    SPH_API_BEGIN
     std::vector<std::pair<uint64_t, uint64_t>> ranges;
     ranges.reserve(n_cells);
+    uint64_t hash = 0xCBF29CE484222325ull ^ n_cells;        // FNV-1a over the (first, count) pairs
     for (uint32_t c = 0; c < n_cells; ++c) {
-        if (cells[c].first + cells[c].count > s->n) return fail(SPH_ERR_RANGE, "cell %u: [%llu, +%u) exceeds the store (%llu)", c,
-                                                               (unsigned long long)cells[c].first, cells[c].count, (unsigned long long)s->n);
+        if (cells[c].first > s->n || cells[c].count > s->n - cells[c].first)
+            return fail(SPH_ERR_RANGE, "cell %u: [%llu, +%u) exceeds the store (%llu)", c,
+                        (unsigned long long)cells[c].first, cells[c].count, (unsigned long long)s->n);
         if (cells[c].count) ranges.emplace_back(cells[c].first, cells[c].first + cells[c].count);
+        hash = (hash ^ cells[c].first) * 0x100000001B3ull;
+        hash = (hash ^ cells[c].count) * 0x100000001B3ull;
     }
     std::sort(ranges.begin(), ranges.end());
     for (size_t k = 1; k < ranges.size(); ++k)
         if (ranges[k].first < ranges[k - 1].second) return fail(SPH_ERR_RANGE, "cell ranges overlap at particle %llu", (unsigned long long)ranges[k].first);
     s->cells.assign(cells, cells + n_cells);
+    s->cells_hash = hash;
     return SPH_OK;
+    SPH_API_END
 }
 
 // ------------------------------------------------------------------ hot path entry points
@@ -497,20 +506,35 @@ static int32_t cell_range(const sph_batch* b, uint32_t cell_first, uint32_t cell
     return SPH_OK;
 }
 
-int32_t sph_pack_cells(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes,
-                       uint32_t cell_first, uint32_t cell_count, void* stream) {
+// A batch indexes particles through the cell table it was built against: it may be used with any store that holds the
+// same number of particles under the same cell table (e.g. an AoS and a split-AoS store of one particle set).
+static int32_t batch_store_check(const sph_store* s, const sph_batch* b) {
+    if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
+    if (b->cells_hash != s->cells_hash) return fail(SPH_ERR_INVALID_ARG, "batch was built against another cell table than the store's");
+    return SPH_OK;
+}
+
+static int32_t transfer_check(const sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf) {
     if (int32_t rc = store_check(s)) return rc;
     if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
-    if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
+    if (!set) return fail(SPH_ERR_INVALID_ARG, "attribute set is NULL");
+    return batch_store_check(s, b);
+}
+
+int32_t sph_pack_cells(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes,
+                       uint32_t cell_first, uint32_t cell_count, void* stream) {
+    if (int32_t rc = transfer_check(s, b, set, d_buf)) return rc;
+    SPH_API_BEGIN
     Program prog;
     if (int32_t rc = build_pack_program(s->layout, *set, &prog)) return rc;
-    const OffsetTable* ot = find_offsets(b, prog.rec_words * 4);
-    if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
+    const OffsetTable* ot = nullptr;
+    if (int32_t rc = ensure_offsets(b, prog.rec_words * 4, &ot)) return rc;
     if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
     uint32_t cc0 = 0, ncc = 0;
     if (int32_t rc = cell_range(b, cell_first, cell_count, &cc0, &ncc)) return rc;
     return launch_pack(s->view(), b, prog, ot->d_occ_off128, (char*)d_buf, cc0, ncc, (cudaStream_t)stream);
+    SPH_API_END
 }
 
 int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set, void* d_buf, uint64_t buf_bytes, void* stream) {
@@ -520,13 +544,12 @@ int32_t sph_pack(const sph_store* s, const sph_batch* b, const sph_attrset* set,
 
 int32_t sph_unpack_cells(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode,
                          uint32_t cell_first, uint32_t cell_count, void* stream) {
-    if (int32_t rc = store_check(s)) return rc;
-    if (!b || !d_buf) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
-    if (b->store_n != s->n) return fail(SPH_ERR_INVALID_ARG, "batch was built for a store of %llu particles", (unsigned long long)b->store_n);
+    if (int32_t rc = transfer_check(s, b, set, d_buf)) return rc;
+    SPH_API_BEGIN
     Program prog;
     if (int32_t rc = build_unpack_program(s->layout, *set, mode, &prog)) return rc;
-    const OffsetTable* ot = find_offsets(b, prog.rec_words * 4);
-    if (!ot) return fail(SPH_ERR_INVALID_ARG, "no offset table for %u-byte records: call sph_batch_buffer_bytes first", prog.rec_words * 4);
+    const OffsetTable* ot = nullptr;
+    if (int32_t rc = ensure_offsets(b, prog.rec_words * 4, &ot)) return rc;
     if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
     if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
     uint32_t cc0 = 0, ncc = 0;
@@ -534,6 +557,7 @@ int32_t sph_unpack_cells(sph_store* s, const sph_batch* b, const sph_attrset* se
     bool all_assign = true;
     for (uint32_t w = 0; w < prog.rec_words; ++w) all_assign &= prog.word[w].kind == W_ASSIGN || prog.word[w].kind == W_ASSIGN_BYTE;
     return launch_unpack(s->view(), b, prog, ot->d_occ_off128, (const char*)d_buf, all_assign, mode == SPH_UNPACK_REDUCE_ZERO, cc0, ncc, (cudaStream_t)stream);
+    SPH_API_END
 }
 
 int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes, int32_t mode, void* stream) {
@@ -544,9 +568,8 @@ int32_t sph_unpack(sph_store* s, const sph_batch* b, const sph_attrset* set, con
 static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, uint32_t rec_in,
                           uint32_t rec_out, const OffsetTable** oin, const OffsetTable** oout) {
     if (!b || !d_in || !d_out) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
-    *oin = find_offsets(b, rec_in);
-    *oout = find_offsets(b, rec_out);
-    if (!*oin || !*oout) return fail(SPH_ERR_INVALID_ARG, "canonical offset tables missing");
+    if (int32_t rc = ensure_offsets(b, rec_in, oin)) return rc;
+    if (int32_t rc = ensure_offsets(b, rec_out, oout)) return rc;
     if (in_bytes < (*oin)->total) return fail(SPH_ERR_RANGE, "input buffer of %llu bytes, %llu needed", (unsigned long long)in_bytes, (unsigned long long)(*oin)->total);
     if (out_bytes < (*oout)->total) return fail(SPH_ERR_RANGE, "output buffer of %llu bytes, %llu needed", (unsigned long long)out_bytes, (unsigned long long)(*oout)->total);
     if (((uintptr_t)d_in | (uintptr_t)d_out) & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
@@ -554,16 +577,20 @@ static int32_t loop_check(const sph_batch* b, const void* d_in, uint64_t in_byte
 }
 
 int32_t sph_density(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, void* stream) {
+    SPH_API_BEGIN
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 20, 16, &oin, &oout)) return rc;
-    return launch_density(b, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+    return launch_density(b, *oin, *oout, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+    SPH_API_END
 }
 
 int32_t sph_force(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, const sph_params* prm, void* stream) {
     if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
+    SPH_API_BEGIN
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 52, 20, &oin, &oout)) return rc;
-    return launch_force(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    return launch_force(b, *oin, *oout, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    SPH_API_END
 }
 
 int32_t sph_ghost(sph_store* s, const sph_params* prm, void* stream) {

@@ -1,7 +1,8 @@
 // Batches ("bundles"): the immutable device tables every kernel of the hot path indexes.
 #include <algorithm>
 #include <cstring>
-#include <new>
+#include <memory>
+#include <numeric>
 
 #include "internal.h"
 
@@ -20,18 +21,17 @@ int32_t upload(const std::vector<T>& v, T** d) {
     return SPH_OK;
 }
 
+struct BatchDeleter { void operator()(sph_batch* b) const { sph_batch_destroy(b); } };
+
 }  // namespace
 
 namespace sph {
 
-const OffsetTable* find_offsets(const sph_batch* b, uint32_t rec_bytes) {
-    auto it = b->offsets.find(rec_bytes);
-    return it == b->offsets.end() ? nullptr : &it->second;
-}
-
 // Block offsets for one record size: every block starts at the next multiple of 128 bytes, every segment at
 // the next multiple of 256 bytes (a segment is laid out exactly like a stand-alone batch of its tasks).
-int32_t ensure_offsets(sph_batch* b, uint32_t rec_bytes, const OffsetTable** out) {
+// Built the first time a record size is used (any thread), found afterwards; the batch's other tables never change.
+int32_t ensure_offsets(const sph_batch* b, uint32_t rec_bytes, const OffsetTable** out) {
+    std::lock_guard<std::mutex> lock(b->mu);
     auto it = b->offsets.find(rec_bytes);
     if (it != b->offsets.end()) { if (out) *out = &it->second; return SPH_OK; }
     OffsetTable ot;
@@ -67,34 +67,33 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     *out = nullptr;
     if (!store || !tasks || n_tasks == 0) return fail(SPH_ERR_INVALID_ARG, "store or tasks is NULL, or no tasks");
     if (store->cells.empty()) return fail(SPH_ERR_INVALID_ARG, "the store has no cell table (sph_store_set_cells)");
-    if (n_tasks >= (1ull << 31)) return fail(SPH_ERR_RANGE, "too many tasks");
+    if (n_tasks >= (1ull << 30)) return fail(SPH_ERR_RANGE, "too many tasks (%llu; side indices are 32-bit)", (unsigned long long)n_tasks);
+    SPH_API_BEGIN
     const uint32_t n_cells = (uint32_t)store->cells.size();
-    sph_batch* b = new (std::nothrow) sph_batch();
-    if (!b) return fail(SPH_ERR_ALLOC, "host allocation failed");
+    std::unique_ptr<sph_batch, BatchDeleter> holder(new sph_batch());
+    sph_batch* b = holder.get();
     b->n_tasks = n_tasks;
     b->store_n = store->n;
+    b->cells_hash = store->cells_hash;
     b->tasks_per_segment = tasks_per_segment;
     b->n_segments = tasks_per_segment ? (uint32_t)((n_tasks + tasks_per_segment - 1) / tasks_per_segment) : 1;
     std::vector<double> frames;
-    std::vector<uint32_t> chunk_side, chunk_src;
+    std::vector<uint32_t> partner;            // per side: the side its targets gather from
     b->task_side0.resize(n_tasks + 1);
     b->sides.reserve(2 * n_tasks);
     frames.reserve(6 * n_tasks);
+    partner.reserve(2 * n_tasks);
     for (uint64_t t = 0; t < n_tasks; ++t) {
         const sph_task& tk = tasks[t];
         b->task_side0[t] = (uint32_t)b->sides.size();
-        if (tk.ci < 0 || (uint32_t)tk.ci >= n_cells || tk.cj < -1 || (tk.cj >= 0 && (uint32_t)tk.cj >= n_cells) || tk.cj == tk.ci) {
-            delete b;
+        if (tk.ci < 0 || (uint32_t)tk.ci >= n_cells || tk.cj < -1 || (tk.cj >= 0 && (uint32_t)tk.cj >= n_cells) || tk.cj == tk.ci)
             return fail(SPH_ERR_RANGE, "task %llu references cells (%d, %d); the store has %u", (unsigned long long)t, tk.ci, tk.cj, n_cells);
-        }
         for (int side = 0; side < (tk.cj >= 0 ? 2 : 1); ++side) {
             const uint32_t c = (uint32_t)(side == 0 ? tk.ci : tk.cj);
             const sph_cell& ce = store->cells[c];
-            SideRec sr{(uint32_t)ce.first, ce.count, (uint32_t)chunk_side.size(), c};
             const uint32_t sidx = (uint32_t)b->sides.size();
-            const uint32_t partner = tk.cj >= 0 ? (side == 0 ? sidx + 1 : sidx - 1) : sidx;
-            for (uint32_t k = 0; k < ce.count; k += kLoopTargets) { chunk_side.push_back(sidx); chunk_src.push_back(partner); }
-            b->sides.push_back(sr);
+            partner.push_back(tk.cj >= 0 ? (side == 0 ? sidx + 1 : sidx - 1) : sidx);
+            b->sides.push_back(SideRec{(uint32_t)ce.first, ce.count, 0u, c});
             const double* fr = side == 0 ? tk.frame_i : tk.frame_j;
             frames.insert(frames.end(), fr, fr + 3);
             b->n_instances += ce.count;
@@ -106,7 +105,6 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     }
     b->task_side0[n_tasks] = (uint32_t)b->sides.size();
     b->n_sides = (uint32_t)b->sides.size();
-    b->n_chunks = (uint32_t)chunk_side.size();
 
     // per-cell occurrence lists in ascending (task, side) order = ascending side index
     std::vector<uint32_t> occ_count(n_cells, 0);
@@ -132,36 +130,68 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     b->cell_chunk0[n_cells] = b->n_cell_chunks;
     b->n_occ = b->n_sides;
 
-    int32_t rc = upload(cell_chunks, &b->d_cell_chunks);
+    if (int32_t rc = upload(cell_chunks, &b->d_cell_chunks)) return rc;
     std::vector<double> occ_frames(3 * (size_t)b->n_sides);
     for (uint32_t o = 0; o < b->n_sides; ++o) std::copy_n(&frames[3 * (size_t)occ_side[o]], 3, &occ_frames[3 * (size_t)o]);
-    if (!rc) rc = upload(occ_frames, &b->d_occ_frames);
+    if (int32_t rc = upload(occ_frames, &b->d_occ_frames)) return rc;
     for (uint32_t rec : {16u, 20u, 52u})
-        if (!rc) rc = ensure_offsets(b, rec, nullptr);
-    // loop work items (one per 32-particle target chunk), for the canonical record sizes of the two loops
-    if (!rc && b->max_count >= (1u << 25)) rc = fail(SPH_ERR_RANGE, "a cell of %u particles is too large for the loop item table", b->max_count);
-    if (!rc) {
-        const std::vector<uint64_t>&o16 = find_offsets(b, 16)->h_off, &o20 = find_offsets(b, 20)->h_off, &o52 = find_offsets(b, 52)->h_off;
-        std::vector<LoopItem> dens(b->n_chunks), forc(b->n_chunks);
-        for (uint32_t ch = 0; ch < b->n_chunks; ++ch) {
-            const uint32_t tgt = chunk_side[ch], src = chunk_src[ch];
-            const uint32_t kc = ch - b->sides[tgt].chunk0;                       // chunk index inside the block
-            const uint32_t nt_ns = std::min(kLoopTargets, b->sides[tgt].count - kLoopTargets * kc) | b->sides[src].count << 7;
-            const uint32_t u = kLoopTargets / 32;                                // 32 records of r bytes = r units of 128 bytes
-            dens[ch] = LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5 * u, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns};
-            forc[ch] = LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13 * u, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns};
+        if (int32_t rc = ensure_offsets(b, rec, nullptr)) return rc;
+
+    // the interaction loops' view: per occurrence where its targets gather from and how the two frames relate;
+    // work items = 64-particle chunks of the touched cells, heaviest first (a cell of 10^5 particles must not start last)
+    {
+        std::vector<LoopOcc> locc(b->n_sides);
+        std::vector<LoopChunk> chunks;
+        std::vector<uint64_t> work;
+        for (uint32_t c = 0; c < n_cells; ++c) {
+            if (!occ_count[c]) continue;
+            const double* f0 = &frames[3 * (size_t)occ_side[occ_start[c]]];      // frame of the cell's first occurrence
+            uint64_t n_src_total = 0;
+            for (uint32_t o = occ_start[c]; o < occ_start[c + 1]; ++o) {
+                const uint32_t s = occ_side[o], p = partner[s], cs = b->sides[p].cell;
+                const double* ft = &frames[3 * (size_t)s];
+                const double* fs = &frames[3 * (size_t)p];
+                const double* f0s = &frames[3 * (size_t)occ_side[occ_start[cs]]];
+                LoopOcc lo{};
+                lo.tgt_side = s; lo.src_side = p; lo.n_src = b->sides[p].count; lo.src_cc0 = b->cell_chunk0[cs];
+                for (int d = 0; d < 3; ++d) {
+                    const double D = ft[d] - f0[d];
+                    lo.D[d] = (float)D;
+                    lo.E[d] = (float)(D + (f0s[d] - fs[d]));
+                }
+                locc[o] = lo;
+                n_src_total += lo.n_src;
+            }
+            const sph_cell& ce = store->cells[c];
+            for (uint32_t k = 0; k < ce.count; k += kLoopTargets) {
+                const uint32_t cnt = std::min(kLoopTargets, ce.count - k);
+                chunks.push_back(LoopChunk{k, cnt, occ_start[c], occ_count[c]});
+                work.push_back((uint64_t)cnt * n_src_total);
+            }
         }
-        rc = upload(dens, &b->d_items_density);
-        if (!rc) rc = upload(forc, &b->d_items_force);
+        std::vector<uint32_t> order(chunks.size());
+        std::iota(order.begin(), order.end(), 0u);
+        std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t c) { return work[a] > work[c]; });
+        std::vector<LoopChunk> sorted(chunks.size());
+        for (size_t k = 0; k < order.size(); ++k) sorted[k] = chunks[order[k]];
+        b->n_chunks = (uint32_t)sorted.size();
+        if (int32_t rc = upload(locc, &b->d_loop_occ)) return rc;
+        if (int32_t rc = upload(sorted, &b->d_loop_chunks)) return rc;
+        for (int k = 0; k < 3; ++k) {
+            if (!b->n_cell_chunks) break;
+            cudaError_t e = cudaMalloc((void**)&b->d_boxes[k], (size_t)b->n_cell_chunks * sizeof(ChunkBox));
+            if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? SPH_ERR_ALLOC : SPH_ERR_CUDA, "cudaMalloc(chunk boxes): %s", cudaGetErrorString(e));
+        }
     }
-    if (rc) { sph_batch_destroy(b); return rc; }
-    *out = b;
+    *out = holder.release();
     return SPH_OK;
+    SPH_API_END
 }
 
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
-    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
+    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_loop_chunks); cudaFree(b->d_loop_occ);
+    for (ChunkBox* p : b->d_boxes) cudaFree(p);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;
@@ -175,18 +205,21 @@ int32_t sph_batch_get_info(const sph_batch* b, sph_batch_info* info) {
     return SPH_OK;
 }
 
-int32_t sph_batch_buffer_bytes(sph_batch* b, const sph_attrset* set, uint64_t* bytes_out) {
+int32_t sph_batch_buffer_bytes(const sph_batch* b, const sph_attrset* set, uint64_t* bytes_out) {
     if (!b || !bytes_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    SPH_API_BEGIN
     uint32_t rec;
     if (int32_t rc = attrset_check(set, &rec)) return rc;
     const OffsetTable* ot;
     if (int32_t rc = ensure_offsets(b, rec, &ot)) return rc;
     *bytes_out = ot->total;
     return SPH_OK;
+    SPH_API_END
 }
 
-int32_t sph_batch_block_offsets(sph_batch* b, const sph_attrset* set, uint64_t* off_out, uint64_t* seg_off_out) {
+int32_t sph_batch_block_offsets(const sph_batch* b, const sph_attrset* set, uint64_t* off_out, uint64_t* seg_off_out) {
     if (!b || !off_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    SPH_API_BEGIN
     uint32_t rec;
     if (int32_t rc = attrset_check(set, &rec)) return rc;
     const OffsetTable* ot;
@@ -197,6 +230,7 @@ int32_t sph_batch_block_offsets(sph_batch* b, const sph_attrset* set, uint64_t* 
     }
     if (seg_off_out) std::copy(ot->seg_off.begin(), ot->seg_off.end(), seg_off_out);
     return SPH_OK;
+    SPH_API_END
 }
 
 }  // extern "C"

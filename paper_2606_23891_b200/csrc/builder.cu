@@ -1,6 +1,6 @@
 // Host-side setup: cell grid / octree and the task list.
 // Plain C++ (no device code); written independently of the oracle's builders and cross-checked against them
-// in tests/test_host_builder.py.
+// in tests/test_host_side.py.
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
@@ -36,6 +36,31 @@ inline double gap_1d(double a, double wa, double b, double wb, double box, doubl
     return g[best];
 }
 
+// Order inside a cell (reading C26): ascending Morton code of the position on a 32^3 sub-grid of the cell, ties in
+// input order.  Spatially compact runs of particles are what lets the interaction loops drop whole chunks of a
+// neighbouring cell before any distance test.  spread5: bits b of a 5-bit number go to bits 3b.
+inline uint32_t spread5(uint32_t v) { return (v & 1u) | (v & 2u) << 2 | (v & 4u) << 4 | (v & 8u) << 6 | (v & 16u) << 8; }
+inline uint32_t sub_cell_code(const double* x, const double* o, double w) {
+    uint32_t q[3];
+    for (int d = 0; d < 3; ++d) {
+        const double f = std::floor((x[d] - o[d]) / w * 32.0);
+        q[d] = f < 0.0 ? 0u : (f > 31.0 ? 31u : (uint32_t)f);
+    }
+    return spread5(q[0]) << 2 | spread5(q[1]) << 1 | spread5(q[2]);
+}
+// idx[lo, hi) -> Morton order inside the cell; scratch holds (code << 32 | position) so that one plain sort is stable
+void order_inside_cell(const double* x3, uint64_t* idx, uint64_t lo, uint64_t hi, const double* o, double w, std::vector<uint64_t>& scratch,
+                       std::vector<uint64_t>& tmp) {
+    const uint64_t cnt = hi - lo;
+    if (cnt < 2) return;
+    scratch.resize(cnt);
+    tmp.resize(cnt);
+    for (uint64_t k = 0; k < cnt; ++k) scratch[k] = (uint64_t)sub_cell_code(x3 + 3 * idx[lo + k], o, w) << 32 | k;
+    std::sort(scratch.begin(), scratch.end());
+    for (uint64_t k = 0; k < cnt; ++k) tmp[k] = idx[lo + (scratch[k] & 0xFFFFFFFFull)];
+    std::copy(tmp.begin(), tmp.end(), idx + lo);
+}
+
 }  // namespace
 
 extern "C" {
@@ -45,6 +70,7 @@ int32_t sph_free(void* p) { std::free(p); return SPH_OK; }
 int32_t sph_cells_build_grid(const double* x3, uint64_t n, uint32_t cpd, double box, uint64_t* perm_out, sph_cell* cells_out) {
     if (!x3 || !perm_out || !cells_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
     if (cpd == 0 || cpd > 1024 || !(box > 0)) return fail(SPH_ERR_INVALID_ARG, "cells_per_dim %u, box %g", cpd, box);
+    SPH_API_BEGIN
     const uint64_t nc = (uint64_t)cpd * cpd * cpd;
     std::vector<uint32_t> key(n);
     std::vector<uint64_t> head(nc + 1, 0);
@@ -73,13 +99,17 @@ int32_t sph_cells_build_grid(const double* x3, uint64_t n, uint32_t cpd, double 
     }
     std::vector<uint64_t> cursor(head.begin(), head.end() - 1);
     for (uint64_t p = 0; p < n; ++p) perm_out[cursor[key[p]]++] = p;   // counting sort: stable
+    std::vector<uint64_t> scratch, tmp;
+    for (uint64_t c = 0; c < nc; ++c) order_inside_cell(x3, perm_out, head[c], head[c + 1], cells_out[c].origin, w, scratch, tmp);
     return SPH_OK;
+    SPH_API_END
 }
 
 int32_t sph_cells_build_octree(const double* x3, const float* h, uint64_t n, uint32_t max_per_leaf, double box, uint64_t* perm_out,
                                sph_cell** cells_out, uint32_t* n_cells_out) {
     if (!x3 || !h || !perm_out || !cells_out || !n_cells_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
     if (max_per_leaf == 0 || !(box > 0)) return fail(SPH_ERR_INVALID_ARG, "max_per_leaf %u, box %g", max_per_leaf, box);
+    SPH_API_BEGIN
     for (uint64_t p = 0; p < n; ++p)
         for (int d = 0; d < 3; ++d)
             if (!(x3[3 * p + d] >= 0.0 && x3[3 * p + d] < box)) return fail(SPH_ERR_RANGE, "particle %llu outside the box", (unsigned long long)p);
@@ -125,6 +155,8 @@ int32_t sph_cells_build_octree(const double* x3, const float* h, uint64_t n, uin
             stack.push_back(ch);
         }
     }
+    std::vector<uint64_t> scratch;
+    for (const sph_cell& ce : leaves) order_inside_cell(x3, idx.data(), ce.first, ce.first + ce.count, ce.origin, ce.width, scratch, tmp);
     std::copy(idx.begin(), idx.end(), perm_out);
     sph_cell* out = (sph_cell*)std::malloc(std::max<size_t>(1, leaves.size()) * sizeof(sph_cell));
     if (!out) return fail(SPH_ERR_ALLOC, "cells allocation failed");
@@ -132,13 +164,21 @@ int32_t sph_cells_build_octree(const double* x3, const float* h, uint64_t n, uin
     *cells_out = out;
     *n_cells_out = (uint32_t)leaves.size();
     return SPH_OK;
+    SPH_API_END
 }
 
 int32_t sph_tasks_build(const sph_cell* cells, const float* hmax, uint32_t n_cells, double box, sph_task** tasks_out, uint64_t* n_self_out,
                         uint64_t* n_pair_out) {
     if (!cells || !hmax || !tasks_out || n_cells == 0) return fail(SPH_ERR_INVALID_ARG, "NULL argument or no cells");
+    SPH_API_BEGIN
     double reach = 0;   // largest cut-off any pair can have
-    for (uint32_t c = 0; c < n_cells; ++c) reach = std::max(reach, 2.0 * (double)hmax[c]);
+    for (uint32_t c = 0; c < n_cells; ++c) {
+        reach = std::max(reach, 2.0 * (double)hmax[c]);
+        // a cell must not see its own periodic image: the self task is not periodic
+        if (cells[c].count && !(box - cells[c].width >= 2.0 * (double)hmax[c]))
+            return fail(SPH_ERR_RANGE, "cell %u (width %g, 2 hmax %g) interacts with its own periodic image in a box of %g", c, cells[c].width,
+                        2.0 * (double)hmax[c], box);
+    }
     // bin the cells on a uniform grid; a cell is listed in every bin its box overlaps
     int nb = (int)std::min(64.0, std::max(1.0, std::floor(box / std::max(reach, 1e-9))));
     nb = std::min(nb, std::max(1, (int)std::cbrt((double)n_cells)));
@@ -200,6 +240,7 @@ int32_t sph_tasks_build(const sph_cell* cells, const float* hmax, uint32_t n_cel
     if (n_self_out) *n_self_out = n_cells;
     if (n_pair_out) *n_pair_out = tasks.size() - n_cells;
     return SPH_OK;
+    SPH_API_END
 }
 
 }  // extern "C"

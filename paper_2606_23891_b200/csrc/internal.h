@@ -7,6 +7,8 @@
 #include <cstdint>
 #include <cstdio>
 #include <map>
+#include <mutex>
+#include <new>
 #include <vector>
 
 #include "sph_b200.h"
@@ -14,6 +16,12 @@
 namespace sph {
 
 int32_t fail(int32_t code, const char* fmt, ...);
+// Every extern "C" body that can allocate sits between these two: nothing is thrown across the C ABI.
+#define SPH_API_BEGIN try {
+#define SPH_API_END                                                                                         \
+    }                                                                                                       \
+    catch (const std::bad_alloc&) { return ::sph::fail(SPH_ERR_ALLOC, "host allocation failed"); }          \
+    catch (...) { return ::sph::fail(SPH_ERR_INVALID_ARG, "unexpected C++ exception"); }
 #define SPH_CUDA_TRY(expr)                                                                             \
     do {                                                                                               \
         cudaError_t e_ = (expr);                                                                       \
@@ -40,7 +48,7 @@ struct StoreView {
 struct SideRec {
     uint32_t first;    // first particle of the cell
     uint32_t count;    // particles in the cell
-    uint32_t chunk0;   // index of the block's first 64-target chunk in the loop item tables
+    uint32_t pad;
     uint32_t cell;
 };
 
@@ -53,14 +61,36 @@ struct CellChunk {
     uint32_t nocc;
 };
 
-// work item of the density / force loops: up to 64 targets of one block (two per lane) against the block they gather from.
-// Offsets in units of 128 bytes into the loop's input / output buffer (chunk starts are multiples of 128 bytes).
+// Work item of the interaction loops: up to 64 consecutive particles of one CELL (two per lane) against every block the cell
+// gathers from in this batch (its occurrences [occ0, occ0 + nocc), ascending (task, side) order).
 constexpr uint32_t kLoopTargets = 64;
-struct LoopItem {
-    uint32_t tin128;     // the targets' input records
-    uint32_t sin128;     // first input record of the source block
-    uint32_t tout128;    // the targets' result records
-    uint32_t nt_ns;      // targets (1..64) | sources << 7
+struct LoopChunk {
+    uint32_t k0;       // offset of the chunk inside its cell (multiple of 64)
+    uint32_t count;    // 1..64
+    uint32_t occ0;
+    uint32_t nocc;
+};
+
+// One occurrence of a cell as a target block, as the loops see it (cell-major, ascending side: same order as occ_side).
+// The chunk's own coordinates are read once, from the cell's FIRST occurrence (frame F0); the sources of occurrence o come
+// in the frame of their own block, and  x_i(o) - x_j(o) = x_i(F0) - (x_j(o) + D_o),  D_o = frame_tgt(o) - F0.
+struct LoopOcc {
+    uint32_t tgt_side;   // the block (side index) the results go to
+    uint32_t src_side;   // the block the targets gather from: the task's other side, or the block itself (self task)
+    uint32_t n_src;      // particles in the source block
+    uint32_t src_cc0;    // first 32-particle chunk of the source CELL in the chunk-box table
+    float D[3];          // added to the source coordinates
+    float pad0;
+    float E[3];          // added to the source cell's chunk boxes (kept in the frame of that cell's first occurrence)
+    float pad1;
+};
+static_assert(sizeof(LoopOcc) == 48, "three 16-byte loads");
+
+// bounding box of the positions of one 32-particle chunk of a cell (frame of the cell's first occurrence) and its largest h
+struct ChunkBox {
+    float lo[3], hi[3];
+    float hmax;
+    float pad;
 };
 
 // word kinds of the pack / unpack programs
@@ -123,6 +153,7 @@ struct sph_store {
     bool owned[SPH_MAX_SUB] = {};
     uint64_t bytes[SPH_MAX_SUB] = {};
     std::vector<sph_cell> cells;
+    uint64_t cells_hash = 0;      // of the (first, count) pairs of the cell table: what a batch is tied to
     sph::StoreView view() const {
         sph::StoreView v{};
         for (uint32_t s = 0; s < layout.n_sub; ++s) { v.base[s] = base[s]; v.stride[s] = layout.stride[s]; }
@@ -134,6 +165,7 @@ struct sph_batch {
     uint64_t n_tasks = 0, n_self = 0, n_pair = 0;
     uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
     uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
+    uint64_t cells_hash = 0;                  // of the cell table the batch was built against
     std::vector<sph::SideRec> sides;          // host copy
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists
     std::vector<uint32_t> task_side0;         // n_tasks + 1
@@ -141,14 +173,19 @@ struct sph_batch {
     // device tables
     double* d_occ_frames = nullptr;           // 3 per occurrence (cell-major, ascending side): the frame of that side
     sph::CellChunk* d_cell_chunks = nullptr;
-    sph::LoopItem* d_items_density = nullptr; // one per 64-target chunk of a block (20-byte in, 16-byte out records)
-    sph::LoopItem* d_items_force = nullptr;   // (52-byte in, 20-byte out records)
-    std::map<uint32_t, sph::OffsetTable> offsets;   // by record bytes
+    sph::LoopChunk* d_loop_chunks = nullptr;  // n_chunks work items of the interaction loops, heaviest first
+    sph::LoopOcc* d_loop_occ = nullptr;       // per occurrence
+    sph::ChunkBox* d_boxes[3] = {};           // per loop kind (density, gradient, force): chunk boxes written by the loop's own
+                                              // first kernel from ITS input buffer (scratch: one call per kind at a time)
+    // block offsets by record bytes: the only part that grows after sph_batch_create (a table is built the first time a
+    // record size is asked for, under the mutex; tables are never removed, so pointers to them stay valid)
+    mutable std::mutex mu;
+    mutable std::map<uint32_t, sph::OffsetTable> offsets;
 };
 
 namespace sph {
-const OffsetTable* find_offsets(const sph_batch* batch, uint32_t rec_bytes);
-int32_t ensure_offsets(sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
+int32_t ensure_offsets(const sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
+int32_t device_sms(int* sms_out);      // SM count of the current device
 
 // kernel launchers (kernels_*.cu)
 // [cc0, cc0 + ncc): the cell chunks to work on
@@ -156,8 +193,9 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
                     uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st);
-int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
-int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
+int32_t launch_density(const sph_batch* b, const OffsetTable& oin, const OffsetTable& oout, const char* d_in, char* d_out, cudaStream_t st);
+int32_t launch_force(const sph_batch* b, const OffsetTable& oin, const OffsetTable& oout, const char* d_in, char* d_out, const sph_params& prm,
+                     cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);
 int32_t launch_ghost(const StoreView& view, uint64_t n, const sph_layout& layout, const sph_params& prm, cudaStream_t st);
 }  // namespace sph

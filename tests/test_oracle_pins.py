@@ -268,17 +268,56 @@ def test_force_continuum_limit_pressure_gradient():
 
 # ------------------------------------------------------------------ cells and tasks
 
+def _morton_code(x, origin, width):
+    """reading C26, restated: 5 bits per axis of floor((x - origin) / width * 32), x most significant in every bit triple"""
+    q = np.clip(np.floor((x - origin) / width * 32.0), 0, 31).astype(np.int64)
+    code = np.zeros(x.shape[0], dtype=np.int64)
+    for b in range(5):
+        for d in range(3):
+            code |= ((q[:, d] >> b) & 1) << (3 * b + (2 - d))
+    return code
+
+
+def test_order_inside_a_cell_is_morton_and_compact():
+    # hand-placed points in one cell of a 3^3 grid: the order is fixed by the definition (octant 4bx + 2by + bz first, then
+    # the same rule inside the octant), whatever order they were generated in
+    w = 1.0 / 3.0
+    rel = np.array([[0.9, 0.9, 0.9], [0.1, 0.1, 0.1], [0.1, 0.1, 0.9], [0.9, 0.1, 0.1], [0.1, 0.9, 0.1], [0.3, 0.1, 0.1], [0.1, 0.1, 0.3],
+                    [0.1, 0.1, 0.1]])
+    parts = np.zeros(rel.shape[0], dtype=si.PART_DTYPE)
+    parts["x"] = (1.0 + rel) * w                       # all in cell (1, 1, 1)
+    parts["id"] = np.arange(rel.shape[0])
+    perm, cells = orc.cells_build_grid(parts["x"], 3)
+    c = 13
+    assert cells["count"][c] == rel.shape[0] and cells["count"].sum() == rel.shape[0]
+    # octant 0: (.1,.1,.1) twice in generator order [1, 7], then z-neighbour (.1,.1,.3) [6], x-neighbour (.3,.1,.1) [5];
+    # then octants 1 (z high) [2], 2 (y high) [4], 4 (x high) [3], 7 [0]
+    assert perm.tolist() == [1, 7, 6, 5, 2, 4, 3, 0]
+    # a jittered lattice: any 8 consecutive particles of a 64-particle cell form one octant of it
+    parts = si.jittered_lattice(12, 3, jitter=0.2)
+    perm, cells = orc.cells_build_grid(parts["x"], 3)
+    ps = parts[perm.astype(np.int64)]
+    for c in (0, 13, 26):
+        f = int(cells["first"][c])
+        assert cells["count"][c] == 64
+        for o in range(8):
+            x = (ps["x"][f + 8 * o:f + 8 * o + 8] - cells["origin"][c]) / cells["width"][c]
+            assert np.all((x >= 0.5) == np.array([(o >> 2) & 1, (o >> 1) & 1, o & 1], dtype=bool))
+
+
 def test_grid_cells_and_tasks_structure():
     parts = si.jittered_lattice(12, 7)
     perm, cells = orc.cells_build_grid(parts["x"], 4)
     assert sorted(perm.tolist()) == list(range(12 ** 3))
     ps = parts[perm.astype(np.int64)]
-    # particles inside their cell's box, cells contiguous, stable order (ids ascending inside a cell)
+    # particles inside their cell's box, cells contiguous, Morton order inside a cell with ties in generator order (C26)
     for c in range(64):
         f, k = int(cells["first"][c]), int(cells["count"][c])
         x = ps["x"][f:f + k]
         assert np.all(x >= cells["origin"][c]) and np.all(x < cells["origin"][c] + cells["width"][c])
-        assert np.all(np.diff(ps["id"][f:f + k]) > 0)
+        code = _morton_code(x, cells["origin"][c], cells["width"][c])
+        key = code.astype(np.int64) * (1 << 32) + ps["id"][f:f + k]
+        assert np.all(np.diff(key) > 0)
     assert cells["first"][0] == 0 and np.all(cells["first"][1:] == np.cumsum(cells["count"])[:-1])
     tasks, ns, npair = orc.tasks_build(cells, orc.cell_hmax(ps, cells))
     assert (ns, npair) == (64, 64 * 13)
