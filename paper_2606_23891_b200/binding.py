@@ -86,7 +86,7 @@ def lib_path() -> str:
 
 
 def _load():
-    path = _build.build()          # (re)builds with nvcc when sources are newer; raises if that is impossible
+    path = os.environ.get("SPH_B200_LIB") or _build.build()   # (re)builds with nvcc when sources are newer; raises if that is impossible
     if not os.path.exists(path):
         raise ImportError(f"{path} is missing: run `python -m paper_2606_23891_b200.build`")
     lib = C.CDLL(path)
@@ -114,6 +114,11 @@ def _ptr(x):
     if hasattr(x, "data_ptr"):
         return C.c_void_p(x.data_ptr())
     return C.c_void_p(int(x))
+
+
+def _ref(struct):
+    """ctypes structure or None -> pointer argument"""
+    return None if struct is None else C.byref(struct)
 
 
 def _nbytes(x):
@@ -294,7 +299,7 @@ def sph_batch_get_info(batch) -> sph_batch_info:
 
 def sph_batch_buffer_bytes(batch, aset: sph_attrset) -> int:
     out = C.c_uint64(0)
-    _check(_lib.sph_batch_buffer_bytes(batch, C.byref(aset), C.byref(out)))
+    _check(_lib.sph_batch_buffer_bytes(batch, _ref(aset), C.byref(out)))
     return out.value
 
 
@@ -303,20 +308,20 @@ def sph_batch_block_offsets(batch, aset: sph_attrset):
     info = sph_batch_get_info(batch)
     off = np.empty(2 * info.n_tasks, dtype=np.uint64)
     seg = np.empty(info.n_segments, dtype=np.uint64)
-    _check(_lib.sph_batch_block_offsets(batch, C.byref(aset), _ptr(off), _ptr(seg)))
+    _check(_lib.sph_batch_block_offsets(batch, _ref(aset), _ptr(off), _ptr(seg)))
     return off, seg
 
 
 def sph_store_zero(store, aset: sph_attrset, stream=None) -> None:
-    _check(_lib.sph_store_zero(store, C.byref(aset), _stream(stream)))
+    _check(_lib.sph_store_zero(store, _ref(aset), _stream(stream)))
 
 
 def sph_pack(store, batch, aset: sph_attrset, d_buf, stream=None) -> None:
-    _check(_lib.sph_pack(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), _stream(stream)))
+    _check(_lib.sph_pack(store, batch, _ref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), _stream(stream)))
 
 
 def sph_pack_cells(store, batch, aset: sph_attrset, d_buf, cell_first: int, cell_count: int, stream=None) -> None:
-    _check(_lib.sph_pack_cells(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_uint32(cell_first), C.c_uint32(cell_count),
+    _check(_lib.sph_pack_cells(store, batch, _ref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_uint32(cell_first), C.c_uint32(cell_count),
                                _stream(stream)))
 
 
@@ -330,11 +335,11 @@ def sph_force(batch, d_in, d_out, params: sph_params, stream=None) -> None:
 
 
 def sph_unpack(store, batch, aset: sph_attrset, d_buf, mode: int = SPH_UNPACK_REDUCE, stream=None) -> None:
-    _check(_lib.sph_unpack(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), _stream(stream)))
+    _check(_lib.sph_unpack(store, batch, _ref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), _stream(stream)))
 
 
 def sph_unpack_cells(store, batch, aset: sph_attrset, d_buf, cell_first: int, cell_count: int, mode: int = SPH_UNPACK_REDUCE, stream=None) -> None:
-    _check(_lib.sph_unpack_cells(store, batch, C.byref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), C.c_uint32(cell_first),
+    _check(_lib.sph_unpack_cells(store, batch, _ref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), C.c_int32(mode), C.c_uint32(cell_first),
                                  C.c_uint32(cell_count), _stream(stream)))
 
 

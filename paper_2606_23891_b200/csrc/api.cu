@@ -580,7 +580,7 @@ int32_t sph_density(const sph_batch* b, const void* d_in, uint64_t in_bytes, voi
     SPH_API_BEGIN
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 20, 16, &oin, &oout)) return rc;
-    return launch_density(b, *oin, *oout, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+    return launch_density(b, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
     SPH_API_END
 }
 
@@ -589,7 +589,7 @@ int32_t sph_force(const sph_batch* b, const void* d_in, uint64_t in_bytes, void*
     SPH_API_BEGIN
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 52, 20, &oin, &oout)) return rc;
-    return launch_force(b, *oin, *oout, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    return launch_force(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
     SPH_API_END
 }
 

@@ -2,7 +2,6 @@
 #include <algorithm>
 #include <cstring>
 #include <memory>
-#include <numeric>
 
 #include "internal.h"
 
@@ -137,52 +136,28 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     for (uint32_t rec : {16u, 20u, 52u})
         if (int32_t rc = ensure_offsets(b, rec, nullptr)) return rc;
 
-    // the interaction loops' view: per occurrence where its targets gather from and how the two frames relate;
-    // work items = 64-particle chunks of the touched cells, heaviest first (a cell of 10^5 particles must not start last)
+    // loop work items (one per 64-target chunk of a block) for the canonical record sizes of the two loops, cell-major: the
+    // chunks of a cell's occurrences follow one another, so the warps that work on one cell run close together in time and
+    // its blocks are still in L2
     {
-        std::vector<LoopOcc> locc(b->n_sides);
-        std::vector<LoopChunk> chunks;
-        std::vector<uint64_t> work;
-        for (uint32_t c = 0; c < n_cells; ++c) {
-            if (!occ_count[c]) continue;
-            const double* f0 = &frames[3 * (size_t)occ_side[occ_start[c]]];      // frame of the cell's first occurrence
-            uint64_t n_src_total = 0;
+        const std::vector<uint64_t> &o16 = b->offsets.at(16).h_off, &o20 = b->offsets.at(20).h_off, &o52 = b->offsets.at(52).h_off;
+        std::vector<LoopItem> dens, forc;
+        for (uint32_t c = 0; c < n_cells; ++c)
             for (uint32_t o = occ_start[c]; o < occ_start[c + 1]; ++o) {
-                const uint32_t s = occ_side[o], p = partner[s], cs = b->sides[p].cell;
-                const double* ft = &frames[3 * (size_t)s];
-                const double* fs = &frames[3 * (size_t)p];
-                const double* f0s = &frames[3 * (size_t)occ_side[occ_start[cs]]];
-                LoopOcc lo{};
-                lo.tgt_side = s; lo.src_side = p; lo.n_src = b->sides[p].count; lo.src_cc0 = b->cell_chunk0[cs];
-                for (int d = 0; d < 3; ++d) {
-                    const double D = ft[d] - f0[d];
-                    lo.D[d] = (float)D;
-                    lo.E[d] = (float)(D + (f0s[d] - fs[d]));
+                const uint32_t tgt = occ_side[o], src = partner[tgt];
+                const uint32_t cnt = b->sides[tgt].count;
+                for (uint32_t k = 0, kc = 0; k < cnt; k += kLoopTargets, ++kc) {
+                    const uint32_t nt_ns = std::min(kLoopTargets, cnt - k) | b->sides[src].count << 7;
+                    const uint32_t u = kLoopTargets / 32;                                // 32 records of r bytes = r units of 128 bytes
+                    dens.push_back(LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5 * u, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns});
+                    forc.push_back(LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13 * u, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns});
                 }
-                locc[o] = lo;
-                n_src_total += lo.n_src;
             }
-            const sph_cell& ce = store->cells[c];
-            for (uint32_t k = 0; k < ce.count; k += kLoopTargets) {
-                const uint32_t cnt = std::min(kLoopTargets, ce.count - k);
-                chunks.push_back(LoopChunk{k, cnt, occ_start[c], occ_count[c]});
-                work.push_back((uint64_t)cnt * n_src_total);
-            }
-        }
-        std::vector<uint32_t> order(chunks.size());
-        std::iota(order.begin(), order.end(), 0u);
-        std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t c) { return work[a] > work[c]; });
-        std::vector<LoopChunk> sorted(chunks.size());
-        for (size_t k = 0; k < order.size(); ++k) sorted[k] = chunks[order[k]];
-        b->n_chunks = (uint32_t)sorted.size();
-        if (int32_t rc = upload(locc, &b->d_loop_occ)) return rc;
-        if (int32_t rc = upload(sorted, &b->d_loop_chunks)) return rc;
-        for (int k = 0; k < 3; ++k) {
-            if (!b->n_cell_chunks) break;
-            cudaError_t e = cudaMalloc((void**)&b->d_boxes[k], (size_t)b->n_cell_chunks * sizeof(ChunkBox));
-            if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? SPH_ERR_ALLOC : SPH_ERR_CUDA, "cudaMalloc(chunk boxes): %s", cudaGetErrorString(e));
-        }
+        b->n_items = (uint32_t)dens.size();
+        if (int32_t rc = upload(dens, &b->d_items_density)) return rc;
+        if (int32_t rc = upload(forc, &b->d_items_force)) return rc;
     }
+
     *out = holder.release();
     return SPH_OK;
     SPH_API_END
@@ -190,8 +165,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
-    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_loop_chunks); cudaFree(b->d_loop_occ);
-    for (ChunkBox* p : b->d_boxes) cudaFree(p);
+    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;

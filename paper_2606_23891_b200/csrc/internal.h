@@ -61,36 +61,13 @@ struct CellChunk {
     uint32_t nocc;
 };
 
-// Work item of the interaction loops: up to 64 consecutive particles of one CELL (two per lane) against every block the cell
-// gathers from in this batch (its occurrences [occ0, occ0 + nocc), ascending (task, side) order).
 constexpr uint32_t kLoopTargets = 64;
-struct LoopChunk {
-    uint32_t k0;       // offset of the chunk inside its cell (multiple of 64)
-    uint32_t count;    // 1..64
-    uint32_t occ0;
-    uint32_t nocc;
-};
-
-// One occurrence of a cell as a target block, as the loops see it (cell-major, ascending side: same order as occ_side).
-// The chunk's own coordinates are read once, from the cell's FIRST occurrence (frame F0); the sources of occurrence o come
-// in the frame of their own block, and  x_i(o) - x_j(o) = x_i(F0) - (x_j(o) + D_o),  D_o = frame_tgt(o) - F0.
-struct LoopOcc {
-    uint32_t tgt_side;   // the block (side index) the results go to
-    uint32_t src_side;   // the block the targets gather from: the task's other side, or the block itself (self task)
-    uint32_t n_src;      // particles in the source block
-    uint32_t src_cc0;    // first 32-particle chunk of the source CELL in the chunk-box table
-    float D[3];          // added to the source coordinates
-    float pad0;
-    float E[3];          // added to the source cell's chunk boxes (kept in the frame of that cell's first occurrence)
-    float pad1;
-};
-static_assert(sizeof(LoopOcc) == 48, "three 16-byte loads");
-
-// bounding box of the positions of one 32-particle chunk of a cell (frame of the cell's first occurrence) and its largest h
-struct ChunkBox {
-    float lo[3], hi[3];
-    float hmax;
-    float pad;
+// work item of the density / force loops: up to 64 targets of one block (two per lane) against the block they gather from.  Offsets in units of 128 bytes into the loop's input / output buffer (chunk starts are multiples of 128 bytes).
+struct LoopItem {
+    uint32_t tin128;     // the targets' input records
+    uint32_t sin128;     // first input record of the source block
+    uint32_t tout128;    // the targets' result records
+    uint32_t nt_ns;      // targets (1..64) | sources << 7
 };
 
 // word kinds of the pack / unpack programs
@@ -163,7 +140,7 @@ struct sph_store {
 
 struct sph_batch {
     uint64_t n_tasks = 0, n_self = 0, n_pair = 0;
-    uint32_t n_sides = 0, n_chunks = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
+    uint32_t n_sides = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
     uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
     uint64_t cells_hash = 0;                  // of the cell table the batch was built against
     std::vector<sph::SideRec> sides;          // host copy
@@ -173,10 +150,9 @@ struct sph_batch {
     // device tables
     double* d_occ_frames = nullptr;           // 3 per occurrence (cell-major, ascending side): the frame of that side
     sph::CellChunk* d_cell_chunks = nullptr;
-    sph::LoopChunk* d_loop_chunks = nullptr;  // n_chunks work items of the interaction loops, heaviest first
-    sph::LoopOcc* d_loop_occ = nullptr;       // per occurrence
-    sph::ChunkBox* d_boxes[3] = {};           // per loop kind (density, gradient, force): chunk boxes written by the loop's own
-                                              // first kernel from ITS input buffer (scratch: one call per kind at a time)
+    sph::LoopItem* d_items_density = nullptr; // one per 64-target chunk of a block (20-byte in, 16-byte out records)
+    sph::LoopItem* d_items_force = nullptr;   // (52-byte in, 20-byte out records)
+    uint32_t n_items = 0;                     // items are cell-major: the chunks of a cell's occurrences follow one another
     // block offsets by record bytes: the only part that grows after sph_batch_create (a table is built the first time a
     // record size is asked for, under the mutex; tables are never removed, so pointers to them stay valid)
     mutable std::mutex mu;
@@ -193,9 +169,8 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
                     uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
                       bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st);
-int32_t launch_density(const sph_batch* b, const OffsetTable& oin, const OffsetTable& oout, const char* d_in, char* d_out, cudaStream_t st);
-int32_t launch_force(const sph_batch* b, const OffsetTable& oin, const OffsetTable& oout, const char* d_in, char* d_out, const sph_params& prm,
-                     cudaStream_t st);
+int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
+int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);
 int32_t launch_ghost(const StoreView& view, uint64_t n, const sph_layout& layout, const sph_params& prm, cudaStream_t st);
 }  // namespace sph

@@ -26,12 +26,13 @@
 //       exactly as the definition does and the exact cut-off applied.
 // Sums are accumulated per target in tile order = source order, so results are bit-reproducible run to run.
 #include "internal.h"
+#include "ptx.cuh"
 
 namespace sph {
 
 namespace {
 
-typedef unsigned long long u64;            // a pair of f32 (lo = target A, hi = target B)
+using namespace ptx;           // u64 = a pair of f32 (lo = target A, hi = target B)
 
 #ifndef SPH_LOOP_WARPS
 #define SPH_LOOP_WARPS 4
@@ -59,71 +60,9 @@ constexpr float kFar = 1.0e15f;            // coordinates of the dummy source (r
 constexpr float kReachSlack = 1.0f + 1.0e-4f;   // the reach box is a superset test; keep it clear of f32 rounding
 constexpr float kFilterEps = 4.0e-6f;      // x (largest |coordinate|)^2 summed over the axes: bounds the rounding of the
                                            // expanded form (about 18 roundings of 2^-24 relative to that scale)
-constexpr uint32_t kFull = 0xFFFFFFFFu;
+constexpr uint32_t kFull = kFullMask;
 
-// order-preserving image of a float in the signed integers, so that REDUX.MIN / REDUX.MAX reduce floats
-__device__ __forceinline__ int ord(float f) { const int k = __float_as_int(f); return k ^ ((k >> 31) & 0x7FFFFFFF); }
-__device__ __forceinline__ float unord(int k) { return __int_as_float(k ^ ((k >> 31) & 0x7FFFFFFF)); }
-__device__ __forceinline__ float warp_min(float v, bool valid) { return unord(__reduce_min_sync(kFull, valid ? ord(v) : 0x7FFFFFFF)); }
-__device__ __forceinline__ float warp_max(float v, bool valid) { return unord(__reduce_max_sync(kFull, valid ? ord(v) : (int)0x80000000)); }
-__device__ __forceinline__ float warp_max_pos(float v) { return __uint_as_float(__reduce_max_sync(kFull, __float_as_uint(v))); }   // v >= 0
-
-__device__ __forceinline__ float sqrt_approx(float x) {
-    float r;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ float rcp_approx(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ float rcp_fast(float x) {    // rcp.approx + one Newton step: within 1 ulp for normal x
-    const float r = rcp_approx(x);
-    return fmaf(r, fmaf(-x, r, 1.0f), r);
-}
-__device__ __forceinline__ uint32_t lanemask_lt() {
-    uint32_t m;
-    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
-    return m;
-}
-__device__ __forceinline__ uint32_t shr_clamp(uint32_t v, uint32_t n) {   // PTX shr clamps the amount: n >= 32 gives 0
-    uint32_t r;
-    asm("shr.b32 %0, %1, %2;" : "=r"(r) : "r"(v), "r"(n));
-    return r;
-}
-// packed pairs of f32 (sm_100: FADD2 / FMUL2 / FFMA2, two values per instruction)
-__device__ __forceinline__ u64 pack2(float lo, float hi) {
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ u64 dup2(float v) { return pack2(v, v); }
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
-    u64 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ u64 add2(u64 a, u64 b) {
-    u64 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ u64 sub2(u64 a, u64 b) {
-    u64 d;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
-    u64 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) { cp_async<16>(smem, gmem); }
 
 // n (<= MAXREC) records of WORDS 4-byte words, contiguous and 16-byte aligned in global memory -> shared, coalesced and asynchronous.
 // A last partial vector reads into the block's pad bytes.
@@ -137,32 +76,6 @@ __device__ __forceinline__ void fetch_records(float* dst, const char* g, uint32_
         if (v < nvec) cp_async16(dst + 4 * v, g + 16 * (size_t)v);
     }
 }
-
-// ---- bulk copies (TMA without a tensor map) completing on the warp's mbarrier ----
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // bytes of n records of WORDS 4-byte words, rounded up to the 16 bytes a bulk copy moves (a last partial vector reads
 // into the block's pad bytes)
@@ -546,7 +459,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
 
     uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
     FetchGroup fg{&sm.bar[0], 0u};
-    if (lane == 0) mbar_init(fg.bar, 1);
+    if (lane == 0) { mbar_init(fg.bar, 1); fence_mbar_init(); }
     __syncwarp();
     fg.issue2(lane, sm.raw, in + (uint64_t)iw.x * 128, rec_bytes16<13>(iw.w & 127u), sm.src[0], in + (uint64_t)iw.y * 128, rec_bytes16<13>(min(32u, iw.w >> 7)));
     uint32_t buf = 0;
@@ -790,9 +703,8 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
 
 template <class K>
 int32_t loop_grid(K kernel, size_t smem, uint32_t* grid) {
-    int dev = 0, sms = 0, per_sm = 0;
-    SPH_CUDA_TRY(cudaGetDevice(&dev));
-    SPH_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int sms = 0, per_sm = 0;
+    if (int32_t rc = device_sms(&sms)) return rc;
     if (smem > 48 * 1024) SPH_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     SPH_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kLoopWarps * 32, smem));
     *grid = (uint32_t)(sms * max(per_sm, 1));
@@ -802,12 +714,11 @@ int32_t loop_grid(K kernel, size_t smem, uint32_t* grid) {
 }  // namespace
 
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st) {
-    if (b->n_chunks == 0) return SPH_OK;
-    static uint32_t full_grid = 0;
-    if (!full_grid)
-        if (int32_t rc = loop_grid(density_kernel, 0, &full_grid)) return rc;
-    const uint32_t grid = min((b->n_chunks + kLoopWarps - 1) / kLoopWarps, full_grid);
-    density_kernel<<<grid, kLoopWarps * 32, 0, st>>>(b->d_items_density, d_in, d_out, b->n_chunks);
+    if (b->n_items == 0) return SPH_OK;
+    uint32_t full_grid = 0;
+    if (int32_t rc = loop_grid(density_kernel, 0, &full_grid)) return rc;
+    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
+    density_kernel<<<grid, kLoopWarps * 32, 0, st>>>(b->d_items_density, d_in, d_out, b->n_items);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -817,17 +728,16 @@ int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaSt
 #endif
 
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
-    if (b->n_chunks == 0) return SPH_OK;
-    static uint32_t full_grid[2] = {0, 0};
+    if (b->n_items == 0) return SPH_OK;
+    uint32_t full_grid[2] = {0, 0};
     constexpr size_t smem = sizeof(ForceWarpSmem) * kLoopWarps;
     // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
     // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
     const bool units = b->n_sides && b->n_instances <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * b->n_sides;
-    if (!full_grid[units])
-        if (int32_t rc = units ? loop_grid(force_kernel<true>, smem, &full_grid[1]) : loop_grid(force_kernel<false>, smem, &full_grid[0])) return rc;
-    const uint32_t grid = min((b->n_chunks + kLoopWarps - 1) / kLoopWarps, full_grid[units]);
-    if (units) force_kernel<true><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_chunks, prm.alpha, prm.beta);
-    else force_kernel<false><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_chunks, prm.alpha, prm.beta);
+    if (int32_t rc = units ? loop_grid(force_kernel<true>, smem, &full_grid[1]) : loop_grid(force_kernel<false>, smem, &full_grid[0])) return rc;
+    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid[units]);
+    if (units) force_kernel<true><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_items, prm.alpha, prm.beta);
+    else force_kernel<false><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_items, prm.alpha, prm.beta);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

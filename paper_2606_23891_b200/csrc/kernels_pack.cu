@@ -1,25 +1,25 @@
-// PACK and UNPACK kernels: pure data movement, HBM-bound.
+// PACK and UNPACK kernels: pure data movement, HBM-bound.  Both are CELL-centric: a cell's particles
+// are read (written) once per launch and copied to (reduced from) every block the cell occurs in.
 //
-// pack: one warp per 32-particle chunk of a block (one side of one task).  The warp
-//   (1) stages the pieces of the substruct arrays that hold the requested fields into shared memory with
-//       coalesced cp.async (16 bytes when the stride allows, else 8 or 4; for power-of-two strides only the
-//       16-byte pieces that are needed: for the 128-byte AoS record that is the difference between touching 2
-//       and 4 sectors), particle 0 of the chunk always landing at the same staging offset;
-//   (2) pre-pass, one lane per particle: x -> f32(x - frame) in place (one f64 subtraction, one RN conversion);
-//   (3) re-slices the staging area into the compact record stream, 16 bytes per lane and store.  Which staging
-//       word feeds which output word is the same for every chunk, so each lane computes its map once per launch.
+// pack (pack_kernel): one warp per 32-particle chunk of a cell and a slice of the cell's occurrences.  The chunk's structs
+//   are staged once into shared memory with coalesced cp.async (only the 16-byte pieces that hold requested fields), re-sliced
+//   once into the compact record stream (a "template"), and per occurrence the three x words are patched with
+//   f32(x - frame) and ONE bulk copy (cp.async.bulk shared -> global) writes the block's slice.  See the kernel's comments.
 //
-// unpack: one warp per 32-particle chunk of a CELL.  The warp walks the cell's blocks in ascending (task, side)
-// order, reading each block's slice with coalesced 16-byte loads (a round of independent loads in flight before
-// the first add), and applies the per-field operator in f32 in that order (bit-reproducible, no atomics, no races:
-// a particle is owned by exactly one warp per launch); the store fields are read and written once per launch.
+// unpack (unpack_kernel): one warp per 32-particle chunk of a cell, a two-stage pipeline of rounds: the chunk's slice of
+//   every block of the round is fetched by one bulk copy per slice (global -> shared, mbarrier), then one lane per particle
+//   applies the per-field operator (+=, max, =) over the slices in ascending (task, side) order in f32: bit-reproducible, no
+//   atomics, no races (a particle is owned by exactly one warp per launch); the store's fields are read and written once.
 #include <algorithm>
 
 #include "internal.h"
+#include "ptx.cuh"
 
 namespace sph {
 
 namespace {
+
+using namespace ptx;
 
 #ifndef SPH_PACK_WARPS
 #define SPH_PACK_WARPS 4
@@ -32,49 +32,6 @@ namespace {
 #endif
 constexpr int kPackWarps = SPH_PACK_WARPS;
 constexpr int kUnpackWarps = SPH_UNPACK_WARPS;
-
-template <int BYTES>
-__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
-    if constexpr (BYTES == 16)
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem));
-    else
-        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem), "n"(BYTES));
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// ---- bulk copies (TMA without a tensor map: cp.async.bulk) and the mbarrier they complete on ----
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// global -> shared, size a multiple of 16 bytes, both addresses 16-byte aligned; completes (in bytes) on `bar`
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// shared -> global, member of the issuing thread's current bulk group
-__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 
 constexpr int kPackK = SPH_PACK_K;                      // record-stream templates per set; two sets alternate
 constexpr uint32_t kPackTableOcc = 32;         // occurrences whose block offsets and frames are staged at a time
@@ -477,25 +434,24 @@ __global__ void ghost_kernel(StoreView view, GhostLoc loc, uint64_t n, double ga
     }
 }
 
-int g_sms = 0;
-int32_t sm_count(int* out) {
-    if (!g_sms) {
-        int dev = 0;
-        SPH_CUDA_TRY(cudaGetDevice(&dev));
-        SPH_CUDA_TRY(cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev));
-    }
-    *out = g_sms;
+int32_t sm_count(int* out) { return device_sms(out); }
+
+}  // namespace
+
+// SM count of the current device, asked for on every launch (no process-wide cache: a process may use several devices)
+int32_t device_sms(int* sms_out) {
+    int dev = 0;
+    SPH_CUDA_TRY(cudaGetDevice(&dev));
+    SPH_CUDA_TRY(cudaDeviceGetAttribute(sms_out, cudaDevAttrMultiProcessorCount, dev));
     return SPH_OK;
 }
+
+namespace {
 
 template <int NIT>
 int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms,
                         uint32_t cc0, uint32_t ncc, cudaStream_t st) {
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    if (smem > 48 * 1024) SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // resident CTAs per SM (shared memory and 64 warps bound it); a cell's occurrences are split into `slices` items
     // when there are fewer cell chunks than about two rounds of resident warps
     const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(64 / kPackWarps, (220 * 1024) / (smem + 1024)));
@@ -513,9 +469,10 @@ int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t*
 #ifndef SPH_UNPACK_RING
 #define SPH_UNPACK_RING 5760
 #endif
-constexpr uint32_t kUnpackRingBytes = SPH_UNPACK_RING;   // per ring: 9 slices of 32 x 20-byte records -- a cell of a periodic grid (27 blocks) takes three
-                                                          // rounds; small rings let 9 CTAs (18 warps) share an SM, which is what overlaps one warp's reduction
-                                                          // with the others' fetches (measured: 27-slice rings 0.36 ms, 9-slice rings 0.23 ms on configs[2])   // per warp: 27 slices of 32 x 20-byte records fit (a cell of a periodic grid occurs 27 times)
+// per ring: 9 slices of 32 x 20-byte records -- a cell of a periodic grid (27 blocks) takes three rounds; small rings let
+// 9 CTAs (18 warps) share an SM, which is what overlaps one warp's reduction with the others' fetches (measured on
+// configs[2]: 27-slice rings 0.36 ms, 9-slice rings 0.23 ms)
+constexpr uint32_t kUnpackRingBytes = SPH_UNPACK_RING;
 
 template <int VEC, int GW>
 int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,
@@ -524,11 +481,7 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
     const uint32_t extra = prog.rec_words <= (uint32_t)GW ? 0 : 1;      // scratch slot of a long record
     const uint32_t slots = last_only ? 1u : std::max(1u, std::min(std::min(32u, b->max_nocc), kUnpackRingBytes / slot_bytes));
     const size_t smem = 128 + (size_t)kUnpackWarps * (2 * slots + extra) * slot_bytes;      // mbarriers, then two rings (+ scratch) per warp
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        SPH_CUDA_TRY(cudaFuncSetAttribute(unpack_kernel<VEC, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    if (smem > 48 * 1024) SPH_CUDA_TRY(cudaFuncSetAttribute(unpack_kernel<VEC, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const uint32_t per_sm = (uint32_t)std::max<size_t>(1, std::min<size_t>(SPH_UNPACK_MAXCTA, (227 * 1024) / (smem + 1024)));
     const uint32_t want = (ncc + kUnpackWarps - 1) / kUnpackWarps;
     const uint32_t grid = std::min(want, (uint32_t)sms * per_sm);

@@ -613,10 +613,36 @@ def test_argument_errors():
     with pytest.raises(sph.SphError) as e:
         sph.sph_pack(g.store, g.batch, aset, small)
     assert e.value.code == 3
-    odd = sph.make_attrset([("x", 0, 3), ("id", 0, 1)])                    # 32-byte records: table not prepared yet
-    with pytest.raises(sph.SphError) as e:
-        sph.sph_pack(g.store, g.batch, odd, torch.zeros(1 << 20, dtype=torch.uint8, device="cuda"))
+    # pack accepts any attribute set, whether or not sph_batch_buffer_bytes was ever asked about its record size
+    odd = sph.make_attrset([("x", 0, 3), ("id", 0, 1)])                    # 32-byte records, first use
+    big = torch.zeros(1 << 20, dtype=torch.uint8, device="cuda")
+    sph.sph_pack(g.store, g.batch, odd, big)
+    torch.cuda.synchronize()
+    oset = ([(orc.X, 0, 3), (orc.ID, 0, 1)], 0)
+    ref = orc.pack(ps, cells, tasks, oset)
+    off, total = orc.block_offsets(cells, tasks, 32)
+    assert sph.sph_batch_buffer_bytes(g.batch, odd) == total
+    m = valid_mask(off, cells, tasks, 32, total)
+    assert np.array_equal(big.cpu().numpy()[:total][m], ref[m])
+    with pytest.raises(sph.SphError) as e:                                # a NULL attribute set is an argument error, not a crash
+        sph.sph_pack(g.store, g.batch, None, big)
     assert e.value.code == 1
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_unpack(g.store, g.batch, None, big, sph.SPH_UNPACK_ASSIGN)
+    assert e.value.code == 1
+    # a batch is tied to the cell table it was built against, not just to the particle count
+    other = cells.copy()
+    k = int(np.argmax(other["count"] > 1))
+    other["count"][k] -= 1
+    store2 = sph.sph_store_create(g.layout, ps.shape[0])
+    sph.sph_store_set_cells(store2, np.ascontiguousarray(other).view(sph.CELL_DTYPE))
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack(store2, g.batch, aset, g.buffer(aset))
+    assert e.value.code == 1
+    sph.sph_store_set_cells(store2, np.ascontiguousarray(cells).view(sph.CELL_DTYPE))      # the same table: accepted
+    sph.sph_pack(store2, g.batch, aset, g.buffer(aset))
+    torch.cuda.synchronize()
+    sph.sph_store_destroy(store2)
     with pytest.raises(sph.SphError) as e:                                # relative coordinates cannot be unpacked
         sph.sph_unpack(g.store, g.batch, aset, g.buffer(aset), sph.SPH_UNPACK_ASSIGN)
     assert e.value.code == 6

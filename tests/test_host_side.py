@@ -183,3 +183,67 @@ def test_no_cpu_fallback_without_device():
     with pytest.raises(sph.SphError) as e:
         sph.sph_store_create(sph.sph_layout_aos(), 128)
     assert e.value.code == 5
+
+
+def _host_store(n, layout=None):
+    """a store over caller-owned (numpy) memory: no CUDA call is made, so the host-side checks run without a device"""
+    layout = layout or sph.sph_layout_aos()
+    bufs = []
+    for s in range(layout.n_sub):
+        raw = np.zeros(sph.sph_store_sub_bytes(layout, n, s) + 256, dtype=np.uint8)
+        off = (-raw.ctypes.data) % 256
+        bufs.append(raw[off:off + sph.sph_store_sub_bytes(layout, n, s)])
+    return sph.sph_store_create(layout, n, sph.SPH_MEM_HOST_PINNED, ext=bufs), bufs
+
+
+def test_cell_table_checks_do_not_wrap():
+    store, keep = _host_store(100)
+    cells = np.zeros(3, dtype=sph.CELL_DTYPE)
+    cells["first"], cells["count"], cells["width"] = [0, 40, 70], [40, 30, 30], 1.0
+    sph.sph_store_set_cells(store, cells)
+    for first, count in [(2 ** 64 - 10, 30), (90, 30), (101, 0)]:          # a huge `first` must not wrap around the range check
+        bad = cells.copy()
+        bad["first"][2], bad["count"][2] = first, count
+        with pytest.raises(sph.SphError) as e:
+            sph.sph_store_set_cells(store, bad)
+        assert e.value.code == 3
+    bad = cells.copy()
+    bad["first"][1] = 39                                                    # overlaps cell 0
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_store_set_cells(store, bad)
+    assert e.value.code == 3
+    sph.sph_store_destroy(store)
+
+
+def test_null_arguments_are_errors_not_crashes():
+    import ctypes as C
+    lib = C.CDLL(sph.lib_path())
+    store, keep = _host_store(64)
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN)
+    out = C.c_uint64(0)
+    fake = C.c_void_p(keep[0].ctypes.data)                                   # any non-NULL buffer pointer
+    assert lib.sph_batch_buffer_bytes(None, C.byref(aset), C.byref(out)) == 1
+    assert lib.sph_pack(store, None, C.byref(aset), fake, C.c_uint64(1024), None) == 1
+    assert lib.sph_pack(None, None, None, None, C.c_uint64(0), None) == 1
+    assert lib.sph_unpack(store, None, None, fake, C.c_uint64(1024), C.c_int32(0), None) == 1
+    assert lib.sph_density(None, fake, C.c_uint64(0), fake, C.c_uint64(0), None) == 1
+    assert lib.sph_force(None, fake, C.c_uint64(0), fake, C.c_uint64(0), None, None) == 1
+    assert lib.sph_store_zero(store, None, None) == 1
+    assert lib.sph_store_set_cells(store, None, C.c_uint32(3)) == 1
+    assert lib.sph_batch_create(store, None, C.c_uint64(1), C.c_uint32(0), C.byref(C.c_void_p())) == 1
+    assert "NULL" in sph.sph_last_error() or "no tasks" in sph.sph_last_error()
+    sph.sph_store_destroy(store)
+
+
+def test_tasks_reject_a_cell_that_sees_its_own_image():
+    # one cell per dimension: the self task is not periodic, so neighbours through the wrap would be lost silently
+    x = np.random.default_rng(1).random((50, 3))
+    perm, cells = sph.sph_cells_build_grid(x, 1)
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_tasks_build(cells, np.array([0.05], dtype=np.float32))
+    assert e.value.code == 3 and "own periodic image" in str(e.value)
+    # two cells per dimension, 2 hmax = 0.6 > box - width = 0.5: the same
+    perm, cells = sph.sph_cells_build_grid(x, 2)
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_tasks_build(cells, np.full(8, 0.3, dtype=np.float32))
+    assert e.value.code == 3
