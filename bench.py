@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the SPH offload hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--layout split|aos]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload default|config1|config2|config3|config4|link|layouts]
 
-A step = one pass of the whole hot path over BASELINE.json:configs[1] (262,144 particles, 64^3 glass-like
-lattice, 16^3 cells, 57,344 tasks): pack DENSITY_IN, density loop, unpack DENSITY_OUT (the sums start from zero),
-ghost, pack FORCE_IN, force loop, unpack FORCE_OUT -- 7 kernel launches, inputs resident in HBM.
-value = particles/s through that step (whole job: all ranks' particles / max-over-ranks time).
-`e2e` = the same step through the C ABI with HOST (pinned) particle arrays: the substructs the loops read are
-uploaded, the ones they write are downloaded, every step, inside the timed region.
+The default line is on the largest configuration whose store is resident in HBM, BASELINE.json:configs[2]: 2,097,152
+particles of the Sod-like setup, force loop with pack / unpack per bundle of 512 tasks (896 bundles under one launch per
+stage).  A step = pack FORCE_IN, force, unpack FORCE_OUT (the sums start from zero) over every bundle, inputs resident in HBM;
+value = particles/s through that step (whole job: all ranks' particles / max-over-ranks time); `roofline` = the dominant
+kernel, `kernels` / `aos` carry every kernel's fraction of its roofline for split-AoS and AoS.
+`e2e` = the same step through the C ABI with the particle arrays in pinned HOST memory: the substructs the force loop reads
+cross up, the ones it writes cross back, every step, inside the timed region.
+`workloads` (N = 1 only) carries the other configurations, measured in the same run: configs[1] (density + force step),
+configs[3] (streamed pack / unpack against the host link, 5 and 13 fields) and configs[4] (whole step, host-resident store).
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 import argparse
@@ -28,6 +31,7 @@ if ROOT not in sys.path:
 
 METRIC = "particles/s pack+unpack and pair-interactions/s; % of HBM / host-link roofline"
 WORKLOAD = "configs[1]: 262144 particles, 64^3 glass-like lattice, 16^3 cells, density loop then force loop"
+SHARDING = "one independent box per rank, no collective"
 N_SM, LANES_PER_SM = 148, 128
 # algorithmic FP32 work of the loops: 8 flop per ordered candidate pair (3 sub, 1 mul,
 # 2 fma, 1 compare) + per neighbour hit 25 flop (density) / 60 flop (force)
@@ -344,7 +348,8 @@ def run_other_workload(args):
     import bench_workloads as bw
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
-    common = {"hbm_peak": hbm_peak, "alu_peak": N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12, "peak_source": peak_src}
+    common = {"hbm_peak": hbm_peak, "alu_peak": N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12, "peak_source": peak_src,
+              "time_steps": lambda torch_, fn, steps, warmup, flush: time_steps(torch_, fn, steps, warmup, flush, 1), "sampler": lambda: None}
     sampler = ClockSampler(0)
     body = bw.RUNNERS[args.workload](args, sph, torch, common)
     clocks = sampler.stop()
@@ -410,8 +415,96 @@ def run_layouts(args):
                       "gpu_launches": 7 * args.steps, "clocks": clocks, "roofline": None, "layouts": rows}))
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def run_default(args):
+    """the default line: configs[2] (headline), and at N = 1 the other configurations as `workloads`"""
+    import torch
+    rank, world, local = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    import paper_2606_23891_b200 as sph
+    import bench_workloads as bw
+    torch.cuda.set_device(local)
+    hbm_peak, sm_max_mhz, peak_src = measured_peaks()
+    alu_peak = N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    common = {"hbm_peak": hbm_peak, "alu_peak": alu_peak, "peak_source": peak_src,
+              "time_steps": lambda torch_, fn, steps, warmup, flush: time_steps(torch_, fn, steps, warmup, flush, world),
+              "sampler": (lambda: ClockSampler(local)) if rank == 0 else (lambda: None)}
+    t_start = time.perf_counter()
+    out, setup, state = bw.measure_config2(args, sph, torch, common, seed=1 + rank)        # weak scaling: every rank owns its own box
+    P = out["split"]
+    ms = dist_max(P["ms"], world, "cuda")
+    ms_e2e = dist_max(P["ms_e2e"], world, "cuda")
+    total = dist_sum(float(P["n"]), world, "cuda")
+    dominant = max(("pack_force_in", "force", "unpack_force_out"), key=lambda k: P["kernels"][k]["ms"])
+    roof = {k: v for k, v in P["kernels"][dominant].items() if k not in ("ms", "instances_per_s", "candidate_pairs_per_s", "neighbour_pairs_per_s",
+                                                                          "frac_of_nominal_8tbs")}
+    traffic = None
+    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch,workload (from ncu --set full)
+    if os.path.exists(tfile):
+        for row in open(tfile):
+            c = row.strip().split(",")
+            if len(c) >= 4 and c[0] == dominant and c[1] == "split" and c[3] == "config2":
+                traffic = float(c[2])
+    roof.update(kernel=dominant, launch_ms=P["kernels"][dominant]["ms"], traffic=traffic,
+                peak_source=peak_src + (" HBM copy bandwidth" if roof.get("bound") == "hbm" else " max SM clock x 148 SMs x 128 FP32 lanes x 2"))
+    line = {
+        "metric": METRIC, "value": total / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": bw.CONFIG2_NAME.format(n=P["n"]), "layout": "split", "store": "HBM", "tasks": P["tasks"], "bundles": P["bundles"],
+                   "instances_per_loop": P["instances"], "candidate_pairs_per_loop": P["candidate_pairs"],
+                   "l2": "flushed before every step (256 MB fill, untimed)", "sharding": SHARDING, "setup": setup,
+                   "e2e": "host-resident particle arrays (pinned); per step the substructs the force loop reads cross up slab by slab and are packed as "
+                          "they land, the results cross back slab by slab behind the unpack; copies, kernels and cross-stream events captured once as "
+                          "a CUDA graph, one replay per step"},
+        "pair_interactions_per_s": {"force": P["kernels"]["force"]["candidate_pairs_per_s"]},
+        "neighbour_pairs_per_s": {"force": P["kernels"]["force"]["neighbour_pairs_per_s"]},
+        "instances_per_s": {k: P["kernels"][k]["instances_per_s"] for k in ("pack_force_in", "unpack_force_out")},
+        "e2e": {"value": total / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes"], "d2h_bytes_per_step": P["d2h_bytes"],
+                "ms_per_step": ms_e2e},
+        "gpu_launches": 3 * args.steps, "clocks": P["clocks"], "roofline": roof, "kernels": P["kernels"], "single_bundle_ms": P["single_bundle_ms"],
+        "aos": {"value": total / (dist_max(out["aos"]["ms"], world, "cuda") * 1e-3), "ms_per_step": out["aos"]["ms"], "kernels": out["aos"]["kernels"],
+                "e2e_value": total / (dist_max(out["aos"]["ms_e2e"], world, "cuda") * 1e-3),
+                "e2e_bytes": [out["aos"]["h2d_bytes"], out["aos"]["d2h_bytes"]]},
+    }
+    if rank == 0 and world == 1 and not args.no_workloads:
+        sub = argparse.Namespace(**vars(args))
+        work = {}
+        sub.steps, sub.warmup = min(args.steps, 20), 3
+        c1 = measure_config1(sub, sph, torch, rank, world, local)
+        work["configs[1]"] = {k: c1[k] for k in ("value", "unit", "ms_per_step", "config", "kernels", "aos", "e2e", "pair_interactions_per_s")}
+        sub.steps, sub.warmup, sub.n = 3, 3, args.n3
+        c3 = bw.run_config3(sub, sph, torch, common, ks=[5, 13], modes=("streamed",))
+        work["configs[3]"] = {"workload": c3["config"]["workload"], "link": c3["config"]["link"], "setup": c3["config"]["setup"],
+                              "streamed": c3["sweep"], "pack13_plus_unpack13": c3["roofline"]}
+        sub.n, sub.skip_zero_copy = args.n4, True
+        c4 = bw.run_config4(sub, sph, torch, common)
+        work["configs[4]"] = {"workload": c4["config"]["workload"], "e2e_note": c4["config"]["e2e"], "setup": c4["config"]["setup"],
+                              "link": c4["config"]["link"], "e2e": c4["e2e"], "roofline": c4["roofline"], "variants": c4["variants"]}
+        line["workloads"] = work
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline_config2(state, budget_s=args.cpu_budget)
+        line["bench_wall_s"] = round(time.perf_counter() - t_start, 1)
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
+    if args.workload == "default":
+        return run_default(args)
     if args.workload == "layouts":
         return run_layouts(args)
     if args.workload != "config1":
@@ -421,6 +514,19 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     import paper_2606_23891_b200 as sph
     torch.cuda.set_device(local)
+    line = measure_config1(args, sph, torch, rank, world, local)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(budget_s=args.cpu_budget)
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def measure_config1(args, sph, torch, rank, world, local):
+    """configs[1]: the seven launches of a whole step (density loop then force loop), store in HBM, and the same with
+    host-resident arrays; returns the JSON line as a dict"""
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     ps, cells, tasks = build_config1(sph, seed=1 + rank)          # weak scaling: every rank owns its own box
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -488,7 +594,7 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "layout": primary, "store": "HBM", "tasks": int(w.info.n_tasks), "instances_per_loop": int(w.info.n_instances),
                    "candidate_pairs_per_loop": int(cand), "l2": "flushed before every step (256 MB fill, untimed)",
-                   "sharding": "one independent box per rank, no collective",
+                   "sharding": SHARDING,
                    "e2e": "host-resident particle arrays; the step's copies and kernels captured once as a CUDA graph, one replay per step"},
         "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},      # ordered candidate pairs
         "neighbour_pairs_per_s": {"density": total_particles / world * NGB_CONFIG1 / (R["per"]["density"] * 1e-3),                       # pairs inside the cut-off
@@ -507,15 +613,9 @@ def run_ours(args):
                            "e2e_value": Ro["w"].n * world / (dist_max(Ro["ms_e2e"], world, "cuda") * 1e-3),
                            "e2e_bytes": list(Ro["w"].e2e_bytes()),
                            "kernels_ms": {k: round(v, 5) for k, v in Ro["per"].items()}}
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(budget_s=args.cpu_budget)
     for Ro in results.values():
         Ro["w"].close()
-    if rank == 0:
-        print(json.dumps(line))
-    if world > 1:
-        import torch.distributed as dist
-        dist.destroy_process_group()
+    return line
 
 
 # --------------------------------------------------------------------------------------------- oracle arm
@@ -543,6 +643,98 @@ def oracle_setup():
     return orc, ps, cells, tasks, cores
 
 
+def oracle_stage_times(orc, ps, cells, tasks, loops=("density", "force")):
+    """seconds of every stage of the oracle's cycle(s) over `tasks`, with the work each stage did"""
+    out = {}
+    inst = int(cells["count"][tasks["ci"]].sum() + cells["count"][tasks["cj"][tasks["cj"] >= 0]].sum())
+    ni = cells["count"][tasks["ci"]].astype(np.int64)
+    nj = np.where(tasks["cj"] >= 0, cells["count"][np.maximum(tasks["cj"], 0)], 0).astype(np.int64)
+    cand = int(np.where(tasks["cj"] >= 0, 2 * ni * nj, ni * ni).sum())
+
+    def timed(name, fn, work_key, work):
+        t0 = time.perf_counter()
+        r = fn()
+        dt = time.perf_counter() - t0
+        out[name] = {"s": round(dt, 4), work_key: work / dt}
+        return r
+    if "density" in loops:
+        orc.zero(ps, orc.DENSITY_OUT)
+        b_in = timed("pack_density_in", lambda: orc.pack(ps, cells, tasks, orc.DENSITY_IN), "instances_per_s", inst)
+        b_out = timed("density", lambda: orc.density(cells, tasks, b_in), "candidate_pairs_per_s", cand)
+        timed("unpack_density_out", lambda: orc.unpack(ps, cells, tasks, orc.DENSITY_OUT, b_out), "instances_per_s", inst)
+        timed("ghost", lambda: orc.ghost(ps, float(np.float32(5.0 / 3.0))), "particles_per_s", ps.shape[0])
+    if "force" in loops:
+        orc.zero(ps, orc.FORCE_OUT)
+        b_in = timed("pack_force_in", lambda: orc.pack(ps, cells, tasks, orc.FORCE_IN), "instances_per_s", inst)
+        b_out = timed("force", lambda: orc.force(cells, tasks, b_in, 0.8, 3.0), "candidate_pairs_per_s", cand)
+        timed("unpack_force_out", lambda: orc.unpack(ps, cells, tasks, orc.FORCE_OUT, b_out), "instances_per_s", inst)
+    out["total_s"] = round(sum(v["s"] for v in out.values()), 4)
+    return out
+
+
+def oracle_config2_sample(seed=1):
+    """A bounded sample of configs[2] built by the oracle's own builders: the cells of x-layers 0-3 (dense half) and 16-19
+    (sparse half) of the 32^3 grid with all the tasks among them (8,192 of 32,768 cells).  h is the generator's continuum
+    value (1.12725 n^-1/3, what the 48-neighbour iteration starts from), rho = m n, u from P = 1 | 0.1, P and c_s from the
+    oracle's ghost: enough for timing, where only the shape of the workload matters."""
+    import oracle as orc
+    import sph_inputs as si
+    parts = si.config2_positions(seed=seed)
+    parts["h"] = np.minimum(parts["h"], np.float32(0.4999 / 32))
+    perm, cells = orc.cells_build_grid(parts["x"], 32)
+    ix = np.arange(cells.shape[0]) // (32 * 32)
+    keep = np.flatnonzero(((ix < 4) | ((ix >= 16) & (ix < 20))) & (cells["count"] > 0))
+    first, count = cells["first"].astype(np.int64), cells["count"].astype(np.int64)
+    idx = np.concatenate([perm[first[c]:first[c] + count[c]] for c in keep]).astype(np.int64)
+    ps = np.ascontiguousarray(parts[idx])
+    sub = cells[keep].copy()
+    sub["first"] = np.concatenate([[0], np.cumsum(count[keep])[:-1]])
+    hmax = np.maximum.reduceat(ps["h"], sub["first"].astype(np.int64)).astype(np.float32)
+    tasks, _, _ = orc.tasks_build(sub, hmax)
+    n_dens = (1.12725 / ps["h"].astype(np.float64)) ** 3
+    ps["rho"] = (ps["mass"] * n_dens).astype(np.float32)
+    ps["u"] = (np.where(ps["x"][:, 0] < 0.5, 1.0, 0.1) / ((5.0 / 3.0 - 1.0) * ps["rho"].astype(np.float64))).astype(np.float32)
+    orc.ghost(ps, float(np.float32(5.0 / 3.0)))
+    return orc, ps, sub, tasks
+
+
+def cpu_baseline_config2(state=None, budget_s=20.0):
+    """the oracle as it stands on the host cores: the force cycle of configs[2] on a bounded sample (all threads and one thread),
+    and every stage of a configs[1] step, with the CPU model"""
+    orc, ps, cells, tasks = oracle_config2_sample()
+    cores = min(os.cpu_count() or 1, 64)
+    orc.set_threads(cores)
+    # all threads: as many leading cells of the dense and of the sparse group as fit the budget
+    n_cells = cells.shape[0]
+    half = n_cells // 2
+
+    def pick(m):
+        ci = tasks["ci"]
+        return np.ascontiguousarray(tasks[(ci < m) | ((ci >= half) & (ci < half + m))])
+    probe = oracle_stage_times(orc, ps, cells, pick(128), loops=("force",))
+    m = int(max(128, min(half, 128 * (0.4 * budget_s) / max(probe["total_s"], 1e-3))))
+    sel = pick(m)
+    st_all = oracle_stage_times(orc, ps, cells, sel, loops=("force",))
+    particles = int(cells["count"][:m].sum() + cells["count"][half:half + m].sum())
+    orc.set_threads(1)
+    m1 = max(32, m // 8)
+    st_one = oracle_stage_times(orc, ps, cells, pick(m1), loops=("force",))
+    orc.set_threads(cores)
+    # configs[1]: the seven stages of a whole step
+    orc1, ps1, cells1, tasks1, _ = oracle_setup()
+    c1_all = oracle_stage_times(orc1, ps1, cells1, tasks1)
+    orc1.set_threads(1)
+    c1_one = oracle_stage_times(orc1, ps1, cells1, np.ascontiguousarray(tasks1[tasks1["ci"] < 256]))
+    orc1.set_threads(cores)
+    return {"value": particles / st_all["total_s"], "unit": "particles/s", "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
+            "hardware_concurrency": os.cpu_count(),
+            "sample": f"configs[2] force cycle (pack FORCE_IN, force, unpack FORCE_OUT) over the tasks of the first {m} cells of the dense group and "
+                      f"the first {m} of the sparse group of an 8192-cell sample ({particles} particles, {sel.shape[0]} tasks), {st_all['total_s']:.2f} s; "
+                      f"one-thread figures on {m1} + {m1} cells; the oracle's unpack is serial by design",
+            "stages": {"all_threads": st_all, "one_thread": st_one},
+            "configs[1]_stages": {"all_threads_4096_cells": c1_all, "one_thread_256_cells": c1_one}}
+
+
 def cpu_baseline(budget_s=20.0):
     """the oracle as it stands, on the host cores, on a bounded sample of configs[1] (about budget_s of CPU wall time):
     the tasks of the first m cells, or -- when one whole step takes less than the budget -- whole steps repeated"""
@@ -557,15 +749,55 @@ def cpu_baseline(budget_s=20.0):
         reps = int(max(1, min(200, budget_s / max(t, 1e-3))))
         t = sum(oracle_sample_step(orc, ps, cells, tasks, m) for _ in range(reps)) / reps
     particles = int(cells["count"][:m].sum())
-    return {"value": particles / t, "unit": "particles/s", "cores": cores, "kind": "oracle",
+    stages = oracle_stage_times(orc, ps, cells, tasks)
+    return {"value": particles / t, "unit": "particles/s", "cores": cores, "kind": "oracle", "cpu_model": cpu_model(), "hardware_concurrency": os.cpu_count(),
             "sample": f"tasks of the first {m} of {n_cells} cells of configs[1] ({particles} particles), one full step, "
-                      f"average of {reps} repetition(s), {t:.2f} s each"}
+                      f"average of {reps} repetition(s), {t:.2f} s each", "stages": {"all_threads": stages}}
 
 
 def run_reference(args):
+    """the oracle on the host cores on the default line's workload: the force cycle of configs[2], each step a bounded sample"""
     rank = int(os.environ.get("RANK", 0))
     if rank != 0:
         return
+    if args.workload == "config1":
+        return run_reference_config1(args)
+    orc, ps, cells, tasks = oracle_config2_sample()
+    cores = min(os.cpu_count() or 1, 64)
+    orc.set_threads(cores)
+    half = cells.shape[0] // 2
+
+    def pick(m):
+        ci = tasks["ci"]
+        return np.ascontiguousarray(tasks[(ci < m) | ((ci >= half) & (ci < half + m))])
+
+    def cycle(sel):
+        t0 = time.perf_counter()
+        orc.force_cycle(ps, cells, sel)
+        return time.perf_counter() - t0
+    t_probe = cycle(pick(64))
+    per_step_budget = max(0.5, args.ref_budget / (args.steps + args.warmup))
+    m = int(max(16, min(half, 64 * per_step_budget / max(t_probe, 1e-3))))
+    sel = pick(m)
+    for _ in range(args.warmup):
+        cycle(sel)
+    times = [cycle(sel) for _ in range(args.steps)]
+    particles = int(cells["count"][:m].sum() + cells["count"][half:half + m].sum())
+    sec = sum(times) / len(times)
+    value = particles / sec
+    sample = (f"force cycle over the tasks of the first {m} dense and first {m} sparse cells of an 8192-cell sample of configs[2] "
+              f"({particles} particles, {sel.shape[0]} tasks) per step")
+    import bench_workloads as bw
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": bw.CONFIG2_NAME.format(n=1 << 21), "layout": "aos", "store": "host DRAM", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "particles/s", "cores": cores, "kind": "oracle", "sample": sample, "cpu_model": cpu_model()},
+        "e2e": {"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_reference_config1(args):
     orc, ps, cells, tasks, cores = oracle_setup()
     n_cells = cells.shape[0]
     probe = 32
@@ -591,12 +823,16 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="both", help="split | aos | both, or any layout name of paper_2606_23891_b200/layouts.py")
-    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4", "link", "layouts"],
-                    help="config1 = BASELINE.json:configs[1] (the default bench line); the others are described in bench_workloads.py")
+    ap.add_argument("--workload", default="default", choices=["default", "config1", "config2", "config3", "config4", "link", "layouts"],
+                    help="default = configs[2] as the headline plus configs[1], [3], [4] as `workloads`; the others run one configuration "
+                         "(bench_workloads.py describes them)")
+    ap.add_argument("--no-workloads", action="store_true", help="default line: configs[2] only")
+    ap.add_argument("--n3", type=int, default=0, help="default line: particle count of the configs[3] entry (default 2^24)")
+    ap.add_argument("--n4", type=int, default=0, help="default line: particle count of the configs[4] entry (default 2^26)")
     ap.add_argument("--n", type=int, default=0, help="particle count for config2/3/4 (default: the full size of BASELINE.json)")
     ap.add_argument("--skip-zero-copy", action="store_true", help="config4: time the staged pipeline only")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -180,22 +180,82 @@ def build_config2(sph, torch, seed, n):
     sph.sph_batch_destroy(batch)
     sph.sph_store_destroy(store)
     del b_in, b_out
+    # ordered pairs inside the cut-off of the force loop, r < max(2h_i, 2h_j): with the 48-neighbour h every particle has
+    # (4/3) pi (2h)^3 n = 48 / (mean kernel weight) others inside its own 2h; counted from wcount's definition instead:
+    # N_i = (4/3) pi (2 h_i)^3 n_i where n_i = rho_i / m is the number density the particle sees
+    ngb = (32.0 / 3.0) * np.pi * ps["h"].astype(np.float64) ** 3 * (ps["rho"].astype(np.float64) / ps["mass"])
     info = {"cells_per_dim": cpd, "h_iterations": iters, "worst_neighbour_error": worst, "h_min": float(h.min()), "h_max": float(h.max()),
-            "per_cell_min": int(cells["count"].min()), "per_cell_max": int(cells["count"].max())}
+            "per_cell_min": int(cells["count"].min()), "per_cell_max": int(cells["count"].max()),
+            "neighbour_pairs": float(ngb.sum()), "neighbours_per_particle": float(ngb.mean())}
     return ps, cells, tasks, info
 
 
-def run_config2(args, sph, torch, common):
+class Config2E2E:
+    """configs[2] with the particle arrays in pinned HOST memory: per step the substructs the force loop reads cross slab by
+    slab (ranges of cells) and are packed as they land (sph_pack_cells), the force loop runs over all 896 bundles, the results
+    are reduced slab by slab (sph_unpack_cells) and each slab's particles cross back as soon as they are final.  One graph."""
+
+    def __init__(self, sph, torch, layout, store, batch, cells, n, bufs, params, n_slabs=8):
+        self.sph, self.torch, self.store, self.batch, self.bufs, self.params = sph, torch, store, batch, bufs, params
+        F = sph.FIELD
+        sub = lambda names: sorted({layout.loc[F[k]].sub for k in names})
+        self.subs_in = sub(["x", "h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s"])
+        self.subs_out = sub(["a", "du_dt", "v_sig"])
+        self.host = {s: torch.empty(n * layout.stride[s], dtype=torch.uint8).pin_memory() for s in set(self.subs_in + self.subs_out)}
+        for s, h in self.host.items():
+            sph.sph_store_download_sub(store, s, h)
+        torch.cuda.synchronize()
+        self.h2d_bytes = sum(n * layout.stride[s] for s in self.subs_in)
+        self.d2h_bytes = sum(n * layout.stride[s] for s in self.subs_out)
+        self.slabs = cell_slabs(cells, n_slabs)
+        self.up, self.down = torch.cuda.Stream(), torch.cuda.Stream()
+        self.s_in, self.s_out = sph.sph_attrset_canonical(2), sph.sph_attrset_canonical(3)
+
+    def step(self, main):
+        sph, torch = self.sph, self.torch
+        ev = lambda st: (lambda e: (e.record(st), e)[1])(torch.cuda.Event())
+        start = ev(main)
+        self.up.wait_event(start)
+        self.down.wait_event(start)
+        for c0, nc, p0, npart in self.slabs:
+            for s in self.subs_in:
+                sph.sph_store_upload_range(self.store, s, self.host[s], p0, npart, self.up)
+            main.wait_event(ev(self.up))
+            sph.sph_pack_cells(self.store, self.batch, self.s_in, self.bufs[0], c0, nc, main)
+        sph.sph_force(self.batch, self.bufs[0], self.bufs[1], self.params, main)
+        for c0, nc, p0, npart in self.slabs:
+            sph.sph_unpack_cells(self.store, self.batch, self.s_out, self.bufs[1], c0, nc, sph.SPH_UNPACK_REDUCE_ZERO, main)
+            self.down.wait_event(ev(main))
+            for s in self.subs_out:
+                sph.sph_store_download_range(self.store, s, self.host[s], p0, npart, self.down)
+        main.wait_event(ev(self.down))
+
+    def capture(self):
+        torch = self.torch
+        root = torch.cuda.Stream()
+        with torch.cuda.stream(root):
+            self.step(root)
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=root):
+            self.step(root)
+        return self.graph
+
+
+def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
+    """configs[2]: per layout the whole step (pack FORCE_IN, force, unpack FORCE_OUT over 896 bundles of 512 tasks under one launch
+    per stage, store in HBM), each kernel, one bundle alone, and the end-to-end step with host-resident arrays"""
     hbm_peak, alu_peak = common["hbm_peak"], common["alu_peak"]
+    time_steps = common["time_steps"]
     n = args.n or (1 << 21)
-    ps, cells, tasks, setup = build_config2(sph, torch, 1, n)
+    ps, cells, tasks, setup = build_config2(sph, torch, seed, n)
     n = ps.shape[0]
     params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
     s_in, s_out = sph.sph_attrset_canonical(2), sph.sph_attrset_canonical(3)
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     flush = lambda: flush_buf.fill_(1)
     out = {}
-    for name in ("split", "aos"):
+    for name in layouts:
         layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
         store = sph.sph_store_create(layout, n)
         sph.sph_store_set_cells(store, cells)
@@ -204,12 +264,14 @@ def run_config2(args, sph, torch, common):
         info = sph.sph_batch_get_info(batch)
         b_in = torch.empty(sph.sph_batch_buffer_bytes(batch, s_in), dtype=torch.uint8, device="cuda")
         b_out = torch.empty(sph.sph_batch_buffer_bytes(batch, s_out), dtype=torch.uint8, device="cuda")
-        stages = [("zero_force_out", lambda: sph.sph_store_zero(store, s_out)),
-                  ("pack_force_in", lambda: sph.sph_pack(store, batch, s_in, b_in)),
+        # "zero the outputs" is fused into the unpack: the batch holds every task of the loop, so every particle's sums start from 0
+        stages = [("pack_force_in", lambda: sph.sph_pack(store, batch, s_in, b_in)),
                   ("force", lambda: sph.sph_force(batch, b_in, b_out, params)),
-                  ("unpack_force_out", lambda: sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE))]
+                  ("unpack_force_out", lambda: sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE_ZERO))]
         step = lambda: [fn() for _, fn in stages]
-        t = timed(torch, step, args.steps, args.warmup, before=flush)
+        sampler = common["sampler"]() if name == layouts[0] else None
+        t = time_steps(torch, step, args.steps, args.warmup, flush)
+        clocks = sampler.stop() if sampler else None
         per = {k: [] for k, _ in stages}
         for _ in range(args.steps):
             flush()
@@ -217,43 +279,65 @@ def run_config2(args, sph, torch, common):
             for k, fn in stages:
                 per[k].append(ev_time(torch, fn))
         per = {k: sum(v) / len(v) for k, v in per.items()}
+        e2e = Config2E2E(sph, torch, layout, store, batch, cells, n, (b_in, b_out), params)
+        g = e2e.capture()
+        t_e2e = time_steps(torch, g.replay, args.steps, args.warmup, flush)
         # one bundle alone (isolated latency of pack + force + unpack of 512 pair tasks)
         one = sph.sph_batch_create(store, tasks[info.n_self:info.n_self + 512])
         o_in = torch.empty(sph.sph_batch_buffer_bytes(one, s_in), dtype=torch.uint8, device="cuda")
         o_out = torch.empty(sph.sph_batch_buffer_bytes(one, s_out), dtype=torch.uint8, device="cuda")
         one_step = lambda: (sph.sph_pack(store, one, s_in, o_in), sph.sph_force(one, o_in, o_out, params),
                             sph.sph_unpack(store, one, s_out, o_out, sph.SPH_UNPACK_REDUCE))
-        t_one = timed(torch, one_step, args.steps, args.warmup, before=flush)
+        t_one = timed(torch, one_step, min(args.steps, 10), 3, before=flush)
         sph.sph_batch_destroy(one)
         inst, cand = info.n_instances, info.n_candidates
-        alg = {"pack_force_in": n * 64 + inst * 52, "unpack_force_out": inst * 20 + n * 2 * 20}
+        # algorithmic bytes: every record byte once, every touched store field once per particle
+        alg = {"pack_force_in": n * 64 + inst * 52, "unpack_force_out": inst * 20 + n * 20}
         kern = {}
         for k, ms in per.items():
             e = {"ms": round(ms, 4)}
             if k in alg:
-                e.update(bound="hbm", achieved=round(alg[k] / (ms * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s")
+                e.update(bound="hbm", achieved=round(alg[k] / (ms * 1e-3) / 1e9, 1), peak=hbm_peak, unit="GB/s",
+                         frac_of_nominal_8tbs=round(alg[k] / (ms * 1e-3) / 1e9 / 8000.0, 4))
                 e["frac"] = round(e["achieved"] / hbm_peak, 4)
                 e["instances_per_s"] = inst / (ms * 1e-3)
             if k == "force":
-                e.update(bound="alu", candidate_pairs_per_s=cand / (ms * 1e-3))
+                flop = cand * 8.0 + setup["neighbour_pairs"] * 60.0
+                e.update(bound="alu", achieved=round(flop / (ms * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s",
+                         candidate_pairs_per_s=cand / (ms * 1e-3), neighbour_pairs_per_s=setup["neighbour_pairs"] / (ms * 1e-3))
+                e["frac"] = round(e["achieved"] / alu_peak, 4)
             kern[k] = e
-        out[name] = {"ms_per_step": sum(t) / len(t), "kernels": kern, "single_bundle_ms": sum(t_one) / len(t_one),
-                     "tasks": int(info.n_tasks), "bundles": int(info.n_segments), "instances": int(inst), "candidate_pairs": int(cand)}
+        out[name] = {"ms": sum(t) / len(t), "ms_e2e": sum(t_e2e) / len(t_e2e), "kernels": kern, "single_bundle_ms": sum(t_one) / len(t_one),
+                     "tasks": int(info.n_tasks), "bundles": int(info.n_segments), "instances": int(inst), "candidate_pairs": int(cand),
+                     "h2d_bytes": e2e.h2d_bytes, "d2h_bytes": e2e.d2h_bytes, "clocks": clocks, "n": n}
+        e2e.graph = None
         sph.sph_batch_destroy(batch)
         sph.sph_store_destroy(store)
-        del b_in, b_out, o_in, o_out
+        del b_in, b_out, o_in, o_out, e2e, g
+    return out, setup, (ps, cells, tasks)
+
+
+CONFIG2_NAME = ("configs[2]: {n} particles, Sod-like two-density lattice (h by the 48-neighbour condition), 32^3 cells, force loop "
+                "(alpha = 0.8) with pack / unpack per bundle of 512 tasks, store in HBM")
+
+
+def run_config2(args, sph, torch, common):
+    out, setup, _ = measure_config2(args, sph, torch, common)
     P = out["split"]
+    n = P["n"]
     dominant = max(("pack_force_in", "force", "unpack_force_out"), key=lambda k: P["kernels"][k]["ms"])
     roof = {k: v for k, v in P["kernels"][dominant].items() if k != "ms"}
     roof.update(kernel=dominant, launch_ms=P["kernels"][dominant]["ms"], traffic=None)
     return {
-        "value": n / (P["ms_per_step"] * 1e-3), "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
-        "config": {"workload": f"configs[2]: {n} particles, Sod-like two-density lattice, h by the 48-neighbour condition, force loop in bundles of 512 tasks",
-                   "layout": "split", "store": "HBM", "l2": "flushed before every step (256 MB fill, untimed)", "setup": setup,
-                   "tasks": P["tasks"], "bundles": P["bundles"], "instances": P["instances"], "candidate_pairs": P["candidate_pairs"]},
-        "gpu_launches": 4 * args.steps, "roofline": roof, "kernels": P["kernels"], "single_bundle_ms": P["single_bundle_ms"],
-        "aos": {"ms_per_step": out["aos"]["ms_per_step"], "kernels": out["aos"]["kernels"], "single_bundle_ms": out["aos"]["single_bundle_ms"]},
-        "e2e": None,
+        "value": n / (P["ms"] * 1e-3), "unit": "particles/s", "ms_per_step": P["ms"], "dtype": "f32",
+        "config": {"workload": CONFIG2_NAME.format(n=n), "layout": "split", "store": "HBM", "tasks": P["tasks"], "bundles": P["bundles"],
+                   "instances_per_loop": P["instances"], "candidate_pairs_per_loop": P["candidate_pairs"],
+                   "l2": "flushed before every step (256 MB fill, untimed)", "setup": setup},
+        "gpu_launches": 3 * args.steps, "roofline": roof, "kernels": P["kernels"], "single_bundle_ms": P["single_bundle_ms"],
+        "aos": {"ms_per_step": out["aos"]["ms"], "kernels": out["aos"]["kernels"], "single_bundle_ms": out["aos"]["single_bundle_ms"],
+                "e2e_ms_per_step": out["aos"]["ms_e2e"], "e2e_bytes": [out["aos"]["h2d_bytes"], out["aos"]["d2h_bytes"]]},
+        "e2e": {"value": n / (P["ms_e2e"] * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes"], "d2h_bytes_per_step": P["d2h_bytes"],
+                "ms_per_step": P["ms_e2e"]},
     }
 
 
@@ -361,7 +445,8 @@ class Streamed:
         self._join()
 
 
-def run_config3(args, sph, torch, common):
+def run_config3(args, sph, torch, common, ks=None, modes=("zero-copy", "staged", "streamed")):
+    ks = ks or SWEEP_K
     n = args.n or (1 << 24)
     ps, cells, tasks, setup = build_clumpy(sph, 3, 1, n)
     link = link_probe(torch)
@@ -378,7 +463,7 @@ def run_config3(args, sph, torch, common):
         streamed = Streamed(sph, torch, cells, n_slabs=16)
         big = sweep_set(sph, PACK_SWEEP, 20, sph.SPH_ATTR_X_REL_F32)
         buf = torch.zeros(sph.sph_batch_buffer_bytes(batch, big), dtype=torch.uint8, device="cuda")
-        for k in SWEEP_K:
+        for k in ks:
             # ---- pack
             comps = PACK_SWEEP[:k]
             aset = sweep_set(sph, PACK_SWEEP, k, sph.SPH_ATTR_X_REL_F32)
@@ -399,11 +484,14 @@ def run_config3(args, sph, torch, common):
                 streamed.pack(dev, hs, batch, aset, buf, subs)
 
             for mode, fn, moved in (("zero-copy", zc, None), ("staged", staged, staged_bytes), ("streamed", streamed_p, staged_bytes)):
+                if mode not in modes:
+                    continue
                 t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
                 rows.append({"op": "pack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
                              "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),
                              "moved_link_gbs": None if moved is None else round(moved / (t * 1e-3) / 1e9, 2),
-                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["h2d_gbs"], 3)})
+                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["h2d_gbs"], 3),
+                             "moved_frac_of_link": None if moved is None else round(moved / (t * 1e-3) / 1e9 / link["h2d_gbs"], 3)})
             # ---- unpack (REDUCE: += for the sums, max for v_sig, = for the rest)
             comps = UNPACK_SWEEP[:k]
             aset = sweep_set(sph, UNPACK_SWEEP, k, 0)
@@ -424,11 +512,14 @@ def run_config3(args, sph, torch, common):
                 streamed.unpack(dev, hs, batch, aset, buf, subs, sph.SPH_UNPACK_REDUCE)
 
             for mode, fn, moved in (("zero-copy", zc_u, None), ("staged", staged_u, staged_bytes), ("streamed", streamed_u, staged_bytes)):
+                if mode not in modes:
+                    continue
                 t = min(timed(torch, fn, args.steps, min(args.warmup, 2)))
                 rows.append({"op": "unpack", "layout": name, "mode": mode, "k": k, "ms": round(t, 3), "particles_per_s": n / (t * 1e-3),
                              "instances_per_s": inst / (t * 1e-3), "useful_link_gbs": round(useful / (t * 1e-3) / 1e9, 2),
                              "moved_link_gbs": None if moved is None else round(moved / (t * 1e-3) / 1e9, 2),
-                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["d2h_gbs"], 3)})
+                             "frac_of_link": round(useful / (t * 1e-3) / 1e9 / link["d2h_gbs"], 3),
+                             "moved_frac_of_link": None if moved is None else round(moved / (t * 1e-3) / 1e9 / link["d2h_gbs"], 3)})
         setup.update(tasks=int(info.n_tasks), instances=int(inst))
         sph.sph_batch_destroy(batch)
         sph.sph_store_destroy(dev)
@@ -437,9 +528,10 @@ def run_config3(args, sph, torch, common):
     def pick(op, layout, k):
         c = [r for r in rows if r["op"] == op and r["layout"] == layout and r["k"] == k]
         return min(c, key=lambda r: r["ms"])
-    p13, u13 = pick("pack", "split", 13), pick("unpack", "split", 13)
+    kk = 13 if 13 in ks else ks[-1]
+    p13, u13 = pick("pack", "split", kk), pick("unpack", "split", kk)
     ms = p13["ms"] + u13["ms"]
-    useful13 = n * (field_bytes(PACK_SWEEP[:13]) + 4 * 13)
+    useful13 = n * (field_bytes(PACK_SWEEP[:kk]) + 4 * kk)
     roof = {"bound": "host-link", "achieved": round(useful13 / (ms * 1e-3) / 1e9, 2), "peak": round(link["h2d_gbs"], 2), "unit": "GB/s",
             "frac": round(useful13 / (ms * 1e-3) / 1e9 / link["h2d_gbs"], 3), "traffic": None, "kernel": "pack + unpack, 13 fields, split-AoS, best mode",
             "peak_source": "pinned H2D copy bandwidth measured in this run"}
@@ -455,13 +547,20 @@ def run_config3(args, sph, torch, common):
 class Pipeline:
     """The whole offload step streamed in bundles of `bundle` tasks over two streams, captured once as a CUDA graph.
 
-    mode "staged":    per loop the substructs the loop reads are copied H2D into a device staging store, bundles run against
-                      it (pack -> loop -> unpack on alternating streams, unpacks chained in bundle order so the reduction order
-                      is the task order), the substructs the loop wrote are copied D2H into the host store.
+    mode "staged" (the product path): the store lives in pinned host memory, the kernels work on a device staging store.
+        * the density loop's inputs cross slab by slab (16 ranges of cells) on a copy stream; the self bundles of a slab start
+          as soon as it has landed (a self task needs no other cell), the pair bundles when the last slab has;
+        * pack -> loop -> unpack of a bundle run on alternating streams, unpacks chained in bundle order so the reduction order
+          is the task order;
+        * the force loop's extra inputs (the substructs holding v, u) cross during the density loop; what the density loop left
+          on the device (rho, rho_dh, then P, c_s of the ghost) is NOT sent back up for the force loop: the device keeps it
+          within the step (`shadow_bytes` says how much more the link would carry otherwise);
+        * the density loop's results cross back during the force loop, the force loop's results slab by slab BEHIND the
+          bundles: a cell is final once every task with ci <= cell has been unpacked.
     mode "zero-copy": the same kernels read and write the mapped host store directly over the host link.
     """
 
-    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode):
+    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode, n_slabs=16):
         self.sph, self.torch, self.layout, self.hs, self.mode = sph, torch, layout, hs, mode
         n = hs.n
         self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
@@ -474,9 +573,15 @@ class Pipeline:
             self.dev = None
             self.work = hs.store
         self.batches = []
+        self.first_task = []          # first task of every bundle
         for lo, hi in ((0, n_self), (n_self, tasks.shape[0])):          # homogeneous bundles: self tasks, then pair tasks (C22)
             for s in range(lo, hi, bundle):
                 self.batches.append(sph.sph_batch_create(hs.store, tasks[s:min(hi, s + bundle)]))
+                self.first_task.append(s)
+        self.n_self_bundles = sum(1 for s in self.first_task if s < n_self)
+        self.n_self, self.n_tasks, self.bundle = n_self, int(tasks.shape[0]), bundle
+        assert n_self == cells.shape[0] and np.all(tasks["cj"][:n_self] < 0), "the pipeline expects one self task per cell, listed first"
+        self.task_ci = tasks["ci"].astype(np.int64)
         need = [0, 0, 0, 0]
         self.instances = 0
         self.candidates = 0
@@ -489,57 +594,100 @@ class Pipeline:
         self.bufs = [[torch.empty(max(nb, 256), dtype=torch.uint8, device="cuda") for nb in need] for _ in range(2)]
         self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         self.copy = torch.cuda.Stream()
+        self.slabs = cell_slabs(cells, n_slabs)                               # (cell_first, cell_count, particle_first, particle_count)
+        self.slab_cell_end = np.array([c0 + nc for c0, nc, _, _ in self.slabs])
         F = sph.FIELD
         sub = lambda names: sorted({layout.loc[F[k]].sub for k in names})
-        self.up_density, self.down_density = sub(["x", "h", "mass"]), sub(["rho", "rho_dh", "wcount", "wcount_dh"])
-        self.up_force = [s for s in sub(["v", "u", "P", "c_s"]) if s not in self.up_density and s not in self.down_density]
-        self.down_force = sorted(set(sub(["a", "du_dt", "v_sig"]) + sub(["P", "c_s"])))
-        self.h2d_bytes = sum(n * layout.stride[s] for s in self.up_density + self.up_force) if mode == "staged" else 0
-        self.d2h_bytes = sum(n * layout.stride[s] for s in self.down_density + self.down_force) if mode == "staged" else 0
+        self.up_density = sub(["x", "h", "mass"])
+        out_density, out_force = sub(["rho", "rho_dh", "wcount", "wcount_dh"]), sorted(set(sub(["a", "du_dt", "v_sig"]) + sub(["P", "c_s"])))
+        self.up_force = [s for s in sub(["v", "u"]) if s not in self.up_density]
+        self.down_force = out_force
+        self.down_density = [s for s in out_density if s not in out_force]      # a substruct the force loop sends back anyway crosses once
+        stride = lambda subs: sum(n * layout.stride[s] for s in subs)
+        self.h2d_bytes = stride(self.up_density + self.up_force) if mode == "staged" else 0
+        self.d2h_bytes = stride(self.down_density + self.down_force) if mode == "staged" else 0
+        # what re-sending the force loop's inputs from the host store would add (SURVEY.md 8(d) "no device shadow across loops")
+        self.shadow_bytes = stride(sorted(set(sub(["x", "h", "mass", "rho", "rho_dh", "P", "c_s"])) - set(self.up_force))) if mode == "staged" else 0
         self.launches = 0
 
-    def _loop(self, root, k_in, k_out, kernel, ups, downs):
+    def _bundles(self, root, k_in, k_out, kernel, slab_events):
+        """pack -> loop -> unpack of every bundle on alternating streams; yields (bundle index, event of its unpack)"""
         sph, torch = self.sph, self.torch
         s_in, s_out = self.sets[k_in], self.sets[k_out]
-        if self.mode == "staged":
-            self.copy.wait_stream(root)
-            for s in ups:
-                sph.sph_store_upload_sub(self.dev, s, self.hs.sub(s), self.copy)
-            root.wait_stream(self.copy)
-        sph.sph_store_zero(self.work, s_out, root)
-        self.launches += 1
+        # "zero the outputs" is fused into the unpacks of the self bundles (every cell has exactly one self task, and the self
+        # bundles come first): a cell's sums start from 0 when its self task is reduced -- after its slab has landed, which a
+        # separate zero launch could not wait for in the AoS layout, where inputs and outputs share the uploaded struct
         for st in self.streams:
             st.wait_stream(root)
         prev = None
+        waited_all = [False, False]
         for b, batch in enumerate(self.batches):
             st, bufs = self.streams[b & 1], self.bufs[b & 1]
+            if slab_events is not None:
+                if b < self.n_self_bundles:          # self tasks [t0, t1) = cells [t0, t1): wait for the slab holding the last one
+                    last_cell = min(self.first_task[b] + self.bundle, self.n_self) - 1
+                    st.wait_event(slab_events[int(np.searchsorted(self.slab_cell_end, last_cell, side="right"))])
+                elif not waited_all[b & 1]:
+                    st.wait_event(slab_events[-1])
+                    waited_all[b & 1] = True
             sph.sph_pack(self.work, batch, s_in, bufs[k_in], st)
             kernel(batch, bufs[k_in], bufs[k_out], st)
             if prev is not None:
                 st.wait_event(prev)                                       # unpacks in bundle order
-            sph.sph_unpack(self.work, batch, s_out, bufs[k_out], sph.SPH_UNPACK_REDUCE, st)
+            sph.sph_unpack(self.work, batch, s_out, bufs[k_out], sph.SPH_UNPACK_REDUCE_ZERO if b < self.n_self_bundles else sph.SPH_UNPACK_REDUCE, st)
             prev = torch.cuda.Event()
             prev.record(st)
             self.launches += 3
+            yield b, prev
         for st in self.streams:
             root.wait_stream(st)
-        if self.mode == "staged" and downs:
-            self.copy.wait_stream(root)
-            for s in downs:
-                sph.sph_store_download_sub(self.dev, s, self.hs.sub(s), self.copy)
-            # the copy-out overlaps whatever follows on `root`; joined at the end of the step
 
     def step(self, root):
-        sph = self.sph
+        sph, torch = self.sph, self.torch
         self.launches = 0
-        self._loop(root, 0, 1, lambda b, i, o, st: sph.sph_density(b, i, o, st), self.up_density, self.down_density)
-        if self.mode == "staged":
-            for s in self.up_force:
-                sph.sph_store_upload_sub(self.dev, s, self.hs.sub(s), root)
+        staged = self.mode == "staged"
+        slab_events = None
+        if staged:
+            self.copy.wait_stream(root)
+            slab_events = []
+            for c0, nc, p0, npart in self.slabs:
+                for s in self.up_density:
+                    sph.sph_store_upload_range(self.dev, s, self.hs.host[s], p0, npart, self.copy)
+                ev = torch.cuda.Event()
+                ev.record(self.copy)
+                slab_events.append(ev)
+            for s in self.up_force:                                       # crosses during the density loop
+                sph.sph_store_upload_sub(self.dev, s, self.hs.sub(s), self.copy)
+            up2 = torch.cuda.Event()
+            up2.record(self.copy)
+        for _ in self._bundles(root, 0, 1, lambda b, i, o, st: sph.sph_density(b, i, o, st), slab_events):
+            pass
+        if staged:
+            root.wait_event(up2)                                          # the ghost writes P, c_s next to v, u
         sph.sph_ghost(self.work, self.params, root)
         self.launches += 1
-        self._loop(root, 2, 3, lambda b, i, o, st: sph.sph_force(b, i, o, self.params, st), [], self.down_force)
-        if self.mode == "staged":
+        if staged:
+            self.copy.wait_stream(root)                                   # density results (and nothing the force loop writes) cross back
+            for s in self.down_density:
+                sph.sph_store_download_sub(self.dev, s, self.hs.sub(s), self.copy)
+        done_slab = 0
+        for b, ev in self._bundles(root, 2, 3, lambda b, i, o, st: sph.sph_force(b, i, o, self.params, st), None):
+            if not staged or b < self.n_self_bundles:
+                continue
+            # every task with ci < frontier is unpacked once bundle b is: those cells are final
+            nxt = self.first_task[b] + self.bundle
+            frontier = int(self.task_ci[nxt]) if nxt < self.n_tasks else int(self.slab_cell_end[-1])
+            while done_slab < len(self.slabs) and self.slab_cell_end[done_slab] <= frontier:
+                _, _, p0, npart = self.slabs[done_slab]
+                self.copy.wait_event(ev)
+                for s in self.down_force:
+                    sph.sph_store_download_range(self.dev, s, self.hs.host[s], p0, npart, self.copy)
+                done_slab += 1
+        if staged:
+            self.copy.wait_stream(root)
+            for _, _, p0, npart in self.slabs[done_slab:]:                # (only when there is no pair bundle at all)
+                for s in self.down_force:
+                    sph.sph_store_download_range(self.dev, s, self.hs.host[s], p0, npart, self.copy)
             root.wait_stream(self.copy)
 
     def capture(self):
@@ -560,13 +708,13 @@ class Pipeline:
             self.sph.sph_store_destroy(self.dev)
 
 
-def run_config4(args, sph, torch, common):
+def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
     n = args.n or (1 << 26)
     ps, cells, tasks, setup = build_clumpy(sph, 4, 1, n)
     n_self = int(cells.shape[0])
     link = link_probe(torch)
     res = {}
-    for name in ("split", "aos"):
+    for name in layout_names:
         layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
         hs = HostStore(sph, torch, layout, ps, cells)
         for mode in ("staged", "zero-copy"):
@@ -580,6 +728,7 @@ def run_config4(args, sph, torch, common):
             ms = sum(t) / len(t)
             res[f"{name}/{mode}"] = {"ms_per_step": ms, "particles_per_s": n / (ms * 1e-3), "bundles": len(pl.batches), "launches_per_step": pl.launches,
                                      "h2d_bytes_per_step": pl.h2d_bytes, "d2h_bytes_per_step": pl.d2h_bytes,
+                                     "h2d_bytes_if_no_device_shadow": pl.h2d_bytes + pl.shadow_bytes,
                                      "link_gbs": round((pl.h2d_bytes + pl.d2h_bytes) / (ms * 1e-3) / 1e9, 2) if mode == "staged" else None,
                                      "instances_per_loop": int(pl.instances), "candidate_pairs_per_loop": int(pl.candidates),
                                      "capture_s": round(cap_s, 1)}
@@ -592,10 +741,14 @@ def run_config4(args, sph, torch, common):
     roof = {"bound": "host-link", "achieved": P["link_gbs"], "peak": round(link["h2d_gbs"], 2), "unit": "GB/s",
             "frac": None if not P["link_gbs"] else round(P["link_gbs"] / (link["h2d_gbs"] + link["d2h_gbs"]), 3), "traffic": None,
             "kernel": "whole step (H2D + pack/loop/unpack bundles + D2H)", "link_bound_ms": link_time,
+            "step_over_link_time": None if not link_time else round(P["ms_per_step"] / link_time, 2),
             "peak_source": "pinned H2D / D2H copy bandwidth measured in this run"}
     return {"value": P["particles_per_s"], "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
             "config": {"workload": f"configs[4]: {n} particles (uniform + clumps), whole step in bundles of 4096 tasks over 2 streams, store in pinned host memory",
-                       "layout": key, "store": "pinned host", "l2": "inputs larger than L2", "setup": setup, "link": link},
+                       "layout": key, "store": "pinned host", "l2": "inputs larger than L2", "setup": setup, "link": link,
+                       "e2e": "staged: density inputs cross slab by slab ahead of the bundles, force inputs (v, u) during the density loop, results "
+                              "behind the bundles; what the density loop and the ghost left on the device (rho, rho_dh, P, c_s; x, h, mass) is not "
+                              "re-sent for the force loop (device shadow within the step; h2d_bytes_if_no_device_shadow says what it saves)"},
             "gpu_launches": P["launches_per_step"] * args.steps, "roofline": roof, "variants": res,
             "e2e": {"value": P["particles_per_s"], "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes_per_step"],
                     "d2h_bytes_per_step": P["d2h_bytes_per_step"], "ms_per_step": P["ms_per_step"]}}

@@ -93,9 +93,9 @@ typedef struct { int32_t ci, cj; double frame_i[3]; double frame_j[3]; } sph_tas
 typedef struct { float gamma, alpha, beta; } sph_params;   /* ideal-gas gamma; viscosity alpha, beta */
 
 enum { SPH_MEM_DEVICE = 0, SPH_MEM_HOST_PINNED = 1 };
-enum { SPH_UNPACK_REDUCE = 0,   /* per-field operator: += for RHO, RHO_DH, WCOUNT, WCOUNT_DH, A, DU_DT; max for V_SIG;
-                                   overwrite for every other field -- applied in ascending task order, side i
-                                   before side j, in f32 (bit-reproducible) */
+enum { SPH_UNPACK_REDUCE = 0,   /* per-field operator: += for the neighbour sums RHO, RHO_DH, WCOUNT, WCOUNT_DH, DIV_V, ROT_V, A,
+                                   DU_DT; max for V_SIG; overwrite for every other field -- applied in ascending task
+                                   order, side i before side j, in f32 (bit-reproducible) */
        SPH_UNPACK_ASSIGN = 1,   /* overwrite for every field, same order (last task wins) */
        SPH_UNPACK_REDUCE_ZERO = 2 }; /* SPH_UNPACK_REDUCE preceded by "zero the outputs" for the particles of the cells the call
                                    * touches: the sums start from 0 instead of the store's values (bit-identical to

@@ -34,6 +34,10 @@ DENSITY_OUT = ([(RHO, 0, 1), (RHO_DH, 0, 1), (WCOUNT, 0, 1), (WCOUNT_DH, 0, 1)],
 FORCE_IN = ([(X, 0, 3), (H, 0, 1), (MASS, 0, 1), (RHO, 0, 1), (RHO_DH, 0, 1), (V, 0, 3), (U, 0, 1), (P, 0, 1), (CS, 0, 1)],
             FLAG_X_REL_F32)
 FORCE_OUT = ([(A, 0, 3), (DU_DT, 0, 1), (V_SIG, 0, 1)], 0)
+# the three-loop cycle (reading C34): Table 1's p-g column; div_v, rot_v out; the force inputs plus div_v, rot_v, time_bin
+GRADIENT_IN = ([(X, 0, 3), (V, 0, 3), (MASS, 0, 1), (H, 0, 1), (U, 0, 1), (RHO, 0, 1)], FLAG_X_REL_F32)
+GRADIENT_OUT = ([(DIV_V, 0, 1), (ROT_V, 0, 3)], 0)
+FORCE3_IN = (FORCE_IN[0] + [(DIV_V, 0, 1), (ROT_V, 0, 3), (TIME_BIN, 0, 1)], FLAG_X_REL_F32)
 
 
 def build(force: bool = False) -> str:
@@ -61,6 +65,7 @@ def lib():
         _lib.orc_cells_build_octree.restype = C.c_int64
         _lib.orc_tasks_build.restype = C.c_int64
         _lib.orc_iterate_h.restype = C.c_int64
+        _lib.orc_compare_blocks.restype = C.c_int64
     return _lib
 
 
@@ -193,6 +198,40 @@ def force(cells, tasks, buf_in, alpha: float = 0.8, beta: float = 3.0, fill: int
     return out
 
 
+def compare_blocks(cells, tasks, rec_bytes: int, buf_a, buf_b) -> int:
+    """test support: -1 if the two buffers agree on every record byte (pad bytes skipped), else the first differing offset"""
+    assert buf_a.dtype == np.uint8 and buf_b.dtype == np.uint8 and buf_a.flags.c_contiguous and buf_b.flags.c_contiguous
+    return int(lib().orc_compare_blocks(_p(cells), _p(tasks), C.c_int64(tasks.shape[0]), C.c_int(rec_bytes), _p(buf_a), _p(buf_b)))
+
+
+def flag_cutoff_pairs(cells, tasks, buf_in, rel: float = 1e-5) -> np.ndarray:
+    """reading C31: bool[n], True where a particle has a partner within rel of the cut-off in some task (buf_in: FORCE_IN)."""
+    n = int((cells["first"].astype(np.int64) + cells["count"]).max())
+    flags = np.zeros(n, dtype=np.uint8)
+    lib().orc_flag_cutoff_pairs(_p(cells), _p(tasks), C.c_int64(tasks.shape[0]), _p(buf_in), C.c_double(rel), _p(flags))
+    return flags.astype(bool)
+
+
+def gradient(cells, tasks, buf_in, fill: int = 0xCD) -> np.ndarray:
+    _, total = block_offsets(cells, tasks, 16)
+    out = np.full(total, fill, dtype=np.uint8)
+    lib().orc_gradient(_p(cells), _p(tasks), C.c_int64(tasks.shape[0]), _p(buf_in), _p(out))
+    return out
+
+
+def force3(cells, tasks, buf_in, alpha: float = 0.8, beta: float = 3.0, fill: int = 0xCD) -> np.ndarray:
+    _, total = block_offsets(cells, tasks, 20)
+    out = np.full(total, fill, dtype=np.uint8)
+    lib().orc_force3(_p(cells), _p(tasks), C.c_int64(tasks.shape[0]), _p(buf_in), _p(out), C.c_double(alpha), C.c_double(beta))
+    return out
+
+
+def brute_gradient(parts, box: float = 1.0) -> np.ndarray:
+    out = np.empty((parts.shape[0], 4), dtype=np.float64)
+    lib().orc_brute_gradient(_p(parts), C.c_uint64(parts.shape[0]), C.c_double(box), _p(out))
+    return out
+
+
 def ghost(parts, gamma: float = 5.0 / 3.0) -> None:
     lib().orc_ghost(_p(parts), C.c_uint64(parts.shape[0]), C.c_double(gamma))
 
@@ -238,3 +277,19 @@ def force_cycle(parts, cells, tasks, batch: int = 0, alpha: float = 0.8, beta: f
     for s in range(0, tasks.shape[0], nb):
         t = tasks[s:s + nb]
         unpack(parts, cells, t, FORCE_OUT, force(cells, t, pack(parts, cells, t, FORCE_IN), alpha, beta))
+
+
+def gradient_cycle(parts, cells, tasks, batch: int = 0):
+    zero(parts, GRADIENT_OUT)
+    nb = tasks.shape[0] if batch <= 0 else batch
+    for s in range(0, tasks.shape[0], nb):
+        t = tasks[s:s + nb]
+        unpack(parts, cells, t, GRADIENT_OUT, gradient(cells, t, pack(parts, cells, t, GRADIENT_IN)))
+
+
+def force3_cycle(parts, cells, tasks, batch: int = 0, alpha: float = 0.8, beta: float = 3.0):
+    zero(parts, FORCE_OUT)
+    nb = tasks.shape[0] if batch <= 0 else batch
+    for s in range(0, tasks.shape[0], nb):
+        t = tasks[s:s + nb]
+        unpack(parts, cells, t, FORCE_OUT, force3(cells, t, pack(parts, cells, t, FORCE3_IN), alpha, beta))

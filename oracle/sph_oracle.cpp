@@ -20,6 +20,7 @@
 //                            cubic spline, support 2h, grad-h terms, Monaghan viscosity (C1, C2, C9-C13)
 //   unpack ................. PAPER.md:82 ("performs all required reductions")  (C8)
 //   ghost .................. PAPER.md:62 (linear update kernels)               (C12)
+//   gradient loop, Balsara . PAPER.md:41, Table 1 columns p-g / u-g / p-f (47-58)  (C34; next-scope row f2)
 //
 // Arithmetic: record values are f32 (Table 1); the loops promote them to f64,
 // accumulate in f64 and round once to f32.  pack does one f64 subtraction and
@@ -213,6 +214,80 @@ void force_block(const float* tgt, uint32_t n_t, const float* src, uint32_t n_s,
             }
         }
         float* o = out + 5 * i;                       // FORCE_OUT = [a0 a1 a2 du_dt v_sig]
+        o[0] = (float)ax; o[1] = (float)ay; o[2] = (float)az; o[3] = (float)dudt; o[4] = (float)vsig;
+    }
+}
+
+// ---- gradient partial sums ("a third gradient loop between the density and the force loops"; reading C34) ----
+// records: GRADIENT_IN = [xr0 xr1 xr2 v0 v1 v2 mass h u rho] f32 (Table 1, column p-g: x, v, mass, h, u, rho; u is packed as
+// the table says, its consumer -- Sphenix' diffusion term -- is not part of this reading).
+// For instance i over j != i with 0 < r < 2 h_i:  g = (m_j / rho_j) dW/dr(r, h_i),  e = (x_i - x_j) / r,  dv = v_j - v_i
+//   div_v += g (dv . e)        rot_v += g (e x dv)
+// GRADIENT_OUT = [div_v rot_v0 rot_v1 rot_v2].
+void gradient_block(const float* tgt, uint32_t n_t, const float* src, uint32_t n_s, bool self, float* out) {
+    for (uint32_t i = 0; i < n_t; ++i) {
+        const float* ri = tgt + 10 * i;
+        const double hi = ri[7];
+        double div = 0, rx = 0, ry = 0, rz = 0;
+        for (uint32_t j = 0; j < n_s; ++j) {
+            if (self && j == i) continue;
+            const float* rj = src + 10 * j;
+            const double dx = (double)ri[0] - (double)rj[0], dy = (double)ri[1] - (double)rj[1], dz = (double)ri[2] - (double)rj[2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 > 0.0 && r2 < 4.0 * hi * hi) {
+                const double r = std::sqrt(r2);
+                const double ex = dx / r, ey = dy / r, ez = dz / r;
+                const double g = (double)rj[6] / (double)rj[9] * dW_dr(r, hi);
+                const double dvx = (double)rj[3] - (double)ri[3], dvy = (double)rj[4] - (double)ri[4], dvz = (double)rj[5] - (double)ri[5];
+                div += g * (dvx * ex + dvy * ey + dvz * ez);
+                rx += g * (ey * dvz - ez * dvy); ry += g * (ez * dvx - ex * dvz); rz += g * (ex * dvy - ey * dvx);
+            }
+        }
+        float* o = out + 4 * i;
+        o[0] = (float)div; o[1] = (float)rx; o[2] = (float)ry; o[3] = (float)rz;
+    }
+}
+
+// Balsara-type switch (reading C34): B = |div v| / (|div v| + |rot v| + 1e-4 c_s / h): 1 in pure compression, 0 in pure shear
+double balsara(const float* r18) {
+    const double div = std::fabs((double)r18[13]);
+    const double rot = std::sqrt((double)r18[14] * r18[14] + (double)r18[15] * r18[15] + (double)r18[16] * r18[16]);
+    return div / (div + rot + 1.0e-4 * (double)r18[12] / (double)r18[3]);
+}
+
+// ---- force partial sums of the three-loop cycle: force_block with the viscous term scaled by (B_i + B_j) / 2 ----
+// records: FORCE3_IN = [xr0 xr1 xr2 h mass rho rho_dh v0 v1 v2 u P cs div_v rot_v0 rot_v1 rot_v2 time_bin] (time_bin as Table 1's
+// column p-f lists it; every particle is active, reading C14, so no arithmetic depends on it)
+void force3_block(const float* tgt, uint32_t n_t, const float* src, uint32_t n_s, bool self, float* out, double alpha, double beta) {
+    for (uint32_t i = 0; i < n_t; ++i) {
+        const float* ri = tgt + 18 * i;
+        const double hi = ri[3], rhoi = ri[5], rho_dhi = ri[6], Pi = ri[11], ci = ri[12];
+        const double Ai = Pi / ((1.0 + hi * rho_dhi / (3.0 * rhoi)) * rhoi * rhoi);
+        const double Bi = balsara(ri);
+        double ax = 0, ay = 0, az = 0, dudt = 0, vsig = 0;
+        for (uint32_t j = 0; j < n_s; ++j) {
+            if (self && j == i) continue;
+            const float* rj = src + 18 * j;
+            const double hj = rj[3], mj = rj[4], rhoj = rj[5], rho_dhj = rj[6], Pj = rj[11], cj = rj[12];
+            const double dx = (double)ri[0] - (double)rj[0], dy = (double)ri[1] - (double)rj[1], dz = (double)ri[2] - (double)rj[2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            const double hcut = std::max(2.0 * hi, 2.0 * hj);
+            if (r2 > 0.0 && r2 < hcut * hcut) {
+                const double r = std::sqrt(r2);
+                const double ex = dx / r, ey = dy / r, ez = dz / r;
+                const double Aj = Pj / ((1.0 + hj * rho_dhj / (3.0 * rhoj)) * rhoj * rhoj);
+                const double Gi = dW_dr(r, hi), Gj = dW_dr(r, hj), Gbar = 0.5 * (Gi + Gj);
+                const double vr = ((double)ri[7] - (double)rj[7]) * ex + ((double)ri[8] - (double)rj[8]) * ey + ((double)ri[9] - (double)rj[9]) * ez;
+                const double mu = std::min(0.0, vr);
+                const double vs = ci + cj - beta * mu;
+                const double Pi_visc = 0.5 * (Bi + balsara(rj)) * (-0.5 * alpha * vs * mu / (0.5 * (rhoi + rhoj)));
+                const double fr = -mj * (Ai * Gi + Aj * Gj + Pi_visc * Gbar);
+                ax += fr * ex; ay += fr * ey; az += fr * ez;
+                dudt += mj * (Ai * Gi + 0.5 * Pi_visc * Gbar) * vr;
+                vsig = std::max(vsig, vs);
+            }
+        }
+        float* o = out + 5 * i;
         o[0] = (float)ax; o[1] = (float)ay; o[2] = (float)az; o[3] = (float)dudt; o[4] = (float)vsig;
     }
 }
@@ -486,7 +561,7 @@ int orc_unpack(Part* parts, const Cell* cells, const Task* tasks, int64_t n_task
                             float val; std::memcpy(&val, in, 4); in += 4;
                             float* dst = f32_member(p, a.field) + comp;
                             const bool is_sum = a.field == RHO || a.field == RHO_DH || a.field == WCOUNT || a.field == WCOUNT_DH ||
-                                                a.field == A || a.field == DU_DT;
+                                                a.field == A || a.field == DU_DT || a.field == DIV_V || a.field == ROT_V;
                             if (mode == MODE_REDUCE && is_sum) *dst = *dst + val;
                             else if (mode == MODE_REDUCE && a.field == V_SIG) *dst = std::fmax(*dst, val);
                             else std::memcpy(dst, &val, 4);
@@ -550,6 +625,120 @@ int orc_force(const Cell* cells, const Task* tasks, int64_t n_tasks, const uint8
         float* oj = (float*)(out + off_out[2 * t + 1]);
         force_block(bi, ni, bj, nj, false, oi, alpha, beta);
         force_block(bj, nj, bi, ni, false, oj, alpha, beta);
+    }
+    return 0;
+}
+
+// ---- test support: compare two buffers of the same tasks block by block (pad bytes are unspecified and skipped).
+// Returns -1 if every record byte agrees, else the byte offset of the first difference inside some block.
+int64_t orc_compare_blocks(const Cell* cells, const Task* tasks, int64_t n_tasks, int rec_bytes, const uint8_t* a, const uint8_t* b) {
+    std::vector<uint64_t> off(2 * (size_t)n_tasks);
+    block_offsets(cells, tasks, n_tasks, rec_bytes, off.data());
+    int64_t first_bad = -1;
+#pragma omp parallel for schedule(dynamic, 256) num_threads(g_threads)
+    for (int64_t t = 0; t < n_tasks; ++t) {
+        for (int side = 0; side < 2; ++side) {
+            const int32_t c = side == 0 ? tasks[t].ci : tasks[t].cj;
+            if (c < 0) continue;
+            const uint64_t o = off[2 * t + side], nb = (uint64_t)cells[c].count * rec_bytes;
+            if (std::memcmp(a + o, b + o, nb) != 0) {
+                uint64_t k = 0;
+                while (a[o + k] == b[o + k]) ++k;
+#pragma omp critical
+                if (first_bad < 0 || (int64_t)(o + k) < first_bad) first_bad = (int64_t)(o + k);
+            }
+        }
+    }
+    return first_bad;
+}
+
+// ---- reading C31 (test support, not a step of the method): v_sig is a maximum, so it jumps when a pair sits exactly on
+// the cut-off r = max(2 h_i, 2 h_j) and f32 / f64 arithmetic decide it differently.  flags_out[p] = 1 for every particle
+// that has, in some task, a partner with |r - R_cut| < rel * R_cut; those particles are exempt from the v_sig comparison.
+// in: FORCE_IN blocks as packed by orc_pack.
+int orc_flag_cutoff_pairs(const Cell* cells, const Task* tasks, int64_t n_tasks, const uint8_t* in, double rel, uint8_t* flags_out) {
+    std::vector<uint64_t> off_in(2 * (size_t)n_tasks);
+    block_offsets(cells, tasks, n_tasks, 52, off_in.data());
+#pragma omp parallel for schedule(dynamic, 16) num_threads(g_threads)
+    for (int64_t t = 0; t < n_tasks; ++t) {
+        const int32_t ci = tasks[t].ci, cj = tasks[t].cj < 0 ? tasks[t].ci : tasks[t].cj;
+        const float* bi = (const float*)(in + off_in[2 * t]);
+        const float* bj = tasks[t].cj < 0 ? bi : (const float*)(in + off_in[2 * t + 1]);
+        for (uint32_t i = 0; i < cells[ci].count; ++i)
+            for (uint32_t j = 0; j < cells[cj].count; ++j) {
+                const float *ri = bi + 13 * i, *rj = bj + 13 * j;
+                const double dx = (double)ri[0] - (double)rj[0], dy = (double)ri[1] - (double)rj[1], dz = (double)ri[2] - (double)rj[2];
+                const double r = std::sqrt(dx * dx + dy * dy + dz * dz), cut = std::max(2.0 * (double)ri[3], 2.0 * (double)rj[3]);
+                if (std::fabs(r - cut) < rel * cut) {          // benign race: every writer stores 1
+                    flags_out[cells[ci].first + i] = 1;
+                    flags_out[cells[cj].first + j] = 1;
+                }
+            }
+    }
+    return 0;
+}
+
+// ---- gradient loop over tasks (reading C34): in GRADIENT_IN blocks (40-byte records), out GRADIENT_OUT blocks (16-byte records)
+int orc_gradient(const Cell* cells, const Task* tasks, int64_t n_tasks, const uint8_t* in, uint8_t* out) {
+    std::vector<uint64_t> off_in(2 * (size_t)n_tasks), off_out(2 * (size_t)n_tasks);
+    block_offsets(cells, tasks, n_tasks, 40, off_in.data());
+    block_offsets(cells, tasks, n_tasks, 16, off_out.data());
+#pragma omp parallel for schedule(dynamic, 16) num_threads(g_threads)
+    for (int64_t t = 0; t < n_tasks; ++t) {
+        const uint32_t ni = cells[tasks[t].ci].count;
+        const float* bi = (const float*)(in + off_in[2 * t]);
+        float* oi = (float*)(out + off_out[2 * t]);
+        if (tasks[t].cj < 0) { gradient_block(bi, ni, bi, ni, true, oi); continue; }
+        const uint32_t nj = cells[tasks[t].cj].count;
+        const float* bj = (const float*)(in + off_in[2 * t + 1]);
+        float* oj = (float*)(out + off_out[2 * t + 1]);
+        gradient_block(bi, ni, bj, nj, false, oi);
+        gradient_block(bj, nj, bi, ni, false, oj);
+    }
+    return 0;
+}
+
+// ---- force loop of the three-loop cycle: in FORCE3_IN blocks (72-byte records), out FORCE_OUT blocks (20-byte records)
+int orc_force3(const Cell* cells, const Task* tasks, int64_t n_tasks, const uint8_t* in, uint8_t* out, double alpha, double beta) {
+    std::vector<uint64_t> off_in(2 * (size_t)n_tasks), off_out(2 * (size_t)n_tasks);
+    block_offsets(cells, tasks, n_tasks, 72, off_in.data());
+    block_offsets(cells, tasks, n_tasks, 20, off_out.data());
+#pragma omp parallel for schedule(dynamic, 16) num_threads(g_threads)
+    for (int64_t t = 0; t < n_tasks; ++t) {
+        const uint32_t ni = cells[tasks[t].ci].count;
+        const float* bi = (const float*)(in + off_in[2 * t]);
+        float* oi = (float*)(out + off_out[2 * t]);
+        if (tasks[t].cj < 0) { force3_block(bi, ni, bi, ni, true, oi, alpha, beta); continue; }
+        const uint32_t nj = cells[tasks[t].cj].count;
+        const float* bj = (const float*)(in + off_in[2 * t + 1]);
+        float* oj = (float*)(out + off_out[2 * t + 1]);
+        force3_block(bi, ni, bj, nj, false, oi, alpha, beta);
+        force3_block(bj, nj, bi, ni, false, oj, alpha, beta);
+    }
+    return 0;
+}
+
+// brute force O(N^2) with minimum image on the ORIGINAL f64 positions: div_v, rot_v (f64) from v, mass, h, rho as stored
+int orc_brute_gradient(const Part* parts, uint64_t n, double box, double* out4) {
+#pragma omp parallel for schedule(static) num_threads(g_threads)
+    for (int64_t i = 0; i < (int64_t)n; ++i) {
+        const Part& pi = parts[i];
+        const double hi = pi.h;
+        double s[4] = {0, 0, 0, 0};
+        for (uint64_t j = 0; j < n; ++j) {
+            if ((uint64_t)i == j) continue;
+            const Part& pj = parts[j];
+            double d[3], r2 = 0;
+            for (int k = 0; k < 3; ++k) { d[k] = pi.x[k] - pj.x[k]; d[k] -= box * std::round(d[k] / box); r2 += d[k] * d[k]; }
+            if (r2 > 0.0 && r2 < 4.0 * hi * hi) {
+                const double r = std::sqrt(r2), g = (double)pj.mass / (double)pj.rho * dW_dr(r, hi);
+                const double e[3] = {d[0] / r, d[1] / r, d[2] / r};
+                const double dv[3] = {(double)pj.v[0] - pi.v[0], (double)pj.v[1] - pi.v[1], (double)pj.v[2] - pi.v[2]};
+                s[0] += g * (dv[0] * e[0] + dv[1] * e[1] + dv[2] * e[2]);
+                s[1] += g * (e[1] * dv[2] - e[2] * dv[1]); s[2] += g * (e[2] * dv[0] - e[0] * dv[2]); s[3] += g * (e[0] * dv[1] - e[1] * dv[0]);
+            }
+        }
+        for (int k = 0; k < 4; ++k) out4[4 * i + k] = s[k];
     }
     return 0;
 }

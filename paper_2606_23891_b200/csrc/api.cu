@@ -146,7 +146,7 @@ int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, i
         if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32))
             return fail(SPH_ERR_UNSUPPORTED, "X packed as relative f32 cannot be unpacked (the frame shift is not invertible in f32)");
         const bool is_sum = a.field == SPH_RHO || a.field == SPH_RHO_DH || a.field == SPH_WCOUNT || a.field == SPH_WCOUNT_DH ||
-                            a.field == SPH_A || a.field == SPH_DU_DT;
+                            a.field == SPH_A || a.field == SPH_DU_DT || a.field == SPH_DIV_V || a.field == SPH_ROT_V;
         for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
             const uint32_t off = loc.off + c * field_elem_bytes(a.field);
             if (a.field == SPH_X || a.field == SPH_ID) {

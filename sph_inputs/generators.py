@@ -135,18 +135,47 @@ def _min_image(d: np.ndarray) -> np.ndarray:
 
 def mixture_density(x: np.ndarray, centres: np.ndarray, n_total: int, frac_clumps: float,
                     sigma: float, chunk: int = 1 << 18) -> np.ndarray:
-    """Analytic number density of the uniform + Gaussian-clump mixture (nearest image)."""
+    """Analytic number density of the uniform + Gaussian-clump mixture (nearest image).
+
+    A clump's term is dropped beyond 6.25 sigma (exp(-19.5) = 3e-9 of its peak): the points are binned on a
+    coarse periodic grid once and every clump visits only the bins within reach, which is what makes the
+    2^26-particle workload generate in seconds instead of minutes.
+    """
     n_c = centres.shape[0]
     norm = (2.0 * np.pi) ** -1.5 / sigma ** 3
-    out = np.empty(x.shape[0], dtype=np.float64)
-    for s in range(0, x.shape[0], chunk):
-        xs = x[s:s + chunk]
-        acc = np.zeros(xs.shape[0])
+    reach = 6.25 * sigma
+    nb = max(1, min(32, int(np.floor(1.0 / reach))))            # bins per dimension, bin width >= reach
+    acc = np.zeros(x.shape[0])
+    if nb < 3 or x.shape[0] < (1 << 16):                         # small problem or wide clumps: every clump sees every point
+        for s in range(0, x.shape[0], chunk):
+            xs = x[s:s + chunk]
+            a = np.zeros(xs.shape[0])
+            for c in range(n_c):
+                d = _min_image(xs - centres[c])
+                r2 = np.einsum("ij,ij->i", d, d)
+                a += np.where(r2 < reach * reach, np.exp(-0.5 * r2 / sigma ** 2), 0.0)
+            acc[s:s + chunk] = a
+    else:
+        b = np.minimum((x * nb).astype(np.int64), nb - 1)
+        key = (b[:, 0] * nb + b[:, 1]) * nb + b[:, 2]
+        order = np.argsort(key, kind="stable")
+        start = np.searchsorted(key[order], np.arange(nb ** 3 + 1))
+        xo = x[order]
+        ao = np.zeros(x.shape[0])
         for c in range(n_c):
-            d = _min_image(xs - centres[c])
-            acc += np.exp(-0.5 * np.einsum("ij,ij->i", d, d) / sigma ** 2)
-        out[s:s + chunk] = n_total * ((1.0 - frac_clumps) + frac_clumps / n_c * norm * acc)
-    return out
+            cb = np.minimum((centres[c] * nb).astype(np.int64), nb - 1)
+            for da in (-1, 0, 1):
+                for db in (-1, 0, 1):
+                    k0 = (((cb[0] + da) % nb) * nb + (cb[1] + db) % nb) * nb
+                    for dc in (-1, 0, 1):
+                        k = k0 + (cb[2] + dc) % nb
+                        lo, hi = start[k], start[k + 1]
+                        if hi > lo:
+                            d = _min_image(xo[lo:hi] - centres[c])
+                            r2 = np.einsum("ij,ij->i", d, d)
+                            ao[lo:hi] += np.where(r2 < reach * reach, np.exp(-0.5 * r2 / sigma ** 2), 0.0)
+        acc[order] = ao
+    return n_total * ((1.0 - frac_clumps) + frac_clumps / n_c * norm * acc)
 
 
 def clumpy_mixture(n: int, seed: int, n_clumps: int = 64, frac_clumps: float = 0.7,

@@ -3,9 +3,14 @@
 configs[1] (262,144 particles, 57,344 tasks in ONE batch, exactly what `bench.py` runs): the oracle finishes a whole
 step of it in about a second on the box's cores, so everything is compared in full -- pack buffers and unpack results
 byte for byte, the physics of every particle within the north_star tolerances, for both store layouts.
-configs[2] (2^21 particles, bundles of 512 tasks): pack FORCE_IN and unpack FORCE_OUT compared in full, byte for byte,
-in the segmented launch configuration; the force loop on bundles sampled across the box (left, interface, right),
-each recomputed by the oracle from the same packed records.
+configs[2] (2^21 particles, bundles of 512 tasks, h from the oracle's 48-neighbour iteration, rho / P / c_s from its density
+cycle and ghost): pack FORCE_IN and unpack FORCE_OUT compared in full, byte for byte, in the segmented launch configuration;
+the force loop on bundles sampled across the box (left, interface, right), each recomputed by the oracle from the same
+packed records; the library's own h iteration (bench setup) against the oracle's.
+configs[3] (2^24 clustered particles, octree <= 400 per leaf): pack and unpack compared in full, byte for byte.
+configs[4] (2^26 particles): the two-stream bundle pipeline of bench.py on the full set, 1,024 sampled cells recomputed by the
+oracle from all their tasks, momentum and energy invariants on the full output.  (The same pipeline is compared in full,
+bit for bit and against the oracle, on a 2^19 instance in test_gpu_pipeline.py.)
 """
 import numpy as np
 import pytest
@@ -31,8 +36,10 @@ def config1():
         ref = raw_copy(ps)
         orc.density_cycle(ref, cells, tasks)
         orc.ghost(ref, GAMMA)
+        f_in = orc.pack(ref, cells, tasks, orc.FORCE_IN)
+        exempt = orc.flag_cutoff_pairs(cells, tasks, f_in)              # C31: particles with a partner on the cut-off
         orc.force_cycle(ref, cells, tasks)
-        _C1.update(ps=ps, cells=cells, tasks=tasks, ref=ref)
+        _C1.update(ps=ps, cells=cells, tasks=tasks, ref=ref, exempt=exempt)
     return _C1["ps"], _C1["cells"], _C1["tasks"], _C1["ref"]
 
 
@@ -51,6 +58,16 @@ def _block_mask(cells, tasks, rec, total):
     return np.cumsum(m[:-1]) > 0
 
 
+def _record_particles(cells, tasks):
+    """particle index of every record of a buffer, in buffer order (task ascending, side i then side j)"""
+    c = np.stack([tasks["ci"], tasks["cj"]], axis=1).ravel().astype(np.int64)
+    c = c[c >= 0]
+    cnt = cells["count"][c].astype(np.int64)
+    start = np.repeat(cells["first"][c].astype(np.int64), cnt)
+    within = np.arange(cnt.sum()) - np.repeat(np.cumsum(cnt) - cnt, cnt)
+    return start + within
+
+
 @pytest.mark.parametrize("layout", ["split", "aos"])
 def test_config1_whole_step_every_particle(layout):
     ps, cells, tasks, ref = config1()
@@ -60,7 +77,7 @@ def test_config1_whole_step_every_particle(layout):
     assert np.array_equal(canon(gpu_step(g)), canon(got))      # the seven-launch step equals the nine-launch one bit for bit
     check_store_physics(got, ref)
     vs_ok = np.abs(got["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
-    assert vs_ok.mean() > 0.999                          # C31: only particles with a neighbour on the cut-off may differ
+    assert np.all(vs_ok | _C1["exempt"]) and _C1["exempt"].mean() < 0.01      # C31: only particles with a partner on the cut-off may differ
     for fld in ("x", "v", "mass", "h", "u", "div_v", "rot_v", "id", "time_bin"):
         assert np.array_equal(got[fld], ps[fld]), fld
     m = got["mass"].astype(np.float64)
@@ -119,7 +136,8 @@ def test_config1_loops_every_record():
     amax, dumax = np.abs(ref["a"]).max(), np.abs(ref["du_dt"]).max()
     assert np.all(np.abs(g5[:, :3] - w5[:, :3]) <= np.maximum(1e-4 * np.abs(w5[:, :3]), 1e-6 * amax))
     assert np.all(np.abs(g5[:, 3] - w5[:, 3]) <= np.maximum(1e-4 * np.abs(w5[:, 3]), 1e-6 * dumax))
-    assert (np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])).mean() > 0.999
+    exempt = _C1["exempt"][_record_particles(cells, tasks)]              # C31
+    assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt)
     g.close()
 
 
@@ -129,19 +147,24 @@ _C2 = {}
 
 
 def config2():
-    """2^21 particles of the Sod-like setup in cell order with seeded (not iterated) variable h: the byte-level checks
-    need only the shape of the workload (102 / 26 particles per cell, bundles of 512), not converged physics."""
+    """2^21 particles of the Sod-like setup in cell order, in the state the force loop of configs[2] starts from, every
+    value produced by the oracle: h from the 48-neighbour iteration (reading C20), rho and rho_dh from the density cycle,
+    u such that P = 1 | 0.1 (reading C18), P and c_s from the ghost."""
     if not _C2:
         orc.set_threads(64)
         parts = si.config2_positions(seed=1)
+        h, bad = orc.iterate_h(parts["x"], parts["h"], h_cap=0.4999 / 32)
+        assert bad == 0
+        parts["h"] = h
         ps, cells, tasks, n_self, n_pair = sort_grid(parts, 32)
         assert ps.shape[0] == 1 << 21 and n_self == 32768
-        rng = np.random.default_rng(5)
-        for name in ("v",):
-            ps[name] = (0.1 * rng.standard_normal((ps.shape[0], 3))).astype(np.float32)
-        for name in ("rho", "P", "c_s", "u"):
-            ps[name] = (rng.random(ps.shape[0]) + 0.5).astype(np.float32)
-        ps["rho_dh"] = (rng.standard_normal(ps.shape[0]) * 0.1).astype(np.float32)
+        orc.density_cycle(ps, cells, tasks)
+        p_target = np.where(ps["x"][:, 0] < 0.5, 1.0, 0.1)
+        ps["u"] = (p_target / ((GAMMA - 1.0) * ps["rho"].astype(np.float64))).astype(np.float32)
+        orc.ghost(ps, GAMMA)
+        nn = 32.0 / 3.0 * np.pi * ps["h"].astype(np.float64) ** 3 * ps["wcount"]
+        assert np.abs(nn - 48.0).max() < 0.02                                # the condition holds through the independent pipeline
+        assert ps["rho"][ps["x"][:, 0] < 0.5].mean() > 2.5 * ps["rho"][ps["x"][:, 0] >= 0.5].mean()      # two densities
         _C2.update(ps=ps, cells=cells, tasks=tasks)
     return _C2["ps"], _C2["cells"], _C2["tasks"]
 
@@ -181,9 +204,6 @@ def test_config2_pack_unpack_bundles_of_512_bytes_in_full():
 
 def test_config2_force_on_sampled_bundles():
     ps, cells, tasks = config2()
-    ps = raw_copy(ps)
-    ps["rho"] = np.where(ps["x"][:, 0] < 0.5, 1.568, 0.4).astype(np.float32)      # plausible densities of the two halves
-    ps["rho_dh"] = 0
     g = GpuCase(ps, cells, tasks, "split", tasks_per_segment=512)
     s_in, s_out = to_attrset(orc.FORCE_IN), to_attrset(orc.FORCE_OUT)
     b_in = g.pack(s_in)
@@ -204,5 +224,133 @@ def test_config2_force_on_sampled_bundles():
         amax, dumax = np.abs(w5[:, :3]).max(), np.abs(w5[:, 3]).max()
         assert np.all(np.abs(g5[:, :3] - w5[:, :3]) <= np.maximum(1e-4 * np.abs(w5[:, :3]), 1e-6 * amax)), b
         assert np.all(np.abs(g5[:, 3] - w5[:, 3]) <= np.maximum(1e-4 * np.abs(w5[:, 3]), 1e-6 * dumax)), b
-        assert (np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4]) + 1e-30).mean() > 0.995, b
+        exempt = orc.flag_cutoff_pairs(cells, sel, want_in)[_record_particles(cells, sel)]      # C31, this bundle's own pairs
+        assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt) and exempt.mean() < 0.01, b
     g.close()
+
+
+def test_library_h_iteration_matches_the_oracles():
+    """bench_workloads.iterate_h_on_gpu (the library's density loop driving Newton steps; setup of the configs[2] bench)
+    against orc.iterate_h (reading C20) on a 2^15 Sod-like box: both solve (4/3) pi (2h)^3 wcount = 48, to 1e-3 here."""
+    import bench_workloads as bw
+    parts = si.config2_positions(seed=3, n_yz=32, n_left=25, n_right=6)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 8)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    cap = np.float32(0.4999 * float(cells["width"][0]))
+    ps["h"] = np.minimum(ps["h"], cap)
+    tasks, _, _ = sph.sph_tasks_build(cells, np.full(cells.shape[0], cap, dtype=np.float32))
+    h_gpu, worst, iters = bw.iterate_h_on_gpu(sph, torch, ps, cells, tasks, tol=1e-3, max_iter=30)
+    h_orc, bad = orc.iterate_h(ps["x"], ps["h"], h_cap=float(cap), tol=1e-3, max_iter=60)
+    assert bad == 0 and worst <= 1e-3 and iters < 30
+    assert np.max(np.abs(h_gpu.astype(np.float64) - h_orc) / h_orc) <= 1e-5
+    assert h_orc.max() / h_orc.min() > 1.4                                   # really two densities
+
+
+# ------------------------------------------------------------------ configs[3]
+
+def test_config3_pack_and_unpack_bytes_in_full():
+    """2^24 clustered particles, octree <= 400 per leaf, ~2.0e6 tasks / 5.2e8 instances: the 5- and 13-field packs (C21) of
+    every task and the 13-field REDUCE unpack, byte for byte, AoS and split-AoS.  The buffers are tens of GB, so tasks go
+    through in slices of 2^17, each slice its own batch (what a slice packs is exactly what a stand-alone batch packs)."""
+    import bench_workloads as bw
+    from test_gpu_parity import PACK_SWEEP, UNPACK_SWEEP, fill_all_fields, sweep_set
+    orc.set_threads(64)
+    ps, cells, tasks, info = bw.build_clumpy(sph, 3, 1, 1 << 24)
+    oc, ot = cells.view(orc.CELL_DTYPE), tasks.view(orc.TASK_DTYPE)
+    assert info["per_cell_max"] <= 448 and ps.shape[0] == 1 << 24
+    ps = fill_all_fields(ps, 11)
+    step = 1 << 17
+    u_set = sweep_set(UNPACK_SWEEP, 13, 0)
+    for layout in ("split", "aos"):
+        lay = sph.sph_layout_split() if layout == "split" else sph.sph_layout_aos()
+        store = sph.sph_store_create(lay, ps.shape[0])
+        sph.sph_store_import_aos(store, ps)
+        sph.sph_store_set_cells(store, cells)
+        want_store = raw_copy(ps)
+        batches = []
+        for t0 in range(0, tasks.shape[0], step):                                # every pack first: the store is still pristine
+            sel, osel = tasks[t0:t0 + step], ot[t0:t0 + step]
+            batch = sph.sph_batch_create(store, np.ascontiguousarray(sel))
+            batches.append(batch)
+            for k in (5, 13):
+                if layout == "aos" and k == 13 and (t0 // step) % 4:
+                    continue                                                     # AoS, 13 fields: every fourth slice
+                oset = sweep_set(PACK_SWEEP, k, orc.FLAG_X_REL_F32)
+                aset = to_attrset(oset)
+                buf = torch.empty(sph.sph_batch_buffer_bytes(batch, aset), dtype=torch.uint8, device="cuda")
+                sph.sph_pack(store, batch, aset, buf)
+                got = buf.cpu().numpy()
+                want = orc.pack(ps, oc, osel, oset)
+                assert got.shape == want.shape and orc.compare_blocks(oc, osel, 4 * k, got, want) == -1, (layout, k, t0)
+                del buf
+        # then the unpack of seeded result records, slice after slice (ascending task order = the order of the definition)
+        aset = to_attrset(u_set)
+        for n_slice, batch in enumerate(batches):
+            osel = ot[n_slice * step:(n_slice + 1) * step]
+            res = _random_result_buffer(sph.sph_batch_buffer_bytes(batch, aset), 900 + n_slice)
+            sph.sph_unpack(store, batch, aset, torch.from_numpy(res).cuda(), sph.SPH_UNPACK_REDUCE)
+            if layout == "split":
+                orc.unpack(want_store, oc, osel, u_set, res, orc.MODE_REDUCE)
+            sph.sph_batch_destroy(batch)
+        torch.cuda.synchronize()
+        got_store = np.zeros_like(ps)
+        sph.sph_store_export_aos(store, got_store)
+        if layout == "split":
+            _C3_WANT["store"] = want_store
+        assert np.array_equal(canon(got_store), canon(_C3_WANT["store"])), layout
+        sph.sph_store_destroy(store)
+
+
+_C3_WANT = {}
+
+
+# ------------------------------------------------------------------ configs[4]
+
+def test_config4_pipeline_sampled_cells_and_invariants():
+    """2^26 particles through bench.py's configs[4] pipeline (bundles of 4,096 tasks, two streams, host-resident split-AoS store,
+    streamed staging, one graph replay).  1,024 seeded cells are recomputed by the oracle from ALL their tasks: the density
+    cycle over every task that touches a sampled cell or one of its partners (so the partners' rho, P, c_s are complete too),
+    the ghost, the force cycle over every task that touches a sampled cell."""
+    import bench_workloads as bw
+    orc.set_threads(64)
+    ps, cells, tasks, info = bw.build_clumpy(sph, 4, 1, 1 << 26)
+    n_cells, n = int(cells.shape[0]), ps.shape[0]
+    layout = sph.sph_layout_split()
+    hs = bw.HostStore(sph, torch, layout, ps, cells)
+    pl = bw.Pipeline(sph, torch, layout, hs, cells, tasks, n_cells, 4096, "staged")
+    pl.capture().replay()
+    torch.cuda.synchronize()
+    pl.close()
+    got = np.zeros_like(ps)
+    sph.sph_store_export_aos(hs.store, got)
+    hs.close()
+    # invariants on the full output (north_star: total momentum change <= 1e-6 relative)
+    m, a = got["mass"].astype(np.float64), got["a"].astype(np.float64)
+    assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+    en = m * (np.einsum("ij,ij->i", got["v"].astype(np.float64), a) + got["du_dt"])
+    assert abs(en.sum()) <= 1e-6 * np.abs(m * got["du_dt"].astype(np.float64)).sum()
+    # the sample
+    rng = np.random.default_rng(2026)
+    sample = np.zeros(n_cells, dtype=bool)
+    sample[rng.choice(n_cells, 1024, replace=False)] = True
+    ci, cj = tasks["ci"].astype(np.int64), np.where(tasks["cj"] < 0, tasks["ci"], tasks["cj"]).astype(np.int64)
+    touch_s = sample[ci] | sample[cj]
+    ring = sample.copy()
+    ring[ci[touch_s]] = True
+    ring[cj[touch_s]] = True
+    touch_r = ring[ci] | ring[cj]
+    oc = cells.view(orc.CELL_DTYPE)
+    t_dens, t_force = np.ascontiguousarray(tasks[touch_r]).view(orc.TASK_DTYPE), np.ascontiguousarray(tasks[touch_s]).view(orc.TASK_DTYPE)
+    ref = ps                                            # the oracle works in place on the inputs (8.6 GB: no second copy)
+    orc.density_cycle(ref, oc, t_dens)
+    orc.ghost(ref, GAMMA)
+    f_in = orc.pack(ref, oc, t_force, orc.FORCE_IN)
+    exempt = orc.flag_cutoff_pairs(oc, t_force, f_in)
+    orc.force_cycle(ref, oc, t_force)
+    first, count = cells["first"].astype(np.int64), cells["count"].astype(np.int64)
+    idx = np.concatenate([np.arange(first[c], first[c] + count[c]) for c in np.flatnonzero(sample)])
+    assert idx.shape[0] > 100000
+    g, r = got[idx], ref[idx]
+    check_store_physics(g, r, a_scale=float(np.abs(got["a"]).max()), du_scale=float(np.abs(got["du_dt"]).max()))
+    ok = np.abs(g["v_sig"] - r["v_sig"]) <= 1e-4 * r["v_sig"]
+    assert np.all(ok | exempt[idx]) and exempt[idx].mean() < 0.01

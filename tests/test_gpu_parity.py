@@ -194,23 +194,12 @@ def test_density_loop_vs_oracle(name):
 
 def _near_cutoff(ps, cells, tasks, buf_in, rel=1e-5):
     """particles that have a neighbour with |r - R_cut| < rel * R_cut in some task (v_sig is discontinuous there, C31)."""
-    off, _ = orc.block_offsets(cells, tasks, 52)
-    flagged = np.zeros(ps.shape[0], dtype=bool)
-    for t in range(tasks.shape[0]):
-        ci, cj = int(tasks["ci"][t]), int(tasks["cj"][t])
-        ki = int(cells["count"][ci])
-        ri = buf_in[int(off[2 * t]):int(off[2 * t]) + 52 * ki].view(np.float32).reshape(ki, 13).astype(np.float64)
-        if cj < 0:
-            rj, kj, fj = ri, ki, int(cells["first"][ci])
-        else:
-            kj, fj = int(cells["count"][cj]), int(cells["first"][cj])
-            rj = buf_in[int(off[2 * t + 1]):int(off[2 * t + 1]) + 52 * kj].view(np.float32).reshape(kj, 13).astype(np.float64)
-        d = np.sqrt(((ri[:, None, :3] - rj[None, :, :3]) ** 2).sum(-1))
-        cut = 2 * np.maximum(ri[:, None, 3], rj[None, :, 3])
-        near = np.abs(d - cut) < rel * cut
-        flagged[int(cells["first"][ci]):int(cells["first"][ci]) + ki] |= near.any(1)
-        flagged[fj:fj + kj] |= near.any(0)
-    return flagged
+    return orc.flag_cutoff_pairs(cells, tasks, buf_in, rel)
+
+
+def vsig_exempt(ref_after_ghost, cells, tasks, rel=1e-5):
+    """C31 exemption mask of a whole step: the flags of the force loop's inputs as the oracle packs them"""
+    return _near_cutoff(ref_after_ghost, cells, tasks, orc.pack(ref_after_ghost, cells, tasks, orc.FORCE_IN), rel)
 
 
 @pytest.mark.parametrize("name", ["config0", "ragged", "octree", "bigcells", "hugecells"])
@@ -487,7 +476,8 @@ def gpu_step(g, do_force=True, fused_zero=False):
     return g.export()
 
 
-def check_store_physics(got, ref):
+def check_store_physics(got, ref, a_scale=None, du_scale=None):
+    """north_star tolerances on the store; a_scale / du_scale: max |a|, max |du/dt| of the whole set when got / ref are a sample"""
     h = ref["h"].astype(np.float64)
     for name, dname in (("rho", "rho_dh"), ("wcount", "wcount_dh")):
         r, v = ref[name].astype(np.float64), got[name].astype(np.float64)
@@ -496,9 +486,9 @@ def check_store_physics(got, ref):
         assert np.max(np.abs(vd - rd) / np.maximum(np.abs(rd), r / h)) <= 2e-5, dname
     assert np.max(np.abs(got["P"] - ref["P"]) / ref["P"]) <= 2e-5 and np.max(np.abs(got["c_s"] - ref["c_s"]) / ref["c_s"]) <= 1e-6
     a_r, a_g = ref["a"].astype(np.float64), got["a"].astype(np.float64)
-    assert np.all(np.abs(a_g - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * np.abs(a_r).max()))
+    assert np.all(np.abs(a_g - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * (a_scale or np.abs(a_r).max())))
     d_r, d_g = ref["du_dt"].astype(np.float64), got["du_dt"].astype(np.float64)
-    assert np.all(np.abs(d_g - d_r) <= np.maximum(1e-4 * np.abs(d_r), 1e-6 * np.abs(d_r).max()))
+    assert np.all(np.abs(d_g - d_r) <= np.maximum(1e-4 * np.abs(d_r), 1e-6 * (du_scale or np.abs(d_r).max())))
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
@@ -509,12 +499,13 @@ def test_full_step_vs_oracle(name, layout):
     orc.set_threads(8)
     orc.density_cycle(ref, cells, tasks)
     orc.ghost(ref, GAMMA)
+    exempt = vsig_exempt(ref, cells, tasks)
     orc.force_cycle(ref, cells, tasks)
     g = GpuCase(ps, cells, tasks, layout)
     got = gpu_step(g)
     check_store_physics(got, ref)
     vs_ok = np.abs(got["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
-    assert vs_ok.mean() > 0.99
+    assert np.all(vs_ok | exempt) and exempt.mean() < 0.01      # C31: only particles with a partner on the cut-off may differ
     # fields no loop writes are untouched, bit for bit
     for fld in ("x", "v", "mass", "h", "u", "div_v", "rot_v", "id", "time_bin"):
         assert np.array_equal(got[fld], ps[fld]), fld
@@ -523,7 +514,7 @@ def test_full_step_vs_oracle(name, layout):
     a = got["a"].astype(np.float64)
     assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
     en = m * (np.einsum("ij,ij->i", got["v"].astype(np.float64), a) + got["du_dt"])
-    assert abs(en.sum()) <= 1e-5 * np.abs(m * got["du_dt"].astype(np.float64)).sum()
+    assert abs(en.sum()) <= 1e-6 * np.abs(m * got["du_dt"].astype(np.float64)).sum()
     g.close()
 
 

@@ -1,0 +1,102 @@
+"""The configs[4] offload pipeline of bench.py (bench_workloads.Pipeline: bundles of 4,096 tasks over two streams, host-resident
+store, streamed staging, one CUDA graph per step) against the oracle and against a plain one-stream run (needs a B200).
+
+PAPER.md:76-82 (section 2.3: pack / launch / unpack per bundle), PAPER.md:98 (asynchronous memory streams); SURVEY.md 8(d)
+"Parity at scale".  Three things are checked on a 2^19-particle instance of the configs[4] generator (6,000 octree leaves,
+~25 bundles, every stream / event / slab path of the full-size run):
+  * the pipeline's final HOST store equals, bit for bit, what the same kernels give when the bundles run one after the other
+    on one stream against a device store (so the cross-stream unpack chain, the slab-wise uploads and the downloads behind
+    the bundle frontier lose or reorder nothing);
+  * that result is within the north_star tolerances of the oracle's density cycle, ghost, force cycle over the same tasks;
+  * momentum and energy invariants on the pipeline's output.
+"""
+import numpy as np
+import pytest
+import torch
+
+import bench_workloads as bw
+import oracle as orc
+import paper_2606_23891_b200 as sph
+from gpu_setup import GAMMA, PARAMS, canon
+from orc_setup import raw_copy
+from test_gpu_parity import check_store_physics, vsig_exempt
+
+pytestmark = pytest.mark.gpu
+
+_CASE = {}
+
+
+def small_config4():
+    if not _CASE:
+        ps, cells, tasks, info = bw.build_clumpy(sph, 4, 7, 1 << 19)
+        ref = raw_copy(ps)
+        orc.set_threads(64)
+        oc, ot = cells.view(orc.CELL_DTYPE), tasks.view(orc.TASK_DTYPE)
+        orc.density_cycle(ref, oc, ot, batch=4096)
+        orc.ghost(ref, GAMMA)
+        exempt = vsig_exempt(ref, oc, ot)
+        orc.force_cycle(ref, oc, ot, batch=4096)
+        _CASE.update(ps=ps, cells=cells, tasks=tasks, ref=ref, exempt=exempt, info=info)
+    return _CASE
+
+
+def one_stream_reference(layout, ps, cells, tasks, n_self, bundle):
+    """the same bundles, one after the other on the current stream, store in HBM"""
+    store = sph.sph_store_create(layout, ps.shape[0])
+    sph.sph_store_import_aos(store, ps)
+    sph.sph_store_set_cells(store, cells)
+    sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+    batches = []
+    for lo, hi in ((0, n_self), (n_self, tasks.shape[0])):
+        for s in range(lo, hi, bundle):
+            batches.append(sph.sph_batch_create(store, tasks[s:min(hi, s + bundle)]))
+    for k_in, k_out, loop in ((0, 1, lambda b, i, o: sph.sph_density(b, i, o)), (2, 3, lambda b, i, o: sph.sph_force(b, i, o, PARAMS))):
+        sph.sph_store_zero(store, sets[k_out])
+        for b in batches:
+            b_in = torch.empty(sph.sph_batch_buffer_bytes(b, sets[k_in]), dtype=torch.uint8, device="cuda")
+            b_out = torch.empty(sph.sph_batch_buffer_bytes(b, sets[k_out]), dtype=torch.uint8, device="cuda")
+            sph.sph_pack(store, b, sets[k_in], b_in)
+            loop(b, b_in, b_out)
+            sph.sph_unpack(store, b, sets[k_out], b_out, sph.SPH_UNPACK_REDUCE)
+        if k_in == 0:
+            sph.sph_ghost(store, PARAMS)
+    torch.cuda.synchronize()
+    out = np.zeros_like(ps)
+    sph.sph_store_export_aos(store, out)
+    for b in batches:
+        sph.sph_batch_destroy(b)
+    sph.sph_store_destroy(store)
+    return out
+
+
+@pytest.mark.parametrize("mode", ["staged", "zero-copy"])
+@pytest.mark.parametrize("layout_name", ["split", "aos"])
+def test_pipeline_equals_one_stream_run_and_oracle(layout_name, mode):
+    c = small_config4()
+    ps, cells, tasks, ref = c["ps"], c["cells"], c["tasks"], c["ref"]
+    n_self = int(cells.shape[0])
+    layout = sph.sph_layout_split() if layout_name == "split" else sph.sph_layout_aos()
+    hs = bw.HostStore(sph, torch, layout, ps, cells)
+    pl = bw.Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, mode)
+    assert len(pl.batches) >= 8 and pl.n_self_bundles >= 2
+    graph = pl.capture()                      # runs the step once outside the graph, then captures it
+    for _ in range(2):                        # a replayed step starts from whatever the previous one left in the stores
+        graph.replay()
+    torch.cuda.synchronize()
+    got = np.zeros_like(ps)
+    sph.sph_store_export_aos(hs.store, got)
+    want = one_stream_reference(layout, ps, cells, tasks, n_self, 4096)
+    assert np.array_equal(canon(got), canon(want))
+    check_store_physics(got, ref)
+    ok = np.abs(got["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
+    assert np.all(ok | c["exempt"]) and c["exempt"].mean() < 0.01
+    m, a = got["mass"].astype(np.float64), got["a"].astype(np.float64)
+    assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+    en = m * (np.einsum("ij,ij->i", got["v"].astype(np.float64), a) + got["du_dt"])
+    assert abs(en.sum()) <= 1e-6 * np.abs(m * got["du_dt"].astype(np.float64)).sum()
+    if mode == "staged":
+        n = ps.shape[0]
+        assert pl.h2d_bytes == (n * (32 + 24) if layout_name == "split" else n * 128)
+        assert pl.d2h_bytes == (n * (16 + 20 + 24) if layout_name == "split" else n * 128)
+    pl.close()
+    hs.close()

@@ -615,3 +615,149 @@ def test_h_iteration_on_lattice():
     orc.density_cycle(ps, cells, tasks)
     nngb = 4.0 / 3.0 * math.pi * (2.0 * ps["h"].astype(np.float64)) ** 3 * ps["wcount"]
     assert np.allclose(nngb, 48.0, atol=1e-3)
+
+
+# ------------------------------------------------------------------ gradient loop and Balsara switch (reading C34, row f2)
+
+def _gold_omega(h_over_dx):
+    for row in _gold_rows():
+        if abs(row[0] - h_over_dx) < 1e-12:
+            rho_n, rho_dh_n = row[2], row[3]              # rho dx^3 / m and rho_dh dx^4 / m
+            return 1.0 + h_over_dx * rho_dh_n / (3.0 * rho_n)
+    raise KeyError(h_over_dx)
+
+
+def _velocity_field(parts, A, box=1.0):
+    """v = A (x - centre), kept linear across the periodic wrap by using only particles far from the box faces in the checks"""
+    parts["v"] = ((parts["x"] - 0.5) @ np.asarray(A, dtype=np.float64).T).astype(np.float32)
+    return parts
+
+
+@pytest.mark.parametrize("h_over_dx", [1.2348, 1.0, 1.5])
+def test_gradient_of_a_linear_field_on_a_lattice(h_over_dx):
+    # For v = A x on an unperturbed lattice the estimator gives A's trace (divergence) and antisymmetric part (curl) times
+    # S = -(1/3) sum_j (m_j / rho_j) r dW/dr.  Because dW/dh = -(3 W + r dW/dr) / h, S = 1 + h rho_dh / (3 rho) = Omega: the grad-h
+    # factor of the SAME lattice, whose value comes from the independent lattice sums of tests/golden/ (0.981238565203 at 1.2348).
+    n_side = 16
+    omega_l = _gold_omega(h_over_dx)
+    A = np.array([[0.3, -0.2, 0.5], [0.7, -0.1, 0.05], [-0.4, 0.6, 0.9]])
+    parts = _velocity_field(lattice(n_side, h_over_dx), A)
+    ps, cells, tasks, _, _ = sort_grid(parts, 4)
+    orc.density_cycle(ps, cells, tasks)
+    orc.gradient_cycle(ps, cells, tasks)
+    inner = np.all(np.abs(ps["x"] - 0.5) < 0.5 - 2.1 * h_over_dx / n_side, axis=1)      # the field is linear inside their support
+    assert inner.sum() > 500
+    curl = np.array([A[2, 1] - A[1, 2], A[0, 2] - A[2, 0], A[1, 0] - A[0, 1]])
+    assert np.allclose(ps["div_v"][inner], np.trace(A) * omega_l, rtol=0, atol=3e-6)
+    assert np.allclose(ps["rot_v"][inner], curl * omega_l, rtol=0, atol=3e-6)
+    # a transposed operand (A^T gives -curl), a wrong sign of e or dv, or rho_i instead of rho_j would all show:
+    # rigid rotation about z: div = 0, rot = 2 w z; pure strain: rot = 0
+    w = 0.37
+    parts = _velocity_field(lattice(n_side, h_over_dx), [[0, -w, 0], [w, 0, 0], [0, 0, 0]])
+    ps, cells, tasks, _, _ = sort_grid(parts, 4)
+    orc.density_cycle(ps, cells, tasks)
+    orc.gradient_cycle(ps, cells, tasks)
+    assert np.allclose(ps["rot_v"][inner], np.array([0, 0, 2 * w]) * omega_l, atol=3e-6) and np.allclose(ps["div_v"][inner], 0, atol=3e-6)
+    parts = _velocity_field(lattice(n_side, h_over_dx), [[0.5, 0.2, 0], [0.2, -0.5, 0.1], [0, 0.1, 0]])
+    ps, cells, tasks, _, _ = sort_grid(parts, 4)
+    orc.density_cycle(ps, cells, tasks)
+    orc.gradient_cycle(ps, cells, tasks)
+    assert np.allclose(ps["rot_v"][inner], 0, atol=3e-6) and np.allclose(ps["div_v"][inner], 0, atol=3e-6)
+
+
+def test_gradient_uses_the_neighbours_volume_and_the_targets_h():
+    # two isolated particles, hand-worked: i at the origin (h_i = 0.1), j at distance 0.05 along x (h_j = 0.3 must not matter for i)
+    parts = np.zeros(2, dtype=si.PART_DTYPE)
+    parts["x"] = [[0.40, 0.5, 0.5], [0.45, 0.5, 0.5]]
+    parts["h"], parts["mass"], parts["rho"], parts["u"] = [0.1, 0.3], [2.0, 3.0], [5.0, 7.0], 1.0
+    parts["v"] = [[0.0, 0.0, 0.0], [0.2, 0.6, -0.4]]
+    parts["id"] = [0, 1]
+    cells = np.zeros(1, dtype=orc.CELL_DTYPE)
+    cells["count"], cells["width"] = 2, 1.0
+    tasks = np.zeros(1, dtype=orc.TASK_DTYPE)
+    tasks["cj"] = -1
+    out = orc.gradient(cells, tasks, orc.pack(parts, cells, tasks, orc.GRADIENT_IN)).view(np.float32)[:8].reshape(2, 4)
+    # i: q = 0.5, w'(0.5) = -0.9375, dW/dr = w' / (pi h^4); e = (x_i - x_j) / r = (-1, 0, 0); dv = v_j - v_i
+    g = 3.0 / 7.0 * (-0.9375) / (math.pi * 0.1 ** 4)
+    assert np.allclose(out[0], [g * (-0.2), 0.0, g * (-0.4), g * (-0.6)], rtol=1e-6)       # e x dv = (0, dvz, -dvy) for e = -x
+    # j: h_j = 0.3, q = 1/6 < 1: w' = -3q + 2.25 q^2; neighbour's volume m_i / rho_i; e = (+1, 0, 0); dv = v_i - v_j
+    q = 0.05 / 0.3
+    g = 2.0 / 5.0 * (-3 * q + 2.25 * q * q) / (math.pi * 0.3 ** 4)
+    assert np.allclose(out[1], [g * (-0.2), 0.0, g * (-0.4), g * (-0.6)], rtol=1e-6)      # e = +x, dv = -v_j: e x dv = (0, -dvz, dvy)
+
+
+def test_gradient_pipeline_vs_brute_force():
+    parts = si.jittered_lattice(12, 9, jitter=0.5, sigma_v=0.2, h_spread=0.15, mass_spread=0.3)
+    ps, cells, tasks, _, _ = sort_grid(parts, 4)
+    orc.density_cycle(ps, cells, tasks)
+    orc.gradient_cycle(ps, cells, tasks, batch=31)
+    ref = orc.brute_gradient(ps)
+    scale = np.abs(ref).max()
+    assert np.max(np.abs(ps["div_v"] - ref[:, 0])) < 5e-6 * scale and np.max(np.abs(ps["rot_v"] - ref[:, 1:])) < 5e-6 * scale
+    assert np.abs(ps["div_v"]).max() > 0.1 and np.abs(ps["rot_v"]).max() > 0.1
+
+
+def _three_loop_state(seed):
+    parts = si.jittered_lattice(12, seed, jitter=0.5, sigma_v=0.3, h_spread=0.15, mass_spread=0.3, u_spread=0.3)
+    ps, cells, tasks, _, _ = sort_grid(parts, 4)
+    orc.density_cycle(ps, cells, tasks)
+    orc.ghost(ps, GAMMA)
+    return ps, cells, tasks
+
+
+def test_balsara_switch_limits():
+    ps, cells, tasks = _three_loop_state(21)
+    plain = raw_copy(ps)
+    orc.force_cycle(plain, cells, tasks)
+    off = raw_copy(ps)
+    orc.force_cycle(off, cells, tasks, alpha=0.0)
+    assert np.abs(plain["a"] - off["a"]).max() > 1e-3 * np.abs(plain["a"]).max()         # the viscosity matters in this state
+    # pure compression (rot v = 0, |div v| overwhelming the c_s / h floor): B = 1 exactly, the three-loop force IS the plain force
+    comp = raw_copy(ps)
+    comp["div_v"], comp["rot_v"] = -1.0e30, 0.0
+    orc.force3_cycle(comp, cells, tasks)
+    for k in ("a", "du_dt", "v_sig"):
+        assert np.array_equal(comp[k], plain[k]), k
+    # pure shear (div v = 0): B = 0, the viscous term vanishes -- the plain force with alpha = 0 (v_sig is not switched)
+    shear = raw_copy(ps)
+    shear["div_v"], shear["rot_v"] = 0.0, [[0.3, -2.0, 1.0]]
+    orc.force3_cycle(shear, cells, tasks)
+    assert np.array_equal(shear["a"], off["a"]) and np.array_equal(shear["du_dt"], off["du_dt"]) and np.array_equal(shear["v_sig"], plain["v_sig"])
+    # B = 1/2 everywhere (|div| = |rot|, floor negligible): exactly the plain force at half the alpha
+    half = raw_copy(ps)
+    half["div_v"], half["rot_v"] = 2.0e20, [[0.0, 2.0e20, 0.0]]
+    orc.force3_cycle(half, cells, tasks)
+    ref = raw_copy(ps)
+    orc.force_cycle(ref, cells, tasks, alpha=0.4)
+    assert np.allclose(half["a"], ref["a"], rtol=1e-6, atol=1e-6 * np.abs(ref["a"]).max())
+
+
+def test_three_loop_step_conserves_momentum_and_energy():
+    ps, cells, tasks = _three_loop_state(22)
+    orc.gradient_cycle(ps, cells, tasks)
+    orc.force3_cycle(ps, cells, tasks)
+    B = np.abs(ps["div_v"]) / (np.abs(ps["div_v"]) + np.linalg.norm(ps["rot_v"], axis=1) + 1e-4 * ps["c_s"] / ps["h"])
+    assert B.min() < 0.2 and 0.8 < B.max() <= 1.0 and 0.2 < B.std()                        # the switch really varies from particle to particle
+    m, a = ps["mass"].astype(np.float64), ps["a"].astype(np.float64)
+    assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+    en = m * (np.einsum("ij,ij->i", ps["v"].astype(np.float64), a) + ps["du_dt"])
+    assert abs(en.sum()) <= 1e-6 * np.abs(m * ps["du_dt"].astype(np.float64)).sum()
+
+
+def test_three_loop_record_layouts():
+    # Table 1 (PAPER.md:47-58): p-g = x, v, mass, h, u, rho; p-f adds time_bin
+    assert orc.record_bytes(orc.GRADIENT_IN) == 40 and orc.record_bytes(orc.GRADIENT_OUT) == 16 and orc.record_bytes(orc.FORCE3_IN) == 72
+    parts = _pattern_store(6)
+    cells, tasks = _one_cell_setup(6)
+    rec = orc.pack(parts, cells, tasks, orc.FORCE3_IN)[:72].view(np.float32)
+    f = {name: i for i, name in enumerate(si.FIELDS)}
+    assert rec[3] == f["h"] * 10 and rec[13] == f["div_v"] * 10 and list(rec[14:17]) == [f["rot_v"] * 10 + c for c in range(3)]
+    assert rec[17:18].view(np.uint32)[0] == 0                                              # time_bin of particle 0: one byte, zero-extended
+    # div_v and rot_v are neighbour sums: REDUCE adds them up over the tasks
+    buf = np.zeros(orc.block_offsets(cells, tasks, 16)[1], dtype=np.uint8)
+    off, _ = orc.block_offsets(cells, tasks, 16)
+    for t, side in ((0, 0), (2, 0)):
+        buf[int(off[2 * t + side]):int(off[2 * t + side]) + 16 * 3].view(np.float32)[:] = 1.5
+    p2 = np.zeros(6, dtype=si.PART_DTYPE)
+    orc.unpack(p2, cells, tasks, orc.GRADIENT_OUT, buf, orc.MODE_REDUCE)
+    assert np.all(p2["div_v"][:3] == 3.0) and np.all(p2["rot_v"][:3] == 3.0) and np.all(p2["div_v"][3:] == 0)
