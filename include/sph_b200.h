@@ -86,7 +86,11 @@ typedef struct {
 enum { SPH_SET_DENSITY_IN = 0,  /* [X(rel f32), H, MASS]                        20-byte record */
        SPH_SET_DENSITY_OUT = 1, /* [RHO, RHO_DH, WCOUNT, WCOUNT_DH]             16 */
        SPH_SET_FORCE_IN = 2,    /* [X(rel), H, MASS, RHO, RHO_DH, V, U, P, CS]  52 */
-       SPH_SET_FORCE_OUT = 3 }; /* [A, DU_DT, V_SIG]                            20 */
+       SPH_SET_FORCE_OUT = 3,   /* [A, DU_DT, V_SIG]                            20 */
+       /* the three-loop (Sphenix-like) cycle, PAPER.md:41 and Table 1 columns p-g / p-f (reading C34) */
+       SPH_SET_GRADIENT_IN = 4, /* [X(rel), V, MASS, H, U, RHO]                 40 */
+       SPH_SET_GRADIENT_OUT = 5,/* [DIV_V, ROT_V]                               16 */
+       SPH_SET_FORCE3_IN = 6 }; /* FORCE_IN + [DIV_V, ROT_V, TIME_BIN]          72 */
 
 typedef struct { uint64_t first; uint32_t count; uint32_t pad; double origin[3]; double width; } sph_cell;   /* 48 B */
 typedef struct { int32_t ci, cj; double frame_i[3]; double frame_j[3]; } sph_task;                           /* 56 B */
@@ -209,6 +213,14 @@ int32_t sph_density(const sph_batch* batch, const void* d_in, uint64_t in_bytes,
  * signal velocity with grad-h terms and Monaghan viscosity. */
 int32_t sph_force(const sph_batch* batch, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes,
                   const sph_params* params, void* stream);
+/* GRADIENT LOOP ("a third gradient loop between the density and the force loops"; reading C34):
+ * d_in = GRADIENT_IN buffer, d_out = GRADIENT_OUT buffer.  Per instance i over j != i with r < 2 h_i:
+ * g = (m_j / rho_j) dW/dr(r, h_i), e = (x_i - x_j) / r, dv = v_j - v_i:  div_v += g (dv . e), rot_v += g (e x dv). */
+int32_t sph_gradient(const sph_batch* batch, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, void* stream);
+/* FORCE LOOP of the three-loop cycle: d_in = FORCE3_IN buffer, d_out = FORCE_OUT buffer; sph_force with the viscous term scaled
+ * by (B_i + B_j) / 2, B = |div v| / (|div v| + |rot v| + 1e-4 c_s / h) (Balsara-type switch, reading C34). */
+int32_t sph_force3(const sph_batch* batch, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes,
+                   const sph_params* params, void* stream);
 /* UNPACK: reduce / scatter the records of d_buf [device] into the store, mode = SPH_UNPACK_*.
  * X with X_REL_F32 cannot be unpacked (SPH_ERR_UNSUPPORTED). */
 int32_t sph_unpack(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,

@@ -20,7 +20,8 @@ __all__ = [
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
     "sph_store_upload_range", "sph_store_download_range",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
-    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_unpack", "sph_unpack_cells", "sph_ghost",
+    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack",
+    "sph_unpack_cells", "sph_ghost", "SPH_SET_GRADIENT_IN", "SPH_SET_GRADIENT_OUT", "SPH_SET_FORCE3_IN",
 ]
 
 SPH_NFIELDS, SPH_MAX_SUB, SPH_MAX_ATTR = 18, 8, 32
@@ -31,6 +32,7 @@ SPH_ATTR_X_REL_F32 = 1
 SPH_MEM_DEVICE, SPH_MEM_HOST_PINNED = 0, 1
 SPH_UNPACK_REDUCE, SPH_UNPACK_ASSIGN, SPH_UNPACK_REDUCE_ZERO = 0, 1, 2
 SPH_SET_DENSITY_IN, SPH_SET_DENSITY_OUT, SPH_SET_FORCE_IN, SPH_SET_FORCE_OUT = 0, 1, 2, 3
+SPH_SET_GRADIENT_IN, SPH_SET_GRADIENT_OUT, SPH_SET_FORCE3_IN = 4, 5, 6
 
 #: every symbol include/sph_b200.h declares
 EXPORTS = [
@@ -39,7 +41,7 @@ EXPORTS = [
     "sph_store_export_aos", "sph_store_set_cells", "sph_store_sub_ptr", "sph_store_upload_sub", "sph_store_download_sub",
     "sph_store_upload_range", "sph_store_download_range", "sph_pack_cells", "sph_unpack_cells",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_free", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
-    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_unpack", "sph_ghost",
+    "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack", "sph_ghost",
 ]
 
 
@@ -332,6 +334,15 @@ def sph_density(batch, d_in, d_out, stream=None) -> None:
 def sph_force(batch, d_in, d_out, params: sph_params, stream=None) -> None:
     _check(_lib.sph_force(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)),
                           C.byref(params), _stream(stream)))
+
+
+def sph_gradient(batch, d_in, d_out, stream=None) -> None:
+    _check(_lib.sph_gradient(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)), _stream(stream)))
+
+
+def sph_force3(batch, d_in, d_out, params: sph_params, stream=None) -> None:
+    _check(_lib.sph_force3(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)),
+                           C.byref(params), _stream(stream)))
 
 
 def sph_unpack(store, batch, aset: sph_attrset, d_buf, mode: int = SPH_UNPACK_REDUCE, stream=None) -> None:

@@ -291,6 +291,16 @@ int32_t sph_attrset_canonical(int32_t which, sph_attrset* out) {
             add(SPH_X); add(SPH_H); add(SPH_MASS); add(SPH_RHO); add(SPH_RHO_DH); add(SPH_V); add(SPH_U); add(SPH_P); add(SPH_CS);
             break;
         case SPH_SET_FORCE_OUT: add(SPH_A); add(SPH_DU_DT); add(SPH_V_SIG); break;
+        case SPH_SET_GRADIENT_IN:
+            out->flags = SPH_ATTR_X_REL_F32;
+            add(SPH_X); add(SPH_V); add(SPH_MASS); add(SPH_H); add(SPH_U); add(SPH_RHO);
+            break;
+        case SPH_SET_GRADIENT_OUT: add(SPH_DIV_V); add(SPH_ROT_V); break;
+        case SPH_SET_FORCE3_IN:
+            out->flags = SPH_ATTR_X_REL_F32;
+            add(SPH_X); add(SPH_H); add(SPH_MASS); add(SPH_RHO); add(SPH_RHO_DH); add(SPH_V); add(SPH_U); add(SPH_P); add(SPH_CS);
+            add(SPH_DIV_V); add(SPH_ROT_V); add(SPH_TIME_BIN);
+            break;
         default: return fail(SPH_ERR_INVALID_ARG, "unknown canonical attribute set %d", which);
     }
     return SPH_OK;
@@ -590,6 +600,23 @@ int32_t sph_force(const sph_batch* b, const void* d_in, uint64_t in_bytes, void*
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 52, 20, &oin, &oout)) return rc;
     return launch_force(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    SPH_API_END
+}
+
+int32_t sph_gradient(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, void* stream) {
+    SPH_API_BEGIN
+    const OffsetTable *oin = nullptr, *oout = nullptr;
+    if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 40, 16, &oin, &oout)) return rc;
+    return launch_gradient(b, (const char*)d_in, (char*)d_out, (cudaStream_t)stream);
+    SPH_API_END
+}
+
+int32_t sph_force3(const sph_batch* b, const void* d_in, uint64_t in_bytes, void* d_out, uint64_t out_bytes, const sph_params* prm, void* stream) {
+    if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
+    SPH_API_BEGIN
+    const OffsetTable *oin = nullptr, *oout = nullptr;
+    if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 72, 20, &oin, &oout)) return rc;
+    return launch_force3(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
     SPH_API_END
 }
 

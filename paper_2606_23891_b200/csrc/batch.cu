@@ -133,7 +133,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     std::vector<double> occ_frames(3 * (size_t)b->n_sides);
     for (uint32_t o = 0; o < b->n_sides; ++o) std::copy_n(&frames[3 * (size_t)occ_side[o]], 3, &occ_frames[3 * (size_t)o]);
     if (int32_t rc = upload(occ_frames, &b->d_occ_frames)) return rc;
-    for (uint32_t rec : {16u, 20u, 52u})
+    for (uint32_t rec : {16u, 20u, 52u, 40u, 72u})
         if (int32_t rc = ensure_offsets(b, rec, nullptr)) return rc;
 
     // loop work items (one per 64-target chunk of a block) for the canonical record sizes of the two loops, cell-major: the
@@ -141,7 +141,8 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     // its blocks are still in L2
     {
         const std::vector<uint64_t> &o16 = b->offsets.at(16).h_off, &o20 = b->offsets.at(20).h_off, &o52 = b->offsets.at(52).h_off;
-        std::vector<LoopItem> dens, forc;
+        const std::vector<uint64_t> &o40 = b->offsets.at(40).h_off, &o72 = b->offsets.at(72).h_off;
+        std::vector<LoopItem> dens, forc, grad, forc3;
         for (uint32_t c = 0; c < n_cells; ++c)
             for (uint32_t o = occ_start[c]; o < occ_start[c + 1]; ++o) {
                 const uint32_t tgt = occ_side[o], src = partner[tgt];
@@ -151,11 +152,15 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
                     const uint32_t u = kLoopTargets / 32;                                // 32 records of r bytes = r units of 128 bytes
                     dens.push_back(LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5 * u, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns});
                     forc.push_back(LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13 * u, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns});
+                    grad.push_back(LoopItem{(uint32_t)(o40[tgt] / 128) + kc * 10 * u, (uint32_t)(o40[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns});
+                    forc3.push_back(LoopItem{(uint32_t)(o72[tgt] / 128) + kc * 18 * u, (uint32_t)(o72[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns});
                 }
             }
         b->n_items = (uint32_t)dens.size();
         if (int32_t rc = upload(dens, &b->d_items_density)) return rc;
         if (int32_t rc = upload(forc, &b->d_items_force)) return rc;
+        if (int32_t rc = upload(grad, &b->d_items_gradient)) return rc;
+        if (int32_t rc = upload(forc3, &b->d_items_force3)) return rc;
     }
 
     *out = holder.release();
@@ -165,7 +170,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
 
 int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
-    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force);
+    cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force); cudaFree(b->d_items_gradient); cudaFree(b->d_items_force3);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
     delete b;
     return SPH_OK;

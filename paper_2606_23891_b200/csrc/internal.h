@@ -152,6 +152,8 @@ struct sph_batch {
     sph::CellChunk* d_cell_chunks = nullptr;
     sph::LoopItem* d_items_density = nullptr; // one per 64-target chunk of a block (20-byte in, 16-byte out records)
     sph::LoopItem* d_items_force = nullptr;   // (52-byte in, 20-byte out records)
+    sph::LoopItem* d_items_gradient = nullptr;   // three-loop cycle: 40-byte in, 16-byte out records
+    sph::LoopItem* d_items_force3 = nullptr;     //                   72-byte in, 20-byte out records
     uint32_t n_items = 0;                     // items are cell-major: the chunks of a cell's occurrences follow one another
     // block offsets by record bytes: the only part that grows after sph_batch_create (a table is built the first time a
     // record size is asked for, under the mutex; tables are never removed, so pointers to them stay valid)
@@ -171,6 +173,8 @@ int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& 
                       bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
+int32_t launch_gradient(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
+int32_t launch_force3(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);
 int32_t launch_ghost(const StoreView& view, uint64_t n, const sph_layout& layout, const sph_params& prm, cudaStream_t st);
 }  // namespace sph

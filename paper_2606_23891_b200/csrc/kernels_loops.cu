@@ -354,9 +354,176 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
     }
 }
 
+// ------------------------------------------------------------------------------------------------- gradient
+//
+// The third loop of the Sphenix-like cycle (reading C34): velocity divergence and curl with the
+// volume-weighted estimators, for instance i over j != i with r < 2 h_i:
+//   g = (m_j / rho_j) dW/dr(r, h_i),  e = (x_i - x_j) / r,  dv = v_j - v_i,  div_v += g (dv . e),  rot_v += g (e x dv).
+// Same shape as the density loop (one-sided cut-off 2 h_i, four sums per target), another hit body and wider records:
+// GRADIENT_IN = [xr0 xr1 xr2 v0 v1 v2 mass h u rho] (40 bytes), GRADIENT_OUT = [div_v rot_v0 rot_v1 rot_v2] (16 bytes).
+struct GradientWarpSmem {
+    FilterTile f;
+    float4 tile[2 * kHalf];  // x, y, z, m / rho of the compacted sources; entries 32 and 65 are the dummy
+    float4 tilev[2 * kHalf]; // their vx, vy, vz
+    float4 tgt[64];          // the item's targets: x, y, z, h
+    float4 tgv[64];          //                     vx, vy, vz
+    float4 acc[64];          // their running sums: div, rot (3), before the 1 / (pi h^4)
+    float raw[64 * 10];      // landing area of an item's 64 GRADIENT_IN records
+    float src[2][32 * 10];   // landing areas of the source rounds (double-buffered)
+    uint32_t act[64];        // the active targets of the flush
+};
+
+__global__ void __launch_bounds__(kLoopWarps * 32, 3)
+gradient_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items) {
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    GradientWarpSmem& sm = reinterpret_cast<GradientWarpSmem*>(s_raw)[warp];
+    const uint32_t lt = lanemask_lt();
+    const uint32_t step = gridDim.x * kLoopWarps;
+    uint32_t item = blockIdx.x * kLoopWarps + warp;
+    if (item >= n_items) return;
+    if (lane < 2) { sm.tile[lane * kHalf + 32] = make_float4(kFar, kFar, kFar, 0.f); sm.tilev[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f); }
+    const u64 kTwo = dup2(2.0f), kOne = dup2(1.0f), kThree = dup2(3.0f), kM075 = dup2(-0.75f);
+
+    uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
+    fetch_records<10, 64>(sm.raw, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
+    fetch_records<10, 32>(sm.src[0], in + (uint64_t)iw.y * 128, min(32u, iw.w >> 7), lane);
+    uint32_t buf = 0;
+
+    for (; item < n_items; item += step) {
+        const uint32_t n_t = iw.w & 127u, n_s = iw.w >> 7;
+        const char* sin = in + (uint64_t)iw.y * 128;
+        char* tout = out + (uint64_t)iw.z * 128;
+        const bool has_next = item + step < n_items;
+        uint4 iw_next = iw;
+        if (has_next) iw_next = __ldg(reinterpret_cast<const uint4*>(items) + item + step);
+        cp_async_wait_all();          // this item's targets and first source round
+        __syncwarp();
+        const bool vA = lane < n_t, vB = lane + 32 < n_t;
+        float4 oA = make_float4(0.f, 0.f, 0.f, 0.f), oB = oA, wA4 = oA, wB4 = oA;
+        if (vA) { const float* r = sm.raw + 10 * lane; oA = make_float4(r[0], r[1], r[2], r[7]); wA4 = make_float4(r[3], r[4], r[5], 0.f); }
+        if (vB) { const float* r = sm.raw + 10 * (lane + 32); oB = make_float4(r[0], r[1], r[2], r[7]); wB4 = make_float4(r[3], r[4], r[5], 0.f); }
+        sm.tgt[lane] = oA; sm.tgt[lane + 32] = oB; sm.tgv[lane] = wA4; sm.tgv[lane + 32] = wB4;
+        sm.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f); sm.acc[lane + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncwarp();                 // sm.raw may now receive the next item's targets
+        const float reach = 2.0f * warp_max_pos(fmaxf(oA.w, oB.w)) * kReachSlack;
+        const float lox = warp_min(vB ? fminf(oA.x, oB.x) : oA.x, vA) - reach, hix = warp_max(vB ? fmaxf(oA.x, oB.x) : oA.x, vA) + reach;
+        const float loy = warp_min(vB ? fminf(oA.y, oB.y) : oA.y, vA) - reach, hiy = warp_max(vB ? fmaxf(oA.y, oB.y) : oA.y, vA) + reach;
+        const float loz = warp_min(vB ? fminf(oA.z, oB.z) : oA.z, vA) - reach, hiz = warp_max(vB ? fmaxf(oA.z, oB.z) : oA.z, vA) + reach;
+        const float bx = fmaxf(fabsf(lox), fabsf(hix)), by = fmaxf(fabsf(loy), fabsf(hiy)), bz = fmaxf(fabsf(loz), fabsf(hiz));
+        const float eps = kFilterEps * fmaf(bx, bx, fmaf(by, by, bz * bz));
+        const float cutA = 4.0f * oA.w * oA.w, cutB = 4.0f * oB.w * oB.w;
+
+        auto flush = [&](uint32_t cnt) {
+            const Box box = tile_box(sm.f, cnt, lane);
+            const bool aA = vA && box_dist2(box, oA.x, oA.y, oA.z) < cutA * kReachSlack, aB = vB && box_dist2(box, oB.x, oB.y, oB.z) < cutB * kReachSlack;
+            const uint32_t n_act = compact_targets(sm.act, aA, aB, lane, lt);
+            if (n_act == 0) return;
+            const bool dual = n_act > 32;
+            const bool wA = lane < n_act, wB = dual && lane + 32 < n_act;
+            const uint32_t tA = wA ? sm.act[lane] : 0, tB = wB ? sm.act[lane + 32] : tA;
+            const float4 pA = sm.tgt[tA], pB = sm.tgt[tB], qA = sm.tgv[tA], qB = sm.tgv[tB];
+            const float inv_hA = wA ? rcp_fast(pA.w) : 0.f, inv_hB = dual ? (wB ? rcp_fast(pB.w) : 0.f) : inv_hA;
+            const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - 4.0f * pA.w * pA.w - eps : kNever);
+            const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - 4.0f * pB.w * pB.w - eps : kNever);
+            uint32_t m[4];
+            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
+            const u64 vx2 = pack2(qA.x, qB.x), vy2 = pack2(qA.y, qB.y), vz2 = pack2(qA.z, qB.z), ih2 = pack2(inv_hA, inv_hB);
+            u64 s_d = 0, s_x = 0, s_y = 0, s_z = 0;
+            auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
+                uint32_t ja, jb;
+                while (next_hits(dual, ma, mb, &ja, &jb)) {
+                    const float4 a = sm.tile[base + ja], b = sm.tile[base + jb], va = sm.tilev[base + ja], vb = sm.tilev[base + jb];
+                    // d = x_i - x_j; e = d / r; dv = v_j - v_i
+                    const u64 dx = sub2(x2, pack2(a.x, b.x)), dy = sub2(y2, pack2(a.y, b.y)), dz = sub2(z2, pack2(a.z, b.z));
+                    const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                    float r2a, r2b;
+                    unpack2(r2, r2a, r2b);
+                    // r = 0 is the particle itself (d = 0: every term vanishes); the floor keeps 1 / r finite
+                    const u64 rinv = pack2(rsqrtf(fmaxf(r2a, 1.0e-30f)), rsqrtf(fmaxf(r2b, 1.0e-30f)));
+                    const u64 r = mul2(r2, rinv);
+                    // q >= 2 (a filter false positive, the dummy): w' = 0 exactly
+                    float qa, qb;
+                    unpack2(mul2(r, ih2), qa, qb);
+                    const u64 q = pack2(fminf(qa, 2.0f), fminf(qb, 2.0f));
+                    float ta, tb, ua, ub;
+                    unpack2(sub2(kTwo, q), ta, tb);
+                    unpack2(sub2(kOne, q), ua, ub);
+                    const u64 t = pack2(ta, tb), u = pack2(fmaxf(ua, 0.f), fmaxf(ub, 0.f));
+                    const u64 dw = fma2(kThree, mul2(u, u), mul2(kM075, mul2(t, t)));      // -0.75 (2 - q)^2 + 3 (1 - q)+^2
+                    const u64 g = mul2(mul2(pack2(a.w, b.w), dw), rinv);                    // (m_j / rho_j) w'(q) / r: e = d / r folded in
+                    const u64 wx = sub2(pack2(va.x, vb.x), vx2), wy = sub2(pack2(va.y, vb.y), vy2), wz = sub2(pack2(va.z, vb.z), vz2);
+                    s_d = fma2(g, fma2(wz, dz, fma2(wy, dy, mul2(wx, dx))), s_d);
+                    s_x = fma2(g, sub2(mul2(dy, wz), mul2(dz, wy)), s_x);
+                    s_y = fma2(g, sub2(mul2(dz, wx), mul2(dx, wz)), s_y);
+                    s_z = fma2(g, sub2(mul2(dx, wy), mul2(dy, wx)), s_z);
+                }
+            };
+            hits(m[0], m[2], 0);
+            if (cnt > 32) hits(m[1], m[3], kHalf);
+            float d0, d1, x0, x1, y0, y1, z0, z1;
+            unpack2(s_d, d0, d1); unpack2(s_x, x0, x1); unpack2(s_y, y0, y1); unpack2(s_z, z0, z1);
+            if (dual) {
+                if (wA) { float4 c = sm.acc[tA]; c.x += d0; c.y += x0; c.z += y0; c.w += z0; sm.acc[tA] = c; }
+                if (wB) { float4 c = sm.acc[tB]; c.x += d1; c.y += x1; c.z += y1; c.w += z1; sm.acc[tB] = c; }
+            } else if (wA) {
+                float4 c = sm.acc[tA];
+                c.x += d0 + d1; c.y += x0 + x1; c.z += y0 + y1; c.w += z0 + z1;
+                sm.acc[tA] = c;
+            }
+        };
+
+        uint32_t cnt = 0;
+        const uint32_t n_rounds = max(1u, (n_s + 31) >> 5);
+        for (uint32_t r = 0; r < n_rounds; ++r) {
+            const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
+            if (r > 0) { cp_async_wait_all(); __syncwarp(); }
+            if (r + 1 < n_rounds) {
+                fetch_records<10, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 40, min(32u, n_s - j0 - 32), lane);
+            } else if (has_next) {
+                fetch_records<10, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+                fetch_records<10, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
+            }
+            float4 s = make_float4(0.f, 0.f, 0.f, 0.f), sv = s;
+            bool ok = false;
+            if (lane < nj) {
+                const float* rec = sm.src[buf] + 10 * lane;
+                s = make_float4(rec[0], rec[1], rec[2], 0.f);
+                ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
+                if (ok) { s.w = rec[6] * rcp_fast(rec[9]); sv = make_float4(rec[3], rec[4], rec[5], 0.f); }
+            }
+            const uint32_t ball = __ballot_sync(kFull, ok), c = __popc(ball);
+            if (cnt + c > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
+            if (ok) {
+                const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);
+                sm.tile[e] = s; sm.tilev[e] = sv;
+                filter_put(sm.f, pos, s.x, s.y, s.z, fmaf(s.x, s.x, fmaf(s.y, s.y, s.z * s.z)));
+            }
+            cnt += c;
+            buf ^= 1;
+        }
+        if (cnt) flush(cnt);
+        __syncwarp();
+        if (vA) {
+            const float ih = rcp_fast(oA.w), n4 = kInvPi * (ih * ih) * (ih * ih);
+            const float4 c = sm.acc[lane];
+            reinterpret_cast<float4*>(tout)[lane] = make_float4(c.x * n4, c.y * n4, c.z * n4, c.w * n4);
+        }
+        if (vB) {
+            const float ih = rcp_fast(oB.w), n4 = kInvPi * (ih * ih) * (ih * ih);
+            const float4 c = sm.acc[lane + 32];
+            reinterpret_cast<float4*>(tout)[lane + 32] = make_float4(c.x * n4, c.y * n4, c.z * n4, c.w * n4);
+        }
+        __syncwarp();
+        iw = iw_next;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------- force
 
-struct ForceWarpSmem {
+template <int RW>
+struct ForceWarpSmemT {
     FilterTile f;
     float4 ta[2 * kHalf];    // sources: x, y, z, 4 h^2           (entries 32 and 65: the dummy)
     float4 tb[2 * kHalf];    //          vx, vy, vz, m
@@ -364,12 +531,15 @@ struct ForceWarpSmem {
     float4 t0[64];           // targets: x, y, z, 4 h^2
     float4 t1[64];           //          vx, vy, vz, c_s
     float4 t2[64];           //          1/h, 1/(pi h^4), rho, A
-    float raw[64 * 13];      // landing area of an item's 64 FORCE_IN records: xr0 xr1 xr2 h m rho rho_dh v0 v1 v2 u P cs;
+    float raw[64 * RW];      // landing area of an item's 64 FORCE_IN records: xr0 xr1 xr2 h m rho rho_dh v0 v1 v2 u P cs;
                              // once the target table is built: the 64 x 5 running results, in FORCE_OUT record layout
-    float src[2][32 * 13];   // landing areas of the source rounds (double-buffered)
+    float src[2][32 * RW];   // landing areas of the source rounds (double-buffered)
     uint32_t act[64];        // the active targets of the flush
     uint64_t bar[2];         // [0]: the mbarrier the record fetches complete on
+    float tB[64];            // targets: Balsara factor (three-loop cycle only)
+    float sB[2 * kHalf];     // sources: the same
 };
+typedef ForceWarpSmemT<13> ForceWarpSmem;
 
 // -0.75 (2 - q)+^2 + 3 (1 - q)+^2 = w'(q) of the cubic spline for a pair of q
 __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree, u64 kM075) {
@@ -386,6 +556,7 @@ __device__ __forceinline__ u64 spline_dw2(u64 q, u64 kTwo, u64 kOne, u64 kThree,
 struct ForceTargets2 {      // the targets' constants, one target per half
     u64 x, y, z, vx, vy, vz, cs, inv_h, n4, rho, A;
     float hc2a, hc2b;       // (2 h_i)^2
+    u64 B;                  // Balsara factors (three-loop cycle; unused otherwise)
 };
 struct ForcePair2 {
     u64 fr, ex, ey, ez, dg, vr;
@@ -394,8 +565,9 @@ struct ForcePair2 {
 struct ForceConsts2 {
     u64 two, one, three, m075, half, mhalf, onehalf, invpi, mbeta, malpha;
 };
+template <bool SWITCH = false>
 __device__ __forceinline__ ForcePair2 force_pair2(const ForceTargets2& T, const ForceConsts2& K, const float4& a, const float4& b,
-                                                  const float4& va, const float4& vb, const float4& ca, const float4& cb) {
+                                                  const float4& va, const float4& vb, const float4& ca, const float4& cb, u64 Bj = 0) {
     ForcePair2 o;
     o.ex = sub2(pack2(a.x, b.x), T.x); o.ey = sub2(pack2(a.y, b.y), T.y); o.ez = sub2(pack2(a.z, b.z), T.z);
     const u64 r2 = fma2(o.ez, o.ez, fma2(o.ey, o.ey, mul2(o.ex, o.ex)));
@@ -422,7 +594,8 @@ __device__ __forceinline__ ForcePair2 force_pair2(const ForceTargets2& T, const 
     float rsa, rsb, vsa, vsb;
     unpack2(add2(T.rho, pack2(ca.x, cb.x)), rsa, rsb);
     unpack2(vs, vsa, vsb);
-    const u64 visc = mul2(mul2(mul2(K.malpha, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
+    u64 visc = mul2(mul2(mul2(K.malpha, vs), mu), pack2(rcp_approx(rsa), rcp_approx(rsb)));   // -(alpha/2) vs mu / ((rho_i+rho_j)/2)
+    if constexpr (SWITCH) visc = mul2(visc, mul2(K.half, add2(T.B, Bj)));                            // Balsara: (B_i + B_j) / 2
     const u64 vG = mul2(mul2(visc, K.half), add2(Gi, Gj));
     const u64 AG = mul2(T.A, Gi), BG = mul2(pack2(ca.y, cb.y), Gj);
     const u64 mm = pack2(hitA ? va.w : 0.f, hitB ? vb.w : 0.f);
@@ -440,12 +613,20 @@ __device__ __forceinline__ void kahan2(u64& sum, u64& c, u64 a, u64 b) {
     sum = t;
 }
 
-template <bool UNITS>
+// Balsara-type switch (reading C34): B = |div v| / (|div v| + |rot v| + 1e-4 c_s / h)
+__device__ __forceinline__ float balsara(const float* r) {      // r: a FORCE3_IN record
+    const float div = fabsf(r[13]), rot = sqrtf(fmaf(r[14], r[14], fmaf(r[15], r[15], r[16] * r[16])));
+    return div * rcp_fast(div + rot + 1.0e-4f * r[12] * rcp_fast(r[3]));
+}
+
+template <bool UNITS, bool SWITCH>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    ForceWarpSmem& sm = reinterpret_cast<ForceWarpSmem*>(s_raw)[warp];
+    constexpr int RW = SWITCH ? 18 : 13;      // words of an input record: FORCE_IN, or FORCE3_IN = FORCE_IN + div_v rot_v[3] time_bin
+    typedef ForceWarpSmemT<RW> Smem;
+    Smem& sm = reinterpret_cast<Smem*>(s_raw)[warp];
     const uint32_t lt = lanemask_lt();
     const uint32_t step = gridDim.x * kLoopWarps;
     uint32_t item = blockIdx.x * kLoopWarps + warp;
@@ -454,6 +635,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         sm.ta[lane * kHalf + 32] = make_float4(kFar, kFar, kFar, 0.f);
         sm.tb[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
         sm.tc[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
+        sm.sB[lane * kHalf + 32] = 0.f;
     }
     const ForceConsts2 K{dup2(2.0f), dup2(1.0f), dup2(3.0f), dup2(-0.75f), dup2(0.5f), dup2(-0.5f), dup2(1.5f), dup2(kInvPi), dup2(-beta), dup2(-alpha)};
 
@@ -461,7 +643,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
     FetchGroup fg{&sm.bar[0], 0u};
     if (lane == 0) { mbar_init(fg.bar, 1); fence_mbar_init(); }
     __syncwarp();
-    fg.issue2(lane, sm.raw, in + (uint64_t)iw.x * 128, rec_bytes16<13>(iw.w & 127u), sm.src[0], in + (uint64_t)iw.y * 128, rec_bytes16<13>(min(32u, iw.w >> 7)));
+    fg.issue2(lane, sm.raw, in + (uint64_t)iw.x * 128, rec_bytes16<RW>(iw.w & 127u), sm.src[0], in + (uint64_t)iw.y * 128, rec_bytes16<RW>(min(32u, iw.w >> 7)));
     uint32_t buf = 0;
 
     for (; item < n_items; item += step) {
@@ -481,12 +663,13 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const uint32_t t = lane + 32 * k;
             float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0, p2 = make_float4(0.f, 0.f, 1.f, 0.f);
             if (t < n_t) {
-                const float* r = sm.raw + 13 * t;
+                const float* r = sm.raw + RW * t;
                 const float h = r[3], rho = r[5], ih = rcp_fast(h);
                 p0 = make_float4(r[0], r[1], r[2], 4.0f * h * h);
                 p1 = make_float4(r[7], r[8], r[9], r[12]);
                 p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11] * rcp_fast(fmaf(h * r[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho));
                 if (k == 0) hA = h; else hB = h;
+                if constexpr (SWITCH) sm.tB[t] = balsara(r);
             }
             sm.t0[t] = p0; sm.t1[t] = p1; sm.t2[t] = p2;
             if (k == 0) oA = p0; else oB = p0;
@@ -540,13 +723,15 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             if constexpr (!UNITS) {
                 const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
                 const ForceTargets2 T{pack2(pA.x, pB.x), pack2(pA.y, pB.y), pack2(pA.z, pB.z), pack2(qA.x, qB.x), pack2(qA.y, qB.y), pack2(qA.z, qB.z),
-                                      pack2(qA.w, qB.w), pack2(sA.x, sB.x), pack2(sA.y, sB.y), pack2(sA.z, sB.z), pack2(sA.w, sB.w), pA.w, pB.w};
+                                      pack2(qA.w, qB.w), pack2(sA.x, sB.x), pack2(sA.y, sB.y), pack2(sA.z, sB.z), pack2(sA.w, sB.w), pA.w, pB.w,
+                                      SWITCH ? pack2(sm.tB[tA], sm.tB[tB]) : 0ull};
                 u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
                 float vsig0 = 0.f, vsig1 = 0.f;
                 auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
                     uint32_t ja, jb;
                     while (next_hits(dual, ma, mb, &ja, &jb)) {
-                        const ForcePair2 o = force_pair2(T, K, sm.ta[base + ja], sm.ta[base + jb], sm.tb[base + ja], sm.tb[base + jb], sm.tc[base + ja], sm.tc[base + jb]);
+                        const ForcePair2 o = force_pair2<SWITCH>(T, K, sm.ta[base + ja], sm.ta[base + jb], sm.tb[base + ja], sm.tb[base + jb], sm.tc[base + ja],
+                                                                 sm.tc[base + jb], SWITCH ? pack2(sm.sB[base + ja], sm.sB[base + jb]) : 0ull);
                         kahan2(ax, cx, o.fr, o.ex); kahan2(ay, cy, o.fr, o.ey); kahan2(az, cz, o.fr, o.ez);
                         du = fma2(o.dg, o.vr, du);
                         vsig0 = fmaxf(vsig0, o.vsa); vsig1 = fmaxf(vsig1, o.vsb);
@@ -601,11 +786,12 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                             e[q] = ebase + j;
                         }
                         const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
-                        const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w};
+                        const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w, SWITCH ? dup2(sm.tB[t]) : 0ull};
                         u64 ax = 0, ay = 0, az = 0, du = 0;
                         float vsig = 0.f;
                         auto two = [&](uint32_t ja, uint32_t jb) {
-                            const ForcePair2 o = force_pair2(T, K, sm.ta[ja], sm.ta[jb], sm.tb[ja], sm.tb[jb], sm.tc[ja], sm.tc[jb]);
+                            const ForcePair2 o = force_pair2<SWITCH>(T, K, sm.ta[ja], sm.ta[jb], sm.tb[ja], sm.tb[jb], sm.tc[ja], sm.tc[jb],
+                                                                     SWITCH ? pack2(sm.sB[ja], sm.sB[jb]) : 0ull);
                             ax = fma2(o.fr, o.ex, ax); ay = fma2(o.fr, o.ey, ay); az = fma2(o.fr, o.ez, az);
                             du = fma2(o.dg, o.vr, du);
                             vsig = fmaxf(vsig, fmaxf(o.vsa, o.vsb));
@@ -659,12 +845,12 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
             if (r > 0) fg.wait();
             // one step ahead: the next round of this item (the next item's records are fetched once the results have left sm.raw)
-            if (r + 1 < n_rounds) fg.issue1(lane, sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 52, rec_bytes16<13>(min(32u, n_s - j0 - 32)));
+            if (r + 1 < n_rounds) fg.issue1(lane, sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * (RW * 4), rec_bytes16<RW>(min(32u, n_s - j0 - 32)));
             float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
             float s2 = 0.f;
             bool ok = false;
             if (lane < nj) {
-                const float* rec = sm.src[buf] + 13 * lane;
+                const float* rec = sm.src[buf] + RW * lane;
                 const float h = rec[3], rho = rec[5];
                 const float reach = fmaxf(reach_t, 2.0f * h) * kReachSlack;
                 a = make_float4(rec[0], rec[1], rec[2], 4.0f * h * h);
@@ -680,6 +866,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             if (ok) {
                 const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);      // half * 33 + index in the half
                 sm.ta[e] = a; sm.tb[e] = b; sm.tc[e] = c;
+                if constexpr (SWITCH) sm.sB[e] = balsara(sm.src[buf] + RW * lane);
                 filter_put(sm.f, pos, a.x, a.y, a.z, s2);
             }
             tile_hc2 = fmaxf(tile_hc2, warp_max_pos(ok ? a.w : 0.f));
@@ -694,8 +881,8 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         for (uint32_t v = lane; v < nvec; v += 32) reinterpret_cast<uint4*>(tout)[v] = reinterpret_cast<const uint4*>(sm.raw)[v];
         __syncwarp();
         if (has_next) {
-            fg.issue2(lane, sm.raw, in + (uint64_t)iw_next.x * 128, rec_bytes16<13>(iw_next.w & 127u),
-                      sm.src[buf], in + (uint64_t)iw_next.y * 128, rec_bytes16<13>(min(32u, iw_next.w >> 7)));
+            fg.issue2(lane, sm.raw, in + (uint64_t)iw_next.x * 128, rec_bytes16<RW>(iw_next.w & 127u),
+                      sm.src[buf], in + (uint64_t)iw_next.y * 128, rec_bytes16<RW>(min(32u, iw_next.w >> 7)));
         }
         iw = iw_next;
     }
@@ -723,23 +910,43 @@ int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaSt
     return SPH_OK;
 }
 
+int32_t launch_gradient(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st) {
+    if (b->n_items == 0) return SPH_OK;
+    uint32_t full_grid = 0;
+    constexpr size_t smem = sizeof(GradientWarpSmem) * kLoopWarps;
+    if (int32_t rc = loop_grid(gradient_kernel, smem, &full_grid)) return rc;
+    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
+    gradient_kernel<<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_gradient, d_in, d_out, b->n_items);
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
 #ifndef SPH_UNITS_MAX_MEAN_BLOCK
 #define SPH_UNITS_MAX_MEAN_BLOCK 80
 #endif
 
-int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
+template <bool SWITCH>
+static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
     if (b->n_items == 0) return SPH_OK;
-    uint32_t full_grid[2] = {0, 0};
-    constexpr size_t smem = sizeof(ForceWarpSmem) * kLoopWarps;
+    uint32_t full_grid = 0;
+    constexpr size_t smem = sizeof(ForceWarpSmemT<SWITCH ? 18 : 13>) * kLoopWarps;
     // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
     // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
     const bool units = b->n_sides && b->n_instances <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * b->n_sides;
-    if (int32_t rc = units ? loop_grid(force_kernel<true>, smem, &full_grid[1]) : loop_grid(force_kernel<false>, smem, &full_grid[0])) return rc;
-    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid[units]);
-    if (units) force_kernel<true><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_items, prm.alpha, prm.beta);
-    else force_kernel<false><<<grid, kLoopWarps * 32, smem, st>>>(b->d_items_force, d_in, d_out, b->n_items, prm.alpha, prm.beta);
+    if (int32_t rc = units ? loop_grid(force_kernel<true, SWITCH>, smem, &full_grid) : loop_grid(force_kernel<false, SWITCH>, smem, &full_grid)) return rc;
+    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
+    if (units) force_kernel<true, SWITCH><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta);
+    else force_kernel<false, SWITCH><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
+}
+
+int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
+    return launch_force_t<false>(b, b->d_items_force, d_in, d_out, prm, st);
+}
+
+int32_t launch_force3(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
+    return launch_force_t<true>(b, b->d_items_force3, d_in, d_out, prm, st);
 }
 
 }  // namespace sph

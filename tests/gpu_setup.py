@@ -64,3 +64,22 @@ def canon(parts):
     raw[:, 108:112] = 0
     raw[:, 121:128] = 0
     return raw
+
+
+def vec_scale(ref):
+    """max |a|: the largest vector magnitude of a set of vectors (rows), or the largest |value| of scalars"""
+    ref = np.asarray(ref, dtype=np.float64)
+    return float(np.sqrt((ref * ref).sum(-1)).max()) if ref.ndim == 2 else float(np.abs(ref).max())
+
+
+def within_1e4_or_1e6(got, ref, scale=None):
+    """north_star: "within 1e-4 relative or 1e-6 * max|a| absolute" (reading C35).  For a vector quantity
+    (rows of 3: a, rot_v) |.| is the vector's magnitude: |got - ref|_2 <= max(1e-4 |ref|_2, 1e-6 max|ref|_2) per
+    particle; for a scalar (du/dt, div_v) the absolute value.  scale overrides max|ref| (samples of a larger set)."""
+    got, ref = np.asarray(got, dtype=np.float64), np.asarray(ref, dtype=np.float64)
+    scale = vec_scale(ref) if scale is None else scale
+    if ref.ndim == 2:
+        err, mag = np.sqrt(((got - ref) ** 2).sum(-1)), np.sqrt((ref * ref).sum(-1))
+    else:
+        err, mag = np.abs(got - ref), np.abs(ref)
+    return bool(np.all(err <= np.maximum(1e-4 * mag, 1e-6 * scale)))

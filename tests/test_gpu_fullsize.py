@@ -19,7 +19,7 @@ import torch
 import oracle as orc
 import paper_2606_23891_b200 as sph
 import sph_inputs as si
-from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask
+from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
 from orc_setup import raw_copy, sort_grid
 from test_gpu_parity import _random_result_buffer, _records, check_store_physics, gpu_step
 
@@ -133,9 +133,7 @@ def test_config1_loops_every_record():
     got = f_out.cpu().numpy()
     mask = _block_mask(cells, tasks, 20, want.shape[0])
     w5, g5 = want[mask].view(np.float32).reshape(-1, 5).astype(np.float64), got[mask].view(np.float32).reshape(-1, 5).astype(np.float64)
-    amax, dumax = np.abs(ref["a"]).max(), np.abs(ref["du_dt"]).max()
-    assert np.all(np.abs(g5[:, :3] - w5[:, :3]) <= np.maximum(1e-4 * np.abs(w5[:, :3]), 1e-6 * amax))
-    assert np.all(np.abs(g5[:, 3] - w5[:, 3]) <= np.maximum(1e-4 * np.abs(w5[:, 3]), 1e-6 * dumax))
+    assert within_1e4_or_1e6(g5[:, :3], w5[:, :3], vec_scale(ref["a"])) and within_1e4_or_1e6(g5[:, 3], w5[:, 3], vec_scale(ref["du_dt"]))
     exempt = _C1["exempt"][_record_particles(cells, tasks)]              # C31
     assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt)
     g.close()
@@ -221,9 +219,7 @@ def test_config2_force_on_sampled_bundles():
         lo = int(seg_out[b])
         w5 = want[mask].view(np.float32).reshape(-1, 5).astype(np.float64)
         g5 = got_out[lo:lo + want.shape[0]][mask].view(np.float32).reshape(-1, 5).astype(np.float64)
-        amax, dumax = np.abs(w5[:, :3]).max(), np.abs(w5[:, 3]).max()
-        assert np.all(np.abs(g5[:, :3] - w5[:, :3]) <= np.maximum(1e-4 * np.abs(w5[:, :3]), 1e-6 * amax)), b
-        assert np.all(np.abs(g5[:, 3] - w5[:, 3]) <= np.maximum(1e-4 * np.abs(w5[:, 3]), 1e-6 * dumax)), b
+        assert within_1e4_or_1e6(g5[:, :3], w5[:, :3]) and within_1e4_or_1e6(g5[:, 3], w5[:, 3]), b
         exempt = orc.flag_cutoff_pairs(cells, sel, want_in)[_record_particles(cells, sel)]      # C31, this bundle's own pairs
         assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt) and exempt.mean() < 0.01, b
     g.close()
@@ -351,6 +347,21 @@ def test_config4_pipeline_sampled_cells_and_invariants():
     idx = np.concatenate([np.arange(first[c], first[c] + count[c]) for c in np.flatnonzero(sample)])
     assert idx.shape[0] > 100000
     g, r = got[idx], ref[idx]
-    check_store_physics(g, r, a_scale=float(np.abs(got["a"]).max()), du_scale=float(np.abs(got["du_dt"]).max()))
+    check_store_physics(g, r, a_scale=vec_scale(got["a"]), du_scale=vec_scale(got["du_dt"]))
     ok = np.abs(g["v_sig"] - r["v_sig"]) <= 1e-4 * r["v_sig"]
     assert np.all(ok | exempt[idx]) and exempt[idx].mean() < 0.01
+
+
+def test_config1_three_loop_step_every_particle():
+    """configs[1] through the three-loop cycle (density, ghost, gradient, Balsara-switched force; reading C34), one batch"""
+    from test_gpu_parity import check_three_loop, gpu_three_loop_step
+    ps, cells, tasks, _ = config1()
+    ref = raw_copy(ps)
+    orc.density_cycle(ref, cells, tasks)
+    orc.ghost(ref, GAMMA)
+    orc.gradient_cycle(ref, cells, tasks)
+    exempt = orc.flag_cutoff_pairs(cells, tasks, orc.pack(ref, cells, tasks, orc.FORCE_IN))
+    orc.force3_cycle(ref, cells, tasks)
+    g = GpuCase(ps, cells, tasks, "split")
+    check_three_loop(gpu_three_loop_step(g), ref, exempt)
+    g.close()

@@ -11,7 +11,7 @@ import torch
 import oracle as orc
 import paper_2606_23891_b200 as sph
 import sph_inputs as si
-from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask
+from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
 from orc_setup import raw_copy, sort_grid, sort_octree
 
 pytestmark = pytest.mark.gpu
@@ -221,9 +221,7 @@ def test_force_loop_vs_oracle(name):
     r5, pidx = _records(ref, off, cells, tasks, 5)
     g5, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 5)
     r5, g5 = r5.astype(np.float64), g5.astype(np.float64)
-    amax, dumax = np.abs(r5[:, :3]).max(), np.abs(r5[:, 3]).max()
-    assert np.all(np.abs(g5[:, :3] - r5[:, :3]) <= np.maximum(1e-4 * np.abs(r5[:, :3]), 1e-6 * amax))
-    assert np.all(np.abs(g5[:, 3] - r5[:, 3]) <= np.maximum(1e-4 * np.abs(r5[:, 3]), 1e-6 * dumax))
+    assert within_1e4_or_1e6(g5[:, :3], r5[:, :3]) and within_1e4_or_1e6(g5[:, 3], r5[:, 3])
     exempt = _near_cutoff(ps, cells, tasks, buf_in)[pidx]
     ok = np.abs(g5[:, 4] - r5[:, 4]) <= 1e-4 * np.abs(r5[:, 4])
     assert np.all(ok | exempt) and exempt.mean() < 0.01
@@ -274,10 +272,10 @@ def test_unpack_reduce_zero_equals_zero_then_reduce(name, layout):
         for f, c, _n in oset[0]:                              # zero the reduced fields (every cell occurs in these batches)
             name_f = ("x", "v", "a", "mass", "h", "u", "du_dt", "rho", "rho_dh", "wcount", "wcount_dh", "div_v", "rot_v", "P", "c_s", "v_sig",
                       "id", "time_bin")[f]
-            if name_f in ("rho", "rho_dh", "wcount", "wcount_dh", "du_dt", "v_sig"):
+            if name_f in ("rho", "rho_dh", "wcount", "wcount_dh", "du_dt", "v_sig", "div_v"):
                 ref[name_f] = 0
-            elif name_f == "a":
-                ref["a"][:, c:c + _n] = 0
+            elif name_f in ("a", "rot_v"):
+                ref[name_f][:, c:c + _n] = 0
         orc.unpack(ref, cells, tasks, oset, buf, orc.MODE_REDUCE)
         sph.sph_store_import_aos(g.store, ps)                 # the store holds non-zero values in those fields
         assert sph.sph_batch_buffer_bytes(g.batch, aset) == total
@@ -486,9 +484,9 @@ def check_store_physics(got, ref, a_scale=None, du_scale=None):
         assert np.max(np.abs(vd - rd) / np.maximum(np.abs(rd), r / h)) <= 2e-5, dname
     assert np.max(np.abs(got["P"] - ref["P"]) / ref["P"]) <= 2e-5 and np.max(np.abs(got["c_s"] - ref["c_s"]) / ref["c_s"]) <= 1e-6
     a_r, a_g = ref["a"].astype(np.float64), got["a"].astype(np.float64)
-    assert np.all(np.abs(a_g - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * (a_scale or np.abs(a_r).max())))
+    assert within_1e4_or_1e6(a_g, a_r, a_scale)
     d_r, d_g = ref["du_dt"].astype(np.float64), got["du_dt"].astype(np.float64)
-    assert np.all(np.abs(d_g - d_r) <= np.maximum(1e-4 * np.abs(d_r), 1e-6 * (du_scale or np.abs(d_r).max())))
+    assert within_1e4_or_1e6(d_g, d_r, du_scale)
 
 
 @pytest.mark.parametrize("layout", ["aos", "split"])
@@ -554,7 +552,7 @@ def test_segmented_batch_equals_standalone_batches(layout):
     orc.force_cycle(ref, cells, tasks, batch=seg)
     got = g.export()
     a_r = ref["a"].astype(np.float64)
-    assert np.all(np.abs(got["a"] - a_r) <= np.maximum(1e-4 * np.abs(a_r), 1e-6 * np.abs(a_r).max()))
+    assert within_1e4_or_1e6(got["a"], a_r)
     g.close()
 
 
@@ -664,4 +662,105 @@ def test_streams_are_honoured():
     off, total = orc.block_offsets(cells, tasks, 20)
     m = valid_mask(off, cells, tasks, 20, total)
     assert np.array_equal(buf.cpu().numpy()[m], ref[m])
+    g.close()
+
+
+# ------------------------------------------------------------------ three-loop cycle: gradient loop, Balsara-switched force (reading C34)
+
+def _sum_tol(got, ref, scale):
+    """sign-changing neighbour sums: 1e-4 relative or 1e-6 of the largest value of the launch (the north_star's clause for a, C35)"""
+    return within_1e4_or_1e6(got, ref, scale)
+
+
+@pytest.mark.parametrize("name", ["ragged", "octree", "bigcells", "hugecells"])
+def test_gradient_loop_vs_oracle(name):
+    ps, cells, tasks = case(name)
+    ps = physical(raw_copy(ps), cells, tasks)
+    buf_in = orc.pack(ps, cells, tasks, orc.GRADIENT_IN)
+    ref = orc.gradient(cells, tasks, buf_in)
+    g = GpuCase(ps, cells, tasks)
+    # the library packs the same 40-byte records (Table 1's p-g column), byte for byte
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_GRADIENT_IN)
+    assert sph.sph_attrset_record_bytes(aset) == 40
+    off_in, total_in = orc.block_offsets(cells, tasks, 40)
+    m = valid_mask(off_in, cells, tasks, 40, total_in)
+    assert np.array_equal(g.pack(aset).cpu().numpy()[m], buf_in[m])
+    d_out = g.buffer(sph.sph_attrset_canonical(sph.SPH_SET_GRADIENT_OUT))
+    sph.sph_gradient(g.batch, torch.from_numpy(buf_in).cuda(), d_out)
+    torch.cuda.synchronize()
+    off, _ = orc.block_offsets(cells, tasks, 16)
+    r4, _ = _records(ref, off, cells, tasks, 4)
+    g4, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 4)
+    r4, g4 = r4.astype(np.float64), g4.astype(np.float64)
+    scale = max(np.abs(r4[:, 0]).max(), vec_scale(r4[:, 1:]))
+    assert scale > 0 and _sum_tol(g4[:, 0], r4[:, 0], scale) and _sum_tol(g4[:, 1:], r4[:, 1:], scale)
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "hugecells"])
+def test_switched_force_loop_vs_oracle(name):
+    ps, cells, tasks = case(name)
+    ps = physical(raw_copy(ps), cells, tasks)
+    if name == "config0":
+        ps["v"] = (0.2 * np.random.default_rng(3).standard_normal((ps.shape[0], 3))).astype(np.float32)      # configs[0] is at rest
+    orc.gradient_cycle(ps, cells, tasks)
+    buf_in = orc.pack(ps, cells, tasks, orc.FORCE3_IN)
+    ref = orc.force3(cells, tasks, buf_in, 0.8, 3.0)
+    plain = orc.force(cells, tasks, orc.pack(ps, cells, tasks, orc.FORCE_IN), 0.8, 3.0)
+    g = GpuCase(ps, cells, tasks)
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_FORCE3_IN)
+    off_in, total_in = orc.block_offsets(cells, tasks, 72)
+    m = valid_mask(off_in, cells, tasks, 72, total_in)
+    assert np.array_equal(g.pack(aset).cpu().numpy()[m], buf_in[m])
+    d_out = g.buffer(to_attrset(orc.FORCE_OUT))
+    sph.sph_force3(g.batch, torch.from_numpy(buf_in).cuda(), d_out, PARAMS)
+    torch.cuda.synchronize()
+    off, _ = orc.block_offsets(cells, tasks, 20)
+    r5, pidx = _records(ref, off, cells, tasks, 5)
+    g5, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 5)
+    p5, _ = _records(plain, off, cells, tasks, 5)
+    r5, g5 = r5.astype(np.float64), g5.astype(np.float64)
+    assert np.abs(r5[:, :3] - p5[:, :3]).max() > 1e-3 * np.abs(r5[:, :3]).max()         # the switch changes the result in this state
+    assert _sum_tol(g5[:, :3], r5[:, :3], vec_scale(r5[:, :3])) and _sum_tol(g5[:, 3], r5[:, 3], np.abs(r5[:, 3]).max())
+    exempt = _near_cutoff(ps, cells, tasks, orc.pack(ps, cells, tasks, orc.FORCE_IN))[pidx]
+    assert np.all((np.abs(g5[:, 4] - r5[:, 4]) <= 1e-4 * np.abs(r5[:, 4])) | exempt)
+    g.close()
+
+
+def gpu_three_loop_step(g):
+    """density cycle, ghost, gradient cycle, switched force cycle through the C ABI (zeroing fused into the unpacks)"""
+    S = [sph.sph_attrset_canonical(k) for k in range(7)]
+    mode = sph.SPH_UNPACK_REDUCE_ZERO
+    b = [g.buffer(s) for s in S]
+    sph.sph_pack(g.store, g.batch, S[0], b[0]); sph.sph_density(g.batch, b[0], b[1]); sph.sph_unpack(g.store, g.batch, S[1], b[1], mode)
+    sph.sph_ghost(g.store, PARAMS)
+    sph.sph_pack(g.store, g.batch, S[4], b[4]); sph.sph_gradient(g.batch, b[4], b[5]); sph.sph_unpack(g.store, g.batch, S[5], b[5], mode)
+    sph.sph_pack(g.store, g.batch, S[6], b[6]); sph.sph_force3(g.batch, b[6], b[3], PARAMS); sph.sph_unpack(g.store, g.batch, S[3], b[3], mode)
+    torch.cuda.synchronize()
+    return g.export()
+
+
+def check_three_loop(got, ref, exempt):
+    check_store_physics(got, ref)
+    for k in ("div_v", "rot_v"):
+        assert _sum_tol(got[k], ref[k], max(np.abs(ref["div_v"]).max(), vec_scale(ref["rot_v"]))), k
+    ok = np.abs(got["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
+    assert np.all(ok | exempt)
+    m, a = got["mass"].astype(np.float64), got["a"].astype(np.float64)
+    assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+
+
+@pytest.mark.parametrize("layout", ["aos", "split"])
+@pytest.mark.parametrize("name", ["ragged", "octree", "hugecells"])
+def test_three_loop_step_vs_oracle(name, layout):
+    ps, cells, tasks = case(name)
+    ref = raw_copy(ps)
+    orc.set_threads(8)
+    orc.density_cycle(ref, cells, tasks)
+    orc.ghost(ref, GAMMA)
+    orc.gradient_cycle(ref, cells, tasks)
+    exempt = vsig_exempt(ref, cells, tasks)
+    orc.force3_cycle(ref, cells, tasks)
+    g = GpuCase(ps, cells, tasks, layout)
+    check_three_loop(gpu_three_loop_step(g), ref, exempt)
     g.close()
