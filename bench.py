@@ -35,7 +35,7 @@ SHARDING = "one independent box per rank, no collective"
 N_SM, LANES_PER_SM = 148, 128
 # algorithmic FP32 work of the loops: 8 flop per ordered candidate pair (3 sub, 1 mul,
 # 2 fma, 1 compare) + per neighbour hit 25 flop (density) / 60 flop (force)
-FLOP_CAND, FLOP_HIT_DENSITY, FLOP_HIT_FORCE = 8.0, 25.0, 60.0
+FLOP_CAND, FLOP_HIT_DENSITY, FLOP_HIT_FORCE, FLOP_HIT_GRADIENT = 8.0, 25.0, 60.0, 45.0
 NGB_CONFIG1 = 63.04    # (32/3) pi (1.2348)^3: neighbours per particle incl. self at h = 1.2348 dx
 
 
@@ -167,13 +167,14 @@ def dist_sum(value, world, device="cpu"):
 # --------------------------------------------------------------------------------------------- our arm
 
 class Workload:
-    """configs[1] resident on the current device in one layout, one batch holding every task of a loop."""
+    """configs[1] resident on the current device in one layout, one batch holding every task of a loop; the two-loop cycle
+    (density, force) or the three-loop cycle (density, gradient, Balsara-switched force: PAPER.md:41, reading C34)."""
 
-    def __init__(self, sph, torch, ps, cells, tasks, layout_name):
+    def __init__(self, sph, torch, ps, cells, tasks, layout_name, loops=2):
         self.sph, self.torch = sph, torch
-        self.layout_name = layout_name
+        self.layout_name, self.loops = layout_name, loops
         from paper_2606_23891_b200 import layouts as _layouts
-        self.layout = _layouts.layout(sph, layout_name)
+        self.layout = _layouts.layout(sph, layout_name, loops=loops)
         self.n = ps.shape[0]
         self.cells = cells
         self.store = sph.sph_store_create(self.layout, self.n)
@@ -181,7 +182,7 @@ class Workload:
         sph.sph_store_set_cells(self.store, cells)
         self.batch = sph.sph_batch_create(self.store, tasks)
         self.info = sph.sph_batch_get_info(self.batch)
-        self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+        self.sets = [sph.sph_attrset_canonical(k) for k in range(7 if loops == 3 else 4)]
         self.rec = [sph.sph_attrset_record_bytes(s) for s in self.sets]
         self.bufs = [torch.empty(sph.sph_batch_buffer_bytes(self.batch, s), dtype=torch.uint8, device="cuda") for s in self.sets]
         self.params = sph.sph_params(np.float32(5.0 / 3.0), 0.8, 3.0)
@@ -193,27 +194,41 @@ class Workload:
             self.host.append(h)
         # which substructs a step reads from / writes to the host copy
         f = sph.FIELD
-        ins = {self.layout.loc[f[k]].sub for k in ("x", "h", "mass", "v", "u")}
-        outs = {self.layout.loc[f[k]].sub for k in ("rho", "rho_dh", "wcount", "wcount_dh", "P", "c_s", "a", "du_dt", "v_sig")}
+        sub = lambda names: {self.layout.loc[f[k]].sub for k in names}
+        self.sub = sub
+        ins = sub(("x", "h", "mass", "v", "u") + (("time_bin",) if loops == 3 else ()))
+        outs = sub(("rho", "rho_dh", "wcount", "wcount_dh", "P", "c_s", "a", "du_dt", "v_sig") + (("div_v", "rot_v") if loops == 3 else ()))
         self.subs_in, self.subs_out = sorted(ins), sorted(outs)
         for s in range(self.layout.n_sub):
             sph.sph_store_download_sub(self.store, s, self.host[s])
         torch.cuda.synchronize()
 
-    # the seven launches of a step, as (name, callable)
+    # the launches of a step, as (name, callable): seven (two loops) or ten (three loops)
     def launches(self, stream=None):
         stream = stream if stream is not None else self.torch.cuda.current_stream()
         sph, st, b, S, B, p = self.sph, self.store, self.batch, self.sets, self.bufs, self.params
         # "zero the outputs of the loop about to run" is fused into the unpack (SPH_UNPACK_REDUCE_ZERO: one batch holds the whole
         # loop, so every particle's sums start from 0 there) -- bit-identical to sph_store_zero + SPH_UNPACK_REDUCE
-        return [
+        Z = sph.SPH_UNPACK_REDUCE_ZERO
+        head = [
             ("pack_density_in", lambda: sph.sph_pack(st, b, S[0], B[0], stream)),
             ("density", lambda: sph.sph_density(b, B[0], B[1], stream)),
-            ("unpack_density_out", lambda: sph.sph_unpack(st, b, S[1], B[1], sph.SPH_UNPACK_REDUCE_ZERO, stream)),
+            ("unpack_density_out", lambda: sph.sph_unpack(st, b, S[1], B[1], Z, stream)),
             ("ghost", lambda: sph.sph_ghost(st, p, stream)),
+        ]
+        if self.loops == 3:
+            return head + [
+                ("pack_gradient_in", lambda: sph.sph_pack(st, b, S[4], B[4], stream)),
+                ("gradient", lambda: sph.sph_gradient(b, B[4], B[5], stream)),
+                ("unpack_gradient_out", lambda: sph.sph_unpack(st, b, S[5], B[5], Z, stream)),
+                ("pack_force_in", lambda: sph.sph_pack(st, b, S[6], B[6], stream)),
+                ("force", lambda: sph.sph_force3(b, B[6], B[3], p, stream)),
+                ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], Z, stream)),
+            ]
+        return head + [
             ("pack_force_in", lambda: sph.sph_pack(st, b, S[2], B[2], stream)),
             ("force", lambda: sph.sph_force(b, B[2], B[3], p, stream)),
-            ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], sph.SPH_UNPACK_REDUCE_ZERO, stream)),
+            ("unpack_force_out", lambda: sph.sph_unpack(st, b, S[3], B[3], Z, stream)),
         ]
 
     def step(self, stream=None):
@@ -222,24 +237,37 @@ class Workload:
 
     def step_e2e(self, stream=None):
         """The step with the particle arrays in pinned HOST memory.  Uploads run on a copy stream ahead of the kernels that need
-        them, downloads on a second one as soon as a substruct holds its final values, so that with split-AoS the force
-        inputs cross during the density loop and the density results during the force loop; the first pack and the last unpack
-        are streamed in four slabs of cells (sph_pack_cells / sph_unpack_cells) against their copies.  The calling stream waits for the last download: its events bracket the whole step."""
+        them, downloads on a second one as soon as a substruct holds its final values, so that with split-AoS the later loops'
+        inputs cross during the density loop and each loop's results during the next loop; the first pack and the last unpack
+        are streamed in four slabs of cells (sph_pack_cells / sph_unpack_cells) against their copies.  A substruct that holds
+        both a later loop's inputs and an earlier loop's outputs (pack-density, pack-gradient, ...) is uploaded BEFORE the
+        kernel that writes those outputs runs.  The calling stream waits for the last download: its events bracket the step."""
         torch, sph = self.torch, self.sph
         main = stream if stream is not None else torch.cuda.current_stream()
         if not hasattr(self, "_e2e"):
-            f, loc = sph.FIELD, self.layout.loc
-            sub = lambda names: {loc[f[k]].sub for k in names}
-            d_in, f_in = sub(("x", "h", "mass")), sub(("v", "u"))
-            d_out, g_out, f_out = sub(("rho", "rho_dh", "wcount", "wcount_dh")), sub(("P", "c_s")), sub(("a", "du_dt", "v_sig"))
-            self._e2e = {"up": torch.cuda.Stream(), "down": torch.cuda.Stream(), "up1": sorted(d_in), "up2": sorted(f_in - d_in),
-                         "down1": sorted(d_out - g_out - f_out), "down2": sorted(g_out - f_out), "down3": sorted(f_out)}
+            sub = self.sub
+            d_in = sub(("x", "h", "mass"))
+            later_in = sub(("v", "u") + (("time_bin",) if self.loops == 3 else ())) - d_in
+            # the stages that write the store, in order, and the substructs each one writes
+            writes = [("unpack_density_out", sub(("rho", "rho_dh", "wcount", "wcount_dh"))), ("ghost", sub(("P", "c_s")))]
+            if self.loops == 3:
+                writes.append(("unpack_gradient_out", sub(("div_v", "rot_v"))))
+            writes.append(("unpack_force_out", sub(("a", "du_dt", "v_sig"))))
+            last = {}
+            for k, subs in writes:
+                for s_ in subs:
+                    last[s_] = k                      # a substruct leaves after the last stage that writes it
+            written = set().union(*[subs for _, subs in writes])
+            self._e2e = {"up": torch.cuda.Stream(), "down": torch.cuda.Stream(), "up1": sorted(d_in), "up2": sorted(later_in),
+                         "down_after": {k: sorted(s_ for s_, kk in last.items() if kk == k) for k, _ in writes},
+                         # the later loops' inputs must have landed before the first kernel that writes their substruct (else
+                         # before the first kernel that reads them: the ghost reads u)
+                         "up2_before": next((k for k, subs in writes if subs & later_in), None) if later_in & written else None}
             from bench_workloads import cell_slabs
             self._e2e["slabs"] = cell_slabs(self.cells, 4)
         E = self._e2e
         up, down = E["up"], E["down"]
         ev = lambda st: (lambda e: (e.record(st), e)[1])(torch.cuda.Event())
-        L = dict(self.launches(main))
         start = ev(main)
         up.wait_event(start)
         down.wait_event(start)
@@ -253,23 +281,23 @@ class Workload:
         for s in E["up2"]:
             sph.sph_store_upload_sub(self.store, s, self.host[s], up)
         e2 = ev(up)
-        for k in ("density", "unpack_density_out"):
-            L[k]()
-        down.wait_event(ev(main))
-        for s in E["down1"]:
-            sph.sph_store_download_sub(self.store, s, self.host[s], down)
-        main.wait_event(e2)
-        L["ghost"]()
-        down.wait_event(ev(main))
-        for s in E["down2"]:
-            sph.sph_store_download_sub(self.store, s, self.host[s], down)
-        for k in ("pack_force_in", "force"):
-            L[k]()
+        waited = False
+        for k, fn in self.launches(main)[1:]:
+            if not waited and k in (E["up2_before"], "ghost"):        # the ghost reads u
+                main.wait_event(e2)
+                waited = True
+            if k == "unpack_force_out":
+                break
+            fn()
+            if E["down_after"].get(k):
+                down.wait_event(ev(main))
+                for s in E["down_after"][k]:
+                    sph.sph_store_download_sub(self.store, s, self.host[s], down)
         # the force results are reduced slab by slab; each slab's particles leave as soon as they are final
         for c0, nc, p0, npart in E["slabs"]:
             sph.sph_unpack_cells(st, b, S[3], B[3], c0, nc, sph.SPH_UNPACK_REDUCE_ZERO, main)
             down.wait_event(ev(main))
-            for s in E["down3"]:
+            for s in E["down_after"]["unpack_force_out"]:
                 sph.sph_store_download_range(st, s, self.host[s], p0, npart, down)
         main.wait_event(ev(down))
 
@@ -294,14 +322,24 @@ class Workload:
         field once per particle per launch (re-reads of a cell by its 27 tasks are cache hits, not algorithmic traffic)."""
         n, inst, cand = self.n, self.info.n_instances, self.info.n_candidates
         r = self.rec
-        return {
+        F = self.sph.FIELD
+        width = lambda f: 8 if f in (F["x"], F["id"]) else (1 if f == F["time_bin"] else 4)
+        fields_in = lambda k: sum(int(e.ncomp) * width(int(e.field)) for e in list(self.sets[k].ent)[:self.sets[k].n])      # store bytes read per particle
+        out = {
             "pack_density_in": {"bound": "hbm", "bytes": n * 32 + inst * r[0]},
             "unpack_density_out": {"bound": "hbm", "bytes": inst * r[1] + n * 16},       # REDUCE_ZERO: the fields are written, not read
-            "pack_force_in": {"bound": "hbm", "bytes": n * 64 + inst * r[2]},
             "unpack_force_out": {"bound": "hbm", "bytes": inst * r[3] + n * 20},
             "density": {"bound": "alu", "flop": cand * FLOP_CAND + n * NGB_CONFIG1 * FLOP_HIT_DENSITY},
             "force": {"bound": "alu", "flop": cand * FLOP_CAND + n * (NGB_CONFIG1 - 1) * FLOP_HIT_FORCE},
         }
+        if self.loops == 3:
+            out["pack_gradient_in"] = {"bound": "hbm", "bytes": n * fields_in(4) + inst * r[4]}
+            out["unpack_gradient_out"] = {"bound": "hbm", "bytes": inst * r[5] + n * 16}
+            out["pack_force_in"] = {"bound": "hbm", "bytes": n * fields_in(6) + inst * r[6]}
+            out["gradient"] = {"bound": "alu", "flop": cand * FLOP_CAND + n * (NGB_CONFIG1 - 1) * FLOP_HIT_GRADIENT}
+        else:
+            out["pack_force_in"] = {"bound": "hbm", "bytes": n * 64 + inst * r[2]}
+        return out
 
     def close(self):
         self.graph = None
@@ -375,8 +413,9 @@ def run_layouts(args):
     flush = lambda: flush_buf.fill_(1)
     sampler = ClockSampler(0)
     rows = {}
-    for name in layouts.NAMES:
-        w = Workload(sph, torch, ps, cells, tasks, name)
+    loops = args.loops
+    for name in (layouts.NAMES3 if loops == 3 else layouts.NAMES):
+        w = Workload(sph, torch, ps, cells, tasks, name, loops=loops)
         t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, 1)
         g_e2e = w.capture_e2e()
         t_e2e = time_steps(torch, g_e2e.replay, args.steps, args.warmup, flush, 1)
@@ -392,7 +431,7 @@ def run_layouts(args):
             for k, a, b in evs:
                 per[k].append(a.elapsed_time(b))
         per = {k: sum(v) / len(v) for k, v in per.items()}
-        pu = sum(per[k] for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out"))
+        pu = sum(v for k, v in per.items() if k.startswith(("pack_", "unpack_")))
         bi, bo = w.e2e_bytes()
         rows[name] = {"substructs": [int(w.layout.stride[s]) for s in range(w.layout.n_sub)], "ms_per_step": round(sum(t_ms) / len(t_ms), 5),
                       "pack_unpack_ms": round(pu, 5), "e2e_ms_per_step": round(sum(t_e2e) / len(t_e2e), 5), "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
@@ -408,11 +447,12 @@ def run_layouts(args):
     print(json.dumps({"metric": METRIC, "value": n / (rows[best]["ms_per_step"] * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": rows[best]["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f32", "data": "synthetic",
-                      "config": {"workload": WORKLOAD + "; every particle layout of the paper", "layout": best, "store": "HBM (step) / pinned host (e2e)",
+                      "config": {"workload": WORKLOAD + ("; three-loop cycle (density, gradient, switched force)" if loops == 3 else "") + "; every particle layout of the paper",
+                                 "layout": best, "loops": loops, "store": "HBM (step) / pinned host (e2e)",
                                  "l2": "flushed before every step (256 MB fill, untimed)"},
                       "e2e": {"value": n / (rows[best]["e2e_ms_per_step"] * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": rows[best]["h2d_bytes_per_step"],
                               "d2h_bytes_per_step": rows[best]["d2h_bytes_per_step"]},
-                      "gpu_launches": 7 * args.steps, "clocks": clocks, "roofline": None, "layouts": rows}))
+                      "gpu_launches": (10 if loops == 3 else 7) * args.steps, "clocks": clocks, "roofline": None, "layouts": rows}))
 
 
 def cpu_model():
@@ -534,7 +574,7 @@ def measure_config1(args, sph, torch, rank, world, local):
 
     results = {}
     for name in ([args.layout] if args.layout != "both" else ["split", "aos"]):
-        w = Workload(sph, torch, ps, cells, tasks, name)
+        w = Workload(sph, torch, ps, cells, tasks, name, loops=args.loops)
         sampler = ClockSampler(local) if rank == 0 else None
         t_ms = time_steps(torch, w.step, args.steps, args.warmup, flush, world)
         clocks = sampler.stop() if sampler else None
@@ -599,10 +639,10 @@ def measure_config1(args, sph, torch, rank, world, local):
         "pair_interactions_per_s": {"density": cand / (R["per"]["density"] * 1e-3), "force": cand / (R["per"]["force"] * 1e-3)},      # ordered candidate pairs
         "neighbour_pairs_per_s": {"density": total_particles / world * NGB_CONFIG1 / (R["per"]["density"] * 1e-3),                       # pairs inside the cut-off
                                   "force": total_particles / world * (NGB_CONFIG1 - 1) / (R["per"]["force"] * 1e-3)},
-        "instances_per_s": {k: w.info.n_instances / (R["per"][k] * 1e-3) for k in ("pack_density_in", "unpack_density_out", "pack_force_in", "unpack_force_out")},
+        "instances_per_s": {k: w.info.n_instances / (v * 1e-3) for k, v in R["per"].items() if k.startswith(("pack_", "unpack_"))},
         "e2e": {"value": total_particles / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
                 "ms_per_step": ms_e2e},
-        "gpu_launches": 7 * args.steps,
+        "gpu_launches": len(w.launches()) * args.steps,
         "clocks": R["clocks"],
         "roofline": roof,
         "kernels": kernels,
@@ -830,6 +870,7 @@ def main():
     ap.add_argument("--workload", default="default", choices=["default", "config1", "config2", "config3", "config4", "link", "layouts"],
                     help="default = configs[2] as the headline plus configs[1], [3], [4] as `workloads`; the others run one configuration "
                          "(bench_workloads.py describes them)")
+    ap.add_argument("--loops", type=int, default=2, choices=[2, 3], help="layouts / config1: the two-loop cycle or the three-loop cycle (density, gradient, force)")
     ap.add_argument("--no-workloads", action="store_true", help="default line: configs[2] only")
     ap.add_argument("--n3", type=int, default=0, help="default line: particle count of the configs[3] entry (default 2^24)")
     ap.add_argument("--n4", type=int, default=0, help="default line: particle count of the configs[4] entry (default 2^26)")

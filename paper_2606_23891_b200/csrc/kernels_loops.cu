@@ -27,6 +27,7 @@
 // Sums are accumulated per target in tile order = source order, so results are bit-reproducible run to run.
 #include "internal.h"
 #include "ptx.cuh"
+#include <type_traits>
 
 namespace sph {
 
@@ -522,8 +523,13 @@ gradient_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in,
 
 // ------------------------------------------------------------------------------------------------- force
 
+struct NoSwitchSmem {};
+struct SwitchSmem {
+    float tB[64];            // targets: Balsara factor (three-loop cycle only)
+    float sB[2 * kHalf];     // sources: the same
+};
 template <int RW>
-struct ForceWarpSmemT {
+struct ForceWarpSmemT : std::conditional<RW == 18, SwitchSmem, NoSwitchSmem>::type {
     FilterTile f;
     float4 ta[2 * kHalf];    // sources: x, y, z, 4 h^2           (entries 32 and 65: the dummy)
     float4 tb[2 * kHalf];    //          vx, vy, vz, m
@@ -536,8 +542,6 @@ struct ForceWarpSmemT {
     float src[2][32 * RW];   // landing areas of the source rounds (double-buffered)
     uint32_t act[64];        // the active targets of the flush
     uint64_t bar[2];         // [0]: the mbarrier the record fetches complete on
-    float tB[64];            // targets: Balsara factor (three-loop cycle only)
-    float sB[2 * kHalf];     // sources: the same
 };
 typedef ForceWarpSmemT<13> ForceWarpSmem;
 
@@ -619,6 +623,13 @@ __device__ __forceinline__ float balsara(const float* r) {      // r: a FORCE3_I
     return div * rcp_fast(div + rot + 1.0e-4f * r[12] * rcp_fast(r[3]));
 }
 
+// the Balsara factors of two targets (tgt) or two tile entries, packed; nothing without the switch
+template <bool SWITCH, class Smem>
+__device__ __forceinline__ u64 switch_pair(const Smem& sm, uint32_t a, uint32_t b, bool tgt) {
+    if constexpr (SWITCH) return tgt ? pack2(sm.tB[a], sm.tB[b]) : pack2(sm.sB[a], sm.sB[b]);
+    else return 0ull;
+}
+
 template <bool UNITS, bool SWITCH>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
@@ -635,7 +646,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         sm.ta[lane * kHalf + 32] = make_float4(kFar, kFar, kFar, 0.f);
         sm.tb[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
         sm.tc[lane * kHalf + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
-        sm.sB[lane * kHalf + 32] = 0.f;
+        if constexpr (SWITCH) sm.sB[lane * kHalf + 32] = 0.f;
     }
     const ForceConsts2 K{dup2(2.0f), dup2(1.0f), dup2(3.0f), dup2(-0.75f), dup2(0.5f), dup2(-0.5f), dup2(1.5f), dup2(kInvPi), dup2(-beta), dup2(-alpha)};
 
@@ -724,14 +735,14 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                 const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
                 const ForceTargets2 T{pack2(pA.x, pB.x), pack2(pA.y, pB.y), pack2(pA.z, pB.z), pack2(qA.x, qB.x), pack2(qA.y, qB.y), pack2(qA.z, qB.z),
                                       pack2(qA.w, qB.w), pack2(sA.x, sB.x), pack2(sA.y, sB.y), pack2(sA.z, sB.z), pack2(sA.w, sB.w), pA.w, pB.w,
-                                      SWITCH ? pack2(sm.tB[tA], sm.tB[tB]) : 0ull};
+                                      switch_pair<SWITCH>(sm, tA, tB, true)};
                 u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
                 float vsig0 = 0.f, vsig1 = 0.f;
                 auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
                     uint32_t ja, jb;
                     while (next_hits(dual, ma, mb, &ja, &jb)) {
                         const ForcePair2 o = force_pair2<SWITCH>(T, K, sm.ta[base + ja], sm.ta[base + jb], sm.tb[base + ja], sm.tb[base + jb], sm.tc[base + ja],
-                                                                 sm.tc[base + jb], SWITCH ? pack2(sm.sB[base + ja], sm.sB[base + jb]) : 0ull);
+                                                                 sm.tc[base + jb], switch_pair<SWITCH>(sm, base + ja, base + jb, false));
                         kahan2(ax, cx, o.fr, o.ex); kahan2(ay, cy, o.fr, o.ey); kahan2(az, cz, o.fr, o.ez);
                         du = fma2(o.dg, o.vr, du);
                         vsig0 = fmaxf(vsig0, o.vsa); vsig1 = fmaxf(vsig1, o.vsb);
@@ -786,12 +797,12 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                             e[q] = ebase + j;
                         }
                         const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
-                        const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w, SWITCH ? dup2(sm.tB[t]) : 0ull};
+                        const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w, switch_pair<SWITCH>(sm, t, t, true)};
                         u64 ax = 0, ay = 0, az = 0, du = 0;
                         float vsig = 0.f;
                         auto two = [&](uint32_t ja, uint32_t jb) {
                             const ForcePair2 o = force_pair2<SWITCH>(T, K, sm.ta[ja], sm.ta[jb], sm.tb[ja], sm.tb[jb], sm.tc[ja], sm.tc[jb],
-                                                                     SWITCH ? pack2(sm.sB[ja], sm.sB[jb]) : 0ull);
+                                                                     switch_pair<SWITCH>(sm, ja, jb, false));
                             ax = fma2(o.fr, o.ex, ax); ay = fma2(o.fr, o.ey, ay); az = fma2(o.fr, o.ez, az);
                             du = fma2(o.dg, o.vr, du);
                             vsig = fmaxf(vsig, fmaxf(o.vsa, o.vsb));

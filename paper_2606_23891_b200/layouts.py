@@ -26,9 +26,30 @@ GROUPS = {
 }
 NAMES = ["aos", "random-order", "split"] + list(GROUPS)
 
+# The three-loop cycle (density, gradient, force; reading C34) -- the paper's own three sAoS subflavours:
+#   GRADIENT_IN = {x, v, mass, h, u, rho} is a subset of FORCE3_IN = GRADIENT_IN + {rho_dh, P, c_s, div_v, rot_v, time_bin};
+#   DENSITY_IN = {x, h, mass} is a subset of both.
+#   pack-gradient  "all variables required for [the gradient pack] are placed into its associated struct, disadvantaging the
+#                  force packing loop's access thereof": the force pack gathers from two structs
+#   pack-force     every variable the force pack needs in one struct (92 bytes): the gradient and density packs gather out of it
+#   pack-shared    "all variables shared between those two operations in a separate 'shared' struct", applied to all three
+#                  packs: {x, h, mass} (all three), {v, u, rho} (gradient and force), the force-only rest
+#   *-type         every substruct further split by data type
+_REST3 = [["wcount", "wcount_dh"], ["a", "du_dt", "v_sig"]]
+_F_ONLY = ["rho_dh", "P", "c_s", "div_v", "rot_v"]
+GROUPS3 = {
+    "pack-gradient": [["x", "v", "mass", "h", "u", "rho"], _F_ONLY + ["time_bin"]] + _REST3 + [["id"]],
+    "pack-force": [["x", "h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s", "div_v", "rot_v", "time_bin"]] + _REST3 + [["id"]],
+    "pack-shared": [["x", "h", "mass"], ["v", "u", "rho"], _F_ONLY + ["time_bin"]] + _REST3 + [["id"]],
+    "pack-gradient-type": [["x"], ["v", "mass", "h", "u", "rho"], _F_ONLY, ["time_bin"]] + _REST3 + [["id"]],
+    "pack-force-type": [["x"], ["h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s", "div_v", "rot_v"], ["time_bin"]] + _REST3 + [["id"]],
+    "pack-shared-type": [["x"], ["h", "mass"], ["v", "u", "rho"], _F_ONLY, ["time_bin"]] + _REST3 + [["id"]],
+}
+NAMES3 = ["aos", "random-order", "split"] + list(GROUPS3)
 
-def layout(sph, name: str, seed: int = 1):
-    """the named layout as an sph_layout (sph = the binding module)"""
+
+def layout(sph, name: str, seed: int = 1, loops: int = 2):
+    """the named layout as an sph_layout (sph = the binding module); loops = 3 selects the three-loop groupings"""
     if name == "aos":
         return sph.sph_layout_aos()
     if name == "split":
@@ -36,4 +57,4 @@ def layout(sph, name: str, seed: int = 1):
     if name == "random-order":
         order = [AOS_ORDER[i] for i in np.random.default_rng(seed).permutation(len(AOS_ORDER))]
         return sph.sph_layout_from_groups([order], min_stride=[128])
-    return sph.sph_layout_from_groups(GROUPS[name])
+    return sph.sph_layout_from_groups((GROUPS3 if loops == 3 else GROUPS)[name])

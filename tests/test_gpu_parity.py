@@ -764,3 +764,19 @@ def test_three_loop_step_vs_oracle(name, layout):
     g = GpuCase(ps, cells, tasks, layout)
     check_three_loop(gpu_three_loop_step(g), ref, exempt)
     g.close()
+
+
+@pytest.mark.parametrize("variant", ["pack-gradient", "pack-force", "pack-shared", "pack-gradient-type", "pack-force-type", "pack-shared-type"])
+def test_three_loop_layout_variants(variant):
+    """The paper's three sAoS subflavours and their splits by type hold the same bytes as the AoS store after a
+    three-loop step: the layout moves nothing but addresses."""
+    from paper_2606_23891_b200 import layouts
+    ps, cells, tasks = case("ragged")
+    g0 = GpuCase(ps, cells, tasks, "aos")
+    ref = gpu_three_loop_step(g0)
+    g0.close()
+    g = GpuCase(ps, cells, tasks, layouts.layout(sph, variant, loops=3))
+    assert np.array_equal(canon(g.export()), canon(ps))
+    got = gpu_three_loop_step(g)
+    assert np.array_equal(canon(got), canon(ref)), variant
+    g.close()

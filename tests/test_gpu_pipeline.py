@@ -100,3 +100,56 @@ def test_pipeline_equals_one_stream_run_and_oracle(layout_name, mode):
         assert pl.d2h_bytes == (n * (16 + 20 + 24) if layout_name == "split" else n * 128)
     pl.close()
     hs.close()
+
+
+# ------------------------------------------------------------------ bench.py's end-to-end step (host-resident arrays, three streams, one graph)
+
+def _bench_layout_cases():
+    from paper_2606_23891_b200 import layouts
+    return [(n, 2) for n in layouts.NAMES] + [(n, 3) for n in layouts.NAMES3]
+
+
+@pytest.mark.parametrize("name,loops", _bench_layout_cases())
+def test_bench_e2e_step_equals_plain_step(name, loops):
+    """bench.Workload.step_e2e (uploads, slab-wise first pack / last unpack, downloads, cross-stream events, replayed as a CUDA graph)
+    leaves in the HOST mirrors exactly what the plain device-resident step leaves in the store -- for every layout, including those
+    where a later loop's inputs share a substruct with an earlier loop's outputs (pack-density, pack-gradient, ...: the upload must
+    be ordered before the unpack that writes that substruct).  The host mirrors start from garbage in every output field."""
+    import bench
+    import sph_inputs as si
+    parts = si.jittered_lattice(16, seed=11)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 4)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    hmax = np.full(cells.shape[0], ps["h"].max(), dtype=np.float32)
+    tasks, _, _ = sph.sph_tasks_build(cells, hmax)
+    w = bench.Workload(sph, torch, ps, cells, tasks, name, loops=loops)
+    w.step()
+    torch.cuda.synchronize()
+    ref = np.zeros(ps.shape[0], dtype=ps.dtype)
+    sph.sph_store_export_aos(w.store, ref)
+    w.close()
+    dirty = ps.copy()
+    rng = np.random.default_rng(5)
+    for k in ("rho", "rho_dh", "wcount", "wcount_dh", "P", "c_s", "du_dt", "v_sig", "div_v"):
+        dirty[k] = rng.standard_normal(ps.shape[0]).astype(np.float32)
+    for k in ("a", "rot_v"):
+        dirty[k] = rng.standard_normal((ps.shape[0], 3)).astype(np.float32)
+    w = bench.Workload(sph, torch, dirty, cells, tasks, name, loops=loops)      # host mirrors = dirty
+    g = w.capture_e2e()
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    # read the host mirrors back through a scratch store
+    scratch = sph.sph_store_create(w.layout, ps.shape[0])
+    for s_ in range(w.layout.n_sub):
+        sph.sph_store_upload_sub(scratch, s_, w.host[s_])
+    torch.cuda.synchronize()
+    got = np.zeros(ps.shape[0], dtype=ps.dtype)
+    sph.sph_store_export_aos(scratch, got)
+    sph.sph_store_destroy(scratch)
+    w.close()
+    outs = ["rho", "rho_dh", "wcount", "wcount_dh", "P", "c_s", "a", "du_dt", "v_sig"] + (["div_v", "rot_v"] if loops == 3 else [])
+    for k in outs:
+        assert np.array_equal(got[k].view(np.uint32), ref[k].view(np.uint32)), (name, loops, k)
+    for k in ("x", "v", "h", "mass", "u", "id", "time_bin"):
+        assert np.array_equal(got[k], ps[k]), (name, loops, k)

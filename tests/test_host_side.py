@@ -66,8 +66,8 @@ def test_paper_layout_variants():
     """random-order AoS, kernel-driven sAoS variants and their splits by type, via sph_layout_from_groups"""
     from paper_2606_23891_b200 import layouts
     sizes = {"x": 24, "v": 12, "a": 12, "rot_v": 12, "id": 8, "time_bin": 1}
-    for name in layouts.NAMES:
-        lay = layouts.layout(sph, name, seed=3)
+    for name, loops in [(n, 2) for n in layouts.NAMES] + [(n, 3) for n in layouts.NAMES3]:
+        lay = layouts.layout(sph, name, seed=3, loops=loops)
         sph.sph_layout_validate(lay)
         spans = {}
         for fname, f in sph.FIELD.items():
@@ -82,6 +82,18 @@ def test_paper_layout_variants():
     pf, pd = layouts.layout(sph, "pack-force"), layouts.layout(sph, "pack-density")
     assert pf.stride[pf.loc[sph.FIELD["x"]].sub] == 64 and pd.stride[pd.loc[sph.FIELD["x"]].sub] == 32
     assert {pf.loc[sph.FIELD[k]].sub for k in ("x", "h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s")} == {0}
+    # three-loop flavours: pack-gradient keeps the six gradient inputs in one 48-byte struct, pack-force all twelve
+    # force inputs in one, pack-shared puts what all three packs share, what gradient and force share and the force-only rest apart
+    F = sph.FIELD
+    G_IN = ("x", "v", "mass", "h", "u", "rho")
+    F_ONLY = ("rho_dh", "P", "c_s", "div_v", "rot_v", "time_bin")
+    pg, pf3, psh = (layouts.layout(sph, k, loops=3) for k in ("pack-gradient", "pack-force", "pack-shared"))
+    assert {pg.loc[F[k]].sub for k in G_IN} == {0} and pg.stride[0] == 56 and {pg.loc[F[k]].sub for k in F_ONLY} == {1}
+    assert {pf3.loc[F[k]].sub for k in G_IN + F_ONLY} == {0}
+    assert [len({psh.loc[F[k]].sub for k in grp}) for grp in (("x", "h", "mass"), ("v", "u", "rho"), F_ONLY)] == [1, 1, 1]
+    assert len({psh.loc[F[k]].sub for k in ("x", "v", "rho_dh")}) == 3
+    pgt = layouts.layout(sph, "pack-gradient-type", loops=3)
+    assert pgt.stride[pgt.loc[F["x"]].sub] == 24 and pgt.stride[pgt.loc[F["time_bin"]].sub] <= 4
     ro = layouts.layout(sph, "random-order", seed=3)
     assert ro.n_sub == 1 and ro.stride[0] == 128
     assert [ro.loc[f].off for f in range(18)] != [sph.sph_layout_aos().loc[f].off for f in range(18)]
