@@ -124,38 +124,49 @@ __device__ __forceinline__ FilterTarget filter_target(float x, float y, float z,
 // Phase 1 over the first `cnt` tile entries for the lane's targets: bit (31 - j) of m[0] = "source j may be a
 // neighbour of target A" (j < 32), m[1] likewise for sources 32..63; m[2], m[3] for target B (DUAL only).
 template <bool DUAL>
-__device__ __forceinline__ void filter_masks(const FilterTile& f, uint32_t cnt, const FilterTarget& A, const FilterTarget& B, uint32_t (&m)[4]) {
-    const uint32_t np = ((cnt + 3) & ~3u) >> 1, np0 = min(np, 16u);
-    uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
-    auto test2 = [&](uint32_t p, uint32_t& ma, uint32_t& mb) {
-        const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(&f.a[p]);
-        const ulonglong2 b = *reinterpret_cast<const ulonglong2*>(&f.b[p]);
-        const u64 ta = fma2(A.mx2, a.x, fma2(A.my2, a.y, fma2(A.mz2, b.x, add2(b.y, A.nt2))));
-        uint32_t lo, hi;
-        asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(ta));
-        ma = __funnelshift_l(lo, ma, 1);      // (m << 1) | sign(t_lo)
-        ma = __funnelshift_l(hi, ma, 1);
-        if constexpr (DUAL) {
-            const u64 tb = fma2(B.mx2, a.x, fma2(B.my2, a.y, fma2(B.mz2, b.x, add2(b.y, B.nt2))));
-            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(tb));
-            mb = __funnelshift_l(lo, mb, 1);
-            mb = __funnelshift_l(hi, mb, 1);
+__device__ __forceinline__ void filter_half(const FilterTile& f, uint32_t lo, uint32_t hi, const FilterTarget& A, const FilterTarget& B, uint32_t& ma, uint32_t& mb) {
+    // the tile is padded to a multiple of eight entries (tile_box): four packed source pairs per trip, no remainder loop
+#pragma unroll 1
+    for (uint32_t p0 = lo; p0 < hi; p0 += 4) {
+#pragma unroll
+        for (uint32_t k = 0; k < 4; ++k) {
+            const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(&f.a[p0 + k]);
+            const ulonglong2 b = *reinterpret_cast<const ulonglong2*>(&f.b[p0 + k]);
+            const u64 ta = fma2(A.mx2, a.x, fma2(A.my2, a.y, fma2(A.mz2, b.x, add2(b.y, A.nt2))));
+            uint32_t lo32, hi32;
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(lo32), "=r"(hi32) : "l"(ta));
+            ma = __funnelshift_l(lo32, ma, 1);      // (m << 1) | sign(t_lo)
+            ma = __funnelshift_l(hi32, ma, 1);
+            if constexpr (DUAL) {
+                const u64 tb = fma2(B.mx2, a.x, fma2(B.my2, a.y, fma2(B.mz2, b.x, add2(b.y, B.nt2))));
+                asm("mov.b64 {%0, %1}, %2;" : "=r"(lo32), "=r"(hi32) : "l"(tb));
+                mb = __funnelshift_l(lo32, mb, 1);
+                mb = __funnelshift_l(hi32, mb, 1);
+            }
         }
-    };
-    for (uint32_t p = 0; p < np0; p += 2) { test2(p, a0, b0); test2(p + 1, a0, b0); }
-    a0 <<= 32 - 2 * np0; b0 <<= 32 - 2 * np0;
-    if (np > 16) {
-        for (uint32_t p = 16; p < np; p += 2) { test2(p, a1, b1); test2(p + 1, a1, b1); }
-        a1 <<= 32 - 2 * (np - 16); b1 <<= 32 - 2 * (np - 16);
     }
-    m[0] = a0; m[1] = a1; m[2] = b0; m[3] = b1;
+}
+__device__ __forceinline__ void filter_masks(const FilterTile& f, uint32_t cnt, bool dual, const FilterTarget& A, const FilterTarget& B, uint32_t (&m)[4]) {
+    const uint32_t np = ((cnt + 7) & ~7u) >> 1;          // packed source pairs, a multiple of four
+    // ONE copy of each loop serves both tile halves: the loops' code must stay inside the SM's instruction cache (ncu: "no
+    // instruction" was the first stall reason of the r01 kernels, whose bodies were 85-115 KB)
+#pragma unroll 1
+    for (uint32_t h = 0; h < 2; ++h) {
+        const uint32_t lo = 16 * h, hi = min(np, lo + 16);
+        uint32_t ma = 0, mb = 0;
+        if (hi > lo) {
+            if (dual) filter_half<true>(f, lo, hi, A, B, ma, mb); else filter_half<false>(f, lo, hi, A, B, ma, mb);
+            ma <<= 32 - 2 * (hi - lo); mb <<= 32 - 2 * (hi - lo);
+        }
+        if (h == 0) { m[0] = ma; m[2] = mb; } else { m[1] = ma; m[3] = mb; }
+    }
 }
 
-// pads the filter tile to a multiple of four entries and returns the bounding box of its first cnt sources
+// pads the filter tile to a multiple of eight entries and returns the bounding box of its first cnt sources
 struct Box { float lox, hix, loy, hiy, loz, hiz; };
 __device__ __forceinline__ Box tile_box(FilterTile& f, uint32_t cnt, uint32_t lane) {
-    const uint32_t n4 = (cnt + 3) & ~3u;
-    if (lane < n4 - cnt) filter_put(f, cnt + lane, 0.f, 0.f, 0.f, kNever);
+    const uint32_t n8 = (cnt + 7) & ~7u;
+    if (lane < n8 - cnt) filter_put(f, cnt + lane, 0.f, 0.f, 0.f, kNever);
     __syncwarp();
     // entries lane and lane + 32 of the tile
     const float* a = reinterpret_cast<const float*>(&f.a[lane >> 1]) + (lane & 1);
@@ -270,7 +281,7 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
             const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - 4.0f * pA.w * pA.w - eps : kNever);
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - 4.0f * pB.w * pB.w - eps : kNever);
             uint32_t m[4];
-            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            filter_masks(sm.f, cnt, dual, fA, fB, m);
             const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
             u64 s_mw = 0, s_mg = 0, s_w = 0, s_g = 0;
             // phase 2 over one half of the tile
@@ -295,8 +306,8 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
                     s_w = add2(s_w, w); s_g = add2(s_g, g);
                 }
             };
-            hits(m[0], m[2], sm.tile);
-            if (cnt > 32) hits(m[1], m[3], sm.tile + kHalf);
+#pragma unroll 1
+            for (uint32_t h = 0; h < 2 && 32 * h < cnt; ++h) hits(h ? m[1] : m[0], h ? m[3] : m[2], sm.tile + h * kHalf);
             float mw0, mw1, mg0, mg1, w0, w1, g0, g1;
             unpack2(s_mw, mw0, mw1); unpack2(s_mg, mg0, mg1); unpack2(s_w, w0, w1); unpack2(s_g, g0, g1);
             if (dual) {
@@ -311,34 +322,37 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
 
         uint32_t cnt = 0;
         const uint32_t n_rounds = max(1u, (n_s + 31) >> 5);
-        for (uint32_t r = 0; r < n_rounds; ++r) {
-            const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
-            if (r > 0) { cp_async_wait_all(); __syncwarp(); }
-            // one step ahead: the next round of this item, or the next item's targets and first round
-            if (r + 1 < n_rounds) {
-                fetch_records<5, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 20, min(32u, n_s - j0 - 32), lane);
-            } else if (has_next) {
-                fetch_records<5, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
-                fetch_records<5, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
-            }
+        // round n_rounds is the closing one: nothing new, what is left in the tile is flushed (one flush site: code size)
+        for (uint32_t r = 0; r <= n_rounds; ++r) {
             float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
             bool ok = false;
-            if (lane < nj) {
-                const float* rec = sm.src[buf] + 5 * lane;
-                s = make_float4(rec[0], rec[1], rec[2], rec[4]);
-                ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
+            uint32_t ball = 0, c = 0;
+            if (r < n_rounds) {
+                const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
+                if (r > 0) { cp_async_wait_all(); __syncwarp(); }
+                // one step ahead: the next round of this item, or the next item's targets and first round
+                if (r + 1 < n_rounds) {
+                    fetch_records<5, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 20, min(32u, n_s - j0 - 32), lane);
+                } else if (has_next) {
+                    fetch_records<5, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+                    fetch_records<5, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
+                }
+                if (lane < nj) {
+                    const float* rec = sm.src[buf] + 5 * lane;
+                    s = make_float4(rec[0], rec[1], rec[2], rec[4]);
+                    ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
+                }
+                ball = __ballot_sync(kFull, ok); c = __popc(ball);
             }
-            const uint32_t ball = __ballot_sync(kFull, ok), c = __popc(ball);
-            if (cnt + c > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
+            if (cnt + c > kTile || (r == n_rounds && cnt)) { flush(cnt); __syncwarp(); cnt = 0; }
             if (ok) {
                 const uint32_t pos = cnt + __popc(ball & lt);
                 sm.tile[pos + (pos >> 5)] = s;        // half * 33 + index in the half
                 filter_put(sm.f, pos, s.x, s.y, s.z, fmaf(s.x, s.x, fmaf(s.y, s.y, s.z * s.z)));
             }
             cnt += c;
-            buf ^= 1;
+            buf ^= r < n_rounds;
         }
-        if (cnt) flush(cnt);
         __syncwarp();
         if (vA) {
             const float ih = rcp_fast(oA.w), n3 = kInvPi * ih * ih * ih, n4 = n3 * ih;
@@ -428,7 +442,7 @@ gradient_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in,
             const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - 4.0f * pA.w * pA.w - eps : kNever);
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - 4.0f * pB.w * pB.w - eps : kNever);
             uint32_t m[4];
-            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            filter_masks(sm.f, cnt, dual, fA, fB, m);
             const u64 x2 = pack2(pA.x, pB.x), y2 = pack2(pA.y, pB.y), z2 = pack2(pA.z, pB.z);
             const u64 vx2 = pack2(qA.x, qB.x), vy2 = pack2(qA.y, qB.y), vz2 = pack2(qA.z, qB.z), ih2 = pack2(inv_hA, inv_hB);
             u64 s_d = 0, s_x = 0, s_y = 0, s_z = 0;
@@ -461,8 +475,8 @@ gradient_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in,
                     s_z = fma2(g, sub2(mul2(dx, wy), mul2(dy, wx)), s_z);
                 }
             };
-            hits(m[0], m[2], 0);
-            if (cnt > 32) hits(m[1], m[3], kHalf);
+#pragma unroll 1
+            for (uint32_t h = 0; h < 2 && 32 * h < cnt; ++h) hits(h ? m[1] : m[0], h ? m[3] : m[2], h * kHalf);
             float d0, d1, x0, x1, y0, y1, z0, z1;
             unpack2(s_d, d0, d1); unpack2(s_x, x0, x1); unpack2(s_y, y0, y1); unpack2(s_z, z0, z1);
             if (dual) {
@@ -477,34 +491,36 @@ gradient_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in,
 
         uint32_t cnt = 0;
         const uint32_t n_rounds = max(1u, (n_s + 31) >> 5);
-        for (uint32_t r = 0; r < n_rounds; ++r) {
-            const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
-            if (r > 0) { cp_async_wait_all(); __syncwarp(); }
-            if (r + 1 < n_rounds) {
-                fetch_records<10, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 40, min(32u, n_s - j0 - 32), lane);
-            } else if (has_next) {
-                fetch_records<10, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
-                fetch_records<10, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
-            }
+        for (uint32_t r = 0; r <= n_rounds; ++r) {      // round n_rounds: the closing flush (one flush site)
             float4 s = make_float4(0.f, 0.f, 0.f, 0.f), sv = s;
             bool ok = false;
-            if (lane < nj) {
-                const float* rec = sm.src[buf] + 10 * lane;
-                s = make_float4(rec[0], rec[1], rec[2], 0.f);
-                ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
-                if (ok) { s.w = rec[6] * rcp_fast(rec[9]); sv = make_float4(rec[3], rec[4], rec[5], 0.f); }
+            uint32_t ball = 0, c = 0;
+            if (r < n_rounds) {
+                const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
+                if (r > 0) { cp_async_wait_all(); __syncwarp(); }
+                if (r + 1 < n_rounds) {
+                    fetch_records<10, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 40, min(32u, n_s - j0 - 32), lane);
+                } else if (has_next) {
+                    fetch_records<10, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+                    fetch_records<10, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
+                }
+                if (lane < nj) {
+                    const float* rec = sm.src[buf] + 10 * lane;
+                    s = make_float4(rec[0], rec[1], rec[2], 0.f);
+                    ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
+                    if (ok) { s.w = rec[6] * rcp_fast(rec[9]); sv = make_float4(rec[3], rec[4], rec[5], 0.f); }
+                }
+                ball = __ballot_sync(kFull, ok); c = __popc(ball);
             }
-            const uint32_t ball = __ballot_sync(kFull, ok), c = __popc(ball);
-            if (cnt + c > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
+            if (cnt + c > kTile || (r == n_rounds && cnt)) { flush(cnt); __syncwarp(); cnt = 0; }
             if (ok) {
                 const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);
                 sm.tile[e] = s; sm.tilev[e] = sv;
                 filter_put(sm.f, pos, s.x, s.y, s.z, fmaf(s.x, s.x, fmaf(s.y, s.y, s.z * s.z)));
             }
             cnt += c;
-            buf ^= 1;
+            buf ^= r < n_rounds;
         }
-        if (cnt) flush(cnt);
         __syncwarp();
         if (vA) {
             const float ih = rcp_fast(oA.w), n4 = kInvPi * (ih * ih) * (ih * ih);
@@ -713,7 +729,7 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const FilterTarget fA = filter_target(pA.x, pA.y, pA.z, wA ? fmaf(pA.x, pA.x, fmaf(pA.y, pA.y, pA.z * pA.z)) - cutA - kFilterEps * (b2 + cutA) : kNever);
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - cutB - kFilterEps * (b2 + cutB) : kNever);
             uint32_t m[4];
-            if (dual) filter_masks<true>(sm.f, cnt, fA, fB, m); else filter_masks<false>(sm.f, cnt, fA, fB, m);
+            filter_masks(sm.f, cnt, dual, fA, fB, m);
             // Phase 2, two ways (two instantiations of the kernel; the launcher picks one from the batch's mean block size).
             //  WALK: every lane walks the set bits of its own targets' masks, one neighbour of target A and one of target B per
             //        iteration (or two of target A when it has one target).  Best when the targets have about as many neighbours
@@ -748,8 +764,8 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                         vsig0 = fmaxf(vsig0, o.vsa); vsig1 = fmaxf(vsig1, o.vsb);
                     }
                 };
-                hits(m[0], m[2], 0);
-                if (cnt > 32) hits(m[1], m[3], kHalf);
+#pragma unroll 1
+                for (uint32_t h = 0; h < 2 && 32 * h < cnt; ++h) hits(h ? m[1] : m[0], h ? m[3] : m[2], h * kHalf);
                 unpack2(ax, axA, axB); unpack2(ay, ayA, ayB); unpack2(az, azA, azB); unpack2(du, duA, duB);
                 vsA = vsig0; vsB = vsig1;
                 if (!dual) { axA += axB; ayA += ayB; azA += azB; duA += duB; vsA = fmaxf(vsA, vsB); }
@@ -789,13 +805,6 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                         const bool valid = u < cum;
                         uint32_t um = valid ? upos[u] : 0u;
                         const uint32_t tw = valid ? utgt[u] : 0u, t = tw & 127u, ebase = (tw >> 7) * kHalf;
-                        uint32_t e[kUnitBits];      // tile entries of the unit's neighbours; a slot without one points at its half's dummy (entry 32)
-#pragma unroll
-                        for (int q = 0; q < kUnitBits; ++q) {
-                            const uint32_t j = __clz(um);
-                            um &= ~shr_clamp(0x80000000u, j);
-                            e[q] = ebase + j;
-                        }
                         const float4 P = sm.t0[t], Q = sm.t1[t], S = sm.t2[t];
                         const ForceTargets2 T{dup2(P.x), dup2(P.y), dup2(P.z), dup2(Q.x), dup2(Q.y), dup2(Q.z), dup2(Q.w), dup2(S.x), dup2(S.y), dup2(S.z), dup2(S.w), P.w, P.w, switch_pair<SWITCH>(sm, t, t, true)};
                         u64 ax = 0, ay = 0, az = 0, du = 0;
@@ -807,10 +816,15 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                             du = fma2(o.dg, o.vr, du);
                             vsig = fmaxf(vsig, fmaxf(o.vsa, o.vsb));
                         };
-                        two(e[0], e[1]);
+                        // the unit's neighbours two by two; a slot without one points at its half's dummy (entry 32)
 #pragma unroll
-                        for (int q = 2; q < kUnitBits; q += 2)
-                            if (__any_sync(kFull, e[q] != ebase + 32u)) two(e[q], e[q + 1]);
+                        for (uint32_t q = 0; q < kUnitBits; q += 2) {
+                            const uint32_t j0 = __clz(um);
+                            um &= ~shr_clamp(0x80000000u, j0);
+                            const uint32_t j1 = __clz(um);
+                            um &= ~shr_clamp(0x80000000u, j1);
+                            if (q == 0 || __any_sync(kFull, j0 != 32u)) two(ebase + j0, ebase + j1);
+                        }
                         if (valid) {
                             float ax0, ax1, ay0, ay1, az0, az1, du0, du1;
                             unpack2(ax, ax0, ax1); unpack2(ay, ay0, ay1); unpack2(az, az0, az1); unpack2(du, du0, du1);
@@ -852,40 +866,44 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
 
         uint32_t cnt = 0;
         const uint32_t n_rounds = max(1u, (n_s + 31) >> 5);
-        for (uint32_t r = 0; r < n_rounds; ++r) {
-            const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
-            if (r > 0) fg.wait();
-            // one step ahead: the next round of this item (the next item's records are fetched once the results have left sm.raw)
-            if (r + 1 < n_rounds) fg.issue1(lane, sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * (RW * 4), rec_bytes16<RW>(min(32u, n_s - j0 - 32)));
+        for (uint32_t r = 0; r <= n_rounds; ++r) {      // round n_rounds: the closing flush (one flush site: code size)
             float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
             float s2 = 0.f;
             bool ok = false;
-            if (lane < nj) {
-                const float* rec = sm.src[buf] + RW * lane;
-                const float h = rec[3], rho = rec[5];
-                const float reach = fmaxf(reach_t, 2.0f * h) * kReachSlack;
-                a = make_float4(rec[0], rec[1], rec[2], 4.0f * h * h);
-                ok = a.x > lox - reach && a.x < hix + reach && a.y > loy - reach && a.y < hiy + reach && a.z > loz - reach && a.z < hiz + reach;
-                if (ok) {
-                    b = make_float4(rec[7], rec[8], rec[9], rec[4]);
-                    c = make_float4(rho, rec[11] * rcp_fast(fmaf(h * rec[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho), rec[12], rcp_fast(h));
-                    s2 = fmaf(a.x, a.x, fmaf(a.y, a.y, a.z * a.z));
+            uint32_t ball = 0, n_ok = 0;
+            if (r < n_rounds) {
+                const uint32_t j0 = 32 * r, nj = min(32u, n_s - j0);
+                if (r > 0) fg.wait();
+                // one step ahead: the next round of this item (the next item's records are fetched once the results have left sm.raw)
+                if (r + 1 < n_rounds) fg.issue1(lane, sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * (RW * 4), rec_bytes16<RW>(min(32u, n_s - j0 - 32)));
+                if (lane < nj) {
+                    const float* rec = sm.src[buf] + RW * lane;
+                    const float h = rec[3], rho = rec[5];
+                    const float reach = fmaxf(reach_t, 2.0f * h) * kReachSlack;
+                    a = make_float4(rec[0], rec[1], rec[2], 4.0f * h * h);
+                    ok = a.x > lox - reach && a.x < hix + reach && a.y > loy - reach && a.y < hiy + reach && a.z > loz - reach && a.z < hiz + reach;
+                    if (ok) {
+                        b = make_float4(rec[7], rec[8], rec[9], rec[4]);
+                        c = make_float4(rho, rec[11] * rcp_fast(fmaf(h * rec[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho), rec[12], rcp_fast(h));
+                        s2 = fmaf(a.x, a.x, fmaf(a.y, a.y, a.z * a.z));
+                    }
                 }
+                ball = __ballot_sync(kFull, ok); n_ok = __popc(ball);
             }
-            const uint32_t ball = __ballot_sync(kFull, ok), n_ok = __popc(ball);
-            if (cnt + n_ok > kTile) { flush(cnt); __syncwarp(); cnt = 0; }
-            if (ok) {
-                const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);      // half * 33 + index in the half
-                sm.ta[e] = a; sm.tb[e] = b; sm.tc[e] = c;
-                if constexpr (SWITCH) sm.sB[e] = balsara(sm.src[buf] + RW * lane);
-                filter_put(sm.f, pos, a.x, a.y, a.z, s2);
+            if (cnt + n_ok > kTile || (r == n_rounds && cnt)) { flush(cnt); __syncwarp(); cnt = 0; }
+            if (r < n_rounds) {
+                if (ok) {
+                    const uint32_t pos = cnt + __popc(ball & lt), e = pos + (pos >> 5);      // half * 33 + index in the half
+                    sm.ta[e] = a; sm.tb[e] = b; sm.tc[e] = c;
+                    if constexpr (SWITCH) sm.sB[e] = balsara(sm.src[buf] + RW * lane);
+                    filter_put(sm.f, pos, a.x, a.y, a.z, s2);
+                }
+                tile_hc2 = fmaxf(tile_hc2, warp_max_pos(ok ? a.w : 0.f));
+                tile_b2 = fmaxf(tile_b2, warp_max_pos(s2));
+                cnt += n_ok;
+                buf ^= 1;
             }
-            tile_hc2 = fmaxf(tile_hc2, warp_max_pos(ok ? a.w : 0.f));
-            tile_b2 = fmaxf(tile_b2, warp_max_pos(s2));
-            cnt += n_ok;
-            buf ^= 1;
         }
-        if (cnt) flush(cnt);
         __syncwarp();
         // the running results are already in FORCE_OUT record layout: they leave as coalesced 16-byte stores
         const uint32_t nvec = (n_t * 5 + 3) >> 2;
