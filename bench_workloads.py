@@ -5,6 +5,8 @@
                                            memory, mapped zero-copy versus stage-then-H2D, AoS and split-AoS
     python bench.py --workload config4     2^26 particles, whole step streamed in bundles of 4,096 tasks over 2 streams, store in pinned host memory
     python bench.py --workload link        pinned H2D / D2H / both-ways copy bandwidth of this box (the host-link roofline)
+    python bench.py --workload eagle       Eagle25-like occupancies (5 .. 125,113 per cell): whole step, every stage timed, load-balance figures
+    python bench.py --workload replay      pack / unpack calls replayed from a seeded synthetic trace of offload actions, per layout
 
 `--n N` shrinks the particle count (a power of two for config3/4, N = planes * 128 * 128 is kept for config2) for quick
 runs; the default is the full size of BASELINE.json.  Everything here is harness: the path itself runs in libsph_b200.
@@ -754,10 +756,160 @@ def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
                     "d2h_bytes_per_step": P["d2h_bytes_per_step"], "ms_per_step": P["ms_per_step"]}}
 
 
+# ------------------------------------------------------------------------------------------------- extreme occupancy, trace replay (8(f3))
+
+def build_eagle(sph, seed, cells_per_dim, n_max=125113):
+    """Eagle25-like occupancies (per cell min 5 / max 125,113 / mean 184 / median 109) on a grid of equal cells"""
+    import sph_inputs as si
+    parts = si.eagle_like(seed=seed, cells_per_dim=cells_per_dim, n_max=n_max)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], cells_per_dim)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    del parts
+    hmax = np.maximum.reduceat(ps["h"], cells["first"].astype(np.int64)).astype(np.float32)
+    tasks, n_self, n_pair = sph.sph_tasks_build(cells, hmax)
+    cnt = cells["count"]
+    info = {"particles": int(ps.shape[0]), "cells": int(cells.shape[0]), "per_cell_min": int(cnt.min()), "per_cell_max": int(cnt.max()),
+            "per_cell_mean": round(float(cnt.mean()), 1), "per_cell_median": float(np.median(cnt)), "self_tasks": int(n_self), "pair_tasks": int(n_pair)}
+    return ps, cells, tasks, info
+
+
+def run_eagle(args, sph, torch, common):
+    """whole step (density cycle, ghost, force cycle) on the extreme-occupancy set, every stage timed, AoS beside split-AoS"""
+    cpd = 32 if not args.n else max(3, int(round((args.n / 190.0) ** (1.0 / 3.0))))
+    ps, cells, tasks, setup = build_eagle(sph, 1, cpd)
+    n = ps.shape[0]
+    params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
+    sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+    res = {}
+    for name in ("split", "aos"):
+        layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
+        store = sph.sph_store_create(layout, n)
+        sph.sph_store_set_cells(store, cells)
+        sph.sph_store_import_aos(store, ps)
+        batch = sph.sph_batch_create(store, tasks)
+        info = sph.sph_batch_get_info(batch)
+        bufs = [torch.empty(sph.sph_batch_buffer_bytes(batch, s), dtype=torch.uint8, device="cuda") for s in sets]
+        Z = sph.SPH_UNPACK_REDUCE_ZERO
+        stages = [("pack_density_in", lambda: sph.sph_pack(store, batch, sets[0], bufs[0])),
+                  ("density", lambda: sph.sph_density(batch, bufs[0], bufs[1])),
+                  ("unpack_density_out", lambda: sph.sph_unpack(store, batch, sets[1], bufs[1], Z)),
+                  ("ghost", lambda: sph.sph_ghost(store, params)),
+                  ("pack_force_in", lambda: sph.sph_pack(store, batch, sets[2], bufs[2])),
+                  ("force", lambda: sph.sph_force(batch, bufs[2], bufs[3], params)),
+                  ("unpack_force_out", lambda: sph.sph_unpack(store, batch, sets[3], bufs[3], Z))]
+        step = lambda: [fn() for _, fn in stages]
+        t = timed(torch, step, args.steps, min(args.warmup, 3))
+        per = {k: [] for k, _ in stages}
+        for _ in range(args.steps):
+            torch.cuda.synchronize()
+            for k, fn in stages:
+                per[k].append(ev_time(torch, fn))
+        per = {k: round(sum(v) / len(v), 4) for k, v in per.items()}
+        inst, cand = int(info.n_instances), int(info.n_candidates)
+        resident_warps = 148 * 16
+        res[name] = {"ms_per_step": sum(t) / len(t), "stages_ms": per, "instances_per_loop": inst, "candidate_pairs_per_loop": cand,
+                     "loop_items": int(info.n_items), "largest_item_candidates": int(info.max_item_candidates),
+                     "largest_item_share_of_candidates": info.max_item_candidates / cand,
+                     "largest_item_over_mean_warp_load": info.max_item_candidates / (cand / resident_warps),
+                     "candidate_pairs_per_s": {"density": cand / (per["density"] * 1e-3), "force": cand / (per["force"] * 1e-3)},
+                     "instances_per_s": {k: inst / (per[k] * 1e-3) for k in per if k.startswith(("pack_", "unpack_"))}}
+        sph.sph_batch_destroy(batch)
+        sph.sph_store_destroy(store)
+        del bufs
+    P = res["split"]
+    return {"value": n / (P["ms_per_step"] * 1e-3), "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
+            "config": {"workload": f"eagle-like: {n} particles in {cpd}^3 cells of 5 .. {setup['per_cell_max']} particles (PAPER.md:164 statistics), "
+                                   "density cycle, ghost, force cycle, one batch, store in HBM", "layout": "split", "store": "HBM",
+                       "l2": "inputs larger than L2", "setup": setup},
+            "gpu_launches": 7 * args.steps, "roofline": None, "split": P, "aos": res["aos"], "e2e": None}
+
+
+def synthetic_trace(n_tasks, n_self, seed, steps=5, bundle_lo=128, bundle_hi=1024):
+    """A seeded stand-in for a recorded trace of offload actions: per simulation step the self tasks, then
+    the pair tasks, are cut into bundles of seeded sizes; every bundle is packed and later unpacked, density before force.
+    -> list of (step, loop, action, first task, task count)"""
+    rng = np.random.default_rng(seed)
+    trace = []
+    for st in range(steps):
+        cuts = []
+        for lo, hi in ((0, n_self), (n_self, n_tasks)):
+            t = lo
+            while t < hi:
+                m = int(min(hi - t, rng.integers(bundle_lo, bundle_hi + 1)))
+                cuts.append((t, m))
+                t += m
+        for loop in ("density", "force"):
+            for t0, m in cuts:
+                trace.append((st, loop, "pack", t0, m))
+                trace.append((st, loop, "unpack", t0, m))
+    return trace
+
+
+def run_replay(args, sph, torch, common):
+    """pack / unpack calls replayed from a synthetic trace (the spirit of SWIFTGPUPACKSIM; real traces are
+    not available): one call per recorded action, no interaction loop in between, for every layout asked for"""
+    from paper_2606_23891_b200 import layouts as L
+    cpd = 16 if not args.n else max(3, int(round((args.n / 190.0) ** (1.0 / 3.0))))
+    ps, cells, tasks, setup = build_eagle(sph, 2, cpd)
+    n = ps.shape[0]
+    n_self = setup["self_tasks"]
+    trace = synthetic_trace(tasks.shape[0], n_self, seed=7)
+    names = ["aos", "split", "pack-force", "pack-force-type"] if args.layout == "both" else [args.layout]
+    sets = {("density", "pack"): sph.sph_attrset_canonical(0), ("density", "unpack"): sph.sph_attrset_canonical(1),
+            ("force", "pack"): sph.sph_attrset_canonical(2), ("force", "unpack"): sph.sph_attrset_canonical(3)}
+    rows = {}
+    for name in names:
+        layout = sph.sph_layout_aos() if name == "aos" else (sph.sph_layout_split() if name == "split" else L.layout(sph, name))
+        store = sph.sph_store_create(layout, n)
+        sph.sph_store_set_cells(store, cells)
+        sph.sph_store_import_aos(store, ps)
+        batches = {}
+        need = {k: 0 for k in sets}
+        inst = {"pack": 0, "unpack": 0}
+        for _, loop, action, t0, m in trace:
+            if (t0, m) not in batches:
+                batches[(t0, m)] = sph.sph_batch_create(store, tasks[t0:t0 + m])
+            b = batches[(t0, m)]
+            need[(loop, action)] = max(need[(loop, action)], sph.sph_batch_buffer_bytes(b, sets[(loop, action)]))
+            inst[action] += int(sph.sph_batch_get_info(b).n_instances)
+        bufs = {k: torch.zeros(max(v, 256), dtype=torch.uint8, device="cuda") for k, v in need.items()}
+
+        def replay(only=None):
+            for _, loop, action, t0, m in trace:
+                if only and action != only:
+                    continue
+                b, key = batches[(t0, m)], (loop, action)
+                if action == "pack":
+                    sph.sph_pack(store, b, sets[key], bufs[key])
+                else:
+                    sph.sph_unpack(store, b, sets[key], bufs[key], sph.SPH_UNPACK_REDUCE)
+        t_all = min(timed(torch, replay, args.steps, 2))
+        t_pack = min(timed(torch, lambda: replay("pack"), args.steps, 1))
+        t_unpack = min(timed(torch, lambda: replay("unpack"), args.steps, 1))
+        rows[name] = {"ms_all": round(t_all, 3), "ms_pack": round(t_pack, 3), "ms_unpack": round(t_unpack, 3), "calls": len(trace),
+                      "pack_instances_per_s": inst["pack"] / (t_pack * 1e-3), "unpack_instances_per_s": inst["unpack"] / (t_unpack * 1e-3),
+                      "us_per_call": round(1e3 * t_all / len(trace), 2)}
+        for b in batches.values():
+            sph.sph_batch_destroy(b)
+        sph.sph_store_destroy(store)
+        del bufs
+    base = rows.get("aos", next(iter(rows.values())))
+    for r in rows.values():
+        r["vs_aos"] = round(r["ms_all"] / base["ms_all"], 3)
+    best = min(rows, key=lambda k: rows[k]["ms_all"])
+    total_inst = (rows[best]["pack_instances_per_s"] * rows[best]["ms_pack"] + rows[best]["unpack_instances_per_s"] * rows[best]["ms_unpack"]) * 1e-3
+    return {"value": total_inst / (rows[best]["ms_all"] * 1e-3), "unit": "instances/s", "ms_per_step": rows[best]["ms_all"], "dtype": "u8",
+            "metric": "particles/s packed + unpacked, trace replay",
+            "config": {"workload": f"replay: synthetic trace of {len(trace)} pack / unpack actions (5 steps, bundles of 128..1024 tasks, density then force) over "
+                                   f"{n} particles in {cpd}^3 cells of 5 .. {setup['per_cell_max']} particles; one call per action, no loops", "layout": best,
+                       "store": "HBM", "l2": "inputs larger than L2", "setup": setup},
+            "gpu_launches": len(trace) * args.steps, "roofline": None, "layouts": rows, "e2e": None}
+
+
 def run_link(args, sph, torch, common):
     link = link_probe(torch, reps=10)
     return {"value": link["h2d_gbs"], "unit": "GB/s", "ms_per_step": None, "dtype": "u8", "metric": "pinned host-link copy bandwidth",
             "config": {"workload": "link: 1 GiB pinned cudaMemcpyAsync, best of 10", "link": link}, "gpu_launches": 0, "roofline": None, "e2e": None}
 
 
-RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link}
+RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link, "eagle": run_eagle, "replay": run_replay}

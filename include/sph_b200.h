@@ -117,6 +117,8 @@ typedef struct {
     uint64_t n_cells_touched;
     uint32_t n_segments;
     uint32_t max_count;      /* largest block */
+    uint64_t n_items;              /* work items of an interaction loop: (<= 64 targets of a block) x (the block they gather from) */
+    uint64_t max_item_candidates;  /* candidate pairs of the largest item: what one warp works through alone (load balance) */
 } sph_batch_info;
 
 /* ---- errors ---- */

@@ -156,6 +156,21 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
                     forc3.push_back(LoopItem{(uint32_t)(o72[tgt] / 128) + kc * 18 * u, (uint32_t)(o72[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns});
                 }
             }
+        // Longest first (occupancies of 5 .. 10^5 per cell).  Warps take items round-robin, so with
+        // items in descending cost every warp gets a similar mix and the one 10^5 x 10^5 task starts at once instead of being
+        // the tail.  Cost classes are powers of two of targets x sources and the sort is stable: inside a class the order stays
+        // cell-major, and a batch whose items all cost the same (grids of equal cells) keeps its order.
+        {
+            auto cls = [](const LoopItem& it) { const uint64_t c = (uint64_t)(it.nt_ns & 127u) * (it.nt_ns >> 7); int k = 0; while ((c >> k) > 1) ++k; return k; };
+            std::vector<uint32_t> order(dens.size());
+            for (uint32_t i = 0; i < order.size(); ++i) order[i] = i;
+            std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return cls(dens[x]) > cls(dens[y]); });
+            auto apply = [&](std::vector<LoopItem>& v) { std::vector<LoopItem> w(v.size()); for (size_t i = 0; i < v.size(); ++i) w[i] = v[order[i]]; v.swap(w); };
+            apply(dens); apply(forc); apply(grad); apply(forc3);
+            uint64_t worst = 0;
+            for (const LoopItem& it : dens) worst = std::max(worst, (uint64_t)(it.nt_ns & 127u) * (it.nt_ns >> 7));
+            b->max_item_candidates = worst;
+        }
         b->n_items = (uint32_t)dens.size();
         if (int32_t rc = upload(dens, &b->d_items_density)) return rc;
         if (int32_t rc = upload(forc, &b->d_items_force)) return rc;
@@ -180,7 +195,7 @@ int32_t sph_batch_get_info(const sph_batch* b, sph_batch_info* info) {
     if (!b || !info) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
     info->n_tasks = b->n_tasks; info->n_self = b->n_self; info->n_pair = b->n_pair; info->n_sides = b->n_sides;
     info->n_instances = b->n_instances; info->n_candidates = b->n_candidates; info->n_cells_touched = b->n_cells_touched;
-    info->n_segments = b->n_segments; info->max_count = b->max_count;
+    info->n_segments = b->n_segments; info->max_count = b->max_count; info->n_items = b->n_items; info->max_item_candidates = b->max_item_candidates;
     return SPH_OK;
 }
 

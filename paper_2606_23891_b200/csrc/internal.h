@@ -141,7 +141,7 @@ struct sph_store {
 struct sph_batch {
     uint64_t n_tasks = 0, n_self = 0, n_pair = 0;
     uint32_t n_sides = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
-    uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0;
+    uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0, max_item_candidates = 0;
     uint64_t cells_hash = 0;                  // of the cell table the batch was built against
     std::vector<sph::SideRec> sides;          // host copy
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists

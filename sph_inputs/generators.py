@@ -217,3 +217,52 @@ def config3(seed: int = 1, n: int = 1 << 24) -> np.ndarray:
 def config4(seed: int = 1, n: int = 1 << 26) -> np.ndarray:
     """configs[4]: uniform-plus-clumps mix, 50 % uniform + 50 % in 256 clumps (reading)."""
     return clumpy_mixture(n, seed, n_clumps=256, frac_clumps=0.5, sigma=0.02)
+
+
+def eagle_like_counts(seed: int, n_cells: int, n_min: int = 5, n_max: int = 125113,
+                      median: float = 109.0, mean: float = 184.0) -> np.ndarray:
+    """Per-cell occupancies with the spread the paper reports for Eagle25 (per-cell min 5,
+    max 125,113, mean 184, median 109): a lognormal body with that median and mean (sigma^2 = 2 ln(mean / median)),
+    clipped below at n_min, plus a short geometric tail -- n_max, n_max / 2, n_max / 4, ... down to ten times the
+    median -- placed in seeded cells (the outliers a lognormal of that width does not produce: dense galaxy cores).
+    """
+    sigma = np.sqrt(2.0 * np.log(mean / median))
+    z = normal01(seed, 40, n_cells)
+    counts = np.maximum(np.floor(median * np.exp(sigma * z)), n_min).astype(np.int64)
+    counts[0] = n_min                                  # the stated minimum is present whatever the draw
+    tail = []
+    c = float(n_max)
+    while c > 10.0 * median and len(tail) < max(1, n_cells // 8):
+        tail.append(int(c))
+        c *= 0.5
+    where = np.argsort(splitmix64(seed, 41, n_cells), kind="stable")[: len(tail)]
+    where = where[where != 0][: len(tail)]
+    counts[where] = np.array(tail[: where.shape[0]], dtype=np.int64)
+    return counts
+
+
+def eagle_like(seed: int = 1, cells_per_dim: int = 16, n_max: int = 125113, n_min: int = 5,
+               median: float = 109.0, mean: float = 184.0) -> np.ndarray:
+    """Extreme-occupancy workload (stand-in for Eagle25's cell statistics).
+
+    A periodic grid of cells_per_dim^3 equal cells whose occupancies are drawn by `eagle_like_counts`; a cell's
+    particles are uniform inside it.  h = 1.12725 (volume / count)^(1/3) of the own cell (48-neighbour continuum
+    value), clipped to 0.4999 of the cell width -- what a cell with a handful of particles gets in a tree code
+    whose leaves cannot grow.  m = 1/N, v ~ N(0, 0.1), u = 1.  Generator order is a seeded shuffle, not cell order.
+    """
+    n_cells = cells_per_dim ** 3
+    counts = eagle_like_counts(seed, n_cells, n_min, n_max, median, mean)
+    n = int(counts.sum())
+    cell = np.repeat(np.arange(n_cells, dtype=np.int64), counts)
+    perm = np.argsort(splitmix64(seed, 200, n), kind="stable")
+    cell = cell[perm]
+    cxyz = np.stack([cell // (cells_per_dim * cells_per_dim), (cell // cells_per_dim) % cells_per_dim, cell % cells_per_dim], axis=1).astype(np.float64)
+    u = np.stack([uniform01(seed, d, n) for d in range(3)], axis=1)
+    parts = np.zeros(n, dtype=PART_DTYPE)
+    parts["x"] = np.minimum((cxyz + u) / cells_per_dim, np.nextafter(1.0, 0.0))
+    width = 1.0 / cells_per_dim
+    parts["h"] = np.minimum(1.12725 * width * counts[cell].astype(np.float64) ** (-1.0 / 3.0), 0.4999 * width).astype(np.float32)
+    parts["v"] = np.stack([0.1 * normal01(seed, 10 + d, n) for d in range(3)], axis=1).astype(np.float32)
+    parts["mass"] = np.float32(1.0 / n)
+    parts["u"] = 1.0
+    return _finish(parts)

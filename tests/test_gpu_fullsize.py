@@ -365,3 +365,47 @@ def test_config1_three_loop_step_every_particle():
     g = GpuCase(ps, cells, tasks, "split")
     check_three_loop(gpu_three_loop_step(g), ref, exempt)
     g.close()
+
+
+# ------------------------------------------------------------------ extreme occupancy
+
+def test_eagle_like_extreme_occupancy():
+    """Cells of 5 .. 20,000 particles in one batch (reduced instance of the Eagle25-like workload): pack and
+    unpack byte for byte, the whole step of every particle against the oracle, both layouts.  One block of 20,000 particles
+    is 625 chunks for pack / unpack and 313 loop items of 64 x 20,000 candidates each; its neighbours hold a few dozen."""
+    orc.set_threads(64)
+    parts = si.eagle_like(seed=3, cells_per_dim=4, n_max=20000)
+    ps, cells, tasks, n_self, n_pair = sort_grid(parts, 4)
+    cnt = cells["count"]
+    assert cnt.min() == 5 and cnt.max() == 20000 and (n_self, n_pair) == (64, 64 * 13)
+    ref = raw_copy(ps)
+    orc.density_cycle(ref, cells, tasks)
+    orc.ghost(ref, GAMMA)
+    f_in = orc.pack(ref, cells, tasks, orc.FORCE_IN)
+    exempt = orc.flag_cutoff_pairs(cells, tasks, f_in)
+    orc.force_cycle(ref, cells, tasks)
+    for layout in ("split", "aos"):
+        g = GpuCase(ps, cells, tasks, layout)
+        info = sph.sph_batch_get_info(g.batch)
+        assert info.max_count == 20000 and info.max_item_candidates == 64 * 20000
+        # pack of the density inputs, byte for byte
+        aset = to_attrset(orc.DENSITY_IN)
+        want = orc.pack(ps, cells, tasks, orc.DENSITY_IN)
+        got = g.pack(aset).cpu().numpy()
+        assert got.shape == want.shape and orc.compare_blocks(cells, tasks, 20, got, want) == -1, layout
+        # REDUCE unpack of seeded result records, byte for byte
+        uset = to_attrset(orc.FORCE_OUT)
+        res = _random_result_buffer(sph.sph_batch_buffer_bytes(g.batch, uset), 77)
+        want_store = raw_copy(ps)
+        orc.unpack(want_store, cells, tasks, orc.FORCE_OUT, res, orc.MODE_REDUCE)
+        sph.sph_unpack(g.store, g.batch, uset, torch.from_numpy(res).cuda(), sph.SPH_UNPACK_REDUCE)
+        assert np.array_equal(canon(g.export()), canon(want_store)), layout
+        # the whole step
+        sph.sph_store_import_aos(g.store, ps)
+        out = gpu_step(g, fused_zero=True)
+        check_store_physics(out, ref)
+        ok = np.abs(out["v_sig"] - ref["v_sig"]) <= 1e-4 * ref["v_sig"]
+        assert np.all(ok | exempt) and exempt.mean() < 0.01, layout
+        m, a = out["mass"].astype(np.float64), out["a"].astype(np.float64)
+        assert np.abs((m[:, None] * a).sum(0)).max() <= 1e-6 * np.abs(m[:, None] * a).sum()
+        g.close()
