@@ -7,6 +7,7 @@
     python bench.py --workload link        pinned H2D / D2H / both-ways copy bandwidth of this box (the host-link roofline)
     python bench.py --workload eagle       Eagle25-like occupancies (5 .. 125,113 per cell): whole step, every stage timed, load-balance figures
     python bench.py --workload replay      pack / unpack calls replayed from a seeded synthetic trace of offload actions, per layout
+    python bench.py --workload slots       configs[1]: de-duplicated cell slots against per-task buffers (bytes, pack time, loop time)
 
 `--n N` shrinks the particle count (a power of two for config3/4, N = planes * 128 * 128 is kept for config2) for quick
 runs; the default is the full size of BASELINE.json.  Everything here is harness: the path itself runs in libsph_b200.
@@ -906,10 +907,63 @@ def run_replay(args, sph, torch, common):
             "gpu_launches": len(trace) * args.steps, "roofline": None, "layouts": rows, "e2e": None}
 
 
+# ------------------------------------------------------------------------------------------------- cell slots (8(f4))
+
+def run_slots(args, sph, torch, common):
+    """configs[1]: per-task buffers (a cell packed once per task side, the parity format) against de-duplicated cell slots (a cell
+    packed once per batch, frames applied in the loop): bytes written by the pack, pack time, loop time, both loops"""
+    import sph_inputs as si
+    parts = si.config1(seed=1)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 16)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    tasks, _, _ = sph.sph_tasks_build(cells, np.full(cells.shape[0], ps["h"].max(), dtype=np.float32))
+    n = ps.shape[0]
+    params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)
+    layout = sph.sph_layout_split()
+    store = sph.sph_store_create(layout, n)
+    sph.sph_store_set_cells(store, cells)
+    sph.sph_store_import_aos(store, ps)
+    batch = sph.sph_batch_create(store, tasks)
+    sets = [sph.sph_attrset_canonical(k) for k in range(4)]
+    bufs = [torch.empty(sph.sph_batch_buffer_bytes(batch, s), dtype=torch.uint8, device="cuda") for s in sets]
+    slots = [torch.empty(sph.sph_batch_slot_bytes(batch, k), dtype=torch.uint8, device="cuda") for k in range(2)]
+    # physically sane inputs for the force loop
+    sph.sph_pack(store, batch, sets[0], bufs[0]); sph.sph_density(batch, bufs[0], bufs[1])
+    sph.sph_unpack(store, batch, sets[1], bufs[1], sph.SPH_UNPACK_REDUCE_ZERO); sph.sph_ghost(store, params)
+    stages = {"pack_density_in": lambda: sph.sph_pack(store, batch, sets[0], bufs[0]),
+              "pack_density_slots": lambda: sph.sph_pack_slots(store, batch, 0, slots[0]),
+              "density": lambda: sph.sph_density(batch, bufs[0], bufs[1]),
+              "density_slots": lambda: sph.sph_density_slots(batch, slots[0], bufs[1]),
+              "pack_force_in": lambda: sph.sph_pack(store, batch, sets[2], bufs[2]),
+              "pack_force_slots": lambda: sph.sph_pack_slots(store, batch, 1, slots[1]),
+              "force": lambda: sph.sph_force(batch, bufs[2], bufs[3], params),
+              "force_slots": lambda: sph.sph_force_slots(batch, slots[1], bufs[3], params)}
+    per = {}
+    for k, fn in stages.items():
+        per[k] = round(sum(timed(torch, fn, args.steps, 3, before=flush)) / args.steps, 5)
+    rows = {"density": {"per_task": {"input_bytes": int(bufs[0].shape[0]), "pack_ms": per["pack_density_in"], "loop_ms": per["density"]},
+                        "slots": {"input_bytes": int(slots[0].shape[0]), "pack_ms": per["pack_density_slots"], "loop_ms": per["density_slots"]}},
+            "force": {"per_task": {"input_bytes": int(bufs[2].shape[0]), "pack_ms": per["pack_force_in"], "loop_ms": per["force"]},
+                      "slots": {"input_bytes": int(slots[1].shape[0]), "pack_ms": per["pack_force_slots"], "loop_ms": per["force_slots"]}}}
+    for r in rows.values():
+        r["bytes_ratio"] = round(r["per_task"]["input_bytes"] / r["slots"]["input_bytes"], 2)
+        r["pack_plus_loop_ratio"] = round((r["slots"]["pack_ms"] + r["slots"]["loop_ms"]) / (r["per_task"]["pack_ms"] + r["per_task"]["loop_ms"]), 3)
+    t_task = sum(per[k] for k in ("pack_density_in", "density", "pack_force_in", "force"))
+    t_slot = sum(per[k] for k in ("pack_density_slots", "density_slots", "pack_force_slots", "force_slots"))
+    sph.sph_batch_destroy(batch)
+    sph.sph_store_destroy(store)
+    return {"value": n / (t_slot * 1e-3), "unit": "particles/s", "ms_per_step": t_slot, "dtype": "f32",
+            "config": {"workload": "slots: configs[1] (262144 particles, 16^3 cells), pack + loop of both loops with de-duplicated cell slots against per-task buffers",
+                       "layout": "split", "store": "HBM", "l2": "flushed before every timed launch (256 MB fill, untimed)"},
+            "gpu_launches": 4 * args.steps, "roofline": None, "per_task_ms": t_task, "slots_ms": t_slot, "formats": rows, "e2e": None}
+
+
 def run_link(args, sph, torch, common):
     link = link_probe(torch, reps=10)
     return {"value": link["h2d_gbs"], "unit": "GB/s", "ms_per_step": None, "dtype": "u8", "metric": "pinned host-link copy bandwidth",
             "config": {"workload": "link: 1 GiB pinned cudaMemcpyAsync, best of 10", "link": link}, "gpu_launches": 0, "roofline": None, "e2e": None}
 
 
-RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link, "eagle": run_eagle, "replay": run_replay}
+RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link, "eagle": run_eagle, "replay": run_replay, "slots": run_slots}

@@ -236,6 +236,21 @@ int32_t sph_pack_cells(const sph_store* store, const sph_batch* batch, const sph
                        uint32_t cell_first, uint32_t cell_count, void* stream);
 int32_t sph_unpack_cells(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,
                          int32_t mode, uint32_t cell_first, uint32_t cell_count, void* stream);
+/* ---- de-duplicated cell slots ("data replication") ----
+ * A second input format for the loops: every cell the batch touches is packed ONCE into a slot (count records, slots in
+ * ascending cell index, each starting at a multiple of 128 bytes) instead of once per task side (about 27 times on a
+ * grid).  A slot record is the loop's input set with x as raw f64 plus time_bin as a last word: density [x f64[3], h,
+ * mass, time_bin] 36 bytes, force [x f64[3], h, mass, rho, rho_dh, v, u, P, c_s, time_bin] 68 bytes (sph_slot_attrset).
+ * The loop applies the frame of each task side itself, (float)(x - frame_side), exactly as sph_pack does, so
+ * sph_density_slots / sph_force_slots write bit for bit the result buffers sph_density / sph_force write from per-task
+ * buffers (which stay the parity format, reading C7); the result buffers and sph_unpack are unchanged.
+ * loop: 0 density, 1 force.  d_slots, d_out [device, 128-byte aligned]; asynchronous on stream.  Errors as sph_pack / sph_density. */
+int32_t sph_slot_attrset(int32_t loop, sph_attrset* out);
+int32_t sph_batch_slot_bytes(const sph_batch* batch, int32_t loop, uint64_t* bytes_out);
+int32_t sph_pack_slots(const sph_store* store, const sph_batch* batch, int32_t loop, void* d_slots, uint64_t slot_bytes, void* stream);
+int32_t sph_density_slots(const sph_batch* batch, const void* d_slots, uint64_t slot_bytes, void* d_out, uint64_t out_bytes, void* stream);
+int32_t sph_force_slots(const sph_batch* batch, const void* d_slots, uint64_t slot_bytes, void* d_out, uint64_t out_bytes,
+                        const sph_params* params, void* stream);
 /* GHOST: P = (gamma-1) rho u, c_s = sqrt(gamma (gamma-1) u) for every particle. */
 int32_t sph_ghost(sph_store* store, const sph_params* params, void* stream);
 

@@ -22,6 +22,7 @@ __all__ = [
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack",
     "sph_unpack_cells", "sph_ghost", "SPH_SET_GRADIENT_IN", "SPH_SET_GRADIENT_OUT", "SPH_SET_FORCE3_IN",
+    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots",
 ]
 
 SPH_NFIELDS, SPH_MAX_SUB, SPH_MAX_ATTR = 18, 8, 32
@@ -42,6 +43,7 @@ EXPORTS = [
     "sph_store_upload_range", "sph_store_download_range", "sph_pack_cells", "sph_unpack_cells",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_free", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack", "sph_ghost",
+    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots",
 ]
 
 
@@ -334,6 +336,31 @@ def sph_density(batch, d_in, d_out, stream=None) -> None:
 def sph_force(batch, d_in, d_out, params: sph_params, stream=None) -> None:
     _check(_lib.sph_force(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)),
                           C.byref(params), _stream(stream)))
+
+
+def sph_slot_attrset(loop: int) -> sph_attrset:
+    out = sph_attrset()
+    _check(_lib.sph_slot_attrset(C.c_int32(loop), C.byref(out)))
+    return out
+
+
+def sph_batch_slot_bytes(batch, loop: int) -> int:
+    out = C.c_uint64(0)
+    _check(_lib.sph_batch_slot_bytes(batch, C.c_int32(loop), C.byref(out)))
+    return int(out.value)
+
+
+def sph_pack_slots(store, batch, loop: int, d_slots, stream=None) -> None:
+    _check(_lib.sph_pack_slots(store, batch, C.c_int32(loop), _ptr(d_slots), C.c_uint64(_nbytes(d_slots)), _stream(stream)))
+
+
+def sph_density_slots(batch, d_slots, d_out, stream=None) -> None:
+    _check(_lib.sph_density_slots(batch, _ptr(d_slots), C.c_uint64(_nbytes(d_slots)), _ptr(d_out), C.c_uint64(_nbytes(d_out)), _stream(stream)))
+
+
+def sph_force_slots(batch, d_slots, d_out, params: sph_params, stream=None) -> None:
+    _check(_lib.sph_force_slots(batch, _ptr(d_slots), C.c_uint64(_nbytes(d_slots)), _ptr(d_out), C.c_uint64(_nbytes(d_out)),
+                                C.byref(params), _stream(stream)))
 
 
 def sph_gradient(batch, d_in, d_out, stream=None) -> None:

@@ -620,6 +620,73 @@ int32_t sph_force3(const sph_batch* b, const void* d_in, uint64_t in_bytes, void
     SPH_API_END
 }
 
+// ---- de-duplicated cell slots ----
+
+int32_t sph_slot_attrset(int32_t loop, sph_attrset* out) {
+    if (!out) return fail(SPH_ERR_INVALID_ARG, "out is NULL");
+    if (loop < 0 || loop > 1) return fail(SPH_ERR_INVALID_ARG, "loop must be 0 (density) or 1 (force)");
+    if (int32_t rc = sph_attrset_canonical(loop == 0 ? SPH_SET_DENSITY_IN : SPH_SET_FORCE_IN, out)) return rc;
+    out->flags = 0;                                                                   // x as raw f64: the loop applies the frame
+    out->ent[out->n++] = sph_attr{(uint8_t)SPH_TIME_BIN, 0, 1, 0};                    // odd record length (9 / 17 words)
+    return SPH_OK;
+}
+
+int32_t sph_batch_slot_bytes(const sph_batch* b, int32_t loop, uint64_t* bytes_out) {
+    if (!b || !bytes_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    SPH_API_BEGIN
+    const SlotTables* sl = nullptr;
+    if (int32_t rc = ensure_slots(b, loop, &sl)) return rc;
+    *bytes_out = sl->total;
+    return SPH_OK;
+    SPH_API_END
+}
+
+int32_t sph_pack_slots(const sph_store* s, const sph_batch* b, int32_t loop, void* d_slots, uint64_t slot_bytes, void* stream) {
+    if (int32_t rc = store_check(s)) return rc;
+    if (!b || !d_slots) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    if (int32_t rc = batch_store_check(s, b)) return rc;
+    SPH_API_BEGIN
+    sph_attrset set;
+    if (int32_t rc = sph_slot_attrset(loop, &set)) return rc;
+    const SlotTables* sl = nullptr;
+    if (int32_t rc = ensure_slots(b, loop, &sl)) return rc;
+    Program prog;
+    if (int32_t rc = build_pack_program(s->layout, set, &prog)) return rc;
+    if (prog.rec_words * 4 != sl->rec_bytes) return fail(SPH_ERR_LAYOUT, "slot record of %u bytes, %u expected", prog.rec_words * 4, sl->rec_bytes);
+    if (slot_bytes < sl->total) return fail(SPH_ERR_RANGE, "slot buffer of %llu bytes, %llu needed", (unsigned long long)slot_bytes, (unsigned long long)sl->total);
+    if ((uintptr_t)d_slots & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    return launch_pack_tables(s->view(), prog, sl->d_chunks, sl->d_slot_off128, sl->d_zero_frames, (char*)d_slots, sl->n_chunks, (cudaStream_t)stream);
+    SPH_API_END
+}
+
+static int32_t slot_loop_check(const sph_batch* b, int loop, const void* d_slots, uint64_t slot_bytes, void* d_out, uint64_t out_bytes, const SlotTables** sl) {
+    if (!b || !d_slots || !d_out) return fail(SPH_ERR_INVALID_ARG, "batch or buffer is NULL");
+    if (int32_t rc = ensure_slots(b, loop, sl)) return rc;
+    const OffsetTable* oout = nullptr;
+    if (int32_t rc = ensure_offsets(b, loop == 0 ? 16 : 20, &oout)) return rc;
+    if (slot_bytes < (*sl)->total) return fail(SPH_ERR_RANGE, "slot buffer of %llu bytes, %llu needed", (unsigned long long)slot_bytes, (unsigned long long)(*sl)->total);
+    if (out_bytes < oout->total) return fail(SPH_ERR_RANGE, "output buffer of %llu bytes, %llu needed", (unsigned long long)out_bytes, (unsigned long long)oout->total);
+    if (((uintptr_t)d_slots | (uintptr_t)d_out) & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    return SPH_OK;
+}
+
+int32_t sph_density_slots(const sph_batch* b, const void* d_slots, uint64_t slot_bytes, void* d_out, uint64_t out_bytes, void* stream) {
+    SPH_API_BEGIN
+    const SlotTables* sl = nullptr;
+    if (int32_t rc = slot_loop_check(b, 0, d_slots, slot_bytes, d_out, out_bytes, &sl)) return rc;
+    return launch_density_slots(b, *sl, (const char*)d_slots, (char*)d_out, (cudaStream_t)stream);
+    SPH_API_END
+}
+
+int32_t sph_force_slots(const sph_batch* b, const void* d_slots, uint64_t slot_bytes, void* d_out, uint64_t out_bytes, const sph_params* prm, void* stream) {
+    if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");
+    SPH_API_BEGIN
+    const SlotTables* sl = nullptr;
+    if (int32_t rc = slot_loop_check(b, 1, d_slots, slot_bytes, d_out, out_bytes, &sl)) return rc;
+    return launch_force_slots(b, *sl, (const char*)d_slots, (char*)d_out, *prm, (cudaStream_t)stream);
+    SPH_API_END
+}
+
 int32_t sph_ghost(sph_store* s, const sph_params* prm, void* stream) {
     if (int32_t rc = store_check(s)) return rc;
     if (!prm) return fail(SPH_ERR_INVALID_ARG, "params is NULL");

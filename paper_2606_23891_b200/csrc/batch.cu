@@ -57,6 +57,58 @@ int32_t ensure_offsets(const sph_batch* b, uint32_t rec_bytes, const OffsetTable
     return SPH_OK;
 }
 
+// Slot tables of one loop: every touched cell gets one slot of `count` records (x raw f64, so the frame can be applied in
+// the loop exactly as the pack applies it: (float)(x - frame)), slots in ascending cell index, each starting at a multiple of
+// 128 bytes; the loop's items are the batch's items with their record offsets pointing into the slot buffer.
+int32_t ensure_slots(const sph_batch* b, int loop, const SlotTables** out) {
+    if (loop < 0 || loop > 1) return fail(SPH_ERR_INVALID_ARG, "loop must be 0 (density) or 1 (force)");
+    std::lock_guard<std::mutex> lock(b->mu);
+    SlotTables& sl = b->slots[loop];
+    if (sl.built) { *out = &sl; return SPH_OK; }
+    const uint32_t rec = loop == 0 ? 36u : 68u, out_rec = loop == 0 ? 16u : 20u;
+    const uint32_t n_cells = (uint32_t)b->cell_chunk0.size() - 1;
+    std::vector<uint32_t> cell_first(n_cells, 0), cell_count(n_cells, 0);
+    std::vector<char> touched(n_cells, 0);
+    for (const SideRec& s : b->sides) { touched[s.cell] = 1; cell_first[s.cell] = s.first; cell_count[s.cell] = s.count; }
+    std::vector<uint32_t> slot128(n_cells, 0), off128;
+    std::vector<CellChunk> chunks;
+    uint64_t run = 0;
+    uint32_t idx = 0;
+    for (uint32_t c = 0; c < n_cells; ++c) {
+        if (!touched[c]) continue;
+        slot128[c] = (uint32_t)(run / 128);
+        off128.push_back(slot128[c]);
+        for (uint32_t k = 0; k < cell_count[c]; k += 32) chunks.push_back(CellChunk{cell_first[c] + k, std::min(32u, cell_count[c] - k), k, idx, 1u});
+        run = (run + (uint64_t)cell_count[c] * rec + 127) / 128 * 128;
+        ++idx;
+    }
+    if (run / 128 >= (1ull << 32)) return fail(SPH_ERR_RANGE, "slot buffer exceeds the 512 GiB offset range");
+    auto it = b->offsets.find(out_rec);
+    if (it == b->offsets.end()) return fail(SPH_ERR_INVALID_ARG, "batch has no result offsets");
+    const std::vector<uint64_t>& oout = it->second.h_off;
+    std::vector<LoopItem> items(b->item_side.size());
+    std::vector<double> ifr(6 * b->item_side.size());
+    for (size_t i = 0; i < items.size(); ++i) {
+        const ItemSide& is = b->item_side[i];
+        const SideRec &t = b->sides[is.tgt], &s = b->sides[is.src];
+        items[i] = LoopItem{slot128[t.cell] + is.kc * 2 * (rec / 4), slot128[s.cell], (uint32_t)(oout[is.tgt] / 128) + is.kc * 2 * (out_rec / 4),
+                            std::min(kLoopTargets, t.count - is.kc * kLoopTargets) | s.count << 7};
+        std::copy_n(&b->side_frames[3 * (size_t)is.tgt], 3, &ifr[6 * i]);
+        std::copy_n(&b->side_frames[3 * (size_t)is.src], 3, &ifr[6 * i + 3]);
+    }
+    std::vector<double> zeros(3 * (size_t)idx, 0.0);
+    SlotTables tmp;
+    if (int32_t rc = upload(chunks, &tmp.d_chunks)) return rc;
+    if (int32_t rc = upload(off128, &tmp.d_slot_off128)) return rc;
+    if (int32_t rc = upload(zeros, &tmp.d_zero_frames)) return rc;
+    if (int32_t rc = upload(items, &tmp.d_items)) return rc;
+    if (int32_t rc = upload(ifr, &tmp.d_item_frames)) return rc;
+    tmp.rec_bytes = rec; tmp.total = run; tmp.n_chunks = (uint32_t)chunks.size(); tmp.built = true;
+    sl = tmp;
+    *out = &sl;
+    return SPH_OK;
+}
+
 }  // namespace sph
 
 extern "C" {
@@ -104,6 +156,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     }
     b->task_side0[n_tasks] = (uint32_t)b->sides.size();
     b->n_sides = (uint32_t)b->sides.size();
+    b->side_frames = frames;
 
     // per-cell occurrence lists in ascending (task, side) order = ascending side index
     std::vector<uint32_t> occ_count(n_cells, 0);
@@ -143,6 +196,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
         const std::vector<uint64_t> &o16 = b->offsets.at(16).h_off, &o20 = b->offsets.at(20).h_off, &o52 = b->offsets.at(52).h_off;
         const std::vector<uint64_t> &o40 = b->offsets.at(40).h_off, &o72 = b->offsets.at(72).h_off;
         std::vector<LoopItem> dens, forc, grad, forc3;
+        std::vector<ItemSide>& ids = b->item_side;
         for (uint32_t c = 0; c < n_cells; ++c)
             for (uint32_t o = occ_start[c]; o < occ_start[c + 1]; ++o) {
                 const uint32_t tgt = occ_side[o], src = partner[tgt];
@@ -150,6 +204,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
                 for (uint32_t k = 0, kc = 0; k < cnt; k += kLoopTargets, ++kc) {
                     const uint32_t nt_ns = std::min(kLoopTargets, cnt - k) | b->sides[src].count << 7;
                     const uint32_t u = kLoopTargets / 32;                                // 32 records of r bytes = r units of 128 bytes
+                    ids.push_back(ItemSide{tgt, src, kc});
                     dens.push_back(LoopItem{(uint32_t)(o20[tgt] / 128) + kc * 5 * u, (uint32_t)(o20[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns});
                     forc.push_back(LoopItem{(uint32_t)(o52[tgt] / 128) + kc * 13 * u, (uint32_t)(o52[src] / 128), (uint32_t)(o20[tgt] / 128) + kc * 5 * u, nt_ns});
                     grad.push_back(LoopItem{(uint32_t)(o40[tgt] / 128) + kc * 10 * u, (uint32_t)(o40[src] / 128), (uint32_t)(o16[tgt] / 128) + kc * 4 * u, nt_ns});
@@ -167,6 +222,7 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
             std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return cls(dens[x]) > cls(dens[y]); });
             auto apply = [&](std::vector<LoopItem>& v) { std::vector<LoopItem> w(v.size()); for (size_t i = 0; i < v.size(); ++i) w[i] = v[order[i]]; v.swap(w); };
             apply(dens); apply(forc); apply(grad); apply(forc3);
+            { std::vector<ItemSide> w(ids.size()); for (size_t i = 0; i < ids.size(); ++i) w[i] = ids[order[i]]; ids.swap(w); }
             uint64_t worst = 0;
             for (const LoopItem& it : dens) worst = std::max(worst, (uint64_t)(it.nt_ns & 127u) * (it.nt_ns >> 7));
             b->max_item_candidates = worst;
@@ -187,6 +243,7 @@ int32_t sph_batch_destroy(sph_batch* b) {
     if (!b) return SPH_OK;
     cudaFree(b->d_cell_chunks); cudaFree(b->d_occ_frames); cudaFree(b->d_items_density); cudaFree(b->d_items_force); cudaFree(b->d_items_gradient); cudaFree(b->d_items_force3);
     for (auto& kv : b->offsets) { cudaFree(kv.second.d_off128); cudaFree(kv.second.d_occ_off128); }
+    for (SlotTables& sl : b->slots) { cudaFree(sl.d_chunks); cudaFree(sl.d_slot_off128); cudaFree(sl.d_zero_frames); cudaFree(sl.d_items); cudaFree(sl.d_item_frames); }
     delete b;
     return SPH_OK;
 }

@@ -112,6 +112,22 @@ struct Program {
 int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog);
 int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, int32_t mode, Program* prog);
 
+// De-duplicated cell slots ("data replication"): every cell the batch touches is packed once,
+// x as raw f64, and the loops' items index slots and carry the frames of their two sides.  One set of tables per loop.
+struct SlotTables {
+    bool built = false;
+    uint32_t rec_bytes = 0;                // 36 (density) or 68 (force)
+    uint64_t total = 0;                    // bytes of the slot buffer
+    uint32_t n_chunks = 0;
+    CellChunk* d_chunks = nullptr;         // 32-particle chunks of the touched cells; every chunk has one occurrence: its cell's slot
+    uint32_t* d_slot_off128 = nullptr;     // per touched cell: slot start in units of 128 bytes
+    double* d_zero_frames = nullptr;       // 3 zeros per touched cell (the pack kernel subtracts nothing)
+    LoopItem* d_items = nullptr;           // the loop's items with tin128 / sin128 pointing into the slot buffer
+    double* d_item_frames = nullptr;       // per item: frame of the targets' side (3), frame of the sources' side (3)
+};
+
+struct ItemSide { uint32_t tgt, src, kc; };    // a loop item: 64-target chunk kc of block tgt against block src
+
 struct OffsetTable {
     uint32_t* d_off128 = nullptr;          // per side: block start in units of 128 bytes
     uint32_t* d_occ_off128 = nullptr;      // per occurrence (cell-major, ascending side): the same, for the ordered unpack
@@ -159,10 +175,15 @@ struct sph_batch {
     // record size is asked for, under the mutex; tables are never removed, so pointers to them stay valid)
     mutable std::mutex mu;
     mutable std::map<uint32_t, sph::OffsetTable> offsets;
+    // cell slots (built the first time a slot call needs them, under the mutex)
+    std::vector<sph::ItemSide> item_side;     // the items in launch order
+    std::vector<double> side_frames;          // 3 per side
+    mutable sph::SlotTables slots[2];         // [0] density, [1] force
 };
 
 namespace sph {
 int32_t ensure_offsets(const sph_batch* batch, uint32_t rec_bytes, const OffsetTable** out);
+int32_t ensure_slots(const sph_batch* batch, int loop, const SlotTables** out);      // loop: 0 density, 1 force
 int32_t device_sms(int* sms_out);      // SM count of the current device
 
 // kernel launchers (kernels_*.cu)
@@ -173,6 +194,10 @@ int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& 
                       bool last_only, bool from_zero, uint32_t cc0, uint32_t ncc, cudaStream_t st);
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
+int32_t launch_density_slots(const sph_batch* b, const SlotTables& sl, const char* d_slots, char* d_out, cudaStream_t st);
+int32_t launch_force_slots(const sph_batch* b, const SlotTables& sl, const char* d_slots, char* d_out, const sph_params& prm, cudaStream_t st);
+int32_t launch_pack_tables(const StoreView& view, const Program& prog, const CellChunk* d_chunks, const uint32_t* d_occ_off128, const double* d_occ_frames,
+                           char* d_buf, uint32_t ncc, cudaStream_t st);
 int32_t launch_gradient(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st);
 int32_t launch_force3(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st);
 int32_t launch_zero(const StoreView& view, uint64_t n, const Program& prog, cudaStream_t st);

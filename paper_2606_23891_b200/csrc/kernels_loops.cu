@@ -213,20 +213,35 @@ __device__ __forceinline__ uint32_t compact_targets(uint32_t* sm_act, bool aA, b
     return nA + __popc(bB);
 }
 
+// Cell-slot records: x travels as raw f64 (words 0-5) and the frame of the item's side is applied here,
+// exactly as the pack applies it -- one f64 subtraction, one rounding -- so a loop over slots sees bit for bit the inputs of
+// a loop over per-task records.  Every other field sits three words further on; a last word (time_bin) makes the record
+// length odd (9 / 17 words), so that one record per lane reads conflict-free out of the landing area.
+template <bool SLOTS>
+__device__ __forceinline__ float rec_x(const float* r, int d, const double* frame) {
+    if constexpr (SLOTS) return (float)(__hiloint2double(__float_as_int(r[2 * d + 1]), __float_as_int(r[2 * d])) - frame[d]);
+    else return r[d];
+}
+
 // ------------------------------------------------------------------------------------------------- density
 
-struct DensityWarpSmem {
+template <int RW>
+struct DensityWarpSmemT {
     FilterTile f;
     float4 tile[2 * kHalf];  // x, y, z, m of the compacted sources; entries 32 and 65 are the dummy
     float4 tgt[64];          // the item's targets: x, y, z, h
     float4 acc[64];          // their running sums: m w, m (3w + q w'), w, (3w + q w')
-    float raw[64 * 5];       // landing area of an item's 64 DENSITY_IN records: xr0 xr1 xr2 h m
-    float src[2][32 * 5];    // landing areas of the source rounds (double-buffered)
+    float raw[64 * RW];      // landing area of an item's 64 DENSITY_IN records: xr0 xr1 xr2 h m (slots: x f64[3] h m time_bin)
+    float src[2][32 * RW];   // landing areas of the source rounds (double-buffered)
     uint32_t act[64];        // the active targets of the flush
 };
 
+template <bool SLOTS>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_DENS_MINB)
-density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items) {
+density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items,
+               const double* __restrict__ item_frames) {
+    constexpr int RW = SLOTS ? 9 : 5, O = SLOTS ? 3 : 0;      // record words; offset of the fields behind x
+    typedef DensityWarpSmemT<RW> DensityWarpSmem;
     __shared__ __align__(16) DensityWarpSmem s_all[kLoopWarps];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     DensityWarpSmem& sm = s_all[warp];
@@ -238,8 +253,8 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
     const u64 kTwo = dup2(2.0f), kThree = dup2(3.0f), kQuarter = dup2(0.25f), kM075 = dup2(-0.75f);
 
     uint4 iw = __ldg(reinterpret_cast<const uint4*>(items) + item);
-    fetch_records<5, 64>(sm.raw, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
-    fetch_records<5, 32>(sm.src[0], in + (uint64_t)iw.y * 128, min(32u, iw.w >> 7), lane);
+    fetch_records<RW, 64>(sm.raw, in + (uint64_t)iw.x * 128, iw.w & 127u, lane);
+    fetch_records<RW, 32>(sm.src[0], in + (uint64_t)iw.y * 128, min(32u, iw.w >> 7), lane);
     uint32_t buf = 0;
 
     for (; item < n_items; item += step) {
@@ -253,9 +268,14 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
         __syncwarp();
         // the lane's own two targets (lane, lane + 32): table entries, zeroed sums, reach box of the whole item
         const bool vA = lane < n_t, vB = lane + 32 < n_t;
+        double ft[3] = {0.0, 0.0, 0.0}, fs[3] = {0.0, 0.0, 0.0};      // slots: the frames of the targets' and of the sources' side
+        if constexpr (SLOTS) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { ft[d] = __ldg(item_frames + 6 * (size_t)item + d); fs[d] = __ldg(item_frames + 6 * (size_t)item + 3 + d); }
+        }
         float4 oA = make_float4(0.f, 0.f, 0.f, 0.f), oB = oA;
-        if (vA) { const float* r = sm.raw + 5 * lane; oA = make_float4(r[0], r[1], r[2], r[3]); }
-        if (vB) { const float* r = sm.raw + 5 * (lane + 32); oB = make_float4(r[0], r[1], r[2], r[3]); }
+        if (vA) { const float* r = sm.raw + RW * lane; oA = make_float4(rec_x<SLOTS>(r, 0, ft), rec_x<SLOTS>(r, 1, ft), rec_x<SLOTS>(r, 2, ft), r[3 + O]); }
+        if (vB) { const float* r = sm.raw + RW * (lane + 32); oB = make_float4(rec_x<SLOTS>(r, 0, ft), rec_x<SLOTS>(r, 1, ft), rec_x<SLOTS>(r, 2, ft), r[3 + O]); }
         sm.tgt[lane] = oA; sm.tgt[lane + 32] = oB;
         sm.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f); sm.acc[lane + 32] = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncwarp();                 // sm.raw may now receive the next item's targets
@@ -332,14 +352,14 @@ density_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, 
                 if (r > 0) { cp_async_wait_all(); __syncwarp(); }
                 // one step ahead: the next round of this item, or the next item's targets and first round
                 if (r + 1 < n_rounds) {
-                    fetch_records<5, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * 20, min(32u, n_s - j0 - 32), lane);
+                    fetch_records<RW, 32>(sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * (RW * 4), min(32u, n_s - j0 - 32), lane);
                 } else if (has_next) {
-                    fetch_records<5, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
-                    fetch_records<5, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
+                    fetch_records<RW, 64>(sm.raw, in + (uint64_t)iw_next.x * 128, iw_next.w & 127u, lane);
+                    fetch_records<RW, 32>(sm.src[buf ^ 1], in + (uint64_t)iw_next.y * 128, min(32u, iw_next.w >> 7), lane);
                 }
                 if (lane < nj) {
-                    const float* rec = sm.src[buf] + 5 * lane;
-                    s = make_float4(rec[0], rec[1], rec[2], rec[4]);
+                    const float* rec = sm.src[buf] + RW * lane;
+                    s = make_float4(rec_x<SLOTS>(rec, 0, fs), rec_x<SLOTS>(rec, 1, fs), rec_x<SLOTS>(rec, 2, fs), rec[4 + O]);
                     ok = s.x > lox && s.x < hix && s.y > loy && s.y < hiy && s.z > loz && s.z < hiz;
                 }
                 ball = __ballot_sync(kFull, ok); c = __popc(ball);
@@ -646,12 +666,15 @@ __device__ __forceinline__ u64 switch_pair(const Smem& sm, uint32_t a, uint32_t 
     else return 0ull;
 }
 
-template <bool UNITS, bool SWITCH>
+template <bool UNITS, bool SWITCH, bool SLOTS>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
-force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta) {
+force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta,
+             const double* __restrict__ item_frames) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    constexpr int RW = SWITCH ? 18 : 13;      // words of an input record: FORCE_IN, or FORCE3_IN = FORCE_IN + div_v rot_v[3] time_bin
+    static_assert(!(SWITCH && SLOTS), "the switched force loop has no slot variant");
+    constexpr int RW = SLOTS ? 17 : (SWITCH ? 18 : 13);      // words of an input record: FORCE_IN, FORCE3_IN = FORCE_IN + div_v rot_v[3] time_bin, or a cell slot
+    constexpr int O = SLOTS ? 3 : 0;                          // slots: x is f64[3], every other field three words further on
     typedef ForceWarpSmemT<RW> Smem;
     Smem& sm = reinterpret_cast<Smem*>(s_raw)[warp];
     const uint32_t lt = lanemask_lt();
@@ -683,6 +706,11 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
         fg.wait();                    // this item's targets and first source round
         // the lane's own two targets (lane, lane + 32): table entries; bounding box of the whole item
         const bool vA = lane < n_t, vB = lane + 32 < n_t;
+        double ft[3] = {0.0, 0.0, 0.0};      // slots: the frame of the targets' side (the sources' is re-read per round: registers)
+        if constexpr (SLOTS) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) ft[d] = __ldg(item_frames + 6 * (size_t)item + d);
+        }
         float4 oA = make_float4(0.f, 0.f, 0.f, 0.f), oB = oA;      // x, y, z, 4 h^2
         float hA = 0.f, hB = 0.f;
 #pragma unroll
@@ -691,10 +719,10 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0, p2 = make_float4(0.f, 0.f, 1.f, 0.f);
             if (t < n_t) {
                 const float* r = sm.raw + RW * t;
-                const float h = r[3], rho = r[5], ih = rcp_fast(h);
-                p0 = make_float4(r[0], r[1], r[2], 4.0f * h * h);
-                p1 = make_float4(r[7], r[8], r[9], r[12]);
-                p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11] * rcp_fast(fmaf(h * r[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho));
+                const float h = r[3 + O], rho = r[5 + O], ih = rcp_fast(h);
+                p0 = make_float4(rec_x<SLOTS>(r, 0, ft), rec_x<SLOTS>(r, 1, ft), rec_x<SLOTS>(r, 2, ft), 4.0f * h * h);
+                p1 = make_float4(r[7 + O], r[8 + O], r[9 + O], r[12 + O]);
+                p2 = make_float4(ih, kInvPi * (ih * ih) * (ih * ih), rho, r[11 + O] * rcp_fast(fmaf(h * r[6 + O], rcp_fast(3.0f * rho), 1.0f) * rho * rho));
                 if (k == 0) hA = h; else hB = h;
                 if constexpr (SWITCH) sm.tB[t] = balsara(r);
             }
@@ -878,13 +906,18 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
                 if (r + 1 < n_rounds) fg.issue1(lane, sm.src[buf ^ 1], sin + (uint64_t)(j0 + 32) * (RW * 4), rec_bytes16<RW>(min(32u, n_s - j0 - 32)));
                 if (lane < nj) {
                     const float* rec = sm.src[buf] + RW * lane;
-                    const float h = rec[3], rho = rec[5];
+                    const float h = rec[3 + O], rho = rec[5 + O];
+                    double fs[3] = {0.0, 0.0, 0.0};
+                    if constexpr (SLOTS) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) fs[d] = __ldg(item_frames + 6 * (size_t)item + 3 + d);
+                    }
                     const float reach = fmaxf(reach_t, 2.0f * h) * kReachSlack;
-                    a = make_float4(rec[0], rec[1], rec[2], 4.0f * h * h);
+                    a = make_float4(rec_x<SLOTS>(rec, 0, fs), rec_x<SLOTS>(rec, 1, fs), rec_x<SLOTS>(rec, 2, fs), 4.0f * h * h);
                     ok = a.x > lox - reach && a.x < hix + reach && a.y > loy - reach && a.y < hiy + reach && a.z > loz - reach && a.z < hiz + reach;
                     if (ok) {
-                        b = make_float4(rec[7], rec[8], rec[9], rec[4]);
-                        c = make_float4(rho, rec[11] * rcp_fast(fmaf(h * rec[6], rcp_fast(3.0f * rho), 1.0f) * rho * rho), rec[12], rcp_fast(h));
+                        b = make_float4(rec[7 + O], rec[8 + O], rec[9 + O], rec[4 + O]);
+                        c = make_float4(rho, rec[11 + O] * rcp_fast(fmaf(h * rec[6 + O], rcp_fast(3.0f * rho), 1.0f) * rho * rho), rec[12 + O], rcp_fast(h));
                         s2 = fmaf(a.x, a.x, fmaf(a.y, a.y, a.z * a.z));
                     }
                 }
@@ -932,9 +965,19 @@ int32_t loop_grid(K kernel, size_t smem, uint32_t* grid) {
 int32_t launch_density(const sph_batch* b, const char* d_in, char* d_out, cudaStream_t st) {
     if (b->n_items == 0) return SPH_OK;
     uint32_t full_grid = 0;
-    if (int32_t rc = loop_grid(density_kernel, 0, &full_grid)) return rc;
+    if (int32_t rc = loop_grid(density_kernel<false>, 0, &full_grid)) return rc;
     const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
-    density_kernel<<<grid, kLoopWarps * 32, 0, st>>>(b->d_items_density, d_in, d_out, b->n_items);
+    density_kernel<false><<<grid, kLoopWarps * 32, 0, st>>>(b->d_items_density, d_in, d_out, b->n_items, nullptr);
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int32_t launch_density_slots(const sph_batch* b, const SlotTables& sl, const char* d_slots, char* d_out, cudaStream_t st) {
+    if (b->n_items == 0) return SPH_OK;
+    uint32_t full_grid = 0;
+    if (int32_t rc = loop_grid(density_kernel<true>, 0, &full_grid)) return rc;
+    const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
+    density_kernel<true><<<grid, kLoopWarps * 32, 0, st>>>(sl.d_items, d_slots, d_out, b->n_items, sl.d_item_frames);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -954,28 +997,32 @@ int32_t launch_gradient(const sph_batch* b, const char* d_in, char* d_out, cudaS
 #define SPH_UNITS_MAX_MEAN_BLOCK 80
 #endif
 
-template <bool SWITCH>
-static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
+template <bool SWITCH, bool SLOTS>
+static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const double* item_frames, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
     if (b->n_items == 0) return SPH_OK;
     uint32_t full_grid = 0;
-    constexpr size_t smem = sizeof(ForceWarpSmemT<SWITCH ? 18 : 13>) * kLoopWarps;
+    constexpr size_t smem = sizeof(ForceWarpSmemT<SLOTS ? 17 : (SWITCH ? 18 : 13)>) * kLoopWarps;
     // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
     // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
     const bool units = b->n_sides && b->n_instances <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * b->n_sides;
-    if (int32_t rc = units ? loop_grid(force_kernel<true, SWITCH>, smem, &full_grid) : loop_grid(force_kernel<false, SWITCH>, smem, &full_grid)) return rc;
+    if (int32_t rc = units ? loop_grid(force_kernel<true, SWITCH, SLOTS>, smem, &full_grid) : loop_grid(force_kernel<false, SWITCH, SLOTS>, smem, &full_grid)) return rc;
     const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
-    if (units) force_kernel<true, SWITCH><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta);
-    else force_kernel<false, SWITCH><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta);
+    if (units) force_kernel<true, SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);
+    else force_kernel<false, SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
 
 int32_t launch_force(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
-    return launch_force_t<false>(b, b->d_items_force, d_in, d_out, prm, st);
+    return launch_force_t<false, false>(b, b->d_items_force, nullptr, d_in, d_out, prm, st);
 }
 
 int32_t launch_force3(const sph_batch* b, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
-    return launch_force_t<true>(b, b->d_items_force3, d_in, d_out, prm, st);
+    return launch_force_t<true, false>(b, b->d_items_force3, nullptr, d_in, d_out, prm, st);
+}
+
+int32_t launch_force_slots(const sph_batch* b, const SlotTables& sl, const char* d_slots, char* d_out, const sph_params& prm, cudaStream_t st) {
+    return launch_force_t<false, true>(b, sl.d_items, sl.d_item_frames, d_slots, d_out, prm, st);
 }
 
 }  // namespace sph

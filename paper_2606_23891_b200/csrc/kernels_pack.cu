@@ -449,8 +449,8 @@ int32_t device_sms(int* sms_out) {
 namespace {
 
 template <int NIT>
-int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms,
-                        uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+int32_t launch_pack_nit(const CellChunk* d_chunks, const double* d_occ_frames, const Program& prog, const uint32_t* d_occ_off128, char* d_buf, size_t smem, int sms,
+                        uint32_t ncc, cudaStream_t st) {
     if (smem > 48 * 1024) SPH_CUDA_TRY(cudaFuncSetAttribute(pack_kernel<NIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // resident CTAs per SM (shared memory and 64 warps bound it); a cell's occurrences are split into `slices` items
     // when there are fewer cell chunks than about two rounds of resident warps
@@ -459,7 +459,7 @@ int32_t launch_pack_nit(const sph_batch* b, const Program& prog, const uint32_t*
     const uint32_t slices = std::min(8u, std::max(1u, (2 * resident_warps + ncc - 1) / ncc));
     const uint64_t items = (uint64_t)ncc * slices;
     const uint32_t grid = (uint32_t)std::min<uint64_t>((items + kPackWarps - 1) / kPackWarps, (uint64_t)sms * per_sm);
-    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, b->d_cell_chunks + cc0, d_occ_off128, b->d_occ_frames, ncc, slices, d_buf);
+    pack_kernel<NIT><<<grid, kPackWarps * 32, smem, st>>>(prog, d_chunks, d_occ_off128, d_occ_frames, ncc, slices, d_buf);
     return SPH_OK;
 }
 
@@ -492,8 +492,8 @@ int32_t launch_unpack_t(const StoreView& view, const sph_batch* b, const Program
 
 }  // namespace
 
-int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog_in, const uint32_t* d_occ_off128, char* d_buf,
-                    uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+int32_t launch_pack_tables(const StoreView& view, const Program& prog_in, const CellChunk* d_chunks, const uint32_t* d_occ_off128, const double* d_occ_frames,
+                           char* d_buf, uint32_t ncc, cudaStream_t st) {
     if (ncc == 0) return SPH_OK;
     Program prog = prog_in;
     for (uint32_t u = 0; u < prog.n_sub_used; ++u) prog.su[u].base = view.base[prog.su[u].sub];
@@ -503,15 +503,20 @@ int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& pr
     if (smem > 200 * 1024) return fail(SPH_ERR_UNSUPPORTED, "layout needs %zu bytes of staging per CTA", smem);
     const uint32_t nit = (prog.rec_words + 3) / 4;   // 16-byte vectors per lane for a full chunk: ceil(32 R / 4 / 32)
     int32_t rc;
-    if (nit <= 1) rc = launch_pack_nit<1>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
-    else if (nit <= 2) rc = launch_pack_nit<2>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
-    else if (nit <= 4) rc = launch_pack_nit<4>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
-    else if (nit <= 6) rc = launch_pack_nit<6>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
-    else if (nit <= 9) rc = launch_pack_nit<9>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
-    else rc = launch_pack_nit<12>(b, prog, d_occ_off128, d_buf, smem, sms, cc0, ncc, st);
+    if (nit <= 1) rc = launch_pack_nit<1>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
+    else if (nit <= 2) rc = launch_pack_nit<2>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
+    else if (nit <= 4) rc = launch_pack_nit<4>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
+    else if (nit <= 6) rc = launch_pack_nit<6>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
+    else if (nit <= 9) rc = launch_pack_nit<9>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
+    else rc = launch_pack_nit<12>(d_chunks, d_occ_frames, prog, d_occ_off128, d_buf, smem, sms, ncc, st);
     if (rc) return rc;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
+}
+
+int32_t launch_pack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, char* d_buf,
+                    uint32_t cc0, uint32_t ncc, cudaStream_t st) {
+    return launch_pack_tables(view, prog, b->d_cell_chunks + cc0, d_occ_off128, b->d_occ_frames, d_buf, ncc, st);
 }
 
 int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& prog, const uint32_t* d_occ_off128, const char* d_buf,

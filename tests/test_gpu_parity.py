@@ -780,3 +780,45 @@ def test_three_loop_layout_variants(variant):
     got = gpu_three_loop_step(g)
     assert np.array_equal(canon(got), canon(ref)), variant
     g.close()
+
+
+# ------------------------------------------------------------------ de-duplicated cell slots
+
+@pytest.mark.parametrize("name", ["config0", "ragged", "octree", "hugecells"])
+def test_cell_slots_equal_per_task_buffers(name):
+    """Every touched cell packed once (x raw f64, frames applied in the loop): the slot buffer is what the oracle packs for one
+    self task per cell with the slot set, and the loops over slots write bit for bit the result buffers of the loops over
+    per-task buffers; a batch that touches only some cells (pair tasks of a slice) included."""
+    ps, cells, tasks = case(name)
+    ps = physical(ps, cells, tasks)
+    n_self = int((tasks["cj"] < 0).sum())
+    for sel in (tasks, np.ascontiguousarray(tasks[n_self + 3:n_self + 3 + max(5, (tasks.shape[0] - n_self) // 7)])):
+        g = GpuCase(ps, cells, sel)
+        touched = np.unique(np.concatenate([sel["ci"], sel["cj"][sel["cj"] >= 0]]))
+        self_tasks = np.ascontiguousarray(tasks[:n_self][touched])
+        assert np.all(self_tasks["cj"] < 0) and np.array_equal(self_tasks["ci"], touched)
+        for loop, (set_in, set_out, rec_out) in enumerate(((sph.SPH_SET_DENSITY_IN, sph.SPH_SET_DENSITY_OUT, 16), (sph.SPH_SET_FORCE_IN, sph.SPH_SET_FORCE_OUT, 20))):
+            sset = sph.sph_slot_attrset(loop)
+            assert sph.sph_attrset_record_bytes(sset) == (36, 68)[loop]
+            # the slot buffer against the oracle's pack of one self task per touched cell
+            oset = ([(int(e.field), int(e.comp0), int(e.ncomp)) for e in list(sset.ent)[:sset.n]], 0)
+            want = orc.pack(ps, cells, self_tasks, oset)
+            nbytes = sph.sph_batch_slot_bytes(g.batch, loop)
+            assert nbytes == want.shape[0]
+            slots = torch.full((nbytes,), 0xCD, dtype=torch.uint8, device="cuda")
+            sph.sph_pack_slots(g.store, g.batch, loop, slots)
+            assert orc.compare_blocks(cells, self_tasks, (36, 68)[loop], slots.cpu().numpy(), want) == -1, (name, loop)
+            # loops: per-task buffers versus slots
+            a_in, a_out = sph.sph_attrset_canonical(set_in), sph.sph_attrset_canonical(set_out)
+            b_in = g.pack(a_in)
+            o_task, o_slot = g.buffer(a_out, 0xAB), g.buffer(a_out, 0xAB)
+            if loop == 0:
+                sph.sph_density(g.batch, b_in, o_task)
+                sph.sph_density_slots(g.batch, slots, o_slot)
+            else:
+                sph.sph_force(g.batch, b_in, o_task, PARAMS)
+                sph.sph_force_slots(g.batch, slots, o_slot, PARAMS)
+            torch.cuda.synchronize()
+            assert orc.compare_blocks(cells, sel, rec_out, o_slot.cpu().numpy(), o_task.cpu().numpy()) == -1, (name, loop)
+            assert nbytes * 4 < b_in.shape[0] or sel.shape[0] < tasks.shape[0]      # whole task lists: several times fewer input bytes
+        g.close()

@@ -26,6 +26,17 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, name), name
 
 
+def test_slot_attribute_sets():
+    """cell-slot records (row f4): the loop's input set with x as raw f64 and time_bin as a last word -- 9 and 17 words"""
+    for loop, (nbytes, canon) in enumerate(((36, sph.SPH_SET_DENSITY_IN), (68, sph.SPH_SET_FORCE_IN))):
+        s, c = sph.sph_slot_attrset(loop), sph.sph_attrset_canonical(canon)
+        assert sph.sph_attrset_record_bytes(s) == nbytes and s.flags == 0 and s.n == c.n + 1
+        assert [int(e.field) for e in list(s.ent)[:c.n]] == [int(e.field) for e in list(c.ent)[:c.n]]
+        assert int(s.ent[c.n].field) == sph.FIELD["time_bin"]
+    with pytest.raises(sph.SphError):
+        sph.sph_slot_attrset(2)
+
+
 def test_library_is_built_for_sm_100a_only():
     import subprocess
     out = subprocess.run(["cuobjdump", "-lelf", sph.lib_path()], capture_output=True, text=True).stdout
