@@ -867,7 +867,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="both", help="split | aos | both, or any layout name of paper_2606_23891_b200/layouts.py")
-    ap.add_argument("--workload", default="default", choices=["default", "config1", "config2", "config3", "config4", "link", "layouts", "eagle", "replay", "slots"],
+    ap.add_argument("--workload", default="default", choices=["default", "config1", "config2", "config3", "config4", "link", "layouts", "eagle", "replay", "slots", "fission"],
                     help="default = configs[2] as the headline plus configs[1], [3], [4] as `workloads`; the others run one configuration "
                          "(bench_workloads.py describes them)")
     ap.add_argument("--loops", type=int, default=2, choices=[2, 3], help="layouts / config1: the two-loop cycle or the three-loop cycle (density, gradient, force)")

@@ -8,6 +8,7 @@
     python bench.py --workload eagle       Eagle25-like occupancies (5 .. 125,113 per cell): whole step, every stage timed, load-balance figures
     python bench.py --workload replay      pack / unpack calls replayed from a seeded synthetic trace of offload actions, per layout
     python bench.py --workload slots       configs[1]: de-duplicated cell slots against per-task buffers (bytes, pack time, loop time)
+    python bench.py --workload fission     configs[1]: the fused pack against split pack loops (by-struct / by-element / by-type), per layout
 
 `--n N` shrinks the particle count (a power of two for config3/4, N = planes * 128 * 128 is kept for config2) for quick
 runs; the default is the full size of BASELINE.json.  Everything here is harness: the path itself runs in libsph_b200.
@@ -960,10 +961,53 @@ def run_slots(args, sph, torch, common):
             "gpu_launches": 4 * args.steps, "roofline": None, "per_task_ms": t_task, "slots_ms": t_slot, "formats": rows, "e2e": None}
 
 
+def run_fission(args, sph, torch, common):
+    """configs[1], pack of both loops' inputs: the fused pack kernel against the GPU analogues of the paper's split pack loops
+    (Fig. 4): one pass per substruct / per quantity / per data type / per (substruct, type)"""
+    import sph_inputs as si
+    from paper_2606_23891_b200 import layouts as L
+    parts = si.config1(seed=1)
+    perm, cells = sph.sph_cells_build_grid(parts["x"], 16)
+    ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
+    tasks, _, _ = sph.sph_tasks_build(cells, np.full(cells.shape[0], ps["h"].max(), dtype=np.float32))
+    n = ps.shape[0]
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)
+    names = ["aos", "split", "pack-force-type"] if args.layout == "both" else [args.layout]
+    split_names = ["by-struct", "by-element", "by-type", "by-struct-and-type"]
+    rows = {}
+    for name in names:
+        layout = L.layout(sph, name)
+        store = sph.sph_store_create(layout, n)
+        sph.sph_store_set_cells(store, cells)
+        sph.sph_store_import_aos(store, ps)
+        batch = sph.sph_batch_create(store, tasks)
+        row = {}
+        for label, which in (("density_in", 0), ("force_in", 2)):
+            aset = sph.sph_attrset_canonical(which)
+            buf = torch.empty(sph.sph_batch_buffer_bytes(batch, aset), dtype=torch.uint8, device="cuda")
+            t = {"by-particle (fused)": round(min(timed(torch, lambda: sph.sph_pack(store, batch, aset, buf), args.steps, 3, before=flush)), 5)}
+            passes = {}
+            for k, sname in enumerate(split_names):
+                masks = sph.sph_pack_pass_masks(layout, aset, k)
+                t[sname] = round(min(timed(torch, lambda: [sph.sph_pack_pass(store, batch, aset, m, buf) for m in masks], args.steps, 3, before=flush)), 5)
+                passes[sname] = len(masks)
+            row[label] = {"ms": t, "passes": passes, "vs_fused": {k: round(v / t["by-particle (fused)"], 2) for k, v in t.items()}}
+            del buf
+        rows[name] = row
+        sph.sph_batch_destroy(batch)
+        sph.sph_store_destroy(store)
+    base = rows[names[0]]["force_in"]["ms"]["by-particle (fused)"]
+    return {"value": n / (base * 1e-3), "unit": "particles/s", "ms_per_step": base, "dtype": "u8",
+            "config": {"workload": "fission: configs[1], pack DENSITY_IN and FORCE_IN, fused kernel against one pass per substruct / quantity / data type",
+                       "layout": names[0], "store": "HBM", "l2": "flushed before every timed pack (256 MB fill, untimed)"},
+            "gpu_launches": args.steps, "roofline": None, "layouts": rows, "e2e": None}
+
+
 def run_link(args, sph, torch, common):
     link = link_probe(torch, reps=10)
     return {"value": link["h2d_gbs"], "unit": "GB/s", "ms_per_step": None, "dtype": "u8", "metric": "pinned host-link copy bandwidth",
             "config": {"workload": "link: 1 GiB pinned cudaMemcpyAsync, best of 10", "link": link}, "gpu_launches": 0, "roofline": None, "e2e": None}
 
 
-RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link, "eagle": run_eagle, "replay": run_replay, "slots": run_slots}
+RUNNERS = {"config2": run_config2, "config3": run_config3, "config4": run_config4, "link": run_link, "eagle": run_eagle, "replay": run_replay, "slots": run_slots, "fission": run_fission}

@@ -236,6 +236,16 @@ int32_t sph_pack_cells(const sph_store* store, const sph_batch* batch, const sph
                        uint32_t cell_first, uint32_t cell_count, void* stream);
 int32_t sph_unpack_cells(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,
                          int32_t mode, uint32_t cell_first, uint32_t cell_count, void* stream);
+/* ---- split pack loops ("loop fission", Fig. 4) ----
+ * The paper splits the pack loop into several loops that each touch one substruct (by-struct), one quantity (by-element),
+ * one data type (by-type) or one (substruct, type) pair.  GPU analogue: sph_pack_pass writes only the record words named in
+ * word_mask (bit w = 4-byte word w of the record) for every block of the batch; the passes of a partition together write
+ * exactly the bytes of sph_pack.  sph_pack_pass_masks gives the partition: split 0 by-struct, 1 by-element (one attribute
+ * entry each), 2 by-type (f64 / f32 / i64 / i8), 3 by-struct-and-type; masks_out [host, >= 48], n_out [host] their number. */
+int32_t sph_pack_pass_masks(const sph_layout* layout, const sph_attrset* set, int32_t split, uint64_t* masks_out, uint32_t* n_out);
+int32_t sph_pack_pass(const sph_store* store, const sph_batch* batch, const sph_attrset* set, uint64_t word_mask, void* d_buf,
+                      uint64_t buf_bytes, void* stream);
+
 /* ---- de-duplicated cell slots ("data replication") ----
  * A second input format for the loops: every cell the batch touches is packed ONCE into a slot (count records, slots in
  * ascending cell index, each starting at a multiple of 128 bytes) instead of once per task side (about 27 times on a

@@ -22,7 +22,8 @@ __all__ = [
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack",
     "sph_unpack_cells", "sph_ghost", "SPH_SET_GRADIENT_IN", "SPH_SET_GRADIENT_OUT", "SPH_SET_FORCE3_IN",
-    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots",
+    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots", "sph_pack_pass_masks", "sph_pack_pass",
+    "SPLIT_BY_STRUCT", "SPLIT_BY_ELEMENT", "SPLIT_BY_TYPE", "SPLIT_BY_STRUCT_AND_TYPE",
 ]
 
 SPH_NFIELDS, SPH_MAX_SUB, SPH_MAX_ATTR = 18, 8, 32
@@ -43,7 +44,7 @@ EXPORTS = [
     "sph_store_upload_range", "sph_store_download_range", "sph_pack_cells", "sph_unpack_cells",
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_free", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack", "sph_ghost",
-    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots",
+    "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots", "sph_pack_pass_masks", "sph_pack_pass",
 ]
 
 
@@ -336,6 +337,21 @@ def sph_density(batch, d_in, d_out, stream=None) -> None:
 def sph_force(batch, d_in, d_out, params: sph_params, stream=None) -> None:
     _check(_lib.sph_force(batch, _ptr(d_in), C.c_uint64(_nbytes(d_in)), _ptr(d_out), C.c_uint64(_nbytes(d_out)),
                           C.byref(params), _stream(stream)))
+
+
+SPLIT_BY_STRUCT, SPLIT_BY_ELEMENT, SPLIT_BY_TYPE, SPLIT_BY_STRUCT_AND_TYPE = 0, 1, 2, 3
+
+
+def sph_pack_pass_masks(layout: sph_layout, aset: sph_attrset, split: int):
+    """word masks of the passes of a split pack loop"""
+    masks = (C.c_uint64 * 48)()
+    n = C.c_uint32(0)
+    _check(_lib.sph_pack_pass_masks(C.byref(layout), _ref(aset), C.c_int32(split), masks, C.byref(n)))
+    return [int(masks[k]) for k in range(n.value)]
+
+
+def sph_pack_pass(store, batch, aset: sph_attrset, word_mask: int, d_buf, stream=None) -> None:
+    _check(_lib.sph_pack_pass(store, batch, _ref(aset), C.c_uint64(word_mask), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), _stream(stream)))
 
 
 def sph_slot_attrset(loop: int) -> sph_attrset:

@@ -50,6 +50,34 @@ int32_t attrset_check(const sph_attrset* set, uint32_t* rec_bytes) {
     return SPH_OK;
 }
 
+// every record word of (layout, set) as a store location, with the groups the split pack loops partition by
+int32_t build_pass_words(const sph_layout& layout, const sph_attrset& set, PassProgram* all) {
+    uint32_t rec_bytes = 0;
+    if (int32_t rc = attrset_check(&set, &rec_bytes)) return rc;
+    std::memset(all, 0, sizeof(*all));
+    all->rec_words = rec_bytes / 4;
+    uint32_t w = 0;
+    for (uint32_t k = 0; k < set.n; ++k) {
+        const sph_attr& a = set.ent[k];
+        const auto& loc = layout.loc[a.field];
+        const uint16_t stride = (uint16_t)layout.stride[loc.sub];
+        const uint8_t type = a.field == SPH_X ? 0 : (a.field == SPH_ID ? 2 : (a.field == SPH_TIME_BIN ? 3 : 1));
+        auto put = [&](uint32_t off, uint8_t kind, uint8_t comp) {
+            all->sel[w] = PassWord{off, stride, loc.sub, kind, (uint8_t)w, comp, {loc.sub, (uint8_t)k, type, (uint8_t)(loc.sub * 4 + type)}};
+            ++w;
+        };
+        for (uint32_t c = a.comp0; c < (uint32_t)a.comp0 + a.ncomp; ++c) {
+            const uint32_t off = loc.off + c * field_elem_bytes(a.field);
+            if (a.field == SPH_X && (set.flags & SPH_ATTR_X_REL_F32)) put(off, W_XREL, (uint8_t)c);
+            else if (a.field == SPH_X || a.field == SPH_ID) { put(off, W_COPY, 0); put(off + 4, W_COPY, 0); }
+            else if (a.field == SPH_TIME_BIN) put(off, W_TIMEBIN, 0);
+            else put(off, W_COPY, 0);
+        }
+    }
+    all->n_sel = w;
+    return SPH_OK;
+}
+
 // PACK program: which substruct arrays to stage (and which 16-byte pieces of them), the pre-pass, and for every
 // record word the staging offset it is copied from.
 int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog) {
@@ -617,6 +645,45 @@ int32_t sph_force3(const sph_batch* b, const void* d_in, uint64_t in_bytes, void
     const OffsetTable *oin = nullptr, *oout = nullptr;
     if (int32_t rc = loop_check(b, d_in, in_bytes, d_out, out_bytes, 72, 20, &oin, &oout)) return rc;
     return launch_force3(b, (const char*)d_in, (char*)d_out, *prm, (cudaStream_t)stream);
+    SPH_API_END
+}
+
+// ---- split pack loops ----
+
+int32_t sph_pack_pass_masks(const sph_layout* layout, const sph_attrset* set, int32_t split, uint64_t* masks_out, uint32_t* n_out) {
+    if (!layout || !masks_out || !n_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    if (split < 0 || split > 3) return fail(SPH_ERR_INVALID_ARG, "split must be 0 (by-struct), 1 (by-element), 2 (by-type) or 3 (by-struct-and-type)");
+    if (int32_t rc = sph_layout_validate(layout)) return rc;
+    PassProgram all;
+    if (int32_t rc = build_pass_words(*layout, *set, &all)) return rc;
+    uint32_t n = 0;
+    int key_of[kMaxRecWords];
+    for (uint32_t w = 0; w < all.n_sel; ++w) {
+        const int key = all.sel[w].group[split];
+        uint32_t g = 0;
+        while (g < n && key_of[g] != key) ++g;
+        if (g == n) { key_of[n] = key; masks_out[n++] = 0; }
+        masks_out[g] |= 1ull << w;
+    }
+    *n_out = n;
+    return SPH_OK;
+}
+
+int32_t sph_pack_pass(const sph_store* s, const sph_batch* b, const sph_attrset* set, uint64_t word_mask, void* d_buf, uint64_t buf_bytes, void* stream) {
+    if (int32_t rc = transfer_check(s, b, set, d_buf)) return rc;
+    SPH_API_BEGIN
+    PassProgram all, pp;
+    if (int32_t rc = build_pass_words(s->layout, *set, &all)) return rc;
+    if (all.rec_words < 64 && (word_mask >> all.rec_words)) return fail(SPH_ERR_RANGE, "word mask names a word beyond the record's %u", all.rec_words);
+    pp = all;
+    pp.n_sel = 0;
+    for (uint32_t w = 0; w < all.n_sel; ++w)
+        if (word_mask >> w & 1) pp.sel[pp.n_sel++] = all.sel[w];
+    const OffsetTable* ot = nullptr;
+    if (int32_t rc = ensure_offsets(b, all.rec_words * 4, &ot)) return rc;
+    if (buf_bytes < ot->total) return fail(SPH_ERR_RANGE, "buffer of %llu bytes, %llu needed", (unsigned long long)buf_bytes, (unsigned long long)ot->total);
+    if ((uintptr_t)d_buf & 127) return fail(SPH_ERR_INVALID_ARG, "buffer is not 128-byte aligned");
+    return launch_pack_pass(s->view(), pp, b->d_cell_chunks, ot->d_occ_off128, b->d_occ_frames, (char*)d_buf, b->n_cell_chunks, (cudaStream_t)stream);
     SPH_API_END
 }
 

@@ -109,6 +109,23 @@ struct Program {
     uint8_t vec4[kMaxRecWords];    // unpack: words w..w+3 are 16 contiguous, 16-byte aligned bytes of one substruct (all plain f32 words)
 };
 
+// One pass of a split pack loop (PAPER.md:150-152 loop fission): the selected record words only, each read
+// straight from the store and written into its place in every record of every block.
+struct PassWord {
+    uint32_t off;        // byte offset inside the substruct (W_XREL: of the f64 coordinate)
+    uint16_t stride;
+    uint8_t sub, kind;   // W_COPY, W_XREL, W_TIMEBIN
+    uint8_t w, comp;     // record word; W_XREL: which coordinate
+    uint8_t group[4];    // substruct, attribute entry, data type (0 f64, 1 f32, 2 i64, 3 i8), substruct x type
+};
+struct PassProgram {
+    uint32_t rec_words, n_sel;
+    PassWord sel[kMaxRecWords];
+};
+int32_t build_pass_words(const sph_layout& layout, const sph_attrset& set, PassProgram* all);      // every record word, in record order
+int32_t launch_pack_pass(const StoreView& view, const PassProgram& pp, const CellChunk* d_chunks, const uint32_t* d_occ_off128, const double* d_occ_frames,
+                         char* d_buf, uint32_t ncc, cudaStream_t st);
+
 int32_t build_pack_program(const sph_layout& layout, const sph_attrset& set, Program* prog);
 int32_t build_unpack_program(const sph_layout& layout, const sph_attrset& set, int32_t mode, Program* prog);
 

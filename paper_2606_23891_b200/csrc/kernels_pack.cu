@@ -412,6 +412,38 @@ unpack_kernel(StoreView view, Program prog, const CellChunk* __restrict__ cell_c
 
 // ---------------------------------------------------------------------------------------------------------
 
+// ------------------------------------------------------------------------------------------------- pack passes (loop fission)
+//
+// GPU analogue of the paper's split pack loops (by-struct, by-element, by-type, by-struct-and-type): ONE pass
+// writes a subset of the record words -- each selected word is read once per particle straight from its substruct array and
+// stored into its place in the record of every block the cell occurs in.  The passes of a partition together write exactly
+// what the fused pack_kernel writes; every pass re-touches every output sector, which is what the comparison measures.
+__global__ void __launch_bounds__(128)
+pack_pass_kernel(StoreView view, PassProgram pp, const CellChunk* __restrict__ cell_chunks, const uint32_t* __restrict__ occ_off128,
+                 const double* __restrict__ occ_frames, uint32_t n_cell_chunks, char* __restrict__ buf) {
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t rec_bytes = 4 * pp.rec_words;
+    for (uint32_t cc = blockIdx.x * 4 + (threadIdx.x >> 5); cc < n_cell_chunks; cc += gridDim.x * 4) {
+        const CellChunk c = cell_chunks[cc];
+        if (lane >= c.count) continue;
+        const uint64_t p = (uint64_t)c.first + lane;
+        const uint64_t rec0 = (uint64_t)(c.k0 + lane) * rec_bytes;
+        for (uint32_t s = 0; s < pp.n_sel; ++s) {
+            const PassWord w = pp.sel[s];
+            const char* src = view.base[w.sub] + p * w.stride + w.off;
+            if (w.kind == W_XREL) {
+                const double x = *reinterpret_cast<const double*>(src);
+                for (uint32_t o = 0; o < c.nocc; ++o)
+                    *reinterpret_cast<float*>(buf + (uint64_t)occ_off128[c.occ0 + o] * 128 + rec0 + 4 * w.w) = (float)(x - occ_frames[3 * (size_t)(c.occ0 + o) + w.comp]);
+            } else {
+                const uint32_t v = w.kind == W_TIMEBIN ? (uint32_t) * reinterpret_cast<const unsigned char*>(src) : *reinterpret_cast<const uint32_t*>(src);
+                for (uint32_t o = 0; o < c.nocc; ++o)
+                    *reinterpret_cast<uint32_t*>(buf + (uint64_t)occ_off128[c.occ0 + o] * 128 + rec0 + 4 * w.w) = v;
+            }
+        }
+    }
+}
+
 __global__ void zero_kernel(StoreView view, Program prog, uint64_t n) {
     const uint64_t total = n * prog.rec_words;
     for (uint64_t g = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; g < total; g += (uint64_t)gridDim.x * blockDim.x) {
@@ -534,6 +566,17 @@ int32_t launch_unpack(const StoreView& view, const sph_batch* b, const Program& 
     else if (R % 5 == 0) rc = launch_unpack_t<1, 5>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
     else rc = launch_unpack_t<1, 8>(view, b, prog, d_occ_off128, d_buf, last_only, all_sum, from_zero, sms, cc0, ncc, st);
     if (rc) return rc;
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int32_t launch_pack_pass(const StoreView& view, const PassProgram& pp, const CellChunk* d_chunks, const uint32_t* d_occ_off128, const double* d_occ_frames,
+                         char* d_buf, uint32_t ncc, cudaStream_t st) {
+    if (ncc == 0 || pp.n_sel == 0) return SPH_OK;
+    int sms = 0;
+    if (int32_t rc = sm_count(&sms)) return rc;
+    const uint32_t grid = std::min((ncc + 3) / 4, (uint32_t)sms * 16);
+    pack_pass_kernel<<<grid, 128, 0, st>>>(view, pp, d_chunks, d_occ_off128, d_occ_frames, ncc, d_buf);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

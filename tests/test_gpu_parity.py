@@ -822,3 +822,32 @@ def test_cell_slots_equal_per_task_buffers(name):
             assert orc.compare_blocks(cells, sel, rec_out, o_slot.cpu().numpy(), o_task.cpu().numpy()) == -1, (name, loop)
             assert nbytes * 4 < b_in.shape[0] or sel.shape[0] < tasks.shape[0]      # whole task lists: several times fewer input bytes
         g.close()
+
+
+# ------------------------------------------------------------------ split pack loops
+
+@pytest.mark.parametrize("layout", ["aos", "split", "pack-force-type"])
+def test_split_pack_loops_write_what_the_fused_pack_writes(layout):
+    """by-struct, by-element, by-type, by-struct-and-type passes together == the fused pack == the oracle"""
+    from paper_2606_23891_b200 import layouts
+    ps, cells, tasks = case("octree")
+    g = GpuCase(ps, cells, tasks, layouts.layout(sph, layout))
+    for oset in (orc.DENSITY_IN, orc.FORCE_IN, CUSTOM):
+        aset, rec = to_attrset(oset), orc.record_bytes(oset)
+        want = orc.pack(ps, cells, tasks, oset)
+        for split in range(4):
+            masks = sph.sph_pack_pass_masks(g.layout, aset, split)
+            buf = g.buffer(aset, 0xEE)
+            for m in masks:
+                sph.sph_pack_pass(g.store, g.batch, aset, m, buf)
+            torch.cuda.synchronize()
+            assert orc.compare_blocks(cells, tasks, rec, buf.cpu().numpy(), want) == -1, (layout, rec, split)
+        # one pass alone leaves every other word untouched
+        buf = g.buffer(aset, 0xEE)
+        sph.sph_pack_pass(g.store, g.batch, aset, 1 << (rec // 4 - 1), buf)
+        got = buf.cpu().numpy().view(np.uint32)
+        off, _ = orc.block_offsets(cells, tasks, rec)
+        o0 = int(off[0]) // 4
+        blk = got[o0:o0 + int(cells["count"][int(tasks["ci"][0])]) * (rec // 4)].reshape(-1, rec // 4)
+        assert np.all(blk[:, :-1] == 0xEEEEEEEE) and np.array_equal(blk[:, -1], want.view(np.uint32)[o0:o0 + blk.size].reshape(blk.shape)[:, -1])
+    g.close()

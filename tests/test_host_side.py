@@ -37,6 +37,24 @@ def test_slot_attribute_sets():
         sph.sph_slot_attrset(2)
 
 
+def test_split_pack_loop_partitions():
+    """row f4 / PAPER.md:150-152: the passes of every split are a partition of the record's words"""
+    f_in = sph.sph_attrset_canonical(sph.SPH_SET_FORCE_IN)          # x(3) h m rho rho_dh v(3) u P cs: 13 words
+    split, aos = sph.sph_layout_split(), sph.sph_layout_aos()
+    for lay in (split, aos):
+        for mode in range(4):
+            masks = sph.sph_pack_pass_masks(lay, f_in, mode)
+            assert sum(masks) == (1 << 13) - 1 and all(a & b == 0 for i, a in enumerate(masks) for b in masks[i + 1:])
+    # split-AoS: x h m in S0, rho rho_dh in S1, v u P cs in S2; AoS: one struct
+    assert sph.sph_pack_pass_masks(split, f_in, sph.SPLIT_BY_STRUCT) == [0b0000000011111, 0b0000001100000, 0b1111110000000]
+    assert sph.sph_pack_pass_masks(aos, f_in, sph.SPLIT_BY_STRUCT) == [(1 << 13) - 1]
+    assert len(sph.sph_pack_pass_masks(split, f_in, sph.SPLIT_BY_ELEMENT)) == 9
+    assert sph.sph_pack_pass_masks(aos, f_in, sph.SPLIT_BY_TYPE) == [0b111, ((1 << 13) - 1) ^ 0b111]            # f64 coordinates, f32 rest
+    assert len(sph.sph_pack_pass_masks(split, f_in, sph.SPLIT_BY_STRUCT_AND_TYPE)) == 4
+    with pytest.raises(sph.SphError):
+        sph.sph_pack_pass_masks(split, f_in, 4)
+
+
 def test_library_is_built_for_sm_100a_only():
     import subprocess
     out = subprocess.run(["cuobjdump", "-lelf", sph.lib_path()], capture_output=True, text=True).stdout
