@@ -375,6 +375,24 @@ def time_steps(torch, fn, steps, warmup, flush, world):
     return [a.elapsed_time(b) for a, b in ev]
 
 
+def same_size_copy_gbs(torch, nbytes, flush, reps=7):
+    """The yardstick for one HBM-bound launch of `nbytes` algorithmic bytes: a device-to-device copy that moves the same bytes
+    (half read, half written; torch's copy kernel) as ONE launch on a flushed L2, timed with CUDA events the way the kernels
+    are.  The MEASURED_PEAKS figure is a 4 GiB copy; a launch of 100-400 MB pays its ramp-up and tail on a cold L2."""
+    half = max(1 << 20, int(nbytes) // 2)
+    a = torch.empty(half, dtype=torch.uint8, device="cuda")
+    b = torch.empty(half, dtype=torch.uint8, device="cuda")
+    best = None
+    for _ in range(reps):
+        flush()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); b.copy_(a); e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return 2 * half / (best * 1e-3) / 1e9
+
+
 def run_other_workload(args):
     """configs[2..4] and the link probe (bench_workloads.py); single GPU, same JSON contract"""
     import torch
@@ -476,7 +494,7 @@ def run_default(args):
     torch.cuda.set_device(local)
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     alu_peak = N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    common = {"hbm_peak": hbm_peak, "alu_peak": alu_peak, "peak_source": peak_src,
+    common = {"hbm_peak": hbm_peak, "alu_peak": alu_peak, "peak_source": peak_src, "same_size_copy": same_size_copy_gbs,
               "time_steps": lambda torch_, fn, steps, warmup, flush: time_steps(torch_, fn, steps, warmup, flush, world),
               "sampler": (lambda: ClockSampler(local)) if rank == 0 else (lambda: None)}
     t_start = time.perf_counter()
@@ -530,6 +548,19 @@ def run_default(args):
         c4 = bw.run_config4(sub, sph, torch, common)
         work["configs[4]"] = {"workload": c4["config"]["workload"], "e2e_note": c4["config"]["e2e"], "setup": c4["config"]["setup"],
                               "link": c4["config"]["link"], "e2e": c4["e2e"], "roofline": c4["roofline"], "variants": c4["variants"]}
+        # rows (f3) / (f4) of the scope table: extreme occupancy, trace replay, cell slots, split pack loops
+        sub.n, sub.steps, sub.warmup = 0, 5, 3
+        eg = bw.run_eagle(sub, sph, torch, common)
+        work["eagle-like"] = {"workload": eg["config"]["workload"], "setup": eg["config"]["setup"], "ms_per_step": eg["ms_per_step"], "split": eg["split"],
+                              "aos_stages_ms": eg["aos"]["stages_ms"]}
+        sub.steps = 3
+        rp = bw.run_replay(sub, sph, torch, common)
+        work["trace-replay"] = {"workload": rp["config"]["workload"], "layouts": rp["layouts"]}
+        sub.steps = 10
+        sl = bw.run_slots(sub, sph, torch, common)
+        work["cell-slots"] = {"workload": sl["config"]["workload"], "per_task_ms": sl["per_task_ms"], "slots_ms": sl["slots_ms"], "formats": sl["formats"]}
+        fi = bw.run_fission(sub, sph, torch, common)
+        work["split-pack-loops"] = {"workload": fi["config"]["workload"], "layouts": fi["layouts"]}
         line["workloads"] = work
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_config2(state, budget_s=args.cpu_budget)
@@ -613,6 +644,9 @@ def measure_config1(args, sph, torch, rank, world, local):
             else:
                 e.update(bound="alu", achieved=round(alg[k]["flop"] / (d * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s")
             e["frac"] = round(e["achieved"] / e["peak"], 4)
+            if alg[k]["bound"] == "hbm":      # the same bytes as one plain copy launch on a flushed L2 (what a launch of this size can reach at all)
+                e["same_size_copy_gbs"] = round(same_size_copy_gbs(torch, alg[k]["bytes"], flush), 1)
+                e["frac_of_same_size_copy"] = round(e["achieved"] / e["same_size_copy_gbs"], 4)
         kernels[k] = e
     dominant = max(R["per"], key=R["per"].get)
     traffic = None

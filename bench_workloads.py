@@ -305,6 +305,9 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
                          frac_of_nominal_8tbs=round(alg[k] / (ms * 1e-3) / 1e9 / 8000.0, 4))
                 e["frac"] = round(e["achieved"] / hbm_peak, 4)
                 e["instances_per_s"] = inst / (ms * 1e-3)
+                if "same_size_copy" in common:
+                    e["same_size_copy_gbs"] = round(common["same_size_copy"](torch, alg[k], flush), 1)
+                    e["frac_of_same_size_copy"] = round(e["achieved"] / e["same_size_copy_gbs"], 4)
             if k == "force":
                 flop = cand * 8.0 + setup["neighbour_pairs"] * 60.0
                 e.update(bound="alu", achieved=round(flop / (ms * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s",
