@@ -650,11 +650,11 @@ def measure_config1(args, sph, torch, rank, world, local):
         kernels[k] = e
     dominant = max(R["per"], key=R["per"].get)
     traffic = None
-    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch (from ncu --set full)
+    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch,workload (from ncu --set full)
     if os.path.exists(tfile):
         for line in open(tfile):
             c = line.strip().split(",")
-            if len(c) >= 3 and c[0] == dominant and c[1] == primary:
+            if len(c) >= 4 and c[0] == dominant and c[1] == primary and c[3] == "config1":
                 traffic = float(c[2])
     roof = dict(kernels[dominant])
     roof.pop("ms", None)
