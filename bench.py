@@ -540,6 +540,10 @@ def run_default(args):
         sub.steps, sub.warmup = min(args.steps, 20), 3
         c1 = measure_config1(sub, sph, torch, rank, world, local)
         work["configs[1]"] = {k: c1[k] for k in ("value", "unit", "ms_per_step", "config", "kernels", "aos", "e2e", "pair_interactions_per_s")}
+        sub.loops = 3                                     # row (f2): density, gradient, Balsara-switched force (ten launches)
+        c1b = measure_config1(sub, sph, torch, rank, world, local)
+        work["configs[1] three-loop cycle"] = {k: c1b[k] for k in ("value", "unit", "ms_per_step", "kernels", "aos", "e2e")}
+        sub.loops = 2
         sub.steps, sub.warmup, sub.n = 3, 3, args.n3
         c3 = bw.run_config3(sub, sph, torch, common, ks=[5, 13], modes=("streamed",))
         work["configs[3]"] = {"workload": c3["config"]["workload"], "link": c3["config"]["link"], "setup": c3["config"]["setup"],

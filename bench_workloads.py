@@ -297,6 +297,9 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
         inst, cand = info.n_instances, info.n_candidates
         # algorithmic bytes: every record byte once, every touched store field once per particle
         alg = {"pack_force_in": n * 64 + inst * 52, "unpack_force_out": inst * 20 + n * 20}
+        # AoS moves whole 32-byte sectors of the 128-byte record (SURVEY.md 8(d)'s sector table): the pack touches all four, the
+        # unpack writes two (a, du_dt in bytes 32-63; v_sig in 96-127) and DRAM fills the rest of each partially written sector
+        moved = {"pack_force_in": n * 128 + inst * 52, "unpack_force_out": inst * 20 + n * (64 + 64)} if name == "aos" else None
         kern = {}
         for k, ms in per.items():
             e = {"ms": round(ms, 4)}
@@ -305,6 +308,9 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
                          frac_of_nominal_8tbs=round(alg[k] / (ms * 1e-3) / 1e9 / 8000.0, 4))
                 e["frac"] = round(e["achieved"] / hbm_peak, 4)
                 e["instances_per_s"] = inst / (ms * 1e-3)
+                if moved:
+                    e["moved_bytes_sector_model"] = int(moved[k])
+                    e["frac_on_moved_bytes"] = round(moved[k] / (ms * 1e-3) / 1e9 / hbm_peak, 4)
                 if "same_size_copy" in common:
                     e["same_size_copy_gbs"] = round(common["same_size_copy"](torch, alg[k], flush), 1)
                     e["frac_of_same_size_copy"] = round(e["achieved"] / e["same_size_copy_gbs"], 4)
