@@ -195,11 +195,18 @@ def build_config2(sph, torch, seed, n):
 
 
 class Config2E2E:
-    """configs[2] with the particle arrays in pinned HOST memory: per step the substructs the force loop reads cross slab by
-    slab (ranges of cells) and are packed as they land (sph_pack_cells), the force loop runs over all 896 bundles, the results
-    are reduced slab by slab (sph_unpack_cells) and each slab's particles cross back as soon as they are final.  One graph."""
+    """configs[2] with the particle arrays in pinned HOST memory, one step = one CUDA graph:
+      * the substructs the force loop reads cross slab by slab (ranges of cells) and are packed as they land (sph_pack_cells into the
+        one buffer that holds all 896 bundles);
+      * the slabs grow (3/16, 1/16, 1/8, 1/8, 1/4, 1/4 of the particles): the first is what the first tasks need, later ones are
+        large enough to keep launches few -- the loop, not the link, sets the pace once it has started;
+      * the force loop does not wait for the last slab: it runs GROUP by group of bundles (a group = a batch over a run of consecutive
+        segments whose inputs are complete with the same slab; its buffers are the matching slices of the big ones, a segmented batch
+        being the concatenation of its bundles' stand-alone buffers), each group as soon as that slab is packed -- so most of the loop
+        overlaps the uploads; groups whose tasks reach through the periodic boundary to the far end of the cell table run last;
+      * the results are reduced slab by slab (sph_unpack_cells) and each slab's particles cross back as soon as they are final."""
 
-    def __init__(self, sph, torch, layout, store, batch, cells, n, bufs, params, n_slabs=8):
+    def __init__(self, sph, torch, layout, store, batch, cells, tasks, n, bufs, params, fractions=(3, 1, 2, 2, 4, 4), max_segs_per_group=1 << 30, bundle=512):
         self.sph, self.torch, self.store, self.batch, self.bufs, self.params = sph, torch, store, batch, bufs, params
         F = sph.FIELD
         sub = lambda names: sorted({layout.loc[F[k]].sub for k in names})
@@ -211,9 +218,29 @@ class Config2E2E:
         torch.cuda.synchronize()
         self.h2d_bytes = sum(n * layout.stride[s] for s in self.subs_in)
         self.d2h_bytes = sum(n * layout.stride[s] for s in self.subs_out)
-        self.slabs = cell_slabs(cells, n_slabs)
+        self.slabs = cell_slabs(cells, fractions=fractions)
         self.up, self.down = torch.cuda.Stream(), torch.cuda.Stream()
+        self.loop_streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         self.s_in, self.s_out = sph.sph_attrset_canonical(2), sph.sph_attrset_canonical(3)
+        # groups = runs of consecutive segments whose inputs are complete with the same slab
+        _, seg_in = sph.sph_batch_block_offsets(batch, self.s_in)
+        _, seg_out = sph.sph_batch_block_offsets(batch, self.s_out)
+        slab_end = np.array([c0 + nc for c0, nc, _, _ in self.slabs])
+        n_seg = seg_in.shape[0]
+        top = np.maximum(tasks["ci"], tasks["cj"]).astype(np.int64)
+        seg_top = np.maximum.reduceat(top, np.arange(0, tasks.shape[0], bundle))
+        seg_need = np.searchsorted(slab_end, seg_top, side="right")
+        assert seg_need.shape[0] == n_seg
+        self.groups = []
+        g0 = 0
+        while g0 < n_seg:
+            g1 = g0 + 1
+            while g1 < n_seg and seg_need[g1] == seg_need[g0] and g1 - g0 < max_segs_per_group:
+                g1 += 1
+            gb = sph.sph_batch_create(store, tasks[g0 * bundle:min(tasks.shape[0], g1 * bundle)], bundle)
+            self.groups.append({"batch": gb, "need": int(seg_need[g0]), "in": bufs[0][int(seg_in[g0]):], "out": bufs[1][int(seg_out[g0]):], "first": g0})
+            g0 = g1
+        self.order = sorted(range(len(self.groups)), key=lambda k: (self.groups[k]["need"], k))
 
     def step(self, main):
         sph, torch = self.sph, self.torch
@@ -221,12 +248,25 @@ class Config2E2E:
         start = ev(main)
         self.up.wait_event(start)
         self.down.wait_event(start)
-        for c0, nc, p0, npart in self.slabs:
+        todo = list(self.order)
+        for st in self.loop_streams:
+            st.wait_event(start)
+        n_launched = 0
+        for k, (c0, nc, p0, npart) in enumerate(self.slabs):
             for s in self.subs_in:
                 sph.sph_store_upload_range(self.store, s, self.host[s], p0, npart, self.up)
             main.wait_event(ev(self.up))
             sph.sph_pack_cells(self.store, self.batch, self.s_in, self.bufs[0], c0, nc, main)
-        sph.sph_force(self.batch, self.bufs[0], self.bufs[1], self.params, main)
+            packed = ev(main)
+            while todo and self.groups[todo[0]]["need"] <= k:          # every slab this group's tasks touch is packed
+                g = self.groups[todo.pop(0)]
+                st = self.loop_streams[n_launched & 1]                  # two streams: a group's tail overlaps the next group's start
+                st.wait_event(packed)
+                sph.sph_force(g["batch"], g["in"], g["out"], self.params, st)
+                n_launched += 1
+        assert not todo
+        for st in self.loop_streams:
+            main.wait_event(ev(st))
         for c0, nc, p0, npart in self.slabs:
             sph.sph_unpack_cells(self.store, self.batch, self.s_out, self.bufs[1], c0, nc, sph.SPH_UNPACK_REDUCE_ZERO, main)
             self.down.wait_event(ev(main))
@@ -244,6 +284,12 @@ class Config2E2E:
         with torch.cuda.graph(self.graph, stream=root):
             self.step(root)
         return self.graph
+
+    def close(self):
+        self.graph = None
+        for g in self.groups:
+            self.sph.sph_batch_destroy(g["batch"])
+        self.groups = []
 
 
 def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
@@ -283,7 +329,7 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
             for k, fn in stages:
                 per[k].append(ev_time(torch, fn))
         per = {k: sum(v) / len(v) for k, v in per.items()}
-        e2e = Config2E2E(sph, torch, layout, store, batch, cells, n, (b_in, b_out), params)
+        e2e = Config2E2E(sph, torch, layout, store, batch, cells, tasks, n, (b_in, b_out), params)
         g = e2e.capture()
         t_e2e = time_steps(torch, g.replay, args.steps, args.warmup, flush)
         # one bundle alone (isolated latency of pack + force + unpack of 512 pair tasks)
@@ -323,7 +369,7 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
         out[name] = {"ms": sum(t) / len(t), "ms_e2e": sum(t_e2e) / len(t_e2e), "kernels": kern, "single_bundle_ms": sum(t_one) / len(t_one),
                      "tasks": int(info.n_tasks), "bundles": int(info.n_segments), "instances": int(inst), "candidate_pairs": int(cand),
                      "h2d_bytes": e2e.h2d_bytes, "d2h_bytes": e2e.d2h_bytes, "clocks": clocks, "n": n}
-        e2e.graph = None
+        e2e.close()
         sph.sph_batch_destroy(batch)
         sph.sph_store_destroy(store)
         del b_in, b_out, o_in, o_out, e2e, g
@@ -397,14 +443,18 @@ def field_bytes(comps):
     return sum(8 if f == "x" else 4 for f, _ in comps)
 
 
-def cell_slabs(cells, n_slabs):
-    """[(cell_first, cell_count, particle_first, particle_count)]: contiguous cell ranges of about equal particle counts"""
+def cell_slabs(cells, n_slabs=0, fractions=None):
+    """[(cell_first, cell_count, particle_first, particle_count)]: contiguous cell ranges of about equal particle counts, or of the
+    given relative sizes (fractions: weights, e.g. (3, 1, 2, 2, 4, 4))"""
     first = cells["first"].astype(np.int64)
     end = first + cells["count"].astype(np.int64)
     n = int(end[-1])
+    if fractions is None:
+        fractions = [1] * n_slabs
+    cum = np.cumsum(fractions) / float(sum(fractions))
     cuts = [0]
-    for k in range(1, n_slabs):
-        c = int(np.searchsorted(end, k * n // n_slabs))
+    for k in range(len(fractions) - 1):
+        c = int(np.searchsorted(end, int(cum[k] * n)))
         cuts.append(max(c, cuts[-1]))
     cuts.append(cells.shape[0])
     out = []
@@ -573,8 +623,11 @@ class Pipeline:
     mode "zero-copy": the same kernels read and write the mapped host store directly over the host link.
     """
 
-    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode, n_slabs=16):
+    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode, n_slabs=16, group=1):
+        """group: bundles under ONE launch per stage and stream (a batch of `group` segments of `bundle` tasks: every bundle keeps its own
+        buffer slice, laid out and reduced exactly like a stand-alone bundle)"""
         self.sph, self.torch, self.layout, self.hs, self.mode = sph, torch, layout, hs, mode
+        self.group, self.span = group, bundle * group
         n = hs.n
         self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
         self.params = sph.sph_params(np.float32(GAMMA), 0.8, 3.0)
@@ -588,8 +641,8 @@ class Pipeline:
         self.batches = []
         self.first_task = []          # first task of every bundle
         for lo, hi in ((0, n_self), (n_self, tasks.shape[0])):          # homogeneous bundles: self tasks, then pair tasks (C22)
-            for s in range(lo, hi, bundle):
-                self.batches.append(sph.sph_batch_create(hs.store, tasks[s:min(hi, s + bundle)]))
+            for s in range(lo, hi, self.span):
+                self.batches.append(sph.sph_batch_create(hs.store, tasks[s:min(hi, s + self.span)], bundle if group > 1 else 0))
                 self.first_task.append(s)
         self.n_self_bundles = sum(1 for s in self.first_task if s < n_self)
         self.n_self, self.n_tasks, self.bundle = n_self, int(tasks.shape[0]), bundle
@@ -598,6 +651,7 @@ class Pipeline:
         need = [0, 0, 0, 0]
         self.instances = 0
         self.candidates = 0
+        self.n_bundles = sum(-(-(min(hi, s + self.span) - s) // bundle) for lo, hi in ((0, n_self), (n_self, tasks.shape[0])) for s in range(lo, hi, self.span))
         for b in self.batches:
             for k in range(4):
                 need[k] = max(need[k], sph.sph_batch_buffer_bytes(b, self.sets[k]))
@@ -638,7 +692,7 @@ class Pipeline:
             st, bufs = self.streams[b & 1], self.bufs[b & 1]
             if slab_events is not None:
                 if b < self.n_self_bundles:          # self tasks [t0, t1) = cells [t0, t1): wait for the slab holding the last one
-                    last_cell = min(self.first_task[b] + self.bundle, self.n_self) - 1
+                    last_cell = min(self.first_task[b] + self.span, self.n_self) - 1
                     st.wait_event(slab_events[int(np.searchsorted(self.slab_cell_end, last_cell, side="right"))])
                 elif not waited_all[b & 1]:
                     st.wait_event(slab_events[-1])
@@ -688,7 +742,7 @@ class Pipeline:
             if not staged or b < self.n_self_bundles:
                 continue
             # every task with ci < frontier is unpacked once bundle b is: those cells are final
-            nxt = self.first_task[b] + self.bundle
+            nxt = self.first_task[b] + self.span
             frontier = int(self.task_ci[nxt]) if nxt < self.n_tasks else int(self.slab_cell_end[-1])
             while done_slab < len(self.slabs) and self.slab_cell_end[done_slab] <= frontier:
                 _, _, p0, npart = self.slabs[done_slab]
@@ -721,6 +775,9 @@ class Pipeline:
             self.sph.sph_store_destroy(self.dev)
 
 
+CONFIG4_GROUP = 8      # bundles of 4,096 tasks under one launch per stage and stream
+
+
 def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
     n = args.n or (1 << 26)
     ps, cells, tasks, setup = build_clumpy(sph, 4, 1, n)
@@ -733,13 +790,14 @@ def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
         for mode in ("staged", "zero-copy"):
             if mode == "zero-copy" and args.skip_zero_copy:
                 continue
-            pl = Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, mode)
+            pl = Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, mode, group=CONFIG4_GROUP)
             t0 = time.perf_counter()
             g = pl.capture()
             cap_s = time.perf_counter() - t0
             t = timed(torch, g.replay, args.steps, min(args.warmup, 2))
             ms = sum(t) / len(t)
-            res[f"{name}/{mode}"] = {"ms_per_step": ms, "particles_per_s": n / (ms * 1e-3), "bundles": len(pl.batches), "launches_per_step": pl.launches,
+            res[f"{name}/{mode}"] = {"ms_per_step": ms, "particles_per_s": n / (ms * 1e-3), "bundles": pl.n_bundles, "bundles_per_launch": pl.group,
+                                     "launches_per_step": pl.launches,
                                      "h2d_bytes_per_step": pl.h2d_bytes, "d2h_bytes_per_step": pl.d2h_bytes,
                                      "h2d_bytes_if_no_device_shadow": pl.h2d_bytes + pl.shadow_bytes,
                                      "link_gbs": round((pl.h2d_bytes + pl.d2h_bytes) / (ms * 1e-3) / 1e9, 2) if mode == "staged" else None,
@@ -757,7 +815,7 @@ def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
             "step_over_link_time": None if not link_time else round(P["ms_per_step"] / link_time, 2),
             "peak_source": "pinned H2D / D2H copy bandwidth measured in this run"}
     return {"value": P["particles_per_s"], "unit": "particles/s", "ms_per_step": P["ms_per_step"], "dtype": "f32",
-            "config": {"workload": f"configs[4]: {n} particles (uniform + clumps), whole step in bundles of 4096 tasks over 2 streams, store in pinned host memory",
+            "config": {"workload": f"configs[4]: {n} particles (uniform + clumps), whole step in bundles of 4096 tasks ({CONFIG4_GROUP} under one launch per stage) over 2 streams, store in pinned host memory",
                        "layout": key, "store": "pinned host", "l2": "inputs larger than L2", "setup": setup, "link": link,
                        "e2e": "staged: density inputs cross slab by slab ahead of the bundles, force inputs (v, u) during the density loop, results "
                               "behind the bundles; what the density loop and the ghost left on the device (rho, rho_dh, P, c_s; x, h, mass) is not "

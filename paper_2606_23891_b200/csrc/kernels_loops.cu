@@ -993,10 +993,6 @@ int32_t launch_gradient(const sph_batch* b, const char* d_in, char* d_out, cudaS
     return SPH_OK;
 }
 
-#ifndef SPH_UNITS_MAX_MEAN_BLOCK
-#define SPH_UNITS_MAX_MEAN_BLOCK 80
-#endif
-
 template <bool SWITCH, bool SLOTS>
 static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const double* item_frames, const char* d_in, char* d_out, const sph_params& prm, cudaStream_t st) {
     if (b->n_items == 0) return SPH_OK;
@@ -1004,7 +1000,9 @@ static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const d
     constexpr size_t smem = sizeof(ForceWarpSmemT<SLOTS ? 17 : (SWITCH ? 18 : 13)>) * kLoopWarps;
     // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
     // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
-    const bool units = b->n_sides && b->n_instances <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * b->n_sides;
+    // The choice is a property of the STORE's cell table (mean occupancy of its non-empty cells, taken at sph_batch_create), so
+    // every batch over one store -- a whole task list or any group of its bundles -- runs the same arithmetic, bit for bit.
+    const bool units = b->loop_units;
     if (int32_t rc = units ? loop_grid(force_kernel<true, SWITCH, SLOTS>, smem, &full_grid) : loop_grid(force_kernel<false, SWITCH, SLOTS>, smem, &full_grid)) return rc;
     const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
     if (units) force_kernel<true, SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);

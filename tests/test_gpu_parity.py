@@ -211,8 +211,9 @@ def test_force_loop_vs_oracle(name):
     g = GpuCase(ps, cells, tasks)
     # the force loop has two instantiations, picked by the batch's mean block size (<= 80: "units", else "walk"): both are covered
     info = sph.sph_batch_get_info(g.batch)
-    mean_block = info.n_instances / info.n_sides
-    assert (mean_block <= 80) == (name in ("config0", "ragged")), (name, mean_block)
+    mean_cell = ps.shape[0] / int((cells["count"] > 0).sum())
+    assert info.force_units == int(mean_cell <= 80), (name, mean_cell)
+    assert info.force_units == int(name in ("config0", "ragged")), (name, mean_cell)
     d_in = torch.from_numpy(buf_in).cuda()
     d_out = g.buffer(to_attrset(orc.FORCE_OUT))
     sph.sph_force(g.batch, d_in, d_out, PARAMS)

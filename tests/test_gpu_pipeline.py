@@ -102,6 +102,71 @@ def test_pipeline_equals_one_stream_run_and_oracle(layout_name, mode):
     hs.close()
 
 
+def test_pipeline_with_grouped_bundles_equals_one_bundle_per_launch():
+    """bench.py runs configs[4] with several bundles of 4,096 tasks under one launch per stage (a batch of segments): the host store
+    ends up bit for bit as with one bundle per launch, which the test above ties to the one-stream run and to the oracle"""
+    c = small_config4()
+    ps, cells, tasks = c["ps"], c["cells"], c["tasks"]
+    n_self = int(cells.shape[0])
+    layout = sph.sph_layout_split()
+    out = []
+    for group in (1, 4):
+        hs = bw.HostStore(sph, torch, layout, ps, cells)
+        pl = bw.Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, "staged", group=group)
+        assert pl.n_bundles == -(-n_self // 4096) + -(-(tasks.shape[0] - n_self) // 4096)
+        pl.capture().replay()
+        torch.cuda.synchronize()
+        got = np.zeros_like(ps)
+        sph.sph_store_export_aos(hs.store, got)
+        out.append((canon(got), len(pl.batches)))
+        pl.close()
+        hs.close()
+    assert out[1][1] < out[0][1] and np.array_equal(out[0][0], out[1][0])
+
+
+@pytest.mark.parametrize("layout_name", ["split", "aos"])
+def test_config2_e2e_graph_equals_plain_step(layout_name):
+    """bench.py's configs[2] end-to-end step (bench_workloads.Config2E2E: slab-wise uploads and packs, the force loop launched per
+    group of bundles as its slabs land, slab-wise unpacks and downloads, one CUDA graph) leaves in the HOST arrays exactly what the
+    three plain launches leave in the store; reduced instance (31,744 particles, 8^3 cells, 14 bundles of 512 tasks)."""
+    ps, cells, tasks, _ = bw.build_config2(sph, torch, 3, 1 << 15)
+    n = ps.shape[0]
+    layout = sph.sph_layout_split() if layout_name == "split" else sph.sph_layout_aos()
+    store = sph.sph_store_create(layout, n)
+    sph.sph_store_set_cells(store, cells)
+    sph.sph_store_import_aos(store, ps)
+    batch = sph.sph_batch_create(store, tasks, 512)
+    s_in, s_out = sph.sph_attrset_canonical(2), sph.sph_attrset_canonical(3)
+    b_in = torch.empty(sph.sph_batch_buffer_bytes(batch, s_in), dtype=torch.uint8, device="cuda")
+    b_out = torch.empty(sph.sph_batch_buffer_bytes(batch, s_out), dtype=torch.uint8, device="cuda")
+    e2e = bw.Config2E2E(sph, torch, layout, store, batch, cells, tasks, n, (b_in, b_out), PARAMS, fractions=(1, 1, 2, 4), max_segs_per_group=3)
+    assert len(e2e.groups) >= 5 and len(e2e.slabs) == 4 and sorted(e2e.order) == list(range(len(e2e.groups)))
+    # the plain step
+    sph.sph_pack(store, batch, s_in, b_in)
+    sph.sph_force(batch, b_in, b_out, PARAMS)
+    sph.sph_unpack(store, batch, s_out, b_out, sph.SPH_UNPACK_REDUCE_ZERO)
+    torch.cuda.synchronize()
+    want = {s: torch.empty(n * layout.stride[s], dtype=torch.uint8) for s in e2e.subs_out}
+    for s, h in want.items():
+        sph.sph_store_download_sub(store, s, h)
+    torch.cuda.synchronize()
+    assert any(int(h.view(torch.int32).abs().max()) for h in want.values())
+    # the graph, from poisoned buffers and (where the substruct holds no input) poisoned host outputs
+    b_in.fill_(0x7F); b_out.fill_(0x7F)
+    for s in e2e.subs_out:
+        if s not in e2e.subs_in:
+            e2e.host[s].fill_(0x5A)
+    g = e2e.capture()
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    for s in e2e.subs_out:
+        assert torch.equal(e2e.host[s], want[s]), (layout_name, s)
+    e2e.close()
+    sph.sph_batch_destroy(batch)
+    sph.sph_store_destroy(store)
+
+
 # ------------------------------------------------------------------ bench.py's end-to-end step (host-resident arrays, three streams, one graph)
 
 def _bench_layout_cases():
