@@ -119,9 +119,6 @@ typedef struct {
     uint32_t max_count;      /* largest block */
     uint64_t n_items;              /* work items of an interaction loop: (<= 64 targets of a block) x (the block they gather from) */
     uint64_t max_item_candidates;  /* candidate pairs of the largest item: what one warp works through alone (load balance) */
-    uint32_t force_units;          /* 1: the force loop runs its small-cell instantiation for this batch, 0: the large-cell one; a
-                                    * property of the store's cell table (mean occupancy <= 80), the same for every batch over it */
-    uint32_t reserved;
 } sph_batch_info;
 
 /* ---- errors ---- */

@@ -71,7 +71,7 @@ class sph_params(C.Structure):
 class sph_batch_info(C.Structure):
     _fields_ = [("n_tasks", C.c_uint64), ("n_self", C.c_uint64), ("n_pair", C.c_uint64), ("n_sides", C.c_uint64),
                 ("n_instances", C.c_uint64), ("n_candidates", C.c_uint64), ("n_cells_touched", C.c_uint64),
-                ("n_segments", C.c_uint32), ("max_count", C.c_uint32), ("n_items", C.c_uint64), ("max_item_candidates", C.c_uint64), ("force_units", C.c_uint32), ("reserved", C.c_uint32)]
+                ("n_segments", C.c_uint32), ("max_count", C.c_uint32), ("n_items", C.c_uint64), ("max_item_candidates", C.c_uint64)]
 
 
 CELL_DTYPE = np.dtype({"names": ["first", "count", "pad", "origin", "width"],

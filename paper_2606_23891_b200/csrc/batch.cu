@@ -126,11 +126,6 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     b->n_tasks = n_tasks;
     b->store_n = store->n;
     b->cells_hash = store->cells_hash;
-    {
-        uint64_t nonempty = 0;
-        for (const sph_cell& ce : store->cells) nonempty += ce.count > 0;
-        b->loop_units = store->n <= (uint64_t)SPH_UNITS_MAX_MEAN_BLOCK * std::max<uint64_t>(nonempty, 1);
-    }
     b->tasks_per_segment = tasks_per_segment;
     b->n_segments = tasks_per_segment ? (uint32_t)((n_tasks + tasks_per_segment - 1) / tasks_per_segment) : 1;
     std::vector<double> frames;
@@ -258,7 +253,6 @@ int32_t sph_batch_get_info(const sph_batch* b, sph_batch_info* info) {
     info->n_tasks = b->n_tasks; info->n_self = b->n_self; info->n_pair = b->n_pair; info->n_sides = b->n_sides;
     info->n_instances = b->n_instances; info->n_candidates = b->n_candidates; info->n_cells_touched = b->n_cells_touched;
     info->n_segments = b->n_segments; info->max_count = b->max_count; info->n_items = b->n_items; info->max_item_candidates = b->max_item_candidates;
-    info->force_units = b->loop_units ? 1u : 0u; info->reserved = 0;
     return SPH_OK;
 }
 

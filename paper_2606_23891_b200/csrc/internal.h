@@ -61,9 +61,6 @@ struct CellChunk {
     uint32_t nocc;
 };
 
-#ifndef SPH_UNITS_MAX_MEAN_BLOCK
-#define SPH_UNITS_MAX_MEAN_BLOCK 80
-#endif
 constexpr uint32_t kLoopTargets = 64;
 // work item of the density / force loops: up to 64 targets of one block (two per lane) against the block they gather from.  Offsets in units of 128 bytes into the loop's input / output buffer (chunk starts are multiples of 128 bytes).
 struct LoopItem {
@@ -179,7 +176,6 @@ struct sph_batch {
     uint32_t n_sides = 0, n_cell_chunks = 0, n_occ = 0, n_segments = 1, tasks_per_segment = 0, max_count = 0, max_nocc = 0;
     uint64_t n_instances = 0, n_candidates = 0, n_cells_touched = 0, store_n = 0, max_item_candidates = 0;
     uint64_t cells_hash = 0;                  // of the cell table the batch was built against
-    bool loop_units = true;                   // force loop: the UNITS instantiation (small cells) or the WALK one (kernels_loops.cu)
     std::vector<sph::SideRec> sides;          // host copy
     std::vector<uint32_t> occ_side;           // host copy of the occurrence lists
     std::vector<uint32_t> task_side0;         // n_tasks + 1

@@ -645,14 +645,6 @@ __device__ __forceinline__ ForcePair2 force_pair2(const ForceTargets2& T, const 
     return o;
 }
 
-// sum += a * b with the rounding error of the addition carried in c (Kahan), for a pair of sums
-__device__ __forceinline__ void kahan2(u64& sum, u64& c, u64 a, u64 b) {
-    const u64 y = fma2(a, b, c);          // c holds minus the error so far
-    const u64 t = add2(sum, y);
-    c = sub2(y, sub2(t, sum));            // y - (t - sum): what the addition dropped
-    sum = t;
-}
-
 // Balsara-type switch (reading C34): B = |div v| / (|div v| + |rot v| + 1e-4 c_s / h)
 __device__ __forceinline__ float balsara(const float* r) {      // r: a FORCE3_IN record
     const float div = fabsf(r[13]), rot = sqrtf(fmaf(r[14], r[14], fmaf(r[15], r[15], r[16] * r[16])));
@@ -666,7 +658,7 @@ __device__ __forceinline__ u64 switch_pair(const Smem& sm, uint32_t a, uint32_t 
     else return 0ull;
 }
 
-template <bool UNITS, bool SWITCH, bool SLOTS>
+template <bool SWITCH, bool SLOTS>
 __global__ void __launch_bounds__(kLoopWarps * 32, SPH_FORCE_MINB)
 force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, char* __restrict__ out, uint32_t n_items, float alpha, float beta,
              const double* __restrict__ item_frames) {
@@ -758,46 +750,24 @@ force_kernel(const LoopItem* __restrict__ items, const char* __restrict__ in, ch
             const FilterTarget fB = filter_target(pB.x, pB.y, pB.z, wB ? fmaf(pB.x, pB.x, fmaf(pB.y, pB.y, pB.z * pB.z)) - cutB - kFilterEps * (b2 + cutB) : kNever);
             uint32_t m[4];
             filter_masks(sm.f, cnt, dual, fA, fB, m);
-            // Phase 2, two ways (two instantiations of the kernel; the launcher picks one from the batch's mean block size).
-            //  WALK: every lane walks the set bits of its own targets' masks, one neighbour of target A and one of target B per
-            //        iteration (or two of target A when it has one target).  Best when the targets have about as many neighbours
-            //        each (a cell against itself, large cells).
-            //  UNITS: inside a pair of small cells the number of neighbours per target is heavy-tailed (0 .. ~30: targets next to
-            //        the other cell against targets three layers away) and walking leaves most of the warp idle.  Instead
-            //        (a) every lane cuts its masks into units (target, <= 4 set bits of one mask word), numbered RANK-major over the
-            //            lanes (all first units, then all second units, ...: making the units, and adding up their partial sums,
-            //            takes as many warp steps as the busiest lane has units);
-            //        (b) the units are evaluated 32 at a time, one per lane, each leaving its partial sums in shared memory;
-            //        (c) the lane that made a unit adds its partial sums to the target's running sums, in unit order.
+            // Phase 2.  Inside a pair of cells the number of neighbours per target is heavy-tailed (0 .. ~30: targets next to the
+            // other cell against targets three layers away), so lanes that walked their own targets' masks would leave most of
+            // the warp idle.  Instead
+            //   (a) every lane cuts its masks into UNITS (target, <= 4 set bits of one mask word), numbered RANK-major over the
+            //       lanes (all first units, then all second units, ...: making the units, and adding up their partial sums,
+            //       takes as many warp steps as the busiest lane has units);
+            //   (b) the units are evaluated 32 at a time, one per lane, each leaving its partial sums in shared memory;
+            //   (c) the lane that made a unit adds its partial sums to the target's running sums, in unit order.
             // Acceleration sums ~60 terms an order of magnitude larger than the result (pressure forces cancel): compensated (Kahan)
-            // adds keep the rounding of the running sums out of the 1e-6 max|a| budget, in both ways.
+            // adds keep the rounding of the running sums out of the 1e-6 max|a| budget.
+            // (r01 / early r02 also had a WALK instantiation for large cells -- every lane walking its own two targets' masks; with
+            // particles in Morton order inside cells the units win on every workload: eagle-like force 32.6 -> 26.0 ms, configs[4]
+            // at 2^23 particles 42.5 -> 39.1 ms per step, configs[2] 3.83 -> 3.44 ms, configs[1] 413 -> 349 us -- so it is gone.)
             const uint32_t cA0 = __popc(m[0]), cA1 = __popc(m[1]), cB0 = __popc(m[2]), cB1 = __popc(m[3]);
             const uint32_t nuA = (cA0 + kUnitBits - 1) / kUnitBits + (cA1 + kUnitBits - 1) / kUnitBits;
             const uint32_t nuB = (cB0 + kUnitBits - 1) / kUnitBits + (cB1 + kUnitBits - 1) / kUnitBits, nu = nuA + nuB;
             float axA = 0.f, ayA = 0.f, azA = 0.f, duA = 0.f, vsA = 0.f, axB = 0.f, ayB = 0.f, azB = 0.f, duB = 0.f, vsB = 0.f;
-            if constexpr (!UNITS) {
-                const float4 qA = sm.t1[tA], qB = sm.t1[tB], sA = sm.t2[tA], sB = sm.t2[tB];
-                const ForceTargets2 T{pack2(pA.x, pB.x), pack2(pA.y, pB.y), pack2(pA.z, pB.z), pack2(qA.x, qB.x), pack2(qA.y, qB.y), pack2(qA.z, qB.z),
-                                      pack2(qA.w, qB.w), pack2(sA.x, sB.x), pack2(sA.y, sB.y), pack2(sA.z, sB.z), pack2(sA.w, sB.w), pA.w, pB.w,
-                                      switch_pair<SWITCH>(sm, tA, tB, true)};
-                u64 ax = 0, ay = 0, az = 0, du = 0, cx = 0, cy = 0, cz = 0;
-                float vsig0 = 0.f, vsig1 = 0.f;
-                auto hits = [&](uint32_t ma, uint32_t mb, uint32_t base) {
-                    uint32_t ja, jb;
-                    while (next_hits(dual, ma, mb, &ja, &jb)) {
-                        const ForcePair2 o = force_pair2<SWITCH>(T, K, sm.ta[base + ja], sm.ta[base + jb], sm.tb[base + ja], sm.tb[base + jb], sm.tc[base + ja],
-                                                                 sm.tc[base + jb], switch_pair<SWITCH>(sm, base + ja, base + jb, false));
-                        kahan2(ax, cx, o.fr, o.ex); kahan2(ay, cy, o.fr, o.ey); kahan2(az, cz, o.fr, o.ez);
-                        du = fma2(o.dg, o.vr, du);
-                        vsig0 = fmaxf(vsig0, o.vsa); vsig1 = fmaxf(vsig1, o.vsb);
-                    }
-                };
-#pragma unroll 1
-                for (uint32_t h = 0; h < 2 && 32 * h < cnt; ++h) hits(h ? m[1] : m[0], h ? m[3] : m[2], h * kHalf);
-                unpack2(ax, axA, axB); unpack2(ay, ayA, ayB); unpack2(az, azA, azB); unpack2(du, duA, duB);
-                vsA = vsig0; vsB = vsig1;
-                if (!dual) { axA += axB; ayA += ayB; azA += azB; duA += duB; vsA = fmaxf(vsA, vsB); }
-            } else {
+            {
                 const uint32_t max_nu = __reduce_max_sync(kFull, nu);
                 __syncwarp();     // the filter has read sm.f: its first bytes now hold the unit list
                 uint32_t* upos = reinterpret_cast<uint32_t*>(&sm.f);                        // [kUnitCap] the unit's (up to) four bits of a mask word
@@ -998,15 +968,9 @@ static int32_t launch_force_t(const sph_batch* b, const LoopItem* items, const d
     if (b->n_items == 0) return SPH_OK;
     uint32_t full_grid = 0;
     constexpr size_t smem = sizeof(ForceWarpSmemT<SLOTS ? 17 : (SWITCH ? 18 : 13)>) * kLoopWarps;
-    // Small cells (a few tens of particles: neighbour counts per target inside a cell pair are heavy-tailed) take the UNITS
-    // way of phase 2, large cells the WALK way (measured: 64 per cell 332 vs 357 us; octree leaves of 131 on average 73 vs 65 ms).
-    // The choice is a property of the STORE's cell table (mean occupancy of its non-empty cells, taken at sph_batch_create), so
-    // every batch over one store -- a whole task list or any group of its bundles -- runs the same arithmetic, bit for bit.
-    const bool units = b->loop_units;
-    if (int32_t rc = units ? loop_grid(force_kernel<true, SWITCH, SLOTS>, smem, &full_grid) : loop_grid(force_kernel<false, SWITCH, SLOTS>, smem, &full_grid)) return rc;
+    if (int32_t rc = loop_grid(force_kernel<SWITCH, SLOTS>, smem, &full_grid)) return rc;
     const uint32_t grid = min((b->n_items + kLoopWarps - 1) / kLoopWarps, full_grid);
-    if (units) force_kernel<true, SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);
-    else force_kernel<false, SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);
+    force_kernel<SWITCH, SLOTS><<<grid, kLoopWarps * 32, smem, st>>>(items, d_in, d_out, b->n_items, prm.alpha, prm.beta, item_frames);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
