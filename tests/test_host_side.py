@@ -288,3 +288,50 @@ def test_tasks_reject_a_cell_that_sees_its_own_image():
     with pytest.raises(sph.SphError) as e:
         sph.sph_tasks_build(cells, np.full(8, 0.3, dtype=np.float32))
     assert e.value.code == 3
+
+
+def test_eagle_like_occupancies_have_the_papers_statistics():
+    """row (f3), reading C37: PAPER.md:164 gives per-cell min 5, max 125,113, mean 184, median 109 for Eagle25"""
+    c = si.eagle_like_counts(seed=1, n_cells=32 ** 3)
+    assert c.min() == 5 and c.max() == 125113
+    assert 100 <= np.median(c) <= 118 and 170 <= c.mean() <= 200
+    small = si.eagle_like(seed=3, cells_per_dim=4, n_max=20000)
+    perm, cells = sph.sph_cells_build_grid(small["x"], 4)
+    assert cells["count"].min() == 5 and cells["count"].max() == 20000 and int(cells["count"].sum()) == small.shape[0]
+    # a cell's particles keep h <= half the cell width, so the 27-cell stencil holds whatever the occupancy
+    assert float(small["h"].max()) < 0.5 * 0.25
+    assert np.array_equal(np.sort(small["id"]), np.arange(small.shape[0]))
+
+
+def test_synthetic_trace_covers_every_task_once_per_loop_and_step():
+    """row (f3), reading C38: every bundle of a step is packed and unpacked once per loop, density before force, self before pair"""
+    import bench_workloads as bw
+    n_tasks, n_self = 5000, 700
+    trace = bw.synthetic_trace(n_tasks, n_self, seed=7, steps=3)
+    for st in range(3):
+        for loop in ("density", "force"):
+            for action in ("pack", "unpack"):
+                rows = [(t0, m) for s_, l_, a_, t0, m in trace if (s_, l_, a_) == (st, loop, action)]
+                covered = np.zeros(n_tasks, dtype=int)
+                for t0, m in rows:
+                    covered[t0:t0 + m] += 1
+                    assert 1 <= m <= 1024 and (t0 + m <= n_self or t0 >= n_self)        # homogeneous bundles (C22)
+                assert np.all(covered == 1)
+    order = [(s_, l_) for s_, l_, _, _, _ in trace]
+    assert order == sorted(order, key=lambda x: (x[0], x[1] != "density"))
+    assert trace == bw.synthetic_trace(n_tasks, n_self, seed=7, steps=3) and trace != bw.synthetic_trace(n_tasks, n_self, seed=8, steps=3)
+
+
+def test_cell_slabs_cover_the_cell_table_in_order():
+    import bench_workloads as bw
+    cells = np.zeros(1000, dtype=sph.CELL_DTYPE)
+    rng = np.random.default_rng(3)
+    cells["count"] = rng.integers(1, 200, 1000)
+    cells["first"] = np.concatenate([[0], np.cumsum(cells["count"])[:-1]])
+    for slabs in (bw.cell_slabs(cells, 16), bw.cell_slabs(cells, fractions=(3, 1, 2, 2, 4, 4))):
+        assert slabs[0][0] == 0 and sum(s[1] for s in slabs) == 1000 and sum(s[3] for s in slabs) == int(cells["count"].sum())
+        for (c0, nc, p0, npart), nxt in zip(slabs, slabs[1:] + [None]):
+            assert p0 == int(cells["first"][c0]) and npart == int(cells["count"][c0:c0 + nc].sum())
+            assert nxt is None or nxt[0] == c0 + nc
+    big = bw.cell_slabs(cells, fractions=(3, 1, 2, 2, 4, 4))
+    assert big[0][3] > 2 * big[1][3] and big[-1][3] > big[2][3]
