@@ -393,6 +393,21 @@ def same_size_copy_gbs(torch, nbytes, flush, reps=7):
     return 2 * half / (best * 1e-3) / 1e9
 
 
+def same_size_fill_gbs(torch, nbytes, flush, reps=7):
+    """The write-only yardstick (a pack launch is ~94 % writes): torch's fill kernel over the same number of bytes, one launch on a
+    flushed L2, timed the same way.  HBM writes run below the read + write copy figure."""
+    a = torch.empty(max(1 << 20, int(nbytes)), dtype=torch.uint8, device="cuda")
+    best = None
+    for _ in range(reps):
+        flush()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); a.fill_(3); e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return a.numel() / (best * 1e-3) / 1e9
+
+
 def run_other_workload(args):
     """configs[2..4] and the link probe (bench_workloads.py); single GPU, same JSON contract"""
     import torch
@@ -494,7 +509,7 @@ def run_default(args):
     torch.cuda.set_device(local)
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     alu_peak = N_SM * LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    common = {"hbm_peak": hbm_peak, "alu_peak": alu_peak, "peak_source": peak_src, "same_size_copy": same_size_copy_gbs,
+    common = {"hbm_peak": hbm_peak, "alu_peak": alu_peak, "peak_source": peak_src, "same_size_copy": same_size_copy_gbs, "same_size_fill": same_size_fill_gbs,
               "time_steps": lambda torch_, fn, steps, warmup, flush: time_steps(torch_, fn, steps, warmup, flush, world),
               "sampler": (lambda: ClockSampler(local)) if rank == 0 else (lambda: None)}
     t_start = time.perf_counter()
@@ -651,6 +666,8 @@ def measure_config1(args, sph, torch, rank, world, local):
             if alg[k]["bound"] == "hbm":      # the same bytes as one plain copy launch on a flushed L2 (what a launch of this size can reach at all)
                 e["same_size_copy_gbs"] = round(same_size_copy_gbs(torch, alg[k]["bytes"], flush), 1)
                 e["frac_of_same_size_copy"] = round(e["achieved"] / e["same_size_copy_gbs"], 4)
+                if k.startswith("pack_"):
+                    e["same_size_fill_gbs"] = round(same_size_fill_gbs(torch, alg[k]["bytes"], flush), 1)
         kernels[k] = e
     dominant = max(R["per"], key=R["per"].get)
     traffic = None

@@ -360,6 +360,8 @@ def measure_config2(args, sph, torch, common, seed=1, layouts=("split", "aos")):
                 if "same_size_copy" in common:
                     e["same_size_copy_gbs"] = round(common["same_size_copy"](torch, alg[k], flush), 1)
                     e["frac_of_same_size_copy"] = round(e["achieved"] / e["same_size_copy_gbs"], 4)
+                if "same_size_fill" in common and k.startswith("pack_"):
+                    e["same_size_fill_gbs"] = round(common["same_size_fill"](torch, alg[k], flush), 1)
             if k == "force":
                 flop = cand * 8.0 + setup["neighbour_pairs"] * 60.0
                 e.update(bound="alu", achieved=round(flop / (ms * 1e-3) / 1e12, 3), peak=round(alu_peak, 2), unit="TFLOP/s",

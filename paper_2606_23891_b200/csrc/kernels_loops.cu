@@ -20,10 +20,11 @@
 //       t = |s|^2 - 2 x_i.s + (|x_i|^2 - (2h)^2 - eps) = r^2 - (2h)^2 - eps, four packed operations per source pair
 //       and target; the sign bit of t is funnel-shifted straight into a per-target hit mask (one SHF per source).
 //       eps covers the rounding of the expanded form, so the mask is a superset of the neighbours;
-//   (d) phase 2: every lane walks the set bits of its two masks in source order, one hit of target A and one of
-//       target B per iteration, the pair evaluated with packed f32x2 arithmetic (a target that has run out of
-//       hits is fed a far-away dummy source whose contribution is exactly zero).  r^2 = |x_i - s|^2 is recomputed
-//       exactly as the definition does and the exact cut-off applied.
+//   (d) phase 2, density and gradient loops: every lane walks the set bits of its two masks in source order, one hit of
+//       target A and one of target B per iteration, the pair evaluated with packed f32x2 arithmetic (a target that has
+//       run out of hits is fed a far-away dummy source whose contribution is exactly zero); force loop (expensive hits,
+//       heavy-tailed counts per target): the masks are cut into units of <= 4 hits evaluated 32 at a time (see the kernel).
+//       r^2 = |x_i - s|^2 is recomputed exactly as the definition does and the exact cut-off applied.
 // Sums are accumulated per target in tile order = source order, so results are bit-reproducible run to run.
 #include "internal.h"
 #include "ptx.cuh"
