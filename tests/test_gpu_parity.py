@@ -847,3 +847,39 @@ def test_split_pack_loops_write_what_the_fused_pack_writes(layout):
         blk = got[o0:o0 + int(cells["count"][int(tasks["ci"][0])]) * (rec // 4)].reshape(-1, rec // 4)
         assert np.all(blk[:, :-1] == 0xEEEEEEEE) and np.array_equal(blk[:, -1], want.view(np.uint32)[o0:o0 + blk.size].reshape(blk.shape)[:, -1])
     g.close()
+
+
+def test_slot_and_pass_argument_errors():
+    """row (f4) entry points: sizes, ranges and alignment are checked before any launch"""
+    ps, cells, tasks = case("ragged")
+    g = GpuCase(ps, cells, tasks)
+    need = sph.sph_batch_slot_bytes(g.batch, 1)
+    slots = torch.zeros(need, dtype=torch.uint8, device="cuda")
+    out = g.buffer(sph.sph_attrset_canonical(sph.SPH_SET_FORCE_OUT))
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_batch_slot_bytes(g.batch, 2)
+    assert e.value.code == 1
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack_slots(g.store, g.batch, 1, slots[:need - 128])
+    assert e.value.code == 3
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack_slots(g.store, g.batch, 1, torch.zeros(need + 64, dtype=torch.uint8, device="cuda")[64:])      # misaligned
+    assert e.value.code == 1
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_force_slots(g.batch, slots, out[:128], PARAMS)
+    assert e.value.code == 3
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_density_slots(g.batch, slots[:256], g.buffer(sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_OUT)))
+    assert e.value.code == 3
+    aset = sph.sph_attrset_canonical(sph.SPH_SET_DENSITY_IN)          # 5 words
+    buf = g.buffer(aset)
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack_pass(g.store, g.batch, aset, 1 << 5, buf)
+    assert e.value.code == 3
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_pack_pass(g.store, g.batch, aset, 1, buf[:1024])
+    assert e.value.code == 3
+    sph.sph_pack_pass(g.store, g.batch, aset, 0, buf)                 # an empty pass is a no-op, not an error
+    torch.cuda.synchronize()
+    assert int(buf.min()) == 0xCD and int(buf.max()) == 0xCD
+    g.close()

@@ -273,6 +273,14 @@ def test_null_arguments_are_errors_not_crashes():
     assert lib.sph_store_set_cells(store, None, C.c_uint32(3)) == 1
     assert lib.sph_batch_create(store, None, C.c_uint64(1), C.c_uint32(0), C.byref(C.c_void_p())) == 1
     assert "NULL" in sph.sph_last_error() or "no tasks" in sph.sph_last_error()
+    # the row (f4) entry points check their arguments the same way
+    assert lib.sph_batch_slot_bytes(None, C.c_int32(0), C.byref(out)) == 1
+    assert lib.sph_pack_slots(store, None, C.c_int32(0), fake, C.c_uint64(1024), None) == 1
+    assert lib.sph_density_slots(None, fake, C.c_uint64(0), fake, C.c_uint64(0), None) == 1
+    assert lib.sph_force_slots(None, fake, C.c_uint64(0), fake, C.c_uint64(0), None, None) == 1
+    assert lib.sph_pack_pass(store, None, C.byref(aset), C.c_uint64(1), fake, C.c_uint64(1024), None) == 1
+    assert lib.sph_pack_pass_masks(None, C.byref(aset), C.c_int32(0), None, None) == 1
+    assert lib.sph_slot_attrset(C.c_int32(0), None) == 1
     sph.sph_store_destroy(store)
 
 
