@@ -56,10 +56,6 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 
-// ---- programmatic dependent launch ----
-__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-
 // ---- packed pairs of f32 (sm_100: FADD2 / FMUL2 / FFMA2, two values per instruction) ----
 __device__ __forceinline__ u64 pack2(float lo, float hi) {
     u64 r;
