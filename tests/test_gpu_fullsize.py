@@ -303,8 +303,8 @@ _C3_WANT = {}
 # ------------------------------------------------------------------ configs[4]
 
 def test_config4_pipeline_sampled_cells_and_invariants():
-    """2^26 particles through bench.py's configs[4] pipeline (bundles of 4,096 tasks, two streams, host-resident split-AoS store,
-    streamed staging, one graph replay).  1,024 seeded cells are recomputed by the oracle from ALL their tasks: the density
+    """2^26 particles through bench.py's configs[4] pipeline (bundles of 4,096 tasks, eight under one launch per stage, two streams,
+    host-resident split-AoS store, streamed staging, one graph replay).  1,024 seeded cells are recomputed by the oracle from ALL their tasks: the density
     cycle over every task that touches a sampled cell or one of its partners (so the partners' rho, P, c_s are complete too),
     the ghost, the force cycle over every task that touches a sampled cell."""
     import bench_workloads as bw
@@ -313,7 +313,7 @@ def test_config4_pipeline_sampled_cells_and_invariants():
     n_cells, n = int(cells.shape[0]), ps.shape[0]
     layout = sph.sph_layout_split()
     hs = bw.HostStore(sph, torch, layout, ps, cells)
-    pl = bw.Pipeline(sph, torch, layout, hs, cells, tasks, n_cells, 4096, "staged")
+    pl = bw.Pipeline(sph, torch, layout, hs, cells, tasks, n_cells, 4096, "staged", group=bw.CONFIG4_GROUP)      # bench.py's launch configuration
     pl.capture().replay()
     torch.cuda.synchronize()
     pl.close()
