@@ -241,7 +241,10 @@ int32_t sph_unpack_cells(sph_store* store, const sph_batch* batch, const sph_att
  * one data type (by-type) or one (substruct, type) pair.  GPU analogue: sph_pack_pass writes only the record words named in
  * word_mask (bit w = 4-byte word w of the record) for every block of the batch; the passes of a partition together write
  * exactly the bytes of sph_pack.  sph_pack_pass_masks gives the partition: split 0 by-struct, 1 by-element (one attribute
- * entry each), 2 by-type (f64 / f32 / i64 / i8), 3 by-struct-and-type; masks_out [host, >= 48], n_out [host] their number. */
+ * entry each), 2 by-type (f64 / f32 / i64 / i8), 3 by-struct-and-type; masks_out [host, >= 48], n_out [host] their number.
+ * d_buf [device, 128-byte aligned, >= sph_batch_buffer_bytes]; asynchronous on stream; an empty mask is a no-op.  Errors, before
+ * any launch: SPH_ERR_INVALID_ARG (NULL, misaligned, unknown split), SPH_ERR_RANGE (a mask bit beyond the record's words, buffer
+ * too small), SPH_ERR_LAYOUT (bad attribute set). */
 int32_t sph_pack_pass_masks(const sph_layout* layout, const sph_attrset* set, int32_t split, uint64_t* masks_out, uint32_t* n_out);
 int32_t sph_pack_pass(const sph_store* store, const sph_batch* batch, const sph_attrset* set, uint64_t word_mask, void* d_buf,
                       uint64_t buf_bytes, void* stream);
