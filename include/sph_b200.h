@@ -236,6 +236,36 @@ int32_t sph_pack_cells(const sph_store* store, const sph_batch* batch, const sph
                        uint32_t cell_first, uint32_t cell_count, void* stream);
 int32_t sph_unpack_cells(sph_store* store, const sph_batch* batch, const sph_attrset* set, const void* d_buf, uint64_t buf_bytes,
                          int32_t mode, uint32_t cell_first, uint32_t cell_count, void* stream);
+/* ---- PACK without any allocation (for callers that must not call cudaMalloc) ----
+ * sph_pack needs a batch, and sph_batch_create allocates device memory for the batch's tables.  Some hosts cannot do that
+ * where they pack: a task-based SPH code (the paper's setting) takes its device memory once at start-up
+ * and then runs many worker threads, each feeding its own stream -- a cudaMalloc / cudaFree inside a worker may wait for
+ * the whole device and so stalls every other worker's stream, and on a GPU filled by the particle store it may just fail.
+ * sph_pack_static is sph_pack for those callers: it takes the tasks themselves [host array, n_tasks entries] instead of a
+ * batch, builds the tables for this one call in fixed host arrays, uploads them into a fixed scratch array inside the
+ * library's device image (2.1 MiB per GPU that loads the library, held until the process exits) and launches the same pack
+ * kernel.  It calls no cudaMalloc, cudaFree, cudaHostAlloc or other allocating routine, and uses no host heap.
+ *  - store: any store; one created over caller memory (sph_store_create with ext_ptrs) never allocated device memory
+ *    either.  set, d_buf [device, 128-byte aligned], stream: as sph_pack.  The buffer is laid out exactly as that of a
+ *    one-segment batch of the same tasks (sph_batch_create with tasks_per_segment = 0), block bytes identical to sph_pack's.
+ *  - bytes_needed_out [host, may be NULL]: receives the buffer size for these tasks and this set.  With d_buf = NULL the call
+ *    is only that size query.
+ *  - limits: n_tasks <= SPH_PACK_STATIC_MAX_TASKS, and the cells of the call together hold at most
+ *    SPH_PACK_STATIC_MAX_CHUNKS slices of 32 particles (a cell of c particles counts ceil(c / 32), once however often it
+ *    occurs).  Beyond either: SPH_ERR_RANGE before anything is uploaded or launched -- split the bundle.
+ *  - the first call on each device looks up where the scratch array lives on that device (with that device current); make
+ *    that first call during set-up, before any stream capture is begun.
+ *  - ALL calls share the one scratch array.  A call overwrites every table entry its kernel reads, so nothing has to be
+ *    cleared between calls, but two calls whose GPU work can overlap (different streams without an event between them, or
+ *    two host threads on two streams) race: the later upload replaces tables the earlier kernel may still be reading.  Calls
+ *    on one stream are safe, as are calls ordered by events.  On the host the calls of all threads take turns (a lock).
+ *  - errors as sph_pack, plus the limits above; every call re-uploads its tables (36 bytes per block + 20 per slice), so
+ *    where allocation is allowed sph_batch_create + sph_pack remains the faster path for a bundle that is packed repeatedly. */
+#define SPH_PACK_STATIC_MAX_TASKS 16384u
+#define SPH_PACK_STATIC_MAX_CHUNKS 65536u
+int32_t sph_pack_static(const sph_store* store, const sph_task* tasks, uint32_t n_tasks, const sph_attrset* set, void* d_buf,
+                        uint64_t buf_bytes, uint64_t* bytes_needed_out, void* stream);
+
 /* ---- split pack loops ("loop fission", Fig. 4) ----
  * The paper splits the pack loop into several loops that each touch one substruct (by-struct), one quantity (by-element),
  * one data type (by-type) or one (substruct, type) pair.  GPU analogue: sph_pack_pass writes only the record words named in

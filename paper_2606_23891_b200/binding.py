@@ -23,6 +23,7 @@ __all__ = [
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_pack_cells", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack",
     "sph_unpack_cells", "sph_ghost", "SPH_SET_GRADIENT_IN", "SPH_SET_GRADIENT_OUT", "SPH_SET_FORCE3_IN",
     "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots", "sph_pack_pass_masks", "sph_pack_pass",
+    "sph_pack_static", "SPH_PACK_STATIC_MAX_TASKS", "SPH_PACK_STATIC_MAX_CHUNKS",
     "SPLIT_BY_STRUCT", "SPLIT_BY_ELEMENT", "SPLIT_BY_TYPE", "SPLIT_BY_STRUCT_AND_TYPE",
 ]
 
@@ -45,6 +46,7 @@ EXPORTS = [
     "sph_cells_build_grid", "sph_cells_build_octree", "sph_tasks_build", "sph_free", "sph_batch_create", "sph_batch_destroy", "sph_batch_get_info", "sph_batch_buffer_bytes",
     "sph_batch_block_offsets", "sph_store_zero", "sph_pack", "sph_density", "sph_force", "sph_gradient", "sph_force3", "sph_unpack", "sph_ghost",
     "sph_slot_attrset", "sph_batch_slot_bytes", "sph_pack_slots", "sph_density_slots", "sph_force_slots", "sph_pack_pass_masks", "sph_pack_pass",
+    "sph_pack_static",
 ]
 
 
@@ -323,6 +325,20 @@ def sph_store_zero(store, aset: sph_attrset, stream=None) -> None:
 
 def sph_pack(store, batch, aset: sph_attrset, d_buf, stream=None) -> None:
     _check(_lib.sph_pack(store, batch, _ref(aset), _ptr(d_buf), C.c_uint64(_nbytes(d_buf)), _stream(stream)))
+
+
+SPH_PACK_STATIC_MAX_TASKS, SPH_PACK_STATIC_MAX_CHUNKS = 16384, 65536
+
+
+def sph_pack_static(store, tasks: np.ndarray, aset: sph_attrset, d_buf=None, stream=None) -> int:
+    """sph_pack for callers that must not allocate device memory (see include/sph_b200.h): takes the tasks instead of a
+    batch and works out of a fixed scratch array inside the library.  Returns the buffer size the tasks need; with
+    d_buf=None it only reports that size."""
+    assert tasks.dtype.itemsize == 56 and tasks.flags.c_contiguous
+    need = C.c_uint64(0)
+    _check(_lib.sph_pack_static(store, _ptr(tasks), C.c_uint32(tasks.shape[0]), _ref(aset), _ptr(d_buf),
+                                C.c_uint64(0 if d_buf is None else _nbytes(d_buf)), C.byref(need), _stream(stream)))
+    return int(need.value)
 
 
 def sph_pack_cells(store, batch, aset: sph_attrset, d_buf, cell_first: int, cell_count: int, stream=None) -> None:

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph_b200.so")
-SOURCES = ["api.cu", "builder.cu", "batch.cu", "kernels_pack.cu", "kernels_loops.cu"]
+SOURCES = ["api.cu", "builder.cu", "batch.cu", "kernels_pack.cu", "kernels_loops.cu", "pack_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
