@@ -651,8 +651,9 @@ int32_t sph_force3(const sph_batch* b, const void* d_in, uint64_t in_bytes, void
 // ---- split pack loops ----
 
 int32_t sph_pack_pass_masks(const sph_layout* layout, const sph_attrset* set, int32_t split, uint64_t* masks_out, uint32_t* n_out) {
-    if (!layout || !masks_out || !n_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
+    if (!layout || !set || !masks_out || !n_out) return fail(SPH_ERR_INVALID_ARG, "NULL argument");
     if (split < 0 || split > 3) return fail(SPH_ERR_INVALID_ARG, "split must be 0 (by-struct), 1 (by-element), 2 (by-type) or 3 (by-struct-and-type)");
+    SPH_API_BEGIN
     if (int32_t rc = sph_layout_validate(layout)) return rc;
     PassProgram all;
     if (int32_t rc = build_pass_words(*layout, *set, &all)) return rc;
@@ -667,6 +668,7 @@ int32_t sph_pack_pass_masks(const sph_layout* layout, const sph_attrset* set, in
     }
     *n_out = n;
     return SPH_OK;
+    SPH_API_END
 }
 
 int32_t sph_pack_pass(const sph_store* s, const sph_batch* b, const sph_attrset* set, uint64_t word_mask, void* d_buf, uint64_t buf_bytes, void* stream) {

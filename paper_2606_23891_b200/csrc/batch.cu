@@ -97,14 +97,19 @@ int32_t ensure_slots(const sph_batch* b, int loop, const SlotTables** out) {
         std::copy_n(&b->side_frames[3 * (size_t)is.src], 3, &ifr[6 * i + 3]);
     }
     std::vector<double> zeros(3 * (size_t)idx, 0.0);
-    SlotTables tmp;
-    if (int32_t rc = upload(chunks, &tmp.d_chunks)) return rc;
-    if (int32_t rc = upload(off128, &tmp.d_slot_off128)) return rc;
-    if (int32_t rc = upload(zeros, &tmp.d_zero_frames)) return rc;
-    if (int32_t rc = upload(items, &tmp.d_items)) return rc;
-    if (int32_t rc = upload(ifr, &tmp.d_item_frames)) return rc;
-    tmp.rec_bytes = rec; tmp.total = run; tmp.n_chunks = (uint32_t)chunks.size(); tmp.built = true;
-    sl = tmp;
+    // upload straight into the batch's tables: if one upload fails, sph_batch_destroy frees the arrays made so far and
+    // a later call starts over (`built` is set last)
+    auto drop = [&](int32_t rc) {
+        cudaFree(sl.d_chunks); cudaFree(sl.d_slot_off128); cudaFree(sl.d_zero_frames); cudaFree(sl.d_items); cudaFree(sl.d_item_frames);
+        sl = SlotTables{};
+        return rc;
+    };
+    if (int32_t rc = upload(chunks, &sl.d_chunks)) return drop(rc);
+    if (int32_t rc = upload(off128, &sl.d_slot_off128)) return drop(rc);
+    if (int32_t rc = upload(zeros, &sl.d_zero_frames)) return drop(rc);
+    if (int32_t rc = upload(items, &sl.d_items)) return drop(rc);
+    if (int32_t rc = upload(ifr, &sl.d_item_frames)) return drop(rc);
+    sl.rec_bytes = rec; sl.total = run; sl.n_chunks = (uint32_t)chunks.size(); sl.built = true;
     *out = &sl;
     return SPH_OK;
 }
@@ -156,6 +161,8 @@ int32_t sph_batch_create(const sph_store* store, const sph_task* tasks, uint64_t
     }
     b->task_side0[n_tasks] = (uint32_t)b->sides.size();
     b->n_sides = (uint32_t)b->sides.size();
+    // a loop item carries its source count as nt_ns = targets | count << 7 (32 bits)
+    if (b->max_count >= (1u << 25)) return fail(SPH_ERR_RANGE, "a cell of %u particles: the loops' item tables hold cell counts below 2^25", b->max_count);
     b->side_frames = frames;
 
     // per-cell occurrence lists in ascending (task, side) order = ascending side index

@@ -280,7 +280,27 @@ def test_null_arguments_are_errors_not_crashes():
     assert lib.sph_force_slots(None, fake, C.c_uint64(0), fake, C.c_uint64(0), None, None) == 1
     assert lib.sph_pack_pass(store, None, C.byref(aset), C.c_uint64(1), fake, C.c_uint64(1024), None) == 1
     assert lib.sph_pack_pass_masks(None, C.byref(aset), C.c_int32(0), None, None) == 1
+    masks, n_masks = (C.c_uint64 * 48)(), C.c_uint32(0)
+    assert lib.sph_pack_pass_masks(C.byref(sph.sph_layout_aos()), None, C.c_int32(0), masks, C.byref(n_masks)) == 1      # NULL set
     assert lib.sph_slot_attrset(C.c_int32(0), None) == 1
+    sph.sph_store_destroy(store)
+
+
+def test_batch_rejects_a_cell_too_large_for_the_item_tables():
+    """a loop item holds its source count in 25 bits: a cell of 2^25 particles is an error, not a silently cut count"""
+    import ctypes as C
+    n = 1 << 25
+    raw = np.zeros(512, dtype=np.uint8)                       # never touched: the check comes before any table is built
+    base = (raw.ctypes.data + 255) // 256 * 256
+    store = sph.sph_store_create(sph.sph_layout_aos(), n, sph.SPH_MEM_HOST_PINNED, ext=[base])
+    cells = np.zeros(1, dtype=sph.CELL_DTYPE)
+    cells["first"], cells["count"], cells["width"] = 0, n, 1.0
+    sph.sph_store_set_cells(store, cells)
+    task = np.zeros(1, dtype=sph.TASK_DTYPE)
+    task["ci"], task["cj"] = 0, -1
+    with pytest.raises(sph.SphError) as e:
+        sph.sph_batch_create(store, task)
+    assert e.value.code == 3 and "2^25" in str(e.value)
     sph.sph_store_destroy(store)
 
 
