@@ -1,18 +1,17 @@
 #!/usr/bin/env python
-"""bench.py -- one JSON line for the SPH offload hot path on B200.
+"""bench.py -- one JSON line (< 4 KB) for the SPH offload hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload default|config1|config2|config3|config4|link|layouts]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload default|config1|config2|config3|config4|link|layouts|...]
 
-The default line is on the largest configuration whose store is resident in HBM, BASELINE.json:configs[2]: 2,097,152
-particles of the Sod-like setup, force loop with pack / unpack per bundle of 512 tasks (896 bundles under one launch per
-stage).  A step = pack FORCE_IN, force, unpack FORCE_OUT (the sums start from zero) over every bundle, inputs resident in HBM;
-value = particles/s through that step (whole job: all ranks' particles / max-over-ranks time); `roofline` = the dominant
-kernel, `kernels` / `aos` carry every kernel's fraction of its roofline for split-AoS and AoS.
-`e2e` = the same step through the C ABI with the particle arrays in pinned HOST memory: the substructs the force loop reads
-cross up, the ones it writes cross back, every step, inside the timed region.
-`workloads` (N = 1 only) carries the other configurations, measured in the same run: configs[1] (density + force step),
-configs[3] (streamed pack / unpack against the host link, 5 and 13 fields) and configs[4] (whole step, host-resident store).
---impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+The default line is on BASELINE.json:configs[4], the largest single-GPU configuration and the B200 counterpart of the paper's
+whole offload cycle: 2^26 particles, per step pack -> density -> unpack -> ghost -> pack -> force -> unpack in
+bundles of 4,096 tasks over two streams.  `value` = particles/s through that step with the store resident in HBM (whole job: all
+ranks' particles / max-over-ranks time); `e2e` = the same step with the store in pinned HOST memory through the C-ABI calls, every
+host<->device copy inside the timed region; `roofline` = the dominant kernel (the force loop) against the FP32 peak; `kernels` =
+name -> fraction of its roofline for the stages of this step and (N = 1) for configs[2]'s pack / force / unpack in both layouts and
+configs[3]'s streamed pack / unpack against the host link.  Everything else -- per-stage tables, the other configurations -- is
+written to gpurun_out/bench_side.json, never to stdout.  (--workload X runs one configuration and prints its own line.)
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same configs[4] input.
 """
 import argparse
 import json
@@ -30,7 +29,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "particles/s pack+unpack and pair-interactions/s; % of HBM / host-link roofline"
-WORKLOAD = "configs[1]: 262144 particles, 64^3 glass-like lattice, 16^3 cells, density loop then force loop"
+CONFIG1_NAME = "configs[1]: 262144 particles, 64^3 glass-like lattice, 16^3 cells, density loop then force loop"
 SHARDING = "one independent box per rank, no collective"
 N_SM, LANES_PER_SM = 148, 128
 # algorithmic FP32 work of the loops: 8 flop per ordered candidate pair (3 sub, 1 mul,
@@ -480,7 +479,7 @@ def run_layouts(args):
     print(json.dumps({"metric": METRIC, "value": n / (rows[best]["ms_per_step"] * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": rows[best]["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f32", "data": "synthetic",
-                      "config": {"workload": WORKLOAD + ("; three-loop cycle (density, gradient, switched force)" if loops == 3 else "") + "; every particle layout of the paper",
+                      "config": {"workload": CONFIG1_NAME + ("; three-loop cycle (density, gradient, switched force)" if loops == 3 else "") + "; every particle layout of the paper",
                                  "layout": best, "loops": loops, "store": "HBM (step) / pinned host (e2e)",
                                  "l2": "flushed before every step (256 MB fill, untimed)"},
                       "e2e": {"value": n / (rows[best]["e2e_ms_per_step"] * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": rows[best]["h2d_bytes_per_step"],
@@ -498,8 +497,27 @@ def cpu_model():
     return "unknown"
 
 
+def side_path():
+    d = os.path.join(ROOT, "gpurun_out")
+    os.makedirs(d, exist_ok=True)
+    return os.path.join(d, "bench_side.json")
+
+
+def compact(line, limit=4000):
+    """the driver keeps only what it can parse from one stdout line: stay well below 4 KB (drop the optional keys first)"""
+    for key in ("kernels", "aos", "pair_interactions_per_s", "side_file"):
+        if len(json.dumps(line)) <= limit:
+            break
+        line.pop(key, None)
+    return line
+
+
 def run_default(args):
-    """the default line: configs[2] (headline), and at N = 1 the other configurations as `workloads`"""
+    """The default line: BASELINE.json:configs[4], the largest single-GPU configuration and the one that is the paper's whole offload
+    cycle (pack, transfer, loop, transfer back, unpack; where its time goes) -- 2^26 particles, the whole
+    step (density loop, ghost, force loop) in bundles of 4,096 tasks over two streams.  value = the step on an HBM-resident store;
+    e2e = the same step with the store in pinned host memory, every copy inside the timed region.  One stdout line (< 4 KB);
+    everything else (per-stage tables, the other configurations) goes to gpurun_out/bench_side.json."""
     import torch
     rank, world, local = dist_setup(args.gpus)
     if not torch.cuda.is_available():
@@ -513,79 +531,99 @@ def run_default(args):
               "time_steps": lambda torch_, fn, steps, warmup, flush: time_steps(torch_, fn, steps, warmup, flush, world),
               "sampler": (lambda: ClockSampler(local)) if rank == 0 else (lambda: None)}
     t_start = time.perf_counter()
-    out, setup, state = bw.measure_config2(args, sph, torch, common, seed=1 + rank)        # weak scaling: every rank owns its own box
-    P = out["split"]
-    ms = dist_max(P["ms"], world, "cuda")
-    ms_e2e = dist_max(P["ms_e2e"], world, "cuda")
-    total = dist_sum(float(P["n"]), world, "cuda")
-    dominant = max(("pack_force_in", "force", "unpack_force_out"), key=lambda k: P["kernels"][k]["ms"])
-    roof = {k: v for k, v in P["kernels"][dominant].items() if k not in ("ms", "instances_per_s", "candidate_pairs_per_s", "neighbour_pairs_per_s",
-                                                                          "frac_of_nominal_8tbs")}
-    traffic = None
-    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch,workload (from ncu --set full)
-    if os.path.exists(tfile):
-        for row in open(tfile):
-            c = row.strip().split(",")
-            if len(c) >= 4 and c[0] == dominant and c[1] == "split" and c[3] == "config2":
-                traffic = float(c[2])
-    roof.update(kernel=dominant, launch_ms=P["kernels"][dominant]["ms"], traffic=traffic,
-                peak_source=peak_src + (" HBM copy bandwidth" if roof.get("bound") == "hbm" else " max SM clock x 148 SMs x 128 FP32 lanes x 2"))
+    extras = rank == 0 and world == 1 and not args.no_workloads
+    R, setup, state = bw.measure_config4(args, sph, torch, common, seed=1 + rank, extras=extras)       # weak scaling: every rank owns its own box
+    n = R["n"]
+    ms = dist_max(R["split/resident"]["ms"], world, "cuda")
+    E = R["split/staged"]
+    ms_e2e = dist_max(E["ms"], world, "cuda")
+    total = dist_sum(float(n), world, "cuda")
+    K = R["kernel_ms"]                                                    # stage -> (ms summed over one step's launches, launches)
+    dominant = max(K, key=lambda k: K[k][0])
+    cand, inst, pairs = R["candidates"], R["instances"], R["neighbour_pairs"]
+    flop = {"density": cand * FLOP_CAND + (pairs + n) * FLOP_HIT_DENSITY, "force": cand * FLOP_CAND + pairs * FLOP_HIT_FORCE}
+    rec = {"pack_density_in": 20, "unpack_density_out": 16, "pack_force_in": 52, "unpack_force_out": 20}
+    kernels = {}
+    for k, (kms, cnt) in K.items():
+        if k in flop:
+            kernels[k] = round(flop[k] / (kms * 1e-3) / 1e12 / alu_peak, 4)
+        elif k in rec:      # record bytes only: the store side of a bundle's pack / unpack (each touched cell once per launch) is left out
+            kernels[k] = round(inst * rec[k] / (kms * 1e-3) / 1e9 / hbm_peak, 4)
+    kms, cnt = K[dominant]
+    if dominant in flop:
+        roof = {"bound": "alu", "achieved": round(flop[dominant] / (kms * 1e-3) / 1e12, 3), "peak": round(alu_peak, 2), "unit": "TFLOP/s",
+                "peak_source": peak_src + " max SM clock x 148 SMs x 128 FP32 lanes x 2"}
+    else:
+        roof = {"bound": "hbm", "achieved": round(inst * rec[dominant] / (kms * 1e-3) / 1e9, 1), "peak": hbm_peak, "unit": "GB/s",
+                "peak_source": peak_src + " HBM copy bandwidth"}
+    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), kernel=dominant, launches_per_step=cnt, launch_ms=round(kms / cnt, 4),
+                share_of_step=round(kms / sum(v[0] for v in K.values()), 3), traffic=None,
+                work="8 flop x ordered candidate pairs + 60 (force) / 25 (density) flop x pairs inside 2 h_i")
     line = {
         "metric": METRIC, "value": total / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": bw.CONFIG2_NAME.format(n=P["n"]), "layout": "split", "store": "HBM", "tasks": P["tasks"], "bundles": P["bundles"],
-                   "instances_per_loop": P["instances"], "candidate_pairs_per_loop": P["candidate_pairs"],
-                   "l2": "flushed before every step (256 MB fill, untimed)", "sharding": SHARDING, "setup": setup,
-                   "e2e": "host-resident particle arrays (pinned); per step the substructs the force loop reads cross up slab by slab and are packed as "
-                          "they land, the results cross back slab by slab behind the unpack; copies, kernels and cross-stream events captured once as "
-                          "a CUDA graph, one replay per step"},
-        "pair_interactions_per_s": {"force": P["kernels"]["force"]["candidate_pairs_per_s"]},
-        "neighbour_pairs_per_s": {"force": P["kernels"]["force"]["neighbour_pairs_per_s"]},
-        "instances_per_s": {k: P["kernels"][k]["instances_per_s"] for k in ("pack_force_in", "unpack_force_out")},
-        "e2e": {"value": total / (ms_e2e * 1e-3), "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes"], "d2h_bytes_per_step": P["d2h_bytes"],
-                "ms_per_step": ms_e2e},
-        "gpu_launches": 3 * args.steps, "clocks": P["clocks"], "roofline": roof, "kernels": P["kernels"], "single_bundle_ms": P["single_bundle_ms"],
-        "aos": {"value": total / (dist_max(out["aos"]["ms"], world, "cuda") * 1e-3), "ms_per_step": out["aos"]["ms"], "kernels": out["aos"]["kernels"],
-                "e2e_value": total / (dist_max(out["aos"]["ms_e2e"], world, "cuda") * 1e-3),
-                "e2e_bytes": [out["aos"]["h2d_bytes"], out["aos"]["d2h_bytes"]]},
+        "config": {"workload": bw.CONFIG4_NAME.format(n=n), "layout": "split", "store": "HBM (value) / pinned host (e2e)",
+                   "tasks": R["tasks"], "bundles": E["bundles"], "cells": setup["cells"], "l2": "inputs larger than L2 (8 GB store)", "sharding": SHARDING,
+                   "timing": "one CUDA graph replay per step"},
+        "pair_interactions_per_s": {"density": cand / (K["density"][0] * 1e-3), "force": cand / (K["force"][0] * 1e-3)},
+        "e2e": {"value": total / (ms_e2e * 1e-3), "unit": "particles/s", "ms_per_step": ms_e2e, "h2d_bytes_per_step": E["h2d_bytes"],
+                "d2h_bytes_per_step": E["d2h_bytes"],
+                "path": "store in pinned host memory; density inputs up slab by slab, v and u during the density loop, results down behind the bundles; "
+                        "rho, rho_dh, P, c_s, x, h, mass stay on the device between the two loops (device shadow)",
+                "host_link_gbs": round((E["h2d_bytes"] + E["d2h_bytes"]) / (ms_e2e * 1e-3) / 1e9, 2),
+                "link_peak_gbs": [round(R["link"]["h2d_gbs"], 1), round(R["link"]["d2h_gbs"], 1)]},
+        "gpu_launches": R["split/resident"]["launches"] * args.steps, "clocks": R.get("clocks"), "roofline": roof, "kernels": kernels,
     }
-    if rank == 0 and world == 1 and not args.no_workloads:
+    side = {"configs[4]": {"results": R, "setup": setup}}
+    if "split/staged/no-shadow" in R:
+        ns = R["split/staged/no-shadow"]
+        line["e2e"].update(no_shadow_ms_per_step=round(ns["ms"], 3), no_shadow_bytes=[ns["h2d_bytes"], ns["d2h_bytes"]])
+    if "aos/staged" in R:
+        line["aos"] = {"e2e_ms_per_step": round(R["aos/staged"]["ms"], 3), "e2e_bytes": [R["aos/staged"]["h2d_bytes"], R["aos/staged"]["d2h_bytes"]],
+                       "split_over_aos": round(ms_e2e / R["aos/staged"]["ms"], 3)}
+    if extras:
         sub = argparse.Namespace(**vars(args))
-        work = {}
+
+        def attempt(name, fn):
+            try:
+                side[name] = fn()
+            except Exception as exc:      # a failing side benchmark must not lose the headline
+                side[name] = {"failed": repr(exc)}
+                torch.cuda.synchronize()
+            return side[name]
+        sub.n = 0
+        c2 = attempt("configs[2]", lambda: bw.measure_config2(sub, sph, torch, dict(common, sampler=lambda: None), seed=1)[0])
+        for lay in ("split", "aos"):
+            for k in ("pack_force_in", "force", "unpack_force_out"):
+                try:
+                    kernels[f"c2.{lay}.{k}"] = c2[lay]["kernels"][k]["frac"]
+                except (KeyError, TypeError):
+                    pass
         sub.steps, sub.warmup = min(args.steps, 20), 3
-        c1 = measure_config1(sub, sph, torch, rank, world, local)
-        work["configs[1]"] = {k: c1[k] for k in ("value", "unit", "ms_per_step", "config", "kernels", "aos", "e2e", "pair_interactions_per_s")}
-        sub.loops = 3                                     # row (f2): density, gradient, Balsara-switched force (ten launches)
-        c1b = measure_config1(sub, sph, torch, rank, world, local)
-        work["configs[1] three-loop cycle"] = {k: c1b[k] for k in ("value", "unit", "ms_per_step", "kernels", "aos", "e2e")}
-        sub.loops = 2
+        attempt("configs[1]", lambda: {k: v for k, v in measure_config1(sub, sph, torch, rank, world, local).items()
+                                       if k in ("value", "ms_per_step", "kernels", "aos", "e2e", "roofline")})
         sub.steps, sub.warmup, sub.n = 3, 3, args.n3
-        c3 = bw.run_config3(sub, sph, torch, common, ks=[5, 13], modes=("streamed",))
-        work["configs[3]"] = {"workload": c3["config"]["workload"], "link": c3["config"]["link"], "setup": c3["config"]["setup"],
-                              "streamed": c3["sweep"], "pack13_plus_unpack13": c3["roofline"]}
-        sub.n, sub.skip_zero_copy = args.n4, True
-        c4 = bw.run_config4(sub, sph, torch, common)
-        work["configs[4]"] = {"workload": c4["config"]["workload"], "e2e_note": c4["config"]["e2e"], "setup": c4["config"]["setup"],
-                              "link": c4["config"]["link"], "e2e": c4["e2e"], "roofline": c4["roofline"], "variants": c4["variants"]}
-        # rows (f3) / (f4) of the scope table: extreme occupancy, trace replay, cell slots, split pack loops
-        sub.n, sub.steps, sub.warmup = 0, 5, 3
-        eg = bw.run_eagle(sub, sph, torch, common)
-        work["eagle-like"] = {"workload": eg["config"]["workload"], "setup": eg["config"]["setup"], "ms_per_step": eg["ms_per_step"], "split": eg["split"],
-                              "aos_stages_ms": eg["aos"]["stages_ms"]}
-        sub.steps = 3
-        rp = bw.run_replay(sub, sph, torch, common)
-        work["trace-replay"] = {"workload": rp["config"]["workload"], "layouts": rp["layouts"]}
-        sub.steps = 10
-        sl = bw.run_slots(sub, sph, torch, common)
-        work["cell-slots"] = {"workload": sl["config"]["workload"], "per_task_ms": sl["per_task_ms"], "slots_ms": sl["slots_ms"], "formats": sl["formats"]}
-        fi = bw.run_fission(sub, sph, torch, common)
-        work["split-pack-loops"] = {"workload": fi["config"]["workload"], "layouts": fi["layouts"]}
-        line["workloads"] = work
+        c3 = attempt("configs[3]", lambda: bw.run_config3(sub, sph, torch, common, ks=[5, 13], modes=("streamed",)))
+        for r in c3.get("sweep", []):
+            kernels[f"c3.{r['layout']}.{r['op']}{r['k']}.link"] = r["moved_frac_of_link"]
+        if args.full:
+            sub.n, sub.steps, sub.warmup, sub.loops = 0, 5, 3, 2
+            attempt("eagle-like", lambda: bw.run_eagle(sub, sph, torch, common))
+            attempt("trace-replay", lambda: bw.run_replay(sub, sph, torch, common))
+            attempt("cell-slots", lambda: bw.run_slots(sub, sph, torch, common))
+            attempt("split-pack-loops", lambda: bw.run_fission(sub, sph, torch, common))
         if not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline_config2(state, budget_s=args.cpu_budget)
-        line["bench_wall_s"] = round(time.perf_counter() - t_start, 1)
+            line["cpu_baseline"] = cpu_baseline_config4(state[0], budget_s=args.cpu_budget)
     if rank == 0:
-        print(json.dumps(line))
+        line["bench_wall_s"] = round(time.perf_counter() - t_start, 1)
+        try:
+            with open(side_path(), "w") as f:
+                json.dump({"line": line, "side": side}, f, indent=1, default=str)
+            line["side_file"] = "gpurun_out/bench_side.json"
+        except OSError:
+            pass
+        sys.stdout.flush()
+        print(json.dumps(compact(line)), flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -687,7 +725,7 @@ def measure_config1(args, sph, torch, rank, world, local):
         "metric": METRIC, "value": total_particles / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "layout": primary, "store": "HBM", "tasks": int(w.info.n_tasks), "instances_per_loop": int(w.info.n_instances),
+        "config": {"workload": CONFIG1_NAME, "layout": primary, "store": "HBM", "tasks": int(w.info.n_tasks), "instances_per_loop": int(w.info.n_instances),
                    "candidate_pairs_per_loop": int(cand), "l2": "flushed before every step (256 MB fill, untimed)",
                    "sharding": SHARDING,
                    "e2e": "host-resident particle arrays; the step's copies and kernels captured once as a CUDA graph, one replay per step"},
@@ -850,46 +888,68 @@ def cpu_baseline(budget_s=20.0):
                       f"average of {reps} repetition(s), {t:.2f} s each", "stages": {"all_threads": stages}}
 
 
+CONFIG4_SAMPLE_EDGE = 0.2     # the oracle's sample of configs[4]: the particles of the sub-cube [0, 0.2)^3 (0.8 % of the box)
+
+
+def oracle_config4_sample(parts):
+    """A bounded sample of the default line's input for the oracle: the particles of configs[4] (same generator, same seed, same h)
+    that lie in the sub-cube [0, 0.2)^3 -- background and whatever clumps fall there -- with cells (octree, <= 400 per leaf) and
+    tasks built by the oracle's own builders.  Nothing here comes from the CUDA path."""
+    import oracle as orc
+    inside = np.all(parts["x"] < CONFIG4_SAMPLE_EDGE, axis=1)
+    sub = np.ascontiguousarray(parts[inside])
+    perm, cells = orc.cells_build_octree(sub["x"], sub["h"], 400, 1.0)
+    ps = np.ascontiguousarray(sub[perm.astype(np.int64)])
+    tasks, _, _ = orc.tasks_build(cells, orc.cell_hmax(ps, cells), 1.0)
+    return orc, ps, cells, tasks
+
+
+def oracle_config4_run(parts, steps, warmup, budget_s):
+    """the oracle's whole step (density cycle, ghost, force cycle) over the tasks of the first m cells of the sample, m sized so that
+    warmup + steps passes take about budget_s; -> (particles per step, seconds per step, cores, sample text)"""
+    orc, ps, cells, tasks = oracle_config4_sample(parts)
+    cores = min(os.cpu_count() or 1, 64)
+    orc.set_threads(cores)
+    n_cells = cells.shape[0]
+    probe = min(n_cells, 64)
+    t_probe = oracle_sample_step(orc, ps, cells, tasks, probe)
+    m = int(max(8, min(n_cells, probe * (budget_s / (steps + warmup)) / max(t_probe, 1e-3))))
+    for _ in range(warmup):
+        oracle_sample_step(orc, ps, cells, tasks, m)
+    times = [oracle_sample_step(orc, ps, cells, tasks, m) for _ in range(steps)]
+    particles = int(cells["count"][:m].sum())
+    n_tasks = int((tasks["ci"] < m).sum())
+    sample = (f"configs[4] input (same generator, seed and h), particles inside [0, {CONFIG4_SAMPLE_EDGE})^3 = {ps.shape[0]} in {n_cells} octree cells; "
+              f"per step the whole cycle (pack, density, unpack, ghost, pack, force, unpack) over the {n_tasks} tasks of the first {m} cells "
+              f"({particles} particles); the oracle's unpack is serial by design")
+    return particles, sum(times) / len(times), cores, sample
+
+
+def cpu_baseline_config4(parts, budget_s=20.0):
+    particles, sec, cores, sample = oracle_config4_run(parts, steps=2, warmup=1, budget_s=budget_s)
+    return {"value": particles / sec, "unit": "particles/s", "cores": cores, "kind": "oracle", "cpu_model": cpu_model(), "sample": sample}
+
+
 def run_reference(args):
-    """the oracle on the host cores on the default line's workload: the force cycle of configs[2], each step a bounded sample"""
+    """the oracle on the host cores on the default line's workload (configs[4]), each step a bounded sample of it"""
     rank = int(os.environ.get("RANK", 0))
     if rank != 0:
         return
     if args.workload == "config1":
         return run_reference_config1(args)
-    orc, ps, cells, tasks = oracle_config2_sample()
-    cores = min(os.cpu_count() or 1, 64)
-    orc.set_threads(cores)
-    half = cells.shape[0] // 2
-
-    def pick(m):
-        ci = tasks["ci"]
-        return np.ascontiguousarray(tasks[(ci < m) | ((ci >= half) & (ci < half + m))])
-
-    def cycle(sel):
-        t0 = time.perf_counter()
-        orc.force_cycle(ps, cells, sel)
-        return time.perf_counter() - t0
-    t_probe = cycle(pick(64))
-    per_step_budget = max(0.5, args.ref_budget / (args.steps + args.warmup))
-    m = int(max(16, min(half, 64 * per_step_budget / max(t_probe, 1e-3))))
-    sel = pick(m)
-    for _ in range(args.warmup):
-        cycle(sel)
-    times = [cycle(sel) for _ in range(args.steps)]
-    particles = int(cells["count"][:m].sum() + cells["count"][half:half + m].sum())
-    sec = sum(times) / len(times)
-    value = particles / sec
-    sample = (f"force cycle over the tasks of the first {m} dense and first {m} sparse cells of an 8192-cell sample of configs[2] "
-              f"({particles} particles, {sel.shape[0]} tasks) per step")
+    import sph_inputs as si
     import bench_workloads as bw
+    n = args.n4 or args.n or (1 << 26)
+    parts = si.config4(1, n)
+    particles, sec, cores, sample = oracle_config4_run(parts, args.steps, args.warmup, args.ref_budget)
+    value = particles / sec
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": bw.CONFIG2_NAME.format(n=1 << 21), "layout": "aos", "store": "host DRAM", "sample": sample},
+        "dtype": "f64", "data": "synthetic", "config": {"workload": bw.CONFIG4_NAME.format(n=n), "layout": "aos", "store": "host DRAM", "sample": sample},
         "cpu_baseline": {"value": value, "unit": "particles/s", "cores": cores, "kind": "oracle", "sample": sample, "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-    }))
+    }), flush=True)
 
 
 def run_reference_config1(args):
@@ -909,7 +969,7 @@ def run_reference_config1(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "layout": "aos", "store": "host DRAM", "sample": sample},
+        "dtype": "f64", "data": "synthetic", "config": {"workload": CONFIG1_NAME, "layout": "aos", "store": "host DRAM", "sample": sample},
         "cpu_baseline": {"value": value, "unit": "particles/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -918,7 +978,7 @@ def run_reference_config1(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="both", help="split | aos | both, or any layout name of paper_2606_23891_b200/layouts.py")
@@ -926,7 +986,8 @@ def main():
                     help="default = configs[2] as the headline plus configs[1], [3], [4] as `workloads`; the others run one configuration "
                          "(bench_workloads.py describes them)")
     ap.add_argument("--loops", type=int, default=2, choices=[2, 3], help="layouts / config1: the two-loop cycle or the three-loop cycle (density, gradient, force)")
-    ap.add_argument("--no-workloads", action="store_true", help="default line: configs[2] only")
+    ap.add_argument("--no-workloads", action="store_true", help="default line: the configs[4] headline only (split-AoS resident + staged)")
+    ap.add_argument("--full", action="store_true", help="default line: also run the eagle / replay / slots / fission workloads into the side file")
     ap.add_argument("--n3", type=int, default=0, help="default line: particle count of the configs[3] entry (default 2^24)")
     ap.add_argument("--n4", type=int, default=0, help="default line: particle count of the configs[4] entry (default 2^26)")
     ap.add_argument("--n", type=int, default=0, help="particle count for config2/3/4 (default: the full size of BASELINE.json)")

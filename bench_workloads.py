@@ -626,10 +626,14 @@ class Pipeline:
     mode "resident": the same bundles on a store that already sits in HBM, no copies: what the step costs in kernels alone.
     """
 
-    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode, n_slabs=16, group=1):
+    def __init__(self, sph, torch, layout, hs, cells, tasks, n_self, bundle, mode, n_slabs=16, group=1, shadow=True):
         """group: bundles under ONE launch per stage and stream (a batch of `group` segments of `bundle` tasks: every bundle keeps its own
-        buffer slice, laid out and reduced exactly like a stand-alone bundle)"""
+        buffer slice, laid out and reduced exactly like a stand-alone bundle).
+        shadow=False (staged only): SURVEY.md 8(d)'s rule for the host-resident configurations -- nothing a loop left on the device is
+        used by the next one: after the ghost everything the density loop and the ghost wrote goes down to the host store, and every
+        substruct the force loop reads comes up from it again, slab by slab ahead of the force bundles."""
         self.sph, self.torch, self.layout, self.hs, self.mode = sph, torch, layout, hs, mode
+        self.shadow = shadow or mode != "staged"
         self.group, self.span = group, bundle * group
         n = hs.n
         self.sets = [sph.sph_attrset_canonical(k) for k in range(4)]
@@ -682,6 +686,12 @@ class Pipeline:
         self.d2h_bytes = stride(self.down_density + self.down_force) if mode == "staged" else 0
         # what re-sending the force loop's inputs from the host store would add (SURVEY.md 8(d) "no device shadow across loops")
         self.shadow_bytes = stride(sorted(set(sub(["x", "h", "mass", "rho", "rho_dh", "P", "c_s"])) - set(self.up_force))) if mode == "staged" else 0
+        if not self.shadow:
+            self.down_mid = sorted(set(out_density + sub(["P", "c_s"])))                    # what the density loop and the ghost wrote
+            self.up_force_all = sub(["x", "h", "mass", "rho", "rho_dh", "v", "u", "P", "c_s"])
+            self.down_force = sub(["a", "du_dt", "v_sig"])
+            self.h2d_bytes = stride(self.up_density) + stride(self.up_force_all)
+            self.d2h_bytes = stride(self.down_mid) + stride(self.down_force)
         self.launches = 0
 
     def _bundles(self, root, k_in, k_out, kernel, slab_events):
@@ -740,12 +750,24 @@ class Pipeline:
             root.wait_event(up2)                                          # the ghost writes P, c_s next to v, u
         sph.sph_ghost(self.work, self.params, root)
         self.launches += 1
-        if staged:
+        force_slab_events = None
+        if staged and self.shadow:
             self.copy.wait_stream(root)                                   # density results (and nothing the force loop writes) cross back
             for s in self.down_density:
                 sph.sph_store_download_sub(self.dev, s, self.hs.sub(s), self.copy)
+        elif staged:
+            self.copy.wait_stream(root)                                   # no device shadow: results down, then the force loop's inputs up again
+            for s in self.down_mid:
+                sph.sph_store_download_sub(self.dev, s, self.hs.sub(s), self.copy)
+            force_slab_events = []
+            for c0, nc, p0, npart in self.slabs:
+                for s in self.up_force_all:
+                    sph.sph_store_upload_range(self.dev, s, self.hs.host[s], p0, npart, self.copy)
+                ev = torch.cuda.Event()
+                ev.record(self.copy)
+                force_slab_events.append(ev)
         done_slab = 0
-        for b, ev in self._bundles(root, 2, 3, lambda b, i, o, st: sph.sph_force(b, i, o, self.params, st), None):
+        for b, ev in self._bundles(root, 2, 3, lambda b, i, o, st: sph.sph_force(b, i, o, self.params, st), force_slab_events):
             if not staged or b < self.n_self_bundles:
                 continue
             # every task with ci < frontier is unpacked once bundle b is: those cells are final
@@ -774,6 +796,37 @@ class Pipeline:
         with torch.cuda.graph(self.graph, stream=root):
             self.step(root)
         return self.graph
+
+    def kernel_times(self):
+        """One step launch by launch on the current stream, CUDA events around every launch (same batches, same buffers, nothing
+        overlapping): {stage: (milliseconds summed over the step's launches, launches)}.  The store and buffers are far larger than
+        L2, so consecutive launches do not find each other's data there."""
+        sph, torch = self.sph, self.torch
+        st = torch.cuda.current_stream()
+        evs = []
+
+        def timed(name, fn):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st); fn(); b.record(st)
+            evs.append((name, a, b))
+        bufs = self.bufs[0]
+        for loop, (k_in, k_out) in (("density", (0, 1)), ("force", (2, 3))):
+            for b, batch in enumerate(self.batches):
+                mode = sph.SPH_UNPACK_REDUCE_ZERO if b < self.n_self_bundles else sph.SPH_UNPACK_REDUCE
+                timed(f"pack_{loop}_in", lambda: sph.sph_pack(self.work, batch, self.sets[k_in], bufs[k_in], st))
+                if loop == "density":
+                    timed("density", lambda: sph.sph_density(batch, bufs[0], bufs[1], st))
+                else:
+                    timed("force", lambda: sph.sph_force(batch, bufs[2], bufs[3], self.params, st))
+                timed(f"unpack_{loop}_out", lambda: sph.sph_unpack(self.work, batch, self.sets[k_out], bufs[k_out], mode, st))
+            if loop == "density":
+                timed("ghost", lambda: sph.sph_ghost(self.work, self.params, st))
+        torch.cuda.synchronize()
+        out = {}
+        for name, a, b in evs:
+            ms, cnt = out.get(name, (0.0, 0))
+            out[name] = (ms + a.elapsed_time(b), cnt + 1)
+        return out
 
     def close(self):
         for b in self.batches:
@@ -835,6 +888,64 @@ def run_config4(args, sph, torch, common, layout_names=("split", "aos")):
             "gpu_launches": P["launches_per_step"] * args.steps, "roofline": roof, "variants": res,
             "e2e": {"value": P["particles_per_s"], "unit": "particles/s", "h2d_bytes_per_step": P["h2d_bytes_per_step"],
                     "d2h_bytes_per_step": P["d2h_bytes_per_step"], "ms_per_step": P["ms_per_step"]}}
+
+
+CONFIG4_NAME = ("configs[4]: {n} particles (uniform + clumps), octree cells <= 400, whole step (pack, density, unpack, ghost, pack, force, unpack) "
+                "in bundles of 4096 tasks (" + str(CONFIG4_GROUP) + " under one launch per stage) over 2 streams")
+
+
+def measure_config4(args, sph, torch, common, seed=1, extras=True):
+    """The default line's workload.  Split-AoS: the step on an HBM-resident store (`resident`), the same step with the store in pinned
+    host memory (`staged`, the end-to-end figure: copies inside the timed region), per-stage kernel times of one step; with extras
+    also the staged step that keeps no device shadow between the loops, and the AoS store (staged).  Every variant is one CUDA
+    graph replay per step.  Returns (results, setup, (ps, cells, tasks))."""
+    n = args.n4 or args.n or (1 << 26)
+    ps, cells, tasks, setup = build_clumpy(sph, 4, seed, n)
+    n_self = int(cells.shape[0])
+    link = link_probe(torch)
+    time_steps = common["time_steps"]
+    no_flush = lambda: None                      # the store (8 GB) and the buffers are far larger than L2
+    res = {"n": n, "link": link}
+    plan = [("split", "resident", True), ("split", "staged", True)]
+    if extras:
+        plan += [("split", "staged", False), ("aos", "staged", True)]
+    hs, hs_name = None, None
+    for name, mode, shadow in plan:
+        if hs_name != name:
+            if hs is not None:
+                hs.close()
+            layout = sph.sph_layout_split() if name == "split" else sph.sph_layout_aos()
+            hs, hs_name = HostStore(sph, torch, layout, ps, cells), name
+        pl = Pipeline(sph, torch, layout, hs, cells, tasks, n_self, 4096, mode, group=CONFIG4_GROUP, shadow=shadow)
+        g = pl.capture()
+        sampler = common["sampler"]() if (name, mode) == ("split", "resident") else None
+        t = time_steps(torch, g.replay, args.steps, args.warmup, no_flush)
+        key = f"{name}/{mode}" + ("" if shadow else "/no-shadow")
+        res[key] = {"ms": sum(t) / len(t), "h2d_bytes": pl.h2d_bytes, "d2h_bytes": pl.d2h_bytes, "launches": pl.launches, "bundles": pl.n_bundles,
+                    "batches": len(pl.batches)}
+        if sampler is not None:
+            res["clocks"] = sampler.stop()
+        if (name, mode) == ("split", "resident"):
+            res["instances"], res["candidates"], res["tasks"] = int(pl.instances), int(pl.candidates), int(tasks.shape[0])
+            pl.kernel_times()                                                # warm
+            res["kernel_ms"] = {k: (round(v[0], 4), v[1]) for k, v in pl.kernel_times().items()}
+        if (name, mode, shadow) == ("split", "staged", True):
+            # ordered pairs inside the target's own cut-off, r < 2 h_i, from the density the step has just left in the host store:
+            # (32/3) pi h^3 rho / m per particle (a lower bound for the force loop, whose cut-off is max(2 h_i, 2 h_j))
+            torch.cuda.synchronize()
+            F = sph.FIELD
+            def col(field, dtype=np.float32):
+                loc = layout.loc[F[field]]
+                raw = hs.host[loc.sub].numpy()[: n * layout.stride[loc.sub]].reshape(n, layout.stride[loc.sub])
+                return raw[:, loc.off:loc.off + 4].copy().view(dtype).ravel().astype(np.float64)
+            h, rho, m = col("h"), col("rho"), col("mass")
+            ngb = (32.0 / 3.0) * np.pi * h ** 3 * rho / m
+            res["neighbour_pairs"] = float(ngb.sum())
+            res["neighbours_per_particle"] = float(ngb.mean())
+        pl.close()
+        del pl, g
+    hs.close()
+    return res, setup, (ps, cells, tasks)
 
 
 # ------------------------------------------------------------------------------------------------- extreme occupancy, trace replay (8(f3))
