@@ -27,7 +27,8 @@
 // one round-to-nearest conversion per coordinate.  unpack adds in f32, in
 // ascending task order, side i before side j.  Compile with -ffp-contract=off.
 //
-// Parity pins: tests/test_oracle_pins.py (every function below is pinned; none
+// Parity pins: tests/test_oracle_pins.py (every function below is pinned, the test-support functions orc_compare_blocks and
+// orc_flag_cutoff_pairs and the floor of balsara() included since round 3; none
 // is "parity unpinned" except v_sig exactly at the cut-off, reading C31).
 #include <algorithm>
 #include <cmath>

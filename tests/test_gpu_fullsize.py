@@ -19,7 +19,7 @@ import torch
 import oracle as orc
 import paper_2606_23891_b200 as sph
 import sph_inputs as si
-from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
+from gpu_setup import GAMMA, PARAMS, GpuCase, canon, per_component_ok, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
 from orc_setup import raw_copy, sort_grid
 from test_gpu_parity import _random_result_buffer, _records, check_store_physics, gpu_step
 
@@ -134,6 +134,7 @@ def test_config1_loops_every_record():
     mask = _block_mask(cells, tasks, 20, want.shape[0])
     w5, g5 = want[mask].view(np.float32).reshape(-1, 5).astype(np.float64), got[mask].view(np.float32).reshape(-1, 5).astype(np.float64)
     assert within_1e4_or_1e6(g5[:, :3], w5[:, :3], vec_scale(ref["a"])) and within_1e4_or_1e6(g5[:, 3], w5[:, 3], vec_scale(ref["du_dt"]))
+    assert per_component_ok(g5[:, :3], w5[:, :3], vec_scale(ref["a"]), "a (sampled records)")
     exempt = _C1["exempt"][_record_particles(cells, tasks)]              # C31
     assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt)
     g.close()
@@ -220,6 +221,7 @@ def test_config2_force_on_sampled_bundles():
         w5 = want[mask].view(np.float32).reshape(-1, 5).astype(np.float64)
         g5 = got_out[lo:lo + want.shape[0]][mask].view(np.float32).reshape(-1, 5).astype(np.float64)
         assert within_1e4_or_1e6(g5[:, :3], w5[:, :3]) and within_1e4_or_1e6(g5[:, 3], w5[:, 3]), b
+        assert per_component_ok(g5[:, :3], w5[:, :3], what=f"a (bundle {b})"), b
         exempt = orc.flag_cutoff_pairs(cells, sel, want_in)[_record_particles(cells, sel)]      # C31, this bundle's own pairs
         assert np.all((np.abs(g5[:, 4] - w5[:, 4]) <= 1e-4 * np.abs(w5[:, 4])) | exempt) and exempt.mean() < 0.01, b
     g.close()

@@ -11,7 +11,7 @@ import torch
 import oracle as orc
 import paper_2606_23891_b200 as sph
 import sph_inputs as si
-from gpu_setup import GAMMA, PARAMS, GpuCase, canon, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
+from gpu_setup import GAMMA, PARAMS, GpuCase, canon, per_component_ok, to_attrset, valid_mask, vec_scale, within_1e4_or_1e6
 from orc_setup import raw_copy, sort_grid, sort_octree
 
 pytestmark = pytest.mark.gpu
@@ -218,6 +218,7 @@ def test_force_loop_vs_oracle(name):
     g5, _ = _records(d_out.cpu().numpy(), off, cells, tasks, 5)
     r5, g5 = r5.astype(np.float64), g5.astype(np.float64)
     assert within_1e4_or_1e6(g5[:, :3], r5[:, :3]) and within_1e4_or_1e6(g5[:, 3], r5[:, 3])
+    assert per_component_ok(g5[:, :3], r5[:, :3], what="a (records)")
     exempt = _near_cutoff(ps, cells, tasks, buf_in)[pidx]
     ok = np.abs(g5[:, 4] - r5[:, 4]) <= 1e-4 * np.abs(r5[:, 4])
     assert np.all(ok | exempt) and exempt.mean() < 0.01
@@ -481,6 +482,7 @@ def check_store_physics(got, ref, a_scale=None, du_scale=None):
     assert np.max(np.abs(got["P"] - ref["P"]) / ref["P"]) <= 2e-5 and np.max(np.abs(got["c_s"] - ref["c_s"]) / ref["c_s"]) <= 1e-6
     a_r, a_g = ref["a"].astype(np.float64), got["a"].astype(np.float64)
     assert within_1e4_or_1e6(a_g, a_r, a_scale)
+    assert per_component_ok(a_g, a_r, a_scale, "a")
     d_r, d_g = ref["du_dt"].astype(np.float64), got["du_dt"].astype(np.float64)
     assert within_1e4_or_1e6(d_g, d_r, du_scale)
 

@@ -761,3 +761,115 @@ def test_three_loop_record_layouts():
     p2 = np.zeros(6, dtype=si.PART_DTYPE)
     orc.unpack(p2, cells, tasks, orc.GRADIENT_OUT, buf, orc.MODE_REDUCE)
     assert np.all(p2["div_v"][:3] == 3.0) and np.all(p2["rot_v"][:3] == 3.0) and np.all(p2["div_v"][3:] == 0)
+
+
+# ------------------------------------------------------------------ pins of the test-support functions and of the Balsara floor
+
+def test_compare_blocks_finds_the_first_differing_record_byte_and_skips_pad_bytes():
+    """orc.compare_blocks is the only comparator of four GPU tests: it must say -1 for equal block bytes whatever the pad bytes
+    hold, and the smallest differing offset otherwise -- on side i and side j, in the first and in a later task."""
+    cells = np.zeros(3, dtype=orc.CELL_DTYPE)
+    cells["count"], cells["first"], cells["width"] = [3, 5, 2], [0, 3, 8], 1.0
+    tasks = np.zeros(4, dtype=orc.TASK_DTYPE)
+    tasks["ci"], tasks["cj"] = [0, 1, 0, 2], [-1, -1, 1, -1]
+    rec = 20
+    off, total = orc.block_offsets(cells, tasks, rec)
+    # blocks of 60, 100, 60, 100, 40 bytes, each starting on a 128-byte line
+    assert [int(o) for o in off[[0, 2, 4, 5, 6]]] == [0, 128, 256, 384, 512] and total == 640
+    rng = np.random.default_rng(3)
+    a = rng.integers(0, 256, total).astype(np.uint8)
+    b = a.copy()
+    assert orc.compare_blocks(cells, tasks, rec, a, b) == -1
+    b[60:128] ^= 0xFF                                            # the pad bytes behind the first block, all of them
+    b[484:512] ^= 0xFF                                           # ... and behind side j of the pair task
+    assert orc.compare_blocks(cells, tasks, rec, a, b) == -1
+    for where in (0, 59, 128 + 99, 256 + 17, 384, 384 + 99, 512 + 39):      # first / last byte of blocks, side i and side j of the pair task
+        c = b.copy()
+        c[where] ^= 0x01
+        assert orc.compare_blocks(cells, tasks, rec, a, c) == where, where
+        assert orc.compare_blocks(cells, tasks, rec, c, a) == where, where
+    c = b.copy()
+    c[512 + 5] ^= 0x80
+    c[384 + 70] ^= 0x80
+    c[256 + 59] ^= 0x80
+    assert orc.compare_blocks(cells, tasks, rec, a, c) == 256 + 59      # the smallest offset, whichever thread finds which
+
+
+def _force3_pair(div_i, rot_i, div_j, rot_j):
+    """the two-particle FORCE_IN case of test_force_two_particles_hand_worked as FORCE3_IN records (18 words)"""
+    rec = np.zeros((2, 18), dtype=np.float32)
+    #            xr0   xr1  xr2  h    m    rho  rho_dh v0    v1   v2   u    P    cs
+    rec[0, :13] = [0.00, 0.0, 0.0, 0.1, 1.5, 2.0, 0.0, 0.3, 0.0, 0.0, 1.0, 2.0, 1.0]
+    rec[1, :13] = [0.05, 0.0, 0.0, 0.1, 2.5, 3.0, 0.0, -0.1, 0.0, 0.0, 1.0, 3.0, 1.25]
+    rec[0, 13], rec[0, 14:17] = div_i, rot_i
+    rec[1, 13], rec[1, 14:17] = div_j, rot_j
+    cells = np.zeros(1, dtype=orc.CELL_DTYPE)
+    cells["count"], cells["width"] = 2, 1.0
+    tasks = np.zeros(1, dtype=orc.TASK_DTYPE)
+    tasks["cj"] = -1
+    buf = np.zeros(256, dtype=np.uint8)
+    buf[:144] = rec.view(np.uint8).ravel()
+    return orc.force3(cells, tasks, buf, alpha=0.8, beta=3.0)[:40].view(np.float32).reshape(2, 5)
+
+
+def test_balsara_floor_hand_worked():
+    """B = |div v| / (|div v| + |rot v| + 1e-4 c_s / h) (reading C34; Table 1 column p-f) with the floor term a
+    quarter of the denominator, every factor a number chosen here: a floor of 1e-3 or 1e-5, c_s h instead of c_s / h, or the
+    rotation entering by a component instead of its norm all miss the expected values by far more than the tolerance."""
+    # i: c_s / h = 1.0 / 0.1 -> floor 1.0e-3;  |div| = 2.0e-3, |rot| = 0.5e-3  -> B_i = 2 / (2 + 0.5 + 1)        = 4/7
+    # j: c_s / h = 1.25 / 0.1 -> floor 1.25e-3; |div| = 3.0e-3, |rot| = |(0.75, 0, 1) e-3| = 1.25e-3 -> B_j = 3 / 5.5 = 6/11
+    out = _force3_pair(-2.0e-3, [0.0, 0.0, 0.5e-3], 3.0e-3, [0.75e-3, 0.0, 1.0e-3])
+    Bbar = 0.5 * (4.0 / 7.0 + 6.0 / 11.0)                      # 43/77
+    assert Bbar == pytest.approx(43.0 / 77.0, rel=1e-15)
+    G = -0.9375 / (math.pi * 1e-4)
+    vr = mu = -0.4
+    vs = 1.0 + 1.25 - 3.0 * mu                                   # 3.45: the signal velocity is not switched
+    visc = Bbar * (-0.5 * 0.8 * vs * mu / 2.5)
+    F = 0.5 * G + (1.0 / 3.0) * G + visc * G
+    assert out[0, 0] == pytest.approx(2.5 * F, rel=2e-6) and out[1, 0] == pytest.approx(-1.5 * F, rel=2e-6)
+    assert out[0, 3] == pytest.approx(2.5 * (0.5 * G + 0.5 * visc * G) * vr, rel=2e-6)
+    assert out[1, 3] == pytest.approx(1.5 * ((1.0 / 3.0) * G + 0.5 * visc * G) * vr, rel=2e-6)
+    assert out[0, 4] == pytest.approx(vs, rel=1e-6) and out[1, 4] == pytest.approx(vs, rel=1e-6)
+    # what the same pair gives without the floor (B_i = 2 / 2.5, B_j = 3 / 4.25) is 40 % away in the viscous term: the pin is sharp
+    no_floor = 0.5 * (0.8 + 3.0 / 4.25)
+    assert abs(no_floor / Bbar - 1.0) > 0.3
+    assert abs(out[0, 0] / (2.5 * (0.5 * G + G / 3.0 + no_floor * (visc / Bbar) * G)) - 1.0) > 0.02
+    # with div v and rot v a million times larger the floor vanishes and B_i = 0.8, B_j = 3 / 4.25
+    big = _force3_pair(-2.0e3, [0.0, 0.0, 0.5e3], 3.0e3, [0.75e3, 0.0, 1.0e3])
+    F_big = 0.5 * G + (1.0 / 3.0) * G + no_floor * (visc / Bbar) * G
+    assert big[0, 0] == pytest.approx(2.5 * F_big, rel=2e-6)
+
+
+def _force_in_records(rows):
+    rec = np.zeros((len(rows), 13), dtype=np.float32)
+    for k, (x, h) in enumerate(rows):
+        rec[k, :3], rec[k, 3], rec[k, 4], rec[k, 5] = x, h, 1.0, 1.0
+    return rec
+
+
+@pytest.mark.parametrize("h_pair", [(0.1, 0.07), (0.07, 0.1)])
+def test_flag_cutoff_pairs_marks_exactly_the_pairs_on_the_cutoff(h_pair):
+    """reading C31: a particle is exempt from the v_sig comparison iff it has a partner with |r - R_cut| < 1e-5 R_cut,
+    R_cut = max(2 h_i, 2 h_j) -- whichever of the two has the larger h, in self tasks and across the two sides of a pair task."""
+    hi, hj = (np.float32(h) for h in h_pair)
+    cut = max(2.0 * float(hi), 2.0 * float(hj))
+    tasks = np.zeros(1, dtype=orc.TASK_DTYPE)
+    for delta, expect in ((5e-6, True), (-5e-6, True), (5e-5, False), (-5e-5, False)):
+        r = cut * (1.0 + delta)
+        # self task, three particles: the pair along y, a bystander 0.05 away from the first (well inside, not on any cut-off)
+        rec = _force_in_records([((0.3, 0.1, 0.2), hi), ((0.3, 0.1 + r, 0.2), hj), ((0.35, 0.1, 0.2), np.float32(0.02))])
+        cells = np.zeros(1, dtype=orc.CELL_DTYPE)
+        cells["count"], cells["width"] = 3, 1.0
+        tasks["ci"], tasks["cj"] = 0, -1
+        buf = np.zeros(256, dtype=np.uint8)
+        buf[:156] = rec.view(np.uint8).ravel()
+        assert orc.flag_cutoff_pairs(cells, tasks, buf).tolist() == [expect, expect, False], (delta, h_pair)
+        # pair task: two particles on side i (cell 1: store particles 2, 3), two on side j (cell 0: particles 0, 1); the pair is (i1, j0)
+        cells = np.zeros(2, dtype=orc.CELL_DTYPE)
+        cells["count"], cells["first"], cells["width"] = 2, [0, 2], 1.0
+        tasks["ci"], tasks["cj"] = 1, 0
+        side_i = _force_in_records([((0.9, 0.9, 0.9), np.float32(0.01)), ((0.0, 0.0, 0.0), hi)])
+        side_j = _force_in_records([((0.0, 0.0, -r), hj), ((0.5, 0.5, 0.5), np.float32(0.01))])
+        buf = np.zeros(256, dtype=np.uint8)
+        buf[:104], buf[128:232] = side_i.view(np.uint8).ravel(), side_j.view(np.uint8).ravel()
+        assert orc.flag_cutoff_pairs(cells, tasks, buf).tolist() == [expect, False, False, expect], (delta, h_pair)
