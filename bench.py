@@ -556,8 +556,17 @@ def run_default(args):
     else:
         roof = {"bound": "hbm", "achieved": round(inst * rec[dominant] / (kms * 1e-3) / 1e9, 1), "peak": hbm_peak, "unit": "GB/s",
                 "peak_source": peak_src + " HBM copy bandwidth"}
+    traffic = None            # dram bytes per launch of the dominant kernel from one ncu --set full capture (a committed constant, not from this run)
+    tfile = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")      # kernel,layout,dram_bytes_per_launch,workload
+    if os.path.exists(tfile):
+        for row in open(tfile):
+            c = row.strip().split(",")
+            if len(c) >= 4 and c[0] == dominant and c[1] == "split" and c[3] == "config4":
+                traffic = float(c[2])
     roof.update(frac=round(roof["achieved"] / roof["peak"], 4), kernel=dominant, launches_per_step=cnt, launch_ms=round(kms / cnt, 4),
-                share_of_step=round(kms / sum(v[0] for v in K.values()), 3), traffic=None,
+                share_of_step=round(kms / sum(v[0] for v in K.values()), 3), traffic=traffic,
+                traffic_source="profiles/traffic_per_launch.csv (ncu --set full, r03: profiles/r03_ncu_full.md), a pair batch at full size",
+                algorithmic_bytes_per_launch=round(inst * (72 if dominant == "force" else 36) / cnt),
                 work="8 flop x ordered candidate pairs + 60 (force) / 25 (density) flop x pairs inside 2 h_i")
     line = {
         "metric": METRIC, "value": total / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

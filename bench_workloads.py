@@ -1178,11 +1178,17 @@ def run_fission(args, sph, torch, common):
             buf = torch.empty(sph.sph_batch_buffer_bytes(batch, aset), dtype=torch.uint8, device="cuda")
             t = {"by-particle (fused)": round(min(timed(torch, lambda: sph.sph_pack(store, batch, aset, buf), args.steps, 3, before=flush)), 5)}
             passes = {}
+            # the control: ONE pass of the same pass kernel with every record word selected.  The pass kernel is simple (4-byte
+            # stores at record stride, no staging); the fused kernel is a tuned cp.async + bulk-copy pipeline -- so "split / fused"
+            # mixes the cost of splitting with the difference between two kernels, "split / one full pass" isolates the split
+            full = (1 << (sph.sph_attrset_record_bytes(aset) // 4)) - 1
+            t["one full pass (same pass kernel)"] = round(min(timed(torch, lambda: sph.sph_pack_pass(store, batch, aset, full, buf), args.steps, 3, before=flush)), 5)
             for k, sname in enumerate(split_names):
                 masks = sph.sph_pack_pass_masks(layout, aset, k)
                 t[sname] = round(min(timed(torch, lambda: [sph.sph_pack_pass(store, batch, aset, m, buf) for m in masks], args.steps, 3, before=flush)), 5)
                 passes[sname] = len(masks)
-            row[label] = {"ms": t, "passes": passes, "vs_fused": {k: round(v / t["by-particle (fused)"], 2) for k, v in t.items()}}
+            row[label] = {"ms": t, "passes": passes, "vs_fused": {k: round(v / t["by-particle (fused)"], 2) for k, v in t.items()},
+                          "vs_one_full_pass": {k: round(v / t["one full pass (same pass kernel)"], 2) for k, v in t.items()}}
             del buf
         rows[name] = row
         sph.sph_batch_destroy(batch)
