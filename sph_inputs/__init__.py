@@ -13,5 +13,5 @@ from .format import PART_DTYPE, FIELDS, FIELD_NCOMP, field_id  # noqa: F401
 from .generators import (  # noqa: F401
     splitmix64, uniform01, normal01,
     config0, config1, config2_positions, config3, config4,
-    jittered_lattice, clumpy_mixture, mixture_density, eagle_like, eagle_like_counts,
+    jittered_lattice, clumpy_mixture, mixture_density, eagle_like, eagle_like_counts, synthetic_trace,
 )

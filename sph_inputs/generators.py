@@ -266,3 +266,24 @@ def eagle_like(seed: int = 1, cells_per_dim: int = 16, n_max: int = 125113, n_mi
     parts["mass"] = np.float32(1.0 / n)
     parts["u"] = 1.0
     return _finish(parts)
+
+
+def synthetic_trace(n_tasks, n_self, seed, steps=5, bundle_lo=128, bundle_hi=1024):
+    """A seeded stand-in for a recorded trace of offload actions: per simulation step the self tasks, then
+    the pair tasks, are cut into bundles of seeded sizes; every bundle is packed and later unpacked, density before force.
+    -> list of (step, loop, action, first task, task count)"""
+    rng = np.random.default_rng(seed)
+    trace = []
+    for st in range(steps):
+        cuts = []
+        for lo, hi in ((0, n_self), (n_self, n_tasks)):
+            t = lo
+            while t < hi:
+                m = int(min(hi - t, rng.integers(bundle_lo, bundle_hi + 1)))
+                cuts.append((t, m))
+                t += m
+        for loop in ("density", "force"):
+            for t0, m in cuts:
+                trace.append((st, loop, "pack", t0, m))
+                trace.append((st, loop, "unpack", t0, m))
+    return trace

@@ -228,9 +228,9 @@ def test_config2_force_on_sampled_bundles():
 
 
 def test_library_h_iteration_matches_the_oracles():
-    """bench_workloads.iterate_h_on_gpu (the library's density loop driving Newton steps; setup of the configs[2] bench)
+    """pipeline.iterate_h_on_gpu (the library's density loop driving Newton steps; setup of the configs[2] bench)
     against orc.iterate_h (reading C20) on a 2^15 Sod-like box: both solve (4/3) pi (2h)^3 wcount = 48, to 1e-3 here."""
-    import bench_workloads as bw
+    from paper_2606_23891_b200 import pipeline as bw, workloads
     parts = si.config2_positions(seed=3, n_yz=32, n_left=25, n_right=6)
     perm, cells = sph.sph_cells_build_grid(parts["x"], 8)
     ps = np.ascontiguousarray(parts[perm.astype(np.int64)])
@@ -250,10 +250,10 @@ def test_config3_pack_and_unpack_bytes_in_full():
     """2^24 clustered particles, octree <= 400 per leaf, ~2.0e6 tasks / 5.2e8 instances: the 5- and 13-field packs (C21) of
     every task and the 13-field REDUCE unpack, byte for byte, AoS and split-AoS.  The buffers are tens of GB, so tasks go
     through in slices of 2^17, each slice its own batch (what a slice packs is exactly what a stand-alone batch packs)."""
-    import bench_workloads as bw
+    from paper_2606_23891_b200 import pipeline as bw, workloads
     from test_gpu_parity import PACK_SWEEP, UNPACK_SWEEP, fill_all_fields, sweep_set
     orc.set_threads(64)
-    ps, cells, tasks, info = bw.build_clumpy(sph, 3, 1, 1 << 24)
+    ps, cells, tasks, info = workloads.build_clumpy(sph, 3, 1, 1 << 24)
     oc, ot = cells.view(orc.CELL_DTYPE), tasks.view(orc.TASK_DTYPE)
     assert info["per_cell_max"] <= 448 and ps.shape[0] == 1 << 24
     ps = fill_all_fields(ps, 11)
@@ -309,9 +309,9 @@ def test_config4_pipeline_sampled_cells_and_invariants():
     host-resident split-AoS store, streamed staging, one graph replay).  1,024 seeded cells are recomputed by the oracle from ALL their tasks: the density
     cycle over every task that touches a sampled cell or one of its partners (so the partners' rho, P, c_s are complete too),
     the ghost, the force cycle over every task that touches a sampled cell."""
-    import bench_workloads as bw
+    from paper_2606_23891_b200 import pipeline as bw, workloads
     orc.set_threads(64)
-    ps, cells, tasks, info = bw.build_clumpy(sph, 4, 1, 1 << 26)
+    ps, cells, tasks, info = workloads.build_clumpy(sph, 4, 1, 1 << 26)
     n_cells, n = int(cells.shape[0]), ps.shape[0]
     layout = sph.sph_layout_split()
     hs = bw.HostStore(sph, torch, layout, ps, cells)

@@ -1,4 +1,4 @@
-"""The configs[4] offload pipeline of bench.py (bench_workloads.Pipeline: bundles of 4,096 tasks over two streams, host-resident
+"""The configs[4] offload pipeline of bench.py (paper_2606_23891_b200.pipeline.Pipeline: bundles of 4,096 tasks over two streams, host-resident
 store, streamed staging, one CUDA graph per step) against the oracle and against a plain one-stream run (needs a B200).
 
 PAPER.md:76-82 (section 2.3: pack / launch / unpack per bundle), PAPER.md:98 (asynchronous memory streams); SURVEY.md 8(d)
@@ -14,7 +14,7 @@ import numpy as np
 import pytest
 import torch
 
-import bench_workloads as bw
+from paper_2606_23891_b200 import pipeline as bw, workloads
 import oracle as orc
 import paper_2606_23891_b200 as sph
 from gpu_setup import GAMMA, PARAMS, canon
@@ -28,7 +28,7 @@ _CASE = {}
 
 def small_config4():
     if not _CASE:
-        ps, cells, tasks, info = bw.build_clumpy(sph, 4, 7, 1 << 19)
+        ps, cells, tasks, info = workloads.build_clumpy(sph, 4, 7, 1 << 19)
         ref = raw_copy(ps)
         orc.set_threads(64)
         oc, ot = cells.view(orc.CELL_DTYPE), tasks.view(orc.TASK_DTYPE)
@@ -126,10 +126,10 @@ def test_pipeline_with_grouped_bundles_equals_one_bundle_per_launch():
 
 @pytest.mark.parametrize("layout_name", ["split", "aos"])
 def test_config2_e2e_graph_equals_plain_step(layout_name):
-    """bench.py's configs[2] end-to-end step (bench_workloads.Config2E2E: slab-wise uploads and packs, the force loop launched per
+    """bench.py's configs[2] end-to-end step (paper_2606_23891_b200.pipeline.Config2E2E: slab-wise uploads and packs, the force loop launched per
     group of bundles as its slabs land, slab-wise unpacks and downloads, one CUDA graph) leaves in the HOST arrays exactly what the
     three plain launches leave in the store; reduced instance (31,744 particles, 8^3 cells, 14 bundles of 512 tasks)."""
-    ps, cells, tasks, _ = bw.build_config2(sph, torch, 3, 1 << 15)
+    ps, cells, tasks, _ = workloads.build_config2(sph, torch, 3, 1 << 15)
     n = ps.shape[0]
     layout = sph.sph_layout_split() if layout_name == "split" else sph.sph_layout_aos()
     store = sph.sph_store_create(layout, n)

@@ -333,9 +333,8 @@ def test_eagle_like_occupancies_have_the_papers_statistics():
 
 def test_synthetic_trace_covers_every_task_once_per_loop_and_step():
     """row (f3), reading C38: every bundle of a step is packed and unpacked once per loop, density before force, self before pair"""
-    import bench_workloads as bw
     n_tasks, n_self = 5000, 700
-    trace = bw.synthetic_trace(n_tasks, n_self, seed=7, steps=3)
+    trace = si.synthetic_trace(n_tasks, n_self, seed=7, steps=3)
     for st in range(3):
         for loop in ("density", "force"):
             for action in ("pack", "unpack"):
@@ -347,11 +346,11 @@ def test_synthetic_trace_covers_every_task_once_per_loop_and_step():
                 assert np.all(covered == 1)
     order = [(s_, l_) for s_, l_, _, _, _ in trace]
     assert order == sorted(order, key=lambda x: (x[0], x[1] != "density"))
-    assert trace == bw.synthetic_trace(n_tasks, n_self, seed=7, steps=3) and trace != bw.synthetic_trace(n_tasks, n_self, seed=8, steps=3)
+    assert trace == si.synthetic_trace(n_tasks, n_self, seed=7, steps=3) and trace != si.synthetic_trace(n_tasks, n_self, seed=8, steps=3)
 
 
 def test_cell_slabs_cover_the_cell_table_in_order():
-    import bench_workloads as bw
+    from paper_2606_23891_b200 import pipeline as bw
     cells = np.zeros(1000, dtype=sph.CELL_DTYPE)
     rng = np.random.default_rng(3)
     cells["count"] = rng.integers(1, 200, 1000)
