@@ -28,7 +28,8 @@ def main():
     prob = slabs.LocalProblem(cells, tasks, owner, rank)
     lp = prob.take(ps)
     orc.density_cycle(lp, prob.cells, prob.tasks)
-    slabs.exchange_fields(lp, prob, ("rho", "rho_dh", "wcount", "wcount_dh"), ps.shape[0], dist)
+    plan = slabs.HaloPlan(cells, tasks, owner, prob, rank)
+    sent = slabs.exchange_fields(lp, prob, ("rho", "rho_dh", "wcount", "wcount_dh"), plan, dist)
     orc.ghost(lp, GAMMA)
     orc.force_cycle(lp, prob.cells, prob.tasks)
     got = slabs.gather_owned(lp, prob, np.zeros_like(ps), dist)
@@ -40,7 +41,8 @@ def main():
         orc.ghost(ref, GAMMA)
         orc.force_cycle(ref, cells, tasks)
         same = bool(np.array_equal(got.view(np.uint8).reshape(-1, 128)[:, :108], ref.view(np.uint8).reshape(-1, 128)[:, :108]))
-        print(json.dumps({"world": world, "identical": same, "n": int(ps.shape[0]), "owned": owned, "halo_particles": int((~prob.owned).sum())}))
+        print(json.dumps({"world": world, "identical": same, "n": int(ps.shape[0]), "owned": owned, "halo_particles": int((~prob.owned).sum()),
+                          "sent_bytes": sent, "n_send": plan.n_send, "n_recv": plan.n_recv}))
     dist.destroy_process_group()
 
 

@@ -910,7 +910,8 @@ def test_slab_split_equals_single_box(world):
         sph.sph_pack(gc.store, gc.batch, S[0], b_in); sph.sph_density(gc.batch, b_in, b_out); sph.sph_unpack(gc.store, gc.batch, S[1], b_out, Z)
         torch.cuda.synchronize()
         local[k] = gc.export()
-    slabs.exchange_fields(local, probs, ("rho", "rho_dh", "wcount", "wcount_dh"), ps.shape[0])      # the one exchange step
+    plans = [slabs.HaloPlan(cells, tasks, owner, p, r) for r, p in enumerate(probs)]
+    slabs.exchange_fields(local, probs, ("rho", "rho_dh", "wcount", "wcount_dh"), plans)      # the one exchange step
     for k, gc in enumerate(cases):                                   # ghost + force cycle per rank
         sph.sph_store_import_aos(gc.store, local[k])
         sph.sph_ghost(gc.store, PARAMS)

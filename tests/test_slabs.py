@@ -58,7 +58,19 @@ def test_slab_split_equals_single_box_oracle(world):
     local = [p.take(ps) for p in probs]
     for lp, p in zip(local, probs):
         orc.density_cycle(lp, p.cells, p.tasks)
-    slabs.exchange_fields(local, probs, HALO_FIELDS, ps.shape[0])
+    plans = [slabs.HaloPlan(cells, tasks, owner, p, r) for r, p in enumerate(probs)]
+    for r, (p, pl) in enumerate(zip(probs, plans)):
+        # the plan covers exactly the rank's halo particles, each once, and what r receives from q is what q sends to r
+        got_idx = np.sort(np.concatenate(list(pl.recv.values()))) if pl.recv else np.zeros(0, np.int64)
+        assert np.array_equal(got_idx, np.flatnonzero(~p.owned))
+        for q, idx in pl.recv.items():
+            assert np.array_equal(p.particle_index[idx], probs[q].particle_index[plans[q].send[r]])
+        assert all(np.all(p.owned[idx]) for idx in pl.send.values())
+    moved = slabs.exchange_fields(local, probs, HALO_FIELDS, plans)
+    halo = sum(int((~p.owned).sum()) for p in probs)
+    # O(halo) bytes: nothing but the halo particles' fields moves (in this small periodic box -- two or three slabs of a 4^3 grid --
+    # nearly every cell is somebody's halo; on a large box the halo is one layer of cells per slab face)
+    assert moved == halo * 4 * len(HALO_FIELDS)
     for lp, p in zip(local, probs):
         orc.ghost(lp, GAMMA)
         orc.force_cycle(lp, p.cells, p.tasks)
@@ -74,3 +86,24 @@ def test_slab_split_over_two_gloo_ranks():
     assert len(lines) == 1, r.stdout
     d = lines[0]
     assert d["world"] == 2 and d["identical"] is True and d["halo_particles"] > 0 and d["owned"] == [d["n"] - d["owned"][1], d["owned"][1]]
+    # O(halo): rank 0 received its halo particles and sent 16 bytes (4 f32 fields) for each particle rank 1 holds as halo
+    assert d["n_recv"] == d["halo_particles"] and d["sent_bytes"] == 16 * d["n_send"] and 0 < d["n_send"] <= d["owned"][0]
+
+
+def test_halo_plan_moves_one_layer_of_cells_per_slab_face():
+    """on a 16^3 periodic grid cut into 4 slabs every rank's halo is one layer of 16^2 cells on each of its two faces, so a refresh
+    sends the fields of 2 x 256 cells' particles per rank -- an eighth of the box in total per rank pair, not the whole box"""
+    import paper_2606_23891_b200 as sph
+    x = np.random.default_rng(11).random((40000, 3))
+    perm, cells = sph.sph_cells_build_grid(x, 16)
+    tasks, _, _ = sph.sph_tasks_build(cells, np.full(cells.shape[0], 0.02, dtype=np.float32))
+    cells, tasks = cells.view(orc.CELL_DTYPE), tasks.view(orc.TASK_DTYPE)
+    world = 4
+    owner = slabs.partition(cells, world)
+    for r in range(world):
+        prob = slabs.LocalProblem(cells, tasks, owner, r)
+        plan = slabs.HaloPlan(cells, tasks, owner, prob, r)
+        assert sorted(plan.recv) == sorted({(r - 1) % world, (r + 1) % world}) == sorted(plan.send)
+        halo_cells = int((owner[prob.cell_index] != r).sum())
+        assert 2 * 256 <= halo_cells <= 2 * 256 + 2 * 16 * 16            # slab cuts follow particle counts, not cell layers: at most one ragged layer more
+        assert plan.n_recv == int((~prob.owned).sum()) and plan.n_recv < 0.2 * x.shape[0] and plan.n_send < 0.2 * x.shape[0]
